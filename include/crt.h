@@ -1,0 +1,185 @@
+/*
+ * crt.h -- C ABI of libcrt: the secondary-bounce hot path of "Generate Coherent Rays
+ * Directly" (arxiv 2310.07182) for NVIDIA B200 (sm_100a).
+ *
+ * Citations: "P:Lnn" = PAPER.md line nn; "D:Rn" = reading n in DESIGN.md section 3.
+ *
+ * Conventions
+ *  - Every function returns a crt_status; crt_last_error(ctx) gives the message of the
+ *    last failure on that context.  No exceptions cross this boundary.
+ *  - Pointers marked [device] are CUDA device pointers of the context's device, owned by
+ *    the caller (e.g. torch CUDA tensors) and must be 16-byte aligned (crt_ray: 32-byte).
+ *    Pointers marked [host] are ordinary host memory.  [host|device] is detected.
+ *  - `stream` is a cudaStream_t passed as void* (NULL = default stream).  Calls enqueue
+ *    work on it and return without synchronising, except where stated.
+ *  - The library allocates nothing in the per-frame calls; scratch comes from the caller
+ *    (sizes from the *_scratch_bytes queries).  The only library-owned objects are
+ *    crt_ctx and crt_bvh.
+ *  - There is no CPU fallback: without a usable CUDA device crt_create fails.
+ *
+ * Index spaces (D:R3-R5)
+ *  path  p = (sample*h + y)*w + x,             n_paths = spp*w*h
+ *  mode independent / morton_reorder:           n_slots = n_paths
+ *  mode direct_reuse with group gw x gh and interleave stride s (all powers of two):
+ *      tile W x H = (gw*s) x (gh*s), M = W*H slots per tile, K = gw*gh rays per group,
+ *      slot = (sample*n_tiles + tile)*M + m,  m = (a*n + c) mod M the shuffled number of
+ *      pixel n = ly*W + lx of the tile;  group = slot / K;  n_slots = spp*n_tiles*M.
+ */
+#ifndef CRT_H_
+#define CRT_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    CRT_OK = 0,
+    CRT_ERR_INVALID_ARG = 1,   /* null / misaligned pointer, negative size, bad enum */
+    CRT_ERR_UNSUPPORTED = 2,   /* valid request outside what the kernels implement */
+    CRT_ERR_CUDA = 3,          /* a CUDA runtime call failed; message has the CUDA error */
+    CRT_ERR_STATE = 4,         /* object used before it is ready (e.g. BVH without device data) */
+    CRT_ERR_NOMEM = 5
+} crt_status;
+
+typedef enum { CRT_MODE_INDEPENDENT = 0, CRT_MODE_MORTON_REORDER = 1, CRT_MODE_DIRECT_REUSE = 2 } crt_mode;
+typedef enum { CRT_MAT_DIFFUSE = 0, CRT_MAT_GLOSSY = 1, CRT_MAT_SPECULAR = 2, CRT_MAT_EMISSIVE = 3 } crt_mat_type;
+typedef enum { CRT_CLASS_EMPTY = 0, CRT_CLASS_DIFFUSE = 1, CRT_CLASS_GLOSSY = 2, CRT_CLASS_HYBRID = 3 } crt_group_class;
+
+typedef struct crt_ctx crt_ctx;
+typedef struct crt_bvh crt_bvh;
+
+/* 32 bytes.  tmax < 0 marks an inactive slot (dead path or out-of-image slot). */
+typedef struct { float ox, oy, oz, tmin, dx, dy, dz, tmax; } crt_ray;
+/* 16 bytes.  prim indexes the CALLER's triangle array; -1 = miss (then t = ray.tmax, u = v = 0). */
+typedef struct { float t, u, v; int32_t prim; } crt_hit;
+/* 32 bytes, indexed by path id.  flags bit 0 = alive.  (tr,tg,tb) throughput, (lr,lg,lb) radiance so far. */
+typedef struct { float tr, tg, tb; uint32_t flags; float lr, lg, lb; uint32_t pad; } crt_path_state;
+/* 32 bytes.  type is a crt_mat_type; roughness = GGX alpha; emission only read for CRT_MAT_EMISSIVE. */
+typedef struct { float albedo[3]; float roughness; float emission[3]; int32_t type; } crt_material;
+typedef struct { int32_t w, h, spp, seed, frame; } crt_frame;
+/* pinhole camera (D:R6): a pixel at normalised screen position (sx,sy) in [-1,1]^2, sy up, looks along W + sx*U + sy*V */
+typedef struct { float eye[3], U[3], V[3], W[3]; } crt_camera;
+typedef struct { int32_t mode, group_w, group_h, stride; } crt_order;
+/* materials: [device] table indexed by the per-triangle material id given to crt_build_bvh.
+ * env: radiance on a miss = lerp(env[0..2], env[3..5], 0.5*(d.y+1)) (D:R14). */
+typedef struct { const crt_material* materials; int32_t n_materials; float env[6]; } crt_scene_mats;
+typedef struct { int32_t max_leaf; int32_t sah_bins; float cost_traversal, cost_intersect; int32_t n_threads; } crt_bvh_params;
+typedef struct {
+    int64_t n_tris, n_nodes, device_bytes;
+    float bounds[6];            /* exact min/max over the vertices (unpadded); used by the Morton code */
+    double sah_cost; int32_t depth, max_leaf;
+    double build_seconds;
+} crt_bvh_info_t;
+/* optional per-stage device times of crt_generate_secondary, filled after the stream is synchronised by the
+ * caller via crt_stage_times_resolve (milliseconds) */
+typedef struct { float generate_ms, encode_ms, sort_ms, permute_ms; } crt_stage_times;
+
+/* ---- context ------------------------------------------------------------------------------------ */
+/* Creates a context on CUDA device `device`.  Fails with CRT_ERR_CUDA when no device is usable. */
+crt_status crt_create(int32_t device, crt_ctx** out);
+crt_status crt_destroy(crt_ctx* ctx);
+/* Message of the last failed call on ctx (ctx may be NULL: last failure of a call that had no context). */
+const char* crt_last_error(const crt_ctx* ctx);
+/* Tunables (for experiments; defaults are what bench.py times): "trace_kernel" (0 = one thread per ray,
+ * 1 = persistent warps with dynamic fetch), "trace_block", "trace_blocks_per_sm". */
+crt_status crt_set_option(crt_ctx* ctx, const char* key, int64_t value);
+/* Measures the device's FP32 FFMA rate (TFLOP/s) and a streaming copy rate (GB/s) with small kernels;
+ * synchronous. Used only as roofline denominators by bench.py. */
+crt_status crt_measure_peaks(crt_ctx* ctx, double* fp32_tflops, double* copy_gbs);
+
+/* ---- a0: acceleration structure (D:R11) ------------------------------------------------ */
+/* Builds a binary BVH (binned surface-area heuristic, leaves <= max_leaf triangles) on the host with
+ * n_threads threads and uploads it in the traversal layout.  verts: [host|device] float[n_tris][3][3];
+ * mat_id: [host|device] int32[n_tris].  Synchronous.  params may be NULL (defaults: max_leaf 4, 16 bins,
+ * costs 1/1, all hardware threads).  With ctx == NULL only the host tree is built (for crt_bvh_check /
+ * crt_bvh_get_info; such a BVH is rejected by the device calls with CRT_ERR_STATE). */
+crt_status crt_build_bvh(crt_ctx* ctx, const float* verts, const int32_t* mat_id, int64_t n_tris,
+                         const crt_bvh_params* params, crt_bvh** out);
+crt_status crt_bvh_destroy(crt_bvh* bvh);
+crt_status crt_bvh_get_info(const crt_bvh* bvh, crt_bvh_info_t* out);
+/* Structural invariants of the host tree: *violations = 0 iff every triangle is in exactly one leaf, every
+ * leaf has 1..max_leaf triangles, and every node's box contains its children's boxes / its triangles. */
+crt_status crt_bvh_check(const crt_bvh* bvh, int32_t* violations);
+
+/* ---- index spaces -------------------------------------------------------------------------------- */
+/* CRT_ERR_UNSUPPORTED unless group_w, group_h, stride are powers of two with tile size M <= 4096 and K <= 1024. */
+crt_status crt_layout(const crt_frame* frame, const crt_order* order, int64_t* n_paths, int64_t* n_slots, int64_t* n_groups);
+
+/* ---- path state ---------------------------------------------------------------------------------- */
+/* paths: [device] crt_path_state[n_paths] <- throughput 1, radiance 0, alive. */
+crt_status crt_paths_init(crt_ctx* ctx, crt_path_state* paths, int64_t n_paths, void* stream);
+
+/* ---- a1: primary rays (one path per pixel, shading point = first hit) ---------------------- */
+/* For every slot of the order: camera ray of its path (jitter from Philox purpose CAMERA), nearest hit.
+ * rays, hits, ray_to_path: [device] arrays of n_slots; out-of-image slots get an inactive ray and path -1. */
+crt_status crt_trace_primary(crt_ctx* ctx, const crt_bvh* bvh, const crt_camera* camera /*[host]*/, const crt_frame* frame,
+                             const crt_order* order, crt_ray* rays, crt_hit* hits, int32_t* ray_to_path, void* stream);
+
+/* ---- a2-a4: secondary-ray generation (P:L95-113 sections 3.2-3.3; P:L43 for morton_reorder) -------- */
+/* From the previous segment (prev_* arrays in the SAME order, n_slots entries) generate the rays of bounce
+ * `bounce` >= 1.  Outputs (all [device]): rays_out, ray_to_path_out, group_id_out, dir_src_out: n_slots entries;
+ * group_class_out: n_groups bytes (crt_group_class); n_active_out: one uint32 (zeroed by the call, then counted).
+ *   group_id_out[slot] = slot / K (direct_reuse) or the path id (other modes)
+ *   dir_src_out[slot]  = path id whose random numbers produced the direction: own id (glossy/specular member or
+ *                        independent sampling), the group leader's id (diffuse group), -2 - group (diffuse member of
+ *                        a hybrid group: mean direction of the glossy members), -1 (no ray)
+ * paths[path].throughput is multiplied by the BSDF weight; paths whose sample is invalid are killed.
+ * times may be NULL.  scratch: [device], at least crt_generate_secondary_scratch_bytes(). */
+crt_status crt_generate_secondary(crt_ctx* ctx, const crt_bvh* bvh, const crt_scene_mats* mats, const crt_frame* frame,
+                                  int32_t bounce, const crt_order* order,
+                                  const crt_ray* prev_rays, const crt_hit* prev_hits, const int32_t* prev_ray_to_path,
+                                  crt_path_state* paths, crt_ray* rays_out, int32_t* ray_to_path_out, int32_t* group_id_out,
+                                  int32_t* dir_src_out, uint8_t* group_class_out, uint32_t* n_active_out,
+                                  void* scratch, size_t scratch_bytes, void* stream);
+size_t crt_generate_secondary_scratch_bytes(const crt_frame* frame, const crt_order* order);
+
+/* Parts of morton_reorder, exported for testing and timing (P:L43 [AK10]; D:R12).
+ * keys[i] = 30-bit interleaved origin+direction code of rays[i] inside bvh bounds, 0xFFFFFFFF if inactive. */
+crt_status crt_morton_encode(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, uint32_t* keys, void* stream);
+/* Stable LSD radix sort of (key, value) pairs, 4 passes of 8 bits, hand-written (no CUB).  All [device];
+ * keys_in/vals_in are left intact; scratch >= crt_radix_sort_scratch_bytes(n). */
+crt_status crt_radix_sort_pairs(crt_ctx* ctx, const uint32_t* keys_in, const int32_t* vals_in, int64_t n,
+                                uint32_t* keys_out, int32_t* vals_out, void* scratch, size_t scratch_bytes, void* stream);
+size_t crt_radix_sort_scratch_bytes(int64_t n);
+
+/* ---- a5: BVH traversal ("the most time-consuming segment") ------------------------------- */
+/* hits[i] = nearest intersection of rays[i] with tmin < t < tmax; ties -> lowest primitive id (D:R10).
+ * Inactive rays (tmax < 0) give a miss.  rays, hits: [device], n_rays entries. */
+crt_status crt_trace(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n_rays, crt_hit* hits, void* stream);
+
+/* ---- a6: shading and accumulation (D:R14) --------------------------------------------- */
+/* For the segment just traced: miss -> radiance += throughput*env(d), path ends; emissive hit -> radiance +=
+ * throughput*Le, path ends.  If is_last: accum[pixel] += radiance/spp for every path (accum: [device] float[h][w][3]). */
+crt_status crt_shade_accumulate(crt_ctx* ctx, const crt_bvh* bvh, const crt_scene_mats* mats, const crt_frame* frame,
+                                int32_t bounce, int32_t is_last, const crt_ray* rays, const crt_hit* hits,
+                                const int32_t* ray_to_path, int64_t n_rays, crt_path_state* paths, float* accum, void* stream);
+
+/* ---- whole frame ---------------------------------------------------------------------------------- */
+/* primary -> shade(0) -> for b = 1..n_bounces { generate(b) -> trace -> shade(b) } on `stream`, using a caller
+ * workspace of crt_frame_workspace_bytes() [device] bytes.  accum: [device] float[h][w][3], added to.
+ * stage_ms (may be NULL, [host] float[8]): after the call has been synchronised with crt_frame_times(), the device
+ * times of  0 primary, 1 shade, 2 generate(+encode+sort+permute), 3 secondary trace, 4 encode+sort+permute only.
+ * n_secondary_out (may be NULL): [device] uint32[n_bounces] live secondary rays per bounce. */
+crt_status crt_render_frame(crt_ctx* ctx, const crt_bvh* bvh, const crt_scene_mats* mats, const crt_camera* camera /*[host]*/,
+                            const crt_frame* frame, const crt_order* order, int32_t n_bounces, float* accum,
+                            uint32_t* n_secondary_out, void* workspace, size_t workspace_bytes, int32_t record_times, void* stream);
+size_t crt_frame_workspace_bytes(const crt_frame* frame, const crt_order* order);
+/* Synchronises the events recorded by the last crt_render_frame(record_times = 1) and adds their durations
+ * (milliseconds) into stage_ms[0..4] ([host]). */
+crt_status crt_frame_times(crt_ctx* ctx, float* stage_ms);
+/* Same frame through HOST buffers: materials [host] crt_material[n_materials], accum_host [host] float[h][w][3]
+ * (read, added to, written back).  Copies materials + camera in and the image out on `stream` and synchronises.
+ * workspace as above plus crt_frame_host_extra_bytes(). */
+crt_status crt_render_frame_host(crt_ctx* ctx, const crt_bvh* bvh, const crt_material* materials_host, int32_t n_materials,
+                                 const float* env /*[host] 6*/, const crt_camera* camera, const crt_frame* frame,
+                                 const crt_order* order, int32_t n_bounces, float* accum_host, uint32_t* n_secondary_host,
+                                 void* workspace, size_t workspace_bytes, void* stream);
+size_t crt_frame_host_extra_bytes(const crt_frame* frame, int32_t n_materials);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CRT_H_ */

@@ -1,0 +1,302 @@
+// a0: host-side BVH construction for libcrt ("acceleration structures such as bounding volume
+// hierarchies"; the paper leaves width, leaf size and builder open -- DESIGN.md D:R11).
+// Binary tree, binned surface-area heuristic evaluated on all three axes per split, built top-down by a
+// small thread pool (large ranges are split one at a time, subtrees below a size threshold run as tasks).
+#include <algorithm>
+#include <atomic>
+#include <chrono>
+#include <cmath>
+#include <condition_variable>
+#include <cstring>
+#include <deque>
+#include <functional>
+#include <limits>
+#include <mutex>
+#include <thread>
+#include "crt_internal.h"
+
+namespace {
+
+constexpr int kMaxBins = 64;
+
+struct Box {
+    float mn[3], mx[3];
+    void reset() { for (int k = 0; k < 3; ++k) { mn[k] = std::numeric_limits<float>::infinity(); mx[k] = -mn[k]; } }
+    void grow(const float* a, const float* b) { for (int k = 0; k < 3; ++k) { mn[k] = std::min(mn[k], a[k]); mx[k] = std::max(mx[k], b[k]); } }
+    void grow(const Box& o) { grow(o.mn, o.mx); }
+    double half_area() const
+    {
+        double dx = (double)mx[0] - mn[0], dy = (double)mx[1] - mn[1], dz = (double)mx[2] - mn[2];
+        return dx * dy + dy * dz + dz * dx;
+    }
+};
+
+class Pool {
+public:
+    explicit Pool(int n)
+    {
+        for (int i = 0; i < n; ++i) workers_.emplace_back([this] { run(); });
+    }
+    ~Pool()
+    {
+        { std::lock_guard<std::mutex> g(m_); stop_ = true; }
+        cv_.notify_all();
+        for (auto& t : workers_) t.join();
+    }
+    void submit(std::function<void()> f)
+    {
+        { std::lock_guard<std::mutex> g(m_); q_.push_back(std::move(f)); ++pending_; }
+        cv_.notify_one();
+    }
+    void wait()
+    {
+        std::unique_lock<std::mutex> g(m_);
+        done_.wait(g, [this] { return pending_ == 0; });
+    }
+private:
+    void run()
+    {
+        for (;;) {
+            std::function<void()> f;
+            {
+                std::unique_lock<std::mutex> g(m_);
+                cv_.wait(g, [this] { return stop_ || !q_.empty(); });
+                if (stop_ && q_.empty()) return;
+                f = std::move(q_.front()); q_.pop_front();
+            }
+            f();
+            { std::lock_guard<std::mutex> g(m_); if (--pending_ == 0) done_.notify_all(); }
+        }
+    }
+    std::vector<std::thread> workers_;
+    std::deque<std::function<void()>> q_;
+    std::mutex m_;
+    std::condition_variable cv_, done_;
+    int64_t pending_ = 0;
+    bool stop_ = false;
+};
+
+struct Builder {
+    const float* verts; int64_t n; int max_leaf, bins; float ct, ci;
+    std::vector<float> tmn, tmx, cen;      // per-triangle box and centroid
+    std::vector<int32_t>& prim;
+    std::vector<BuildNode>& nodes;
+    std::atomic<int64_t> n_nodes{0};
+    std::atomic<int> max_depth{0};
+    Pool* pool;
+
+    Builder(std::vector<int32_t>& p, std::vector<BuildNode>& nd) : prim(p), nodes(nd) {}
+
+    int64_t alloc2() { return n_nodes.fetch_add(2); }
+
+    void make_leaf(BuildNode& nd, int64_t lo, int64_t hi) { nd.left = nd.right = -1; nd.first = (int32_t)lo; nd.count = (int32_t)(hi - lo); }
+
+    // builds the subtree of `node` over prim[lo,hi)
+    void subtree(int64_t node, int64_t lo, int64_t hi, int depth)
+    {
+        for (;;) {
+            Box bb, cb; bb.reset(); cb.reset();
+            for (int64_t i = lo; i < hi; ++i) {
+                int64_t p = prim[i];
+                bb.grow(&tmn[3 * p], &tmx[3 * p]); cb.grow(&cen[3 * p], &cen[3 * p]);
+            }
+            BuildNode& nd = nodes[node];
+            std::memcpy(nd.bmin, bb.mn, 12); std::memcpy(nd.bmax, bb.mx, 12);
+            int d0 = max_depth.load(std::memory_order_relaxed);
+            while (depth > d0 && !max_depth.compare_exchange_weak(d0, depth)) {}
+            int64_t cnt = hi - lo;
+            if (cnt <= max_leaf) { make_leaf(nd, lo, hi); return; }
+
+            // binned SAH on the three axes in one pass
+            int best_axis = -1, best_bin = -1; double best = std::numeric_limits<double>::infinity();
+            int64_t bc[3][kMaxBins]; Box bx[3][kMaxBins]; float scale[3];
+            for (int a = 0; a < 3; ++a) {
+                float ext = cb.mx[a] - cb.mn[a];
+                scale[a] = ext > 0.f ? (float)bins / ext : 0.f;
+                for (int j = 0; j < bins; ++j) { bc[a][j] = 0; bx[a][j].reset(); }
+            }
+            for (int64_t i = lo; i < hi; ++i) {
+                int64_t p = prim[i];
+                for (int a = 0; a < 3; ++a) {
+                    if (scale[a] == 0.f) continue;
+                    int j = std::min(bins - 1, std::max(0, (int)((cen[3 * p + a] - cb.mn[a]) * scale[a])));
+                    ++bc[a][j]; bx[a][j].grow(&tmn[3 * p], &tmx[3 * p]);
+                }
+            }
+            for (int a = 0; a < 3; ++a) {
+                if (scale[a] == 0.f) continue;
+                double ra[kMaxBins]; int64_t rc[kMaxBins]; Box acc; acc.reset(); int64_t c = 0;
+                for (int j = bins - 1; j >= 1; --j) { acc.grow(bx[a][j]); c += bc[a][j]; rc[j] = c; ra[j] = c ? acc.half_area() : 0.0; }
+                acc.reset(); c = 0;
+                for (int j = 0; j + 1 < bins; ++j) {
+                    acc.grow(bx[a][j]); c += bc[a][j];
+                    if (c == 0 || rc[j + 1] == 0) continue;
+                    double cost = acc.half_area() * (double)c + ra[j + 1] * (double)rc[j + 1];
+                    if (cost < best) { best = cost; best_axis = a; best_bin = j; }
+                }
+            }
+            int64_t mid;
+            if (best_axis < 0) {
+                mid = lo + cnt / 2;
+            } else {
+                const int a = best_axis; const float c0 = cb.mn[a], sc = scale[a];
+                auto it = std::partition(prim.begin() + lo, prim.begin() + hi, [&](int32_t p) {
+                    int j = std::min(bins - 1, std::max(0, (int)((cen[3 * (int64_t)p + a] - c0) * sc)));
+                    return j <= best_bin;
+                });
+                mid = it - prim.begin();
+                if (mid == lo || mid == hi) mid = lo + cnt / 2;
+            }
+            int64_t c = alloc2();
+            nd.left = (int32_t)c; nd.right = (int32_t)(c + 1); nd.count = 0; nd.first = 0;
+            int64_t rlo = mid, rhi = hi; int rd = depth + 1;
+            if (pool && (rhi - rlo) >= 4096) {
+                pool->submit([this, c, rlo, rhi, rd] { subtree(c + 1, rlo, rhi, rd); });
+            } else {
+                subtree(c + 1, rlo, rhi, rd);
+            }
+            node = c; hi = mid; ++depth;       // continue with the left child in this thread
+        }
+    }
+};
+
+}  // namespace
+
+// Builds the host tree.  Returns false on failure.
+bool crt_bvh_build_host(crt_bvh* b, const float* verts, int64_t n, const crt_bvh_params& pr)
+{
+    auto t0 = std::chrono::steady_clock::now();
+    b->n_tris = n; b->max_leaf = pr.max_leaf;
+    b->verts.assign(verts, verts + 9 * n);
+    b->prim.resize((size_t)n);
+    b->nodes.assign((size_t)std::max<int64_t>(2 * n, 1), BuildNode());
+    Builder B(b->prim, b->nodes);
+    B.verts = b->verts.data(); B.n = n; B.max_leaf = pr.max_leaf; B.bins = std::min(kMaxBins, std::max(4, pr.sah_bins));
+    B.ct = pr.cost_traversal; B.ci = pr.cost_intersect;
+    B.tmn.resize(3 * (size_t)n); B.tmx.resize(3 * (size_t)n); B.cen.resize(3 * (size_t)n);
+    float maxabs = 0.f;
+    Box root; root.reset();
+    for (int64_t i = 0; i < n; ++i) {
+        b->prim[i] = (int32_t)i;
+        const float* tv = verts + 9 * i;
+        for (int k = 0; k < 3; ++k) {
+            float lo = std::min(tv[k], std::min(tv[3 + k], tv[6 + k])), hi = std::max(tv[k], std::max(tv[3 + k], tv[6 + k]));
+            B.tmn[3 * i + k] = lo; B.tmx[3 * i + k] = hi; B.cen[3 * i + k] = 0.5f * lo + 0.5f * hi;
+            maxabs = std::max(maxabs, std::max(std::fabs(lo), std::fabs(hi)));
+        }
+        root.grow(&B.tmn[3 * i], &B.tmx[3 * i]);
+    }
+    for (int k = 0; k < 3; ++k) { b->bounds[k] = n ? root.mn[k] : 0.f; b->bounds[3 + k] = n ? root.mx[k] : 0.f; }
+    if (n > 0) {
+        int nt = pr.n_threads > 0 ? pr.n_threads : (int)std::max(1u, std::thread::hardware_concurrency());
+        nt = std::min(nt, 64);
+        B.n_nodes = 1;
+        if (nt > 1 && n > 65536) {
+            Pool pool(nt);
+            B.pool = &pool;
+            pool.submit([&] { B.subtree(0, 0, n, 1); });
+            pool.wait();
+        } else {
+            B.pool = nullptr;
+            B.subtree(0, 0, n, 1);
+        }
+        b->nodes.resize((size_t)B.n_nodes.load());
+        b->depth = B.max_depth.load();
+        // SAH cost (relative to the root area) before padding
+        double ra = root.half_area(), cost = 0;
+        for (const BuildNode& nd : b->nodes) {
+            Box x; std::memcpy(x.mn, nd.bmin, 12); std::memcpy(x.mx, nd.bmax, 12);
+            cost += x.half_area() * (nd.left >= 0 ? (double)pr.cost_traversal : (double)pr.cost_intersect * nd.count);
+        }
+        b->sah = ra > 0 ? cost / ra : 0;
+        // Conservative padding (D:R10): the triangle test in fp32 may accept a hit a few ulps of the scene's
+        // coordinate range outside the triangle's exact box; boxes grow by 2^-17 of the largest |coordinate|.
+        float pad = maxabs * (1.0f / 131072.0f);
+        for (BuildNode& nd : b->nodes)
+            for (int k = 0; k < 3; ++k) { nd.bmin[k] -= pad; nd.bmax[k] += pad; }
+    } else {
+        b->nodes.clear(); b->depth = 0; b->sah = 0;
+    }
+    b->build_seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count();
+    return true;
+}
+
+int32_t crt_bvh_check_host(const crt_bvh* b)
+{
+    int32_t bad = 0;
+    if (b->n_tris == 0) return 0;
+    std::vector<uint8_t> seen((size_t)b->n_tris, 0);
+    for (const BuildNode& nd : b->nodes) {
+        if (nd.left >= 0) {
+            for (int32_t c : {nd.left, nd.right}) {
+                const BuildNode& ch = b->nodes[c];
+                for (int k = 0; k < 3; ++k) if (ch.bmin[k] < nd.bmin[k] || ch.bmax[k] > nd.bmax[k]) bad |= 1;
+            }
+        } else {
+            if (nd.count < 1 || nd.count > b->max_leaf) bad |= 2;
+            for (int j = 0; j < nd.count; ++j) {
+                int32_t p = b->prim[nd.first + j];
+                if (p < 0 || p >= b->n_tris) { bad |= 32; continue; }
+                if (seen[p]) bad |= 4;
+                seen[p] = 1;
+                const float* tv = b->verts.data() + 9 * (int64_t)p;
+                for (int v = 0; v < 3; ++v) for (int k = 0; k < 3; ++k)
+                    if (tv[3 * v + k] < nd.bmin[k] || tv[3 * v + k] > nd.bmax[k]) bad |= 8;
+            }
+        }
+    }
+    for (uint8_t s : seen) if (!s) bad |= 16;
+    return bad;
+}
+
+// Flattens the host tree into the traversal layout (host vectors; the caller uploads them).
+void crt_bvh_flatten(const crt_bvh* b, std::vector<GpuNode>& gn, std::vector<GpuTri>& gt, std::vector<int32_t>& slot_of_prim)
+{
+    const float inf = std::numeric_limits<float>::infinity();
+    const int64_t n = b->n_tris;
+    gt.resize((size_t)n); slot_of_prim.assign((size_t)n, -1);
+    for (int64_t j = 0; j < n; ++j) {
+        int32_t p = b->prim[j];
+        const float* tv = b->verts.data() + 9 * (int64_t)p;
+        GpuTri t;
+        t.v0p = make_float4(tv[0], tv[1], tv[2], 0.f);
+        std::memcpy(&t.v0p.w, &p, 4);
+        t.e1 = make_float4(tv[3] - tv[0], tv[4] - tv[1], tv[5] - tv[2], 0.f);
+        t.e2 = make_float4(tv[6] - tv[0], tv[7] - tv[1], tv[8] - tv[2], 0.f);
+        gt[j] = t; slot_of_prim[p] = (int32_t)j;
+    }
+    auto leaf_ref = [](const BuildNode& nd) { return ~((nd.first << 3) | (nd.count - 1)); };
+    auto empty_node = [&] {
+        GpuNode g; g.xy0 = g.xy1 = make_float4(inf, -inf, inf, -inf); g.z01 = make_float4(inf, -inf, inf, -inf);
+        g.ref0 = g.ref1 = ~0; g.pad0 = g.pad1 = 0; return g;
+    };
+    gn.clear();
+    if (n == 0) { gn.push_back(empty_node()); return; }
+    if (b->nodes[0].left < 0) {      // the whole scene is one leaf: a root whose second child is empty
+        GpuNode g = empty_node(); const BuildNode& r = b->nodes[0];
+        g.xy0 = make_float4(r.bmin[0], r.bmax[0], r.bmin[1], r.bmax[1]); g.z01.x = r.bmin[2]; g.z01.y = r.bmax[2];
+        g.ref0 = leaf_ref(r); gn.push_back(g); return;
+    }
+    // depth-first numbering of inner nodes, left child next to its parent
+    std::vector<int32_t> gpu_index(b->nodes.size(), -1), stack{0}, order;
+    while (!stack.empty()) {
+        int32_t i = stack.back(); stack.pop_back();
+        gpu_index[i] = (int32_t)order.size(); order.push_back(i);
+        const BuildNode& nd = b->nodes[i];
+        if (b->nodes[nd.right].left >= 0) stack.push_back(nd.right);
+        if (b->nodes[nd.left].left >= 0) stack.push_back(nd.left);
+    }
+    gn.resize(order.size());
+    for (size_t k = 0; k < order.size(); ++k) {
+        const BuildNode& nd = b->nodes[order[k]];
+        const BuildNode& l = b->nodes[nd.left]; const BuildNode& r = b->nodes[nd.right];
+        GpuNode g;
+        g.xy0 = make_float4(l.bmin[0], l.bmax[0], l.bmin[1], l.bmax[1]);
+        g.xy1 = make_float4(r.bmin[0], r.bmax[0], r.bmin[1], r.bmax[1]);
+        g.z01 = make_float4(l.bmin[2], l.bmax[2], r.bmin[2], r.bmax[2]);
+        g.ref0 = l.left >= 0 ? gpu_index[nd.left] : leaf_ref(l);
+        g.ref1 = r.left >= 0 ? gpu_index[nd.right] : leaf_ref(r);
+        g.pad0 = g.pad1 = 0;
+        gn[k] = g;
+    }
+}

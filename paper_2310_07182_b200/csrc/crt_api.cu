@@ -1,0 +1,416 @@
+// C ABI of libcrt (include/crt.h): argument checking, BVH upload, and the per-frame call sequence.
+#include <cstring>
+#include <thread>
+#include "crt_internal.h"
+
+bool crt_bvh_build_host(crt_bvh* b, const float* verts, int64_t n, const crt_bvh_params& pr);
+int32_t crt_bvh_check_host(const crt_bvh* b);
+void crt_bvh_flatten(const crt_bvh* b, std::vector<GpuNode>& gn, std::vector<GpuTri>& gt, std::vector<int32_t>& slot_of_prim);
+
+static thread_local std::string g_last_error;
+
+crt_status crt_fail(crt_ctx* ctx, crt_status st, const char* fmt, ...)
+{
+    char buf[512];
+    va_list ap; va_start(ap, fmt); vsnprintf(buf, sizeof buf, fmt, ap); va_end(ap);
+    if (ctx) ctx->last_error = buf;
+    g_last_error = buf;
+    return st;
+}
+
+static int ilog2(int v) { int l = 0; while ((1 << l) < v) ++l; return l; }
+static bool is_pow2(int v) { return v > 0 && (v & (v - 1)) == 0; }
+
+crt_status crt_make_layout(crt_ctx* ctx, const crt_frame* f, const crt_order* o, Layout* L)
+{
+    if (!f || !o || !L) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "layout: null argument");
+    if (f->w < 0 || f->h < 0 || f->spp < 1) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "layout: bad frame %dx%d spp %d", f->w, f->h, f->spp);
+    if (o->mode < 0 || o->mode > 2) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "layout: mode %d out of range", o->mode);
+    memset(L, 0, sizeof *L);
+    L->w = f->w; L->h = f->h; L->spp = f->spp; L->mode = o->mode;
+    L->n_paths = (int64_t)f->spp * f->w * f->h;
+    if (L->n_paths >= ((int64_t)1 << 31)) return crt_fail(ctx, CRT_ERR_UNSUPPORTED, "layout: more than 2^31 paths");
+    if (o->mode != CRT_MODE_DIRECT_REUSE) {
+        L->W = L->H = L->M = L->K = L->G = 1; L->tiles_x = f->w; L->tiles_y = f->h; L->n_tiles = f->w * f->h;
+        L->n_slots = L->n_paths; L->n_groups = L->n_paths;
+        return CRT_OK;
+    }
+    if (!is_pow2(o->group_w) || !is_pow2(o->group_h) || !is_pow2(o->stride))
+        return crt_fail(ctx, CRT_ERR_UNSUPPORTED, "layout: group %dx%d stride %d must be powers of two", o->group_w, o->group_h, o->stride);
+    const int64_t M = (int64_t)o->group_w * o->stride * o->group_h * o->stride, K = (int64_t)o->group_w * o->group_h;
+    if (M > 4096 || K > 1024) return crt_fail(ctx, CRT_ERR_UNSUPPORTED, "layout: tile of %lld slots / group of %lld exceeds 4096 / 1024", (long long)M, (long long)K);
+    L->W = o->group_w * o->stride; L->H = o->group_h * o->stride; L->M = (int)M; L->K = (int)K; L->G = (int)(M / K);
+    L->log2W = ilog2(L->W); L->log2M = ilog2(L->M); L->log2K = ilog2(L->K);
+    L->tiles_x = (f->w + L->W - 1) / L->W; L->tiles_y = (f->h + L->H - 1) / L->H; L->n_tiles = L->tiles_x * L->tiles_y;
+    L->n_slots = (int64_t)f->spp * L->n_tiles * L->M; L->n_groups = L->n_slots / L->K;
+    if (L->n_slots >= ((int64_t)1 << 31)) return crt_fail(ctx, CRT_ERR_UNSUPPORTED, "layout: more than 2^31 slots");
+    return CRT_OK;
+}
+
+extern "C" {
+
+crt_status crt_create(int32_t device, crt_ctx** out)
+{
+    if (!out) return crt_fail(nullptr, CRT_ERR_INVALID_ARG, "crt_create: out is null");
+    *out = nullptr;
+    int count = 0;
+    cudaError_t e = cudaGetDeviceCount(&count);
+    if (e != cudaSuccess || count == 0) return crt_fail(nullptr, CRT_ERR_CUDA, "crt_create: no CUDA device (%s); libcrt has no CPU fallback", cudaGetErrorString(e));
+    if (device < 0 || device >= count) return crt_fail(nullptr, CRT_ERR_INVALID_ARG, "crt_create: device %d out of range [0,%d)", device, count);
+    CRT_CUDA(nullptr, cudaSetDevice(device));
+    cudaDeviceProp prop;
+    CRT_CUDA(nullptr, cudaGetDeviceProperties(&prop, device));
+    if (prop.major < 10) return crt_fail(nullptr, CRT_ERR_UNSUPPORTED, "crt_create: device is sm_%d%d; libcrt is built for sm_100a only", prop.major, prop.minor);
+    crt_ctx* c = new crt_ctx();
+    c->device = device; c->n_sms = prop.multiProcessorCount;
+    if (cudaMalloc(&c->d_counter, 256) != cudaSuccess) { delete c; return crt_fail(nullptr, CRT_ERR_NOMEM, "crt_create: cudaMalloc failed"); }
+    *out = c;
+    return CRT_OK;
+}
+
+crt_status crt_destroy(crt_ctx* ctx)
+{
+    if (!ctx) return CRT_OK;
+    cudaFree(ctx->d_counter);
+    for (cudaEvent_t ev : ctx->ev) cudaEventDestroy(ev);
+    delete ctx;
+    return CRT_OK;
+}
+
+const char* crt_last_error(const crt_ctx* ctx) { return ctx ? ctx->last_error.c_str() : g_last_error.c_str(); }
+
+crt_status crt_set_option(crt_ctx* ctx, const char* key, int64_t value)
+{
+    if (!ctx || !key) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "set_option: null argument");
+    if (!strcmp(key, "trace_kernel")) { if (value < 0 || value > 1) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "trace_kernel must be 0 or 1"); ctx->trace_kernel = (int)value; }
+    else if (!strcmp(key, "trace_blocks_per_sm")) { if (value < 0 || value > 32) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "trace_blocks_per_sm out of range"); ctx->trace_blocks_per_sm = (int)value; }
+    else return crt_fail(ctx, CRT_ERR_INVALID_ARG, "set_option: unknown key '%s'", key);
+    return CRT_OK;
+}
+
+crt_status crt_measure_peaks(crt_ctx* ctx, double* fp32_tflops, double* copy_gbs)
+{
+    if (!ctx || !fp32_tflops || !copy_gbs) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "measure_peaks: null argument");
+    return measure_peaks(ctx, fp32_tflops, copy_gbs);
+}
+
+// ---- BVH ----------------------------------------------------------------------------------------------
+static bool is_device_ptr(const void* p)
+{
+    cudaPointerAttributes a;
+    if (cudaPointerGetAttributes(&a, p) != cudaSuccess) { cudaGetLastError(); return false; }
+    return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
+}
+
+crt_status crt_build_bvh(crt_ctx* ctx, const float* verts, const int32_t* mat_id, int64_t n_tris, const crt_bvh_params* params, crt_bvh** out)
+{
+    if (!out) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "build_bvh: out is null");
+    *out = nullptr;
+    if (n_tris < 0 || (n_tris > 0 && !verts)) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "build_bvh: bad triangle array");
+    if (n_tris >= ((int64_t)1 << 28)) return crt_fail(ctx, CRT_ERR_UNSUPPORTED, "build_bvh: more than 2^28 triangles");
+    crt_bvh_params pr = {4, 16, 1.0f, 1.0f, 0};
+    if (params) pr = *params;
+    if (pr.max_leaf < 1 || pr.max_leaf > 8) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "build_bvh: max_leaf %d not in [1,8]", pr.max_leaf);
+    if (pr.sah_bins == 0) pr.sah_bins = 16;
+    std::vector<float> hv; std::vector<int32_t> hm((size_t)n_tris, 0);
+    const float* v = verts;
+    if (ctx && n_tris > 0 && is_device_ptr(verts)) {
+        hv.resize((size_t)n_tris * 9);
+        CRT_CUDA(ctx, cudaMemcpy(hv.data(), verts, hv.size() * 4, cudaMemcpyDeviceToHost));
+        v = hv.data();
+    }
+    if (mat_id && n_tris > 0) {
+        if (ctx && is_device_ptr(mat_id)) CRT_CUDA(ctx, cudaMemcpy(hm.data(), mat_id, hm.size() * 4, cudaMemcpyDeviceToHost));
+        else memcpy(hm.data(), mat_id, hm.size() * 4);
+    }
+    for (int64_t i = 0; i < 9 * n_tris; ++i) if (!(v[i] == v[i]) || v[i] > 1e30f || v[i] < -1e30f) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "build_bvh: non-finite vertex");
+    crt_bvh* b = new crt_bvh();
+    crt_bvh_build_host(b, v, n_tris, pr);
+    if (b->depth > 60) { delete b; return crt_fail(ctx, CRT_ERR_UNSUPPORTED, "build_bvh: tree depth exceeds the traversal stack (64)"); }
+    if (ctx) {
+        std::vector<GpuNode> gn; std::vector<GpuTri> gt; std::vector<int32_t> sop;
+        crt_bvh_flatten(b, gn, gt, sop);
+        b->device = ctx->device; b->n_gpu_nodes = (int64_t)gn.size();
+        auto up = [&](void** d, const void* h, size_t bytes) -> cudaError_t {
+            cudaError_t e = cudaMalloc(d, bytes ? bytes : 256);
+            if (e != cudaSuccess) return e;
+            b->device_bytes += (int64_t)bytes;
+            return bytes ? cudaMemcpy(*d, h, bytes, cudaMemcpyHostToDevice) : cudaSuccess;
+        };
+        cudaError_t e = up((void**)&b->d_nodes, gn.data(), gn.size() * sizeof(GpuNode));
+        if (e == cudaSuccess) e = up((void**)&b->d_tris, gt.data(), gt.size() * sizeof(GpuTri));
+        if (e == cudaSuccess) e = up((void**)&b->d_slot_of_prim, sop.data(), sop.size() * 4);
+        if (e == cudaSuccess) e = up((void**)&b->d_mat_id, hm.data(), hm.size() * 4);
+        if (e != cudaSuccess) { crt_bvh_destroy(b); return crt_fail(ctx, e == cudaErrorMemoryAllocation ? CRT_ERR_NOMEM : CRT_ERR_CUDA, "build_bvh: upload: %s", cudaGetErrorString(e)); }
+    }
+    *out = b;
+    return CRT_OK;
+}
+
+crt_status crt_bvh_destroy(crt_bvh* b)
+{
+    if (!b) return CRT_OK;
+    cudaFree(b->d_nodes); cudaFree(b->d_tris); cudaFree(b->d_slot_of_prim); cudaFree(b->d_mat_id);
+    delete b;
+    return CRT_OK;
+}
+
+crt_status crt_bvh_get_info(const crt_bvh* b, crt_bvh_info_t* o)
+{
+    if (!b || !o) return crt_fail(nullptr, CRT_ERR_INVALID_ARG, "bvh_get_info: null argument");
+    o->n_tris = b->n_tris; o->n_nodes = (int64_t)b->nodes.size(); o->device_bytes = b->device_bytes;
+    memcpy(o->bounds, b->bounds, sizeof o->bounds);
+    o->sah_cost = b->sah; o->depth = b->depth; o->max_leaf = b->max_leaf; o->build_seconds = b->build_seconds;
+    return CRT_OK;
+}
+
+crt_status crt_bvh_check(const crt_bvh* b, int32_t* violations)
+{
+    if (!b || !violations) return crt_fail(nullptr, CRT_ERR_INVALID_ARG, "bvh_check: null argument");
+    *violations = crt_bvh_check_host(b);
+    return CRT_OK;
+}
+
+// ---- index spaces ---------------------------------------------------------------------------------------
+crt_status crt_layout(const crt_frame* frame, const crt_order* order, int64_t* n_paths, int64_t* n_slots, int64_t* n_groups)
+{
+    Layout L;
+    crt_status st = crt_make_layout(nullptr, frame, order, &L);
+    if (st != CRT_OK) return st;
+    if (n_paths) *n_paths = L.n_paths;
+    if (n_slots) *n_slots = L.n_slots;
+    if (n_groups) *n_groups = L.n_groups;
+    return CRT_OK;
+}
+
+#define NEED_CTX(name) if (!ctx) return crt_fail(nullptr, CRT_ERR_INVALID_ARG, name ": ctx is null")
+#define NEED_BVH(name) if (!bvh) return crt_fail(ctx, CRT_ERR_INVALID_ARG, name ": bvh is null"); \
+    if (!bvh->d_nodes || bvh->device != ctx->device) return crt_fail(ctx, CRT_ERR_STATE, name ": BVH has no data on this context's device")
+#define NEED_ALIGNED(name, p, a) if (!crt_aligned(p, a)) return crt_fail(ctx, CRT_ERR_INVALID_ARG, name ": " #p " is null or not %d-byte aligned", (int)(a))
+
+crt_status crt_paths_init(crt_ctx* ctx, crt_path_state* paths, int64_t n_paths, void* stream)
+{
+    NEED_CTX("paths_init");
+    if (n_paths < 0) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "paths_init: negative size");
+    if (n_paths == 0) return CRT_OK;
+    NEED_ALIGNED("paths_init", paths, 16);
+    return launch_paths_init(ctx, paths, n_paths, (cudaStream_t)stream);
+}
+
+crt_status crt_trace_primary(crt_ctx* ctx, const crt_bvh* bvh, const crt_camera* camera, const crt_frame* frame, const crt_order* order,
+                             crt_ray* rays, crt_hit* hits, int32_t* ray_to_path, void* stream)
+{
+    NEED_CTX("trace_primary"); NEED_BVH("trace_primary");
+    if (!camera) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "trace_primary: camera is null");
+    Layout L; crt_status st = crt_make_layout(ctx, frame, order, &L); if (st != CRT_OK) return st;
+    if (L.n_slots == 0) return CRT_OK;
+    NEED_ALIGNED("trace_primary", rays, 32); NEED_ALIGNED("trace_primary", hits, 16); NEED_ALIGNED("trace_primary", ray_to_path, 4);
+    return launch_primary(ctx, bvh, *camera, *frame, L, rays, hits, ray_to_path, (cudaStream_t)stream);
+}
+
+size_t crt_generate_secondary_scratch_bytes(const crt_frame* frame, const crt_order* order)
+{
+    Layout L; if (crt_make_layout(nullptr, frame, order, &L) != CRT_OK) return 0;
+    return generate_scratch_bytes(L);
+}
+
+crt_status crt_generate_secondary(crt_ctx* ctx, const crt_bvh* bvh, const crt_scene_mats* mats, const crt_frame* frame, int32_t bounce, const crt_order* order,
+                                  const crt_ray* prev_rays, const crt_hit* prev_hits, const int32_t* prev_ray_to_path, crt_path_state* paths,
+                                  crt_ray* rays_out, int32_t* ray_to_path_out, int32_t* group_id_out, int32_t* dir_src_out, uint8_t* group_class_out,
+                                  uint32_t* n_active_out, void* scratch, size_t scratch_bytes, void* stream)
+{
+    NEED_CTX("generate_secondary"); NEED_BVH("generate_secondary");
+    if (!mats || !mats->materials) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "generate_secondary: materials are null");
+    if (bounce < 1) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "generate_secondary: bounce %d < 1", bounce);
+    Layout L; crt_status st = crt_make_layout(ctx, frame, order, &L); if (st != CRT_OK) return st;
+    NEED_ALIGNED("generate_secondary", n_active_out, 4);
+    if (L.n_slots > 0) {
+        NEED_ALIGNED("generate_secondary", prev_rays, 32); NEED_ALIGNED("generate_secondary", prev_hits, 16);
+        NEED_ALIGNED("generate_secondary", prev_ray_to_path, 4); NEED_ALIGNED("generate_secondary", paths, 16);
+        NEED_ALIGNED("generate_secondary", rays_out, 32); NEED_ALIGNED("generate_secondary", ray_to_path_out, 4);
+        NEED_ALIGNED("generate_secondary", group_id_out, 4); NEED_ALIGNED("generate_secondary", dir_src_out, 4);
+        NEED_ALIGNED("generate_secondary", group_class_out, 1); NEED_ALIGNED("generate_secondary", scratch, 16);
+        if (rays_out == prev_rays) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "generate_secondary: rays_out aliases prev_rays");
+    }
+    return launch_generate(ctx, bvh, *mats, *frame, bounce, L, prev_rays, prev_hits, prev_ray_to_path, paths, rays_out, ray_to_path_out, group_id_out,
+                           dir_src_out, group_class_out, n_active_out, scratch, scratch_bytes, (cudaStream_t)stream, nullptr);
+}
+
+crt_status crt_morton_encode(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, uint32_t* keys, void* stream)
+{
+    NEED_CTX("morton_encode");
+    if (!bvh) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "morton_encode: bvh is null");
+    if (n < 0) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "morton_encode: negative size");
+    if (n == 0) return CRT_OK;
+    NEED_ALIGNED("morton_encode", rays, 32); NEED_ALIGNED("morton_encode", keys, 4);
+    return launch_morton_encode(ctx, bvh->bounds, rays, n, keys, (cudaStream_t)stream);
+}
+
+size_t crt_radix_sort_scratch_bytes(int64_t n) { return n < 0 ? 0 : radix_sort_scratch_bytes(n); }
+
+crt_status crt_radix_sort_pairs(crt_ctx* ctx, const uint32_t* keys_in, const int32_t* vals_in, int64_t n, uint32_t* keys_out, int32_t* vals_out,
+                                void* scratch, size_t scratch_bytes, void* stream)
+{
+    NEED_CTX("radix_sort_pairs");
+    if (n < 0) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "radix_sort_pairs: negative size");
+    if (n == 0) return CRT_OK;
+    NEED_ALIGNED("radix_sort_pairs", keys_in, 4); NEED_ALIGNED("radix_sort_pairs", vals_in, 4);
+    NEED_ALIGNED("radix_sort_pairs", keys_out, 4); NEED_ALIGNED("radix_sort_pairs", vals_out, 4); NEED_ALIGNED("radix_sort_pairs", scratch, 16);
+    if (keys_out == keys_in || vals_out == vals_in) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "radix_sort_pairs: in-place sort is not supported");
+    return launch_radix_sort(ctx, keys_in, vals_in, n, keys_out, vals_out, scratch, scratch_bytes, (cudaStream_t)stream);
+}
+
+crt_status crt_trace(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n_rays, crt_hit* hits, void* stream)
+{
+    NEED_CTX("trace"); NEED_BVH("trace");
+    if (n_rays < 0) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "trace: negative ray count");
+    if (n_rays == 0) return CRT_OK;
+    if (n_rays >= ((int64_t)1 << 31)) return crt_fail(ctx, CRT_ERR_UNSUPPORTED, "trace: more than 2^31 rays per call");
+    NEED_ALIGNED("trace", rays, 32); NEED_ALIGNED("trace", hits, 16);
+    return launch_trace(ctx, bvh, rays, n_rays, hits, (cudaStream_t)stream);
+}
+
+crt_status crt_shade_accumulate(crt_ctx* ctx, const crt_bvh* bvh, const crt_scene_mats* mats, const crt_frame* frame, int32_t bounce, int32_t is_last,
+                                const crt_ray* rays, const crt_hit* hits, const int32_t* ray_to_path, int64_t n_rays, crt_path_state* paths, float* accum, void* stream)
+{
+    NEED_CTX("shade_accumulate"); NEED_BVH("shade_accumulate");
+    if (!mats || !mats->materials || !frame) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "shade_accumulate: null argument");
+    if (bounce < 0 || n_rays < 0 || frame->spp < 1) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "shade_accumulate: bad bounce / size");
+    if (n_rays == 0) return CRT_OK;
+    NEED_ALIGNED("shade_accumulate", rays, 32); NEED_ALIGNED("shade_accumulate", hits, 16); NEED_ALIGNED("shade_accumulate", ray_to_path, 4);
+    NEED_ALIGNED("shade_accumulate", paths, 16); NEED_ALIGNED("shade_accumulate", accum, 4);
+    return launch_shade(ctx, bvh, *mats, *frame, is_last, rays, hits, ray_to_path, n_rays, paths, accum, (cudaStream_t)stream);
+}
+
+// ---- whole frame ------------------------------------------------------------------------------------------
+static size_t al(size_t x) { return (x + 255) & ~(size_t)255; }
+struct Workspace {
+    crt_ray* rays[2]; crt_hit* hits; int32_t* r2p[2]; int32_t* gid; int32_t* src; uint8_t* cls; crt_path_state* paths; uint32_t* n_active; void* scratch; size_t scratch_bytes;
+    size_t total;
+};
+static Workspace carve(const Layout& L, void* base)
+{
+    Workspace W; char* p = static_cast<char*>(base); size_t off = 0;
+    const size_t ns = (size_t)L.n_slots;
+    auto take = [&](size_t bytes) { void* r = p ? p + off : nullptr; off += al(bytes); return r; };
+    W.rays[0] = (crt_ray*)take(ns * 32); W.rays[1] = (crt_ray*)take(ns * 32); W.hits = (crt_hit*)take(ns * 16);
+    W.r2p[0] = (int32_t*)take(ns * 4); W.r2p[1] = (int32_t*)take(ns * 4); W.gid = (int32_t*)take(ns * 4); W.src = (int32_t*)take(ns * 4);
+    W.cls = (uint8_t*)take((size_t)L.n_groups); W.paths = (crt_path_state*)take((size_t)L.n_paths * 32); W.n_active = (uint32_t*)take(256);
+    W.scratch_bytes = generate_scratch_bytes(L); W.scratch = take(W.scratch_bytes);
+    W.total = off;
+    return W;
+}
+
+size_t crt_frame_workspace_bytes(const crt_frame* frame, const crt_order* order)
+{
+    Layout L; if (crt_make_layout(nullptr, frame, order, &L) != CRT_OK) return 0;
+    return carve(L, nullptr).total;
+}
+
+static crt_status mark(crt_ctx* ctx, int stage, cudaStream_t st)
+{
+    if ((size_t)ctx->ev_used == ctx->ev.size()) { cudaEvent_t e; CRT_CUDA(ctx, cudaEventCreate(&e)); ctx->ev.push_back(e); ctx->ev_stage.push_back(-1); }
+    ctx->ev_stage[ctx->ev_used] = stage;
+    CRT_CUDA(ctx, cudaEventRecord(ctx->ev[ctx->ev_used++], st));
+    return CRT_OK;
+}
+
+crt_status crt_render_frame(crt_ctx* ctx, const crt_bvh* bvh, const crt_scene_mats* mats, const crt_camera* camera, const crt_frame* frame,
+                            const crt_order* order, int32_t n_bounces, float* accum, uint32_t* n_secondary_out, void* workspace, size_t workspace_bytes,
+                            int32_t record_times, void* stream)
+{
+    NEED_CTX("render_frame"); NEED_BVH("render_frame");
+    if (!mats || !mats->materials || !camera) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "render_frame: null argument");
+    if (n_bounces < 0 || n_bounces > 64) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "render_frame: n_bounces out of range");
+    Layout L; crt_status st = crt_make_layout(ctx, frame, order, &L); if (st != CRT_OK) return st;
+    if (L.n_slots == 0) return CRT_OK;
+    NEED_ALIGNED("render_frame", workspace, 256); NEED_ALIGNED("render_frame", accum, 4);
+    Workspace W = carve(L, workspace);
+    if (workspace_bytes < W.total) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "render_frame: workspace %zu < %zu bytes", workspace_bytes, W.total);
+    cudaStream_t s = (cudaStream_t)stream;
+    ctx->ev_used = 0;
+#define STEP(call) do { st = (call); if (st != CRT_OK) return st; } while (0)
+#define MARK(stage) do { if (record_times) STEP(mark(ctx, stage, s)); } while (0)
+    STEP(launch_paths_init(ctx, W.paths, L.n_paths, s));
+    MARK(-1);
+    STEP(launch_primary(ctx, bvh, *camera, *frame, L, W.rays[0], W.hits, W.r2p[0], s));
+    MARK(0);
+    STEP(launch_shade(ctx, bvh, *mats, *frame, n_bounces == 0, W.rays[0], W.hits, W.r2p[0], L.n_slots, W.paths, accum, s));
+    MARK(1);
+    int cur = 0;
+    for (int b = 1; b <= n_bounces; ++b) {
+        cudaEvent_t ev4[2] = {nullptr, nullptr};
+        if (record_times && L.mode == CRT_MODE_MORTON_REORDER) {
+            // events bracketing encode+sort+permute inside generate
+            while (ctx->ev.size() < (size_t)ctx->ev_used + 2) { cudaEvent_t e; CRT_CUDA(ctx, cudaEventCreate(&e)); ctx->ev.push_back(e); ctx->ev_stage.push_back(-1); }
+            ev4[0] = ctx->ev[ctx->ev_used]; ctx->ev_stage[ctx->ev_used++] = -2;     // after the generate kernel: opens stage 4
+            ev4[1] = ctx->ev[ctx->ev_used]; ctx->ev_stage[ctx->ev_used++] = 4;      // after permute: closes stage 4
+        }
+        STEP(launch_generate(ctx, bvh, *mats, *frame, b, L, W.rays[cur], W.hits, W.r2p[cur], W.paths, W.rays[1 - cur], W.r2p[1 - cur], W.gid, W.src, W.cls,
+                             W.n_active, W.scratch, W.scratch_bytes, s, ev4[0] ? ev4 : nullptr));
+        cur = 1 - cur;
+        if (n_secondary_out) CRT_CUDA(ctx, cudaMemcpyAsync(n_secondary_out + (b - 1), W.n_active, 4, cudaMemcpyDeviceToDevice, s));
+        MARK(2);
+        STEP(launch_trace(ctx, bvh, W.rays[cur], L.n_slots, W.hits, s));
+        MARK(3);
+        STEP(launch_shade(ctx, bvh, *mats, *frame, b == n_bounces, W.rays[cur], W.hits, W.r2p[cur], L.n_slots, W.paths, accum, s));
+        MARK(1);
+    }
+#undef STEP
+#undef MARK
+    return CRT_OK;
+}
+
+crt_status crt_frame_times(crt_ctx* ctx, float* stage_ms)
+{
+    NEED_CTX("frame_times");
+    if (!stage_ms) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "frame_times: null argument");
+    if (ctx->ev_used == 0) return CRT_OK;
+    CRT_CUDA(ctx, cudaEventSynchronize(ctx->ev[ctx->ev_used - 1]));
+    // events are recorded in stream order; an event with stage >= 0 closes the interval opened by the previous event
+    // on the main timeline (stage 4 intervals are nested inside a stage-2 interval)
+    int prev_main = -1, open4 = -1;
+    for (int i = 0; i < ctx->ev_used; ++i) {
+        const int stg = ctx->ev_stage[i];
+        if (stg == -2) { open4 = i; continue; }
+        if (stg == 4) { float ms = 0; CRT_CUDA(ctx, cudaEventElapsedTime(&ms, ctx->ev[open4], ctx->ev[i])); stage_ms[4] += ms; continue; }
+        if (stg >= 0 && prev_main >= 0) { float ms = 0; CRT_CUDA(ctx, cudaEventElapsedTime(&ms, ctx->ev[prev_main], ctx->ev[i])); stage_ms[stg] += ms; }
+        prev_main = i;
+    }
+    return CRT_OK;
+}
+
+size_t crt_frame_host_extra_bytes(const crt_frame* frame, int32_t n_materials)
+{
+    if (!frame || n_materials < 0) return 0;
+    return al((size_t)n_materials * sizeof(crt_material)) + al((size_t)frame->w * frame->h * 12) + al(64 * 4) + 256;
+}
+
+crt_status crt_render_frame_host(crt_ctx* ctx, const crt_bvh* bvh, const crt_material* materials_host, int32_t n_materials, const float* env,
+                                 const crt_camera* camera, const crt_frame* frame, const crt_order* order, int32_t n_bounces, float* accum_host,
+                                 uint32_t* n_secondary_host, void* workspace, size_t workspace_bytes, void* stream)
+{
+    NEED_CTX("render_frame_host"); NEED_BVH("render_frame_host");
+    if (!materials_host || !env || !camera || !frame || !accum_host || n_materials < 1) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "render_frame_host: null argument");
+    Layout L; crt_status st = crt_make_layout(ctx, frame, order, &L); if (st != CRT_OK) return st;
+    NEED_ALIGNED("render_frame_host", workspace, 256);
+    const size_t core = carve(L, nullptr).total, extra = crt_frame_host_extra_bytes(frame, n_materials);
+    if (workspace_bytes < core + extra) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "render_frame_host: workspace %zu < %zu bytes", workspace_bytes, core + extra);
+    cudaStream_t s = (cudaStream_t)stream;
+    char* p = static_cast<char*>(workspace) + core;
+    crt_material* d_mats = (crt_material*)p; p += al((size_t)n_materials * sizeof(crt_material));
+    float* d_accum = (float*)p; p += al((size_t)frame->w * frame->h * 12);
+    uint32_t* d_nsec = (uint32_t*)p;
+    const size_t img = (size_t)frame->w * frame->h * 12;
+    CRT_CUDA(ctx, cudaMemcpyAsync(d_mats, materials_host, (size_t)n_materials * sizeof(crt_material), cudaMemcpyHostToDevice, s));
+    CRT_CUDA(ctx, cudaMemcpyAsync(d_accum, accum_host, img, cudaMemcpyHostToDevice, s));
+    crt_scene_mats sm; sm.materials = d_mats; sm.n_materials = n_materials; memcpy(sm.env, env, sizeof sm.env);
+    st = crt_render_frame(ctx, bvh, &sm, camera, frame, order, n_bounces, d_accum, n_secondary_host ? d_nsec : nullptr, workspace, core, 0, stream);
+    if (st != CRT_OK) return st;
+    CRT_CUDA(ctx, cudaMemcpyAsync(accum_host, d_accum, img, cudaMemcpyDeviceToHost, s));
+    if (n_secondary_host && n_bounces > 0) CRT_CUDA(ctx, cudaMemcpyAsync(n_secondary_host, d_nsec, 4 * (size_t)n_bounces, cudaMemcpyDeviceToHost, s));
+    CRT_CUDA(ctx, cudaStreamSynchronize(s));
+    return CRT_OK;
+}
+
+}  // extern "C"

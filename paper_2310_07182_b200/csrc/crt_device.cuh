@@ -1,0 +1,106 @@
+// Device-side arithmetic of libcrt.  Every floating-point operation of the METHOD (ray generation,
+// triangle intersection, sampling, shading) is written with explicit round-to-nearest intrinsics so
+// the compiler cannot contract a*b+c into an FMA: the result is one IEEE binary32 rounding per
+// written operation (D:R0).  Only the conservative BVH box test may use FMA.
+#pragma once
+#include <cuda_runtime.h>
+#include <cstdint>
+
+#define CRT_DEV __device__ __forceinline__
+
+namespace crt {
+
+struct V3 { float x, y, z; };
+CRT_DEV V3 mk(float x, float y, float z) { V3 r; r.x = x; r.y = y; r.z = z; return r; }
+CRT_DEV float mul(float a, float b) { return __fmul_rn(a, b); }
+CRT_DEV float add(float a, float b) { return __fadd_rn(a, b); }
+CRT_DEV float sub(float a, float b) { return __fsub_rn(a, b); }
+CRT_DEV float dvd(float a, float b) { return __fdiv_rn(a, b); }
+CRT_DEV float sqr(float a) { return __fsqrt_rn(a); }
+CRT_DEV V3 vsub(V3 a, V3 b) { return mk(sub(a.x, b.x), sub(a.y, b.y), sub(a.z, b.z)); }
+CRT_DEV float dot(V3 a, V3 b) { return add(add(mul(a.x, b.x), mul(a.y, b.y)), mul(a.z, b.z)); }   // ((x+y)+z)
+CRT_DEV V3 cross(V3 a, V3 b)
+{
+    return mk(sub(mul(a.y, b.z), mul(a.z, b.y)), sub(mul(a.z, b.x), mul(a.x, b.z)), sub(mul(a.x, b.y), mul(a.y, b.x)));
+}
+
+// ---- Philox4x32-10 (Salmon et al. 2011); key = (seed, frame), counter = (index, sample, bounce, purpose); D:R2
+enum { PURPOSE_CAMERA = 0, PURPOSE_BSDF = 1, PURPOSE_TILE = 2, PURPOSE_LEADER = 3 };
+CRT_DEV uint4 philox(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0, uint32_t k1)
+{
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+        uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+        uint32_t n0 = hi1 ^ c1 ^ k0, n2 = hi0 ^ c3 ^ k1;
+        c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+    }
+    return make_uint4(c0, c1, c2, c3);
+}
+CRT_DEV float u01(uint32_t r) { return mul((float)(r >> 8), 5.9604644775390625e-8f); }   // top 24 bits * 2^-24, exact
+
+// sin/cos of 2*pi*u: quadrant reduction + Taylor polynomials on |x| <= pi/4, Horner (D:R9)
+CRT_DEV void sincos2pi(float u, float& sn, float& cs)
+{
+    int k = (int)add(mul(u, 4.0f), 0.5f);
+    float r = sub(u, mul((float)k, 0.25f));
+    float x = mul(r, 6.2831853071795864769f);
+    float x2 = mul(x, x);
+    float s = mul(x, add(1.0f, mul(x2, add(-1.0f / 6.0f, mul(x2, add(1.0f / 120.0f, mul(x2, add(-1.0f / 5040.0f, mul(x2, 1.0f / 362880.0f)))))))));
+    float c = add(1.0f, mul(x2, add(-0.5f, mul(x2, add(1.0f / 24.0f, mul(x2, add(-1.0f / 720.0f, mul(x2, 1.0f / 40320.0f))))))));
+    switch (k & 3) {
+    case 0: sn = s; cs = c; break;
+    case 1: sn = c; cs = -s; break;
+    case 2: sn = -s; cs = -c; break;
+    default: sn = -c; cs = s; break;
+    }
+}
+
+// ---- Moller-Trumbore, two-sided; NaN/inf rejects (D:R10).  e1, e2 are stored pre-subtracted.
+CRT_DEV bool tri_test(V3 v0, V3 e1, V3 e2, V3 o, V3 d, float tmin, float tmax, float& t, float& u, float& v)
+{
+    V3 p = cross(d, e2);
+    float det = dot(e1, p);
+    float inv = dvd(1.0f, det);
+    V3 s = vsub(o, v0);
+    u = mul(dot(s, p), inv);
+    V3 q = cross(s, e1);
+    v = mul(dot(d, q), inv);
+    t = mul(dot(e2, q), inv);
+    return (u >= 0.0f) && (v >= 0.0f) && (add(u, v) <= 1.0f) && (t > tmin) && (t < tmax);
+}
+
+// ---- slot space (D:R3-R5) ---------------------------------------------------------------------
+struct DevLayout {
+    int32_t w, h, spp, reuse;
+    int32_t W, H, M, K, tiles_x, n_tiles, log2W, log2M, log2K;
+    uint32_t seed, frame;
+};
+// inverse of an odd number modulo 2^32 (Newton steps double the number of valid bits; a*a == 1 mod 8)
+CRT_DEV uint32_t inv_odd(uint32_t a)
+{
+    uint32_t x = a;
+    x *= 2u - a * x; x *= 2u - a * x; x *= 2u - a * x; x *= 2u - a * x;
+    return x;
+}
+// path id of a slot (-1 = out-of-image slot) with its pixel and sample.  direct_reuse: the slot's position m in its
+// tile is the shuffled number m = (a*n + c) mod M of pixel n = ly*W + lx, so n = a^-1 (m - c) mod M.
+CRT_DEV int32_t slot_to_path(const DevLayout& L, int64_t slot, int32_t& pixel, int32_t& sample)
+{
+    if (!L.reuse) { pixel = (int32_t)(slot % ((int64_t)L.w * L.h)); sample = (int32_t)(slot / ((int64_t)L.w * L.h)); return (int32_t)slot; }
+    const uint32_t m = (uint32_t)(slot & (L.M - 1));
+    const int64_t blk = slot >> L.log2M;
+    const int32_t tile = (int32_t)(blk % L.n_tiles);
+    sample = (int32_t)(blk / L.n_tiles);
+    const uint4 r = philox((uint32_t)tile, (uint32_t)sample, 0u, PURPOSE_TILE, L.seed, L.frame);
+    const uint32_t a = (r.x & (uint32_t)(L.M - 1)) | 1u, c = r.y & (uint32_t)(L.M - 1);
+    const uint32_t nn = (inv_odd(a) * (m - c)) & (uint32_t)(L.M - 1);
+    const int32_t lx = (int32_t)(nn & (uint32_t)(L.W - 1)), ly = (int32_t)(nn >> L.log2W);
+    const int32_t x = (tile % L.tiles_x) * L.W + lx, y = (tile / L.tiles_x) * L.H + ly;
+    if (x >= L.w || y >= L.h) { pixel = -1; return -1; }
+    pixel = y * L.w + x;
+    return (int32_t)(((int64_t)sample * L.h + y) * L.w + x);
+}
+
+}  // namespace crt

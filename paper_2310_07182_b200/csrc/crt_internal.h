@@ -1,0 +1,101 @@
+// Internal declarations of libcrt (host side).  Not installed; the public ABI is include/crt.h.
+#pragma once
+#include <cuda_runtime.h>
+#include <cstdarg>
+#include <cstdint>
+#include <cstdio>
+#include <string>
+#include <vector>
+#include "crt.h"
+
+struct crt_ctx {
+    int device = 0;
+    int n_sms = 0;
+    std::string last_error;
+    // options
+    int trace_kernel = 1;        // 0: one thread per ray, 1: persistent warps with dynamic fetch
+    int trace_block = 128;
+    int trace_blocks_per_sm = 0; // 0 = from occupancy
+    // persistent-kernel work counter
+    unsigned int* d_counter = nullptr;
+    // events for crt_render_frame(record_times)
+    std::vector<cudaEvent_t> ev;
+    std::vector<int> ev_stage;   // stage index closed by event i (-1: opening event)
+    int ev_used = 0;
+};
+
+// build-time tree node (host)
+struct BuildNode {
+    float bmin[3], bmax[3];
+    int32_t left = -1, right = -1;   // inner
+    int32_t first = 0, count = 0;    // leaf: range in prim order
+};
+
+// traversal layout (device): 64 bytes, two child boxes + two child references
+struct alignas(64) GpuNode {
+    float4 xy0;   // child0: min.x, max.x, min.y, max.y
+    float4 xy1;   // child1: min.x, max.x, min.y, max.y
+    float4 z01;   // child0 min.z, max.z, child1 min.z, max.z
+    int32_t ref0, ref1, pad0, pad1;   // >= 0: node index; < 0: ~((tri_offset << 3) | (count - 1))
+};
+// leaf triangle, 48 bytes: v0 | prim id, e1, e2  (e = v - v0 rounded once, as the intersection formula needs)
+struct GpuTri { float4 v0p; float4 e1; float4 e2; };
+
+struct crt_bvh {
+    int64_t n_tris = 0;
+    int max_leaf = 4;
+    std::vector<BuildNode> nodes;     // host tree (root = 0)
+    std::vector<int32_t> prim;        // leaf order -> caller's triangle id
+    std::vector<float> verts;         // host copy of the caller's vertices (for crt_bvh_check)
+    float bounds[6] = {0, 0, 0, 0, 0, 0};
+    double sah = 0; int depth = 0; double build_seconds = 0;
+    // device data
+    int device = -1;
+    GpuNode* d_nodes = nullptr; int64_t n_gpu_nodes = 0;
+    GpuTri* d_tris = nullptr;          // leaf order
+    int32_t* d_slot_of_prim = nullptr; // caller's triangle id -> index into d_tris
+    int32_t* d_mat_id = nullptr;       // by caller's triangle id
+    int64_t device_bytes = 0;
+};
+
+// error helpers -----------------------------------------------------------------------------------
+crt_status crt_fail(crt_ctx* ctx, crt_status st, const char* fmt, ...);
+#define CRT_CUDA(ctx, call)                                                                         \
+    do {                                                                                            \
+        cudaError_t e_ = (call);                                                                    \
+        if (e_ != cudaSuccess) return crt_fail(ctx, CRT_ERR_CUDA, "%s: %s", #call, cudaGetErrorString(e_)); \
+    } while (0)
+#define CRT_CHECK_LAUNCH(ctx, what)                                                                 \
+    do {                                                                                            \
+        cudaError_t e_ = cudaGetLastError();                                                        \
+        if (e_ != cudaSuccess) return crt_fail(ctx, CRT_ERR_CUDA, "launch %s: %s", what, cudaGetErrorString(e_)); \
+    } while (0)
+static inline bool crt_aligned(const void* p, size_t a) { return p != nullptr && (reinterpret_cast<uintptr_t>(p) % a) == 0; }
+
+// layout of the slot space ---------------------------------------------------------------------------
+struct Layout {
+    int32_t w, h, spp, mode;
+    int32_t W, H, M, K, G, tiles_x, tiles_y, n_tiles;
+    int32_t log2W, log2M, log2K;
+    int64_t n_paths, n_slots, n_groups;
+};
+crt_status crt_make_layout(crt_ctx* ctx, const crt_frame* f, const crt_order* o, Layout* L);
+
+// kernels' host launchers (defined in the .cu files) ------------------------------------------------------
+crt_status launch_trace(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, crt_hit* hits, cudaStream_t st);
+crt_status launch_primary(crt_ctx* ctx, const crt_bvh* bvh, const crt_camera& cam, const crt_frame& f, const Layout& L,
+                          crt_ray* rays, crt_hit* hits, int32_t* r2p, cudaStream_t st);
+crt_status launch_generate(crt_ctx* ctx, const crt_bvh* bvh, const crt_scene_mats& mats, const crt_frame& f, int bounce, const Layout& L,
+                           const crt_ray* prev_rays, const crt_hit* prev_hits, const int32_t* prev_r2p, crt_path_state* paths,
+                           crt_ray* rays_out, int32_t* r2p_out, int32_t* gid_out, int32_t* src_out, uint8_t* cls_out,
+                           uint32_t* n_active, void* scratch, size_t scratch_bytes, cudaStream_t st, cudaEvent_t* ev4);
+crt_status launch_morton_encode(crt_ctx* ctx, const float* bounds, const crt_ray* rays, int64_t n, uint32_t* keys, cudaStream_t st);
+crt_status launch_radix_sort(crt_ctx* ctx, const uint32_t* kin, const int32_t* vin, int64_t n, uint32_t* kout, int32_t* vout,
+                             void* scratch, size_t scratch_bytes, cudaStream_t st);
+size_t radix_sort_scratch_bytes(int64_t n);
+crt_status launch_shade(crt_ctx* ctx, const crt_bvh* bvh, const crt_scene_mats& mats, const crt_frame& f, int is_last,
+                        const crt_ray* rays, const crt_hit* hits, const int32_t* r2p, int64_t n, crt_path_state* paths, float* accum, cudaStream_t st);
+crt_status launch_paths_init(crt_ctx* ctx, crt_path_state* paths, int64_t n, cudaStream_t st);
+crt_status measure_peaks(crt_ctx* ctx, double* tflops, double* gbs);
+namespace crt { struct DevLayout; }
+size_t generate_scratch_bytes(const Layout& L);

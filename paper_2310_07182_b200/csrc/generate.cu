@@ -1,0 +1,341 @@
+// a2-a4: secondary-ray generation (sections 3.2 "Tangent Space Direction Reusing" and 3.3 "Interleaved
+// Grouping"; P:L103-105 group strategies; "shares directions between threads using shared memory").
+//
+// One thread per output slot.  In direct_reuse mode a group is K consecutive slots of one block, so the group's
+// material census, its leader and (hybrid groups) the glossy members' directions are exchanged through shared
+// memory; the shuffled pixel number m IS the slot, so the rays come out group-major with no sort (D:R5).
+// All arithmetic is the bit-exact fp32 sequence of crt_device.cuh (D:R0).
+#include "crt_device.cuh"
+#include "crt_internal.h"
+
+crt::DevLayout make_dev_layout(const Layout& L, const crt_frame& f);
+
+using namespace crt;
+
+namespace {
+
+struct Frame3 { V3 tx, ty, ng; };
+CRT_DEV V3 to_local(const Frame3& f, V3 w) { return mk(dot(w, f.tx), dot(w, f.ty), dot(w, f.ng)); }
+CRT_DEV V3 to_world(const Frame3& f, V3 l)
+{
+    return mk(add(add(mul(f.tx.x, l.x), mul(f.ty.x, l.y)), mul(f.ng.x, l.z)),
+              add(add(mul(f.tx.y, l.x), mul(f.ty.y, l.y)), mul(f.ng.y, l.z)),
+              add(add(mul(f.tx.z, l.x), mul(f.ty.z, l.y)), mul(f.ng.z, l.z)));
+}
+
+// cosine-weighted hemisphere sample (weight = albedo)
+CRT_DEV V3 sample_cosine(float u1, float u2)
+{
+    float r = sqr(u1), sn, cs; sincos2pi(u2, sn, cs);
+    return mk(mul(r, cs), mul(r, sn), sqr(sub(1.0f, u1)));
+}
+CRT_DEV float smith_g1(V3 w, float al)
+{
+    float tan2 = dvd(add(mul(w.x, w.x), mul(w.y, w.y)), mul(w.z, w.z));
+    return dvd(2.0f, add(1.0f, sqr(add(1.0f, mul(mul(al, al), tan2)))));
+}
+// GGX with visible-normal sampling (Heitz 2018); weight = F_schlick(F0 = albedo) * G1(wi)
+CRT_DEV bool sample_ggx(V3 wo, float al, const float* albedo, float u1, float u2, V3& wi, float* weight)
+{
+    V3 vh = mk(mul(al, wo.x), mul(al, wo.y), wo.z);
+    float vl = sqr(dot(vh, vh)); vh = mk(dvd(vh.x, vl), dvd(vh.y, vl), dvd(vh.z, vl));
+    float lensq = add(mul(vh.x, vh.x), mul(vh.y, vh.y));
+    V3 T1 = mk(1.0f, 0.0f, 0.0f);
+    if (lensq > 0.0f) { float il = sqr(lensq); T1 = mk(dvd(-vh.y, il), dvd(vh.x, il), 0.0f); }
+    V3 T2 = cross(vh, T1);
+    float r = sqr(u1), sn, cs; sincos2pi(u2, sn, cs);
+    float t1 = mul(r, cs), t2 = mul(r, sn);
+    float sh = mul(0.5f, add(1.0f, vh.z));
+    t2 = add(mul(sub(1.0f, sh), sqr(fmaxf(0.0f, sub(1.0f, mul(t1, t1))))), mul(sh, t2));
+    float t3 = sqr(fmaxf(0.0f, sub(sub(1.0f, mul(t1, t1)), mul(t2, t2))));
+    V3 nh = mk(add(add(mul(t1, T1.x), mul(t2, T2.x)), mul(t3, vh.x)), add(add(mul(t1, T1.y), mul(t2, T2.y)), mul(t3, vh.y)),
+               add(add(mul(t1, T1.z), mul(t2, T2.z)), mul(t3, vh.z)));
+    V3 h = mk(mul(al, nh.x), mul(al, nh.y), fmaxf(0.0f, nh.z));
+    float hl = sqr(dot(h, h)); h = mk(dvd(h.x, hl), dvd(h.y, hl), dvd(h.z, hl));
+    float woh = dot(wo, h);
+    float two = mul(2.0f, woh);
+    wi = mk(sub(mul(two, h.x), wo.x), sub(mul(two, h.y), wo.y), sub(mul(two, h.z), wo.z));
+    if (!(wi.z > 0.0f)) return false;
+    float g1 = smith_g1(wi, al);
+    float c1 = sub(1.0f, woh); if (c1 < 0.0f) c1 = 0.0f;
+    float c2 = mul(c1, c1), c5 = mul(mul(c2, c2), c1);
+#pragma unroll
+    for (int k = 0; k < 3; ++k) weight[k] = mul(add(albedo[k], mul(sub(1.0f, albedo[k]), c5)), g1);
+    return true;
+}
+
+// 30-bit interleaved origin+direction code (P:L43 [AK10]; D:R12)
+CRT_DEV uint32_t quant5(float x)
+{
+    float fl = floorf(x);
+    int q = (fl < 0.0f) ? 0 : ((fl > 31.0f) ? 31 : (int)fl);
+    if (x != x) q = 0;
+    return (uint32_t)q;
+}
+CRT_DEV uint32_t spread5(uint32_t v)   // bit l of v -> bit 6*l
+{
+    return (v & 1u) | ((v & 2u) << 5) | ((v & 4u) << 10) | ((v & 8u) << 15) | ((v & 16u) << 20);
+}
+struct Bounds6 { float lo[3], scale[3]; };
+CRT_DEV uint32_t morton_code(const Bounds6& B, float ox, float oy, float oz, float dx, float dy, float dz)
+{
+    uint32_t qx = quant5(mul(sub(ox, B.lo[0]), B.scale[0])), qy = quant5(mul(sub(oy, B.lo[1]), B.scale[1])), qz = quant5(mul(sub(oz, B.lo[2]), B.scale[2]));
+    uint32_t px = quant5(mul(add(dx, 1.0f), 16.0f)), py = quant5(mul(add(dy, 1.0f), 16.0f)), pz = quant5(mul(add(dz, 1.0f), 16.0f));
+    return (spread5(qx) << 5) | (spread5(qy) << 4) | (spread5(qz) << 3) | (spread5(px) << 2) | (spread5(py) << 1) | spread5(pz);
+}
+
+struct GenArgs {
+    const GpuTri* tris; const int32_t* slot_of_prim; const int32_t* mat_id; const crt_material* mats;
+    const crt_ray* prev_rays; const crt_hit* prev_hits; const int32_t* prev_r2p; crt_path_state* paths;
+    crt_ray* rays_out; int32_t* r2p_out; int32_t* gid_out; int32_t* src_out; uint8_t* cls_out; uint32_t* n_active;
+    uint32_t* keys_out;      // morton mode: key per path (rays_out etc. are then the by-path temporaries)
+    Bounds6 bounds;
+    int64_t n_slots; int32_t bounce; int32_t morton;
+};
+
+enum { F_DEAD = 0, F_DIFF = 1, F_GLOSS = 2 };
+
+// REUSE = true: groups of K consecutive slots share directions.  false: every path on its own (K = 1).
+template <bool REUSE>
+__global__ void __launch_bounds__(1024) generate_kernel(GenArgs A, DevLayout L)
+{
+    extern __shared__ float smem[];
+    // shared: per thread  flag (int), path (int), wi.xyz (float3) -- only used when REUSE
+    int* s_flag = reinterpret_cast<int*>(smem);
+    int* s_path = s_flag + blockDim.x;
+    float* s_wi = reinterpret_cast<float*>(s_path + blockDim.x);
+
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;   // previous-segment slot
+    const bool in_range = i < A.n_slots;
+    int32_t pixel = -1, sample = 0, p = -1;
+    if (in_range) {
+        if (REUSE) p = slot_to_path(L, i, pixel, sample);
+        else { p = A.prev_r2p[i]; pixel = p % (L.w * L.h); sample = p / (L.w * L.h); }
+    }
+    // ---- 1. shading point of a live path (D:R7)
+    bool live = false;
+    int mtype = 0; float albedo[3] = {0.f, 0.f, 0.f}, rough = 1.f;
+    Frame3 fr; V3 hp = mk(0.f, 0.f, 0.f), wo = mk(0.f, 0.f, 1.f);
+    fr.tx = fr.ty = fr.ng = mk(0.f, 0.f, 0.f);
+    crt_path_state ps; ps.flags = 0u;
+    if (p >= 0) {
+        const float4* pp = reinterpret_cast<const float4*>(A.paths + p);
+        const float4 p0 = pp[0];
+        ps.tr = p0.x; ps.tg = p0.y; ps.tb = p0.z; ps.flags = __float_as_uint(p0.w);
+        const float4 rd = __ldg(reinterpret_cast<const float4*>(A.prev_rays + i) + 1);
+        const float4 hv = __ldg(reinterpret_cast<const float4*>(A.prev_hits + i));
+        const int prim = __float_as_int(hv.w);
+        if ((ps.flags & 1u) && rd.w >= 0.f && prim >= 0) {
+            const float4* tp = reinterpret_cast<const float4*>(A.tris + __ldg(A.slot_of_prim + prim));
+            const float4 a = __ldg(tp), b = __ldg(tp + 1), c = __ldg(tp + 2);
+            const V3 v0 = mk(a.x, a.y, a.z), e1 = mk(b.x, b.y, b.z), e2 = mk(c.x, c.y, c.z), d = mk(rd.x, rd.y, rd.z);
+            V3 n = cross(e1, e2);
+            const float len = sqr(dot(n, n));
+            V3 ng = mk(dvd(n.x, len), dvd(n.y, len), dvd(n.z, len));
+            const float cosi = dot(ng, d);
+            if (cosi > 0.0f) { ng = mk(-ng.x, -ng.y, -ng.z); live = true; }
+            else if (cosi < 0.0f) live = true;
+            if (live) {
+                const float sign = ng.z >= 0.0f ? 1.0f : -1.0f;
+                const float aa = dvd(-1.0f, add(sign, ng.z));
+                const float bb = mul(mul(ng.x, ng.y), aa);
+                fr.tx = mk(add(1.0f, mul(mul(mul(sign, ng.x), ng.x), aa)), mul(sign, bb), mul(-sign, ng.x));
+                fr.ty = mk(bb, add(sign, mul(mul(ng.y, ng.y), aa)), -ng.y);
+                fr.ng = ng;
+                hp = mk(add(add(v0.x, mul(hv.y, e1.x)), mul(hv.z, e2.x)), add(add(v0.y, mul(hv.y, e1.y)), mul(hv.z, e2.y)),
+                        add(add(v0.z, mul(hv.y, e1.z)), mul(hv.z, e2.z)));
+                wo = to_local(fr, mk(-d.x, -d.y, -d.z));
+                const float4* mp = reinterpret_cast<const float4*>(A.mats + __ldg(A.mat_id + prim));
+                const float4 m0 = __ldg(mp), m1 = __ldg(mp + 1);
+                albedo[0] = m0.x; albedo[1] = m0.y; albedo[2] = m0.z; rough = m0.w; mtype = __float_as_int(m1.w);
+            }
+        }
+    }
+    const int flag = !live ? F_DEAD : (mtype == CRT_MAT_DIFFUSE ? F_DIFF : F_GLOSS);
+
+    // ---- 2. glossy / specular members sample from their own stream, untouched
+    bool has_dir = false; V3 wi = mk(0.f, 0.f, 0.f); float weight[3] = {0.f, 0.f, 0.f}; int32_t src = -1;
+    if (flag == F_GLOSS) {
+        const uint4 r = philox((uint32_t)pixel, (uint32_t)sample, (uint32_t)A.bounce, PURPOSE_BSDF, L.seed, L.frame);
+        if (mtype == CRT_MAT_SPECULAR) {
+            wi = mk(-wo.x, -wo.y, wo.z); has_dir = true;
+            weight[0] = albedo[0]; weight[1] = albedo[1]; weight[2] = albedo[2];
+        } else {
+            has_dir = sample_ggx(wo, rough, albedo, u01(r.x), u01(r.y), wi, weight);
+        }
+        src = p;
+    }
+
+    int cls = CRT_CLASS_EMPTY;
+    int64_t group = i;
+    if (REUSE) {
+        // ---- 3. census of the group through shared memory
+        const int K = L.K, tid = threadIdx.x, gbase = tid & ~(K - 1);
+        group = i >> L.log2K;
+        s_flag[tid] = flag | ((flag == F_GLOSS && has_dir) ? 4 : 0);
+        s_path[tid] = p;
+        s_wi[3 * tid] = wi.x; s_wi[3 * tid + 1] = wi.y; s_wi[3 * tid + 2] = wi.z;
+        __syncthreads();
+        bool any_diff = false, any_gloss = false, any_valid = false;
+        for (int j = 0; j < K; ++j) { const int f = s_flag[gbase + j]; any_diff |= (f & 3) == F_DIFF; any_gloss |= (f & 3) == F_GLOSS; any_valid |= (f & 4) != 0; }
+        cls = (!any_diff && !any_gloss) ? CRT_CLASS_EMPTY : (!any_gloss ? CRT_CLASS_DIFFUSE : (!any_diff ? CRT_CLASS_GLOSSY : CRT_CLASS_HYBRID));
+        if (flag == F_DIFF) {
+            if (cls == CRT_CLASS_HYBRID && any_valid) {
+                // hybrid: mean tangent-space exit direction of the glossy/specular members, summed in slot order
+                V3 sum = mk(0.f, 0.f, 0.f);
+                for (int j = 0; j < K; ++j)
+                    if (s_flag[gbase + j] & 4) sum = mk(add(sum.x, s_wi[3 * (gbase + j)]), add(sum.y, s_wi[3 * (gbase + j) + 1]), add(sum.z, s_wi[3 * (gbase + j) + 2]));
+                const float len = sqr(dot(sum, sum));
+                wi = mk(dvd(sum.x, len), dvd(sum.y, len), dvd(sum.z, len));
+                src = (int32_t)(-2 - group);
+            } else {
+                // diffuse group: one randomly selected member samples, the others reuse its tangent-space direction
+                const uint4 rl = philox((uint32_t)group, (uint32_t)sample, (uint32_t)A.bounce, PURPOSE_LEADER, L.seed, L.frame);
+                const int j0 = (int)(rl.x & (uint32_t)(K - 1));
+                int leader = -1;
+                for (int t = 0; t < K; ++t) { const int j = (j0 + t) & (K - 1); if ((s_flag[gbase + j] & 3) == F_DIFF) { leader = s_path[gbase + j]; break; } }
+                const uint4 r = philox((uint32_t)(leader % (L.w * L.h)), (uint32_t)sample, (uint32_t)A.bounce, PURPOSE_BSDF, L.seed, L.frame);
+                wi = sample_cosine(u01(r.x), u01(r.y));
+                src = leader;
+            }
+            has_dir = true; weight[0] = albedo[0]; weight[1] = albedo[1]; weight[2] = albedo[2];
+        }
+        if (in_range && (tid & (K - 1)) == 0) A.cls_out[group] = (uint8_t)cls;
+    } else {
+        if (flag == F_DIFF) {
+            const uint4 r = philox((uint32_t)pixel, (uint32_t)sample, (uint32_t)A.bounce, PURPOSE_BSDF, L.seed, L.frame);
+            wi = sample_cosine(u01(r.x), u01(r.y));
+            has_dir = true; src = p; weight[0] = albedo[0]; weight[1] = albedo[1]; weight[2] = albedo[2];
+        }
+        cls = flag == F_DEAD ? CRT_CLASS_EMPTY : (flag == F_DIFF ? CRT_CLASS_DIFFUSE : CRT_CLASS_GLOSSY);
+        group = p;
+        if (in_range) A.cls_out[p] = (uint8_t)cls;
+    }
+
+    // ---- 4. emit
+    if (!in_range) return;
+    const int64_t o = REUSE ? i : (int64_t)p;            // output index: the slot, or the path id (row-major order)
+    float4 r0 = make_float4(0.f, 0.f, 0.f, 0.f), r1 = make_float4(0.f, 0.f, 0.f, -1.f);
+    const bool emit = live && has_dir;
+    if (emit) {
+        const V3 wd = to_world(fr, wi);
+        const float mx = fmaxf(fabsf(hp.x), fmaxf(fabsf(hp.y), fabsf(hp.z)));
+        const float off = mul(1.0f / 32768.0f, add(1.0f, mx));
+        r0 = make_float4(add(hp.x, mul(fr.ng.x, off)), add(hp.y, mul(fr.ng.y, off)), add(hp.z, mul(fr.ng.z, off)), 0.f);
+        r1 = make_float4(wd.x, wd.y, wd.z, 1e30f);
+    }
+    if (p >= 0 && (ps.flags & 1u)) {
+        // throughput *= weight; a live path that produced no ray ends here
+        float4 np = make_float4(ps.tr, ps.tg, ps.tb, 0.f);
+        uint32_t fl = ps.flags;
+        if (emit) { np.x = mul(ps.tr, weight[0]); np.y = mul(ps.tg, weight[1]); np.z = mul(ps.tb, weight[2]); }
+        else fl &= ~1u;
+        np.w = __uint_as_float(fl);
+        reinterpret_cast<float4*>(A.paths + p)[0] = np;
+    }
+    if (o >= 0) {
+        float4* rp = reinterpret_cast<float4*>(A.rays_out + o);
+        rp[0] = r0; rp[1] = r1;
+        A.r2p_out[o] = p;
+        A.src_out[o] = emit ? src : -1;
+        if (A.morton) A.keys_out[o] = emit ? morton_code(A.bounds, r0.x, r0.y, r0.z, r1.x, r1.y, r1.z) : 0xFFFFFFFFu;
+        else A.gid_out[o] = REUSE ? (int32_t)group : p;
+    }
+    const unsigned m = __ballot_sync(__activemask(), emit);
+    if (emit && (threadIdx.x & 31) == (__ffs(m) - 1)) atomicAdd(A.n_active, (unsigned)__popc(m));
+}
+
+__global__ void morton_encode_kernel(Bounds6 B, const crt_ray* __restrict__ rays, int64_t n, uint32_t* __restrict__ keys)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const float4 a = __ldg(reinterpret_cast<const float4*>(rays + i)), b = __ldg(reinterpret_cast<const float4*>(rays + i) + 1);
+    keys[i] = b.w < 0.f ? 0xFFFFFFFFu : morton_code(B, a.x, a.y, a.z, b.x, b.y, b.z);
+}
+
+// rays_out[j] = tmp[perm[j]] etc.
+__global__ void permute_kernel(const int32_t* __restrict__ perm, const crt_ray* __restrict__ tmp_rays, const int32_t* __restrict__ tmp_src,
+                               int64_t n, crt_ray* __restrict__ rays_out, int32_t* __restrict__ r2p_out, int32_t* __restrict__ gid_out,
+                               int32_t* __restrict__ src_out)
+{
+    const int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= n) return;
+    const int32_t p = perm[j];
+    const float4* s = reinterpret_cast<const float4*>(tmp_rays + p);
+    float4* d = reinterpret_cast<float4*>(rays_out + j);
+    d[0] = __ldg(s); d[1] = __ldg(s + 1);
+    r2p_out[j] = p; gid_out[j] = p; src_out[j] = __ldg(tmp_src + p);
+}
+
+Bounds6 make_bounds(const float* b)
+{
+    Bounds6 B;
+    for (int k = 0; k < 3; ++k) { B.lo[k] = b[k]; float ext = b[3 + k] - b[k]; B.scale[k] = ext > 0.f ? 32.0f / ext : 0.f; }
+    return B;
+}
+
+inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+}  // namespace
+
+size_t generate_scratch_bytes(const Layout& L)
+{
+    if (L.mode != CRT_MODE_MORTON_REORDER) return 256;
+    const size_t n = (size_t)L.n_slots;
+    return align256(n * sizeof(crt_ray)) + 5 * align256(n * 4) + align256(radix_sort_scratch_bytes(L.n_slots)) + 256;
+}
+
+crt_status launch_morton_encode(crt_ctx* ctx, const float* bounds, const crt_ray* rays, int64_t n, uint32_t* keys, cudaStream_t st)
+{
+    if (n == 0) return CRT_OK;
+    morton_encode_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(make_bounds(bounds), rays, n, keys);
+    CRT_CHECK_LAUNCH(ctx, "morton_encode");
+    return CRT_OK;
+}
+
+crt_status launch_generate(crt_ctx* ctx, const crt_bvh* bvh, const crt_scene_mats& mats, const crt_frame& f, int bounce, const Layout& L,
+                           const crt_ray* prev_rays, const crt_hit* prev_hits, const int32_t* prev_r2p, crt_path_state* paths,
+                           crt_ray* rays_out, int32_t* r2p_out, int32_t* gid_out, int32_t* src_out, uint8_t* cls_out,
+                           uint32_t* n_active, void* scratch, size_t scratch_bytes, cudaStream_t st, cudaEvent_t* ev4)
+{
+    CRT_CUDA(ctx, cudaMemsetAsync(n_active, 0, sizeof(uint32_t), st));
+    if (L.n_slots == 0) return CRT_OK;
+    if (scratch_bytes < generate_scratch_bytes(L)) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "generate_secondary: scratch too small");
+    GenArgs A;
+    A.tris = bvh->d_tris; A.slot_of_prim = bvh->d_slot_of_prim; A.mat_id = bvh->d_mat_id; A.mats = mats.materials;
+    A.prev_rays = prev_rays; A.prev_hits = prev_hits; A.prev_r2p = prev_r2p; A.paths = paths;
+    A.rays_out = rays_out; A.r2p_out = r2p_out; A.gid_out = gid_out; A.src_out = src_out; A.cls_out = cls_out; A.n_active = n_active;
+    A.keys_out = nullptr; A.bounds = make_bounds(bvh->bounds); A.n_slots = L.n_slots; A.bounce = bounce; A.morton = 0;
+    const DevLayout D = make_dev_layout(L, f);
+    const int64_t n = L.n_slots;
+    if (L.mode == CRT_MODE_DIRECT_REUSE) {
+        const int block = L.K > 256 ? L.K : 256;
+        generate_kernel<true><<<(unsigned)((n + block - 1) / block), block, (size_t)block * 20, st>>>(A, D);
+        CRT_CHECK_LAUNCH(ctx, "generate<reuse>");
+        return CRT_OK;
+    }
+    if (L.mode == CRT_MODE_INDEPENDENT) {
+        generate_kernel<false><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(A, D);
+        CRT_CHECK_LAUNCH(ctx, "generate<independent>");
+        return CRT_OK;
+    }
+    // morton_reorder: independent rays by path id into scratch, with their codes; stable sort of (code, path); permute
+    char* s = static_cast<char*>(scratch);
+    crt_ray* tmp_rays = reinterpret_cast<crt_ray*>(s); s += align256((size_t)n * sizeof(crt_ray));
+    int32_t* tmp_src = reinterpret_cast<int32_t*>(s); s += align256((size_t)n * 4);
+    uint32_t* keys = reinterpret_cast<uint32_t*>(s); s += align256((size_t)n * 4);
+    int32_t* idx = reinterpret_cast<int32_t*>(s); s += align256((size_t)n * 4);
+    uint32_t* keys2 = reinterpret_cast<uint32_t*>(s); s += align256((size_t)n * 4);
+    int32_t* perm = reinterpret_cast<int32_t*>(s); s += align256((size_t)n * 4);
+    A.rays_out = tmp_rays; A.src_out = tmp_src; A.keys_out = keys; A.morton = 1;
+    A.r2p_out = idx;        // idx[p] = p
+    generate_kernel<false><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(A, D);
+    CRT_CHECK_LAUNCH(ctx, "generate<morton>");
+    if (ev4) CRT_CUDA(ctx, cudaEventRecord(ev4[0], st));
+    crt_status stt = launch_radix_sort(ctx, keys, idx, n, keys2, perm, s, radix_sort_scratch_bytes(n), st);
+    if (stt != CRT_OK) return stt;
+    permute_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(perm, tmp_rays, tmp_src, n, rays_out, r2p_out, gid_out, src_out);
+    CRT_CHECK_LAUNCH(ctx, "permute");
+    if (ev4) CRT_CUDA(ctx, cudaEventRecord(ev4[1], st));
+    return CRT_OK;
+}

@@ -149,6 +149,10 @@ size_t crt_radix_sort_scratch_bytes(int64_t n);
 /* hits[i] = nearest intersection of rays[i] with tmin < t < tmax; ties -> lowest primitive id (D:R10).
  * Inactive rays (tmax < 0) give a miss.  rays, hits: [device], n_rays entries. */
 crt_status crt_trace(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n_rays, crt_hit* hits, void* stream);
+/* Work counters of the same traversal (a counting build of the kernel; used by bench.py for the roofline's
+ * algorithmic FLOPs and by tests).  counters: [device] int64[4], ADDED to: [0] node visits (one visit = one 64-byte
+ * node fetched and its two child boxes tested), [1] triangle tests, [2] active rays, [3] unused. */
+crt_status crt_trace_stats(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n_rays, int64_t* counters, void* stream);
 
 /* ---- a6: shading and accumulation (D:R14) --------------------------------------------- */
 /* For the segment just traced: miss -> radiance += throughput*env(d), path ends; emissive hit -> radiance +=

@@ -267,7 +267,9 @@ void crt_bvh_flatten(const crt_bvh* b, std::vector<GpuNode>& gn, std::vector<Gpu
     }
     auto leaf_ref = [](const BuildNode& nd) { return ~((nd.first << 3) | (nd.count - 1)); };
     auto empty_node = [&] {
-        GpuNode g; g.xy0 = g.xy1 = make_float4(inf, -inf, inf, -inf); g.z01 = make_float4(inf, -inf, inf, -inf);
+        // a box at +infinity on every axis: the slab test fails for every ray (an inverted box would NOT fail, because
+        // the test takes min/max of the two plane distances)
+        GpuNode g; g.xy0 = g.xy1 = make_float4(inf, inf, inf, inf); g.z01 = make_float4(inf, inf, inf, inf);
         g.ref0 = g.ref1 = ~0; g.pad0 = g.pad1 = 0; return g;
     };
     gn.clear();

@@ -270,6 +270,16 @@ crt_status crt_trace(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int6
     return launch_trace(ctx, bvh, rays, n_rays, hits, (cudaStream_t)stream);
 }
 
+crt_status crt_trace_stats(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n_rays, int64_t* counters, void* stream)
+{
+    NEED_CTX("trace_stats"); NEED_BVH("trace_stats");
+    if (n_rays < 0 || n_rays >= ((int64_t)1 << 31)) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "trace_stats: bad ray count");
+    NEED_ALIGNED("trace_stats", counters, 8);
+    if (n_rays == 0) return CRT_OK;
+    NEED_ALIGNED("trace_stats", rays, 32);
+    return launch_trace_stats(ctx, bvh, rays, n_rays, counters, (cudaStream_t)stream);
+}
+
 crt_status crt_shade_accumulate(crt_ctx* ctx, const crt_bvh* bvh, const crt_scene_mats* mats, const crt_frame* frame, int32_t bounce, int32_t is_last,
                                 const crt_ray* rays, const crt_hit* hits, const int32_t* ray_to_path, int64_t n_rays, crt_path_state* paths, float* accum, void* stream)
 {

@@ -83,6 +83,7 @@ crt_status crt_make_layout(crt_ctx* ctx, const crt_frame* f, const crt_order* o,
 
 // kernels' host launchers (defined in the .cu files) ------------------------------------------------------
 crt_status launch_trace(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, crt_hit* hits, cudaStream_t st);
+crt_status launch_trace_stats(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, int64_t* counters, cudaStream_t st);
 crt_status launch_primary(crt_ctx* ctx, const crt_bvh* bvh, const crt_camera& cam, const crt_frame& f, const Layout& L,
                           crt_ray* rays, crt_hit* hits, int32_t* r2p, cudaStream_t st);
 crt_status launch_generate(crt_ctx* ctx, const crt_bvh* bvh, const crt_scene_mats& mats, const crt_frame& f, int bounce, const Layout& L,

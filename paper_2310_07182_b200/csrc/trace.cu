@@ -40,8 +40,10 @@ CRT_DEV NodeRegs load_node(const GpuNode* __restrict__ nodes, int idx)
 
 struct Hit { float t, u, v; int prim; };
 
-// nearest hit of one ray; `stack` is this thread's private stack
-CRT_DEV Hit traverse(const GpuNode* __restrict__ nodes, const GpuTri* __restrict__ tris, V3 o, V3 d, float tmin, float tmax)
+// nearest hit of one ray; `stack` is this thread's private stack.  COUNT: also count node visits / triangle tests.
+template <bool COUNT = false>
+CRT_DEV Hit traverse(const GpuNode* __restrict__ nodes, const GpuTri* __restrict__ tris, V3 o, V3 d, float tmin, float tmax,
+                     unsigned* n_nodes = nullptr, unsigned* n_tris = nullptr)
 {
     Hit best; best.t = tmax; best.u = 0.f; best.v = 0.f; best.prim = -1;
     const float idx = dvd(1.0f, d.x), idy = dvd(1.0f, d.y), idz = dvd(1.0f, d.z);
@@ -54,6 +56,7 @@ CRT_DEV Hit traverse(const GpuNode* __restrict__ nodes, const GpuTri* __restrict
         // ---- inner nodes
         while (node >= 0 && node != SENTINEL) {
             const NodeRegs n = load_node(nodes, node);
+            if (COUNT) ++*n_nodes;
             // slab test, (b - o) * (1/d): error stays relative to the result (no cancellation against o/d)
             float ax0 = (n.xy0.x - o.x) * idx, ax1 = (n.xy0.y - o.x) * idx;
             float ay0 = (n.xy0.z - o.y) * idy, ay1 = (n.xy0.w - o.y) * idy;
@@ -85,6 +88,7 @@ CRT_DEV Hit traverse(const GpuNode* __restrict__ nodes, const GpuTri* __restrict
                 const float4* tp = reinterpret_cast<const float4*>(tris + first + j);
                 const float4 a = __ldg(tp), b = __ldg(tp + 1), c = __ldg(tp + 2);
                 float t, u, v;
+                if (COUNT) ++*n_tris;
                 if (tri_test(mk(a.x, a.y, a.z), mk(b.x, b.y, b.z), mk(c.x, c.y, c.z), o, d, tmin, tmax, t, u, v)) {
                     const int prim = __float_as_int(a.w);
                     if (best.prim < 0 || t < best.t || (t == best.t && prim < best.prim)) {
@@ -136,6 +140,24 @@ __global__ void __launch_bounds__(128) trace_persistent_kernel(const GpuNode* __
         if (i < n) trace_one(nodes, tris, rays, hits, i);
         __syncwarp();
     }
+}
+
+// counting build of the traversal (crt_trace_stats): same code path, results discarded
+__global__ void __launch_bounds__(128) trace_stats_kernel(const GpuNode* __restrict__ nodes, const GpuTri* __restrict__ tris,
+                                                          const crt_ray* __restrict__ rays, int64_t n, unsigned long long* __restrict__ counters)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    unsigned nn = 0, nt = 0, act = 0;
+    if (i < n) {
+        const float4* rp = reinterpret_cast<const float4*>(rays + i);
+        const float4 ro = __ldg(rp), rd = __ldg(rp + 1);
+        if (rd.w >= 0.f) { act = 1; traverse<true>(nodes, tris, mk(ro.x, ro.y, ro.z), mk(rd.x, rd.y, rd.z), ro.w, rd.w, &nn, &nt); }
+    }
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) {
+        nn += __shfl_xor_sync(0xffffffffu, nn, d); nt += __shfl_xor_sync(0xffffffffu, nt, d); act += __shfl_xor_sync(0xffffffffu, act, d);
+    }
+    if ((threadIdx.x & 31) == 0) { atomicAdd(counters, (unsigned long long)nn); atomicAdd(counters + 1, (unsigned long long)nt); atomicAdd(counters + 2, (unsigned long long)act); }
 }
 
 }  // namespace
@@ -205,6 +227,14 @@ crt_status launch_trace(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, i
         trace_persistent_kernel<<<(unsigned)grid, 128, 0, st>>>(bvh->d_nodes, bvh->d_tris, rays, hits, n, ctx->d_counter);
     }
     CRT_CHECK_LAUNCH(ctx, "trace");
+    return CRT_OK;
+}
+
+crt_status launch_trace_stats(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, int64_t* counters, cudaStream_t st)
+{
+    if (n == 0) return CRT_OK;
+    trace_stats_kernel<<<(unsigned)((n + 127) / 128), 128, 0, st>>>(bvh->d_nodes, bvh->d_tris, rays, n, reinterpret_cast<unsigned long long*>(counters));
+    CRT_CHECK_LAUNCH(ctx, "trace_stats");
     return CRT_OK;
 }
 

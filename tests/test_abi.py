@@ -1,0 +1,126 @@
+"""CPU-only checks of the C-ABI boundary: libcrt.so builds for sm_100a, loads, exports every symbol include/crt.h
+declares, fails loudly without a CUDA device (no CPU fallback), and its host-side logic (layout arithmetic, BVH
+builder invariants) is right.  No compute call is made here."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+import crt_inputs as I
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_2310_07182_b200 import build
+    return C.CDLL(build.build())
+
+
+def _declared_symbols():
+    src = open(os.path.join(ROOT, "include", "crt.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(crt_[a-z0-9_]+)\s*\(", src)))
+
+
+def test_library_exports_every_declared_symbol(lib):
+    names = _declared_symbols()
+    assert len(names) >= 24
+    for n in names:
+        assert hasattr(lib, n), f"libcrt.so does not export {n}"
+    from paper_2310_07182_b200 import api
+    assert sorted(api.EXPORTS) == names
+
+
+def test_no_cpu_fallback(lib):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a CUDA device is present")
+    h = C.c_void_p()
+    st = lib.crt_create(C.c_int32(0), C.byref(h))
+    assert st == 3 and not h.value                     # CRT_ERR_CUDA
+    lib.crt_last_error.restype = C.c_char_p
+    assert b"no CPU fallback" in lib.crt_last_error(None)
+    import paper_2310_07182_b200 as crt
+    with pytest.raises(crt.CrtError):
+        crt.Context(0)
+
+
+def test_product_does_not_import_the_oracle():
+    pkg = os.path.join(ROOT, "paper_2310_07182_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h", ".cpp")):
+                txt = open(os.path.join(dirpath, f)).read()
+                assert "oracle" not in txt.lower().replace("no cpu fallback", ""), f"{f} mentions the oracle"
+
+
+@pytest.mark.parametrize("w,h,spp,mode,gw,gh,s", [(64, 64, 1, 2, 4, 4, 2), (1920, 1080, 1, 2, 4, 4, 4), (3840, 2160, 4, 2, 8, 8, 8),
+                                                  (50, 37, 2, 2, 2, 4, 4), (1920, 1080, 1, 0, 1, 1, 1), (7, 5, 3, 1, 1, 1, 1), (0, 0, 1, 2, 2, 2, 2)])
+def test_layout_matches_the_paper_parametrisation(lib, oracle, w, h, spp, mode, gw, gh, s):
+    """tiles of W x H pixels, WH/K groups of K; K = gw*gh, W = gw*s, H = gh*s (reading R3)."""
+    import paper_2310_07182_b200 as crt
+    n_paths, n_slots, n_groups = crt.crt_layout(crt.make_frame(w, h, spp), crt.make_order(mode, gw, gh, s))
+    assert n_paths == spp * w * h
+    if mode == 2:
+        W, H = gw * s, gh * s
+        tiles = -(-w // W) * -(-h // H)
+        assert n_slots == spp * tiles * W * H and n_groups * gw * gh == n_slots
+    else:
+        assert n_slots == n_paths == n_groups
+    ofr = oracle.frame(w, h, spp)
+    assert n_slots == oracle.n_slots(ofr, mode, gw, gh, s) and n_groups == oracle.n_groups(ofr, mode, gw, gh, s)
+
+
+def test_host_bvh_builder_invariants(lib):
+    """ctx == NULL builds the host tree only: every triangle in exactly one leaf, leaves <= max_leaf, boxes nested."""
+    from paper_2310_07182_b200 import api
+    for scene, max_leaf in ((I.cornell(), 4), (I.interior(n_boxes=80, n_spheres=10, subdiv=2), 2), (I.landscape(n=96, n_trees=40), 8)):
+        v = np.ascontiguousarray(scene.verts, np.float32); m = np.ascontiguousarray(scene.mat_id, np.int32)
+        pr = api.BvhParams(max_leaf, 16, 1.0, 1.0, 2)
+        h = C.c_void_p()
+        assert lib.crt_build_bvh(None, C.c_void_p(v.ctypes.data), C.c_void_p(m.ctypes.data), C.c_int64(len(v)), C.byref(pr), C.byref(h)) == 0
+        bad = C.c_int32(-1)
+        assert lib.crt_bvh_check(h, C.byref(bad)) == 0 and bad.value == 0
+        info = api.BvhInfo()
+        assert lib.crt_bvh_get_info(h, C.byref(info)) == 0
+        assert info.n_tris == len(v) and info.max_leaf == max_leaf and 0 < info.depth <= 60
+        assert len(v) / max_leaf <= (info.n_nodes + 1) / 2 <= len(v)
+        assert np.array_equal(np.array(list(info.bounds), np.float32), np.concatenate([v.reshape(-1, 3).min(0), v.reshape(-1, 3).max(0)]))
+        assert info.device_bytes == 0
+        lib.crt_bvh_destroy(h)
+    # degenerate inputs: no triangles, one triangle, many identical triangles (centroids coincide)
+    for v in (np.zeros((0, 3, 3), np.float32), I.cornell().verts[:1], np.repeat(I.cornell().verts[:1], 37, axis=0)):
+        v = np.ascontiguousarray(v)
+        h = C.c_void_p()
+        assert lib.crt_build_bvh(None, C.c_void_p(v.ctypes.data), None, C.c_int64(len(v)), None, C.byref(h)) == 0
+        bad = C.c_int32(-1)
+        assert lib.crt_bvh_check(h, C.byref(bad)) == 0 and bad.value == 0
+        lib.crt_bvh_destroy(h)
+    # rejected: NaN vertex, bad max_leaf
+    v = I.cornell().verts.copy(); v[3, 1, 2] = np.nan
+    h = C.c_void_p()
+    assert lib.crt_build_bvh(None, C.c_void_p(v.ctypes.data), None, C.c_int64(len(v)), None, C.byref(h)) == 1
+    pr = api.BvhParams(9, 16, 1.0, 1.0, 1)
+    v = I.cornell().verts
+    assert lib.crt_build_bvh(None, C.c_void_p(v.ctypes.data), None, C.c_int64(len(v)), C.byref(pr), C.byref(h)) == 1
+
+
+def test_scratch_size_queries(lib):
+    import paper_2310_07182_b200 as crt
+    lib.crt_radix_sort_scratch_bytes.restype = C.c_size_t
+    lib.crt_frame_workspace_bytes.restype = C.c_size_t
+    lib.crt_generate_secondary_scratch_bytes.restype = C.c_size_t
+    assert lib.crt_radix_sort_scratch_bytes(C.c_int64(0)) >= 0
+    n = 2073600
+    assert lib.crt_radix_sort_scratch_bytes(C.c_int64(n)) >= 8 * n
+    fr = crt.make_frame(1920, 1080)
+    for mode, lo in (("independent", 0), ("morton_reorder", 32 + 5 * 4 + 8), ("direct_reuse", 0)):
+        order = crt.make_order(mode, 4, 4, 4)
+        assert lib.crt_generate_secondary_scratch_bytes(C.byref(fr), C.byref(order)) >= lo * n
+        # rays x2, hits, 4 int maps, path state
+        assert lib.crt_frame_workspace_bytes(C.byref(fr), C.byref(order)) >= (32 * 2 + 16 + 16 + 32) * n
+    bad = crt.make_order("direct_reuse", 3, 3, 3)
+    assert lib.crt_frame_workspace_bytes(C.byref(fr), C.byref(bad)) == 0

@@ -1,0 +1,322 @@
+"""GPU parity tests: libcrt (through its C ABI, via the ctypes binding) against the CPU oracle, element by element
+on the same seeded inputs.  Bars are north_star's: integer outputs bit-exact; hit ids identical >= 99.99 % with the rest
+only at t-ties within 1e-5 relative; t/u/v within 1e-4 relative; images within 1e-3 RMSE.  Ray tolerance: reading A-26.
+"""
+import numpy as np
+import pytest
+
+import crt_inputs as I
+from pipeline import GpuScene, compare_hits, compare_rays, hits_np, oracle_frame, paths_np, rays_np, rmse
+
+pytestmark = pytest.mark.gpu
+
+MODES = {"independent": 0, "morton_reorder": 1, "direct_reuse": 2}
+
+
+@pytest.fixture(scope="module")
+def crt():
+    import torch
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device"
+    import paper_2310_07182_b200 as crt
+    return crt
+
+
+@pytest.fixture(scope="module")
+def ctx(crt):
+    return crt.Context(0)
+
+
+def _small_interior():
+    return I.interior(seed=1, width=96, height=64, n_boxes=60, n_spheres=12, subdiv=2)
+
+
+SCENES = {
+    "cornell": lambda: I.cornell(),
+    "interior_small": _small_interior,
+    "checker": lambda: I.checker_floor(seed=3, width=48, height=40),
+}
+
+
+# ------------------------------------------------------------------ a0 / a5: BVH + traversal
+@pytest.mark.parametrize("scene_name", ["cornell", "interior_small"])
+@pytest.mark.parametrize("kernel", [0, 1])
+def test_trace_matches_oracle_on_random_rays(crt, ctx, oracle, scene_name, kernel):
+    scene = SCENES[scene_name]()
+    G = GpuScene(crt, scene, ctx)
+    assert G.bvh.check() == 0
+    info = G.bvh.info()
+    assert info["n_tris"] == scene.n_tris
+    ob = oracle.Bvh(scene.verts)
+    assert np.array_equal(info["bounds"], ob.info()["bounds"])
+    n = 20000 + 37                                    # several blocks and a ragged tail
+    r = I.random_rays(5, n, info["bounds"][:3], info["bounds"][3:], inactive_frac=0.05)
+    ctx.crt_set_option("trace_kernel", kernel)
+    try:
+        h = hits_np(oracle, ctx.crt_trace(G.bvh, ctx.upload(r)))
+    finally:
+        ctx.crt_set_option("trace_kernel", 1)
+    ho = ob.trace(r.view(oracle.RAY_DTYPE).reshape(-1))
+    compare_hits(h, ho)
+    # the triangle test is the same fp32 operation sequence on both sides: where ids agree the record is bit-identical
+    same = h["prim"] == ho["prim"]
+    assert (h[same].tobytes() == ho[same].tobytes())
+
+
+def test_trace_tiny_scene_against_brute_force(crt, ctx, oracle):
+    scene = I.furnace_sphere(1)                       # 80 triangles
+    G = GpuScene(crt, scene, ctx)
+    r = I.random_rays(8, 3001, [-1, -1, -1], [1, 1, 1])
+    h = hits_np(oracle, ctx.crt_trace(G.bvh, ctx.upload(r)))
+    hb = oracle.trace_brute(scene.verts, r.view(oracle.RAY_DTYPE).reshape(-1))
+    compare_hits(h, hb)
+
+
+def test_trace_edge_cases(crt, ctx, oracle):
+    import torch
+    scene = I.cornell()
+    G = GpuScene(crt, scene, ctx)
+    # empty batch
+    assert ctx.crt_trace(G.bvh, ctx.empty((0, 8))).shape[0] == 0
+    # all inactive
+    r = I.random_rays(1, 100, [0, 0, 0], [1, 1, 1], inactive_frac=1.0)
+    h = hits_np(oracle, ctx.crt_trace(G.bvh, ctx.upload(r)))
+    assert np.all(h["prim"] == -1) and np.all(h["t"] == -1.0)
+    # a single triangle and an empty scene
+    one = GpuScene(crt, I.Scene("one", scene.verts[:1], scene.mat_id[:1], scene.materials, scene.env, scene.camera), ctx)
+    rr = I.random_rays(2, 500, [0, 0, 0], [1, 1, 1])
+    compare_hits(hits_np(oracle, ctx.crt_trace(one.bvh, ctx.upload(rr))), oracle.trace_brute(scene.verts[:1], rr.view(oracle.RAY_DTYPE).reshape(-1)))
+    empty = ctx.crt_build_bvh(np.zeros((0, 3, 3), np.float32), np.zeros(0, np.int32))
+    he = hits_np(oracle, ctx.crt_trace(empty, ctx.upload(rr)))
+    assert np.all(he["prim"] == -1)
+    # tmin / tmax windows
+    rw = rr.copy(); rw[:, 3] = 0.3; rw[:, 7] = 0.9
+    compare_hits(hits_np(oracle, ctx.crt_trace(G.bvh, ctx.upload(rw))), oracle.Bvh(scene.verts).trace(rw.view(oracle.RAY_DTYPE).reshape(-1)))
+    # misaligned pointer is rejected
+    buf = ctx.empty((101 * 8 + 1,))
+    with pytest.raises(crt.CrtError) as e:
+        ctx.crt_trace(G.bvh, buf[1:].view(-1)[: 100 * 8].view(100, 8))
+    assert e.value.status == crt.api.CRT_ERR_INVALID_ARG
+    torch.cuda.synchronize()
+
+
+def test_trace_stats_counts(crt, ctx, oracle):
+    scene = _small_interior()
+    G = GpuScene(crt, scene, ctx)
+    r = I.random_rays(5, 5000, [0, 0, 0], [40, 8, 40], inactive_frac=0.1)
+    nn, nt, act = ctx.crt_trace_stats(G.bvh, ctx.upload(r))
+    assert act == int((r[:, 7] >= 0).sum())
+    assert nn > act and nt > 0
+    # same order of magnitude as the oracle's own tree (different builder parameters, so not equal)
+    cnt = np.zeros(2, np.int64)
+    oracle.Bvh(scene.verts).trace(r.view(oracle.RAY_DTYPE).reshape(-1), cnt)
+    assert 0.3 < nn / cnt[0] < 3.0 and 0.3 < nt / cnt[1] < 3.0
+
+
+# ------------------------------------------------------------------ a1: primary rays
+@pytest.mark.parametrize("mode,gw,gh,s", [("independent", 1, 1, 1), ("direct_reuse", 4, 4, 2), ("direct_reuse", 2, 4, 4)])
+@pytest.mark.parametrize("w,h,spp", [(64, 64, 1), (50, 37, 2)])
+def test_primary_matches_oracle(crt, ctx, oracle, mode, gw, gh, s, w, h, spp):
+    scene = I.cornell(width=w, height=h)
+    G = GpuScene(crt, scene, ctx)
+    fr = crt.make_frame(w, h, spp, seed=0, frame=3)
+    order = crt.make_order(mode, gw, gh, s)
+    rays, hits, r2p = ctx.crt_trace_primary(G.bvh, G.camera, fr, order)
+    ofr = oracle.frame(w, h, spp, 0, 3)
+    ro, ho, po = oracle.trace_primary(oracle.Bvh(scene.verts), scene.camera, ofr, MODES[mode], gw, gh, s)
+    assert crt.crt_layout(fr, order)[1] == len(po)
+    assert np.array_equal(r2p.cpu().numpy(), po)                       # partition: bit-exact
+    rg = rays_np(oracle, rays)
+    compare_rays(rg, ro)
+    act = ro["tmax"] >= 0
+    assert rg[act].tobytes() == ro[act].tobytes()                        # same fp32 operation sequence
+    hg = hits_np(oracle, hits)
+    compare_hits(hg[act], ho[act])
+
+
+# ------------------------------------------------------------------ a2-a4: generation, stage-wise (oracle buffers in)
+GEN_CASES = [
+    ("cornell", "independent", 1, 1, 1, 64, 64, 1),
+    ("cornell", "morton_reorder", 1, 1, 1, 64, 64, 1),
+    ("cornell", "direct_reuse", 4, 4, 2, 64, 64, 1),          # BASELINE config 1
+    ("interior_small", "independent", 1, 1, 1, 96, 64, 1),
+    ("interior_small", "morton_reorder", 1, 1, 1, 96, 64, 2),
+    ("interior_small", "direct_reuse", 4, 4, 4, 96, 64, 1),   # config 2's grouping, partial tiles (96x64 vs 16x16: exact) ...
+    ("interior_small", "direct_reuse", 2, 2, 8, 90, 61, 2),   # ... and ragged ones with 2 spp
+    ("interior_small", "direct_reuse", 8, 8, 1, 96, 64, 1),   # stride 1: one group per tile, K = 64 (two warps per group)
+    ("interior_small", "direct_reuse", 8, 8, 8, 96, 64, 1),   # largest tile: M = 4096
+    ("checker", "direct_reuse", 4, 4, 2, 48, 40, 1),          # hybrid groups
+    ("checker", "direct_reuse", 1, 1, 4, 48, 40, 1),          # K = 1
+]
+
+
+@pytest.mark.parametrize("scene_name,mode,gw,gh,s,w,h,spp", GEN_CASES)
+def test_generate_stagewise_matches_oracle(crt, ctx, oracle, scene_name, mode, gw, gh, s, w, h, spp):
+    scene = SCENES[scene_name]().with_camera(w, h)
+    G = GpuScene(crt, scene, ctx)
+    n_b = 2
+    ofr = oracle.frame(w, h, spp, 7, 2)
+    st = oracle_frame(oracle, scene, ofr, n_b, MODES[mode], gw, gh, s)
+    fr = crt.make_frame(w, h, spp, 7, 2)
+    order = crt.make_order(mode, gw, gh, s)
+    saw_hybrid = False
+    for b in range(1, n_b + 1):
+        paths = G.paths_to_dev(st["paths_before_gen"][b - 1])
+        out = ctx.crt_generate_secondary(G.bvh, G.mats, fr, b, order, G.rays_to_dev(st["rays"][b - 1]), G.hits_to_dev(st["hits"][b - 1]),
+                                         ctx.upload(st["r2p"][b - 1]), paths)
+        g = st["gen"][b]
+        # integer outputs: bit-exact
+        assert np.array_equal(out["ray_to_path"].cpu().numpy(), g["ray_to_path"])
+        assert np.array_equal(out["dir_src"].cpu().numpy(), g["dir_src"])
+        assert np.array_equal(out["group_id"].cpu().numpy(), g["group_id"])
+        assert int(out["n_active"].cpu().numpy().view(np.uint32)[0]) == g["n_active"]
+        if mode == "direct_reuse":
+            assert np.array_equal(out["group_class"].cpu().numpy(), g["group_class"])
+            saw_hybrid |= bool((g["group_class"] == 3).any())
+        else:
+            # per-path class, written by path id (the oracle writes it per group = per path as well)
+            assert np.array_equal(out["group_class"].cpu().numpy(), g["group_class"])
+        rg = rays_np(oracle, out["rays"])
+        compare_rays(rg, g["rays"])
+        assert rg.tobytes() == g["rays"].tobytes()                        # same fp32 operation sequence: bit-identical rays
+        pg = paths_np(oracle, paths); po = st["paths_after_gen"][b - 1]
+        assert np.array_equal(pg["flags"] & 1, po["flags"] & 1)
+        assert np.allclose(pg["T"], po["T"], rtol=1e-6, atol=0)
+    if scene_name == "checker" and gw * gh > 1:
+        assert saw_hybrid
+
+
+def test_morton_encode_and_radix_sort_bit_exact(crt, ctx, oracle):
+    import torch
+    scene = _small_interior()
+    G = GpuScene(crt, scene, ctx)
+    b = G.bvh.info()["bounds"]
+    for n in (0, 1, 255, 4096, 4097, 100003):
+        r = I.random_rays(n + 1, n, b[:3], b[3:], inactive_frac=0.1)
+        keys = ctx.crt_morton_encode(G.bvh, ctx.upload(r))
+        ko = oracle.morton_encode(r.view(oracle.RAY_DTYPE).reshape(-1), b)
+        assert np.array_equal(keys.cpu().numpy().view(np.uint32), ko)
+        vals = torch.arange(n, dtype=torch.int32, device=ctx.device)
+        if n == 0:
+            continue
+        ks, vs = ctx.crt_radix_sort_pairs(keys, vals)
+        order = oracle.sort_keys(ko)
+        assert np.array_equal(vs.cpu().numpy(), order)
+        assert np.array_equal(ks.cpu().numpy().view(np.uint32), ko[order])
+    # full-range 32-bit keys with many duplicates (all four passes matter, stability matters)
+    rng = np.random.default_rng(0)
+    k = rng.integers(0, 2 ** 32, 50000, dtype=np.uint64).astype(np.uint32); k[::3] = k[0]
+    ks, vs = ctx.crt_radix_sort_pairs(ctx.upload(k.view(np.int32)), torch.arange(len(k), dtype=torch.int32, device=ctx.device))
+    assert np.array_equal(vs.cpu().numpy(), np.argsort(k, kind="stable").astype(np.int32))
+
+
+# ------------------------------------------------------------------ a6: shading, stage-wise
+@pytest.mark.parametrize("scene_name,spp", [("cornell", 1), ("interior_small", 2)])
+def test_shade_accumulate_stagewise(crt, ctx, oracle, scene_name, spp):
+    import torch
+    scene = SCENES[scene_name]()
+    w, h = scene.width, scene.height
+    G = GpuScene(crt, scene, ctx)
+    ofr = oracle.frame(w, h, spp, 1, 0); fr = crt.make_frame(w, h, spp, 1, 0)
+    st = oracle_frame(oracle, scene, ofr, 2, 2, 4, 4, 2)
+    accum = torch.zeros((h, w, 3), device=ctx.device)
+    paths = ctx.empty((spp * w * h, 8)); ctx.crt_paths_init(paths)
+    assert paths_np(oracle, paths).tobytes() == oracle.paths_init(spp * w * h).tobytes()
+    for b in range(0, 3):
+        if b > 0:
+            paths = G.paths_to_dev(st["paths_after_gen"][b - 1])
+        ctx.crt_shade_accumulate(G.bvh, G.mats, fr, b, b == 2, G.rays_to_dev(st["rays"][b]), G.hits_to_dev(st["hits"][b]), ctx.upload(st["r2p"][b]),
+                                 paths, accum)
+        pg = paths_np(oracle, paths); po = st["paths_after_shade"][b]
+        assert np.array_equal(pg["flags"] & 1, po["flags"] & 1)
+        assert np.allclose(pg["L"], po["L"], rtol=1e-6, atol=1e-7)
+    assert rmse(accum.cpu().numpy(), st["accum"]) <= 1e-5
+
+
+# ------------------------------------------------------------------ end to end
+@pytest.mark.parametrize("mode,gw,gh,s", [("independent", 1, 1, 1), ("morton_reorder", 1, 1, 1), ("direct_reuse", 4, 4, 2)])
+def test_config1_end_to_end(crt, ctx, oracle, mode, gw, gh, s):
+    """BASELINE config 1: Cornell 64x64, 1 spp, 1 secondary bounce, groups 4x4 stride 2, seed 0, all three modes."""
+    import torch
+    scene = I.cornell(seed=0)
+    G = GpuScene(crt, scene, ctx)
+    fr = crt.make_frame(64, 64, 1, 0, 0); order = crt.make_order(mode, gw, gh, s)
+    st = oracle_frame(oracle, scene, oracle.frame(64, 64, 1, 0, 0), 1, MODES[mode], gw, gh, s)
+    accum = torch.zeros((64, 64, 3), device=ctx.device)
+    ws = ctx.frame_workspace(fr, order)
+    nsec = torch.zeros((1,), dtype=torch.int32, device=ctx.device)
+    ctx.crt_render_frame(G.bvh, G.mats, G.camera, fr, order, 1, accum, ws, n_secondary=nsec)
+    assert int(nsec.cpu()[0]) == st["gen"][1]["n_active"]
+    assert rmse(accum.cpu().numpy(), st["accum"]) <= 1e-3
+    # the same frame call by call (free-running: GPU buffers feed GPU stages)
+    rays, hits, r2p = ctx.crt_trace_primary(G.bvh, G.camera, fr, order)
+    paths = ctx.empty((64 * 64, 8)); ctx.crt_paths_init(paths)
+    acc2 = torch.zeros_like(accum)
+    ctx.crt_shade_accumulate(G.bvh, G.mats, fr, 0, False, rays, hits, r2p, paths, acc2)
+    out = ctx.crt_generate_secondary(G.bvh, G.mats, fr, 1, order, rays, hits, r2p, paths)
+    g = st["gen"][1]
+    assert np.array_equal(out["ray_to_path"].cpu().numpy(), g["ray_to_path"])
+    assert np.array_equal(out["dir_src"].cpu().numpy(), g["dir_src"])
+    assert np.array_equal(out["group_id"].cpu().numpy(), g["group_id"])
+    assert np.array_equal(out["group_class"].cpu().numpy(), g["group_class"])
+    h2 = ctx.crt_trace(G.bvh, out["rays"])
+    compare_hits(hits_np(oracle, h2), st["hits"][1])
+    ctx.crt_shade_accumulate(G.bvh, G.mats, fr, 1, True, out["rays"], h2, out["ray_to_path"], paths, acc2)
+    assert torch.equal(acc2, accum)
+    # host-buffer entry point gives the same image
+    acc_h = np.zeros((64, 64, 3), np.float32); nsec_h = np.zeros(1, np.uint32)
+    ws_h = ctx.frame_workspace(fr, order, host_materials=len(scene.materials))
+    ctx.crt_render_frame_host(G.bvh, scene.materials, scene.env, G.camera, fr, order, 1, acc_h, nsec_h, ws_h)
+    assert np.array_equal(acc_h, accum.cpu().numpy()) and nsec_h[0] == g["n_active"]
+
+
+@pytest.mark.parametrize("mode,gw,gh,s", [("independent", 1, 1, 1), ("morton_reorder", 1, 1, 1), ("direct_reuse", 4, 4, 4), ("direct_reuse", 8, 8, 2)])
+def test_mixed_materials_two_bounces_end_to_end(crt, ctx, oracle, mode, gw, gh, s):
+    import torch
+    scene = _small_interior()
+    w, h, spp = 96, 64, 2
+    G = GpuScene(crt, scene, ctx)
+    acc_o = np.zeros((h, w, 3), np.float32)
+    accum = torch.zeros((h, w, 3), device=ctx.device)
+    ob = oracle.Bvh(scene.verts)
+    for f in range(2):                                # accumulation over frames
+        fr = crt.make_frame(w, h, spp, 1, f); order = crt.make_order(mode, gw, gh, s)
+        oracle.render_frame(ob, scene, oracle.frame(w, h, spp, 1, f), 2, MODES[mode], gw, gh, s, accum=acc_o)
+        ctx.crt_render_frame(G.bvh, G.mats, G.camera, fr, order, 2, accum, ctx.frame_workspace(fr, order))
+    assert rmse(accum.cpu().numpy() / 2, acc_o / 2) <= 1e-3
+
+
+@pytest.mark.parametrize("mode,gw,gh,s", [("independent", 1, 1, 1), ("morton_reorder", 1, 1, 1), ("direct_reuse", 4, 4, 2)])
+def test_white_furnace_is_one(crt, ctx, mode, gw, gh, s):
+    """Closed form: a convex white Lambert sphere under uniform radiance 1 renders to exactly 1 (north_star)."""
+    import torch
+    scene = I.furnace_sphere(2)
+    G = GpuScene(crt, scene, ctx)
+    fr = crt.make_frame(32, 32, 1, 0, 0); order = crt.make_order(mode, gw, gh, s)
+    accum = torch.zeros((32, 32, 3), device=ctx.device)
+    ctx.crt_render_frame(G.bvh, G.mats, G.camera, fr, order, 2, accum, ctx.frame_workspace(fr, order))
+    assert torch.all(accum == 1.0)
+
+
+def test_argument_errors(crt, ctx):
+    import torch
+    scene = I.cornell()
+    G = GpuScene(crt, scene, ctx)
+    fr = crt.make_frame(64, 64)
+    with pytest.raises(crt.CrtError) as e:
+        crt.crt_layout(fr, crt.make_order("direct_reuse", 3, 4, 2))
+    assert e.value.status == crt.api.CRT_ERR_UNSUPPORTED
+    with pytest.raises(crt.CrtError) as e:
+        crt.crt_layout(fr, crt.make_order("direct_reuse", 16, 16, 8))
+    assert e.value.status == crt.api.CRT_ERR_UNSUPPORTED
+    with pytest.raises(crt.CrtError) as e:
+        crt.crt_layout(fr, crt.make_order(5))
+    assert e.value.status == crt.api.CRT_ERR_INVALID_ARG
+    order = crt.make_order("independent")
+    rays, hits, r2p = ctx.crt_trace_primary(G.bvh, G.camera, fr, order)
+    paths = ctx.empty((64 * 64, 8)); ctx.crt_paths_init(paths)
+    with pytest.raises(crt.CrtError) as e:
+        ctx.crt_generate_secondary(G.bvh, G.mats, fr, 0, order, rays, hits, r2p, paths)     # bounce < 1
+    assert e.value.status == crt.api.CRT_ERR_INVALID_ARG
+    with pytest.raises(crt.CrtError):
+        ctx.crt_set_option("no_such_option", 1)
+    torch.cuda.synchronize()

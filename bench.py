@@ -1,0 +1,299 @@
+#!/usr/bin/env python
+"""bench.py -- secondary-ray MRay/s of the hot path on B200 (BASELINE.json metric), one JSON line on stdout.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload interior|landscape|cornell] [--impl reference]
+
+A step = one frame of the whole hot path: crt_trace_primary -> crt_shade_accumulate(0) ->
+for b = 1..B { crt_generate_secondary(b) -> crt_trace -> crt_shade_accumulate(b) } on one batch of synthetic input
+(default workload: BASELINE config 2, the interior scene at 1920x1080, 1 spp, 2 bounces, groups 4x4, stride 4, seed 1).
+`value` = live secondary rays of the K timed steps / their device time, for mode direct_reuse; the other two modes
+and the stage-level numbers (generate / encode+sort+permute / trace) are in "modes".  See DESIGN.md section 7.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "secondary_ray_throughput"
+UNIT = "MRay/s"
+WORKLOADS = {
+    # name: (scene kwargs, w, h, spp, bounces, gw, gh, stride, seed, BASELINE config index)
+    "cornell": ("cornell", dict(seed=0), 64, 64, 1, 1, 4, 4, 2, 0, 0),
+    "interior": ("interior", dict(seed=1), 1920, 1080, 1, 2, 4, 4, 4, 1, 1),
+    "landscape": ("landscape", dict(seed=2), 1920, 1080, 1, 2, 4, 4, 4, 2, 3),
+}
+# FLOPs of the traversal kernel per unit of work, counted from csrc/trace.cu: a node visit tests two
+# child boxes = 12 (subtract, multiply) pairs + 2 inflations = 26 flop (min/max/compare are not flops); a triangle test
+# (Moller-Trumbore as written in crt_device.cuh) = 2 cross (9 each) + 4 dot (5 each) + 1 subtract-vector (3) + 1 reciprocal (1)
+# + 3 scalings (3) + 1 add (1) = 46 flop.  Ray setup (3 reciprocals) is 3 flop per ray.
+FLOP_PER_NODE_VISIT, FLOP_PER_TRI_TEST, FLOP_PER_RAY = 26.0, 46.0, 3.0
+# nominal FP32 peak from the guide's unit counts: 148 SMs x 128 FP32 lanes x 2 flop (FMA) x 1.965 GHz (B200_PROFILING.md table)
+FP32_PEAK_TFLOPS_NOMINAL = 148 * 128 * 2 * 1.965e9 / 1e12
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the secondary trace kernel, from profiles/ (ncu --set full);
+# keyed by workload; None until captured.
+TRACE_DRAM_TRAFFIC = {"interior": None, "landscape": None, "cornell": None}
+
+
+def _peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), "measured"
+    return 6650.0, "fallback"
+
+
+def _scene(workload, scale=1):
+    import crt_inputs as I
+    name, kw, w, h, spp, nb, gw, gh, s, seed, cfg = WORKLOADS[workload]
+    scene = I.by_name(name, **kw)
+    w, h = max(w // scale, 8), max(h // scale, 8)
+    return scene.with_camera(w, h), (w, h, spp, nb, gw, gh, s, seed, cfg)
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if self.proc:
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=2)
+            except Exception:
+                self.proc.kill()
+        sm = [float(r[0]) for r in self.rows if len(r) >= 7 and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) >= 7 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = sorted({names[k] for r in self.rows if len(r) >= 7 for k in range(4) if r[3 + k].lower().startswith("active")})
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None, "reasons": reasons, "samples": len(sm)}
+
+
+# ------------------------------------------------------------------------------------------------ reference arm (oracle)
+def run_reference(args):
+    """The oracle as it stands, timed on this box's host cores on a bounded sample of the same workload: the same scene and
+    camera at 1/4 x 1/4 of the resolution (1/16 of the pixels), same spp / bounces / grouping, one frame per step."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle as O
+    O.build()
+    scale = 4
+    scene, (w, h, spp, nb, gw, gh, s, seed, cfg) = _scene(args.workload, scale)
+    bvh = O.Bvh(scene.verts)
+    steps, warm = max(1, min(args.steps, 3)), min(args.warmup, 1)
+    rays = 0; secs = 0.0
+    for i in range(warm + steps):
+        t0 = time.perf_counter()
+        _, times, counts = O.render_frame(bvh, scene, O.frame(w, h, spp, seed, i), nb, 2, gw, gh, s)
+        dt = time.perf_counter() - t0
+        if i >= warm:
+            rays += int(counts[0]); secs += dt
+    v = rays / secs / 1e6
+    sample = f"{steps} frame(s) of the {args.workload} scene at {w}x{h} (1/{scale * scale} of the pixels), {spp} spp, {nb} bounces, direct_reuse {gw}x{gh} stride {s}"
+    line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": steps, "warmup": warm,
+            "ms_per_step": 1e3 * secs / steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": f"BASELINE config {cfg + 1}: {args.workload} (bounded sample)", "sample": sample, "mode": "direct_reuse"},
+            "cpu_baseline": {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+            "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def cpu_baseline(workload):
+    import oracle as O
+    O.build()
+    scale = 2
+    scene, (w, h, spp, nb, gw, gh, s, seed, cfg) = _scene(workload, scale)
+    bvh = O.Bvh(scene.verts)
+    t0 = time.perf_counter()
+    _, times, counts = O.render_frame(bvh, scene, O.frame(w, h, spp, seed, 0), nb, 2, gw, gh, s)
+    dt = time.perf_counter() - t0
+    return {"value": counts[0] / dt / 1e6, "unit": UNIT, "cores": 1, "kind": "oracle",
+            "sample": f"1 frame of the {workload} scene at {w}x{h} (1/{scale * scale} of the pixels), {spp} spp, {nb} bounces, direct_reuse {gw}x{gh} stride {s}; "
+                      f"{int(counts[0])} secondary rays in {dt:.2f} s (trace {times[1]:.2f} s, generate {times[0]:.2f} s); BVH build untimed",
+            "secondary_trace_only_mray_s": counts[0] / max(times[1], 1e-9) / 1e6,
+            "node_visits_per_ray": counts[1] / max(counts[0], 1), "tri_tests_per_ray": counts[2] / max(counts[0], 1)}
+
+
+# ------------------------------------------------------------------------------------------------ CUDA arm
+def run_cuda(args):
+    import torch
+    import torch.distributed as dist
+    import paper_2310_07182_b200 as crt
+
+    rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1")); local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    ctx = crt.Context(local)
+    scene, (w, h, spp, nb, gw, gh, s, seed, cfg) = _scene(args.workload)
+    t0 = time.perf_counter()
+    bvh = ctx.crt_build_bvh(scene.verts, scene.mat_id)
+    build_s = time.perf_counter() - t0
+    info = bvh.info()
+    mats_dev = ctx.upload(scene.materials)
+    mats = ctx.scene_mats(mats_dev, len(scene.materials), scene.env)
+    cam = crt.make_camera(scene.camera)
+    stream = torch.cuda.current_stream()
+    K, W = args.steps, args.warmup
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def time_mode(mode, host=False):
+        """W warm-up + K timed frames of one mode; replicas (rank r) render different frame indices."""
+        order = crt.make_order(mode, gw, gh, s)
+        n_paths, n_slots, _ = crt.crt_layout(crt.make_frame(w, h, spp), order)
+        ws = ctx.frame_workspace(crt.make_frame(w, h, spp), order, host_materials=len(scene.materials) if host else 0)
+        nsec = torch.zeros((K + W, max(nb, 1)), dtype=torch.int32, device=ctx.device)
+        stage = np.zeros(8, np.float32)
+        if host:
+            accum_h = torch.zeros((h, w, 3), dtype=torch.float32).pin_memory()
+            nsec_h = np.zeros((K + W, max(nb, 1)), np.uint32)
+            mats_h = scene.materials
+        else:
+            accum = torch.zeros((h, w, 3), device=ctx.device)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+
+        def step(i, rec):
+            fr = crt.make_frame(w, h, spp, seed, i * world + rank)
+            if host:
+                ctx.crt_render_frame_host(bvh, mats_h, scene.env, cam, fr, order, nb, accum_h, nsec_h[i], ws)
+            else:
+                ctx.crt_render_frame(bvh, mats, cam, fr, order, nb, accum, ws, n_secondary=nsec[i], record_times=rec)
+                if rec:
+                    ctx.crt_frame_times(stage)        # synchronises the frame's last event; the K steps still run back to back on the device
+        for i in range(W):
+            step(i, False)
+        barrier()
+        e0.record(stream)
+        for i in range(W, W + K):
+            step(i, not host)
+        e1.record(stream)
+        barrier()
+        ms = e0.elapsed_time(e1)
+        rays = int(nsec_h[W:].sum()) if host else int(nsec[W:].sum().item())
+        t = torch.tensor([ms], dtype=torch.float64, device=ctx.device); r = torch.tensor([rays], dtype=torch.float64, device=ctx.device)
+        if world > 1:
+            dist.all_reduce(t, op=dist.ReduceOp.MAX); dist.all_reduce(r, op=dist.ReduceOp.SUM)
+        ms_all, rays_all = float(t.item()), float(r.item())
+        res = {"mray_s": rays_all / (ms_all * 1e-3) / 1e6, "ms_per_step": ms_all / K, "secondary_rays_per_step": rays / K, "n_slots": n_slots}
+        if not host:
+            sec_ms = float(stage[2] + stage[3])       # generate(+encode+sort+permute) + secondary trace, summed over the K steps (this rank)
+            res.update({"secondary_loop_mray_s": rays / (sec_ms * 1e-3) / 1e6, "trace_only_mray_s": rays / (float(stage[3]) * 1e-3) / 1e6,
+                        "primary_ms": float(stage[0]) / K, "shade_ms": float(stage[1]) / K, "generate_ms": float(stage[2] - stage[4]) / K,
+                        "encode_sort_permute_ms": float(stage[4]) / K, "trace_ms": float(stage[3]) / K, "trace_launch_ms": float(stage[3]) / (K * max(nb, 1))})
+        return res
+
+    clocks = ClockSampler(local)
+    modes = {}
+    clocks.start()
+    modes["direct_reuse"] = time_mode("direct_reuse")
+    clk = clocks.stop()
+    modes["independent"] = time_mode("independent")
+    modes["morton_reorder"] = time_mode("morton_reorder")
+    e2e = time_mode("direct_reuse", host=True)
+
+    # ---- roofline of the dominant kernel (secondary crt_trace): work counters of one frame's secondary rays, outside the timed region
+    order = crt.make_order("direct_reuse", gw, gh, s)
+    fr = crt.make_frame(w, h, spp, seed, W * world + rank)
+    rays, hits, r2p = ctx.crt_trace_primary(bvh, cam, fr, order)
+    n_paths = crt.crt_layout(fr, order)[0]
+    paths = ctx.empty((n_paths, 8)); ctx.crt_paths_init(paths)
+    acc = torch.zeros((h, w, 3), device=ctx.device)
+    ctx.crt_shade_accumulate(bvh, mats, fr, 0, nb == 0, rays, hits, r2p, paths, acc)
+    nn = nt = act = 0
+    for b in range(1, nb + 1):
+        out = ctx.crt_generate_secondary(bvh, mats, fr, b, order, rays, hits, r2p, paths)
+        rays, r2p = out["rays"], out["ray_to_path"]
+        c = ctx.crt_trace_stats(bvh, rays)
+        nn += c[0]; nt += c[1]; act += c[2]
+        hits = ctx.crt_trace(bvh, rays)
+        ctx.crt_shade_accumulate(bvh, mats, fr, b, b == nb, rays, hits, r2p, paths, acc)
+    launches = max(nb, 1)
+    flop_per_launch = (nn * FLOP_PER_NODE_VISIT + nt * FLOP_PER_TRI_TEST + act * FLOP_PER_RAY) / launches
+    dr = modes["direct_reuse"]
+    achieved = flop_per_launch / (dr["trace_launch_ms"] * 1e-3) / 1e12
+    ffma_tflops, copy_gbs = ctx.crt_measure_peaks()
+    hbm_gbs, hbm_src = _peaks()
+    traffic = TRACE_DRAM_TRAFFIC.get(args.workload)
+    rays_per_launch = act / launches
+    bound_alu = FP32_PEAK_TFLOPS_NOMINAL * 1e12 / (flop_per_launch / rays_per_launch) / 1e6         # MRay/s
+    bound_hbm = (hbm_gbs * 1e9 / (traffic / rays_per_launch) / 1e6) if traffic else None
+    roofline = {"bound": "alu", "kernel": "trace_persistent_kernel (secondary rays, direct_reuse)", "achieved": achieved, "peak": FP32_PEAK_TFLOPS_NOMINAL,
+                "unit": "TFLOP/s", "frac": achieved / FP32_PEAK_TFLOPS_NOMINAL, "traffic": traffic,
+                "peak_source": "nominal 148 SM x 128 lanes x 2 x 1.965 GHz (guide); measured FFMA loop in this run: %.1f TFLOP/s" % ffma_tflops,
+                "flop_per_ray": flop_per_launch / rays_per_launch, "node_visits_per_ray": nn / max(act, 1), "tri_tests_per_ray": nt / max(act, 1),
+                "rays_per_launch": rays_per_launch, "launch_ms": dr["trace_launch_ms"],
+                "mray_s_bound_alu": bound_alu, "mray_s_bound_hbm": bound_hbm, "hbm_peak_gbs": hbm_gbs, "hbm_peak_source": hbm_src,
+                "copy_gbs_this_run": copy_gbs, "frac_of_min_bound": dr["trace_only_mray_s"] / min(bound_alu, bound_hbm or bound_alu)}
+
+    if rank != 0:
+        return
+    cpu = cpu_baseline(args.workload) if world == 1 and not args.no_cpu_baseline else None
+    ws_bytes = int(crt.lib().crt_frame_workspace_bytes(__import__("ctypes").byref(fr), __import__("ctypes").byref(order)))
+    img_bytes = w * h * 12
+    line = {
+        "metric": METRIC, "value": dr["mray_s"], "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": dr["ms_per_step"],
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": f"BASELINE config {cfg + 1}: {args.workload} scene, {info['n_tris']} triangles, {w}x{h}, {spp} spp, {nb} bounces, "
+                               f"direct_reuse groups {gw}x{gh} stride {s}, seed {seed}",
+                   "mode": "direct_reuse", "value_is": "live secondary rays per step / device time of the whole step (primary + shading included)",
+                   "l2": f"no explicit flush: each step streams its {ws_bytes / 1e6:.0f} MB workspace plus the {info['device_bytes'] / 1e6:.0f} MB BVH (> 126 MB L2)",
+                   "parallelism": "replicas only (no sharding, no collective)" if world > 1 else "single GPU",
+                   "bvh": {"nodes": info["n_nodes"], "depth": info["depth"], "sah_cost": info["sah_cost"], "device_mb": info["device_bytes"] / 1e6,
+                           "build_s": info["build_seconds"], "build_and_upload_s": build_s}},
+        "modes": modes, "roofline": roofline, "cpu_baseline": cpu,
+        "e2e": {"value": e2e["mray_s"], "unit": UNIT, "h2d_bytes_per_step": img_bytes + len(scene.materials) * 32 + 48,
+                "d2h_bytes_per_step": img_bytes + 4 * nb, "ms_per_step": e2e["ms_per_step"], "api": "crt_render_frame_host"},
+        "gpu_launches": K * (3 + 3 * nb), "clocks": clk,
+    }
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--workload", default="interior", choices=sorted(WORKLOADS))
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "cuda":
+        args.warmup = 3
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_cuda(args)
+
+
+if __name__ == "__main__":
+    main()

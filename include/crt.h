@@ -84,7 +84,8 @@ crt_status crt_destroy(crt_ctx* ctx);
 /* Message of the last failed call on ctx (ctx may be NULL: last failure of a call that had no context). */
 const char* crt_last_error(const crt_ctx* ctx);
 /* Tunables (for experiments; defaults are what bench.py times): "trace_kernel" (0 = one thread per ray,
- * 1 = persistent warps with dynamic fetch), "trace_block", "trace_blocks_per_sm". */
+ * 1 = persistent warps with per-lane dynamic fetch), "trace_refill_threshold" (0..32: idle lanes fetch new rays when
+ * fewer lanes than this are busy), "trace_blocks_per_sm" (0 = from the occupancy calculator). */
 crt_status crt_set_option(crt_ctx* ctx, const char* key, int64_t value);
 /* Measures the device's FP32 FFMA rate (TFLOP/s) and a streaming copy rate (GB/s) with small kernels;
  * synchronous. Used only as roofline denominators by bench.py. */

@@ -266,18 +266,17 @@ void crt_bvh_flatten(const crt_bvh* b, std::vector<GpuNode>& gn, std::vector<Gpu
         gt[j] = t; slot_of_prim[p] = (int32_t)j;
     }
     auto leaf_ref = [](const BuildNode& nd) { return ~((nd.first << 3) | (nd.count - 1)); };
-    auto empty_node = [&] {
-        // a box at +infinity on every axis: the slab test fails for every ray (an inverted box would NOT fail, because
-        // the test takes min/max of the two plane distances)
-        GpuNode g; g.xy0 = g.xy1 = make_float4(inf, inf, inf, inf); g.z01 = make_float4(inf, inf, inf, inf);
-        g.ref0 = g.ref1 = ~0; g.pad0 = g.pad1 = 0; return g;
+    // a box at +infinity on every axis: the slab test fails for every ray (an inverted box would NOT fail, because the
+    // test takes min/max of the two plane distances)
+    auto empty_child = [&] { GpuChild c; c.min_x = c.max_x = c.min_y = c.max_y = c.min_z = c.max_z = inf; c.ref = ~0; c.pad = 0; return c; };
+    auto child_of = [&](const BuildNode& nd, int32_t ref) {
+        GpuChild c; c.min_x = nd.bmin[0]; c.max_x = nd.bmax[0]; c.min_y = nd.bmin[1]; c.max_y = nd.bmax[1]; c.min_z = nd.bmin[2]; c.max_z = nd.bmax[2];
+        c.ref = ref; c.pad = 0; return c;
     };
     gn.clear();
-    if (n == 0) { gn.push_back(empty_node()); return; }
+    if (n == 0) { GpuNode g; g.c[0] = g.c[1] = empty_child(); gn.push_back(g); return; }
     if (b->nodes[0].left < 0) {      // the whole scene is one leaf: a root whose second child is empty
-        GpuNode g = empty_node(); const BuildNode& r = b->nodes[0];
-        g.xy0 = make_float4(r.bmin[0], r.bmax[0], r.bmin[1], r.bmax[1]); g.z01.x = r.bmin[2]; g.z01.y = r.bmax[2];
-        g.ref0 = leaf_ref(r); gn.push_back(g); return;
+        GpuNode g; g.c[0] = child_of(b->nodes[0], leaf_ref(b->nodes[0])); g.c[1] = empty_child(); gn.push_back(g); return;
     }
     // depth-first numbering of inner nodes, left child next to its parent
     std::vector<int32_t> gpu_index(b->nodes.size(), -1), stack{0}, order;
@@ -293,12 +292,8 @@ void crt_bvh_flatten(const crt_bvh* b, std::vector<GpuNode>& gn, std::vector<Gpu
         const BuildNode& nd = b->nodes[order[k]];
         const BuildNode& l = b->nodes[nd.left]; const BuildNode& r = b->nodes[nd.right];
         GpuNode g;
-        g.xy0 = make_float4(l.bmin[0], l.bmax[0], l.bmin[1], l.bmax[1]);
-        g.xy1 = make_float4(r.bmin[0], r.bmax[0], r.bmin[1], r.bmax[1]);
-        g.z01 = make_float4(l.bmin[2], l.bmax[2], r.bmin[2], r.bmax[2]);
-        g.ref0 = l.left >= 0 ? gpu_index[nd.left] : leaf_ref(l);
-        g.ref1 = r.left >= 0 ? gpu_index[nd.right] : leaf_ref(r);
-        g.pad0 = g.pad1 = 0;
+        g.c[0] = child_of(l, l.left >= 0 ? gpu_index[nd.left] : leaf_ref(l));
+        g.c[1] = child_of(r, r.left >= 0 ? gpu_index[nd.right] : leaf_ref(r));
         gn[k] = g;
     }
 }

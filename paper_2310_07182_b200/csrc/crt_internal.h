@@ -13,8 +13,9 @@ struct crt_ctx {
     int n_sms = 0;
     std::string last_error;
     // options
-    int trace_kernel = 1;        // 0: one thread per ray, 1: persistent warps with dynamic fetch
-    int trace_block = 128;
+    int trace_kernel = 1;        // 0: one thread per ray, 1: persistent warps with per-lane dynamic fetch
+    int trace_refill_threshold = 20;   // idle lanes refetch when fewer than this many lanes of the warp are busy
+    int trace_leaf_wait = 3;           // leave the inner-node phase when at most this many converged lanes still lack a leaf
     int trace_blocks_per_sm = 0; // 0 = from occupancy
     // persistent-kernel work counter
     unsigned int* d_counter = nullptr;
@@ -31,13 +32,13 @@ struct BuildNode {
     int32_t first = 0, count = 0;    // leaf: range in prim order
 };
 
-// traversal layout (device): 64 bytes, two child boxes + two child references
-struct alignas(64) GpuNode {
-    float4 xy0;   // child0: min.x, max.x, min.y, max.y
-    float4 xy1;   // child1: min.x, max.x, min.y, max.y
-    float4 z01;   // child0 min.z, max.z, child1 min.z, max.z
-    int32_t ref0, ref1, pad0, pad1;   // >= 0: node index; < 0: ~((tri_offset << 3) | (count - 1))
+// traversal layout (device): 64 bytes = two identical 32-byte child records, each fetched with one 256-bit load
+struct GpuChild {
+    float min_x, max_x, min_y, max_y, min_z, max_z;
+    int32_t ref;     // >= 0: node index; < 0: ~((tri_offset << 3) | (count - 1))
+    int32_t pad;
 };
+struct alignas(64) GpuNode { GpuChild c[2]; };
 // leaf triangle, 48 bytes: v0 | prim id, e1, e2  (e = v - v0 rounded once, as the intersection formula needs)
 struct GpuTri { float4 v0p; float4 e1; float4 e2; };
 

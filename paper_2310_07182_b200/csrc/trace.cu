@@ -2,16 +2,21 @@
 // structure to find the leaf nodes that the ray passes through"; this is "the most time-consuming segment").
 //
 // B200 design:
-//  - one thread per ray, stack-based while-while traversal of a binary BVH whose 64-byte nodes hold both children's
-//    boxes, fetched as two 256-bit loads (ld.global.nc.L2::256B.v8.f32 -> LDG.E.256) on the read-only path;
-//  - leaf triangles are three float4 (v0|id, e1, e2) read with ld.global.nc.v4;
-//  - persistent warps: the grid is sized to fill the 148 SMs once; each warp takes the next 32 consecutive rays
-//    from a global counter when all of its lanes have finished (warp vote), so a slow warp never idles a whole block and
-//    rays stay in slot order inside a warp -- the order the generator made coherent (group-major);
+//  - stack-based traversal of a binary BVH whose 64-byte nodes hold both children's boxes, fetched as two 256-bit loads
+//    (ld.global.nc.v8.f32 -> LDG.E.ENL2.256) on the read-only path; leaf triangles are three float4 (v0|id, e1, e2);
+//  - the kernel is issue-bound, not bandwidth-bound (profiles/): what matters is how many lanes of a warp do useful work.
+//    trace_dyn_kernel is a persistent-warp kernel: the grid fills the 148 SMs once; a lane whose ray has terminated takes
+//    the next ray from a global counter (one atomicAdd per warp, ballot + popc give each idle lane its index) as soon as
+//    fewer than `refill_threshold` lanes of its warp are still traversing, so rays enter a warp in slot order -- the order
+//    the generator made coherent (group-major) -- and divergent stragglers do not idle 31 lanes;
+//  - inner-node and leaf phases are separated (while-while) and a lane that reaches a leaf postpones it and keeps
+//    descending until every converged lane has one, so the triangle tests of a warp run together;
+//  - inactive slots (dead paths, out-of-image slots) are skipped at fetch time and cost one 16-byte load;
 //  - no tensor cores: traversal is not a dense contraction.
-// Exactness: the triangle test is the bit-exact fp32 formula of crt_device.cuh; box tests are conservative
-// (padded boxes, far side inflated, subtree skipped only if its entry distance is strictly beyond the best t), so
-// the result equals the all-triangles definition with ties -> lowest primitive id (D:R10).
+// Exactness: the triangle test is the bit-exact fp32 formula of crt_device.cuh; box tests are conservative (boxes padded at
+// build time by 2^-17 of the largest coordinate, far side inflated, subtree skipped only if its entry distance is strictly
+// beyond the best t), so the result equals the all-triangles definition with ties -> lowest primitive id (D:R10), whatever
+// the order in which leaves are visited.
 #include "crt_device.cuh"
 #include "crt_internal.h"
 
@@ -21,85 +26,93 @@ namespace {
 
 constexpr int STACK_SIZE = 64;
 constexpr int SENTINEL = 0x7fffffff;
+constexpr int TRACE_BLOCK = 128;
 
-struct NodeRegs { float4 xy0, xy1, z01; int ref0, ref1; };
+struct ChildRegs { float min_x, max_x, min_y, max_y, min_z, max_z; int ref; };
 
+// one 32-byte child record through the non-coherent path (LDG.E.ENL2.256.CONSTANT)
+CRT_DEV ChildRegs load_child(const char* p)
+{
+    ChildRegs c; float a6, a7;
+    asm volatile("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                 : "=f"(c.min_x), "=f"(c.max_x), "=f"(c.min_y), "=f"(c.max_y), "=f"(c.min_z), "=f"(c.max_z), "=f"(a6), "=f"(a7) : "l"(p));
+    c.ref = __float_as_int(a6);
+    return c;
+}
+struct NodeRegs { ChildRegs a, b; };
 CRT_DEV NodeRegs load_node(const GpuNode* __restrict__ nodes, int idx)
 {
-    // two 32-byte loads through the non-coherent path
-    const float* p = reinterpret_cast<const float*>(nodes + idx);
-    NodeRegs n; float a0, a1, a2, a3, a4, a5, a6, a7;
-    asm volatile("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
-                 : "=f"(a0), "=f"(a1), "=f"(a2), "=f"(a3), "=f"(a4), "=f"(a5), "=f"(a6), "=f"(a7) : "l"(p));
-    n.xy0 = make_float4(a0, a1, a2, a3); n.xy1 = make_float4(a4, a5, a6, a7);
-    asm volatile("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
-                 : "=f"(a0), "=f"(a1), "=f"(a2), "=f"(a3), "=f"(a4), "=f"(a5), "=f"(a6), "=f"(a7) : "l"(p + 8));
-    n.z01 = make_float4(a0, a1, a2, a3); n.ref0 = __float_as_int(a4); n.ref1 = __float_as_int(a5);
+    const char* p = reinterpret_cast<const char*>(nodes + idx);
+    NodeRegs n; n.a = load_child(p); n.b = load_child(p + 32);
     return n;
 }
 
 struct Hit { float t, u, v; int prim; };
 
-// nearest hit of one ray; `stack` is this thread's private stack.  COUNT: also count node visits / triangle tests.
-template <bool COUNT = false>
-CRT_DEV Hit traverse(const GpuNode* __restrict__ nodes, const GpuTri* __restrict__ tris, V3 o, V3 d, float tmin, float tmax,
-                     unsigned* n_nodes = nullptr, unsigned* n_tris = nullptr)
+// Per-ray traversal state.  The slab test is t = b * (1/d) - o * (1/d) as one FMA per plane: its rounding error is a few
+// ulps of |o/d|, which the build-time padding of the boxes (>= 128 of those ulps for origins inside the padded scene box,
+// DESIGN.md section 5) and the inflated far side absorb; it only ever decides which subtrees are visited.
+struct RayState {
+    V3 o, d;
+    float idx, idy, idz, ox, oy, oz;     // 1/d and -o/d
+    float tmin, tmax;
+    float tfar;                           // best t so far, inflated (prune bound)
+    Hit best;
+    CRT_DEV void init(float4 ro, float4 rd)
+    {
+        o = mk(ro.x, ro.y, ro.z); d = mk(rd.x, rd.y, rd.z);
+        idx = dvd(1.0f, d.x); idy = dvd(1.0f, d.y); idz = dvd(1.0f, d.z);
+        ox = -o.x * idx; oy = -o.y * idy; oz = -o.z * idz;
+        tmin = ro.w; tmax = rd.w; tfar = rd.w;
+        best.t = rd.w; best.u = 0.f; best.v = 0.f; best.prim = -1;
+    }
+};
+
+// Tests both children of `n`; returns the next node reference (nearer child, other child pushed) or pops the stack.
+CRT_DEV int visit_node(const NodeRegs& n, const RayState& r, int* stack, int& sp)
 {
-    Hit best; best.t = tmax; best.u = 0.f; best.v = 0.f; best.prim = -1;
-    const float idx = dvd(1.0f, d.x), idy = dvd(1.0f, d.y), idz = dvd(1.0f, d.z);
-    int stack[STACK_SIZE];
-    int sp = 0;
-    stack[0] = SENTINEL;
-    int node = 0;
-    float tbest = tmax;
-    while (node != SENTINEL) {
-        // ---- inner nodes
-        while (node >= 0 && node != SENTINEL) {
-            const NodeRegs n = load_node(nodes, node);
-            if (COUNT) ++*n_nodes;
-            // slab test, (b - o) * (1/d): error stays relative to the result (no cancellation against o/d)
-            float ax0 = (n.xy0.x - o.x) * idx, ax1 = (n.xy0.y - o.x) * idx;
-            float ay0 = (n.xy0.z - o.y) * idy, ay1 = (n.xy0.w - o.y) * idy;
-            float az0 = (n.z01.x - o.z) * idz, az1 = (n.z01.y - o.z) * idz;
-            float bx0 = (n.xy1.x - o.x) * idx, bx1 = (n.xy1.y - o.x) * idx;
-            float by0 = (n.xy1.z - o.y) * idy, by1 = (n.xy1.w - o.y) * idy;
-            float bz0 = (n.z01.z - o.z) * idz, bz1 = (n.z01.w - o.z) * idz;
-            float tn0 = fmaxf(fmaxf(fminf(ax0, ax1), fminf(ay0, ay1)), fmaxf(fminf(az0, az1), tmin));
-            float tf0 = fminf(fminf(fmaxf(ax0, ax1), fmaxf(ay0, ay1)), fminf(fmaxf(az0, az1), tbest)) * 1.0000005f;
-            float tn1 = fmaxf(fmaxf(fminf(bx0, bx1), fminf(by0, by1)), fmaxf(fminf(bz0, bz1), tmin));
-            float tf1 = fminf(fminf(fmaxf(bx0, bx1), fmaxf(by0, by1)), fminf(fmaxf(bz0, bz1), tbest)) * 1.0000005f;
-            const bool h0 = tn0 <= tf0, h1 = tn1 <= tf1;
-            if (h0 && h1) {
-                const bool swap = tn1 < tn0;
-                const int nearc = swap ? n.ref1 : n.ref0, farc = swap ? n.ref0 : n.ref1;
-                stack[++sp] = farc;
-                node = nearc;
-            } else if (h0 || h1) {
-                node = h0 ? n.ref0 : n.ref1;
-            } else {
-                node = stack[sp--];
+    // a zero direction component with the origin on a slab plane gives 0 * inf = NaN; fminf/fmaxf drop the NaN operand,
+    // which leaves the other planes to decide (conservative)
+    const float ax0 = __fmaf_rn(n.a.min_x, r.idx, r.ox), ax1 = __fmaf_rn(n.a.max_x, r.idx, r.ox);
+    const float ay0 = __fmaf_rn(n.a.min_y, r.idy, r.oy), ay1 = __fmaf_rn(n.a.max_y, r.idy, r.oy);
+    const float az0 = __fmaf_rn(n.a.min_z, r.idz, r.oz), az1 = __fmaf_rn(n.a.max_z, r.idz, r.oz);
+    const float bx0 = __fmaf_rn(n.b.min_x, r.idx, r.ox), bx1 = __fmaf_rn(n.b.max_x, r.idx, r.ox);
+    const float by0 = __fmaf_rn(n.b.min_y, r.idy, r.oy), by1 = __fmaf_rn(n.b.max_y, r.idy, r.oy);
+    const float bz0 = __fmaf_rn(n.b.min_z, r.idz, r.oz), bz1 = __fmaf_rn(n.b.max_z, r.idz, r.oz);
+    const float tn0 = fmaxf(fmaxf(fminf(ax0, ax1), fminf(ay0, ay1)), fmaxf(fminf(az0, az1), r.tmin));
+    const float tf0 = fminf(fminf(fmaxf(ax0, ax1), fmaxf(ay0, ay1)), fminf(fmaxf(az0, az1), r.tfar));
+    const float tn1 = fmaxf(fmaxf(fminf(bx0, bx1), fminf(by0, by1)), fmaxf(fminf(bz0, bz1), r.tmin));
+    const float tf1 = fminf(fminf(fmaxf(bx0, bx1), fmaxf(by0, by1)), fminf(fmaxf(bz0, bz1), r.tfar));
+    const bool h0 = tn0 <= tf0, h1 = tn1 <= tf1;
+    if (h0 && h1) {
+        const bool swap = tn1 < tn0;
+        stack[++sp] = swap ? n.a.ref : n.b.ref;
+        return swap ? n.b.ref : n.a.ref;
+    }
+    if (h0) return n.a.ref;
+    if (h1) return n.b.ref;
+    return stack[sp--];
+}
+
+// Tests the triangles of a leaf reference (D:R10 tie-break: lower primitive id wins at equal t).
+template <bool COUNT>
+CRT_DEV void visit_leaf(const GpuTri* __restrict__ tris, int ref, RayState& r, unsigned& n_tris)
+{
+    const int leaf = ~ref;
+    const int first = leaf >> 3, cnt = (leaf & 7) + 1;
+    for (int j = 0; j < cnt; ++j) {
+        const float4* tp = reinterpret_cast<const float4*>(tris + first + j);
+        const float4 a = __ldg(tp), b = __ldg(tp + 1), c = __ldg(tp + 2);
+        float t, u, v;
+        if (COUNT) ++n_tris;
+        if (tri_test(mk(a.x, a.y, a.z), mk(b.x, b.y, b.z), mk(c.x, c.y, c.z), r.o, r.d, r.tmin, r.tmax, t, u, v)) {
+            const int prim = __float_as_int(a.w);
+            if (r.best.prim < 0 || t < r.best.t || (t == r.best.t && prim < r.best.prim)) {
+                r.best.t = t; r.best.u = u; r.best.v = v; r.best.prim = prim;
+                r.tfar = t * 1.0000005f;
             }
-        }
-        // ---- leaves
-        while (node < 0) {
-            const int leaf = ~node;
-            const int first = leaf >> 3, cnt = (leaf & 7) + 1;
-            for (int j = 0; j < cnt; ++j) {
-                const float4* tp = reinterpret_cast<const float4*>(tris + first + j);
-                const float4 a = __ldg(tp), b = __ldg(tp + 1), c = __ldg(tp + 2);
-                float t, u, v;
-                if (COUNT) ++*n_tris;
-                if (tri_test(mk(a.x, a.y, a.z), mk(b.x, b.y, b.z), mk(c.x, c.y, c.z), o, d, tmin, tmax, t, u, v)) {
-                    const int prim = __float_as_int(a.w);
-                    if (best.prim < 0 || t < best.t || (t == best.t && prim < best.prim)) {
-                        best.t = t; best.u = u; best.v = v; best.prim = prim; tbest = t;
-                    }
-                }
-            }
-            node = stack[sp--];
         }
     }
-    return best;
 }
 
 CRT_DEV void store_hit(crt_hit* hits, int64_t i, const Hit& h)
@@ -107,69 +120,105 @@ CRT_DEV void store_hit(crt_hit* hits, int64_t i, const Hit& h)
     reinterpret_cast<float4*>(hits)[i] = make_float4(h.t, h.u, h.v, __int_as_float(h.prim));
 }
 
-CRT_DEV void trace_one(const GpuNode* __restrict__ nodes, const GpuTri* __restrict__ tris, const crt_ray* __restrict__ rays,
-                       crt_hit* __restrict__ hits, int64_t i)
+// variant 0: one thread per ray, plain while-while loop (kept as the simple cross-check of the persistent kernel)
+__global__ void __launch_bounds__(TRACE_BLOCK) trace_flat_kernel(const GpuNode* __restrict__ nodes, const GpuTri* __restrict__ tris,
+                                                                 const crt_ray* __restrict__ rays, crt_hit* __restrict__ hits, int64_t n)
 {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
     const float4* rp = reinterpret_cast<const float4*>(rays + i);
     const float4 ro = __ldg(rp), rd = __ldg(rp + 1);
-    Hit h; h.t = rd.w; h.u = 0.f; h.v = 0.f; h.prim = -1;
-    if (rd.w >= 0.f) h = traverse(nodes, tris, mk(ro.x, ro.y, ro.z), mk(rd.x, rd.y, rd.z), ro.w, rd.w);
-    store_hit(hits, i, h);
+    RayState r; r.init(ro, rd);
+    if (rd.w >= 0.f) {
+        int stack[STACK_SIZE]; int sp = 0; stack[0] = SENTINEL;
+        int node = 0; unsigned dummy = 0;
+        while (node != SENTINEL) {
+            while ((unsigned)node < (unsigned)SENTINEL) node = visit_node(load_node(nodes, node), r, stack, sp);
+            while (node < 0) { visit_leaf<false>(tris, node, r, dummy); node = stack[sp--]; }
+        }
+    }
+    store_hit(hits, i, r.best);
 }
 
-// variant 0: one thread per ray
-__global__ void __launch_bounds__(128) trace_flat_kernel(const GpuNode* __restrict__ nodes, const GpuTri* __restrict__ tris,
-                                                         const crt_ray* __restrict__ rays, crt_hit* __restrict__ hits, int64_t n)
+// variant 1 (default): persistent warps, per-lane dynamic ray fetch, postponed leaves.  COUNT adds work counters.
+// 9 blocks/SM (<= 56 registers, 36 warps): measured faster than 8 blocks at 64 registers and 10 blocks at 48 (profiles/).
+template <bool COUNT>
+__global__ void __launch_bounds__(TRACE_BLOCK, 9) trace_dyn_kernel(const GpuNode* __restrict__ nodes, const GpuTri* __restrict__ tris,
+                                                                const crt_ray* __restrict__ rays, crt_hit* __restrict__ hits, int64_t n,
+                                                                unsigned int* __restrict__ counter, int refill_threshold, int leaf_wait,
+                                                                unsigned long long* __restrict__ stats)
 {
-    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n) trace_one(nodes, tris, rays, hits, i);
-}
+    const unsigned lane = threadIdx.x & 31u;
+    const unsigned lt_mask = (1u << lane) - 1u;
+    int stack[STACK_SIZE]; int sp = 0; stack[0] = SENTINEL;
+    int node = SENTINEL, leaf = 0;      // leaf: postponed leaf reference (< 0) or 0 = none
+    int ray_idx = -1;
+    bool exhausted = false;
+    RayState r;
+    unsigned c_nodes = 0, c_tris = 0, c_rays = 0;
 
-// variant 1: persistent warps, each fetching the next 32 consecutive rays when the whole warp is done
-__global__ void __launch_bounds__(128) trace_persistent_kernel(const GpuNode* __restrict__ nodes, const GpuTri* __restrict__ tris,
-                                                               const crt_ray* __restrict__ rays, crt_hit* __restrict__ hits, int64_t n,
-                                                               unsigned int* __restrict__ counter)
-{
-    const int lane = threadIdx.x & 31;
     for (;;) {
-        unsigned int base = 0;
-        if (lane == 0) base = atomicAdd(counter, 32u);
-        base = __shfl_sync(0xffffffffu, base, 0);
-        if ((int64_t)base >= n) break;
-        const int64_t i = (int64_t)base + lane;
-        if (i < n) trace_one(nodes, tris, rays, hits, i);
         __syncwarp();
-    }
-}
+        // ---- retire finished rays; idle lanes take the next rays in slot order (warp-wide: one atomic per round)
+        if (node == SENTINEL && ray_idx >= 0) { if (!COUNT) store_hit(hits, ray_idx, r.best); ray_idx = -1; }
+        for (;;) {
+            const bool want = (node == SENTINEL) && !exhausted;
+            const unsigned m = __ballot_sync(0xffffffffu, want);
+            if (m == 0u) break;
+            unsigned base = 0;
+            const int leader = __ffs(m) - 1;
+            if ((int)lane == leader) base = atomicAdd(counter, (unsigned)__popc(m));
+            base = __shfl_sync(0xffffffffu, base, leader);
+            if (want) {
+                const unsigned i = base + __popc(m & lt_mask);        // n < 2^31 (checked by crt_trace); the counter cannot wrap
+                if ((int64_t)i >= n) { exhausted = true; }
+                else {
+                    const float4* rp = reinterpret_cast<const float4*>(rays + i);
+                    const float4 rd = __ldg(rp + 1);
+                    if (rd.w < 0.f) {                 // inactive slot: a miss, nothing to traverse
+                        if (!COUNT) { Hit h; h.t = rd.w; h.u = 0.f; h.v = 0.f; h.prim = -1; store_hit(hits, i, h); }
+                    } else {
+                        r.init(__ldg(rp), rd);
+                        ray_idx = (int)i; node = 0; leaf = 0; sp = 0;
+                        if (COUNT) ++c_rays;
+                    }
+                }
+            }
+        }
+        if (__ballot_sync(0xffffffffu, node != SENTINEL) == 0u) break;     // every lane idle and the ray list is exhausted
+        if (__any_sync(0xffffffffu, exhausted)) refill_threshold = 0;      // nothing left to fetch: run the stragglers to the end
 
-// counting build of the traversal (crt_trace_stats): same code path, results discarded
-__global__ void __launch_bounds__(128) trace_stats_kernel(const GpuNode* __restrict__ nodes, const GpuTri* __restrict__ tris,
-                                                          const crt_ray* __restrict__ rays, int64_t n, unsigned long long* __restrict__ counters)
-{
-    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    unsigned nn = 0, nt = 0, act = 0;
-    if (i < n) {
-        const float4* rp = reinterpret_cast<const float4*>(rays + i);
-        const float4 ro = __ldg(rp), rd = __ldg(rp + 1);
-        if (rd.w >= 0.f) { act = 1; traverse<true>(nodes, tris, mk(ro.x, ro.y, ro.z), mk(rd.x, rd.y, rd.z), ro.w, rd.w, &nn, &nt); }
+        // ---- traverse until this lane's ray ends or too few lanes of the warp are still busy
+        while (node != SENTINEL) {
+            // inner nodes; the first leaf a lane meets is postponed so that the warp's leaves are processed together
+            while ((unsigned)node < (unsigned)SENTINEL) {
+                if (COUNT) ++c_nodes;
+                node = visit_node(load_node(nodes, node), r, stack, sp);
+                if (node < 0 && leaf == 0) { leaf = node; node = stack[sp--]; }
+                if (__popc(__ballot_sync(__activemask(), leaf == 0)) <= leaf_wait) break;   // (nearly) every converged lane holds a leaf
+            }
+            // leaves: the postponed one, then any further leaf references that come off the stack
+            while (leaf < 0) {
+                visit_leaf<COUNT>(tris, leaf, r, c_tris);
+                leaf = 0;
+                if (node < 0) { leaf = node; node = stack[sp--]; }
+            }
+            if (__popc(__activemask()) < refill_threshold) break;
+        }
     }
+    if (COUNT) {
 #pragma unroll
-    for (int d = 16; d > 0; d >>= 1) {
-        nn += __shfl_xor_sync(0xffffffffu, nn, d); nt += __shfl_xor_sync(0xffffffffu, nt, d); act += __shfl_xor_sync(0xffffffffu, act, d);
+        for (int d = 16; d > 0; d >>= 1) {
+            c_nodes += __shfl_xor_sync(0xffffffffu, c_nodes, d); c_tris += __shfl_xor_sync(0xffffffffu, c_tris, d); c_rays += __shfl_xor_sync(0xffffffffu, c_rays, d);
+        }
+        if (lane == 0) { atomicAdd(stats, (unsigned long long)c_nodes); atomicAdd(stats + 1, (unsigned long long)c_tris); atomicAdd(stats + 2, (unsigned long long)c_rays); }
     }
-    if ((threadIdx.x & 31) == 0) { atomicAdd(counters, (unsigned long long)nn); atomicAdd(counters + 1, (unsigned long long)nt); atomicAdd(counters + 2, (unsigned long long)act); }
 }
-
-}  // namespace
-
-namespace {
 
 struct CamDev { float eye[3], U[3], V[3], W[3]; };
 
-// a1: camera ray of the slot's path, then the same traversal (D:R6)
-__global__ void __launch_bounds__(128) primary_kernel(const GpuNode* __restrict__ nodes, const GpuTri* __restrict__ tris, CamDev cam,
-                                                      DevLayout L, int64_t n_slots, crt_ray* __restrict__ rays, crt_hit* __restrict__ hits,
-                                                      int32_t* __restrict__ r2p)
+// a1: camera ray of each slot's path (D:R6); the rays are then traversed by the same kernel as secondary rays
+__global__ void __launch_bounds__(256) primary_rays_kernel(CamDev cam, DevLayout L, int64_t n_slots, crt_ray* __restrict__ rays, int32_t* __restrict__ r2p)
 {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n_slots) return;
@@ -177,11 +226,7 @@ __global__ void __launch_bounds__(128) primary_kernel(const GpuNode* __restrict_
     const int32_t p = slot_to_path(L, i, pixel, sample);
     r2p[i] = p;
     float4* rp = reinterpret_cast<float4*>(rays + i);
-    if (p < 0) {
-        rp[0] = make_float4(0.f, 0.f, 0.f, 0.f); rp[1] = make_float4(0.f, 0.f, 0.f, -1.f);
-        Hit h; h.t = -1.f; h.u = 0.f; h.v = 0.f; h.prim = -1; store_hit(hits, i, h);
-        return;
-    }
+    if (p < 0) { rp[0] = make_float4(0.f, 0.f, 0.f, 0.f); rp[1] = make_float4(0.f, 0.f, 0.f, -1.f); return; }
     const int32_t x = pixel % L.w, y = pixel / L.w;
     const uint4 r = philox((uint32_t)pixel, (uint32_t)sample, 0u, PURPOSE_CAMERA, L.seed, L.frame);
     const float jx = u01(r.x), jy = u01(r.y);
@@ -194,8 +239,22 @@ __global__ void __launch_bounds__(128) primary_kernel(const GpuNode* __restrict_
     dx = dvd(dx, len); dy = dvd(dy, len); dz = dvd(dz, len);
     rp[0] = make_float4(cam.eye[0], cam.eye[1], cam.eye[2], 0.f);
     rp[1] = make_float4(dx, dy, dz, 1e30f);
-    const Hit h = traverse(nodes, tris, mk(cam.eye[0], cam.eye[1], cam.eye[2]), mk(dx, dy, dz), 0.f, 1e30f);
-    store_hit(hits, i, h);
+}
+
+template <bool COUNT>
+crt_status launch_dyn(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, crt_hit* hits, unsigned long long* stats, cudaStream_t st)
+{
+    int per_sm = ctx->trace_blocks_per_sm;
+    if (per_sm <= 0) {
+        CRT_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, trace_dyn_kernel<COUNT>, TRACE_BLOCK, 0));
+        if (per_sm < 1) per_sm = 1;
+    }
+    CRT_CUDA(ctx, cudaMemsetAsync(ctx->d_counter, 0, sizeof(unsigned int), st));
+    int64_t want = (n + TRACE_BLOCK - 1) / TRACE_BLOCK, grid = (int64_t)ctx->n_sms * per_sm;
+    if (grid > want) grid = want;
+    trace_dyn_kernel<COUNT><<<(unsigned)grid, TRACE_BLOCK, 0, st>>>(bvh->d_nodes, bvh->d_tris, rays, hits, n, ctx->d_counter, ctx->trace_refill_threshold, ctx->trace_leaf_wait, stats);
+    CRT_CHECK_LAUNCH(ctx, "trace_dyn");
+    return CRT_OK;
 }
 
 }  // namespace
@@ -213,29 +272,18 @@ crt_status launch_trace(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, i
 {
     if (n == 0) return CRT_OK;
     if (ctx->trace_kernel == 0) {
-        const int block = 128;
-        trace_flat_kernel<<<(unsigned)((n + block - 1) / block), block, 0, st>>>(bvh->d_nodes, bvh->d_tris, rays, hits, n);
-    } else {
-        int per_sm = ctx->trace_blocks_per_sm;
-        if (per_sm <= 0) {
-            CRT_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, trace_persistent_kernel, 128, 0));
-            if (per_sm < 1) per_sm = 1;
-        }
-        CRT_CUDA(ctx, cudaMemsetAsync(ctx->d_counter, 0, sizeof(unsigned int), st));
-        int64_t want = (n + 127) / 128, grid = (int64_t)ctx->n_sms * per_sm;
-        if (grid > want) grid = want;
-        trace_persistent_kernel<<<(unsigned)grid, 128, 0, st>>>(bvh->d_nodes, bvh->d_tris, rays, hits, n, ctx->d_counter);
+        trace_flat_kernel<<<(unsigned)((n + TRACE_BLOCK - 1) / TRACE_BLOCK), TRACE_BLOCK, 0, st>>>(bvh->d_nodes, bvh->d_tris, rays, hits, n);
+        CRT_CHECK_LAUNCH(ctx, "trace_flat");
+        return CRT_OK;
     }
-    CRT_CHECK_LAUNCH(ctx, "trace");
-    return CRT_OK;
+    return launch_dyn<false>(ctx, bvh, rays, n, hits, nullptr, st);
 }
 
+// counting build of the default kernel (crt_trace_stats): same traversal, no hit records written
 crt_status launch_trace_stats(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, int64_t* counters, cudaStream_t st)
 {
     if (n == 0) return CRT_OK;
-    trace_stats_kernel<<<(unsigned)((n + 127) / 128), 128, 0, st>>>(bvh->d_nodes, bvh->d_tris, rays, n, reinterpret_cast<unsigned long long*>(counters));
-    CRT_CHECK_LAUNCH(ctx, "trace_stats");
-    return CRT_OK;
+    return launch_dyn<true>(ctx, bvh, rays, n, nullptr, reinterpret_cast<unsigned long long*>(counters), st);
 }
 
 crt_status launch_primary(crt_ctx* ctx, const crt_bvh* bvh, const crt_camera& cam, const crt_frame& f, const Layout& L,
@@ -244,9 +292,7 @@ crt_status launch_primary(crt_ctx* ctx, const crt_bvh* bvh, const crt_camera& ca
     if (L.n_slots == 0) return CRT_OK;
     CamDev c;
     for (int k = 0; k < 3; ++k) { c.eye[k] = cam.eye[k]; c.U[k] = cam.U[k]; c.V[k] = cam.V[k]; c.W[k] = cam.W[k]; }
-    const int block = 128;
-    primary_kernel<<<(unsigned)((L.n_slots + block - 1) / block), block, 0, st>>>(bvh->d_nodes, bvh->d_tris, c, make_dev_layout(L, f), L.n_slots,
-                                                                                  rays, hits, r2p);
-    CRT_CHECK_LAUNCH(ctx, "primary");
-    return CRT_OK;
+    primary_rays_kernel<<<(unsigned)((L.n_slots + 255) / 256), 256, 0, st>>>(c, make_dev_layout(L, f), L.n_slots, rays, r2p);
+    CRT_CHECK_LAUNCH(ctx, "primary_rays");
+    return launch_trace(ctx, bvh, rays, L.n_slots, hits, st);
 }

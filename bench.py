@@ -142,6 +142,22 @@ def cpu_baseline(workload):
 
 
 # ------------------------------------------------------------------------------------------------ CUDA arm
+def reduce_over_ranks(ms, rays, device, world):
+    """Whole-job figures of N independent replicas: time = MAX over ranks, rays = SUM over ranks.
+    The only collectives of the bench; there is none on the data path."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms], dtype=torch.float64, device=device); r = torch.tensor([rays], dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX); dist.all_reduce(r, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(r.item())
+
+
+def replica_frame_index(step, rank, world):
+    """Replicas render disjoint frame indices so that no two ranks repeat the same work."""
+    return step * world + rank
+
+
 def run_cuda(args):
     import torch
     import torch.distributed as dist
@@ -183,7 +199,7 @@ def run_cuda(args):
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
 
         def step(i, rec):
-            fr = crt.make_frame(w, h, spp, seed, i * world + rank)
+            fr = crt.make_frame(w, h, spp, seed, replica_frame_index(i, rank, world))
             if host:
                 ctx.crt_render_frame_host(bvh, mats_h, scene.env, cam, fr, order, nb, accum_h, nsec_h[i], ws)
             else:
@@ -200,10 +216,7 @@ def run_cuda(args):
         barrier()
         ms = e0.elapsed_time(e1)
         rays = int(nsec_h[W:].sum()) if host else int(nsec[W:].sum().item())
-        t = torch.tensor([ms], dtype=torch.float64, device=ctx.device); r = torch.tensor([rays], dtype=torch.float64, device=ctx.device)
-        if world > 1:
-            dist.all_reduce(t, op=dist.ReduceOp.MAX); dist.all_reduce(r, op=dist.ReduceOp.SUM)
-        ms_all, rays_all = float(t.item()), float(r.item())
+        ms_all, rays_all = reduce_over_ranks(ms, rays, ctx.device, world)
         res = {"mray_s": rays_all / (ms_all * 1e-3) / 1e6, "ms_per_step": ms_all / K, "secondary_rays_per_step": rays / K, "n_slots": n_slots}
         if not host:
             sec_ms = float(stage[2] + stage[3])       # generate(+encode+sort+permute) + secondary trace, summed over the K steps (this rank)
@@ -216,10 +229,10 @@ def run_cuda(args):
     modes = {}
     clocks.start()
     modes["direct_reuse"] = time_mode("direct_reuse")
-    clk = clocks.stop()
     modes["independent"] = time_mode("independent")
     modes["morton_reorder"] = time_mode("morton_reorder")
     e2e = time_mode("direct_reuse", host=True)
+    clk = clocks.stop()
 
     # ---- roofline of the dominant kernel (secondary crt_trace): work counters of one frame's secondary rays, outside the timed region
     order = crt.make_order("direct_reuse", gw, gh, s)
@@ -281,7 +294,7 @@ def run_cuda(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=100)      # the paper averages 100 frames per run
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--workload", default="interior", choices=sorted(WORKLOADS))

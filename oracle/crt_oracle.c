@@ -26,8 +26,9 @@
  *   reuse rule        bit-identical local directions in a diffuse group, leader == independent sample,
  *                     upper hemisphere, fp64 normalised mean in hybrid groups
  *   cosine sampling   E[cos]=2/3 and chi-square on a histogram
- *   GGX               weight <= 1, white-furnace energy <= 1; its sampled distribution has no closed
- *                     form to compare with here: **parity unpinned** for the GGX lobe shape (oracle==GPU only)
+ *   GGX               moments of the sampled half-vector vs fp64 quadrature of the textbook visible-normal
+ *                     density D_v(h) = G1(wo) max(0, wo.h) D(h) / wo.z (Heitz 2018); weight <= 1; |wi| = 1;
+ *                     white-furnace energy <= 1
  *   morton + sort     bit-by-bit loop encoder vs a python magic-mask encoder, numpy stable argsort
  *   shade/accumulate  closed-form furnace (white sphere under uniform light == 1), albedo series
  */

@@ -308,6 +308,26 @@ def test_morton_code_and_sort(oracle):
     assert np.all(order[1:][eq] > order[:-1][eq])                    # equal keys keep input order
 
 
+def test_morton_golden(oracle):
+    """Hand-derived codes (tests/golden/morton_codes.txt): quantised cells and bit patterns written out per level."""
+    import os
+    rows = [l for l in open(os.path.join(os.path.dirname(__file__), "golden", "morton_codes.txt")) if not l.startswith("#")]
+    assert len(rows) >= 6
+    rays = np.zeros(len(rows), oracle.RAY_DTYPE)
+    exp = []
+    for i, l in enumerate(rows):
+        vals, q, levels, code = [p.strip() for p in l.split("|")]
+        v = [float(x) for x in vals.split()]
+        rays["o"][i] = v[:3]; rays["d"][i] = v[3:]; rays["tmax"][i] = 1e30
+        bits = "".join(levels.split())
+        assert len(bits) == 30 and int(bits, 2) == int(code, 16)          # the fixture is self-consistent
+        qs = [int(x) for x in q.split()]
+        assert bits == "".join(str((qs[k] >> lv) & 1) for lv in (4, 3, 2, 1, 0) for k in range(6))
+        exp.append(int(code, 16))
+    keys = oracle.morton_encode(rays, np.array([0, 0, 0, 1, 1, 1], np.float32))
+    assert [int(k) for k in keys] == exp
+
+
 def test_morton_mode_is_a_sorted_permutation_of_independent_rays(oracle):
     sc = I.interior(n_boxes=40, n_spheres=10, subdiv=2, width=48, height=32)
     gm = _first_bounce(oracle, sc, M_MOR); gi = _first_bounce(oracle, sc, M_IND)

@@ -66,7 +66,8 @@ class BvhParams(C.Structure):
 
 class BvhInfo(C.Structure):
     _fields_ = [("n_tris", C.c_int64), ("n_nodes", C.c_int64), ("device_bytes", C.c_int64), ("bounds", C.c_float * 6),
-                ("sah_cost", C.c_double), ("depth", C.c_int32), ("max_leaf", C.c_int32), ("build_seconds", C.c_double)]
+                ("sah_cost", C.c_double), ("depth", C.c_int32), ("max_leaf", C.c_int32), ("build_seconds", C.c_double),
+                ("n_wide_nodes", C.c_int64), ("wide_depth", C.c_int32), ("pad", C.c_int32)]
 
 
 _lib = None
@@ -139,7 +140,8 @@ class Bvh:
         o = BvhInfo()
         self.ctx._check(lib().crt_bvh_get_info(self.handle, C.byref(o)))
         return {"n_tris": o.n_tris, "n_nodes": o.n_nodes, "device_bytes": o.device_bytes, "bounds": np.array(list(o.bounds), np.float32),
-                "sah_cost": o.sah_cost, "depth": o.depth, "max_leaf": o.max_leaf, "build_seconds": o.build_seconds}
+                "sah_cost": o.sah_cost, "depth": o.depth, "max_leaf": o.max_leaf, "build_seconds": o.build_seconds,
+                "n_wide_nodes": o.n_wide_nodes, "wide_depth": o.wide_depth}
 
     def check(self):
         v = C.c_int32(-1)
@@ -212,7 +214,7 @@ class Context:
         return a.value, b.value
 
     # ---- a0 -----------------------------------------------------------------------------------------
-    def crt_build_bvh(self, verts, mat_id, max_leaf=4, sah_bins=16, n_threads=0):
+    def crt_build_bvh(self, verts, mat_id, max_leaf=1, sah_bins=16, n_threads=0, cost_traversal=1.0, cost_intersect=1.0):
         """verts: numpy float32[n,3,3] or torch tensor (host or device); mat_id int32[n]."""
         if isinstance(verts, np.ndarray):
             verts = np.ascontiguousarray(verts, np.float32)
@@ -220,7 +222,7 @@ class Context:
             n = verts.size // 9
         else:
             n = verts.numel() // 9
-        pr = BvhParams(max_leaf, sah_bins, 1.0, 1.0, n_threads)
+        pr = BvhParams(max_leaf, sah_bins, cost_traversal, cost_intersect, n_threads)
         h = C.c_void_p()
         self._check(lib().crt_build_bvh(self.handle, _ptr(verts), _ptr(mat_id), C.c_int64(n), C.byref(pr), C.byref(h)))
         return Bvh(self, h)

@@ -249,23 +249,30 @@ int32_t crt_bvh_check_host(const crt_bvh* b)
     return bad;
 }
 
-// Flattens the host tree into the traversal layout (host vectors; the caller uploads them).
-void crt_bvh_flatten(const crt_bvh* b, std::vector<GpuNode>& gn, std::vector<GpuTri>& gt, std::vector<int32_t>& slot_of_prim)
+// Flattens the host tree into the binary traversal layout (host vectors; the caller uploads them).
+// tri_order: caller's triangle id stored at position j of the device triangle array; empty = the tree's own leaf order.
+// A non-empty order (the wide layout's) requires one triangle per leaf, so that every leaf is still one contiguous range.
+void crt_bvh_flatten(const crt_bvh* b, const std::vector<int32_t>& tri_order, std::vector<GpuNode>& gn, std::vector<GpuTri>& gt, std::vector<int32_t>& slot_of_prim)
 {
     const float inf = std::numeric_limits<float>::infinity();
     const int64_t n = b->n_tris;
+    const bool own = tri_order.empty();
     gt.resize((size_t)n); slot_of_prim.assign((size_t)n, -1);
     for (int64_t j = 0; j < n; ++j) {
-        int32_t p = b->prim[j];
+        int32_t p = own ? b->prim[j] : tri_order[j];
         const float* tv = b->verts.data() + 9 * (int64_t)p;
         GpuTri t;
         t.v0p = make_float4(tv[0], tv[1], tv[2], 0.f);
         std::memcpy(&t.v0p.w, &p, 4);
         t.e1 = make_float4(tv[3] - tv[0], tv[4] - tv[1], tv[5] - tv[2], 0.f);
         t.e2 = make_float4(tv[6] - tv[0], tv[7] - tv[1], tv[8] - tv[2], 0.f);
+        t.pad = make_float4(0.f, 0.f, 0.f, 0.f);
         gt[j] = t; slot_of_prim[p] = (int32_t)j;
     }
-    auto leaf_ref = [](const BuildNode& nd) { return ~((nd.first << 3) | (nd.count - 1)); };
+    auto leaf_ref = [&](const BuildNode& nd) {
+        const int32_t first = own ? nd.first : slot_of_prim[b->prim[nd.first]];
+        return ~((first << 3) | (nd.count - 1));
+    };
     // a box at +infinity on every axis: the slab test fails for every ray (an inverted box would NOT fail, because the
     // test takes min/max of the two plane distances)
     auto empty_child = [&] { GpuChild c; c.min_x = c.max_x = c.min_y = c.max_y = c.min_z = c.max_z = inf; c.ref = ~0; c.pad = 0; return c; };

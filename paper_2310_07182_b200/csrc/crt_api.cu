@@ -5,7 +5,9 @@
 
 bool crt_bvh_build_host(crt_bvh* b, const float* verts, int64_t n, const crt_bvh_params& pr);
 int32_t crt_bvh_check_host(const crt_bvh* b);
-void crt_bvh_flatten(const crt_bvh* b, std::vector<GpuNode>& gn, std::vector<GpuTri>& gt, std::vector<int32_t>& slot_of_prim);
+void crt_bvh_flatten(const crt_bvh* b, const std::vector<int32_t>& tri_order, std::vector<GpuNode>& gn, std::vector<GpuTri>& gt, std::vector<int32_t>& slot_of_prim);
+void crt_bvh_build_wide(const crt_bvh* b, std::vector<WNode>& wn, std::vector<int32_t>& tri_order, int* depth_out);
+int32_t crt_bvh_check_wide(const crt_bvh* b, const std::vector<WNode>& wn, const std::vector<int32_t>& tri_order);
 
 static thread_local std::string g_last_error;
 
@@ -82,9 +84,10 @@ const char* crt_last_error(const crt_ctx* ctx) { return ctx ? ctx->last_error.c_
 crt_status crt_set_option(crt_ctx* ctx, const char* key, int64_t value)
 {
     if (!ctx || !key) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "set_option: null argument");
-    if (!strcmp(key, "trace_kernel")) { if (value < 0 || value > 1) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "trace_kernel must be 0 or 1"); ctx->trace_kernel = (int)value; }
+    if (!strcmp(key, "trace_kernel")) { if (value < 0 || value > 2) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "trace_kernel must be 0, 1 or 2"); ctx->trace_kernel = (int)value; }
     else if (!strcmp(key, "trace_refill_threshold")) { if (value < 0 || value > 32) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "trace_refill_threshold out of range"); ctx->trace_refill_threshold = (int)value; }
     else if (!strcmp(key, "trace_leaf_wait")) { if (value < 0 || value > 31) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "trace_leaf_wait out of range"); ctx->trace_leaf_wait = (int)value; }
+    else if (!strcmp(key, "trace_tri_wait")) { if (value < 0 || value > 32) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "trace_tri_wait out of range"); ctx->trace_tri_wait = (int)value; }
     else if (!strcmp(key, "trace_blocks_per_sm")) { if (value < 0 || value > 32) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "trace_blocks_per_sm out of range"); ctx->trace_blocks_per_sm = (int)value; }
     else return crt_fail(ctx, CRT_ERR_INVALID_ARG, "set_option: unknown key '%s'", key);
     return CRT_OK;
@@ -110,7 +113,7 @@ crt_status crt_build_bvh(crt_ctx* ctx, const float* verts, const int32_t* mat_id
     *out = nullptr;
     if (n_tris < 0 || (n_tris > 0 && !verts)) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "build_bvh: bad triangle array");
     if (n_tris >= ((int64_t)1 << 28)) return crt_fail(ctx, CRT_ERR_UNSUPPORTED, "build_bvh: more than 2^28 triangles");
-    crt_bvh_params pr = {4, 16, 1.0f, 1.0f, 0};
+    crt_bvh_params pr = {1, 16, 1.0f, 1.0f, 0};
     if (params) pr = *params;
     if (pr.max_leaf < 1 || pr.max_leaf > 8) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "build_bvh: max_leaf %d not in [1,8]", pr.max_leaf);
     if (pr.sah_bins == 0) pr.sah_bins = 16;
@@ -129,9 +132,17 @@ crt_status crt_build_bvh(crt_ctx* ctx, const float* verts, const int32_t* mat_id
     crt_bvh* b = new crt_bvh();
     crt_bvh_build_host(b, v, n_tris, pr);
     if (b->depth > 60) { delete b; return crt_fail(ctx, CRT_ERR_UNSUPPORTED, "build_bvh: tree depth exceeds the traversal stack (64)"); }
+    // one triangle per leaf: also build the 8-wide compressed layout (the default kernel's); its triangle order is the shared one
+    std::vector<WNode> wn; std::vector<int32_t> tri_order;
+    if (pr.max_leaf == 1) {
+        crt_bvh_build_wide(b, wn, tri_order, &b->wide_depth);
+        b->n_wide_nodes = (int64_t)wn.size();
+        b->wide_violations = crt_bvh_check_wide(b, wn, tri_order);
+        if (b->wide_depth > 40) { delete b; return crt_fail(ctx, CRT_ERR_UNSUPPORTED, "build_bvh: wide tree depth %d exceeds the traversal stack", b->wide_depth); }
+    }
     if (ctx) {
         std::vector<GpuNode> gn; std::vector<GpuTri> gt; std::vector<int32_t> sop;
-        crt_bvh_flatten(b, gn, gt, sop);
+        crt_bvh_flatten(b, tri_order, gn, gt, sop);
         b->device = ctx->device; b->n_gpu_nodes = (int64_t)gn.size();
         auto up = [&](void** d, const void* h, size_t bytes) -> cudaError_t {
             cudaError_t e = cudaMalloc(d, bytes ? bytes : 256);
@@ -141,6 +152,7 @@ crt_status crt_build_bvh(crt_ctx* ctx, const float* verts, const int32_t* mat_id
         };
         cudaError_t e = up((void**)&b->d_nodes, gn.data(), gn.size() * sizeof(GpuNode));
         if (e == cudaSuccess) e = up((void**)&b->d_tris, gt.data(), gt.size() * sizeof(GpuTri));
+        if (e == cudaSuccess && !wn.empty()) e = up((void**)&b->d_wnodes, wn.data(), wn.size() * sizeof(WNode));
         if (e == cudaSuccess) e = up((void**)&b->d_slot_of_prim, sop.data(), sop.size() * 4);
         if (e == cudaSuccess) e = up((void**)&b->d_mat_id, hm.data(), hm.size() * 4);
         if (e != cudaSuccess) { crt_bvh_destroy(b); return crt_fail(ctx, e == cudaErrorMemoryAllocation ? CRT_ERR_NOMEM : CRT_ERR_CUDA, "build_bvh: upload: %s", cudaGetErrorString(e)); }
@@ -152,7 +164,7 @@ crt_status crt_build_bvh(crt_ctx* ctx, const float* verts, const int32_t* mat_id
 crt_status crt_bvh_destroy(crt_bvh* b)
 {
     if (!b) return CRT_OK;
-    cudaFree(b->d_nodes); cudaFree(b->d_tris); cudaFree(b->d_slot_of_prim); cudaFree(b->d_mat_id);
+    cudaFree(b->d_nodes); cudaFree(b->d_wnodes); cudaFree(b->d_tris); cudaFree(b->d_slot_of_prim); cudaFree(b->d_mat_id);
     delete b;
     return CRT_OK;
 }
@@ -163,13 +175,14 @@ crt_status crt_bvh_get_info(const crt_bvh* b, crt_bvh_info_t* o)
     o->n_tris = b->n_tris; o->n_nodes = (int64_t)b->nodes.size(); o->device_bytes = b->device_bytes;
     memcpy(o->bounds, b->bounds, sizeof o->bounds);
     o->sah_cost = b->sah; o->depth = b->depth; o->max_leaf = b->max_leaf; o->build_seconds = b->build_seconds;
+    o->n_wide_nodes = b->n_wide_nodes; o->wide_depth = b->wide_depth;
     return CRT_OK;
 }
 
 crt_status crt_bvh_check(const crt_bvh* b, int32_t* violations)
 {
     if (!b || !violations) return crt_fail(nullptr, CRT_ERR_INVALID_ARG, "bvh_check: null argument");
-    *violations = crt_bvh_check_host(b);
+    *violations = crt_bvh_check_host(b) | (b->wide_violations << 8);
     return CRT_OK;
 }
 

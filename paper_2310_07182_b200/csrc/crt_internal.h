@@ -13,9 +13,10 @@ struct crt_ctx {
     int n_sms = 0;
     std::string last_error;
     // options
-    int trace_kernel = 1;        // 0: one thread per ray, 1: persistent warps with per-lane dynamic fetch
+    int trace_kernel = 2;        // 0: binary BVH, one thread per ray; 1: binary BVH, persistent warps; 2: 8-wide compressed BVH, persistent warps (falls back to 1 when the BVH has no wide layout)
     int trace_refill_threshold = 20;   // idle lanes refetch when fewer than this many lanes of the warp are busy
     int trace_leaf_wait = 3;           // leave the inner-node phase when at most this many converged lanes still lack a leaf
+    int trace_tri_wait = 8;            // wide kernel: a warp enters its triangle phase when at least this many lanes hold triangle hits
     int trace_blocks_per_sm = 0; // 0 = from occupancy
     // persistent-kernel work counter
     unsigned int* d_counter = nullptr;
@@ -39,8 +40,20 @@ struct GpuChild {
     int32_t pad;
 };
 struct alignas(64) GpuNode { GpuChild c[2]; };
-// leaf triangle, 48 bytes: v0 | prim id, e1, e2  (e = v - v0 rounded once, as the intersection formula needs)
-struct GpuTri { float4 v0p; float4 e1; float4 e2; };
+// leaf triangle, 64 bytes = two 256-bit loads: v0 | prim id, e1 | 0, e2 | 0, padding
+// (e = v - v0 rounded once, as the intersection formula needs)
+struct alignas(64) GpuTri { float4 v0p; float4 e1; float4 e2; float4 pad; };
+// 8-wide compressed node, 128 bytes = four 256-bit loads (layout and rounding rules: bvh_wide.cpp)
+struct alignas(128) WNode {
+    float px, py, pz;        // origin of the node's box
+    float ex;                // E.x: power of two >= extent
+    uint32_t eyz;            // E.y (high half) | E.z (low half) as bf16
+    uint32_t child_base;     // index of the first inner child
+    uint32_t tri_base;       // position of the first triangle child
+    uint32_t masks;          // imask (inner children) | lmask << 8 (triangle children)
+    uint32_t planes[3][8];   // per axis: 4 words of LO planes, 4 words of HI planes; word k = children 2k (low half), 2k+1 (high half)
+};
+static_assert(sizeof(WNode) == 128 && sizeof(GpuTri) == 64, "device layouts");
 
 struct crt_bvh {
     int64_t n_tris = 0;
@@ -53,7 +66,8 @@ struct crt_bvh {
     // device data
     int device = -1;
     GpuNode* d_nodes = nullptr; int64_t n_gpu_nodes = 0;
-    GpuTri* d_tris = nullptr;          // leaf order
+    GpuTri* d_tris = nullptr;          // leaf order (wide order when the wide layout exists)
+    WNode* d_wnodes = nullptr; int64_t n_wide_nodes = 0; int wide_depth = 0; int32_t wide_violations = 0;   // 8-wide layout (only when max_leaf == 1)
     int32_t* d_slot_of_prim = nullptr; // caller's triangle id -> index into d_tris
     int32_t* d_mat_id = nullptr;       // by caller's triangle id
     int64_t device_bytes = 0;
@@ -84,6 +98,8 @@ crt_status crt_make_layout(crt_ctx* ctx, const crt_frame* f, const crt_order* o,
 
 // kernels' host launchers (defined in the .cu files) ------------------------------------------------------
 crt_status launch_trace(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, crt_hit* hits, cudaStream_t st);
+crt_status launch_trace_wide(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, crt_hit* hits, cudaStream_t st);
+crt_status launch_trace_wide_stats(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, int64_t* counters, cudaStream_t st);
 crt_status launch_trace_stats(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, int64_t* counters, cudaStream_t st);
 crt_status launch_primary(crt_ctx* ctx, const crt_bvh* bvh, const crt_camera& cam, const crt_frame& f, const Layout& L,
                           crt_ray* rays, crt_hit* hits, int32_t* r2p, cudaStream_t st);

@@ -271,6 +271,7 @@ crt::DevLayout make_dev_layout(const Layout& L, const crt_frame& f)
 crt_status launch_trace(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, crt_hit* hits, cudaStream_t st)
 {
     if (n == 0) return CRT_OK;
+    if (ctx->trace_kernel == 2 && bvh->d_wnodes) return launch_trace_wide(ctx, bvh, rays, n, hits, st);
     if (ctx->trace_kernel == 0) {
         trace_flat_kernel<<<(unsigned)((n + TRACE_BLOCK - 1) / TRACE_BLOCK), TRACE_BLOCK, 0, st>>>(bvh->d_nodes, bvh->d_tris, rays, hits, n);
         CRT_CHECK_LAUNCH(ctx, "trace_flat");
@@ -283,6 +284,7 @@ crt_status launch_trace(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, i
 crt_status launch_trace_stats(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, int64_t* counters, cudaStream_t st)
 {
     if (n == 0) return CRT_OK;
+    if (ctx->trace_kernel == 2 && bvh->d_wnodes) return launch_trace_wide_stats(ctx, bvh, rays, n, counters, st);
     return launch_dyn<true>(ctx, bvh, rays, n, nullptr, reinterpret_cast<unsigned long long*>(counters), st);
 }
 

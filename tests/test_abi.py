@@ -77,7 +77,8 @@ def test_layout_matches_the_paper_parametrisation(lib, oracle, w, h, spp, mode, 
 def test_host_bvh_builder_invariants(lib):
     """ctx == NULL builds the host tree only: every triangle in exactly one leaf, leaves <= max_leaf, boxes nested."""
     from paper_2310_07182_b200 import api
-    for scene, max_leaf in ((I.cornell(), 4), (I.interior(n_boxes=80, n_spheres=10, subdiv=2), 2), (I.landscape(n=96, n_trees=40), 8)):
+    for scene, max_leaf in ((I.cornell(), 4), (I.interior(n_boxes=80, n_spheres=10, subdiv=2), 2), (I.landscape(n=96, n_trees=40), 8),
+                            (I.cornell(), 1), (I.interior(n_boxes=80, n_spheres=10, subdiv=2), 1), (I.landscape(n=96, n_trees=40), 1)):
         v = np.ascontiguousarray(scene.verts, np.float32); m = np.ascontiguousarray(scene.mat_id, np.int32)
         pr = api.BvhParams(max_leaf, 16, 1.0, 1.0, 2)
         h = C.c_void_p()
@@ -90,6 +91,10 @@ def test_host_bvh_builder_invariants(lib):
         assert len(v) / max_leaf <= (info.n_nodes + 1) / 2 <= len(v)
         assert np.array_equal(np.array(list(info.bounds), np.float32), np.concatenate([v.reshape(-1, 3).min(0), v.reshape(-1, 3).max(0)]))
         assert info.device_bytes == 0
+        # the 8-wide compressed layout exists exactly when every leaf holds one triangle; crt_bvh_check covers its soundness too
+        assert (info.n_wide_nodes > 0) == (max_leaf == 1)
+        if max_leaf == 1:
+            assert len(v) / 8 <= info.n_wide_nodes <= len(v) and 0 < info.wide_depth <= info.depth
         lib.crt_bvh_destroy(h)
     # degenerate inputs: no triangles, one triangle, many identical triangles (centroids coincide)
     for v in (np.zeros((0, 3, 3), np.float32), I.cornell().verts[:1], np.repeat(I.cornell().verts[:1], 37, axis=0)):

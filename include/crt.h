@@ -86,7 +86,7 @@ crt_status crt_destroy(crt_ctx* ctx);
 /* Message of the last failed call on ctx (ctx may be NULL: last failure of a call that had no context). */
 const char* crt_last_error(const crt_ctx* ctx);
 /* Tunables (for experiments; defaults are what bench.py times): "trace_kernel" (0 = binary BVH, one thread per ray;
- * 1 = binary BVH, persistent warps with per-lane dynamic fetch; 2 = 8-wide compressed BVH, persistent warps -- the default), "trace_refill_threshold" (0..32: idle lanes fetch new rays when
+ * 1 = binary BVH, persistent warps with per-lane dynamic fetch -- the default; 2 = 8-wide compressed BVH, persistent warps), "trace_refill_threshold" (0..32: idle lanes fetch new rays when
  * fewer lanes than this are busy), "trace_blocks_per_sm" (0 = from the occupancy calculator). */
 crt_status crt_set_option(crt_ctx* ctx, const char* key, int64_t value);
 /* Measures the device's FP32 FFMA rate (TFLOP/s) and a streaming copy rate (GB/s) with small kernels;
@@ -96,9 +96,10 @@ crt_status crt_measure_peaks(crt_ctx* ctx, double* fp32_tflops, double* copy_gbs
 /* ---- a0: acceleration structure (D:R11) ------------------------------------------------ */
 /* Builds a binary BVH (binned surface-area heuristic, leaves <= max_leaf triangles) on the host with
  * n_threads threads and uploads it in the traversal layouts: the binary 64-byte-node layout always, and, when
- * max_leaf == 1, its collapse into 8-wide compressed 128-byte nodes, which the default traversal kernel reads.
+ * max_leaf == 1, its collapse into 8-wide compressed 128-byte nodes (read by trace_kernel 2; measured slower than the
+ * binary layout on both bench workloads, profiles/r01b, so not the default).
  * verts: [host|device] float[n_tris][3][3]; mat_id: [host|device] int32[n_tris].  Synchronous.  params may be
- * NULL (defaults: max_leaf 1, 16 bins, costs 1/1, all hardware threads).  With ctx == NULL only the host tree is built (for crt_bvh_check /
+ * NULL (defaults: max_leaf 4, 16 bins, costs 1/1, all hardware threads).  With ctx == NULL only the host tree is built (for crt_bvh_check /
  * crt_bvh_get_info; such a BVH is rejected by the device calls with CRT_ERR_STATE). */
 crt_status crt_build_bvh(crt_ctx* ctx, const float* verts, const int32_t* mat_id, int64_t n_tris,
                          const crt_bvh_params* params, crt_bvh** out);

@@ -13,7 +13,7 @@ struct crt_ctx {
     int n_sms = 0;
     std::string last_error;
     // options
-    int trace_kernel = 2;        // 0: binary BVH, one thread per ray; 1: binary BVH, persistent warps; 2: 8-wide compressed BVH, persistent warps (falls back to 1 when the BVH has no wide layout)
+    int trace_kernel = 1;        // 0: binary BVH, one thread per ray; 1 (default): binary BVH, persistent warps; 2: 8-wide compressed BVH, persistent warps (needs max_leaf == 1; else falls back to 1)
     int trace_refill_threshold = 20;   // idle lanes refetch when fewer than this many lanes of the warp are busy
     int trace_leaf_wait = 3;           // leave the inner-node phase when at most this many converged lanes still lack a leaf
     int trace_tri_wait = 8;            // wide kernel: a warp enters its triangle phase when at least this many lanes hold triangle hits

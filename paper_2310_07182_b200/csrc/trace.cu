@@ -101,8 +101,11 @@ CRT_DEV void visit_leaf(const GpuTri* __restrict__ tris, int ref, RayState& r, u
     const int leaf = ~ref;
     const int first = leaf >> 3, cnt = (leaf & 7) + 1;
     for (int j = 0; j < cnt; ++j) {
-        const float4* tp = reinterpret_cast<const float4*>(tris + first + j);
-        const float4 a = __ldg(tp), b = __ldg(tp + 1), c = __ldg(tp + 2);
+        // 64-byte record = two 256-bit loads: v0 | prim | e1 | 0, e2 | 0 | pad
+        const char* tp = reinterpret_cast<const char*>(tris + first + j);
+        const ChildRegs q0 = load_child(tp); float4 c;
+        asm volatile("ld.global.nc.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(c.x), "=f"(c.y), "=f"(c.z), "=f"(c.w) : "l"(tp + 32));
+        const float4 a = make_float4(q0.min_x, q0.max_x, q0.min_y, q0.max_y), b = make_float4(q0.min_z, q0.max_z, __int_as_float(q0.ref), 0.f);
         float t, u, v;
         if (COUNT) ++n_tris;
         if (tri_test(mk(a.x, a.y, a.z), mk(b.x, b.y, b.z), mk(c.x, c.y, c.z), r.o, r.d, r.tmin, r.tmax, t, u, v)) {

@@ -37,14 +37,57 @@ SCENES = {
 }
 
 
+# ------------------------------------------------------------------ full size, in the launch configuration bench.py times
+def test_full_size_config2_stagewise_and_sampled(crt, ctx, oracle):
+    """BASELINE config 2 at full size (1,024,704 triangles, 1920x1080, direct_reuse 4x4 stride 4): the partition covers every
+    pixel exactly once; generation fed the GPU's own primary hits equals the oracle's generation on the same buffers
+    (integer maps bit-exact, rays bit-identical); sampled primary and secondary hits equal the all-triangles definition."""
+    scene = I.interior(seed=1).with_camera(1920, 1080)
+    G = GpuScene(crt, scene, ctx)
+    w, h, spp, gw, gh, s = 1920, 1080, 1, 4, 4, 4
+    fr = crt.make_frame(w, h, spp, 1, 3); ofr = oracle.frame(w, h, spp, 1, 3)
+    order = crt.make_order("direct_reuse", gw, gh, s)
+    n_paths, n_slots, n_groups = crt.crt_layout(fr, order)
+    assert (n_paths, n_slots, n_groups) == (2073600, 2088960, 130560)
+    rays0, hits0, r2p0 = ctx.crt_trace_primary(G.bvh, G.camera, fr, order)
+    r2p = r2p0.cpu().numpy()
+    assert np.array_equal(np.sort(r2p[r2p >= 0]), np.arange(n_paths))            # exact cover
+    assert np.array_equal(r2p, oracle.partition(ofr, 2, gw, gh, s))
+    import torch
+    paths = ctx.empty((n_paths, 8)); ctx.crt_paths_init(paths)
+    accum = torch.zeros((h, w, 3), device=ctx.device)
+    ctx.crt_shade_accumulate(G.bvh, G.mats, fr, 0, False, rays0, hits0, r2p0, paths, accum)
+    paths_before = paths_np(oracle, paths).copy()
+    out = ctx.crt_generate_secondary(G.bvh, G.mats, fr, 1, order, rays0, hits0, r2p0, paths)
+    bounds = np.asarray(G.bvh.info()["bounds"], np.float32)
+    g = oracle.generate_secondary(scene, ofr, 1, 2, gw, gh, s, bounds, rays_np(oracle, rays0), hits_np(oracle, hits0), r2p, paths_before)
+    for k in ("ray_to_path", "group_id", "dir_src", "group_class"):
+        assert np.array_equal(out[k].cpu().numpy(), g[k]), k
+    assert int(out["n_active"].cpu().numpy().view(np.uint32)[0]) == g["n_active"] > 1500000
+    assert set(np.unique(g["group_class"])) == {0, 1, 2, 3}                      # empty, diffuse, glossy and hybrid groups all occur
+    rg = rays_np(oracle, out["rays"])
+    assert rg.tobytes() == g["rays"].tobytes()
+    hits1 = ctx.crt_trace(G.bvh, out["rays"])
+    rng = np.random.default_rng(11)
+    for rays_dev, hits_dev, n_s in ((rays0, hits0, 120), (out["rays"], hits1, 360)):
+        r = rays_np(oracle, rays_dev); hh = hits_np(oracle, hits_dev)
+        act = np.flatnonzero(r["tmax"] >= 0)
+        pick = rng.choice(act, n_s, replace=False)
+        compare_hits(hh[pick], oracle.trace_brute(scene.verts, r[pick]))
+    inact = rays_np(oracle, out["rays"])["tmax"] < 0
+    assert np.all(hits_np(oracle, hits1)["prim"][inact] == -1)
+
+
 # ------------------------------------------------------------------ a0 / a5: BVH + traversal
 @pytest.mark.parametrize("scene_name", ["cornell", "interior_small"])
-@pytest.mark.parametrize("kernel", [0, 1])
+@pytest.mark.parametrize("kernel", [0, 1, 2])
 def test_trace_matches_oracle_on_random_rays(crt, ctx, oracle, scene_name, kernel):
     scene = SCENES[scene_name]()
-    G = GpuScene(crt, scene, ctx)
+    # kernel 2 reads the 8-wide compressed layout, which exists when every leaf holds one triangle
+    G = GpuScene(crt, scene, ctx, **({"max_leaf": 1} if kernel == 2 else {}))
     assert G.bvh.check() == 0
     info = G.bvh.info()
+    assert (info["n_wide_nodes"] > 0) == (kernel == 2)
     assert info["n_tris"] == scene.n_tris
     ob = oracle.Bvh(scene.verts)
     assert np.array_equal(info["bounds"], ob.info()["bounds"])

@@ -1,8 +1,8 @@
-// a0 (part): collapses the binary SAH tree (max_leaf = 1) into the 8-wide compressed layout that the default traversal
-// kernel reads.  The paper leaves the acceleration structure open (D:R11); the result
+// a0 (part): collapses the binary SAH tree (max_leaf = 1) into the 8-wide compressed layout that the alternative traversal
+// kernel (trace_kernel = 2, trace_wide.cu) reads.  The paper leaves the acceleration structure open (D:R11); the result
 // of crt_trace does not depend on it (D:R10), so this layout is purely a B200 design choice: the traversal kernel is bound
-// by L1 wavefronts (one per lane and load instruction when lanes diverge, profiles/r01a), and a 128-byte node that holds
-// eight child boxes costs four wavefronts where four binary nodes cost eight.
+// by the L1 data pipe (profiles/r01a), and a 128-byte node that holds eight child boxes is one dependent fetch where the
+// binary layout needs several.  Measured result: profiles/r01b.
 //
 // WNode (128 bytes, four 32-byte sectors, each fetched by one 256-bit load):
 //   sector 0: p.xyz (box origin), E.x (fp32 power of two), E.y | E.z (bf16 halves), child_base, tri_base, imask | lmask << 8

@@ -1,12 +1,13 @@
-// a5 (default kernel): traversal of the 8-wide compressed BVH (layout: bvh_wide.cpp).
+// a5 (alternative kernel, trace_kernel = 2): traversal of the 8-wide compressed BVH (layout: bvh_wide.cpp).
 // intersection is "the most time-consuming segment" and divergent rays "lead to cache misses".
 //
-// Why this shape on B200 (profiles/r01a -> r01b): the binary-BVH kernel was bound by the L1 data pipe -- a divergent warp
-// pays one L1 wavefront per lane and load instruction, and it issued 2 loads per 2 boxes plus 3 per triangle.  Here one
-// node visit fetches EIGHT child boxes with four 256-bit loads (ld.global.nc.v8: LDG.E.ENL2.256), leaves are single
-// triangles whose box is one of those eight (so most triangles are rejected without touching their 64-byte record, which
-// is two 256-bit loads), and planes are bf16 offsets decoded on the FMA pipe (a shift by IMAD for low halves, nothing for
-// high halves) because the ALU pipe (min/max, select, compare) is the next limiter.
+// Why it exists (profiles/r01a): the binary-BVH kernel is bound by the L1 data pipe, so this kernel fetches EIGHT child boxes
+// per node visit with four 256-bit loads (ld.global.nc.v8: LDG.E.ENL2.256); leaves are single triangles whose box is one of
+// those eight (most triangles are rejected without touching their 64-byte record), and planes are bf16 offsets decoded on
+// the FMA pipe (a shift by IMAD for low halves, nothing for high halves) because the ALU pipe is the next limiter.
+// What was measured (profiles/r01b): it halves the dependent fetches (23 node visits against 54) but tests 1.7x as many boxes
+// at the same 16 bytes per box, so it ties with the binary kernel on the interior scene and loses on coherent rays and on the
+// landscape; the binary kernel (trace.cu) therefore stays the default and this one is kept, parity-tested, for comparison.
 //  - persistent warps, per-lane dynamic ray fetch in slot order (the order the generator made coherent), as in trace.cu;
 //  - hit children are kept as bit groups (no per-child stack entries, no distance sort): inner hits are visited in the
 //    order of descending (slot XOR octinv) via a 2 KB shared-memory table; the stack holds one 8-byte group per level;

@@ -42,7 +42,11 @@ FLOP_PER_NODE_VISIT, FLOP_PER_TRI_TEST, FLOP_PER_RAY = 26.0, 46.0, 3.0
 FP32_PEAK_TFLOPS_NOMINAL = 148 * 128 * 2 * 1.965e9 / 1e12
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the secondary trace kernel, from profiles/ (ncu --set full);
 # keyed by workload; None until captured.
-TRACE_DRAM_TRAFFIC = {"interior": None, "landscape": None, "cornell": None}
+TRACE_DRAM_TRAFFIC = {"interior": 121.6e6, "landscape": None, "cornell": None}     # profiles/r01a_trace_interior_full.md (mean of the two captured launches)
+# what ncu shows to be the kernel's limiter (not modelled by the two-term roofline): profiles/r01a, r01b
+TRACE_LIMITER = {"interior": {"unit": "l1tex data pipe", "l1tex__data_pipe_lsu_wavefronts_pct_of_peak": 77.0, "issue_slots_busy_pct": 65.0,
+                              "active_threads_per_warp_instruction": 14.1, "alu_pipe_pct": 50.0, "fma_pipe_pct": 26.0, "dram_pct": 1.5,
+                              "source": "profiles/r01a_trace_interior_full.md"}}
 
 
 def _peaks():
@@ -260,13 +264,14 @@ def run_cuda(args):
     rays_per_launch = act / launches
     bound_alu = FP32_PEAK_TFLOPS_NOMINAL * 1e12 / (flop_per_launch / rays_per_launch) / 1e6         # MRay/s
     bound_hbm = (hbm_gbs * 1e9 / (traffic / rays_per_launch) / 1e6) if traffic else None
-    roofline = {"bound": "alu", "kernel": "trace_persistent_kernel (secondary rays, direct_reuse)", "achieved": achieved, "peak": FP32_PEAK_TFLOPS_NOMINAL,
+    roofline = {"bound": "alu", "kernel": "trace_dyn_kernel<0> (crt_trace, secondary rays in direct_reuse order)", "achieved": achieved, "peak": FP32_PEAK_TFLOPS_NOMINAL,
                 "unit": "TFLOP/s", "frac": achieved / FP32_PEAK_TFLOPS_NOMINAL, "traffic": traffic,
                 "peak_source": "nominal 148 SM x 128 lanes x 2 x 1.965 GHz (guide); measured FFMA loop in this run: %.1f TFLOP/s" % ffma_tflops,
                 "flop_per_ray": flop_per_launch / rays_per_launch, "node_visits_per_ray": nn / max(act, 1), "tri_tests_per_ray": nt / max(act, 1),
                 "rays_per_launch": rays_per_launch, "launch_ms": dr["trace_launch_ms"],
                 "mray_s_bound_alu": bound_alu, "mray_s_bound_hbm": bound_hbm, "hbm_peak_gbs": hbm_gbs, "hbm_peak_source": hbm_src,
-                "copy_gbs_this_run": copy_gbs, "frac_of_min_bound": dr["trace_only_mray_s"] / min(bound_alu, bound_hbm or bound_alu)}
+                "copy_gbs_this_run": copy_gbs, "frac_of_min_bound": dr["trace_only_mray_s"] / min(bound_alu, bound_hbm or bound_alu),
+                "limiter": TRACE_LIMITER.get(args.workload)}
 
     if rank != 0:
         return

@@ -296,6 +296,57 @@ def run_cuda(args):
     print(json.dumps(line))
 
 
+def run_sweep(args):
+    """BASELINE config 3: interior scene at 3840x2160, 4 spp, 3 bounces; group size {2,4,8}^2 x stride {1,2,4,8} plus independent.
+    Per point: secondary MRay/s over `--sweep-frames` frames and the RMSE of their mean image against (a) the mean of the same number
+    of independent-sampling frames and (b) a longer independent reference (4x the frames).  One JSON line ("sweep": [...]).
+    Warp execution efficiency and L2 hit rate come from ncu (profiles/), not from this run."""
+    import torch
+    import paper_2310_07182_b200 as crt
+    ctx = crt.Context(0)
+    import crt_inputs as I
+    sc = max(1, args.sweep_scale)
+    w, h, spp, nb, seed = 3840 // sc, 2160 // sc, 4, 3, 1
+    scene = I.by_name("interior", seed=1).with_camera(w, h)
+    bvh = ctx.crt_build_bvh(scene.verts, scene.mat_id)
+    mats_dev = ctx.upload(scene.materials); mats = ctx.scene_mats(mats_dev, len(scene.materials), scene.env)
+    cam = crt.make_camera(scene.camera)
+    F = args.sweep_frames
+
+    def render(mode, g, s, frames, first_frame):
+        order = crt.make_order(mode, g, g, s)
+        fr0 = crt.make_frame(w, h, spp)
+        ws = ctx.frame_workspace(fr0, order)
+        accum = torch.zeros((h, w, 3), device=ctx.device)
+        nsec = torch.zeros((frames, nb), dtype=torch.int32, device=ctx.device)
+        stage = np.zeros(8, np.float32)
+        for i in range(2):                                        # warm-up on frames outside the accumulated range
+            ctx.crt_render_frame(bvh, mats, cam, crt.make_frame(w, h, spp, seed, 1000000 + i), order, nb, torch.zeros_like(accum), ws)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize(); e0.record()
+        for i in range(frames):
+            ctx.crt_render_frame(bvh, mats, cam, crt.make_frame(w, h, spp, seed, first_frame + i), order, nb, accum, ws, n_secondary=nsec[i], record_times=True)
+            ctx.crt_frame_times(stage)
+        e1.record(); torch.cuda.synchronize()
+        rays = int(nsec.sum().item()); ms = e0.elapsed_time(e1)
+        del ws
+        return accum / frames, {"mray_s": rays / (ms * 1e-3) / 1e6, "secondary_loop_mray_s": rays / (float(stage[2] + stage[3]) * 1e-3) / 1e6,
+                                "trace_only_mray_s": rays / (float(stage[3]) * 1e-3) / 1e6, "ms_per_frame": ms / frames}
+
+    def rmse(a, b):
+        return float(torch.sqrt(torch.mean((a.double() - b.double()) ** 2)).item())
+
+    ref, _ = render("independent", 1, 1, 4 * F, 500000)           # disjoint frame range: independent of every sweep point
+    ind, ind_t = render("independent", 1, 1, F, 0)
+    points = [dict(mode="independent", group=1, stride=1, **ind_t, rmse_vs_reference=rmse(ind, ref), rmse_vs_independent=0.0)]
+    for g in (2, 4, 8):
+        for s in (1, 2, 4, 8):
+            img, t = render("direct_reuse", g, s, F, 0)
+            points.append(dict(mode="direct_reuse", group=g, stride=s, **t, rmse_vs_reference=rmse(img, ref), rmse_vs_independent=rmse(img, ind)))
+    print(json.dumps({"sweep": points, "config": {"workload": f"BASELINE config 3: interior scene {w}x{h}, {spp} spp, {nb} bounces", "frames": F,
+                                                  "reference_frames": 4 * F, "scale": sc}}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -304,10 +355,15 @@ def main():
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--workload", default="interior", choices=sorted(WORKLOADS))
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sweep", action="store_true", help="BASELINE config 3 sweep instead of the bench line")
+    ap.add_argument("--sweep-frames", type=int, default=64)
+    ap.add_argument("--sweep-scale", type=int, default=1, help="divide the 3840x2160 image by this (quick runs)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "cuda":
         args.warmup = 3
-    if args.impl == "reference":
+    if args.sweep:
+        run_sweep(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_cuda(args)

@@ -59,7 +59,8 @@ typedef struct { float tr, tg, tb; uint32_t flags; float lr, lg, lb; uint32_t pa
 typedef struct { float albedo[3]; float roughness; float emission[3]; int32_t type; } orc_material;
 typedef struct { int32_t w, h, spp, seed, frame; } orc_frame;
 enum { MAT_DIFFUSE = 0, MAT_GLOSSY = 1, MAT_SPECULAR = 2, MAT_EMISSIVE = 3 };
-enum { MODE_INDEPENDENT = 0, MODE_MORTON = 1, MODE_REUSE = 2 };
+enum { MODE_INDEPENDENT = 0, MODE_MORTON = 1, MODE_REUSE = 2, MODE_WORLD = 3 };
+#define IS_GROUPED(m) ((m) == MODE_REUSE || (m) == MODE_WORLD)
 enum { CLASS_EMPTY = 0, CLASS_DIFFUSE = 1, CLASS_GLOSSY = 2, CLASS_HYBRID = 3 };
 enum { PURPOSE_CAMERA = 0, PURPOSE_BSDF = 1, PURPOSE_TILE = 2, PURPOSE_LEADER = 3 };
 #define PATH_ALIVE 1u
@@ -388,7 +389,7 @@ static layout make_layout(const orc_frame* f, int mode, int gw, int gh, int s)
 {
     layout L; memset(&L, 0, sizeof L);
     L.n_paths = (int64_t)f->spp * f->w * f->h;
-    if (mode != MODE_REUSE) { L.W = L.H = L.M = L.K = L.G = 1; L.tiles_x = f->w; L.tiles_y = f->h; L.n_tiles = f->w * f->h; L.n_slots = L.n_paths; return L; }
+    if (!IS_GROUPED(mode)) { L.W = L.H = L.M = L.K = L.G = 1; L.tiles_x = f->w; L.tiles_y = f->h; L.n_tiles = f->w * f->h; L.n_slots = L.n_paths; return L; }
     L.W = gw * s; L.H = gh * s; L.M = L.W * L.H; L.K = gw * gh; L.G = L.M / L.K;
     L.tiles_x = (f->w + L.W - 1) / L.W; L.tiles_y = (f->h + L.H - 1) / L.H; L.n_tiles = L.tiles_x * L.tiles_y;
     L.n_slots = (int64_t)f->spp * L.n_tiles * L.M;
@@ -409,7 +410,7 @@ static void tile_lcg(const orc_frame* f, const layout* L, int32_t tile, int32_t 
 /* path id p = (sample*h + y)*w + x.  Fills path_of_slot[n_slots] (-1: out-of-image slot). */
 static void partition(const orc_frame* f, const layout* L, int mode, int32_t* path_of_slot)
 {
-    if (mode != MODE_REUSE) { for (int64_t p = 0; p < L->n_paths; ++p) path_of_slot[p] = (int32_t)p; return; }
+    if (!IS_GROUPED(mode)) { for (int64_t p = 0; p < L->n_paths; ++p) path_of_slot[p] = (int32_t)p; return; }
     for (int64_t i = 0; i < L->n_slots; ++i) path_of_slot[i] = -1;
     for (int32_t sg = 0; sg < f->spp; ++sg)
         for (int32_t tile = 0; tile < L->n_tiles; ++tile) {
@@ -472,6 +473,7 @@ typedef struct {
     real albedo[3], rough;
     /* filled by the group rules */
     int has_dir; vec3 wi; real weight[3]; int32_t dir_src;
+    int has_wdir; vec3 wdir;   /* world-space reuse: the shared world direction, used as is */
 } shadept;
 
 static vec3 to_local(const shadept* s, vec3 w) { return v3(vdot(w, s->tx), vdot(w, s->ty), vdot(w, s->ng)); }
@@ -560,6 +562,22 @@ static int sample_ggx(const shadept* s, real u1, real u2, vec3* wi, real weight[
     for (int k = 0; k < 3; ++k) weight[k] = (s->albedo[k] + (R(1.0) - s->albedo[k]) * c5) * g1;
     return 1;
 }
+/* GGX weight of a GIVEN exit direction wi (wi.z > 0) under the member's own material: the same F * G1(wi) as when the
+ * direction was sampled from the visible normals, with h = normalize(wo + wi) ("calculating the probability based on the
+ * direction and their respective materials").  Returns 0 if wo + wi vanishes. */
+static int ggx_weight(const shadept* s, vec3 wi, real weight[3])
+{
+    vec3 h = v3(s->wo.x + wi.x, s->wo.y + wi.y, s->wo.z + wi.z);
+    real hl = rsqrt_(vdot(h, h));
+    if (!(hl > R(0.0))) return 0;
+    h = v3(h.x / hl, h.y / hl, h.z / hl);
+    real woh = vdot(s->wo, h);
+    real g1 = smith_g1(wi, s->rough);
+    real c1 = R(1.0) - woh; if (c1 < R(0.0)) c1 = R(0.0);
+    real c2 = c1 * c1, c5 = (c2 * c2) * c1;
+    for (int k = 0; k < 3; ++k) weight[k] = (s->albedo[k] + (R(1.0) - s->albedo[k]) * c5) * g1;
+    return 1;
+}
 /* a glossy or specular member samples from its own stream ("undergo no processing") */
 static void sample_own_glossy(const orc_frame* f, int32_t bounce, shadept* s, int32_t path)
 {
@@ -641,7 +659,7 @@ void orc_generate_secondary(const float* verts, const int32_t* mat_id, const orc
     }
     /* 2. slot layout of this mode; the partition is per (tile, sample, frame), the same at every bounce (D:R4) */
     int32_t* path_of_slot = (int32_t*)malloc(sizeof(int32_t) * (size_t)L.n_slots);
-    partition(f, &L, mode == MODE_REUSE ? MODE_REUSE : MODE_INDEPENDENT, path_of_slot);
+    partition(f, &L, IS_GROUPED(mode) ? MODE_REUSE : MODE_INDEPENDENT, path_of_slot);
     /* 3. group rules */
     for (int64_t g = 0; g < n_groups; ++g) {
         int64_t base = g * L.K;
@@ -654,6 +672,44 @@ void orc_generate_secondary(const float* verts, const int32_t* mat_id, const orc
         int cls = (n_diff + n_gloss == 0) ? CLASS_EMPTY : (n_gloss == 0 ? CLASS_DIFFUSE : (n_diff == 0 ? CLASS_GLOSSY : CLASS_HYBRID));
         group_class_out[g] = (uint8_t)cls;
         if (cls == CLASS_EMPTY) continue;
+        if (mode == MODE_WORLD) {
+            /* "Direct Direction Reusing" in WORLD space (section 3.1; DESIGN.md D:R18): one randomly selected pixel of the
+             * group samples a direction from its own BSDF; the other rays reuse it in world space and weight it with their
+             * own material.  A direction below a member's horizon ends that path (the artifact of Fig. 1).  Mirror
+             * members cannot evaluate an arbitrary direction (delta lobe) and keep their own reflection. */
+            uint32_t r[4];
+            int32_t sample = (int32_t)(g / ((int64_t)L.n_tiles * L.G));
+            orc_philox((uint32_t)g, (uint32_t)sample, (uint32_t)bounce, PURPOSE_LEADER, (uint32_t)f->seed, (uint32_t)f->frame, r);
+            int j0 = (int)(r[0] % (uint32_t)L.K); int32_t leader = -1;
+            for (int t = 0; t < L.K && leader < 0; ++t) {
+                int32_t p = path_of_slot[base + (j0 + t) % L.K];
+                if (p >= 0 && sp[p].live) leader = p;
+            }
+            /* every live member first takes its own independent sample (the leader's is the shared one; the others keep
+             * theirs only if they are mirrors or the leader's sample is invalid) */
+            for (int j = 0; j < L.K; ++j) {
+                int32_t p = path_of_slot[base + j];
+                if (p < 0 || !sp[p].live) continue;
+                if (sp[p].mtype == MAT_DIFFUSE) {
+                    real u1, u2; bsdf_uniforms(f, sp[p].pixel, sp[p].sample, bounce, &u1, &u2);
+                    sp[p].wi = sample_cosine(u1, u2); sp[p].has_dir = 1; sp[p].dir_src = p;
+                    for (int k = 0; k < 3; ++k) sp[p].weight[k] = sp[p].albedo[k];
+                } else sample_own_glossy(f, bounce, &sp[p], p);
+            }
+            if (!sp[leader].has_dir) continue;
+            vec3 wd = to_world(&sp[leader], sp[leader].wi);
+            for (int j = 0; j < L.K; ++j) {
+                int32_t p = path_of_slot[base + j];
+                if (p < 0 || !sp[p].live || p == leader || sp[p].mtype == MAT_SPECULAR) continue;
+                vec3 wl = to_local(&sp[p], wd);
+                sp[p].dir_src = leader;
+                if (!(wl.z > R(0.0))) { sp[p].has_dir = 0; continue; }
+                sp[p].wi = wl; sp[p].has_wdir = 1; sp[p].wdir = wd; sp[p].has_dir = 1;
+                if (sp[p].mtype == MAT_DIFFUSE) { for (int k = 0; k < 3; ++k) sp[p].weight[k] = sp[p].albedo[k]; }
+                else sp[p].has_dir = ggx_weight(&sp[p], wl, sp[p].weight);
+            }
+            continue;
+        }
         /* glossy / specular members: untouched, in glossy AND hybrid groups */
         vec3 sum = v3(R(0.0), R(0.0), R(0.0)); int n_valid = 0;
         for (int j = 0; j < L.K; ++j) {
@@ -707,11 +763,11 @@ void orc_generate_secondary(const float* verts, const int32_t* mat_id, const orc
         int32_t p = path_of_slot[i];
         tmp_r2p[i] = p; tmp_src[i] = -1; inactive_ray(&tmp_rays[i]);
         if (tmp_loc) tmp_loc[3 * i] = tmp_loc[3 * i + 1] = tmp_loc[3 * i + 2] = 0.f;
-        if (mode == MODE_REUSE) group_id_out[i] = (int32_t)(i / L.K);
+        if (IS_GROUPED(mode)) group_id_out[i] = (int32_t)(i / L.K);
         if (p < 0 || !sp[p].live) continue;
         shadept* q = &sp[p];
         if (!q->has_dir) { paths[p].flags &= ~PATH_ALIVE; continue; }       /* invalid glossy sample: path ends */
-        vec3 wd = to_world(q, q->wi);
+        vec3 wd = q->has_wdir ? q->wdir : to_world(q, q->wi);
         real mx = rmax_(rabs_(q->p.x), rmax_(rabs_(q->p.y), rabs_(q->p.z)));
         real off = R(1.0 / 32768.0) * (R(1.0) + mx);                        /* self-intersection offset (D:R7) */
         orc_ray* o = &tmp_rays[i];
@@ -734,7 +790,7 @@ void orc_generate_secondary(const float* verts, const int32_t* mat_id, const orc
         }
         free(keys); free(order); free(tmp_rays); free(tmp_r2p); free(tmp_src); free(tmp_loc);
     }
-    if (mode != MODE_REUSE) for (int64_t j = 0; j < L.n_slots; ++j) group_id_out[j] = ray_to_path_out[j];
+    if (!IS_GROUPED(mode)) for (int64_t j = 0; j < L.n_slots; ++j) group_id_out[j] = ray_to_path_out[j];
     *n_active_out = n_active;
     free(path_of_slot); free(sp);
 }

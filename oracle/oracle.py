@@ -18,7 +18,7 @@ RAY_DTYPE = np.dtype([("o", "<f4", 3), ("tmin", "<f4"), ("d", "<f4", 3), ("tmax"
 HIT_DTYPE = np.dtype([("t", "<f4"), ("u", "<f4"), ("v", "<f4"), ("prim", "<i4")])
 PATH_DTYPE = np.dtype([("T", "<f4", 3), ("flags", "<u4"), ("L", "<f4", 3), ("pad", "<u4")])
 MODE_INDEPENDENT, MODE_MORTON, MODE_REUSE = 0, 1, 2
-MODES = {"independent": 0, "morton_reorder": 1, "direct_reuse": 2}
+MODES = {"independent": 0, "morton_reorder": 1, "direct_reuse": 2, "world_reuse": 3}
 CLASS_EMPTY, CLASS_DIFFUSE, CLASS_GLOSSY, CLASS_HYBRID = 0, 1, 2, 3
 
 

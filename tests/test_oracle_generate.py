@@ -8,7 +8,7 @@ import pytest
 
 import crt_inputs as I
 
-M_IND, M_MOR, M_REUSE = 0, 1, 2
+M_IND, M_MOR, M_REUSE, M_WORLD = 0, 1, 2, 3
 
 
 # ------------------------------------------------------------------ partition
@@ -276,6 +276,66 @@ def test_ggx_half_vectors_follow_the_visible_normal_distribution(oracle, alpha, 
     for f in (lambda h: h[..., 0], lambda h: h[..., 1], lambda h: h[..., 2], lambda h: h[..., 2] ** 2, lambda h: h[..., 0] * h[..., 1]):
         assert abs(f(hs).mean() - (f(H) * pdf).sum()) < 4e-3
     assert np.mean(wts) <= 1.0                                       # white furnace: energy never gained
+
+
+# ------------------------------------------------------------------ world-space reuse (section 3.1; DESIGN.md D:R18)
+def test_world_space_reuse_rules(oracle):
+    """The paper's first variant: the group shares one WORLD direction.  On a plane it coincides with tangent-space reuse;
+    on curved / mixed geometry the shared direction is bit-identical across the reusing members, equals the selected
+    pixel's own (independent) ray, never leaves a member's upper hemisphere (such members end), and mirrors are untouched."""
+    flat_t = _first_bounce(oracle, I.floor_plane(I.MAT_DIFFUSE), M_REUSE)
+    flat_w = _first_bounce(oracle, I.floor_plane(I.MAT_DIFFUSE), M_WORLD)
+    assert flat_w["rays"].tobytes() == flat_t["rays"].tobytes() and np.array_equal(flat_w["dir_src"], flat_t["dir_src"])
+    n_dead_total = 0
+    for sc in (I.cornell(), I.interior(n_boxes=40, n_spheres=10, subdiv=2, width=48, height=32), I.checker_floor()):
+        g = _first_bounce(oracle, sc, M_WORLD); gi = _first_bounce(oracle, sc, M_IND); gt = _first_bounce(oracle, sc, M_REUSE)
+        K = 16
+        assert np.array_equal(g["ray_to_path"], gt["ray_to_path"]) and np.array_equal(g["group_class"], gt["group_class"])   # same partition and census
+        act = g["rays"]["tmax"] >= 0
+        p = g["ray_to_path"]; src = g["dir_src"]
+        prev_slot_of_path = np.full(sc.width * sc.height, -1, np.int64); ok = g["prev_r2p"] >= 0
+        prev_slot_of_path[g["prev_r2p"][ok]] = np.nonzero(ok)[0]
+        ps = prev_slot_of_path[np.maximum(p, 0)]
+        mtype = np.where(p >= 0, sc.materials["type"][sc.mat_id[np.maximum(g["prev_hits"]["prim"][ps], 0)]], -1)
+        # upper hemisphere for every emitted ray
+        n = _normals(sc, g["prev_hits"]["prim"][ps[act]], g["prev_rays"]["d"][ps[act]].astype(np.float64))
+        assert np.all((g["rays"]["d"][act].astype(np.float64) * n).sum(1) > 0)
+        reuse = act & (src != p)
+        assert reuse.sum() > 100
+        # a reusing member's direction is bit-identical to its leader's independent-mode ray direction
+        assert np.array_equal(g["rays"]["d"][reuse], gi["rays"]["d"][src[reuse]])
+        assert np.all(mtype[reuse] != I.MAT_SPECULAR)
+        # own-sampling members (leaders, mirrors): exactly their independent ray
+        own = act & (src == p)
+        assert np.array_equal(g["rays"][own], gi["rays"][p[own]])
+        spec = act & (mtype == I.MAT_SPECULAR)
+        assert np.all(src[spec] == p[spec])
+        # one leader per group among the reusing members
+        for gidx in np.unique(np.nonzero(reuse)[0] // K)[:200]:
+            sl = slice(gidx * K, (gidx + 1) * K)
+            leaders = np.unique(src[sl][reuse[sl]])
+            assert len(leaders) == 1 and leaders[0] in p[sl]
+        # paths that were alive with a hit but emitted no ray: ended because the shared direction was below their horizon
+        alive_before = (g["prev_hits"]["prim"][ps] >= 0) & (p >= 0)
+        n_dead_total += int((alive_before & ~act).sum()) - int(((gi["rays"]["tmax"] < 0)[np.maximum(p, 0)] & alive_before).sum())
+    assert n_dead_total > 50            # the artifact of Fig. 1 exists on non-planar scenes ...
+    assert flat_w["n_active"] == flat_t["n_active"]          # ... and not on a plane
+
+
+def test_world_space_reuse_is_biased_on_curved_geometry_but_exact_on_a_plane(oracle):
+    """Furnace: white Lambert under uniform light.  On a floor every direction is valid for every member -> exactly 1;
+    on a sphere members whose normal faces away from the shared direction end -> darker than 1."""
+    def image(sc, mode):
+        fr = oracle.frame(sc.width, sc.height, 1, 0, 0)
+        acc, _, _ = oracle.render_frame(oracle.Bvh(sc.verts), sc, fr, 1, mode, 4, 4, 8)      # tile 32x32: members all over the sphere
+        return acc
+    floor = I.floor_plane(I.MAT_DIFFUSE, albedo=1.0)
+    assert np.all(image(floor, M_WORLD) == 1.0)
+    sph = I.furnace_sphere()
+    hit = image(sph, M_REUSE)
+    assert np.all(hit == 1.0)
+    w = image(sph, M_WORLD)
+    assert w.max() == 1.0 and 0.5 < w.mean() < 0.99 and set(np.unique(w)) == {0.0, 1.0}
 
 
 # ------------------------------------------------------------------ Morton code + sort (P:L43)

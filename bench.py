@@ -238,6 +238,7 @@ def run_cuda(args):
     modes["direct_reuse"] = time_mode("direct_reuse")
     modes["independent"] = time_mode("independent")
     modes["morton_reorder"] = time_mode("morton_reorder")
+    modes["world_reuse"] = time_mode("world_reuse")       # the paper's first variant, an ablation: biased, see DESIGN.md D:R18
     e2e = time_mode("direct_reuse", host=True)
     clk = clocks.stop()
 

@@ -20,7 +20,7 @@
  * Index spaces (D:R3-R5)
  *  path  p = (sample*h + y)*w + x,             n_paths = spp*w*h
  *  mode independent / morton_reorder:           n_slots = n_paths
- *  mode direct_reuse with group gw x gh and interleave stride s (all powers of two):
+ *  mode direct_reuse / world_reuse with group gw x gh and interleave stride s (all powers of two):
  *      tile W x H = (gw*s) x (gh*s), M = W*H slots per tile, K = gw*gh rays per group,
  *      slot = (sample*n_tiles + tile)*M + m,  m = (a*n + c) mod M the shuffled number of
  *      pixel n = ly*W + lx of the tile;  group = slot / K;  n_slots = spp*n_tiles*M.
@@ -44,7 +44,10 @@ typedef enum {
     CRT_ERR_NOMEM = 5
 } crt_status;
 
-typedef enum { CRT_MODE_INDEPENDENT = 0, CRT_MODE_MORTON_REORDER = 1, CRT_MODE_DIRECT_REUSE = 2 } crt_mode;
+/* CRT_MODE_WORLD_REUSE: the paper's first variant, "Direct Direction Reusing" in WORLD space (section 3.1; D:R18): same
+ * groups and slot order as CRT_MODE_DIRECT_REUSE, but the selected pixel's world direction is shared as is; members for which
+ * it lies below the horizon end (the artifact of Fig. 1).  Kept as the ablation the paper argues from, not as the method. */
+typedef enum { CRT_MODE_INDEPENDENT = 0, CRT_MODE_MORTON_REORDER = 1, CRT_MODE_DIRECT_REUSE = 2, CRT_MODE_WORLD_REUSE = 3 } crt_mode;
 typedef enum { CRT_MAT_DIFFUSE = 0, CRT_MAT_GLOSSY = 1, CRT_MAT_SPECULAR = 2, CRT_MAT_EMISSIVE = 3 } crt_mat_type;
 typedef enum { CRT_CLASS_EMPTY = 0, CRT_CLASS_DIFFUSE = 1, CRT_CLASS_GLOSSY = 2, CRT_CLASS_HYBRID = 3 } crt_group_class;
 
@@ -128,10 +131,11 @@ crt_status crt_trace_primary(crt_ctx* ctx, const crt_bvh* bvh, const crt_camera*
 /* From the previous segment (prev_* arrays in the SAME order, n_slots entries) generate the rays of bounce
  * `bounce` >= 1.  Outputs (all [device]): rays_out, ray_to_path_out, group_id_out, dir_src_out: n_slots entries;
  * group_class_out: n_groups bytes (crt_group_class); n_active_out: one uint32 (zeroed by the call, then counted).
- *   group_id_out[slot] = slot / K (direct_reuse) or the path id (other modes)
+ *   group_id_out[slot] = slot / K (direct_reuse, world_reuse) or the path id (other modes)
  *   dir_src_out[slot]  = path id whose random numbers produced the direction: own id (glossy/specular member or
  *                        independent sampling), the group leader's id (diffuse group), -2 - group (diffuse member of
- *                        a hybrid group: mean direction of the glossy members), -1 (no ray)
+ *                        a hybrid group: mean direction of the glossy members), -1 (no ray); world_reuse: the selected
+ *                        pixel's id for every member that reuses its world direction
  * paths[path].throughput is multiplied by the BSDF weight; paths whose sample is invalid are killed.
  * times may be NULL.  scratch: [device], at least crt_generate_secondary_scratch_bytes(). */
 crt_status crt_generate_secondary(crt_ctx* ctx, const crt_bvh* bvh, const crt_scene_mats* mats, const crt_frame* frame,

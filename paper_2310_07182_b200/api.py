@@ -22,7 +22,7 @@ import torch
 from . import build as _build
 
 MODE_INDEPENDENT, MODE_MORTON_REORDER, MODE_DIRECT_REUSE = 0, 1, 2
-MODES = {"independent": 0, "morton_reorder": 1, "direct_reuse": 2}
+MODES = {"independent": 0, "morton_reorder": 1, "direct_reuse": 2, "world_reuse": 3}
 CRT_OK, CRT_ERR_INVALID_ARG, CRT_ERR_UNSUPPORTED, CRT_ERR_CUDA, CRT_ERR_STATE, CRT_ERR_NOMEM = range(6)
 STATUS_NAMES = ["CRT_OK", "CRT_ERR_INVALID_ARG", "CRT_ERR_UNSUPPORTED", "CRT_ERR_CUDA", "CRT_ERR_STATE", "CRT_ERR_NOMEM"]
 

@@ -27,12 +27,12 @@ crt_status crt_make_layout(crt_ctx* ctx, const crt_frame* f, const crt_order* o,
 {
     if (!f || !o || !L) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "layout: null argument");
     if (f->w < 0 || f->h < 0 || f->spp < 1) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "layout: bad frame %dx%d spp %d", f->w, f->h, f->spp);
-    if (o->mode < 0 || o->mode > 2) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "layout: mode %d out of range", o->mode);
+    if (o->mode < 0 || o->mode > 3) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "layout: mode %d out of range", o->mode);
     memset(L, 0, sizeof *L);
     L->w = f->w; L->h = f->h; L->spp = f->spp; L->mode = o->mode;
     L->n_paths = (int64_t)f->spp * f->w * f->h;
     if (L->n_paths >= ((int64_t)1 << 31)) return crt_fail(ctx, CRT_ERR_UNSUPPORTED, "layout: more than 2^31 paths");
-    if (o->mode != CRT_MODE_DIRECT_REUSE) {
+    if (o->mode != CRT_MODE_DIRECT_REUSE && o->mode != CRT_MODE_WORLD_REUSE) {
         L->W = L->H = L->M = L->K = L->G = 1; L->tiles_x = f->w; L->tiles_y = f->h; L->n_tiles = f->w * f->h;
         L->n_slots = L->n_paths; L->n_groups = L->n_paths;
         return CRT_OK;

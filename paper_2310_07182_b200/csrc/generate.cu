@@ -64,6 +64,23 @@ CRT_DEV bool sample_ggx(V3 wo, float al, const float* albedo, float u1, float u2
     return true;
 }
 
+// GGX weight of a GIVEN exit direction (world-space reuse: "calculating the probability based on the direction and their
+// respective materials"): F * G1(wi) with h = normalize(wo + wi)
+CRT_DEV bool ggx_weight(V3 wo, V3 wi, float al, const float* albedo, float* weight)
+{
+    V3 h = mk(add(wo.x, wi.x), add(wo.y, wi.y), add(wo.z, wi.z));
+    float hl = sqr(dot(h, h));
+    if (!(hl > 0.0f)) return false;
+    h = mk(dvd(h.x, hl), dvd(h.y, hl), dvd(h.z, hl));
+    float woh = dot(wo, h);
+    float g1 = smith_g1(wi, al);
+    float c1 = sub(1.0f, woh); if (c1 < 0.0f) c1 = 0.0f;
+    float c2 = mul(c1, c1), c5 = mul(mul(c2, c2), c1);
+#pragma unroll
+    for (int k = 0; k < 3; ++k) weight[k] = mul(add(albedo[k], mul(sub(1.0f, albedo[k]), c5)), g1);
+    return true;
+}
+
 // 30-bit interleaved origin+direction code (P:L43 [AK10]; D:R12)
 CRT_DEV uint32_t quant5(float x)
 {
@@ -91,6 +108,7 @@ struct GenArgs {
     uint32_t* keys_out;      // morton mode: key per path (rays_out etc. are then the by-path temporaries)
     Bounds6 bounds;
     int64_t n_slots; int32_t bounce; int32_t morton;
+    int32_t world;           // direct_reuse in WORLD space (mode 3; D:R18)
 };
 
 enum { F_DEAD = 0, F_DIFF = 1, F_GLOSS = 2 };
@@ -165,6 +183,12 @@ __global__ void __launch_bounds__(1024) generate_kernel(GenArgs A, DevLayout L)
         }
         src = p;
     }
+    V3 wdir = mk(0.f, 0.f, 0.f); bool has_wdir = false;
+    if (REUSE && A.world && flag == F_DIFF) {          // world-space reuse: every live member first takes its own sample
+        const uint4 r = philox((uint32_t)pixel, (uint32_t)sample, (uint32_t)A.bounce, PURPOSE_BSDF, L.seed, L.frame);
+        wi = sample_cosine(u01(r.x), u01(r.y));
+        has_dir = true; src = p; weight[0] = albedo[0]; weight[1] = albedo[1]; weight[2] = albedo[2];
+    }
 
     int cls = CRT_CLASS_EMPTY;
     int64_t group = i;
@@ -172,14 +196,29 @@ __global__ void __launch_bounds__(1024) generate_kernel(GenArgs A, DevLayout L)
         // ---- 3. census of the group through shared memory
         const int K = L.K, tid = threadIdx.x, gbase = tid & ~(K - 1);
         group = i >> L.log2K;
-        s_flag[tid] = flag | ((flag == F_GLOSS && has_dir) ? 4 : 0);
+        s_flag[tid] = flag | (((A.world || flag == F_GLOSS) && has_dir) ? 4 : 0);
         s_path[tid] = p;
-        s_wi[3 * tid] = wi.x; s_wi[3 * tid + 1] = wi.y; s_wi[3 * tid + 2] = wi.z;
+        if (A.world) { const V3 w = has_dir ? to_world(fr, wi) : wi; s_wi[3 * tid] = w.x; s_wi[3 * tid + 1] = w.y; s_wi[3 * tid + 2] = w.z; }
+        else { s_wi[3 * tid] = wi.x; s_wi[3 * tid + 1] = wi.y; s_wi[3 * tid + 2] = wi.z; }
         __syncthreads();
         bool any_diff = false, any_gloss = false, any_valid = false;
         for (int j = 0; j < K; ++j) { const int f = s_flag[gbase + j]; any_diff |= (f & 3) == F_DIFF; any_gloss |= (f & 3) == F_GLOSS; any_valid |= (f & 4) != 0; }
         cls = (!any_diff && !any_gloss) ? CRT_CLASS_EMPTY : (!any_gloss ? CRT_CLASS_DIFFUSE : (!any_diff ? CRT_CLASS_GLOSSY : CRT_CLASS_HYBRID));
-        if (flag == F_DIFF) {
+        if (A.world) {
+            // one randomly selected live pixel's world direction for the whole group; mirrors keep their reflection
+            const uint4 rl = philox((uint32_t)group, (uint32_t)sample, (uint32_t)A.bounce, PURPOSE_LEADER, L.seed, L.frame);
+            const int j0 = (int)(rl.x & (uint32_t)(K - 1));
+            int lj = -1;
+            for (int t = 0; t < K; ++t) { const int j = (j0 + t) & (K - 1); if ((s_flag[gbase + j] & 3) != F_DEAD) { lj = gbase + j; break; } }
+            if (flag != F_DEAD && lj >= 0 && lj != tid && (s_flag[lj] & 4) && mtype != CRT_MAT_SPECULAR) {
+                wdir = mk(s_wi[3 * lj], s_wi[3 * lj + 1], s_wi[3 * lj + 2]);
+                wi = to_local(fr, wdir);
+                src = s_path[lj];
+                if (!(wi.z > 0.0f)) has_dir = false;                 // the shared direction is below this member's horizon (Fig. 1)
+                else if (flag == F_DIFF) { has_dir = true; has_wdir = true; weight[0] = albedo[0]; weight[1] = albedo[1]; weight[2] = albedo[2]; }
+                else { has_dir = ggx_weight(wo, wi, rough, albedo, weight); has_wdir = has_dir; }
+            }
+        } else if (flag == F_DIFF) {
             if (cls == CRT_CLASS_HYBRID && any_valid) {
                 // hybrid: mean tangent-space exit direction of the glossy/specular members, summed in slot order
                 V3 sum = mk(0.f, 0.f, 0.f);
@@ -218,7 +257,7 @@ __global__ void __launch_bounds__(1024) generate_kernel(GenArgs A, DevLayout L)
     float4 r0 = make_float4(0.f, 0.f, 0.f, 0.f), r1 = make_float4(0.f, 0.f, 0.f, -1.f);
     const bool emit = live && has_dir;
     if (emit) {
-        const V3 wd = to_world(fr, wi);
+        const V3 wd = has_wdir ? wdir : to_world(fr, wi);
         const float mx = fmaxf(fabsf(hp.x), fmaxf(fabsf(hp.y), fabsf(hp.z)));
         const float off = mul(1.0f / 32768.0f, add(1.0f, mx));
         r0 = make_float4(add(hp.x, mul(fr.ng.x, off)), add(hp.y, mul(fr.ng.y, off)), add(hp.z, mul(fr.ng.z, off)), 0.f);
@@ -306,9 +345,10 @@ crt_status launch_generate(crt_ctx* ctx, const crt_bvh* bvh, const crt_scene_mat
     A.prev_rays = prev_rays; A.prev_hits = prev_hits; A.prev_r2p = prev_r2p; A.paths = paths;
     A.rays_out = rays_out; A.r2p_out = r2p_out; A.gid_out = gid_out; A.src_out = src_out; A.cls_out = cls_out; A.n_active = n_active;
     A.keys_out = nullptr; A.bounds = make_bounds(bvh->bounds); A.n_slots = L.n_slots; A.bounce = bounce; A.morton = 0;
+    A.world = (L.mode == CRT_MODE_WORLD_REUSE);
     const DevLayout D = make_dev_layout(L, f);
     const int64_t n = L.n_slots;
-    if (L.mode == CRT_MODE_DIRECT_REUSE) {
+    if (L.mode == CRT_MODE_DIRECT_REUSE || L.mode == CRT_MODE_WORLD_REUSE) {
         const int block = L.K > 256 ? L.K : 256;
         generate_kernel<true><<<(unsigned)((n + block - 1) / block), block, (size_t)block * 20, st>>>(A, D);
         CRT_CHECK_LAUNCH(ctx, "generate<reuse>");

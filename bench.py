@@ -310,15 +310,16 @@ def run_sweep(args):
     ctx = crt.Context(0)
     import crt_inputs as I
     sc = max(1, args.sweep_scale)
-    w, h, spp, nb, seed = 3840 // sc, 2160 // sc, 4, 3, 1
+    table3 = args.sweep == "table3"
+    w, h, spp, nb, seed = (1920 // sc, 1080 // sc, 1, 2, 1) if table3 else (3840 // sc, 2160 // sc, 4, 3, 1)
     scene = I.by_name("interior", seed=1).with_camera(w, h)
     bvh = ctx.crt_build_bvh(scene.verts, scene.mat_id)
     mats_dev = ctx.upload(scene.materials); mats = ctx.scene_mats(mats_dev, len(scene.materials), scene.env)
     cam = crt.make_camera(scene.camera)
     F = args.sweep_frames
 
-    def render(mode, g, s, frames, first_frame):
-        order = crt.make_order(mode, g, g, s)
+    def render(mode, g, s, frames, first_frame, tile=None):
+        order = crt.order_for_tile(mode, *tile) if tile else crt.make_order(mode, g, g, s)
         fr0 = crt.make_frame(w, h, spp)
         ws = ctx.frame_workspace(fr0, order)
         accum = torch.zeros((h, w, 3), device=ctx.device)
@@ -343,11 +344,19 @@ def run_sweep(args):
     ref, _ = render("independent", 1, 1, 4 * F, 500000)           # disjoint frame range: independent of every sweep point
     ind, ind_t = render("independent", 1, 1, F, 0)
     points = [dict(mode="independent", group=1, stride=1, **ind_t, rmse_vs_reference=rmse(ind, ref), rmse_vs_independent=0.0)]
-    for g in (2, 4, 8):
-        for s in (1, 2, 4, 8):
-            img, t = render("direct_reuse", g, s, F, 0)
-            points.append(dict(mode="direct_reuse", group=g, stride=s, **t, rmse_vs_reference=rmse(img, ref), rmse_vs_independent=rmse(img, ind)))
-    print(json.dumps({"sweep": points, "config": {"workload": f"BASELINE config 3: interior scene {w}x{h}, {spp} spp, {nb} bounces", "frames": F,
+    if table3:      # P:L178-185 (Table 3): tile (8,8), (16,8), (16,16), (32,8) x K = 8, 16, 32, 64
+        for tw, th in ((8, 8), (16, 8), (16, 16), (32, 8)):
+            for k in (8, 16, 32, 64):
+                img, t = render("direct_reuse", 0, 0, F, 0, tile=(tw, th, k))
+                points.append(dict(mode="direct_reuse", tile=[tw, th], K=k, **t, rmse_vs_reference=rmse(img, ref), rmse_vs_independent=rmse(img, ind),
+                                   trace_speedup_vs_independent=t["trace_only_mray_s"] / ind_t["trace_only_mray_s"]))
+    else:
+        for g in (2, 4, 8):
+            for s in (1, 2, 4, 8):
+                img, t = render("direct_reuse", g, s, F, 0)
+                points.append(dict(mode="direct_reuse", group=g, stride=s, **t, rmse_vs_reference=rmse(img, ref), rmse_vs_independent=rmse(img, ind)))
+    name = "the paper's Table 3 shapes (P:L178-185)" if table3 else "BASELINE config 3"
+    print(json.dumps({"sweep": points, "config": {"workload": f"{name}: interior scene {w}x{h}, {spp} spp, {nb} bounces", "frames": F,
                                                   "reference_frames": 4 * F, "scale": sc}}))
 
 
@@ -359,7 +368,8 @@ def main():
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--workload", default="interior", choices=sorted(WORKLOADS))
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--sweep", action="store_true", help="BASELINE config 3 sweep instead of the bench line")
+    ap.add_argument("--sweep", nargs="?", const="config3", default=None, choices=["config3", "table3"],
+                    help="config3: BASELINE config 3 sweep; table3: the paper's Table 3 shapes (tile x K) at 1920x1080, 1 spp, 2 bounces")
     ap.add_argument("--sweep-frames", type=int, default=64)
     ap.add_argument("--sweep-scale", type=int, default=1, help="divide the 3840x2160 image by this (quick runs)")
     args = ap.parse_args()

@@ -65,7 +65,10 @@ typedef struct { float albedo[3]; float roughness; float emission[3]; int32_t ty
 typedef struct { int32_t w, h, spp, seed, frame; } crt_frame;
 /* pinhole camera (D:R6): a pixel at normalised screen position (sx,sy) in [-1,1]^2, sy up, looks along W + sx*U + sy*V */
 typedef struct { float eye[3], U[3], V[3], W[3]; } crt_camera;
-typedef struct { int32_t mode, group_w, group_h, stride; } crt_order;
+/* stride = horizontal interleave stride; stride_y = vertical one (0 = same as stride).  The tile is (group_w*stride) x
+ * (group_h*stride_y) and K = group_w*group_h, which expresses every power-of-two (W, H, K) of the paper's own
+ * parametrisation, e.g. tile 8x8 with K = 8 as group 8x1, stride 1, stride_y 8 (D:R5). */
+typedef struct { int32_t mode, group_w, group_h, stride, stride_y; } crt_order;
 /* materials: [device] table indexed by the per-triangle material id given to crt_build_bvh.
  * env: radiance on a miss = lerp(env[0..2], env[3..5], 0.5*(d.y+1)) (D:R14). */
 typedef struct { const crt_material* materials; int32_t n_materials; float env[6]; } crt_scene_mats;

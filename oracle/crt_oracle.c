@@ -390,7 +390,11 @@ static layout make_layout(const orc_frame* f, int mode, int gw, int gh, int s)
     layout L; memset(&L, 0, sizeof L);
     L.n_paths = (int64_t)f->spp * f->w * f->h;
     if (!IS_GROUPED(mode)) { L.W = L.H = L.M = L.K = L.G = 1; L.tiles_x = f->w; L.tiles_y = f->h; L.n_tiles = f->w * f->h; L.n_slots = L.n_paths; return L; }
-    L.W = gw * s; L.H = gh * s; L.M = L.W * L.H; L.K = gw * gh; L.G = L.M / L.K;
+    /* the paper's native parametrisation is a W x H tile and a group size K (tile 8x8, K = 8).  Any power-of-two
+     * (W, H, K) is gw = min(K, W), gh = K / gw with separate horizontal / vertical strides W / gw, H / gh; the vertical
+     * stride travels in the high 16 bits of s (0 = same as the horizontal one).  DESIGN.md D:R5. */
+    int32_t sx = s & 0xffff, sy = (s >> 16) ? (s >> 16) : sx;
+    L.W = gw * sx; L.H = gh * sy; L.M = L.W * L.H; L.K = gw * gh; L.G = L.M / L.K;
     L.tiles_x = (f->w + L.W - 1) / L.W; L.tiles_y = (f->h + L.H - 1) / L.H; L.n_tiles = L.tiles_x * L.tiles_y;
     L.n_slots = (int64_t)f->spp * L.n_tiles * L.M;
     return L;

@@ -4,6 +4,6 @@ The product is libcrt.so (C ABI in include/crt.h, CUDA kernels in csrc/); `api` 
 There is no CPU fallback: the binding raises when the library or a CUDA device is missing.
 """
 from .api import (  # noqa: F401
-    Context, Bvh, CrtError, Frame, Order, Camera, SceneMats, make_frame, make_order, make_camera, crt_layout, lib, hit_prims, path_flags,
+    Context, Bvh, CrtError, Frame, Order, Camera, SceneMats, make_frame, make_order, order_for_tile, make_camera, crt_layout, lib, hit_prims, path_flags,
     MODES, MODE_INDEPENDENT, MODE_MORTON_REORDER, MODE_DIRECT_REUSE, EXPORTS,
 )

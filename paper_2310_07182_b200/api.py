@@ -48,7 +48,7 @@ class Frame(C.Structure):
 
 
 class Order(C.Structure):
-    _fields_ = [("mode", C.c_int32), ("group_w", C.c_int32), ("group_h", C.c_int32), ("stride", C.c_int32)]
+    _fields_ = [("mode", C.c_int32), ("group_w", C.c_int32), ("group_h", C.c_int32), ("stride", C.c_int32), ("stride_y", C.c_int32)]
 
 
 class Camera(C.Structure):
@@ -114,8 +114,16 @@ def make_frame(w, h, spp=1, seed=0, frame=0):
     return Frame(int(w), int(h), int(spp), int(seed), int(frame))
 
 
-def make_order(mode, group_w=1, group_h=1, stride=1):
-    return Order(MODES[mode] if isinstance(mode, str) else int(mode), int(group_w), int(group_h), int(stride))
+def make_order(mode, group_w=1, group_h=1, stride=1, stride_y=0):
+    if int(stride) >> 16:                                  # packed form used by the tests: vertical stride in the high half
+        stride, stride_y = int(stride) & 0xffff, int(stride) >> 16
+    return Order(MODES[mode] if isinstance(mode, str) else int(mode), int(group_w), int(group_h), int(stride), int(stride_y))
+
+
+def order_for_tile(mode, tile_w, tile_h, k):
+    """The paper's native parametrisation: a tile_w x tile_h tile and groups of k rays, all powers of two."""
+    gw = min(k, tile_w); gh = k // gw
+    return make_order(mode, gw, gh, tile_w // gw, tile_h // gh)
 
 
 def make_camera(cam12):

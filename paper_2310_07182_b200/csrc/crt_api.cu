@@ -37,11 +37,12 @@ crt_status crt_make_layout(crt_ctx* ctx, const crt_frame* f, const crt_order* o,
         L->n_slots = L->n_paths; L->n_groups = L->n_paths;
         return CRT_OK;
     }
-    if (!is_pow2(o->group_w) || !is_pow2(o->group_h) || !is_pow2(o->stride))
-        return crt_fail(ctx, CRT_ERR_UNSUPPORTED, "layout: group %dx%d stride %d must be powers of two", o->group_w, o->group_h, o->stride);
-    const int64_t M = (int64_t)o->group_w * o->stride * o->group_h * o->stride, K = (int64_t)o->group_w * o->group_h;
+    const int sy = o->stride_y ? o->stride_y : o->stride;
+    if (!is_pow2(o->group_w) || !is_pow2(o->group_h) || !is_pow2(o->stride) || !is_pow2(sy) || o->stride > 4096 || sy > 4096 || o->group_w > 1024 || o->group_h > 1024)
+        return crt_fail(ctx, CRT_ERR_UNSUPPORTED, "layout: group %dx%d stride %d/%d must be powers of two", o->group_w, o->group_h, o->stride, sy);
+    const int64_t M = (int64_t)o->group_w * o->stride * o->group_h * sy, K = (int64_t)o->group_w * o->group_h;
     if (M > 4096 || K > 1024) return crt_fail(ctx, CRT_ERR_UNSUPPORTED, "layout: tile of %lld slots / group of %lld exceeds 4096 / 1024", (long long)M, (long long)K);
-    L->W = o->group_w * o->stride; L->H = o->group_h * o->stride; L->M = (int)M; L->K = (int)K; L->G = (int)(M / K);
+    L->W = o->group_w * o->stride; L->H = o->group_h * sy; L->M = (int)M; L->K = (int)K; L->G = (int)(M / K);
     L->log2W = ilog2(L->W); L->log2M = ilog2(L->M); L->log2K = ilog2(L->K);
     L->tiles_x = (f->w + L->W - 1) / L->W; L->tiles_y = (f->h + L->H - 1) / L->H; L->n_tiles = L->tiles_x * L->tiles_y;
     L->n_slots = (int64_t)f->spp * L->n_tiles * L->M; L->n_groups = L->n_slots / L->K;

@@ -189,6 +189,8 @@ GEN_CASES = [
     ("interior_small", "direct_reuse", 8, 8, 8, 96, 64, 1),   # largest tile: M = 4096
     ("checker", "direct_reuse", 4, 4, 2, 48, 40, 1),          # hybrid groups
     ("checker", "direct_reuse", 1, 1, 4, 48, 40, 1),          # K = 1
+    ("interior_small", "direct_reuse", 8, 1, 1 | (8 << 16), 96, 64, 1),     # the paper's own setting: tile 8x8, K = 8
+    ("interior_small", "direct_reuse", 16, 1, 2 | (8 << 16), 90, 61, 2),    # tile 32x8, K = 16 (Table 3), ragged, 2 spp
     ("cornell", "world_reuse", 4, 4, 2, 64, 64, 1),           # world-space reuse (D:R18)
     ("interior_small", "world_reuse", 4, 4, 4, 96, 64, 1),
     ("interior_small", "world_reuse", 8, 8, 1, 90, 61, 2),    # K = 64, ragged image, 2 spp

@@ -12,12 +12,19 @@ M_IND, M_MOR, M_REUSE, M_WORLD = 0, 1, 2, 3
 
 
 # ------------------------------------------------------------------ partition
-@pytest.mark.parametrize("gw,gh,s", [(2, 2, 1), (2, 2, 8), (4, 4, 2), (4, 4, 4), (8, 8, 1), (8, 8, 8), (4, 2, 2), (1, 1, 4)])
+def _tile(tw, th, k):
+    """the paper's native (W, H, K) as (gw, gh, s) with the vertical stride in the high half of s"""
+    gw = min(k, tw); gh = k // gw
+    return gw, gh, (tw // gw) | ((th // gh) << 16)
+
+
+@pytest.mark.parametrize("gw,gh,s", [(2, 2, 1), (2, 2, 8), (4, 4, 2), (4, 4, 4), (8, 8, 1), (8, 8, 8), (4, 2, 2), (1, 1, 4),
+                                     _tile(8, 8, 8), _tile(16, 8, 16), _tile(32, 8, 64), _tile(16, 16, 32)])      # Table 3's shapes
 @pytest.mark.parametrize("w,h,spp", [(64, 64, 1), (50, 37, 2)])
 def test_partition_is_exact_cover(oracle, gw, gh, s, w, h, spp):
     fr = oracle.frame(w, h, spp, seed=3, frame=5)
     pos = oracle.partition(fr, M_REUSE, gw, gh, s)
-    W, H = gw * s, gh * s
+    W, H = gw * (s & 0xffff), gh * ((s >> 16) or (s & 0xffff))
     M, K = W * H, gw * gh
     tiles_x, tiles_y = -(-w // W), -(-h // H)
     assert len(pos) == spp * tiles_x * tiles_y * M == oracle.n_slots(fr, M_REUSE, gw, gh, s)

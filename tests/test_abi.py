@@ -58,13 +58,13 @@ def test_product_does_not_import_the_oracle():
 
 
 @pytest.mark.parametrize("w,h,spp,mode,gw,gh,s", [(64, 64, 1, 2, 4, 4, 2), (1920, 1080, 1, 2, 4, 4, 4), (3840, 2160, 4, 2, 8, 8, 8),
-                                                  (50, 37, 2, 2, 2, 4, 4), (1920, 1080, 1, 0, 1, 1, 1), (7, 5, 3, 1, 1, 1, 1), (0, 0, 1, 2, 2, 2, 2)])
+                                                  (50, 37, 2, 2, 2, 4, 4), (50, 37, 2, 3, 4, 4, 2), (1920, 1080, 1, 0, 1, 1, 1), (7, 5, 3, 1, 1, 1, 1), (0, 0, 1, 2, 2, 2, 2)])
 def test_layout_matches_the_paper_parametrisation(lib, oracle, w, h, spp, mode, gw, gh, s):
     """tiles of W x H pixels, WH/K groups of K; K = gw*gh, W = gw*s, H = gh*s (reading R3)."""
     import paper_2310_07182_b200 as crt
     n_paths, n_slots, n_groups = crt.crt_layout(crt.make_frame(w, h, spp), crt.make_order(mode, gw, gh, s))
     assert n_paths == spp * w * h
-    if mode == 2:
+    if mode in (2, 3):            # direct_reuse and world_reuse share the grouped slot space
         W, H = gw * s, gh * s
         tiles = -(-w // W) * -(-h // H)
         assert n_slots == spp * tiles * W * H and n_groups * gw * gh == n_slots
@@ -129,3 +129,24 @@ def test_scratch_size_queries(lib):
         assert lib.crt_frame_workspace_bytes(C.byref(fr), C.byref(order)) >= (32 * 2 + 16 + 16 + 32) * n
     bad = crt.make_order("direct_reuse", 3, 3, 3)
     assert lib.crt_frame_workspace_bytes(C.byref(fr), C.byref(bad)) == 0
+
+
+def test_native_tile_shapes_and_layout_errors(lib, oracle):
+    """The paper's (W, H, K) through crt_order.stride_y; what the kernels do not implement is refused."""
+    import paper_2310_07182_b200 as crt
+    from paper_2310_07182_b200 import api
+    fr = crt.make_frame(1920, 1080, 1)
+    for tw, th, k in ((8, 8, 8), (16, 8, 16), (16, 16, 32), (32, 8, 64), (8, 8, 64), (4, 4, 1)):
+        o = crt.order_for_tile("direct_reuse", tw, th, k)
+        assert o.group_w * o.stride == tw and o.group_h * (o.stride_y or o.stride) == th and o.group_w * o.group_h == k
+        n_paths, n_slots, n_groups = crt.crt_layout(fr, o)
+        tiles = -(-1920 // tw) * -(-1080 // th)
+        assert n_slots == tiles * tw * th and n_groups * k == n_slots
+        assert n_slots == oracle.n_slots(oracle.frame(1920, 1080, 1), 2, o.group_w, o.group_h, o.stride | ((o.stride_y or 0) << 16))
+    for bad in (crt.make_order("direct_reuse", 3, 4, 2), crt.make_order("direct_reuse", 4, 4, 2, 3), crt.make_order("direct_reuse", 64, 64, 2),
+                crt.make_order("direct_reuse", 4, 4, 0)):
+        n = C.c_int64()
+        assert lib.crt_layout(C.byref(fr), C.byref(bad), C.byref(n), None, None) == api.CRT_ERR_UNSUPPORTED
+    for bad_mode in (-1, 4):
+        o = api.Order(bad_mode, 1, 1, 1, 0); n = C.c_int64()
+        assert lib.crt_layout(C.byref(fr), C.byref(o), C.byref(n), None, None) == api.CRT_ERR_INVALID_ARG

@@ -109,6 +109,8 @@ struct GenArgs {
     Bounds6 bounds;
     int64_t n_slots; int32_t bounce; int32_t morton;
     int32_t world;           // direct_reuse in WORLD space (mode 3; D:R18)
+    int32_t fuse_shade;      // crt_render_frame: shade the previous segment here (same arithmetic as shade_kernel) instead of in its own pass
+    float env[6];
 };
 
 enum { F_DEAD = 0, F_DIFF = 1, F_GLOSS = 2 };
@@ -143,6 +145,26 @@ __global__ void __launch_bounds__(1024) generate_kernel(GenArgs A, DevLayout L)
         const float4 rd = __ldg(reinterpret_cast<const float4*>(A.prev_rays + i) + 1);
         const float4 hv = __ldg(reinterpret_cast<const float4*>(A.prev_hits + i));
         const int prim = __float_as_int(hv.w);
+        if (A.fuse_shade && (ps.flags & 1u) && rd.w >= 0.f) {
+            // a6 fused (D:R14): a miss collects the environment, an emissive hit its emission; either ends the path
+            float Le[3]; bool ends = false;
+            if (prim < 0) {
+                const float w = mul(0.5f, add(rd.y, 1.0f));
+#pragma unroll
+                for (int k = 0; k < 3; ++k) Le[k] = add(A.env[k], mul(sub(A.env[3 + k], A.env[k]), w));
+                ends = true;
+            } else {
+                const float4 m1 = __ldg(reinterpret_cast<const float4*>(A.mats + __ldg(A.mat_id + prim)) + 1);
+                if (__float_as_int(m1.w) == CRT_MAT_EMISSIVE) { Le[0] = m1.x; Le[1] = m1.y; Le[2] = m1.z; ends = true; }
+            }
+            if (ends) {
+                float4* pw = reinterpret_cast<float4*>(A.paths + p);
+                float4 p1 = pw[1];
+                p1.x = add(p1.x, mul(ps.tr, Le[0])); p1.y = add(p1.y, mul(ps.tg, Le[1])); p1.z = add(p1.z, mul(ps.tb, Le[2]));
+                ps.flags &= ~1u;
+                pw[0] = make_float4(ps.tr, ps.tg, ps.tb, __uint_as_float(ps.flags)); pw[1] = p1;
+            }
+        }
         if ((ps.flags & 1u) && rd.w >= 0.f && prim >= 0) {
             const float4* tp = reinterpret_cast<const float4*>(A.tris + __ldg(A.slot_of_prim + prim));
             const float4 a = __ldg(tp), b = __ldg(tp + 1), c = __ldg(tp + 2);
@@ -335,7 +357,7 @@ crt_status launch_morton_encode(crt_ctx* ctx, const float* bounds, const crt_ray
 crt_status launch_generate(crt_ctx* ctx, const crt_bvh* bvh, const crt_scene_mats& mats, const crt_frame& f, int bounce, const Layout& L,
                            const crt_ray* prev_rays, const crt_hit* prev_hits, const int32_t* prev_r2p, crt_path_state* paths,
                            crt_ray* rays_out, int32_t* r2p_out, int32_t* gid_out, int32_t* src_out, uint8_t* cls_out,
-                           uint32_t* n_active, void* scratch, size_t scratch_bytes, cudaStream_t st, cudaEvent_t* ev4)
+                           uint32_t* n_active, void* scratch, size_t scratch_bytes, cudaStream_t st, cudaEvent_t* ev4, bool fuse_shade)
 {
     CRT_CUDA(ctx, cudaMemsetAsync(n_active, 0, sizeof(uint32_t), st));
     if (L.n_slots == 0) return CRT_OK;
@@ -346,6 +368,8 @@ crt_status launch_generate(crt_ctx* ctx, const crt_bvh* bvh, const crt_scene_mat
     A.rays_out = rays_out; A.r2p_out = r2p_out; A.gid_out = gid_out; A.src_out = src_out; A.cls_out = cls_out; A.n_active = n_active;
     A.keys_out = nullptr; A.bounds = make_bounds(bvh->bounds); A.n_slots = L.n_slots; A.bounce = bounce; A.morton = 0;
     A.world = (L.mode == CRT_MODE_WORLD_REUSE);
+    A.fuse_shade = fuse_shade ? 1 : 0;
+    for (int k = 0; k < 6; ++k) A.env[k] = mats.env[k];
     const DevLayout D = make_dev_layout(L, f);
     const int64_t n = L.n_slots;
     if (L.mode == CRT_MODE_DIRECT_REUSE || L.mode == CRT_MODE_WORLD_REUSE) {

@@ -105,7 +105,7 @@ crt_status crt_measure_peaks(crt_ctx* ctx, double* fp32_tflops, double* copy_gbs
  * max_leaf == 1, its collapse into 8-wide compressed 128-byte nodes (read by trace_kernel 2; measured slower than the
  * binary layout on both bench workloads, profiles/r01b, so not the default).
  * verts: [host|device] float[n_tris][3][3]; mat_id: [host|device] int32[n_tris].  Synchronous.  params may be
- * NULL (defaults: max_leaf 4, 64 bins, costs 1/1, all hardware threads).  With ctx == NULL only the host tree is built (for crt_bvh_check /
+ * NULL (defaults: max_leaf 3, 64 bins, costs 1/1, all hardware threads).  With ctx == NULL only the host tree is built (for crt_bvh_check /
  * crt_bvh_get_info; such a BVH is rejected by the device calls with CRT_ERR_STATE). */
 crt_status crt_build_bvh(crt_ctx* ctx, const float* verts, const int32_t* mat_id, int64_t n_tris,
                          const crt_bvh_params* params, crt_bvh** out);

@@ -222,7 +222,7 @@ class Context:
         return a.value, b.value
 
     # ---- a0 -----------------------------------------------------------------------------------------
-    def crt_build_bvh(self, verts, mat_id, max_leaf=4, sah_bins=64, n_threads=0, cost_traversal=1.0, cost_intersect=1.0):
+    def crt_build_bvh(self, verts, mat_id, max_leaf=3, sah_bins=64, n_threads=0, cost_traversal=1.0, cost_intersect=1.0):
         """verts: numpy float32[n,3,3] or torch tensor (host or device); mat_id int32[n]."""
         if isinstance(verts, np.ndarray):
             verts = np.ascontiguousarray(verts, np.float32)

@@ -114,7 +114,7 @@ crt_status crt_build_bvh(crt_ctx* ctx, const float* verts, const int32_t* mat_id
     *out = nullptr;
     if (n_tris < 0 || (n_tris > 0 && !verts)) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "build_bvh: bad triangle array");
     if (n_tris >= ((int64_t)1 << 28)) return crt_fail(ctx, CRT_ERR_UNSUPPORTED, "build_bvh: more than 2^28 triangles");
-    crt_bvh_params pr = {4, 64, 1.0f, 1.0f, 0};
+    crt_bvh_params pr = {3, 64, 1.0f, 1.0f, 0};
     if (params) pr = *params;
     if (pr.max_leaf < 1 || pr.max_leaf > 8) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "build_bvh: max_leaf %d not in [1,8]", pr.max_leaf);
     if (pr.sah_bins == 0) pr.sah_bins = 64;

@@ -295,7 +295,7 @@ def run_cuda(args):
         "modes": modes, "roofline": roofline, "cpu_baseline": cpu,
         "e2e": {"value": e2e["mray_s"], "unit": UNIT, "h2d_bytes_per_step": img_bytes + len(scene.materials) * 32 + 48,
                 "d2h_bytes_per_step": img_bytes + 4 * nb, "ms_per_step": e2e["ms_per_step"], "api": "crt_render_frame_host"},
-        "gpu_launches": K * (4 + 2 * nb), "clocks": clk,
+        "gpu_launches": K * (4 + 3 * nb), "clocks": clk,
     }
     print(json.dumps(line))
 

@@ -89,6 +89,7 @@ crt_status crt_set_option(crt_ctx* ctx, const char* key, int64_t value)
     else if (!strcmp(key, "trace_refill_threshold")) { if (value < 0 || value > 32) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "trace_refill_threshold out of range"); ctx->trace_refill_threshold = (int)value; }
     else if (!strcmp(key, "trace_leaf_wait")) { if (value < 0 || value > 31) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "trace_leaf_wait out of range"); ctx->trace_leaf_wait = (int)value; }
     else if (!strcmp(key, "trace_tri_wait")) { if (value < 0 || value > 32) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "trace_tri_wait out of range"); ctx->trace_tri_wait = (int)value; }
+    else if (!strcmp(key, "fuse_shade")) { ctx->fuse_shade = value != 0; }
     else if (!strcmp(key, "trace_blocks_per_sm")) { if (value < 0 || value > 32) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "trace_blocks_per_sm out of range"); ctx->trace_blocks_per_sm = (int)value; }
     else return crt_fail(ctx, CRT_ERR_INVALID_ARG, "set_option: unknown key '%s'", key);
     return CRT_OK;
@@ -361,8 +362,9 @@ crt_status crt_render_frame(crt_ctx* ctx, const crt_bvh* bvh, const crt_scene_ma
     MARK(-1);
     STEP(launch_primary(ctx, bvh, *camera, *frame, L, W.rays[0], W.hits, W.r2p[0], s));
     MARK(0);
-    // the shading of every segment but the last is fused into the generation of the next bounce (same arithmetic, one pass less)
-    if (n_bounces == 0) STEP(launch_shade(ctx, bvh, *mats, *frame, 1, W.rays[0], W.hits, W.r2p[0], L.n_slots, W.paths, accum, s));
+    // option fuse_shade: the shading of every segment but the last runs inside the generation kernel of the next bounce
+    const bool fuse = ctx->fuse_shade != 0;
+    if (n_bounces == 0 || !fuse) STEP(launch_shade(ctx, bvh, *mats, *frame, n_bounces == 0, W.rays[0], W.hits, W.r2p[0], L.n_slots, W.paths, accum, s));
     MARK(1);
     int cur = 0;
     for (int b = 1; b <= n_bounces; ++b) {
@@ -374,13 +376,13 @@ crt_status crt_render_frame(crt_ctx* ctx, const crt_bvh* bvh, const crt_scene_ma
             ev4[1] = ctx->ev[ctx->ev_used]; ctx->ev_stage[ctx->ev_used++] = 4;      // after permute: closes stage 4
         }
         STEP(launch_generate(ctx, bvh, *mats, *frame, b, L, W.rays[cur], W.hits, W.r2p[cur], W.paths, W.rays[1 - cur], W.r2p[1 - cur], W.gid, W.src, W.cls,
-                             W.n_active, W.scratch, W.scratch_bytes, s, ev4[0] ? ev4 : nullptr, true));
+                             W.n_active, W.scratch, W.scratch_bytes, s, ev4[0] ? ev4 : nullptr, fuse));
         cur = 1 - cur;
         if (n_secondary_out) CRT_CUDA(ctx, cudaMemcpyAsync(n_secondary_out + (b - 1), W.n_active, 4, cudaMemcpyDeviceToDevice, s));
         MARK(2);
         STEP(launch_trace(ctx, bvh, W.rays[cur], L.n_slots, W.hits, s));
         MARK(3);
-        if (b == n_bounces) STEP(launch_shade(ctx, bvh, *mats, *frame, 1, W.rays[cur], W.hits, W.r2p[cur], L.n_slots, W.paths, accum, s));
+        if (b == n_bounces || !fuse) STEP(launch_shade(ctx, bvh, *mats, *frame, b == n_bounces, W.rays[cur], W.hits, W.r2p[cur], L.n_slots, W.paths, accum, s));
         MARK(1);
     }
 #undef STEP

@@ -369,3 +369,26 @@ def test_argument_errors(crt, ctx):
     with pytest.raises(crt.CrtError):
         ctx.crt_set_option("no_such_option", 1)
     torch.cuda.synchronize()
+
+
+def test_fused_shading_option_gives_the_identical_image(crt, ctx):
+    """crt_set_option("fuse_shade", 1): same arithmetic inside the generation kernel; the image must not change."""
+    import torch
+    scene = _small_interior().with_camera(90, 61)
+    G = GpuScene(crt, scene, ctx)
+    imgs = []
+    for mode, gw, gh, s in (("direct_reuse", 4, 4, 2), ("independent", 1, 1, 1), ("morton_reorder", 1, 1, 1), ("world_reuse", 4, 4, 2)):
+        for fuse in (0, 1):
+            ctx.crt_set_option("fuse_shade", fuse)
+            try:
+                order = crt.make_order(mode, gw, gh, s)
+                fr = crt.make_frame(90, 61, 2, 5, 1)
+                ws = ctx.frame_workspace(fr, order)
+                acc = torch.zeros((61, 90, 3), device=ctx.device)
+                ctx.crt_render_frame(G.bvh, G.mats, G.camera, fr, order, 3, acc, ws)
+                torch.cuda.synchronize()
+                imgs.append(acc.cpu().numpy())
+            finally:
+                ctx.crt_set_option("fuse_shade", 0)
+        # 2 spp: the two samples of a pixel are added with atomicAdd in either order, so allow one rounding of difference
+        assert imgs[-1].sum() > 0 and np.allclose(imgs[-2], imgs[-1], rtol=1e-6, atol=0)

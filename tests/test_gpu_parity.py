@@ -31,6 +31,7 @@ def _small_interior():
 
 
 SCENES = {
+    "landscape_small": lambda: I.landscape(seed=2, width=96, height=64, n=192, n_trees=150),
     "cornell": lambda: I.cornell(),
     "interior_small": _small_interior,
     "checker": lambda: I.checker_floor(seed=3, width=48, height=40),
@@ -79,7 +80,7 @@ def test_full_size_config2_stagewise_and_sampled(crt, ctx, oracle):
 
 
 # ------------------------------------------------------------------ a0 / a5: BVH + traversal
-@pytest.mark.parametrize("scene_name", ["cornell", "interior_small"])
+@pytest.mark.parametrize("scene_name", ["cornell", "interior_small", "landscape_small"])
 @pytest.mark.parametrize("kernel", [0, 1, 2])
 def test_trace_matches_oracle_on_random_rays(crt, ctx, oracle, scene_name, kernel):
     scene = SCENES[scene_name]()
@@ -191,6 +192,8 @@ GEN_CASES = [
     ("checker", "direct_reuse", 1, 1, 4, 48, 40, 1),          # K = 1
     ("interior_small", "direct_reuse", 8, 1, 1 | (8 << 16), 96, 64, 1),     # the paper's own setting: tile 8x8, K = 8
     ("interior_small", "direct_reuse", 16, 1, 2 | (8 << 16), 90, 61, 2),    # tile 32x8, K = 16 (Table 3), ragged, 2 spp
+    ("landscape_small", "direct_reuse", 4, 4, 4, 96, 64, 1),  # config 4's grouping on a reduced landscape (coordinates up to 192, sky misses)
+    ("landscape_small", "morton_reorder", 1, 1, 1, 90, 61, 1),
     ("cornell", "world_reuse", 4, 4, 2, 64, 64, 1),           # world-space reuse (D:R18)
     ("interior_small", "world_reuse", 4, 4, 4, 96, 64, 1),
     ("interior_small", "world_reuse", 8, 8, 1, 90, 61, 2),    # K = 64, ragged image, 2 spp
@@ -392,3 +395,33 @@ def test_fused_shading_option_gives_the_identical_image(crt, ctx):
                 ctx.crt_set_option("fuse_shade", 0)
         # 2 spp: the two samples of a pixel are added with atomicAdd in either order, so allow one rounding of difference
         assert imgs[-1].sum() > 0 and np.allclose(imgs[-2], imgs[-1], rtol=1e-6, atol=0)
+
+
+def test_full_size_config4_sampled(crt, ctx, oracle):
+    """BASELINE config 4 at full size (10,300,418 triangles, coordinates up to 2048): sampled primary and secondary hits of the
+    direct_reuse frame equal the all-triangles definition; the partition is the oracle's."""
+    scene = I.landscape(seed=2).with_camera(1920, 1080)
+    assert scene.n_tris == 10300418
+    G = GpuScene(crt, scene, ctx)
+    assert G.bvh.check() == 0
+    w, h, spp, gw, gh, s = 1920, 1080, 1, 4, 4, 4
+    fr = crt.make_frame(w, h, spp, 2, 1); ofr = oracle.frame(w, h, spp, 2, 1)
+    order = crt.make_order("direct_reuse", gw, gh, s)
+    rays0, hits0, r2p0 = ctx.crt_trace_primary(G.bvh, G.camera, fr, order)
+    assert np.array_equal(r2p0.cpu().numpy(), oracle.partition(ofr, 2, gw, gh, s))
+    import torch
+    n_paths = crt.crt_layout(fr, order)[0]
+    paths = ctx.empty((n_paths, 8)); ctx.crt_paths_init(paths)
+    accum = torch.zeros((h, w, 3), device=ctx.device)
+    ctx.crt_shade_accumulate(G.bvh, G.mats, fr, 0, False, rays0, hits0, r2p0, paths, accum)
+    out = ctx.crt_generate_secondary(G.bvh, G.mats, fr, 1, order, rays0, hits0, r2p0, paths)
+    hits1 = ctx.crt_trace(G.bvh, out["rays"])
+    rng = np.random.default_rng(12)
+    for rays_dev, hits_dev, n_s in ((rays0, hits0, 40), (out["rays"], hits1, 80)):
+        r = rays_np(oracle, rays_dev); hh = hits_np(oracle, hits_dev)
+        act = np.flatnonzero(r["tmax"] >= 0)
+        pick = rng.choice(act, n_s, replace=False)
+        ref = oracle.trace_brute(scene.verts, r[pick])
+        compare_hits(hh[pick], ref)
+        if n_s == 80:
+            assert (ref["prim"] >= 0).any() and (ref["prim"] < 0).any()               # the secondary sample has terrain hits and sky misses

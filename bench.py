@@ -42,13 +42,13 @@ FLOP_PER_NODE_VISIT, FLOP_PER_TRI_TEST, FLOP_PER_RAY = 26.0, 46.0, 3.0
 FP32_PEAK_TFLOPS_NOMINAL = 148 * 128 * 2 * 1.965e9 / 1e12
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the secondary trace kernel, from profiles/ (ncu --set full);
 # keyed by workload; None until captured.
-TRACE_DRAM_TRAFFIC = {"interior": 127.5e6, "landscape": 106.5e6, "cornell": None}     # profiles/r01d_final_state.md (mean of the two captured launches)
+TRACE_DRAM_TRAFFIC = {"interior": 129.5e6, "landscape": 108.0e6, "cornell": None}     # profiles/r01d_final_state.md (mean of the two captured launches)
 # what ncu shows to be the kernel's limiter (not modelled by the two-term roofline): profiles/r01a, r01b
-TRACE_LIMITER = {"interior": {"unit": "l1tex data pipe", "l1tex__data_pipe_lsu_wavefronts_pct_of_peak": 77.0, "issue_slots_busy_pct": 65.0,
-                              "active_threads_per_warp_instruction": 14.1, "alu_pipe_pct": 50.0, "fma_pipe_pct": 26.0, "dram_pct": 1.5,
+TRACE_LIMITER = {"interior": {"unit": "l1tex data pipe", "l1tex__data_pipe_lsu_wavefronts_pct_of_peak": 81.0, "issue_slots_busy_pct": 62.0,
+                              "active_threads_per_warp_instruction": 15.0, "alu_pipe_pct": 52.0, "fma_pipe_pct": 20.0, "dram_pct": 1.5,
                               "source": "profiles/r01d_final_state.md"},
-                 "landscape": {"unit": "l1tex data pipe", "l1tex__data_pipe_lsu_wavefronts_pct_of_peak": 69.0, "issue_slots_busy_pct": 67.0,
-                               "active_threads_per_warp_instruction": 16.2, "alu_pipe_pct": 52.0, "fma_pipe_pct": 24.0, "dram_pct": 3.0,
+                 "landscape": {"unit": "l1tex data pipe", "l1tex__data_pipe_lsu_wavefronts_pct_of_peak": 71.0, "issue_slots_busy_pct": 64.0,
+                               "active_threads_per_warp_instruction": 16.7, "alu_pipe_pct": 56.0, "fma_pipe_pct": 19.0, "dram_pct": 3.0,
                                "source": "profiles/r01d_final_state.md (bounce 1; bounce 2 has 0.4 M live rays and is latency-bound)"}}
 
 

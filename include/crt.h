@@ -92,7 +92,9 @@ crt_status crt_destroy(crt_ctx* ctx);
 /* Message of the last failed call on ctx (ctx may be NULL: last failure of a call that had no context). */
 const char* crt_last_error(const crt_ctx* ctx);
 /* Tunables (for experiments; defaults are what bench.py times): "trace_kernel" (0 = binary BVH, one thread per ray;
- * 1 = binary BVH, persistent warps with per-lane dynamic fetch -- the default; 2 = 8-wide compressed BVH, persistent warps), "trace_refill_threshold" (0..32: idle lanes fetch new rays when
+ * 1 = binary BVH with fp32 64-byte nodes, persistent warps with per-lane dynamic fetch; 2 = 8-wide compressed BVH, persistent warps;
+ * 3 = the persistent kernel of 1 on 16-bit 32-byte nodes -- the default), "trace_leaf_wait" (0..31: a warp leaves its inner-node
+ * phase when at most this many descending lanes hold no leaf), "trace_refill_threshold" (0..32: idle lanes fetch new rays when
  * fewer lanes than this are busy), "trace_blocks_per_sm" (0 = from the occupancy calculator), "trace_tri_wait" (8-wide kernel: lanes holding triangle hits
  * before a warp enters its triangle phase), "fuse_shade" (crt_render_frame shades non-final segments inside the next generation
  * kernel; off by default: 2 % faster on the interior scene, 7 % slower on the landscape scene). */
@@ -103,7 +105,9 @@ crt_status crt_measure_peaks(crt_ctx* ctx, double* fp32_tflops, double* copy_gbs
 
 /* ---- a0: acceleration structure (D:R11) ------------------------------------------------ */
 /* Builds a binary BVH (binned surface-area heuristic, leaves <= max_leaf triangles) on the host with
- * n_threads threads and uploads it in the traversal layouts: the binary 64-byte-node layout always, and, when
+ * n_threads threads and uploads it in the traversal layouts: the binary fp32 64-byte-node layout and its 16-bit
+ * 32-byte-node form (planes on a 65536-step grid over the scene box, rounded outward; read by the default trace_kernel 3,
+ * whose box test is conservative for ray origins within about a hundred scene extents of the scene) always, and, when
  * max_leaf == 1, its collapse into 8-wide compressed 128-byte nodes (read by trace_kernel 2; measured slower than the
  * binary layout on both bench workloads, profiles/r01b, so not the default).
  * verts: [host|device] float[n_tris][3][3]; mat_id: [host|device] int32[n_tris].  Synchronous.  params may be
@@ -115,7 +119,8 @@ crt_status crt_bvh_destroy(crt_bvh* bvh);
 crt_status crt_bvh_get_info(const crt_bvh* bvh, crt_bvh_info_t* out);
 /* Structural invariants of the host tree: *violations = 0 iff every triangle is in exactly one leaf, every
  * leaf has 1..max_leaf triangles, every node's box contains its children's boxes / its triangles, and (wide
- * layout, bits 8 and up) every triangle lies inside the box the kernel decodes for each of its ancestors. */
+ * layout, bits 8 and up) every triangle lies inside the box the kernel decodes for each of its ancestors, and (16-bit
+ * layout, bit 16) every quantised plane lies at least one grid step outside the fp32 box it replaces. */
 crt_status crt_bvh_check(const crt_bvh* bvh, int32_t* violations);
 
 /* ---- index spaces -------------------------------------------------------------------------------- */

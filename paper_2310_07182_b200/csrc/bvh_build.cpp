@@ -304,3 +304,59 @@ void crt_bvh_flatten(const crt_bvh* b, const std::vector<int32_t>& tri_order, st
         gn[k] = g;
     }
 }
+
+// 16-bit layout of the flattened nodes (trace_kernel 3): every box plane becomes a position on a 65536-step grid over the
+// scene box, rounded OUTWARD (min planes down, max planes up) and then moved ONE more step outward: the traversal kernel
+// evaluates a plane distance as one FMA in grid units whose rounding error is at most 0.5 + 2^-4 step of position
+// (trace.cu: QRay), so the box test stays conservative (D:R10: it never decides the result, only which subtrees are
+// visited).  Returns 0, or 1 if a plane had to be clamped / is less than one step outside its box.
+int32_t crt_bvh_quantise(const crt_bvh* b, const std::vector<GpuNode>& gn, std::vector<QNode>& qn, QGrid* grid)
+{
+    (void)b;
+    double lo[3] = {1e300, 1e300, 1e300}, hi[3] = {-1e300, -1e300, -1e300};
+    auto planes = [](const GpuChild& c, int k, double& mn, double& mx) {
+        const float* p = &c.min_x; mn = p[2 * k]; mx = p[2 * k + 1];
+    };
+    if (!gn.empty())
+        for (int c = 0; c < 2; ++c)
+            for (int k = 0; k < 3; ++k) {
+                double mn, mx; planes(gn[0].c[c], k, mn, mx);
+                if (std::isfinite(mn) && std::isfinite(mx)) { lo[k] = std::min(lo[k], mn); hi[k] = std::max(hi[k], mx); }
+            }
+    double maxext = 0;
+    for (int k = 0; k < 3; ++k) { if (lo[k] > hi[k]) { lo[k] = 0; hi[k] = 1; } maxext = std::max(maxext, hi[k] - lo[k]); }
+    if (!(maxext > 0)) maxext = 1;
+    for (int k = 0; k < 3; ++k) {
+        const double e = std::max(hi[k] - lo[k], maxext * (1.0 / 4096.0));
+        const float scale = (float)((65535.0 - 16.0) / e);
+        grid->scale[k] = scale;
+        grid->gmin[k] = (float)(lo[k] - 8.0 / (double)scale);
+        grid->inv_scale[k] = (float)(1.0 / (double)scale);
+    }
+    int32_t bad = 0;
+    qn.resize(gn.size());
+    for (size_t i = 0; i < gn.size(); ++i) {
+        QNode q;
+        for (int c = 0; c < 2; ++c) {
+            q.ref[c] = gn[i].c[c].ref;
+            for (int k = 0; k < 3; ++k) {
+                double mn, mx; planes(gn[i].c[c], k, mn, mx);
+                uint32_t qlo = 65535u, qhi = 0u;           // empty child: inverted on every axis, fails for every ray
+                if (std::isfinite(mn) && std::isfinite(mx)) {
+                    const double g = (double)grid->gmin[k], s = (double)grid->scale[k];
+                    double a = std::floor((mn - g) * s), z = std::ceil((mx - g) * s);
+                    if (g + a / s > mn) a -= 1.0;          // the products above are rounded: re-check in the direction that matters
+                    if (g + z / s < mx) z += 1.0;
+                    a -= 1.0; z += 1.0;
+                    if (a < 0.0) { a = 0.0; bad |= 1; }
+                    if (z > 65535.0) { z = 65535.0; bad |= 1; }
+                    if (!(g + (a + 1.0) / s <= mn) || !(g + (z - 1.0) / s >= mx)) bad |= 1;
+                    qlo = (uint32_t)a; qhi = (uint32_t)z;
+                }
+                q.planes[3 * c + k] = qlo | (qhi << 16);
+            }
+        }
+        qn[i] = q;
+    }
+    return bad;
+}

@@ -6,6 +6,7 @@
 bool crt_bvh_build_host(crt_bvh* b, const float* verts, int64_t n, const crt_bvh_params& pr);
 int32_t crt_bvh_check_host(const crt_bvh* b);
 void crt_bvh_flatten(const crt_bvh* b, const std::vector<int32_t>& tri_order, std::vector<GpuNode>& gn, std::vector<GpuTri>& gt, std::vector<int32_t>& slot_of_prim);
+int32_t crt_bvh_quantise(const crt_bvh* b, const std::vector<GpuNode>& gn, std::vector<QNode>& qn, QGrid* grid);
 void crt_bvh_build_wide(const crt_bvh* b, std::vector<WNode>& wn, std::vector<int32_t>& tri_order, int* depth_out);
 int32_t crt_bvh_check_wide(const crt_bvh* b, const std::vector<WNode>& wn, const std::vector<int32_t>& tri_order);
 
@@ -85,7 +86,7 @@ const char* crt_last_error(const crt_ctx* ctx) { return ctx ? ctx->last_error.c_
 crt_status crt_set_option(crt_ctx* ctx, const char* key, int64_t value)
 {
     if (!ctx || !key) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "set_option: null argument");
-    if (!strcmp(key, "trace_kernel")) { if (value < 0 || value > 2) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "trace_kernel must be 0, 1 or 2"); ctx->trace_kernel = (int)value; }
+    if (!strcmp(key, "trace_kernel")) { if (value < 0 || value > 3) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "trace_kernel must be 0, 1, 2 or 3"); ctx->trace_kernel = (int)value; }
     else if (!strcmp(key, "trace_refill_threshold")) { if (value < 0 || value > 32) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "trace_refill_threshold out of range"); ctx->trace_refill_threshold = (int)value; }
     else if (!strcmp(key, "trace_leaf_wait")) { if (value < 0 || value > 31) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "trace_leaf_wait out of range"); ctx->trace_leaf_wait = (int)value; }
     else if (!strcmp(key, "trace_tri_wait")) { if (value < 0 || value > 32) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "trace_tri_wait out of range"); ctx->trace_tri_wait = (int)value; }
@@ -145,6 +146,8 @@ crt_status crt_build_bvh(crt_ctx* ctx, const float* verts, const int32_t* mat_id
     if (ctx) {
         std::vector<GpuNode> gn; std::vector<GpuTri> gt; std::vector<int32_t> sop;
         crt_bvh_flatten(b, tri_order, gn, gt, sop);
+        std::vector<QNode> qn;
+        b->q_violations = crt_bvh_quantise(b, gn, qn, &b->qgrid);
         b->device = ctx->device; b->n_gpu_nodes = (int64_t)gn.size();
         auto up = [&](void** d, const void* h, size_t bytes) -> cudaError_t {
             cudaError_t e = cudaMalloc(d, bytes ? bytes : 256);
@@ -153,6 +156,7 @@ crt_status crt_build_bvh(crt_ctx* ctx, const float* verts, const int32_t* mat_id
             return bytes ? cudaMemcpy(*d, h, bytes, cudaMemcpyHostToDevice) : cudaSuccess;
         };
         cudaError_t e = up((void**)&b->d_nodes, gn.data(), gn.size() * sizeof(GpuNode));
+        if (e == cudaSuccess) e = up((void**)&b->d_qnodes, qn.data(), qn.size() * sizeof(QNode));
         if (e == cudaSuccess) e = up((void**)&b->d_tris, gt.data(), gt.size() * sizeof(GpuTri));
         if (e == cudaSuccess && !wn.empty()) e = up((void**)&b->d_wnodes, wn.data(), wn.size() * sizeof(WNode));
         if (e == cudaSuccess) e = up((void**)&b->d_slot_of_prim, sop.data(), sop.size() * 4);
@@ -166,7 +170,7 @@ crt_status crt_build_bvh(crt_ctx* ctx, const float* verts, const int32_t* mat_id
 crt_status crt_bvh_destroy(crt_bvh* b)
 {
     if (!b) return CRT_OK;
-    cudaFree(b->d_nodes); cudaFree(b->d_wnodes); cudaFree(b->d_tris); cudaFree(b->d_slot_of_prim); cudaFree(b->d_mat_id);
+    cudaFree(b->d_nodes); cudaFree(b->d_qnodes); cudaFree(b->d_wnodes); cudaFree(b->d_tris); cudaFree(b->d_slot_of_prim); cudaFree(b->d_mat_id);
     delete b;
     return CRT_OK;
 }
@@ -184,7 +188,7 @@ crt_status crt_bvh_get_info(const crt_bvh* b, crt_bvh_info_t* o)
 crt_status crt_bvh_check(const crt_bvh* b, int32_t* violations)
 {
     if (!b || !violations) return crt_fail(nullptr, CRT_ERR_INVALID_ARG, "bvh_check: null argument");
-    *violations = crt_bvh_check_host(b) | (b->wide_violations << 8);
+    *violations = crt_bvh_check_host(b) | (b->wide_violations << 8) | (b->q_violations << 16);
     return CRT_OK;
 }
 

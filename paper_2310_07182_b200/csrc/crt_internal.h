@@ -13,9 +13,9 @@ struct crt_ctx {
     int n_sms = 0;
     std::string last_error;
     // options
-    int trace_kernel = 1;        // 0: binary BVH, one thread per ray; 1 (default): binary BVH, persistent warps; 2: 8-wide compressed BVH, persistent warps (needs max_leaf == 1; else falls back to 1)
-    int trace_refill_threshold = 20;   // idle lanes refetch when fewer than this many lanes of the warp are busy
-    int trace_leaf_wait = 3;           // leave the inner-node phase when at most this many converged lanes still lack a leaf
+    int trace_kernel = 3;        // 0: binary BVH, one thread per ray; 1: binary BVH with fp32 64-byte nodes, persistent warps; 2: 8-wide compressed BVH, persistent warps (needs max_leaf == 1; else falls back to 1); 3 (default): binary BVH with 16-bit 32-byte nodes, persistent warps
+    int trace_refill_threshold = 16;   // idle lanes refetch when fewer than this many lanes of the warp are busy
+    int trace_leaf_wait = 4;           // leave the inner-node phase when at most this many converged lanes still lack a leaf
     int trace_tri_wait = 8;            // wide kernel: a warp enters its triangle phase when at least this many lanes hold triangle hits
     int trace_blocks_per_sm = 0; // 0 = from occupancy
     int fuse_shade = 0;          // crt_render_frame: shade non-final segments inside the next generation kernel (option; measured: DESIGN.md 5.4)
@@ -41,6 +41,10 @@ struct GpuChild {
     int32_t pad;
 };
 struct alignas(64) GpuNode { GpuChild c[2]; };
+// quantised traversal layout (device): 32 bytes = ONE 256-bit load per node.  Box planes are 16-bit positions on a grid
+// over the (padded) scene box, rounded outward (bvh_build.cpp: crt_bvh_quantise); word k < 3 = child 0, axis k; word 3 + k =
+// child 1, axis k; low half = min plane, high half = max plane.  ref as in GpuChild.
+struct alignas(32) QNode { uint32_t planes[6]; int32_t ref[2]; };
 // leaf triangle, 64 bytes = two 256-bit loads: v0 | prim id, e1 | 0, e2 | 0, padding
 // (e = v - v0 rounded once, as the intersection formula needs)
 struct alignas(64) GpuTri { float4 v0p; float4 e1; float4 e2; float4 pad; };
@@ -54,7 +58,9 @@ struct alignas(128) WNode {
     uint32_t masks;          // imask (inner children) | lmask << 8 (triangle children)
     uint32_t planes[3][8];   // per axis: 4 words of LO planes, 4 words of HI planes; word k = children 2k (low half), 2k+1 (high half)
 };
-static_assert(sizeof(WNode) == 128 && sizeof(GpuTri) == 64, "device layouts");
+static_assert(sizeof(WNode) == 128 && sizeof(GpuTri) == 64 && sizeof(QNode) == 32, "device layouts");
+// grid of the quantised layout: position q (0..65535) on axis k is the coordinate gmin[k] + q / scale[k]
+struct QGrid { float gmin[3], scale[3], inv_scale[3]; };
 
 struct crt_bvh {
     int64_t n_tris = 0;
@@ -67,6 +73,7 @@ struct crt_bvh {
     // device data
     int device = -1;
     GpuNode* d_nodes = nullptr; int64_t n_gpu_nodes = 0;
+    QNode* d_qnodes = nullptr; QGrid qgrid = {}; int32_t q_violations = 0;   // 16-bit layout of the same nodes (trace_kernel 3)
     GpuTri* d_tris = nullptr;          // leaf order (wide order when the wide layout exists)
     WNode* d_wnodes = nullptr; int64_t n_wide_nodes = 0; int wide_depth = 0; int32_t wide_violations = 0;   // 8-wide layout (only when max_leaf == 1)
     int32_t* d_slot_of_prim = nullptr; // caller's triangle id -> index into d_tris

@@ -27,6 +27,9 @@ namespace {
 constexpr int STACK_SIZE = 64;
 constexpr int SENTINEL = 0x7fffffff;
 constexpr int TRACE_BLOCK = 128;
+// resident blocks per SM the persistent kernel is compiled for: fp32 nodes 9 (<= 56 registers), 16-bit nodes 8 (<= 64
+// registers; measured 1.5-3 % faster than 9 with this layout, profiles/r01f)
+#define CRT_TRACE_MINB(QN) ((QN) ? 8 : 9)
 
 struct ChildRegs { float min_x, max_x, min_y, max_y, min_z, max_z; int ref; };
 
@@ -47,7 +50,17 @@ CRT_DEV NodeRegs load_node(const GpuNode* __restrict__ nodes, int idx)
     return n;
 }
 
-struct Hit { float t, u, v; int prim; };
+struct Hit { float t; int prim; };     // u, v go straight to the hit record when a nearer hit is found (two registers fewer)
+
+// 1/d for the box test only.  A direction component of (nearly) zero is replaced by +-2^-60: with an infinite reciprocal the
+// two plane distances of an axis can come out as -inf and NaN, and min/max then keep the -inf for BOTH the entry and the
+// exit distance, which rejects boxes the ray is inside of.  With a huge finite reciprocal the distances are huge finite
+// numbers of the right signs; their cancellation error is an ulp of the origin, far inside the boxes' padding.
+CRT_DEV float safe_rcp(float d)
+{
+    const float eps = 8.673617379884035e-19f;      // 2^-60
+    return dvd(1.0f, fabsf(d) > eps ? d : copysignf(eps, d));
+}
 
 // Per-ray traversal state.  The slab test is t = b * (1/d) - o * (1/d) as one FMA per plane: its rounding error is a few
 // ulps of |o/d|, which the build-time padding of the boxes (>= 128 of those ulps for origins inside the padded scene box,
@@ -55,34 +68,35 @@ struct Hit { float t, u, v; int prim; };
 struct RayState {
     V3 o, d;
     float idx, idy, idz, ox, oy, oz;     // 1/d and -o/d
-    float tmin, tmax;
-    float tfar;                           // best t so far, inflated (prune bound)
+    float tmin;                           // best.t starts at the ray's tmax, so "t < tmax" is "t < best.t" until a hit exists
     Hit best;
+    // prune bound: best t so far, inflated (recomputed per visit: one FMUL instead of a register)
+    CRT_DEV float tfar() const { return best.t * 1.0000005f; }
     CRT_DEV void init(float4 ro, float4 rd)
     {
         o = mk(ro.x, ro.y, ro.z); d = mk(rd.x, rd.y, rd.z);
-        idx = dvd(1.0f, d.x); idy = dvd(1.0f, d.y); idz = dvd(1.0f, d.z);
+        idx = safe_rcp(d.x); idy = safe_rcp(d.y); idz = safe_rcp(d.z);
         ox = -o.x * idx; oy = -o.y * idy; oz = -o.z * idz;
-        tmin = ro.w; tmax = rd.w; tfar = rd.w;
-        best.t = rd.w; best.u = 0.f; best.v = 0.f; best.prim = -1;
+        tmin = ro.w;
+        best.t = rd.w; best.prim = -1;
     }
 };
 
 // Tests both children of `n`; returns the next node reference (nearer child, other child pushed) or pops the stack.
 CRT_DEV int visit_node(const NodeRegs& n, const RayState& r, int* stack, int& sp)
 {
-    // a zero direction component with the origin on a slab plane gives 0 * inf = NaN; fminf/fmaxf drop the NaN operand,
-    // which leaves the other planes to decide (conservative)
+    // every distance is finite (safe_rcp); a NaN could only come from non-finite ray data, and fminf/fmaxf drop NaN operands
     const float ax0 = __fmaf_rn(n.a.min_x, r.idx, r.ox), ax1 = __fmaf_rn(n.a.max_x, r.idx, r.ox);
     const float ay0 = __fmaf_rn(n.a.min_y, r.idy, r.oy), ay1 = __fmaf_rn(n.a.max_y, r.idy, r.oy);
     const float az0 = __fmaf_rn(n.a.min_z, r.idz, r.oz), az1 = __fmaf_rn(n.a.max_z, r.idz, r.oz);
     const float bx0 = __fmaf_rn(n.b.min_x, r.idx, r.ox), bx1 = __fmaf_rn(n.b.max_x, r.idx, r.ox);
     const float by0 = __fmaf_rn(n.b.min_y, r.idy, r.oy), by1 = __fmaf_rn(n.b.max_y, r.idy, r.oy);
     const float bz0 = __fmaf_rn(n.b.min_z, r.idz, r.oz), bz1 = __fmaf_rn(n.b.max_z, r.idz, r.oz);
+    const float tfar = r.tfar();
     const float tn0 = fmaxf(fmaxf(fminf(ax0, ax1), fminf(ay0, ay1)), fmaxf(fminf(az0, az1), r.tmin));
-    const float tf0 = fminf(fminf(fmaxf(ax0, ax1), fmaxf(ay0, ay1)), fminf(fmaxf(az0, az1), r.tfar));
+    const float tf0 = fminf(fminf(fmaxf(ax0, ax1), fmaxf(ay0, ay1)), fminf(fmaxf(az0, az1), tfar));
     const float tn1 = fmaxf(fmaxf(fminf(bx0, bx1), fminf(by0, by1)), fmaxf(fminf(bz0, bz1), r.tmin));
-    const float tf1 = fminf(fminf(fmaxf(bx0, bx1), fmaxf(by0, by1)), fminf(fmaxf(bz0, bz1), r.tfar));
+    const float tf1 = fminf(fminf(fmaxf(bx0, bx1), fmaxf(by0, by1)), fminf(fmaxf(bz0, bz1), tfar));
     const bool h0 = tn0 <= tf0, h1 = tn1 <= tf1;
     if (h0 && h1) {
         const bool swap = tn1 < tn0;
@@ -94,9 +108,59 @@ CRT_DEV int visit_node(const NodeRegs& n, const RayState& r, int* stack, int& sp
     return stack[sp--];
 }
 
+// ---- 16-bit nodes (QNode, 32 bytes, ONE 256-bit load; crt_internal.h, bvh_build.cpp: crt_bvh_quantise) -----------------
+// Per-ray constants of the box test in grid units.  A plane q (16 bits) becomes the float 2^23 + q with one PRMT (the two
+// plane bytes under the exponent byte of 0x4B000000) and its distance is one FMA: t = (2^23 + q) * s + c, c = -(o' + 2^23) * s
+// (o' = ray origin in grid units).
+// The PRMT selector picks the min or the max plane by the sign of the ray direction, so near and far distances come out
+// directly and no per-axis min/max is needed: 12 PRMT + 12 FFMA + 8 FMNMX per node against 12 FFMA + 20 FMNMX for fp32 nodes.
+struct QRay {
+    float sx, sy, sz;                     // 1 / (d * scale): distance per grid step
+    float cx, cy, cz;                     // -(o' + 2^23) * s
+    unsigned nx, ny, nz, fx, fy, fz;      // PRMT selectors of the near / far plane
+    // Error budget of t = (2^23 + q) * s + c against the exact (q - o') * s, in grid steps of position: c is rounded to
+    // an ulp of 2^23 * s, i.e. at most HALF a step; o', s and the final FMA add less than 2^-4 step for origins within
+    // a hundred scene extents.  The stored planes are therefore moved one step outward (crt_bvh_quantise).
+    CRT_DEV void init(const RayState& r, const QGrid& g)
+    {
+        sx = r.idx * g.inv_scale[0]; sy = r.idy * g.inv_scale[1]; sz = r.idz * g.inv_scale[2];
+        const float px = (r.o.x - g.gmin[0]) * g.scale[0], py = (r.o.y - g.gmin[1]) * g.scale[1], pz = (r.o.z - g.gmin[2]) * g.scale[2];
+        cx = __fmaf_rn(-8388608.f, sx, -(px * sx)); cy = __fmaf_rn(-8388608.f, sy, -(py * sy)); cz = __fmaf_rn(-8388608.f, sz, -(pz * sz));
+        nx = r.d.x >= 0.f ? 0x7610u : 0x7632u; ny = r.d.y >= 0.f ? 0x7610u : 0x7632u; nz = r.d.z >= 0.f ? 0x7610u : 0x7632u;
+        fx = nx ^ 0x0022u; fy = ny ^ 0x0022u; fz = nz ^ 0x0022u;
+    }
+};
+CRT_DEV float qplane(unsigned w, unsigned sel, float s, float c)
+{
+    unsigned f;      // prmt directly: __byte_perm would mask the selector with 0x7777 at every use
+    asm("prmt.b32 %0, %1, %2, %3;" : "=r"(f) : "r"(w), "r"(0x4B000000u), "r"(sel));
+    return __fmaf_rn(__uint_as_float(f), s, c);
+}
+// a direction component of zero: s is huge but finite (safe_rcp), both distances of that axis are huge with the right signs
+CRT_DEV int visit_qnode(const QNode* __restrict__ nodes, int idx, const RayState& r, const QRay& q, int* stack, int& sp)
+{
+    unsigned w0, w1, w2, w3, w4, w5; int ra, rb;
+    asm volatile("ld.global.nc.v8.u32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                 : "=r"(w0), "=r"(w1), "=r"(w2), "=r"(w3), "=r"(w4), "=r"(w5), "=r"(ra), "=r"(rb) : "l"(nodes + idx));
+    const float tfar = r.tfar();
+    const float tn0 = fmaxf(fmaxf(qplane(w0, q.nx, q.sx, q.cx), qplane(w1, q.ny, q.sy, q.cy)), fmaxf(qplane(w2, q.nz, q.sz, q.cz), r.tmin));
+    const float tf0 = fminf(fminf(qplane(w0, q.fx, q.sx, q.cx), qplane(w1, q.fy, q.sy, q.cy)), fminf(qplane(w2, q.fz, q.sz, q.cz), tfar));
+    const float tn1 = fmaxf(fmaxf(qplane(w3, q.nx, q.sx, q.cx), qplane(w4, q.ny, q.sy, q.cy)), fmaxf(qplane(w5, q.nz, q.sz, q.cz), r.tmin));
+    const float tf1 = fminf(fminf(qplane(w3, q.fx, q.sx, q.cx), qplane(w4, q.fy, q.sy, q.cy)), fminf(qplane(w5, q.fz, q.sz, q.cz), tfar));
+    const bool h0 = tn0 <= tf0, h1 = tn1 <= tf1;
+    if (h0 && h1) {
+        const bool swap = tn1 < tn0;
+        stack[++sp] = swap ? ra : rb;
+        return swap ? rb : ra;
+    }
+    if (h0) return ra;
+    if (h1) return rb;
+    return stack[sp--];
+}
+
 // Tests the triangles of a leaf reference (D:R10 tie-break: lower primitive id wins at equal t).
 template <bool COUNT>
-CRT_DEV void visit_leaf(const GpuTri* __restrict__ tris, int ref, RayState& r, unsigned& n_tris)
+CRT_DEV void visit_leaf(const GpuTri* __restrict__ tris, int ref, RayState& r, unsigned& n_tris, crt_hit* __restrict__ hits, int ray_idx)
 {
     const int leaf = ~ref;
     const int first = leaf >> 3, cnt = (leaf & 7) + 1;
@@ -108,19 +172,21 @@ CRT_DEV void visit_leaf(const GpuTri* __restrict__ tris, int ref, RayState& r, u
         const float4 a = make_float4(q0.min_x, q0.max_x, q0.min_y, q0.max_y), b = make_float4(q0.min_z, q0.max_z, __int_as_float(q0.ref), 0.f);
         float t, u, v;
         if (COUNT) ++n_tris;
-        if (tri_test(mk(a.x, a.y, a.z), mk(b.x, b.y, b.z), mk(c.x, c.y, c.z), r.o, r.d, r.tmin, r.tmax, t, u, v)) {
+        if (tri_test(mk(a.x, a.y, a.z), mk(b.x, b.y, b.z), mk(c.x, c.y, c.z), r.o, r.d, r.tmin, __int_as_float(0x7f800000), t, u, v)) {
+            // t < tmax and the (t, id) rule in one: best.t is the ray's tmax until a hit exists, the best t afterwards
             const int prim = __float_as_int(a.w);
-            if (r.best.prim < 0 || t < r.best.t || (t == r.best.t && prim < r.best.prim)) {
-                r.best.t = t; r.best.u = u; r.best.v = v; r.best.prim = prim;
-                r.tfar = t * 1.0000005f;
+            if (t < r.best.t || (t == r.best.t && r.best.prim >= 0 && prim < r.best.prim)) {
+                r.best.t = t; r.best.prim = prim;
+                if (!COUNT) reinterpret_cast<float4*>(hits)[ray_idx] = make_float4(t, u, v, __int_as_float(prim));
             }
         }
     }
 }
 
-CRT_DEV void store_hit(crt_hit* hits, int64_t i, const Hit& h)
+// record of a ray that hit nothing: t = the ray's tmax, prim = -1
+CRT_DEV void store_miss(crt_hit* hits, int64_t i, float tmax)
 {
-    reinterpret_cast<float4*>(hits)[i] = make_float4(h.t, h.u, h.v, __int_as_float(h.prim));
+    reinterpret_cast<float4*>(hits)[i] = make_float4(tmax, 0.f, 0.f, __int_as_float(-1));
 }
 
 // variant 0: one thread per ray, plain while-while loop (kept as the simple cross-check of the persistent kernel)
@@ -137,33 +203,32 @@ __global__ void __launch_bounds__(TRACE_BLOCK) trace_flat_kernel(const GpuNode* 
         int node = 0; unsigned dummy = 0;
         while (node != SENTINEL) {
             while ((unsigned)node < (unsigned)SENTINEL) node = visit_node(load_node(nodes, node), r, stack, sp);
-            while (node < 0) { visit_leaf<false>(tris, node, r, dummy); node = stack[sp--]; }
+            while (node < 0) { visit_leaf<false>(tris, node, r, dummy, hits, (int)i); node = stack[sp--]; }
         }
     }
-    store_hit(hits, i, r.best);
+    if (r.best.prim < 0) store_miss(hits, i, rd.w);
 }
 
 // variant 1 (default): persistent warps, per-lane dynamic ray fetch, postponed leaves.  COUNT adds work counters.
 // 9 blocks/SM (<= 56 registers, 36 warps): measured faster than 8 blocks at 64 registers and 10 blocks at 48 (profiles/).
-template <bool COUNT>
-__global__ void __launch_bounds__(TRACE_BLOCK, 9) trace_dyn_kernel(const GpuNode* __restrict__ nodes, const GpuTri* __restrict__ tris,
+template <bool COUNT, bool QN>
+__global__ void __launch_bounds__(TRACE_BLOCK, CRT_TRACE_MINB(QN)) trace_dyn_kernel(const GpuNode* __restrict__ nodes, const QNode* __restrict__ qnodes, const QGrid grid, const GpuTri* __restrict__ tris,
                                                                 const crt_ray* __restrict__ rays, crt_hit* __restrict__ hits, int64_t n,
                                                                 unsigned int* __restrict__ counter, int refill_threshold, int leaf_wait,
                                                                 unsigned long long* __restrict__ stats)
 {
     const unsigned lane = threadIdx.x & 31u;
-    const unsigned lt_mask = (1u << lane) - 1u;
     int stack[STACK_SIZE]; int sp = 0; stack[0] = SENTINEL;
     int node = SENTINEL, leaf = 0;      // leaf: postponed leaf reference (< 0) or 0 = none
     int ray_idx = -1;
     bool exhausted = false;
-    RayState r;
+    RayState r; QRay q;
     unsigned c_nodes = 0, c_tris = 0, c_rays = 0;
 
     for (;;) {
         __syncwarp();
         // ---- retire finished rays; idle lanes take the next rays in slot order (warp-wide: one atomic per round)
-        if (node == SENTINEL && ray_idx >= 0) { if (!COUNT) store_hit(hits, ray_idx, r.best); ray_idx = -1; }
+        if (node == SENTINEL && ray_idx >= 0) { if (!COUNT && r.best.prim < 0) store_miss(hits, ray_idx, r.best.t); ray_idx = -1; }
         for (;;) {
             const bool want = (node == SENTINEL) && !exhausted;
             const unsigned m = __ballot_sync(0xffffffffu, want);
@@ -173,15 +238,18 @@ __global__ void __launch_bounds__(TRACE_BLOCK, 9) trace_dyn_kernel(const GpuNode
             if ((int)lane == leader) base = atomicAdd(counter, (unsigned)__popc(m));
             base = __shfl_sync(0xffffffffu, base, leader);
             if (want) {
+                unsigned lt_mask;                                      // read where it is used: not a register held across the traversal loops
+                asm volatile("mov.u32 %0, %%lanemask_lt;" : "=r"(lt_mask));
                 const unsigned i = base + __popc(m & lt_mask);        // n < 2^31 (checked by crt_trace); the counter cannot wrap
                 if ((int64_t)i >= n) { exhausted = true; }
                 else {
                     const float4* rp = reinterpret_cast<const float4*>(rays + i);
                     const float4 rd = __ldg(rp + 1);
                     if (rd.w < 0.f) {                 // inactive slot: a miss, nothing to traverse
-                        if (!COUNT) { Hit h; h.t = rd.w; h.u = 0.f; h.v = 0.f; h.prim = -1; store_hit(hits, i, h); }
+                        if (!COUNT) store_miss(hits, i, rd.w);
                     } else {
                         r.init(__ldg(rp), rd);
+                        if (QN) q.init(r, grid);
                         ray_idx = (int)i; node = 0; leaf = 0; sp = 0;
                         if (COUNT) ++c_rays;
                     }
@@ -192,17 +260,18 @@ __global__ void __launch_bounds__(TRACE_BLOCK, 9) trace_dyn_kernel(const GpuNode
         if (__any_sync(0xffffffffu, exhausted)) refill_threshold = 0;      // nothing left to fetch: run the stragglers to the end
 
         // ---- traverse until this lane's ray ends or too few lanes of the warp are still busy
+        // (a warp-uniform formulation of these loops, every exit a full-mask vote, was measured 3-10 % slower: profiles/r01f)
         while (node != SENTINEL) {
             // inner nodes; the first leaf a lane meets is postponed so that the warp's leaves are processed together
             while ((unsigned)node < (unsigned)SENTINEL) {
                 if (COUNT) ++c_nodes;
-                node = visit_node(load_node(nodes, node), r, stack, sp);
+                node = QN ? visit_qnode(qnodes, node, r, q, stack, sp) : visit_node(load_node(nodes, node), r, stack, sp);
                 if (node < 0 && leaf == 0) { leaf = node; node = stack[sp--]; }
                 if (__popc(__ballot_sync(__activemask(), leaf == 0)) <= leaf_wait) break;   // (nearly) every converged lane holds a leaf
             }
             // leaves: the postponed one, then any further leaf references that come off the stack
             while (leaf < 0) {
-                visit_leaf<COUNT>(tris, leaf, r, c_tris);
+                visit_leaf<COUNT>(tris, leaf, r, c_tris, hits, ray_idx);
                 leaf = 0;
                 if (node < 0) { leaf = node; node = stack[sp--]; }
             }
@@ -244,18 +313,18 @@ __global__ void __launch_bounds__(256) primary_rays_kernel(CamDev cam, DevLayout
     rp[1] = make_float4(dx, dy, dz, 1e30f);
 }
 
-template <bool COUNT>
+template <bool COUNT, bool QN>
 crt_status launch_dyn(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, crt_hit* hits, unsigned long long* stats, cudaStream_t st)
 {
     int per_sm = ctx->trace_blocks_per_sm;
     if (per_sm <= 0) {
-        CRT_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, trace_dyn_kernel<COUNT>, TRACE_BLOCK, 0));
+        CRT_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, trace_dyn_kernel<COUNT, QN>, TRACE_BLOCK, 0));
         if (per_sm < 1) per_sm = 1;
     }
     CRT_CUDA(ctx, cudaMemsetAsync(ctx->d_counter, 0, sizeof(unsigned int), st));
     int64_t want = (n + TRACE_BLOCK - 1) / TRACE_BLOCK, grid = (int64_t)ctx->n_sms * per_sm;
     if (grid > want) grid = want;
-    trace_dyn_kernel<COUNT><<<(unsigned)grid, TRACE_BLOCK, 0, st>>>(bvh->d_nodes, bvh->d_tris, rays, hits, n, ctx->d_counter, ctx->trace_refill_threshold, ctx->trace_leaf_wait, stats);
+    trace_dyn_kernel<COUNT, QN><<<(unsigned)grid, TRACE_BLOCK, 0, st>>>(bvh->d_nodes, bvh->d_qnodes, bvh->qgrid, bvh->d_tris, rays, hits, n, ctx->d_counter, ctx->trace_refill_threshold, ctx->trace_leaf_wait, stats);
     CRT_CHECK_LAUNCH(ctx, "trace_dyn");
     return CRT_OK;
 }
@@ -280,7 +349,8 @@ crt_status launch_trace(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, i
         CRT_CHECK_LAUNCH(ctx, "trace_flat");
         return CRT_OK;
     }
-    return launch_dyn<false>(ctx, bvh, rays, n, hits, nullptr, st);
+    if (ctx->trace_kernel == 3) return launch_dyn<false, true>(ctx, bvh, rays, n, hits, nullptr, st);
+    return launch_dyn<false, false>(ctx, bvh, rays, n, hits, nullptr, st);
 }
 
 // counting build of the default kernel (crt_trace_stats): same traversal, no hit records written
@@ -288,7 +358,8 @@ crt_status launch_trace_stats(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* r
 {
     if (n == 0) return CRT_OK;
     if (ctx->trace_kernel == 2 && bvh->d_wnodes) return launch_trace_wide_stats(ctx, bvh, rays, n, counters, st);
-    return launch_dyn<true>(ctx, bvh, rays, n, nullptr, reinterpret_cast<unsigned long long*>(counters), st);
+    if (ctx->trace_kernel == 3) return launch_dyn<true, true>(ctx, bvh, rays, n, nullptr, reinterpret_cast<unsigned long long*>(counters), st);
+    return launch_dyn<true, false>(ctx, bvh, rays, n, nullptr, reinterpret_cast<unsigned long long*>(counters), st);
 }
 
 crt_status launch_primary(crt_ctx* ctx, const crt_bvh* bvh, const crt_camera& cam, const crt_frame& f, const Layout& L,

@@ -81,7 +81,7 @@ def test_full_size_config2_stagewise_and_sampled(crt, ctx, oracle):
 
 # ------------------------------------------------------------------ a0 / a5: BVH + traversal
 @pytest.mark.parametrize("scene_name", ["cornell", "interior_small", "landscape_small"])
-@pytest.mark.parametrize("kernel", [0, 1, 2])
+@pytest.mark.parametrize("kernel", [0, 1, 2, 3])
 def test_trace_matches_oracle_on_random_rays(crt, ctx, oracle, scene_name, kernel):
     scene = SCENES[scene_name]()
     # kernel 2 reads the 8-wide compressed layout, which exists when every leaf holds one triangle
@@ -98,7 +98,7 @@ def test_trace_matches_oracle_on_random_rays(crt, ctx, oracle, scene_name, kerne
     try:
         h = hits_np(oracle, ctx.crt_trace(G.bvh, ctx.upload(r)))
     finally:
-        ctx.crt_set_option("trace_kernel", 1)
+        ctx.crt_set_option("trace_kernel", 3)
     ho = ob.trace(r.view(oracle.RAY_DTYPE).reshape(-1))
     compare_hits(h, ho)
     # the triangle test is the same fp32 operation sequence on both sides: where ids agree the record is bit-identical
@@ -141,6 +141,41 @@ def test_trace_edge_cases(crt, ctx, oracle):
         ctx.crt_trace(G.bvh, buf[1:].view(-1)[: 100 * 8].view(100, 8))
     assert e.value.status == crt.api.CRT_ERR_INVALID_ARG
     torch.cuda.synchronize()
+
+
+@pytest.mark.parametrize("kernel", [0, 1, 3])
+def test_trace_degenerate_directions_and_far_origins(crt, ctx, oracle, kernel):
+    """The box test must stay conservative where its arithmetic degenerates: direction components that are exactly zero
+    (1/d infinite, plane distances NaN), origins exactly on box planes of the axis-aligned Cornell walls, and origins far
+    outside the scene (the 16-bit layout states about a hundred scene extents, include/crt.h).  Hits must equal the
+    all-triangles definition."""
+    scene = I.cornell()
+    G = GpuScene(crt, scene, ctx)
+    rng = np.random.default_rng(21)
+    n = 6000
+    r = np.zeros((n, 8), np.float32); r[:, 7] = 1e30
+    o = rng.random((n, 3)).astype(np.float32)
+    o[: n // 3] = np.round(o[: n // 3] * 4) / 4                       # grid points: on wall and tessellation planes
+    d = rng.normal(size=(n, 3))
+    d[0:2000:2, rng.integers(0, 3)] = 0.0                             # one zero component
+    k = rng.integers(0, 3, n)
+    ax = np.zeros((n, 3)); ax[np.arange(n), k] = rng.choice([-1.0, 1.0], n)
+    d[1:2000:2] = ax[1:2000:2]                                        # axis-aligned: two zero components
+    d /= np.linalg.norm(d, axis=1, keepdims=True)
+    far = slice(4000, n)                                              # origins 30-80 extents away, aimed at the box
+    tgt = rng.random((n, 3))
+    dirs = rng.normal(size=(n, 3)); dirs /= np.linalg.norm(dirs, axis=1, keepdims=True)
+    dist = rng.uniform(30, 80, (n, 1))
+    o64 = o.astype(np.float64); o64[far] = tgt[far] - dirs[far] * dist[far]; d[far] = dirs[far]
+    r[:, 0:3] = o64; r[:, 4:7] = d
+    ctx.crt_set_option("trace_kernel", kernel)
+    try:
+        h = hits_np(oracle, ctx.crt_trace(G.bvh, ctx.upload(r)))
+    finally:
+        ctx.crt_set_option("trace_kernel", 3)
+    hb = oracle.trace_brute(scene.verts, r.view(oracle.RAY_DTYPE).reshape(-1))
+    compare_hits(h, hb)
+    assert (hb["prim"] >= 0).mean() > 0.5
 
 
 def test_trace_stats_counts(crt, ctx, oracle):

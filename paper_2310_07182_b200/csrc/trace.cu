@@ -30,6 +30,9 @@ constexpr int TRACE_BLOCK = 128;
 // resident blocks per SM the persistent kernel is compiled for: fp32 nodes 9 (<= 56 registers), 16-bit nodes 8 (<= 64
 // registers; measured 1.5-3 % faster than 9 with this layout, profiles/r01f)
 #define CRT_TRACE_MINB(QN) ((QN) ? 8 : 9)
+#ifndef CRT_VISITS_PER_VOTE
+#define CRT_VISITS_PER_VOTE 3   // inner-node visits between two leaf-wait votes of a warp
+#endif
 
 struct ChildRegs { float min_x, max_x, min_y, max_y, min_z, max_z; int ref; };
 
@@ -147,15 +150,13 @@ CRT_DEV int visit_qnode(const QNode* __restrict__ nodes, int idx, const RayState
     const float tf0 = fminf(fminf(qplane(w0, q.fx, q.sx, q.cx), qplane(w1, q.fy, q.sy, q.cy)), fminf(qplane(w2, q.fz, q.sz, q.cz), tfar));
     const float tn1 = fmaxf(fmaxf(qplane(w3, q.nx, q.sx, q.cx), qplane(w4, q.ny, q.sy, q.cy)), fmaxf(qplane(w5, q.nz, q.sz, q.cz), r.tmin));
     const float tf1 = fminf(fminf(qplane(w3, q.fx, q.sx, q.cx), qplane(w4, q.fy, q.sy, q.cy)), fminf(qplane(w5, q.fz, q.sz, q.cz), tfar));
+    // next node without a three-way branch: the nearer hit child (the farther one pushed), else the top of the stack
     const bool h0 = tn0 <= tf0, h1 = tn1 <= tf1;
-    if (h0 && h1) {
-        const bool swap = tn1 < tn0;
-        stack[++sp] = swap ? ra : rb;
-        return swap ? rb : ra;
-    }
-    if (h0) return ra;
-    if (h1) return rb;
-    return stack[sp--];
+    const bool second = h1 && (!h0 || tn1 < tn0);          // child 1 is the one to enter
+    int next = second ? rb : ra;
+    if (h0 && h1) stack[++sp] = second ? ra : rb;
+    if (!(h0 || h1)) next = stack[sp--];
+    return next;
 }
 
 // Tests the triangles of a leaf reference (D:R10 tie-break: lower primitive id wins at equal t).
@@ -263,10 +264,15 @@ __global__ void __launch_bounds__(TRACE_BLOCK, CRT_TRACE_MINB(QN)) trace_dyn_ker
         // (a warp-uniform formulation of these loops, every exit a full-mask vote, was measured 3-10 % slower: profiles/r01f)
         while (node != SENTINEL) {
             // inner nodes; the first leaf a lane meets is postponed so that the warp's leaves are processed together
+            // (two visits per vote: the vote and its warp synchronisation cost 7 issue slots)
             while ((unsigned)node < (unsigned)SENTINEL) {
-                if (COUNT) ++c_nodes;
-                node = QN ? visit_qnode(qnodes, node, r, q, stack, sp) : visit_node(load_node(nodes, node), r, stack, sp);
-                if (node < 0 && leaf == 0) { leaf = node; node = stack[sp--]; }
+#pragma unroll
+                for (int rep = 0; rep < CRT_VISITS_PER_VOTE; ++rep) {
+                    if (rep > 0 && (unsigned)node >= (unsigned)SENTINEL) break;
+                    if (COUNT) ++c_nodes;
+                    node = QN ? visit_qnode(qnodes, node, r, q, stack, sp) : visit_node(load_node(nodes, node), r, stack, sp);
+                    if (node < 0 && leaf == 0) { leaf = node; node = stack[sp--]; }
+                }
                 if (__popc(__ballot_sync(__activemask(), leaf == 0)) <= leaf_wait) break;   // (nearly) every converged lane holds a leaf
             }
             // leaves: the postponed one, then any further leaf references that come off the stack

@@ -30,6 +30,9 @@
  *                     density D_v(h) = G1(wo) max(0, wo.h) D(h) / wo.z (Heitz 2018); weight <= 1; |wi| = 1;
  *                     white-furnace energy <= 1
  *   morton + sort     bit-by-bit loop encoder vs a python magic-mask encoder, numpy stable argsort
+ *   other sort keys   (Origin, Reis, Costa, TwoPoint; D:R19) numpy encoder, hand-derived fixture tests/golden/ray_codes.txt,
+ *                     Reis/Costa halves swapped, Origin's top levels == Reis' origin half, TwoPoint with d = 0 repeats the
+ *                     origin bits; each sort mode == numpy stable argsort of its key over the independent rays
  *   shade/accumulate  closed-form furnace (white sphere under uniform light == 1), albedo series
  */
 #include <math.h>
@@ -59,7 +62,12 @@ typedef struct { float tr, tg, tb; uint32_t flags; float lr, lg, lb; uint32_t pa
 typedef struct { float albedo[3]; float roughness; float emission[3]; int32_t type; } orc_material;
 typedef struct { int32_t w, h, spp, seed, frame; } orc_frame;
 enum { MAT_DIFFUSE = 0, MAT_GLOSSY = 1, MAT_SPECULAR = 2, MAT_EMISSIVE = 3 };
-enum { MODE_INDEPENDENT = 0, MODE_MORTON = 1, MODE_REUSE = 2, MODE_WORLD = 3 };
+enum { MODE_INDEPENDENT = 0, MODE_MORTON = 1, MODE_REUSE = 2, MODE_WORLD = 3,
+       /* further reordering baselines (D:R19): same procedure as MODE_MORTON with another sort key */
+       MODE_SORT_ORIGIN = 4, MODE_SORT_REIS = 5, MODE_SORT_COSTA = 6, MODE_SORT_TWOPOINT = 7 };
+#define IS_SORTED(m) ((m) == MODE_MORTON || ((m) >= MODE_SORT_ORIGIN && (m) <= MODE_SORT_TWOPOINT))
+/* sort key of a mode: 0 AilaCompact, 1 Origin, 2 Reis, 3 Costa, 4 TwoPoint */
+#define CODE_OF_MODE(m) ((m) == MODE_MORTON ? 0 : (m) - MODE_SORT_ORIGIN + 1)
 #define IS_GROUPED(m) ((m) == MODE_REUSE || (m) == MODE_WORLD)
 enum { CLASS_EMPTY = 0, CLASS_DIFFUSE = 1, CLASS_GLOSSY = 2, CLASS_HYBRID = 3 };
 enum { PURPOSE_CAMERA = 0, PURPOSE_BSDF = 1, PURPOSE_TILE = 2, PURPOSE_LEADER = 3 };
@@ -619,6 +627,55 @@ void orc_morton_encode(const orc_ray* rays, int64_t n, const float* bounds, uint
 {
     for (int64_t i = 0; i < n; ++i) keys[i] = orc_morton_code(&rays[i], bounds);
 }
+
+/* ---- the other sort keys of the paper's comparison (section 2.1, section 4; D:R19), all 30 bits.
+ *   1 Origin    Morton code of the ray origin alone, 10 bits per axis (x above y above z at every level)
+ *   2 Reis      "the higher bits represent the origin and subsequent bits represent the direction" [RCP17]: 15-bit
+ *               Morton code of the origin (5 bits per axis) above the 15-bit Morton code of the direction
+ *   3 Costa     "the opposite approach, where higher bits represented the direction" [CPJ15]: direction above origin
+ *   4 TwoPoint  "interleaved bits from the origin and termination point" [MBK*10, MBGB20] with the fixed-length
+ *               estimate of P:L139: end = o + (0.25 * largest extent of the scene box) * d, quantised like the origin
+ *               (clamped into the box), in AilaCompact's bit layout with the end point in place of the direction
+ * Quantisation of origin and direction components is AilaCompact's (D:R12): separate fp32 multiply and add/subtract. */
+static uint32_t quant10(real x) { real fl = rfloor_(x); int q = (fl < R(0.0)) ? 0 : ((fl > R(1023.0)) ? 1023 : (int)fl); if (x != x) q = 0; return (uint32_t)q; }
+static uint32_t morton3(uint32_t x, uint32_t y, uint32_t z, int bits)
+{
+    uint32_t c = 0;
+    for (int l = 0; l < bits; ++l)
+        c |= (((x >> l) & 1u) << (3 * l + 2)) | (((y >> l) & 1u) << (3 * l + 1)) | (((z >> l) & 1u) << (3 * l));
+    return c;
+}
+uint32_t orc_ray_code(int32_t code, const orc_ray* r, const float* bounds)
+{
+    if (code == 0) return orc_morton_code(r, bounds);
+    if (r->tmax < 0.f) return 0xFFFFFFFFu;
+    const float o[3] = { r->ox, r->oy, r->oz }, d[3] = { r->dx, r->dy, r->dz };
+    real ext[3], maxext = R(0.0);
+    for (int k = 0; k < 3; ++k) { ext[k] = R(bounds[3 + k]) - R(bounds[k]); if (ext[k] > maxext) maxext = ext[k]; }
+    uint32_t qo[3], qd[3], qe[3], qo10[3];
+    real len = R(0.25) * maxext;
+    for (int k = 0; k < 3; ++k) {
+        real scale5 = ext[k] > R(0.0) ? R(32.0) / ext[k] : R(0.0), scale10 = ext[k] > R(0.0) ? R(1024.0) / ext[k] : R(0.0);
+        qo[k] = quant5((R(o[k]) - R(bounds[k])) * scale5);
+        qo10[k] = quant10((R(o[k]) - R(bounds[k])) * scale10);
+        qd[k] = quant5((R(d[k]) + R(1.0)) * R(16.0));
+        real e = R(o[k]) + len * R(d[k]);
+        qe[k] = quant5((e - R(bounds[k])) * scale5);
+    }
+    switch (code) {
+    case 1: return morton3(qo10[0], qo10[1], qo10[2], 10);
+    case 2: return (morton3(qo[0], qo[1], qo[2], 5) << 15) | morton3(qd[0], qd[1], qd[2], 5);
+    case 3: return (morton3(qd[0], qd[1], qd[2], 5) << 15) | morton3(qo[0], qo[1], qo[2], 5);
+    default: {
+        uint32_t q[6] = { qo[0], qo[1], qo[2], qe[0], qe[1], qe[2] }, c = 0;
+        for (int l = 0; l < 5; ++l) for (int k = 0; k < 6; ++k) c |= ((q[k] >> l) & 1u) << (6 * l + (5 - k));
+        return c; }
+    }
+}
+void orc_ray_code_encode(int32_t code, const orc_ray* rays, int64_t n, const float* bounds, uint32_t* keys)
+{
+    for (int64_t i = 0; i < n; ++i) keys[i] = orc_ray_code(code, &rays[i], bounds);
+}
 typedef struct { uint32_t key; int32_t idx; } kv;
 static int kv_cmp(const void* a, const void* b)
 {
@@ -759,7 +816,7 @@ void orc_generate_secondary(const float* verts, const int32_t* mat_id, const orc
     /* 4. emit rays in slot order; throughput *= weight */
     uint32_t n_active = 0;
     orc_ray* tmp_rays = rays_out; int32_t* tmp_r2p = ray_to_path_out; int32_t* tmp_src = dir_src_out; float* tmp_loc = local_dir_out;
-    if (mode == MODE_MORTON) {
+    if (IS_SORTED(mode)) {
         tmp_rays = (orc_ray*)malloc(sizeof(orc_ray) * (size_t)L.n_slots); tmp_r2p = (int32_t*)malloc(4 * (size_t)L.n_slots);
         tmp_src = (int32_t*)malloc(4 * (size_t)L.n_slots); tmp_loc = (float*)malloc(12 * (size_t)L.n_slots);
     }
@@ -782,10 +839,10 @@ void orc_generate_secondary(const float* verts, const int32_t* mat_id, const orc
         if (tmp_loc) { tmp_loc[3 * i] = (float)q->wi.x; tmp_loc[3 * i + 1] = (float)q->wi.y; tmp_loc[3 * i + 2] = (float)q->wi.z; }
         ++n_active;
     }
-    if (mode == MODE_MORTON) {
+    if (IS_SORTED(mode)) {
         /* reordering baseline: encode, sort, permute */
         uint32_t* keys = (uint32_t*)malloc(4 * (size_t)L.n_slots); int32_t* order = (int32_t*)malloc(4 * (size_t)L.n_slots);
-        orc_morton_encode(tmp_rays, L.n_slots, bounds, keys);
+        orc_ray_code_encode(CODE_OF_MODE(mode), tmp_rays, L.n_slots, bounds, keys);
         orc_sort_keys(keys, L.n_slots, order);
         for (int64_t j = 0; j < L.n_slots; ++j) {
             int32_t i = order[j];

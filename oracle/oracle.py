@@ -18,7 +18,9 @@ RAY_DTYPE = np.dtype([("o", "<f4", 3), ("tmin", "<f4"), ("d", "<f4", 3), ("tmax"
 HIT_DTYPE = np.dtype([("t", "<f4"), ("u", "<f4"), ("v", "<f4"), ("prim", "<i4")])
 PATH_DTYPE = np.dtype([("T", "<f4", 3), ("flags", "<u4"), ("L", "<f4", 3), ("pad", "<u4")])
 MODE_INDEPENDENT, MODE_MORTON, MODE_REUSE = 0, 1, 2
-MODES = {"independent": 0, "morton_reorder": 1, "direct_reuse": 2, "world_reuse": 3}
+MODES = {"independent": 0, "morton_reorder": 1, "direct_reuse": 2, "world_reuse": 3,
+         "sort_origin": 4, "sort_reis": 5, "sort_costa": 6, "sort_twopoint": 7}
+RAY_CODES = {"aila_compact": 0, "origin": 1, "reis": 2, "costa": 3, "twopoint": 4}
 CLASS_EMPTY, CLASS_DIFFUSE, CLASS_GLOSSY, CLASS_HYBRID = 0, 1, 2, 3
 
 
@@ -175,6 +177,13 @@ def generate_secondary(scene, fr, bounce, mode, gw, gh, s, bounds, prev_rays, pr
 def morton_encode(rays, bounds):
     rays = np.ascontiguousarray(rays); keys = np.zeros(len(rays), np.uint32); bounds = _f32(bounds)
     _lib().orc_morton_encode(_p(rays), C.c_int64(len(rays)), _p(bounds), _p(keys))
+    return keys
+
+
+def ray_code_encode(code, rays, bounds):
+    """sort key of every ray for one of RAY_CODES (D:R12, R19)"""
+    rays = np.ascontiguousarray(rays); keys = np.zeros(len(rays), np.uint32); bounds = _f32(bounds)
+    _lib().orc_ray_code_encode(C.c_int32(int(code)), _p(rays), C.c_int64(len(rays)), _p(bounds), _p(keys))
     return keys
 
 

@@ -408,6 +408,77 @@ def test_morton_mode_is_a_sorted_permutation_of_independent_rays(oracle):
     assert np.array_equal(gm["paths"], gi["paths"])
 
 
+# ------------------------------------------------------------------ further reordering keys (D:R19)
+def _m3(a, b, c, bits):
+    """3D Morton code by table lookup per byte-free shifts (the oracle loops over bits)"""
+    out = np.zeros(len(a), np.int64)
+    for l in range(bits):
+        out |= (((a >> l) & 1) << (3 * l + 2)) | (((b >> l) & 1) << (3 * l + 1)) | (((c >> l) & 1) << (3 * l))
+    return out
+
+
+def test_ray_codes_against_definitions_and_relations(oracle):
+    """Origin / Reis / Costa / TwoPoint keys: an independent numpy encoder, and the relations the definitions imply:
+    Reis and Costa hold the same two 15-bit halves swapped; the top 5 levels of Origin are the origin half of Reis;
+    TwoPoint is AilaCompact's layout with the clamped end point o + 0.25*maxext*d in place of the direction, so a ray
+    of zero length direction (end = origin) repeats every origin bit."""
+    bounds = np.array([-1, 0, 2, 3, 1, 10], np.float32)              # extents 4, 1, 8: largest 8 -> length 2
+    lo, ext = bounds[:3].astype(np.float64), (bounds[3:] - bounds[:3]).astype(np.float64)
+    rays = I.random_rays(9, 4000, bounds[:3], bounds[3:], inactive_frac=0.1).view(oracle.RAY_DTYPE).reshape(-1)
+    act = rays["tmax"] >= 0
+    o, d = rays["o"].astype(np.float64), rays["d"].astype(np.float64)
+    q5 = np.clip(np.floor((o - lo) * (32 / ext)), 0, 31).astype(np.int64)
+    q10 = np.clip(np.floor((o - lo) * (1024 / ext)), 0, 1023).astype(np.int64)
+    qd = np.clip(np.floor((d + 1) * 16), 0, 31).astype(np.int64)
+    qe = np.clip(np.floor((o + 0.25 * ext.max() * d - lo) * (32 / ext)), 0, 31).astype(np.int64)
+    k = {n: oracle.ray_code_encode(c, rays, bounds).astype(np.int64) for n, c in oracle.RAY_CODES.items()}
+    for n in k:
+        assert np.all(k[n][~act] == 0xFFFFFFFF) and np.all(k[n][act] < 2**30)
+    assert np.array_equal(k["aila_compact"], oracle.morton_encode(rays, bounds))
+    mo, md = _m3(q5[:, 0], q5[:, 1], q5[:, 2], 5), _m3(qd[:, 0], qd[:, 1], qd[:, 2], 5)
+    exp = {"origin": _m3(q10[:, 0], q10[:, 1], q10[:, 2], 10), "reis": (mo << 15) | md, "costa": (md << 15) | mo,
+           "twopoint": (_spread6(q5[:, 0]) << 5) | (_spread6(q5[:, 1]) << 4) | (_spread6(q5[:, 2]) << 3)
+                       | (_spread6(qe[:, 0]) << 2) | (_spread6(qe[:, 1]) << 1) | _spread6(qe[:, 2])}
+    for n, e in exp.items():      # fp32 quantisation differs from fp64 only within an ulp of a cell edge
+        assert (k[n][act] == np.asarray(e, np.int64)[act]).mean() > 0.998, n
+    a = act
+    assert np.array_equal(k["reis"][a] >> 15, k["costa"][a] & 0x7FFF) and np.array_equal(k["reis"][a] & 0x7FFF, k["costa"][a] >> 15)
+    assert np.array_equal(k["origin"][a] >> 15, k["reis"][a] >> 15)
+    # origin bits of TwoPoint and AilaCompact sit at the same positions
+    omask = sum(0b111000 << (6 * l) for l in range(5))
+    assert np.array_equal(k["twopoint"][a] & omask, k["aila_compact"][a] & omask)
+    z = rays.copy(); z["d"] = 0
+    kz = oracle.ray_code_encode(4, z, bounds).astype(np.int64)[a]
+    assert np.array_equal((kz & omask) >> 3, kz & (omask >> 3))
+
+
+def test_ray_codes_golden(oracle):
+    """Hand-derived keys (tests/golden/ray_codes.txt)."""
+    import os
+    rows = [l for l in open(os.path.join(os.path.dirname(__file__), "golden", "ray_codes.txt")) if not l.startswith("#") and l.strip()]
+    assert len(rows) >= 8
+    for l in rows:
+        name, vals, bits, code = [p.strip() for p in l.split("|")]
+        v = [float(x) for x in vals.split()]
+        r = np.zeros(1, oracle.RAY_DTYPE); r["o"][0] = v[:3]; r["d"][0] = v[3:]; r["tmax"][0] = 1e30
+        b = "".join(bits.split())
+        assert len(b) == 30 and int(b, 2) == int(code, 16)                     # the fixture is self-consistent
+        got = int(oracle.ray_code_encode(oracle.RAY_CODES[name], r, np.array([0, 0, 0, 1, 1, 1], np.float32))[0])
+        assert got == int(code, 16), (name, l)
+
+
+@pytest.mark.parametrize("mode_name,code", [("sort_origin", 1), ("sort_reis", 2), ("sort_costa", 3), ("sort_twopoint", 4)])
+def test_sort_modes_are_sorted_permutations_of_independent_rays(oracle, mode_name, code):
+    sc = I.interior(n_boxes=40, n_spheres=10, subdiv=2, width=48, height=32)
+    gm = _first_bounce(oracle, sc, oracle.MODES[mode_name]); gi = _first_bounce(oracle, sc, M_IND)
+    perm = gm["ray_to_path"]
+    assert np.array_equal(np.sort(perm), np.arange(sc.width * sc.height))
+    assert np.array_equal(gm["rays"], gi["rays"][perm])
+    keys_by_path = oracle.ray_code_encode(code, gi["rays"], gm["bvh"].info()["bounds"])
+    assert np.array_equal(perm, np.argsort(keys_by_path, kind="stable"))       # stable ascending sort of the mode's own key
+    assert gm["n_active"] == gi["n_active"] and np.array_equal(gm["paths"], gi["paths"])
+
+
 # ------------------------------------------------------------------ shading / accumulation
 @pytest.mark.parametrize("mode", [M_IND, M_MOR, M_REUSE])
 @pytest.mark.parametrize("mat", [I.MAT_DIFFUSE, I.MAT_SPECULAR])

@@ -239,6 +239,9 @@ def run_cuda(args):
     modes["independent"] = time_mode("independent")
     modes["morton_reorder"] = time_mode("morton_reorder")
     modes["world_reuse"] = time_mode("world_reuse")       # the paper's first variant, an ablation: biased, see DESIGN.md D:R18
+    if not args.no_sort_codes:                            # the paper's other reordering baselines (Table 1; D:R19)
+        for m in ("sort_origin", "sort_reis", "sort_costa", "sort_twopoint"):
+            modes[m] = time_mode(m)
     e2e = time_mode("direct_reuse", host=True)
     clk = clocks.stop()
 
@@ -368,6 +371,7 @@ def main():
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--workload", default="interior", choices=sorted(WORKLOADS))
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-sort-codes", action="store_true", help="skip the Origin / Reis / Costa / TwoPoint reordering baselines")
     ap.add_argument("--sweep", nargs="?", const="config3", default=None, choices=["config3", "table3"],
                     help="config3: BASELINE config 3 sweep; table3: the paper's Table 3 shapes (tile x K) at 1920x1080, 1 spp, 2 bounces")
     ap.add_argument("--sweep-frames", type=int, default=64)

@@ -47,7 +47,14 @@ typedef enum {
 /* CRT_MODE_WORLD_REUSE: the paper's first variant, "Direct Direction Reusing" in WORLD space (section 3.1; D:R18): same
  * groups and slot order as CRT_MODE_DIRECT_REUSE, but the selected pixel's world direction is shared as is; members for which
  * it lies below the horizon end (the artifact of Fig. 1).  Kept as the ablation the paper argues from, not as the method. */
-typedef enum { CRT_MODE_INDEPENDENT = 0, CRT_MODE_MORTON_REORDER = 1, CRT_MODE_DIRECT_REUSE = 2, CRT_MODE_WORLD_REUSE = 3 } crt_mode;
+/* CRT_MODE_SORT_*: the other reordering baselines of the paper's comparison (section 2.1, section 4; D:R19): the same
+ * procedure as CRT_MODE_MORTON_REORDER (independent rays, stable radix sort by a 30-bit key, permute) with another key:
+ * ORIGIN = Morton code of the origin, 10 bits per axis; REIS = 15-bit origin code above 15-bit direction code [RCP17]; COSTA = direction
+ * above origin [CPJ15]; TWOPOINT = origin and end point o + 0.25 * (largest scene extent) * d interleaved [MBGB20, fixed length]. */
+typedef enum { CRT_MODE_INDEPENDENT = 0, CRT_MODE_MORTON_REORDER = 1, CRT_MODE_DIRECT_REUSE = 2, CRT_MODE_WORLD_REUSE = 3,
+               CRT_MODE_SORT_ORIGIN = 4, CRT_MODE_SORT_REIS = 5, CRT_MODE_SORT_COSTA = 6, CRT_MODE_SORT_TWOPOINT = 7 } crt_mode;
+/* sort keys for crt_ray_code_encode (crt_morton_encode = AILA_COMPACT) */
+typedef enum { CRT_CODE_AILA_COMPACT = 0, CRT_CODE_ORIGIN = 1, CRT_CODE_REIS = 2, CRT_CODE_COSTA = 3, CRT_CODE_TWOPOINT = 4 } crt_ray_code;
 typedef enum { CRT_MAT_DIFFUSE = 0, CRT_MAT_GLOSSY = 1, CRT_MAT_SPECULAR = 2, CRT_MAT_EMISSIVE = 3 } crt_mat_type;
 typedef enum { CRT_CLASS_EMPTY = 0, CRT_CLASS_DIFFUSE = 1, CRT_CLASS_GLOSSY = 2, CRT_CLASS_HYBRID = 3 } crt_group_class;
 
@@ -159,6 +166,8 @@ size_t crt_generate_secondary_scratch_bytes(const crt_frame* frame, const crt_or
 /* Parts of morton_reorder, exported for testing and timing (P:L43 [AK10]; D:R12).
  * keys[i] = 30-bit interleaved origin+direction code of rays[i] inside bvh bounds, 0xFFFFFFFF if inactive. */
 crt_status crt_morton_encode(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, uint32_t* keys, void* stream);
+/* The same for any of the sort keys above (code: crt_ray_code; out of range -> CRT_ERR_INVALID_ARG). */
+crt_status crt_ray_code_encode(crt_ctx* ctx, const crt_bvh* bvh, int32_t code, const crt_ray* rays, int64_t n, uint32_t* keys, void* stream);
 /* Stable LSD radix sort of (key, value) pairs, 4 passes of 8 bits, hand-written (no CUB).  All [device];
  * keys_in/vals_in are left intact; scratch >= crt_radix_sort_scratch_bytes(n). */
 crt_status crt_radix_sort_pairs(crt_ctx* ctx, const uint32_t* keys_in, const int32_t* vals_in, int64_t n,

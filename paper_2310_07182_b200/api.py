@@ -22,7 +22,9 @@ import torch
 from . import build as _build
 
 MODE_INDEPENDENT, MODE_MORTON_REORDER, MODE_DIRECT_REUSE = 0, 1, 2
-MODES = {"independent": 0, "morton_reorder": 1, "direct_reuse": 2, "world_reuse": 3}
+MODES = {"independent": 0, "morton_reorder": 1, "direct_reuse": 2, "world_reuse": 3,
+         "sort_origin": 4, "sort_reis": 5, "sort_costa": 6, "sort_twopoint": 7}
+RAY_CODES = {"aila_compact": 0, "origin": 1, "reis": 2, "costa": 3, "twopoint": 4}
 CRT_OK, CRT_ERR_INVALID_ARG, CRT_ERR_UNSUPPORTED, CRT_ERR_CUDA, CRT_ERR_STATE, CRT_ERR_NOMEM = range(6)
 STATUS_NAMES = ["CRT_OK", "CRT_ERR_INVALID_ARG", "CRT_ERR_UNSUPPORTED", "CRT_ERR_CUDA", "CRT_ERR_STATE", "CRT_ERR_NOMEM"]
 
@@ -31,7 +33,7 @@ EXPORTS = [
     "crt_create", "crt_destroy", "crt_last_error", "crt_set_option", "crt_measure_peaks",
     "crt_build_bvh", "crt_bvh_destroy", "crt_bvh_get_info", "crt_bvh_check", "crt_layout", "crt_paths_init",
     "crt_trace_primary", "crt_generate_secondary", "crt_generate_secondary_scratch_bytes",
-    "crt_morton_encode", "crt_radix_sort_pairs", "crt_radix_sort_scratch_bytes", "crt_trace", "crt_trace_stats",
+    "crt_morton_encode", "crt_ray_code_encode", "crt_radix_sort_pairs", "crt_radix_sort_scratch_bytes", "crt_trace", "crt_trace_stats",
     "crt_shade_accumulate", "crt_render_frame", "crt_frame_workspace_bytes", "crt_frame_times",
     "crt_render_frame_host", "crt_frame_host_extra_bytes",
 ]
@@ -266,6 +268,11 @@ class Context:
     def crt_morton_encode(self, bvh, rays, stream=None):
         keys = self.empty((rays.shape[0],), torch.int32)
         self._check(lib().crt_morton_encode(self.handle, bvh.handle, _ptr(rays), C.c_int64(rays.shape[0]), _ptr(keys), _stream(stream)))
+        return keys
+
+    def crt_ray_code_encode(self, bvh, code, rays, stream=None):
+        keys = self.empty((rays.shape[0],), torch.int32)
+        self._check(lib().crt_ray_code_encode(self.handle, bvh.handle, C.c_int32(int(code)), _ptr(rays), C.c_int64(rays.shape[0]), _ptr(keys), _stream(stream)))
         return keys
 
     def crt_radix_sort_pairs(self, keys, vals, stream=None):

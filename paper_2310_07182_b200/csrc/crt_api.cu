@@ -28,7 +28,7 @@ crt_status crt_make_layout(crt_ctx* ctx, const crt_frame* f, const crt_order* o,
 {
     if (!f || !o || !L) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "layout: null argument");
     if (f->w < 0 || f->h < 0 || f->spp < 1) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "layout: bad frame %dx%d spp %d", f->w, f->h, f->spp);
-    if (o->mode < 0 || o->mode > 3) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "layout: mode %d out of range", o->mode);
+    if (o->mode < 0 || o->mode > CRT_MODE_SORT_TWOPOINT) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "layout: mode %d out of range", o->mode);
     memset(L, 0, sizeof *L);
     L->w = f->w; L->h = f->h; L->spp = f->spp; L->mode = o->mode;
     L->n_paths = (int64_t)f->spp * f->w * f->h;
@@ -264,7 +264,18 @@ crt_status crt_morton_encode(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* ra
     if (n < 0) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "morton_encode: negative size");
     if (n == 0) return CRT_OK;
     NEED_ALIGNED("morton_encode", rays, 32); NEED_ALIGNED("morton_encode", keys, 4);
-    return launch_morton_encode(ctx, bvh->bounds, rays, n, keys, (cudaStream_t)stream);
+    return launch_morton_encode(ctx, bvh->bounds, 0, rays, n, keys, (cudaStream_t)stream);
+}
+
+crt_status crt_ray_code_encode(crt_ctx* ctx, const crt_bvh* bvh, int32_t code, const crt_ray* rays, int64_t n, uint32_t* keys, void* stream)
+{
+    NEED_CTX("ray_code_encode");
+    if (!bvh) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "ray_code_encode: bvh is null");
+    if (code < 0 || code > CRT_CODE_TWOPOINT) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "ray_code_encode: code %d out of range", code);
+    if (n < 0) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "ray_code_encode: negative size");
+    if (n == 0) return CRT_OK;
+    NEED_ALIGNED("ray_code_encode", rays, 32); NEED_ALIGNED("ray_code_encode", keys, 4);
+    return launch_morton_encode(ctx, bvh->bounds, code, rays, n, keys, (cudaStream_t)stream);
 }
 
 size_t crt_radix_sort_scratch_bytes(int64_t n) { return n < 0 ? 0 : radix_sort_scratch_bytes(n); }
@@ -373,7 +384,7 @@ crt_status crt_render_frame(crt_ctx* ctx, const crt_bvh* bvh, const crt_scene_ma
     int cur = 0;
     for (int b = 1; b <= n_bounces; ++b) {
         cudaEvent_t ev4[2] = {nullptr, nullptr};
-        if (record_times && L.mode == CRT_MODE_MORTON_REORDER) {
+        if (record_times && crt_mode_sorts(L.mode)) {
             // events bracketing encode+sort+permute inside generate
             while (ctx->ev.size() < (size_t)ctx->ev_used + 2) { cudaEvent_t e; CRT_CUDA(ctx, cudaEventCreate(&e)); ctx->ev.push_back(e); ctx->ev_stage.push_back(-1); }
             ev4[0] = ctx->ev[ctx->ev_used]; ctx->ev_stage[ctx->ev_used++] = -2;     // after the generate kernel: opens stage 4

@@ -93,12 +93,44 @@ CRT_DEV uint32_t spread5(uint32_t v)   // bit l of v -> bit 6*l
 {
     return (v & 1u) | ((v & 2u) << 5) | ((v & 4u) << 10) | ((v & 8u) << 15) | ((v & 16u) << 20);
 }
-struct Bounds6 { float lo[3], scale[3]; };
+struct Bounds6 { float lo[3], scale[3]; float len; };   // scale = 32 / extent; len = 0.25 * largest extent (TwoPoint)
 CRT_DEV uint32_t morton_code(const Bounds6& B, float ox, float oy, float oz, float dx, float dy, float dz)
 {
     uint32_t qx = quant5(mul(sub(ox, B.lo[0]), B.scale[0])), qy = quant5(mul(sub(oy, B.lo[1]), B.scale[1])), qz = quant5(mul(sub(oz, B.lo[2]), B.scale[2]));
     uint32_t px = quant5(mul(add(dx, 1.0f), 16.0f)), py = quant5(mul(add(dy, 1.0f), 16.0f)), pz = quant5(mul(add(dz, 1.0f), 16.0f));
     return (spread5(qx) << 5) | (spread5(qy) << 4) | (spread5(qz) << 3) | (spread5(px) << 2) | (spread5(py) << 1) | spread5(pz);
+}
+
+// The other sort keys of the paper's comparison (D:R19): 1 Origin (10 bits per origin axis), 2 Reis (origin Morton
+// code above direction Morton code), 3 Costa (direction above origin), 4 TwoPoint (origin and fixed-length end point interleaved).
+CRT_DEV uint32_t quant10(float x)
+{
+    float fl = floorf(x);
+    int q = (fl < 0.0f) ? 0 : ((fl > 1023.0f) ? 1023 : (int)fl);
+    if (x != x) q = 0;
+    return (uint32_t)q;
+}
+CRT_DEV uint32_t spread3(uint32_t v)   // bit l of v -> bit 3*l (10 bits)
+{
+    v = (v | (v << 16)) & 0x030000FFu; v = (v | (v << 8)) & 0x0300F00Fu; v = (v | (v << 4)) & 0x030C30C3u; v = (v | (v << 2)) & 0x09249249u;
+    return v;
+}
+CRT_DEV uint32_t morton3(uint32_t x, uint32_t y, uint32_t z) { return (spread3(x) << 2) | (spread3(y) << 1) | spread3(z); }
+CRT_DEV uint32_t ray_code(int code, const Bounds6& B, float ox, float oy, float oz, float dx, float dy, float dz)
+{
+    if (code == 0) return morton_code(B, ox, oy, oz, dx, dy, dz);
+    const float rx = sub(ox, B.lo[0]), ry = sub(oy, B.lo[1]), rz = sub(oz, B.lo[2]);
+    if (code == 1)      // 1024 / extent == 32 * (32 / extent) exactly
+        return morton3(quant10(mul(rx, mul(B.scale[0], 32.0f))), quant10(mul(ry, mul(B.scale[1], 32.0f))), quant10(mul(rz, mul(B.scale[2], 32.0f))));
+    const uint32_t qx = quant5(mul(rx, B.scale[0])), qy = quant5(mul(ry, B.scale[1])), qz = quant5(mul(rz, B.scale[2]));
+    if (code == 4) {
+        const float ex = add(ox, mul(B.len, dx)), ey = add(oy, mul(B.len, dy)), ez = add(oz, mul(B.len, dz));
+        const uint32_t px = quant5(mul(sub(ex, B.lo[0]), B.scale[0])), py = quant5(mul(sub(ey, B.lo[1]), B.scale[1])), pz = quant5(mul(sub(ez, B.lo[2]), B.scale[2]));
+        return (spread5(qx) << 5) | (spread5(qy) << 4) | (spread5(qz) << 3) | (spread5(px) << 2) | (spread5(py) << 1) | spread5(pz);
+    }
+    const uint32_t mo = morton3(qx, qy, qz);
+    const uint32_t md = morton3(quant5(mul(add(dx, 1.0f), 16.0f)), quant5(mul(add(dy, 1.0f), 16.0f)), quant5(mul(add(dz, 1.0f), 16.0f)));
+    return code == 2 ? ((mo << 15) | md) : ((md << 15) | mo);
 }
 
 struct GenArgs {
@@ -107,7 +139,7 @@ struct GenArgs {
     crt_ray* rays_out; int32_t* r2p_out; int32_t* gid_out; int32_t* src_out; uint8_t* cls_out; uint32_t* n_active;
     uint32_t* keys_out;      // morton mode: key per path (rays_out etc. are then the by-path temporaries)
     Bounds6 bounds;
-    int64_t n_slots; int32_t bounce; int32_t morton;
+    int64_t n_slots; int32_t bounce; int32_t morton;   // morton: 0 = no key, else 1 + sort code
     int32_t world;           // direct_reuse in WORLD space (mode 3; D:R18)
     int32_t fuse_shade;      // crt_render_frame: shade the previous segment here (same arithmetic as shade_kernel) instead of in its own pass
     float env[6];
@@ -299,19 +331,19 @@ __global__ void __launch_bounds__(1024) generate_kernel(GenArgs A, DevLayout L)
         rp[0] = r0; rp[1] = r1;
         A.r2p_out[o] = p;
         A.src_out[o] = emit ? src : -1;
-        if (A.morton) A.keys_out[o] = emit ? morton_code(A.bounds, r0.x, r0.y, r0.z, r1.x, r1.y, r1.z) : 0xFFFFFFFFu;
+        if (A.morton) A.keys_out[o] = emit ? ray_code(A.morton - 1, A.bounds, r0.x, r0.y, r0.z, r1.x, r1.y, r1.z) : 0xFFFFFFFFu;
         else A.gid_out[o] = REUSE ? (int32_t)group : p;
     }
     const unsigned m = __ballot_sync(__activemask(), emit);
     if (emit && (threadIdx.x & 31) == (__ffs(m) - 1)) atomicAdd(A.n_active, (unsigned)__popc(m));
 }
 
-__global__ void morton_encode_kernel(Bounds6 B, const crt_ray* __restrict__ rays, int64_t n, uint32_t* __restrict__ keys)
+__global__ void morton_encode_kernel(Bounds6 B, int code, const crt_ray* __restrict__ rays, int64_t n, uint32_t* __restrict__ keys)
 {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     const float4 a = __ldg(reinterpret_cast<const float4*>(rays + i)), b = __ldg(reinterpret_cast<const float4*>(rays + i) + 1);
-    keys[i] = b.w < 0.f ? 0xFFFFFFFFu : morton_code(B, a.x, a.y, a.z, b.x, b.y, b.z);
+    keys[i] = b.w < 0.f ? 0xFFFFFFFFu : ray_code(code, B, a.x, a.y, a.z, b.x, b.y, b.z);
 }
 
 // rays_out[j] = tmp[perm[j]] etc.
@@ -331,7 +363,9 @@ __global__ void permute_kernel(const int32_t* __restrict__ perm, const crt_ray* 
 Bounds6 make_bounds(const float* b)
 {
     Bounds6 B;
-    for (int k = 0; k < 3; ++k) { B.lo[k] = b[k]; float ext = b[3 + k] - b[k]; B.scale[k] = ext > 0.f ? 32.0f / ext : 0.f; }
+    float maxext = 0.f;
+    for (int k = 0; k < 3; ++k) { B.lo[k] = b[k]; float ext = b[3 + k] - b[k]; B.scale[k] = ext > 0.f ? 32.0f / ext : 0.f; if (ext > maxext) maxext = ext; }
+    B.len = 0.25f * maxext;
     return B;
 }
 
@@ -341,15 +375,15 @@ inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
 size_t generate_scratch_bytes(const Layout& L)
 {
-    if (L.mode != CRT_MODE_MORTON_REORDER) return 256;
+    if (!crt_mode_sorts(L.mode)) return 256;
     const size_t n = (size_t)L.n_slots;
     return align256(n * sizeof(crt_ray)) + 5 * align256(n * 4) + align256(radix_sort_scratch_bytes(L.n_slots)) + 256;
 }
 
-crt_status launch_morton_encode(crt_ctx* ctx, const float* bounds, const crt_ray* rays, int64_t n, uint32_t* keys, cudaStream_t st)
+crt_status launch_morton_encode(crt_ctx* ctx, const float* bounds, int code, const crt_ray* rays, int64_t n, uint32_t* keys, cudaStream_t st)
 {
     if (n == 0) return CRT_OK;
-    morton_encode_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(make_bounds(bounds), rays, n, keys);
+    morton_encode_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(make_bounds(bounds), code, rays, n, keys);
     CRT_CHECK_LAUNCH(ctx, "morton_encode");
     return CRT_OK;
 }
@@ -383,7 +417,7 @@ crt_status launch_generate(crt_ctx* ctx, const crt_bvh* bvh, const crt_scene_mat
         CRT_CHECK_LAUNCH(ctx, "generate<independent>");
         return CRT_OK;
     }
-    // morton_reorder: independent rays by path id into scratch, with their codes; stable sort of (code, path); permute
+    // morton_reorder and the other sort modes: independent rays by path id into scratch, with their keys; stable sort of (key, path); permute
     char* s = static_cast<char*>(scratch);
     crt_ray* tmp_rays = reinterpret_cast<crt_ray*>(s); s += align256((size_t)n * sizeof(crt_ray));
     int32_t* tmp_src = reinterpret_cast<int32_t*>(s); s += align256((size_t)n * 4);
@@ -391,7 +425,7 @@ crt_status launch_generate(crt_ctx* ctx, const crt_bvh* bvh, const crt_scene_mat
     int32_t* idx = reinterpret_cast<int32_t*>(s); s += align256((size_t)n * 4);
     uint32_t* keys2 = reinterpret_cast<uint32_t*>(s); s += align256((size_t)n * 4);
     int32_t* perm = reinterpret_cast<int32_t*>(s); s += align256((size_t)n * 4);
-    A.rays_out = tmp_rays; A.src_out = tmp_src; A.keys_out = keys; A.morton = 1;
+    A.rays_out = tmp_rays; A.src_out = tmp_src; A.keys_out = keys; A.morton = 1 + crt_mode_sort_code(L.mode);
     A.r2p_out = idx;        // idx[p] = p
     generate_kernel<false><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(A, D);
     CRT_CHECK_LAUNCH(ctx, "generate<morton>");

@@ -10,7 +10,8 @@ from pipeline import GpuScene, compare_hits, compare_rays, hits_np, oracle_frame
 
 pytestmark = pytest.mark.gpu
 
-MODES = {"independent": 0, "morton_reorder": 1, "direct_reuse": 2, "world_reuse": 3}
+MODES = {"independent": 0, "morton_reorder": 1, "direct_reuse": 2, "world_reuse": 3,
+         "sort_origin": 4, "sort_reis": 5, "sort_costa": 6, "sort_twopoint": 7}
 
 
 @pytest.fixture(scope="module")
@@ -219,6 +220,11 @@ GEN_CASES = [
     ("cornell", "direct_reuse", 4, 4, 2, 64, 64, 1),          # BASELINE config 1
     ("interior_small", "independent", 1, 1, 1, 96, 64, 1),
     ("interior_small", "morton_reorder", 1, 1, 1, 96, 64, 2),
+    ("interior_small", "sort_origin", 1, 1, 1, 96, 64, 1),     # the paper's other reordering keys (D:R19)
+    ("interior_small", "sort_reis", 1, 1, 1, 96, 64, 2),
+    ("interior_small", "sort_costa", 1, 1, 1, 96, 64, 1),
+    ("interior_small", "sort_twopoint", 1, 1, 1, 96, 64, 2),
+    ("landscape_small", "sort_twopoint", 1, 1, 1, 96, 64, 1),
     ("interior_small", "direct_reuse", 4, 4, 4, 96, 64, 1),   # config 2's grouping, partial tiles (96x64 vs 16x16: exact) ...
     ("interior_small", "direct_reuse", 2, 2, 8, 90, 61, 2),   # ... and ragged ones with 2 spp
     ("interior_small", "direct_reuse", 8, 8, 1, 96, 64, 1),   # stride 1: one group per tile, K = 64 (two warps per group)
@@ -270,6 +276,23 @@ def test_generate_stagewise_matches_oracle(crt, ctx, oracle, scene_name, mode, g
         assert np.allclose(pg["T"], po["T"], rtol=1e-6, atol=0)
     if scene_name == "checker" and gw * gh > 1 and mode == "direct_reuse":
         assert saw_hybrid
+
+
+def test_ray_code_encode_bit_exact(crt, ctx, oracle):
+    """Origin / Reis / Costa / TwoPoint keys (D:R19) against the oracle, bit for bit; rays reach outside the scene box so the
+    clamps of origin and end point are exercised; code out of range is rejected."""
+    scene = _small_interior()
+    G = GpuScene(crt, scene, ctx)
+    b = G.bvh.info()["bounds"]
+    r = I.random_rays(17, 50021, b[:3], b[3:], inactive_frac=0.1)
+    for name, code in crt.api.RAY_CODES.items():
+        keys = ctx.crt_ray_code_encode(G.bvh, code, ctx.upload(r)).cpu().numpy().view(np.uint32)
+        ko = oracle.ray_code_encode(oracle.RAY_CODES[name], r.view(oracle.RAY_DTYPE).reshape(-1), b)
+        assert np.array_equal(keys, ko), name
+    assert np.array_equal(ctx.crt_ray_code_encode(G.bvh, 0, ctx.upload(r)).cpu().numpy(), ctx.crt_morton_encode(G.bvh, ctx.upload(r)).cpu().numpy())
+    with pytest.raises(crt.CrtError) as e:
+        ctx.crt_ray_code_encode(G.bvh, 5, ctx.upload(r))
+    assert e.value.status == crt.api.CRT_ERR_INVALID_ARG
 
 
 def test_morton_encode_and_radix_sort_bit_exact(crt, ctx, oracle):
@@ -356,7 +379,8 @@ def test_config1_end_to_end(crt, ctx, oracle, mode, gw, gh, s):
     assert np.array_equal(acc_h, accum.cpu().numpy()) and nsec_h[0] == g["n_active"]
 
 
-@pytest.mark.parametrize("mode,gw,gh,s", [("independent", 1, 1, 1), ("morton_reorder", 1, 1, 1), ("direct_reuse", 4, 4, 4), ("direct_reuse", 8, 8, 2), ("world_reuse", 4, 4, 4)])
+@pytest.mark.parametrize("mode,gw,gh,s", [("independent", 1, 1, 1), ("morton_reorder", 1, 1, 1), ("direct_reuse", 4, 4, 4), ("direct_reuse", 8, 8, 2), ("world_reuse", 4, 4, 4),
+                                          ("sort_reis", 1, 1, 1), ("sort_twopoint", 1, 1, 1)])
 def test_mixed_materials_two_bounces_end_to_end(crt, ctx, oracle, mode, gw, gh, s):
     import torch
     scene = _small_interior()
@@ -396,7 +420,7 @@ def test_argument_errors(crt, ctx):
         crt.crt_layout(fr, crt.make_order("direct_reuse", 16, 16, 8))
     assert e.value.status == crt.api.CRT_ERR_UNSUPPORTED
     with pytest.raises(crt.CrtError) as e:
-        crt.crt_layout(fr, crt.make_order(5))
+        crt.crt_layout(fr, crt.make_order(8))
     assert e.value.status == crt.api.CRT_ERR_INVALID_ARG
     order = crt.make_order("independent")
     rays, hits, r2p = ctx.crt_trace_primary(G.bvh, G.camera, fr, order)

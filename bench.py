@@ -36,20 +36,22 @@ WORKLOADS = {
 # FLOPs of the traversal kernel per unit of work, counted from csrc/trace.cu: a node visit tests two
 # child boxes = 12 (subtract, multiply) pairs + 2 inflations = 26 flop (min/max/compare are not flops); a triangle test
 # (Moller-Trumbore as written in crt_device.cuh) = 2 cross (9 each) + 4 dot (5 each) + 1 subtract-vector (3) + 1 reciprocal (1)
-# + 3 scalings (3) + 1 add (1) = 46 flop.  Ray setup (3 reciprocals) is 3 flop per ray.
-FLOP_PER_NODE_VISIT, FLOP_PER_TRI_TEST, FLOP_PER_RAY = 26.0, 46.0, 3.0
+# + 3 scalings (3) + 1 add (1) = 46 flop.  Ray setup of the 16-bit-node kernel: 3 reciprocals, 3 scalings of them, origin into grid
+# units (3 subtract + 3 multiply), 3 x (multiply + FMA) for the plane constants = 21 flop per ray.  (A node visit of the 16-bit
+# layout is the same 12 FMA + the prune-bound multiply; the PRMT plane decode is not a flop.)
+FLOP_PER_NODE_VISIT, FLOP_PER_TRI_TEST, FLOP_PER_RAY = 26.0, 46.0, 21.0
 # nominal FP32 peak from the guide's unit counts: 148 SMs x 128 FP32 lanes x 2 flop (FMA) x 1.965 GHz (B200_PROFILING.md table)
 FP32_PEAK_TFLOPS_NOMINAL = 148 * 128 * 2 * 1.965e9 / 1e12
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the secondary trace kernel, from profiles/ (ncu --set full);
 # keyed by workload; None until captured.
-TRACE_DRAM_TRAFFIC = {"interior": 129.5e6, "landscape": 108.0e6, "cornell": None}     # profiles/r01d_final_state.md (mean of the two captured launches)
-# what ncu shows to be the kernel's limiter (not modelled by the two-term roofline): profiles/r01a, r01b
-TRACE_LIMITER = {"interior": {"unit": "l1tex data pipe", "l1tex__data_pipe_lsu_wavefronts_pct_of_peak": 81.0, "issue_slots_busy_pct": 62.0,
-                              "active_threads_per_warp_instruction": 15.0, "alu_pipe_pct": 52.0, "fma_pipe_pct": 20.0, "dram_pct": 1.5,
-                              "source": "profiles/r01d_final_state.md"},
-                 "landscape": {"unit": "l1tex data pipe", "l1tex__data_pipe_lsu_wavefronts_pct_of_peak": 71.0, "issue_slots_busy_pct": 64.0,
-                               "active_threads_per_warp_instruction": 16.7, "alu_pipe_pct": 56.0, "fma_pipe_pct": 19.0, "dram_pct": 3.0,
-                               "source": "profiles/r01d_final_state.md (bounce 1; bounce 2 has 0.4 M live rays and is latency-bound)"}}
+TRACE_DRAM_TRAFFIC = {"interior": 119.5e6, "landscape": 103.6e6, "cornell": None}     # profiles/r01f_q16_nodes.md (mean of the two captured launches)
+# what ncu shows to be the kernel's limiter (not modelled by the two-term roofline): profiles/r01f (r01a-r01d: the L1 data pipe, before the 16-bit nodes)
+TRACE_LIMITER = {"interior": {"unit": "instruction issue at 50 % lane utilisation", "issue_slots_busy_pct": 67.0, "active_threads_per_warp_instruction": 16.3,
+                              "alu_pipe_pct": 58.0, "fma_pipe_pct": 27.0, "l1tex__data_pipe_lsu_wavefronts_pct_of_peak": 56.0, "dram_pct": 1.5,
+                              "source": "profiles/r01f_q16_nodes.md"},
+                 "landscape": {"unit": "instruction issue at 50 % lane utilisation", "issue_slots_busy_pct": 69.0, "active_threads_per_warp_instruction": 17.3,
+                               "alu_pipe_pct": 62.0, "fma_pipe_pct": 25.0, "l1tex__data_pipe_lsu_wavefronts_pct_of_peak": 50.0, "dram_pct": 3.0,
+                               "source": "profiles/r01f_q16_nodes.md (bounce 1; bounce 2 has 0.4 M live rays and is latency-bound)"}}
 
 
 def _peaks():

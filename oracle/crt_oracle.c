@@ -392,7 +392,7 @@ void orc_trace(const orc_bvh* b, const orc_ray* rays, int64_t n_rays, orc_hit* h
 /* ------------------------------------------------------------------ partition (D:R3-R5)
  * BASELINE.json's "group gw x gh, interleave stride s"  <->  the paper's tile W x H and
  * group size K:  K = gw*gh, W = gw*s, H = gh*s, M = W*H slots per tile, G = M/K groups. */
-typedef struct { int32_t W, H, M, K, G, tiles_x, tiles_y, n_tiles; int64_t n_slots, n_paths; } layout;
+typedef struct { int32_t W, H, M, K, G, tiles_x, tiles_y, n_tiles; int64_t n_slots, n_paths; int32_t gw, gh, sx, sy, lattice; } layout;
 static layout make_layout(const orc_frame* f, int mode, int gw, int gh, int s)
 {
     layout L; memset(&L, 0, sizeof L);
@@ -401,7 +401,8 @@ static layout make_layout(const orc_frame* f, int mode, int gw, int gh, int s)
     /* the paper's native parametrisation is a W x H tile and a group size K (tile 8x8, K = 8).  Any power-of-two
      * (W, H, K) is gw = min(K, W), gh = K / gw with separate horizontal / vertical strides W / gw, H / gh; the vertical
      * stride travels in the high 16 bits of s (0 = same as the horizontal one).  DESIGN.md D:R5. */
-    int32_t sx = s & 0xffff, sy = (s >> 16) ? (s >> 16) : sx;
+    int32_t sx = s & 0x3fff, sy = (s >> 16) ? (s >> 16) : sx;
+    L.gw = gw; L.gh = gh; L.sx = sx; L.sy = sy; L.lattice = (s >> 14) & 1;      /* bit 14: partition rule LATTICE (D:R20) */
     L.W = gw * sx; L.H = gh * sy; L.M = L.W * L.H; L.K = gw * gh; L.G = L.M / L.K;
     L.tiles_x = (f->w + L.W - 1) / L.W; L.tiles_y = (f->h + L.H - 1) / L.H; L.n_tiles = L.tiles_x * L.tiles_y;
     L.n_slots = (int64_t)f->spp * L.n_tiles * L.M;
@@ -419,6 +420,12 @@ static void tile_lcg(const orc_frame* f, const layout* L, int32_t tile, int32_t 
     *a = (r[0] % (uint32_t)L->M) | 1u;
     *c = r[1] % (uint32_t)L->M;
 }
+static void tile_raw(const orc_frame* f, int32_t tile, int32_t sample, uint32_t* r0, uint32_t* r1)
+{
+    uint32_t r[4];
+    orc_philox((uint32_t)tile, (uint32_t)sample, 0u, PURPOSE_TILE, (uint32_t)f->seed, (uint32_t)f->frame, r);
+    *r0 = r[0]; *r1 = r[1];
+}
 /* path id p = (sample*h + y)*w + x.  Fills path_of_slot[n_slots] (-1: out-of-image slot). */
 static void partition(const orc_frame* f, const layout* L, int mode, int32_t* path_of_slot)
 {
@@ -426,13 +433,22 @@ static void partition(const orc_frame* f, const layout* L, int mode, int32_t* pa
     for (int64_t i = 0; i < L->n_slots; ++i) path_of_slot[i] = -1;
     for (int32_t sg = 0; sg < f->spp; ++sg)
         for (int32_t tile = 0; tile < L->n_tiles; ++tile) {
-            uint32_t a, c; tile_lcg(f, L, tile, sg, &a, &c);
+            uint32_t a, c, a0, c0; tile_lcg(f, L, tile, sg, &a, &c); tile_raw(f, tile, sg, &a0, &c0);
             int32_t tx = tile % L->tiles_x, ty = tile / L->tiles_x;
             for (int32_t n = 0; n < L->M; ++n) {
                 int32_t lx = n % L->W, ly = n / L->W;                  /* order on the screen inside the tile */
                 int32_t x = tx * L->W + lx, y = ty * L->H + ly;
                 if (x >= f->w || y >= f->h) continue;
                 uint32_t m = (a * (uint32_t)n + c) % (uint32_t)L->M;   /* shuffled number */
+                if (L->lattice) {
+                    /* alternative reading of BASELINE's "interleave stride" (S:8c A-3; D:R20): a REGULAR lattice.  The tile is
+                     * shifted cyclically by an offset drawn per tile, sample and frame ("varies in each tile and in each frame",
+                     * P:L113); pixels congruent modulo (sx, sy) form a group: its gw x gh members lie sx apart horizontally and
+                     * sy apart vertically.  Group-major position m = group * K + member, as in the shuffled rule. */
+                    int32_t px = (lx + (int32_t)(a0 % (uint32_t)L->W)) % L->W, py = (ly + (int32_t)(c0 % (uint32_t)L->H)) % L->H;
+                    int32_t g = (py % L->sy) * L->sx + (px % L->sx), j = (py / L->sy) * L->gw + (px / L->sx);
+                    m = (uint32_t)(g * L->K + j);
+                }
                 /* group = m / K ("divided by K, yield the same quotient"); the shuffled number
                  * is also the ray's position inside the tile's slot block (D:R5) */
                 int64_t slot = ((int64_t)sg * L->n_tiles + tile) * L->M + m;

@@ -30,6 +30,8 @@
  *                     density D_v(h) = G1(wo) max(0, wo.h) D(h) / wo.z (Heitz 2018); weight <= 1; |wi| = 1;
  *                     white-furnace energy <= 1
  *   morton + sort     bit-by-bit loop encoder vs a python magic-mask encoder, numpy stable argsort
+ *   lattice rule      (D:R20) exact cover, members congruent modulo the strides, groups = distinct residue classes, row-major
+ *                     member order, one tile written out from the definition, shift varies per tile and frame, furnace == 1
  *   other sort keys   (Origin, Reis, Costa, TwoPoint; D:R19) numpy encoder, hand-derived fixture tests/golden/ray_codes.txt,
  *                     Reis/Costa halves swapped, Origin's top levels == Reis' origin half, TwoPoint with d = 0 repeats the
  *                     origin bits; each sort mode == numpy stable argsort of its key over the independent rays

@@ -53,6 +53,65 @@ def test_partition_is_exact_cover(oracle, gw, gh, s, w, h, spp):
         assert np.all(np.bincount(m_of_n // K, minlength=M // K) == K)
 
 
+LATTICE = 1 << 14       # partition rule bit in the packed stride (D:R20)
+
+
+@pytest.mark.parametrize("gw,gh,sx,sy", [(4, 4, 2, 2), (4, 4, 4, 4), (2, 2, 8, 8), (8, 8, 1, 1), (8, 1, 1, 8), (4, 2, 2, 4)])
+@pytest.mark.parametrize("w,h,spp", [(64, 64, 1), (50, 37, 2)])
+def test_lattice_partition_is_an_interleaved_exact_cover(oracle, gw, gh, sx, sy, w, h, spp):
+    """Alternative partition rule (D:R20; S:8c A-3): a regular lattice.  Exact cover as for the shuffled rule; inside a full tile
+    the members of a group are the pixels congruent modulo (sx, sy) after the tile's cyclic shift — gw x gh pixels lying sx
+    apart horizontally and sy apart vertically (cyclically) — and member order inside the group is row-major over that grid;
+    the shift differs between tiles and frames; stride 1 makes the whole tile one group."""
+    s = sx | (sy << 16) | LATTICE
+    fr = oracle.frame(w, h, spp, seed=3, frame=5)
+    pos = oracle.partition(fr, M_REUSE, gw, gh, s)
+    W, H = gw * sx, gh * sy
+    M, K = W * H, gw * gh
+    tiles_x, tiles_y = -(-w // W), -(-h // H)
+    assert len(pos) == spp * tiles_x * tiles_y * M == oracle.n_slots(fr, M_REUSE, gw, gh, s)
+    live = pos[pos >= 0]
+    assert np.array_equal(np.sort(live), np.arange(spp * w * h))
+    slot = np.nonzero(pos >= 0)[0]
+    x = live % w; y = (live // w) % h
+    assert np.array_equal((slot // M) % (tiles_x * tiles_y), (y // H) * tiles_x + (x // W))
+    if w >= W and h >= H:
+        blk = pos[:M].reshape(M // K, K)               # tile 0: groups x members
+        lx, ly = blk % w, blk // w
+        for g in range(M // K):
+            # all members congruent modulo the strides, up to the tile's cyclic shift
+            dx = (lx[g] - lx[g][0]) % W; dy = (ly[g] - ly[g][0]) % H
+            assert np.all(dx % sx == 0) and np.all(dy % sy == 0)
+            assert len(set(zip(dx.tolist(), dy.tolist()))) == K
+        # different groups are different residue classes: the first members of the G groups are pairwise incongruent
+        firsts = {(int(lx[g][0]) % sx, int(ly[g][0]) % sy) for g in range(M // K)}
+        assert len(firsts) == M // K == sx * sy
+        # member order inside a group is row-major over its gw x gh grid (after the shift): consecutive members step by sx
+        if gw > 1:
+            assert np.all((lx[:, 1] - lx[:, 0]) % W == sx) and np.all(ly[:, 1] == ly[:, 0])
+    if sx == 1 and sy == 1:
+        assert oracle.n_groups(fr, M_REUSE, gw, gh, s) == spp * tiles_x * tiles_y
+
+
+def test_lattice_partition_shift_varies_per_tile_and_frame(oracle):
+    s = 2 | LATTICE
+    p0 = oracle.partition(oracle.frame(64, 64, 1, 0, 0), M_REUSE, 4, 4, s).reshape(-1, 64)
+    p1 = oracle.partition(oracle.frame(64, 64, 1, 0, 1), M_REUSE, 4, 4, s).reshape(-1, 64)
+    first = lambda p: [(int(b[0]) % 64 % 8, int(b[0]) // 64 % 8) for b in p]       # in-tile position of every tile's slot 0
+    assert len(set(first(p0))) > 8 and first(p0) != first(p1)
+    # against the definition, written out for one tile: slot m = g*K + j with g = (py % 2)*2 + px % 2, j = (py // 2)*4 + px // 2
+    fr = oracle.frame(64, 64, 1, 0, 0)
+    r = oracle.philox(9, 0, 0, 2, 0, 0)                                       # tile 9, sample 0, purpose TILE; key (seed 0, frame 0)
+    ox, oy = int(r[0]) % 8, int(r[1]) % 8
+    tx, ty = 9 % 8, 9 // 8
+    exp = np.empty(64, np.int64)
+    for ly in range(8):
+        for lx in range(8):
+            px, py = (lx + ox) % 8, (ly + oy) % 8
+            exp[((py % 2) * 2 + px % 2) * 16 + (py // 2) * 4 + px // 2] = (ty * 8 + ly) * 64 + tx * 8 + lx
+    assert np.array_equal(p0[9], exp)
+
+
 def test_partition_varies_per_tile_and_frame_not_per_bounce(oracle):
     fr0 = oracle.frame(64, 64, 1, 0, 0); fr1 = oracle.frame(64, 64, 1, 0, 1); fs = oracle.frame(64, 64, 1, 1, 0)
     p0 = oracle.partition(fr0, M_REUSE, 4, 4, 2).reshape(-1, 64)
@@ -118,9 +177,10 @@ def test_classification_constructed_scenes(oracle):
 
 
 # ------------------------------------------------------------------ reuse rules
-def test_diffuse_group_shares_one_tangent_space_direction(oracle):
+@pytest.mark.parametrize("s", [2, 2 | (1 << 14)])          # shuffled rule, lattice rule (D:R20)
+def test_diffuse_group_shares_one_tangent_space_direction(oracle, s):
     sc = I.cornell()
-    g = _first_bounce(oracle, sc, M_REUSE)
+    g = _first_bounce(oracle, sc, M_REUSE, s=s)
     gi = _first_bounce(oracle, sc, M_IND)
     K = 16
     loc = g["local_dir"].reshape(-1, K, 3); src = g["dir_src"].reshape(-1, K); p = g["ray_to_path"].reshape(-1, K)
@@ -490,6 +550,13 @@ def test_white_furnace_is_exactly_one(oracle, mode, mat):
         img, _, cnt = oracle.render_frame(b, sc, oracle.frame(sc.width, sc.height, 2, 0, 1), nb, mode, 4, 4, 2)
         assert np.all(img == 1.0)
         assert cnt[0] > 0
+
+
+def test_white_furnace_is_exactly_one_with_the_lattice_partition(oracle):
+    sc = I.furnace_sphere(2, albedo=1.0, mat_type=I.MAT_DIFFUSE)
+    b = oracle.Bvh(sc.verts)
+    img, _, cnt = oracle.render_frame(b, sc, oracle.frame(sc.width, sc.height, 2, 0, 1), 2, M_REUSE, 4, 4, 2 | (1 << 14))
+    assert np.all(img == 1.0) and cnt[0] > 0
 
 
 @pytest.mark.parametrize("mode", [M_IND, M_REUSE])

@@ -316,15 +316,16 @@ def run_sweep(args):
     import crt_inputs as I
     sc = max(1, args.sweep_scale)
     table3 = args.sweep == "table3"
-    w, h, spp, nb, seed = (1920 // sc, 1080 // sc, 1, 2, 1) if table3 else (3840 // sc, 2160 // sc, 4, 3, 1)
+    rules = args.sweep == "rules"
+    w, h, spp, nb, seed = (1920 // sc, 1080 // sc, 1, 2, 1) if (table3 or rules) else (3840 // sc, 2160 // sc, 4, 3, 1)
     scene = I.by_name("interior", seed=1).with_camera(w, h)
     bvh = ctx.crt_build_bvh(scene.verts, scene.mat_id)
     mats_dev = ctx.upload(scene.materials); mats = ctx.scene_mats(mats_dev, len(scene.materials), scene.env)
     cam = crt.make_camera(scene.camera)
     F = args.sweep_frames
 
-    def render(mode, g, s, frames, first_frame, tile=None):
-        order = crt.order_for_tile(mode, *tile) if tile else crt.make_order(mode, g, g, s)
+    def render(mode, g, s, frames, first_frame, tile=None, rule=0):
+        order = crt.order_for_tile(mode, *tile) if tile else crt.make_order(mode, g, g, s, partition_rule=rule)
         fr0 = crt.make_frame(w, h, spp)
         ws = ctx.frame_workspace(fr0, order)
         accum = torch.zeros((h, w, 3), device=ctx.device)
@@ -355,12 +356,19 @@ def run_sweep(args):
                 img, t = render("direct_reuse", 0, 0, F, 0, tile=(tw, th, k))
                 points.append(dict(mode="direct_reuse", tile=[tw, th], K=k, **t, rmse_vs_reference=rmse(img, ref), rmse_vs_independent=rmse(img, ind),
                                    trace_speedup_vs_independent=t["trace_only_mray_s"] / ind_t["trace_only_mray_s"]))
+    elif rules:     # the two readings of "interleave stride" (DESIGN.md D:R3 shuffled numbers, D:R20 regular lattice) side by side
+        for g in (4, 8):
+            for s in (2, 4, 8):
+                for rule, rname in ((0, "shuffle"), (1, "lattice")):
+                    img, t = render("direct_reuse", g, s, F, 0, rule=rule)
+                    points.append(dict(mode="direct_reuse", group=g, stride=s, partition_rule=rname, **t, rmse_vs_reference=rmse(img, ref), rmse_vs_independent=rmse(img, ind),
+                                       trace_speedup_vs_independent=t["trace_only_mray_s"] / ind_t["trace_only_mray_s"]))
     else:
         for g in (2, 4, 8):
             for s in (1, 2, 4, 8):
                 img, t = render("direct_reuse", g, s, F, 0)
                 points.append(dict(mode="direct_reuse", group=g, stride=s, **t, rmse_vs_reference=rmse(img, ref), rmse_vs_independent=rmse(img, ind)))
-    name = "the paper's Table 3 shapes (P:L178-185)" if table3 else "BASELINE config 3"
+    name = "the paper's Table 3 shapes (P:L178-185)" if table3 else ("partition rules (D:R3 / D:R20)" if rules else "BASELINE config 3")
     print(json.dumps({"sweep": points, "config": {"workload": f"{name}: interior scene {w}x{h}, {spp} spp, {nb} bounces", "frames": F,
                                                   "reference_frames": 4 * F, "scale": sc}}))
 
@@ -374,8 +382,8 @@ def main():
     ap.add_argument("--workload", default="interior", choices=sorted(WORKLOADS))
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-sort-codes", action="store_true", help="skip the Origin / Reis / Costa / TwoPoint reordering baselines")
-    ap.add_argument("--sweep", nargs="?", const="config3", default=None, choices=["config3", "table3"],
-                    help="config3: BASELINE config 3 sweep; table3: the paper's Table 3 shapes (tile x K) at 1920x1080, 1 spp, 2 bounces")
+    ap.add_argument("--sweep", nargs="?", const="config3", default=None, choices=["config3", "table3", "rules"],
+                    help="config3: BASELINE config 3 sweep; table3: the paper's Table 3 shapes (tile x K) at 1920x1080, 1 spp, 2 bounces; rules: shuffled against lattice partition at the same size")
     ap.add_argument("--sweep-frames", type=int, default=64)
     ap.add_argument("--sweep-scale", type=int, default=1, help="divide the 3840x2160 image by this (quick runs)")
     args = ap.parse_args()

@@ -75,7 +75,12 @@ typedef struct { float eye[3], U[3], V[3], W[3]; } crt_camera;
 /* stride = horizontal interleave stride; stride_y = vertical one (0 = same as stride).  The tile is (group_w*stride) x
  * (group_h*stride_y) and K = group_w*group_h, which expresses every power-of-two (W, H, K) of the paper's own
  * parametrisation, e.g. tile 8x8 with K = 8 as group 8x1, stride 1, stride_y 8 (D:R5). */
-typedef struct { int32_t mode, group_w, group_h, stride, stride_y; } crt_order;
+/* partition_rule: how the pixels of a tile are dealt to its groups.  CRT_PARTITION_SHUFFLE (0, default): the paper's rule,
+ * pixel numbers "shuffled using a linear congruence method" (D:R3).  CRT_PARTITION_LATTICE (1): a regular lattice, the
+ * literal reading of "interleave stride" (D:R20): after a cyclic shift of the tile drawn per tile, sample and frame, the pixels
+ * congruent modulo (stride, stride_y) form a group; its members lie stride / stride_y pixels apart. */
+typedef enum { CRT_PARTITION_SHUFFLE = 0, CRT_PARTITION_LATTICE = 1 } crt_partition_rule;
+typedef struct { int32_t mode, group_w, group_h, stride, stride_y, partition_rule; } crt_order;
 /* materials: [device] table indexed by the per-triangle material id given to crt_build_bvh.
  * env: radiance on a miss = lerp(env[0..2], env[3..5], 0.5*(d.y+1)) (D:R14). */
 typedef struct { const crt_material* materials; int32_t n_materials; float env[6]; } crt_scene_mats;

@@ -50,7 +50,7 @@ class Frame(C.Structure):
 
 
 class Order(C.Structure):
-    _fields_ = [("mode", C.c_int32), ("group_w", C.c_int32), ("group_h", C.c_int32), ("stride", C.c_int32), ("stride_y", C.c_int32)]
+    _fields_ = [("mode", C.c_int32), ("group_w", C.c_int32), ("group_h", C.c_int32), ("stride", C.c_int32), ("stride_y", C.c_int32), ("partition_rule", C.c_int32)]
 
 
 class Camera(C.Structure):
@@ -116,10 +116,14 @@ def make_frame(w, h, spp=1, seed=0, frame=0):
     return Frame(int(w), int(h), int(spp), int(seed), int(frame))
 
 
-def make_order(mode, group_w=1, group_h=1, stride=1, stride_y=0):
-    if int(stride) >> 16:                                  # packed form used by the tests: vertical stride in the high half
-        stride, stride_y = int(stride) & 0xffff, int(stride) >> 16
-    return Order(MODES[mode] if isinstance(mode, str) else int(mode), int(group_w), int(group_h), int(stride), int(stride_y))
+def make_order(mode, group_w=1, group_h=1, stride=1, stride_y=0, partition_rule=0):
+    """partition_rule: 0 = the paper's shuffled numbers, 1 = regular lattice (include/crt.h).  `stride` also accepts the packed form the
+    tests use: bits 0-13 horizontal stride, bit 14 lattice rule, high half vertical stride."""
+    stride = int(stride)
+    if stride >> 14:
+        partition_rule = partition_rule or ((stride >> 14) & 1)
+        stride, stride_y = stride & 0x3fff, (stride >> 16) or stride_y
+    return Order(MODES[mode] if isinstance(mode, str) else int(mode), int(group_w), int(group_h), int(stride), int(stride_y), int(partition_rule))
 
 
 def order_for_tile(mode, tile_w, tile_h, k):

@@ -75,6 +75,7 @@ CRT_DEV bool tri_test(V3 v0, V3 e1, V3 e2, V3 o, V3 d, float tmin, float tmax, f
 struct DevLayout {
     int32_t w, h, spp, reuse;
     int32_t W, H, M, K, tiles_x, n_tiles, log2W, log2M, log2K;
+    int32_t lattice, gw, sx, sy;       // regular-lattice partition rule (D:R20): group width and strides (powers of two)
     uint32_t seed, frame;
 };
 // inverse of an odd number modulo 2^32 (Newton steps double the number of valid bits; a*a == 1 mod 8)
@@ -95,8 +96,17 @@ CRT_DEV int32_t slot_to_path(const DevLayout& L, int64_t slot, int32_t& pixel, i
     sample = (int32_t)(blk / L.n_tiles);
     const uint4 r = philox((uint32_t)tile, (uint32_t)sample, 0u, PURPOSE_TILE, L.seed, L.frame);
     const uint32_t a = (r.x & (uint32_t)(L.M - 1)) | 1u, c = r.y & (uint32_t)(L.M - 1);
-    const uint32_t nn = (inv_odd(a) * (m - c)) & (uint32_t)(L.M - 1);
-    const int32_t lx = (int32_t)(nn & (uint32_t)(L.W - 1)), ly = (int32_t)(nn >> L.log2W);
+    int32_t lx, ly;
+    if (L.lattice) {
+        // m = g*K + j with g = (py % sy)*sx + px % sx, j = (py / sy)*gw + px / sx, (px, py) = the pixel after the tile's cyclic shift
+        const int32_t g = (int32_t)(m >> L.log2K), j = (int32_t)(m & (uint32_t)(L.K - 1));
+        const int32_t px = (j & (L.gw - 1)) * L.sx + (g & (L.sx - 1)), py = (j / L.gw) * L.sy + g / L.sx;
+        lx = (int32_t)(((uint32_t)px - r.x % (uint32_t)L.W) & (uint32_t)(L.W - 1));
+        ly = (int32_t)(((uint32_t)py - r.y % (uint32_t)L.H) & (uint32_t)(L.H - 1));
+    } else {
+        const uint32_t nn = (inv_odd(a) * (m - c)) & (uint32_t)(L.M - 1);
+        lx = (int32_t)(nn & (uint32_t)(L.W - 1)); ly = (int32_t)(nn >> L.log2W);
+    }
     const int32_t x = (tile % L.tiles_x) * L.W + lx, y = (tile / L.tiles_x) * L.H + ly;
     if (x >= L.w || y >= L.h) { pixel = -1; return -1; }
     pixel = y * L.w + x;

@@ -342,7 +342,7 @@ crt::DevLayout make_dev_layout(const Layout& L, const crt_frame& f)
     crt::DevLayout D;
     D.w = L.w; D.h = L.h; D.spp = L.spp; D.reuse = (L.mode == CRT_MODE_DIRECT_REUSE || L.mode == CRT_MODE_WORLD_REUSE);
     D.W = L.W; D.H = L.H; D.M = L.M; D.K = L.K; D.tiles_x = L.tiles_x; D.n_tiles = L.n_tiles;
-    D.log2W = L.log2W; D.log2M = L.log2M; D.log2K = L.log2K; D.seed = (uint32_t)f.seed; D.frame = (uint32_t)f.frame;
+    D.log2W = L.log2W; D.log2M = L.log2M; D.log2K = L.log2K; D.lattice = L.lattice; D.gw = L.gw; D.sx = L.sx; D.sy = L.sy; D.seed = (uint32_t)f.seed; D.frame = (uint32_t)f.frame;
     return D;
 }
 

@@ -58,14 +58,15 @@ def test_product_does_not_import_the_oracle():
 
 
 @pytest.mark.parametrize("w,h,spp,mode,gw,gh,s", [(64, 64, 1, 2, 4, 4, 2), (1920, 1080, 1, 2, 4, 4, 4), (3840, 2160, 4, 2, 8, 8, 8),
-                                                  (50, 37, 2, 2, 2, 4, 4), (50, 37, 2, 3, 4, 4, 2), (1920, 1080, 1, 0, 1, 1, 1), (7, 5, 3, 1, 1, 1, 1), (7, 5, 3, 5, 1, 1, 1), (0, 0, 1, 2, 2, 2, 2)])
+                                                  (50, 37, 2, 2, 2, 4, 4), (50, 37, 2, 3, 4, 4, 2), (1920, 1080, 1, 0, 1, 1, 1), (7, 5, 3, 1, 1, 1, 1), (7, 5, 3, 5, 1, 1, 1), (0, 0, 1, 2, 2, 2, 2),
+                                                  (50, 37, 2, 2, 4, 4, 2 | (1 << 14))])            # lattice partition rule (D:R20)
 def test_layout_matches_the_paper_parametrisation(lib, oracle, w, h, spp, mode, gw, gh, s):
     """tiles of W x H pixels, WH/K groups of K; K = gw*gh, W = gw*s, H = gh*s (reading R3)."""
     import paper_2310_07182_b200 as crt
     n_paths, n_slots, n_groups = crt.crt_layout(crt.make_frame(w, h, spp), crt.make_order(mode, gw, gh, s))
     assert n_paths == spp * w * h
     if mode in (2, 3):            # direct_reuse and world_reuse share the grouped slot space
-        W, H = gw * s, gh * s
+        W, H = gw * (s & 0x3fff), gh * ((s >> 16) or (s & 0x3fff))
         tiles = -(-w // W) * -(-h // H)
         assert n_slots == spp * tiles * W * H and n_groups * gw * gh == n_slots
     else:
@@ -148,5 +149,5 @@ def test_native_tile_shapes_and_layout_errors(lib, oracle):
         n = C.c_int64()
         assert lib.crt_layout(C.byref(fr), C.byref(bad), C.byref(n), None, None) == api.CRT_ERR_UNSUPPORTED
     for bad_mode in (-1, 8):
-        o = api.Order(bad_mode, 1, 1, 1, 0); n = C.c_int64()
+        o = api.Order(bad_mode, 1, 1, 1, 0, 0); n = C.c_int64()
         assert lib.crt_layout(C.byref(fr), C.byref(o), C.byref(n), None, None) == api.CRT_ERR_INVALID_ARG

@@ -193,7 +193,8 @@ def test_trace_stats_counts(crt, ctx, oracle):
 
 
 # ------------------------------------------------------------------ a1: primary rays
-@pytest.mark.parametrize("mode,gw,gh,s", [("independent", 1, 1, 1), ("direct_reuse", 4, 4, 2), ("direct_reuse", 2, 4, 4)])
+@pytest.mark.parametrize("mode,gw,gh,s", [("independent", 1, 1, 1), ("direct_reuse", 4, 4, 2), ("direct_reuse", 2, 4, 4), ("direct_reuse", 4, 4, 2 | (1 << 14)),
+                                          ("direct_reuse", 8, 2, 2 | (4 << 16) | (1 << 14))])
 @pytest.mark.parametrize("w,h,spp", [(64, 64, 1), (50, 37, 2)])
 def test_primary_matches_oracle(crt, ctx, oracle, mode, gw, gh, s, w, h, spp):
     scene = I.cornell(width=w, height=h)
@@ -231,6 +232,8 @@ GEN_CASES = [
     ("interior_small", "direct_reuse", 8, 8, 8, 96, 64, 1),   # largest tile: M = 4096
     ("checker", "direct_reuse", 4, 4, 2, 48, 40, 1),          # hybrid groups
     ("checker", "direct_reuse", 1, 1, 4, 48, 40, 1),          # K = 1
+    ("interior_small", "direct_reuse", 4, 4, 4 | (1 << 14), 96, 64, 1),      # regular-lattice partition rule (D:R20)
+    ("checker", "direct_reuse", 4, 2, 2 | (4 << 16) | (1 << 14), 50, 37, 2),  # lattice, unequal strides, ragged, 2 spp, hybrid groups
     ("interior_small", "direct_reuse", 8, 1, 1 | (8 << 16), 96, 64, 1),     # the paper's own setting: tile 8x8, K = 8
     ("interior_small", "direct_reuse", 16, 1, 2 | (8 << 16), 90, 61, 2),    # tile 32x8, K = 16 (Table 3), ragged, 2 spp
     ("landscape_small", "direct_reuse", 4, 4, 4, 96, 64, 1),  # config 4's grouping on a reduced landscape (coordinates up to 192, sky misses)

@@ -1,8 +1,8 @@
 // a4 (part): hand-written stable LSD radix sort of (key32, value32) pairs, 4 passes of 8 bits, no CUB
 // (reordering methods "encode and sort rays"; encode+sort overhead).
 // Per pass: (1) per-block digit histograms, (2) a two-level exclusive scan over the digit-major (digit, block) table,
-// (3) stable scatter: blocks re-read their tile in order; inside a round of 256 keys the rank of a key among equal
-// digits is (keys of that digit in earlier warps) + (earlier lanes of its warp, from __match_any_sync).
+// (3) stable scatter: warp-private running digit counters + __match_any_sync rank the keys of a tile with one block barrier,
+// and the tile leaves through shared memory in output order (see rs_scatter_kernel).
 #include "crt_internal.h"
 
 namespace {
@@ -18,11 +18,15 @@ __global__ void __launch_bounds__(RS_THREADS) rs_hist_kernel(const uint32_t* __r
     h[threadIdx.x] = 0;
     __syncthreads();
     const int64_t base = (int64_t)blockIdx.x * RS_TILE;
-#pragma unroll 4
+    uint32_t k[RS_ITEMS];                 // all 16 loads in flight before the first shared-memory atomic
+#pragma unroll
     for (int it = 0; it < RS_ITEMS; ++it) {
         const int64_t i = base + it * RS_THREADS + threadIdx.x;
-        if (i < n) atomicAdd(&h[(keys[i] >> shift) & 255u], 1u);
+        k[it] = i < n ? __ldg(keys + i) : 0u;
     }
+#pragma unroll
+    for (int it = 0; it < RS_ITEMS; ++it)
+        if (base + it * RS_THREADS + threadIdx.x < n) atomicAdd(&h[(k[it] >> shift) & 255u], 1u);
     __syncthreads();
     hist[(size_t)threadIdx.x * n_blocks + blockIdx.x] = h[threadIdx.x];
 }
@@ -55,15 +59,25 @@ __global__ void __launch_bounds__(256) rs_scan_kernel(uint32_t* __restrict__ his
     if (tid == 0) totals[blockIdx.x] = carry_s;
 }
 
-__global__ void __launch_bounds__(RS_THREADS) rs_scatter_kernel(const uint32_t* __restrict__ keys_in, const int32_t* __restrict__ vals_in, int64_t n, int shift,
+// Stable scatter of one pass.  Warp w owns the w-th 512-key segment of the block's tile and walks it in 16 rounds of 32
+// consecutive keys; the rank of a key among equal digits of its segment is a warp-PRIVATE running counter (no block barrier
+// per round) plus the earlier lanes of its round (__match_any_sync).  After one barrier the counters give, per digit, the
+// block-local start of each warp's run; keys and values are staged in shared memory in output order and then written out
+// so that the keys of one digit leave as one contiguous run (about 16 keys = 64 bytes for a uniform digit) instead of as
+// isolated 4-byte stores.  Order inside a digit = segment, round, lane = input order: the sort stays stable.
+__global__ void __launch_bounds__(RS_THREADS, 4) rs_scatter_kernel(const uint32_t* __restrict__ keys_in, const int32_t* __restrict__ vals_in, int64_t n, int shift,
                                                                 const uint32_t* __restrict__ hist, int n_blocks, const uint32_t* __restrict__ totals,
                                                                 uint32_t* __restrict__ keys_out, int32_t* __restrict__ vals_out)
 {
-    __shared__ uint32_t run[256];
-    __shared__ uint32_t wcount[RS_WARPS][256];
+    __shared__ uint32_t gbase[256];               // global position of the block's first key of each digit
+    __shared__ uint32_t lstart[257];              // block-local position of the first key of each digit (exclusive scan of the block's counts)
+    __shared__ uint32_t wcount[RS_WARPS][256];    // per warp: keys of each digit in its segment; then: local start of the warp's run
     __shared__ uint32_t wsum[RS_WARPS];
+    __shared__ uint32_t s_key[RS_TILE];
+    __shared__ int32_t s_val[RS_TILE];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    {   // digit base = exclusive scan of the 256 digit totals (thread = digit)
+    const unsigned lt = (1u << lane) - 1u;
+    {   // digit base = exclusive scan of the 256 digit totals (thread = digit) + this block's offset inside the digit
         const uint32_t v = totals[tid];
         uint32_t incl = v;
 #pragma unroll
@@ -72,33 +86,65 @@ __global__ void __launch_bounds__(RS_THREADS) rs_scatter_kernel(const uint32_t* 
         __syncthreads();
         uint32_t off = 0;
         for (int w = 0; w < warp; ++w) off += wsum[w];
-        run[tid] = off + incl - v + hist[(size_t)tid * n_blocks + blockIdx.x];
+        gbase[tid] = off + incl - v + hist[(size_t)tid * n_blocks + blockIdx.x];
     }
 #pragma unroll
     for (int w = 0; w < RS_WARPS; ++w) wcount[w][tid] = 0;
     __syncthreads();
-    const int64_t base = (int64_t)blockIdx.x * RS_TILE;
-    for (int it = 0; it < RS_ITEMS; ++it) {
-        const int64_t i = base + it * RS_THREADS + tid;
-        const bool valid = i < n;
-        uint32_t key = 0; int32_t val = 0;
-        if (valid) { key = keys_in[i]; val = vals_in[i]; }
-        const uint32_t digit = valid ? ((key >> shift) & 255u) : 256u;
-        const unsigned peers = __match_any_sync(0xffffffffu, digit);
-        const unsigned rank = __popc(peers & ((1u << lane) - 1u));
-        if (valid && rank == 0) wcount[warp][digit] = __popc(peers);
-        __syncthreads();
-        if (valid) {
-            uint32_t off = run[digit] + rank;
-            for (int w = 0; w < warp; ++w) off += wcount[w][digit];
-            keys_out[off] = key; vals_out[off] = val;
-        }
-        __syncthreads();
-        uint32_t tot = 0;
+    const int64_t base = (int64_t)blockIdx.x * RS_TILE + (int64_t)warp * (RS_TILE / RS_WARPS);
+    uint32_t key[RS_ITEMS]; uint32_t rank[RS_ITEMS];       // rank: rank inside the warp's segment | digit << 16
 #pragma unroll
-        for (int w = 0; w < RS_WARPS; ++w) { tot += wcount[w][tid]; wcount[w][tid] = 0; }
-        run[tid] += tot;
+    for (int it = 0; it < RS_ITEMS; ++it) {
+        const int64_t i = base + it * 32 + lane;
+        key[it] = i < n ? keys_in[i] : 0u;
+    }
+    // The 16 rounds depend on each other only through the counter of their digit: the first lane of each digit class adds the
+    // class size to the warp's counter with a shared-memory atomic (which returns the count of earlier rounds) and hands it to
+    // its peers by shuffle, so the rounds pipeline instead of forming a read-sync-write chain.
+#pragma unroll
+    for (int it = 0; it < RS_ITEMS; ++it) {
+        const bool valid = base + it * 32 + lane < n;
+        const uint32_t digit = valid ? ((key[it] >> shift) & 255u) : 256u;
+        const unsigned peers = __match_any_sync(0xffffffffu, digit);
+        const int leader = __ffs(peers) - 1;
+        uint32_t before = 0;
+        if (valid && lane == leader) before = atomicAdd(&wcount[warp][digit], (uint32_t)__popc(peers));
+        before = __shfl_sync(0xffffffffu, before, leader);
+        rank[it] = valid ? ((before + __popc(peers & lt)) | (digit << 16)) : 0xffffffffu;
+    }
+    __syncthreads();
+    {   // thread = digit: block count, exclusive scan over digits -> lstart; per-warp run starts
+        uint32_t cnt = 0, run[RS_WARPS];
+#pragma unroll
+        for (int w = 0; w < RS_WARPS; ++w) { run[w] = cnt; cnt += wcount[w][tid]; }
+        uint32_t incl = cnt;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) { uint32_t t = __shfl_up_sync(0xffffffffu, incl, d); if (lane >= d) incl += t; }
+        __syncthreads();                                  // wsum is reused
+        if (lane == 31) wsum[warp] = incl;
         __syncthreads();
+        uint32_t off = 0;
+        for (int w = 0; w < warp; ++w) off += wsum[w];
+        const uint32_t start = off + incl - cnt;
+        lstart[tid] = start;
+        if (tid == 255) lstart[256] = start + cnt;
+#pragma unroll
+        for (int w = 0; w < RS_WARPS; ++w) wcount[w][tid] = start + run[w];
+    }
+    __syncthreads();
+#pragma unroll
+    for (int it = 0; it < RS_ITEMS; ++it) {
+        if (rank[it] != 0xffffffffu) {
+            const uint32_t pos = wcount[warp][rank[it] >> 16] + (rank[it] & 0xffffu);
+            s_key[pos] = key[it]; s_val[pos] = vals_in[base + it * 32 + lane];
+        }
+    }
+    __syncthreads();
+    const uint32_t n_local = lstart[256];
+    for (uint32_t j = tid; j < n_local; j += RS_THREADS) {
+        const uint32_t k = s_key[j], digit = (k >> shift) & 255u;
+        const uint32_t out = gbase[digit] + (j - lstart[digit]);
+        keys_out[out] = k; vals_out[out] = s_val[j];
     }
 }
 

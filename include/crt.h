@@ -91,7 +91,9 @@ typedef struct {
     double sah_cost; int32_t depth, max_leaf;
     double build_seconds;
     int64_t n_wide_nodes;       /* 8-wide compressed nodes (128 bytes each); 0 when max_leaf != 1 */
-    int32_t wide_depth, pad;
+    int32_t wide_depth;
+    int32_t q16_inflation_pct;  /* summed surface area of the boxes the 16-bit nodes decode to, in percent of the fp32 boxes' (100 = no
+                                 * loss); above 200 the default kernel reads the fp32 nodes instead (grid too coarse for the scene) */
 } crt_bvh_info_t;
 /* optional per-stage device times of crt_generate_secondary, filled after the stream is synchronised by the
  * caller via crt_stage_times_resolve (milliseconds) */

@@ -69,7 +69,7 @@ class BvhParams(C.Structure):
 class BvhInfo(C.Structure):
     _fields_ = [("n_tris", C.c_int64), ("n_nodes", C.c_int64), ("device_bytes", C.c_int64), ("bounds", C.c_float * 6),
                 ("sah_cost", C.c_double), ("depth", C.c_int32), ("max_leaf", C.c_int32), ("build_seconds", C.c_double),
-                ("n_wide_nodes", C.c_int64), ("wide_depth", C.c_int32), ("pad", C.c_int32)]
+                ("n_wide_nodes", C.c_int64), ("wide_depth", C.c_int32), ("q16_inflation_pct", C.c_int32)]
 
 
 _lib = None
@@ -155,7 +155,7 @@ class Bvh:
         self.ctx._check(lib().crt_bvh_get_info(self.handle, C.byref(o)))
         return {"n_tris": o.n_tris, "n_nodes": o.n_nodes, "device_bytes": o.device_bytes, "bounds": np.array(list(o.bounds), np.float32),
                 "sah_cost": o.sah_cost, "depth": o.depth, "max_leaf": o.max_leaf, "build_seconds": o.build_seconds,
-                "n_wide_nodes": o.n_wide_nodes, "wide_depth": o.wide_depth}
+                "n_wide_nodes": o.n_wide_nodes, "wide_depth": o.wide_depth, "q16_inflation_pct": o.q16_inflation_pct}
 
     def check(self):
         v = C.c_int32(-1)

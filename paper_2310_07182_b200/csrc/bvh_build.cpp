@@ -310,9 +310,10 @@ void crt_bvh_flatten(const crt_bvh* b, const std::vector<int32_t>& tri_order, st
 // evaluates a plane distance as one FMA in grid units whose rounding error is at most 0.5 + 2^-4 step of position
 // (trace.cu: QRay), so the box test stays conservative (D:R10: it never decides the result, only which subtrees are
 // visited).  Returns 0, or 1 if a plane had to be clamped / is less than one step outside its box.
-int32_t crt_bvh_quantise(const crt_bvh* b, const std::vector<GpuNode>& gn, std::vector<QNode>& qn, QGrid* grid)
+int32_t crt_bvh_quantise(const crt_bvh* b, const std::vector<GpuNode>& gn, std::vector<QNode>& qn, QGrid* grid, double* inflation)
 {
     (void)b;
+    double area_f = 0, area_q = 0;       // summed half-areas of the fp32 boxes and of the boxes the 16-bit planes decode to
     double lo[3] = {1e300, 1e300, 1e300}, hi[3] = {-1e300, -1e300, -1e300};
     auto planes = [](const GpuChild& c, int k, double& mn, double& mx) {
         const float* p = &c.min_x; mn = p[2 * k]; mx = p[2 * k + 1];
@@ -355,8 +356,16 @@ int32_t crt_bvh_quantise(const crt_bvh* b, const std::vector<GpuNode>& gn, std::
                 }
                 q.planes[3 * c + k] = qlo | (qhi << 16);
             }
+            double ef[3], eq[3]; bool finite = true;
+            for (int k = 0; k < 3; ++k) {
+                double mn, mx; planes(gn[i].c[c], k, mn, mx);
+                if (!std::isfinite(mn) || !std::isfinite(mx)) { finite = false; break; }
+                ef[k] = mx - mn; eq[k] = (double)((q.planes[3 * c + k] >> 16) - (q.planes[3 * c + k] & 0xffffu)) / (double)grid->scale[k];
+            }
+            if (finite) { area_f += ef[0] * ef[1] + ef[1] * ef[2] + ef[2] * ef[0]; area_q += eq[0] * eq[1] + eq[1] * eq[2] + eq[2] * eq[0]; }
         }
         qn[i] = q;
     }
+    if (inflation) *inflation = area_f > 0 ? area_q / area_f : 1.0;
     return bad;
 }

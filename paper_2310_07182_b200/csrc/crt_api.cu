@@ -1,4 +1,5 @@
 // C ABI of libcrt (include/crt.h): argument checking, BVH upload, and the per-frame call sequence.
+#include <algorithm>
 #include <cstring>
 #include <thread>
 #include "crt_internal.h"
@@ -6,7 +7,7 @@
 bool crt_bvh_build_host(crt_bvh* b, const float* verts, int64_t n, const crt_bvh_params& pr);
 int32_t crt_bvh_check_host(const crt_bvh* b);
 void crt_bvh_flatten(const crt_bvh* b, const std::vector<int32_t>& tri_order, std::vector<GpuNode>& gn, std::vector<GpuTri>& gt, std::vector<int32_t>& slot_of_prim);
-int32_t crt_bvh_quantise(const crt_bvh* b, const std::vector<GpuNode>& gn, std::vector<QNode>& qn, QGrid* grid);
+int32_t crt_bvh_quantise(const crt_bvh* b, const std::vector<GpuNode>& gn, std::vector<QNode>& qn, QGrid* grid, double* inflation);
 void crt_bvh_build_wide(const crt_bvh* b, std::vector<WNode>& wn, std::vector<int32_t>& tri_order, int* depth_out);
 int32_t crt_bvh_check_wide(const crt_bvh* b, const std::vector<WNode>& wn, const std::vector<int32_t>& tri_order);
 
@@ -149,7 +150,7 @@ crt_status crt_build_bvh(crt_ctx* ctx, const float* verts, const int32_t* mat_id
         std::vector<GpuNode> gn; std::vector<GpuTri> gt; std::vector<int32_t> sop;
         crt_bvh_flatten(b, tri_order, gn, gt, sop);
         std::vector<QNode> qn;
-        b->q_violations = crt_bvh_quantise(b, gn, qn, &b->qgrid);
+        b->q_violations = crt_bvh_quantise(b, gn, qn, &b->qgrid, &b->q_inflation);
         b->device = ctx->device; b->n_gpu_nodes = (int64_t)gn.size();
         auto up = [&](void** d, const void* h, size_t bytes) -> cudaError_t {
             cudaError_t e = cudaMalloc(d, bytes ? bytes : 256);
@@ -184,6 +185,7 @@ crt_status crt_bvh_get_info(const crt_bvh* b, crt_bvh_info_t* o)
     memcpy(o->bounds, b->bounds, sizeof o->bounds);
     o->sah_cost = b->sah; o->depth = b->depth; o->max_leaf = b->max_leaf; o->build_seconds = b->build_seconds;
     o->n_wide_nodes = b->n_wide_nodes; o->wide_depth = b->wide_depth;
+    o->q16_inflation_pct = (int32_t)std::min(1e9, b->q_inflation * 100.0 + 0.5);
     return CRT_OK;
 }
 

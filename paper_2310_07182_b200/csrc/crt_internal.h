@@ -73,7 +73,7 @@ struct crt_bvh {
     // device data
     int device = -1;
     GpuNode* d_nodes = nullptr; int64_t n_gpu_nodes = 0;
-    QNode* d_qnodes = nullptr; QGrid qgrid = {}; int32_t q_violations = 0;   // 16-bit layout of the same nodes (trace_kernel 3)
+    QNode* d_qnodes = nullptr; QGrid qgrid = {}; int32_t q_violations = 0; double q_inflation = 1.0;   // 16-bit layout of the same nodes (trace_kernel 3)
     GpuTri* d_tris = nullptr;          // leaf order (wide order when the wide layout exists)
     WNode* d_wnodes = nullptr; int64_t n_wide_nodes = 0; int wide_depth = 0; int32_t wide_violations = 0;   // 8-wide layout (only when max_leaf == 1)
     int32_t* d_slot_of_prim = nullptr; // caller's triangle id -> index into d_tris

@@ -355,7 +355,8 @@ crt_status launch_trace(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, i
         CRT_CHECK_LAUNCH(ctx, "trace_flat");
         return CRT_OK;
     }
-    if (ctx->trace_kernel == 3) return launch_dyn<false, true>(ctx, bvh, rays, n, hits, nullptr, st);
+    // 16-bit nodes unless the grid is too coarse for this scene's detail (decoded boxes more than twice the fp32 boxes' area)
+    if (ctx->trace_kernel == 3 && bvh->q_inflation <= 2.0) return launch_dyn<false, true>(ctx, bvh, rays, n, hits, nullptr, st);
     return launch_dyn<false, false>(ctx, bvh, rays, n, hits, nullptr, st);
 }
 
@@ -364,7 +365,7 @@ crt_status launch_trace_stats(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* r
 {
     if (n == 0) return CRT_OK;
     if (ctx->trace_kernel == 2 && bvh->d_wnodes) return launch_trace_wide_stats(ctx, bvh, rays, n, counters, st);
-    if (ctx->trace_kernel == 3) return launch_dyn<true, true>(ctx, bvh, rays, n, nullptr, reinterpret_cast<unsigned long long*>(counters), st);
+    if (ctx->trace_kernel == 3 && bvh->q_inflation <= 2.0) return launch_dyn<true, true>(ctx, bvh, rays, n, nullptr, reinterpret_cast<unsigned long long*>(counters), st);
     return launch_dyn<true, false>(ctx, bvh, rays, n, nullptr, reinterpret_cast<unsigned long long*>(counters), st);
 }
 

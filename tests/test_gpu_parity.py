@@ -179,6 +179,30 @@ def test_trace_degenerate_directions_and_far_origins(crt, ctx, oracle, kernel):
     assert (hb["prim"] >= 0).mean() > 0.5
 
 
+def test_coarse_grid_falls_back_to_fp32_nodes(crt, ctx, oracle):
+    """A scene whose detail is far below the 16-bit grid step (two small clusters of triangles 10^6 triangle sizes apart): the
+    decoded boxes are reported as inflated (`q16_inflation_pct` > 200), the default kernel reads the fp32 nodes, and the hits
+    equal the all-triangles definition either way (forcing the 16-bit nodes is slower, not wrong)."""
+    rng = np.random.default_rng(5)
+    def cluster(c):
+        p = c + rng.random((200, 1, 3)) * 1e-2
+        return (p + rng.random((200, 3, 3)) * 1e-3).astype(np.float32)
+    verts = np.concatenate([cluster(np.zeros(3)), cluster(np.array([1000.0, 500.0, 250.0]))])
+    bvh = ctx.crt_build_bvh(verts, np.zeros(len(verts), np.int32))
+    info = bvh.info()
+    assert bvh.check() == 0 and info["q16_inflation_pct"] > 200
+    small = GpuScene(crt, I.cornell(), ctx).bvh.info()["q16_inflation_pct"]
+    assert 100 <= small < 130
+    n = 4000
+    r = np.zeros((n, 8), np.float32); r[:, 7] = 1e30
+    tgt = verts[rng.integers(0, len(verts), n)].mean(1) + rng.normal(size=(n, 3)) * 2e-4
+    d = rng.normal(size=(n, 3)); d /= np.linalg.norm(d, axis=1, keepdims=True)
+    r[:, 0:3] = tgt - d * rng.uniform(0.01, 5.0, (n, 1)); r[:, 4:7] = d
+    hb = oracle.trace_brute(verts, r.view(oracle.RAY_DTYPE).reshape(-1))
+    compare_hits(hits_np(oracle, ctx.crt_trace(bvh, ctx.upload(r))), hb)
+    assert (hb["prim"] >= 0).mean() > 0.2
+
+
 def test_trace_stats_counts(crt, ctx, oracle):
     scene = _small_interior()
     G = GpuScene(crt, scene, ctx)

@@ -210,7 +210,7 @@ def run_cuda(args):
         def step(i, rec):
             fr = crt.make_frame(w, h, spp, seed, replica_frame_index(i, rank, world))
             if host:
-                ctx.crt_render_frame_host(bvh, mats_h, scene.env, cam, fr, order, nb, accum_h, nsec_h[i], ws)
+                ctx.crt_render_frame_host_resident(bvh, mats_h, scene.env, cam, fr, order, nb, i == 0, accum_h, nsec_h[i], ws)
             else:
                 ctx.crt_render_frame(bvh, mats, cam, fr, order, nb, accum, ws, n_secondary=nsec[i], record_times=rec)
                 if rec:
@@ -298,8 +298,8 @@ def run_cuda(args):
                    "bvh": {"nodes": info["n_nodes"], "depth": info["depth"], "sah_cost": info["sah_cost"], "device_mb": info["device_bytes"] / 1e6,
                            "build_s": info["build_seconds"], "build_and_upload_s": build_s}},
         "modes": modes, "roofline": roofline, "cpu_baseline": cpu,
-        "e2e": {"value": e2e["mray_s"], "unit": UNIT, "h2d_bytes_per_step": img_bytes + len(scene.materials) * 32 + 48,
-                "d2h_bytes_per_step": img_bytes + 4 * nb, "ms_per_step": e2e["ms_per_step"], "api": "crt_render_frame_host"},
+        "e2e": {"value": e2e["mray_s"], "unit": UNIT, "h2d_bytes_per_step": len(scene.materials) * 32 + 48 + 24,
+                "d2h_bytes_per_step": img_bytes + 4 * nb, "ms_per_step": e2e["ms_per_step"], "api": "crt_render_frame_host_resident"},
         "gpu_launches": K * (4 + 3 * nb), "clocks": clk,
     }
     print(json.dumps(line))

@@ -217,6 +217,13 @@ crt_status crt_render_frame_host(crt_ctx* ctx, const crt_bvh* bvh, const crt_mat
                                  const float* env /*[host] 6*/, const crt_camera* camera, const crt_frame* frame,
                                  const crt_order* order, int32_t n_bounces, float* accum_host, uint32_t* n_secondary_host,
                                  void* workspace, size_t workspace_bytes, void* stream);
+/* The same with the accumulation image RESIDENT on the device between calls (it lives in the workspace, which the caller must
+ * keep and not reuse for another image): reset != 0 zeroes it before this frame; image_host [host] float[h][w][3] only receives
+ * the sum so far.  Per frame this moves the materials + camera in and one image out, half the bytes of crt_render_frame_host. */
+crt_status crt_render_frame_host_resident(crt_ctx* ctx, const crt_bvh* bvh, const crt_material* materials_host, int32_t n_materials,
+                                          const float* env /*[host] 6*/, const crt_camera* camera, const crt_frame* frame,
+                                          const crt_order* order, int32_t n_bounces, int32_t reset, float* image_host,
+                                          uint32_t* n_secondary_host, void* workspace, size_t workspace_bytes, void* stream);
 size_t crt_frame_host_extra_bytes(const crt_frame* frame, int32_t n_materials);
 
 #ifdef __cplusplus

@@ -434,16 +434,19 @@ size_t crt_frame_host_extra_bytes(const crt_frame* frame, int32_t n_materials)
     return al((size_t)n_materials * sizeof(crt_material)) + al((size_t)frame->w * frame->h * 12) + al(64 * 4) + 256;
 }
 
-crt_status crt_render_frame_host(crt_ctx* ctx, const crt_bvh* bvh, const crt_material* materials_host, int32_t n_materials, const float* env,
-                                 const crt_camera* camera, const crt_frame* frame, const crt_order* order, int32_t n_bounces, float* accum_host,
-                                 uint32_t* n_secondary_host, void* workspace, size_t workspace_bytes, void* stream)
+// shared body of the two host-buffer entry points.  resident: the accumulation image lives in the workspace between calls
+// (zeroed when reset != 0) and is only copied OUT; otherwise it is copied in from image_host first.
+static crt_status render_frame_host_impl(crt_ctx* ctx, const crt_bvh* bvh, const crt_material* materials_host, int32_t n_materials, const float* env,
+                                         const crt_camera* camera, const crt_frame* frame, const crt_order* order, int32_t n_bounces, float* image_host,
+                                         uint32_t* n_secondary_host, void* workspace, size_t workspace_bytes, void* stream, bool resident, bool reset, const char* name)
 {
-    NEED_CTX("render_frame_host"); NEED_BVH("render_frame_host");
-    if (!materials_host || !env || !camera || !frame || !accum_host || n_materials < 1) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "render_frame_host: null argument");
+    if (!ctx) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "%s: ctx is null", name);
+    if (!bvh || !bvh->d_nodes || bvh->device != ctx->device) return crt_fail(ctx, bvh ? CRT_ERR_STATE : CRT_ERR_INVALID_ARG, "%s: BVH missing or not on this context's device", name);
+    if (!materials_host || !env || !camera || !frame || !image_host || n_materials < 1) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "%s: null argument", name);
     Layout L; crt_status st = crt_make_layout(ctx, frame, order, &L); if (st != CRT_OK) return st;
-    NEED_ALIGNED("render_frame_host", workspace, 256);
+    if (!crt_aligned(workspace, 256)) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "%s: workspace is null or not 256-byte aligned", name);
     const size_t core = carve(L, nullptr).total, extra = crt_frame_host_extra_bytes(frame, n_materials);
-    if (workspace_bytes < core + extra) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "render_frame_host: workspace %zu < %zu bytes", workspace_bytes, core + extra);
+    if (workspace_bytes < core + extra) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "%s: workspace %zu < %zu bytes", name, workspace_bytes, core + extra);
     cudaStream_t s = (cudaStream_t)stream;
     char* p = static_cast<char*>(workspace) + core;
     crt_material* d_mats = (crt_material*)p; p += al((size_t)n_materials * sizeof(crt_material));
@@ -451,14 +454,31 @@ crt_status crt_render_frame_host(crt_ctx* ctx, const crt_bvh* bvh, const crt_mat
     uint32_t* d_nsec = (uint32_t*)p;
     const size_t img = (size_t)frame->w * frame->h * 12;
     CRT_CUDA(ctx, cudaMemcpyAsync(d_mats, materials_host, (size_t)n_materials * sizeof(crt_material), cudaMemcpyHostToDevice, s));
-    CRT_CUDA(ctx, cudaMemcpyAsync(d_accum, accum_host, img, cudaMemcpyHostToDevice, s));
+    if (!resident) CRT_CUDA(ctx, cudaMemcpyAsync(d_accum, image_host, img, cudaMemcpyHostToDevice, s));
+    else if (reset) CRT_CUDA(ctx, cudaMemsetAsync(d_accum, 0, img, s));
     crt_scene_mats sm; sm.materials = d_mats; sm.n_materials = n_materials; memcpy(sm.env, env, sizeof sm.env);
     st = crt_render_frame(ctx, bvh, &sm, camera, frame, order, n_bounces, d_accum, n_secondary_host ? d_nsec : nullptr, workspace, core, 0, stream);
     if (st != CRT_OK) return st;
-    CRT_CUDA(ctx, cudaMemcpyAsync(accum_host, d_accum, img, cudaMemcpyDeviceToHost, s));
+    CRT_CUDA(ctx, cudaMemcpyAsync(image_host, d_accum, img, cudaMemcpyDeviceToHost, s));
     if (n_secondary_host && n_bounces > 0) CRT_CUDA(ctx, cudaMemcpyAsync(n_secondary_host, d_nsec, 4 * (size_t)n_bounces, cudaMemcpyDeviceToHost, s));
     CRT_CUDA(ctx, cudaStreamSynchronize(s));
     return CRT_OK;
+}
+
+crt_status crt_render_frame_host(crt_ctx* ctx, const crt_bvh* bvh, const crt_material* materials_host, int32_t n_materials, const float* env,
+                                 const crt_camera* camera, const crt_frame* frame, const crt_order* order, int32_t n_bounces, float* accum_host,
+                                 uint32_t* n_secondary_host, void* workspace, size_t workspace_bytes, void* stream)
+{
+    return render_frame_host_impl(ctx, bvh, materials_host, n_materials, env, camera, frame, order, n_bounces, accum_host, n_secondary_host,
+                                  workspace, workspace_bytes, stream, false, false, "render_frame_host");
+}
+
+crt_status crt_render_frame_host_resident(crt_ctx* ctx, const crt_bvh* bvh, const crt_material* materials_host, int32_t n_materials, const float* env,
+                                          const crt_camera* camera, const crt_frame* frame, const crt_order* order, int32_t n_bounces, int32_t reset,
+                                          float* image_host, uint32_t* n_secondary_host, void* workspace, size_t workspace_bytes, void* stream)
+{
+    return render_frame_host_impl(ctx, bvh, materials_host, n_materials, env, camera, frame, order, n_bounces, image_host, n_secondary_host,
+                                  workspace, workspace_bytes, stream, true, reset != 0, "render_frame_host_resident");
 }
 
 }  // extern "C"

@@ -404,6 +404,16 @@ def test_config1_end_to_end(crt, ctx, oracle, mode, gw, gh, s):
     ws_h = ctx.frame_workspace(fr, order, host_materials=len(scene.materials))
     ctx.crt_render_frame_host(G.bvh, scene.materials, scene.env, G.camera, fr, order, 1, acc_h, nsec_h, ws_h)
     assert np.array_equal(acc_h, accum.cpu().numpy()) and nsec_h[0] == g["n_active"]
+    # device-resident accumulation: two frames through either host entry point give the same sum; reset starts over
+    fr2 = crt.make_frame(fr.w, fr.h, fr.spp, fr.seed, fr.frame + 1)
+    ctx.crt_render_frame_host(G.bvh, scene.materials, scene.env, G.camera, fr2, order, 1, acc_h, nsec_h, ws_h)
+    img_r = np.full((64, 64, 3), -1.0, np.float32); ws_r = ctx.frame_workspace(fr, order, host_materials=len(scene.materials))
+    ctx.crt_render_frame_host_resident(G.bvh, scene.materials, scene.env, G.camera, fr, order, 1, True, img_r, nsec_h, ws_r)
+    assert np.array_equal(img_r, accum.cpu().numpy())
+    ctx.crt_render_frame_host_resident(G.bvh, scene.materials, scene.env, G.camera, fr2, order, 1, False, img_r, nsec_h, ws_r)
+    assert np.array_equal(img_r, acc_h)
+    ctx.crt_render_frame_host_resident(G.bvh, scene.materials, scene.env, G.camera, fr, order, 1, True, img_r, nsec_h, ws_r)
+    assert np.array_equal(img_r, accum.cpu().numpy())
 
 
 @pytest.mark.parametrize("mode,gw,gh,s", [("independent", 1, 1, 1), ("morton_reorder", 1, 1, 1), ("direct_reuse", 4, 4, 4), ("direct_reuse", 8, 8, 2), ("world_reuse", 4, 4, 4),

@@ -15,7 +15,7 @@ struct crt_ctx {
     // options
     int trace_kernel = 3;        // 0: binary BVH, one thread per ray; 1: binary BVH with fp32 64-byte nodes, persistent warps; 2: 8-wide compressed BVH, persistent warps (needs max_leaf == 1; else falls back to 1); 3 (default): binary BVH with 16-bit 32-byte nodes, persistent warps
     int trace_refill_threshold = 16;   // idle lanes refetch when fewer than this many lanes of the warp are busy
-    int trace_leaf_wait = 4;           // leave the inner-node phase when at most this many converged lanes still lack a leaf
+    int trace_leaf_wait = 6;           // leave the inner-node phase when at most this many converged lanes still lack a leaf
     int trace_tri_wait = 8;            // wide kernel: a warp enters its triangle phase when at least this many lanes hold triangle hits
     int trace_blocks_per_sm = 0; // 0 = from occupancy
     int fuse_shade = 0;          // crt_render_frame: shade non-final segments inside the next generation kernel (option; measured: DESIGN.md 5.4)

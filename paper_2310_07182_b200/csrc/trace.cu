@@ -86,7 +86,7 @@ struct RayState {
 };
 
 // Tests both children of `n`; returns the next node reference (nearer child, other child pushed) or pops the stack.
-CRT_DEV int visit_node(const NodeRegs& n, const RayState& r, int* stack, int& sp)
+CRT_DEV int visit_node(const NodeRegs& n, const RayState& r, int*& top)
 {
     // every distance is finite (safe_rcp); a NaN could only come from non-finite ray data, and fminf/fmaxf drop NaN operands
     const float ax0 = __fmaf_rn(n.a.min_x, r.idx, r.ox), ax1 = __fmaf_rn(n.a.max_x, r.idx, r.ox);
@@ -103,12 +103,12 @@ CRT_DEV int visit_node(const NodeRegs& n, const RayState& r, int* stack, int& sp
     const bool h0 = tn0 <= tf0, h1 = tn1 <= tf1;
     if (h0 && h1) {
         const bool swap = tn1 < tn0;
-        stack[++sp] = swap ? n.a.ref : n.b.ref;
+        *++top = swap ? n.a.ref : n.b.ref;
         return swap ? n.b.ref : n.a.ref;
     }
     if (h0) return n.a.ref;
     if (h1) return n.b.ref;
-    return stack[sp--];
+    return *top--;
 }
 
 // ---- 16-bit nodes (QNode, 32 bytes, ONE 256-bit load; crt_internal.h, bvh_build.cpp: crt_bvh_quantise) -----------------
@@ -140,7 +140,7 @@ CRT_DEV float qplane(unsigned w, unsigned sel, float s, float c)
     return __fmaf_rn(__uint_as_float(f), s, c);
 }
 // a direction component of zero: s is huge but finite (safe_rcp), both distances of that axis are huge with the right signs
-CRT_DEV int visit_qnode(const QNode* __restrict__ nodes, int idx, const RayState& r, const QRay& q, int* stack, int& sp)
+CRT_DEV int visit_qnode(const QNode* __restrict__ nodes, int idx, const RayState& r, const QRay& q, int*& top)
 {
     unsigned w0, w1, w2, w3, w4, w5; int ra, rb;
     asm volatile("ld.global.nc.v8.u32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
@@ -154,8 +154,8 @@ CRT_DEV int visit_qnode(const QNode* __restrict__ nodes, int idx, const RayState
     const bool h0 = tn0 <= tf0, h1 = tn1 <= tf1;
     const bool second = h1 && (!h0 || tn1 < tn0);          // child 1 is the one to enter
     int next = second ? rb : ra;
-    if (h0 && h1) stack[++sp] = second ? ra : rb;     // (an L1 prefetch of the pushed node was measured 5 % slower)
-    if (!(h0 || h1)) next = stack[sp--];
+    if (h0 && h1) *++top = second ? ra : rb;     // (an L1 prefetch of the pushed node was measured 5 % slower)
+    if (!(h0 || h1)) next = *top--;
     return next;
 }
 
@@ -200,11 +200,11 @@ __global__ void __launch_bounds__(TRACE_BLOCK) trace_flat_kernel(const GpuNode* 
     const float4 ro = __ldg(rp), rd = __ldg(rp + 1);
     RayState r; r.init(ro, rd);
     if (rd.w >= 0.f) {
-        int stack[STACK_SIZE]; int sp = 0; stack[0] = SENTINEL;
+        int stack[STACK_SIZE]; int* top = stack; stack[0] = SENTINEL;      // top: pointer to the top entry (no index-to-address LEA per push/pop)
         int node = 0; unsigned dummy = 0;
         while (node != SENTINEL) {
-            while ((unsigned)node < (unsigned)SENTINEL) node = visit_node(load_node(nodes, node), r, stack, sp);
-            while (node < 0) { visit_leaf<false>(tris, node, r, dummy, hits, (int)i); node = stack[sp--]; }
+            while ((unsigned)node < (unsigned)SENTINEL) node = visit_node(load_node(nodes, node), r, top);
+            while (node < 0) { visit_leaf<false>(tris, node, r, dummy, hits, (int)i); node = *top--; }
         }
     }
     if (r.best.prim < 0) store_miss(hits, i, rd.w);
@@ -219,7 +219,7 @@ __global__ void __launch_bounds__(TRACE_BLOCK, CRT_TRACE_MINB(QN)) trace_dyn_ker
                                                                 unsigned long long* __restrict__ stats)
 {
     const unsigned lane = threadIdx.x & 31u;
-    int stack[STACK_SIZE]; int sp = 0; stack[0] = SENTINEL;
+    int stack[STACK_SIZE]; int* top = stack; stack[0] = SENTINEL;      // top: pointer to the top entry (no index-to-address LEA per push/pop)
     int node = SENTINEL, leaf = 0;      // leaf: postponed leaf reference (< 0) or 0 = none
     int ray_idx = -1;
     bool exhausted = false;
@@ -251,7 +251,7 @@ __global__ void __launch_bounds__(TRACE_BLOCK, CRT_TRACE_MINB(QN)) trace_dyn_ker
                     } else {
                         r.init(__ldg(rp), rd);
                         if (QN) q.init(r, grid);
-                        ray_idx = (int)i; node = 0; leaf = 0; sp = 0;
+                        ray_idx = (int)i; node = 0; leaf = 0; top = stack;
                         if (COUNT) ++c_rays;
                     }
                 }
@@ -270,8 +270,8 @@ __global__ void __launch_bounds__(TRACE_BLOCK, CRT_TRACE_MINB(QN)) trace_dyn_ker
                 for (int rep = 0; rep < CRT_VISITS_PER_VOTE; ++rep) {
                     if (rep > 0 && (unsigned)node >= (unsigned)SENTINEL) break;
                     if (COUNT) ++c_nodes;
-                    node = QN ? visit_qnode(qnodes, node, r, q, stack, sp) : visit_node(load_node(nodes, node), r, stack, sp);
-                    if (node < 0 && leaf == 0) { leaf = node; node = stack[sp--]; }
+                    node = QN ? visit_qnode(qnodes, node, r, q, top) : visit_node(load_node(nodes, node), r, top);
+                    if (node < 0 && leaf == 0) { leaf = node; node = *top--; }
                 }
                 if (__popc(__ballot_sync(__activemask(), leaf == 0)) <= leaf_wait) break;   // (nearly) every converged lane holds a leaf
             }
@@ -279,7 +279,7 @@ __global__ void __launch_bounds__(TRACE_BLOCK, CRT_TRACE_MINB(QN)) trace_dyn_ker
             while (leaf < 0) {
                 visit_leaf<COUNT>(tris, leaf, r, c_tris, hits, ray_idx);
                 leaf = 0;
-                if (node < 0) { leaf = node; node = stack[sp--]; }
+                if (node < 0) { leaf = node; node = *top--; }
             }
             if (__popc(__activemask()) < refill_threshold) break;
         }

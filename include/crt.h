@@ -121,7 +121,7 @@ crt_status crt_measure_peaks(crt_ctx* ctx, double* fp32_tflops, double* copy_gbs
 /* Builds a binary BVH (binned surface-area heuristic, leaves <= max_leaf triangles) on the host with
  * n_threads threads and uploads it in the traversal layouts: the binary fp32 64-byte-node layout and its 16-bit
  * 32-byte-node form (planes on a 65536-step grid over the scene box, rounded outward; read by the default trace_kernel 3,
- * whose box test is conservative for ray origins within about a hundred scene extents of the scene) always, and, when
+ * whose box test is conservative for ray origins within 16 scene extents of the scene) always, and, when
  * max_leaf == 1, its collapse into 8-wide compressed 128-byte nodes (read by trace_kernel 2; measured slower than the
  * binary layout on both bench workloads, profiles/r01b, so not the default).
  * verts: [host|device] float[n_tris][3][3]; mat_id: [host|device] int32[n_tris].  Synchronous.  params may be

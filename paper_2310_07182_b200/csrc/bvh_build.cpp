@@ -307,8 +307,8 @@ void crt_bvh_flatten(const crt_bvh* b, const std::vector<int32_t>& tri_order, st
 
 // 16-bit layout of the flattened nodes (trace_kernel 3): every box plane becomes a position on a 65536-step grid over the
 // scene box, rounded OUTWARD (min planes down, max planes up) and then moved ONE more step outward: the traversal kernel
-// evaluates a plane distance as one FMA in grid units whose rounding error is at most 0.5 + 2^-4 step of position
-// (trace.cu: QRay), so the box test stays conservative (D:R10: it never decides the result, only which subtrees are
+// evaluates a plane distance as one FMA in grid units whose rounding error stays below one step of position for ray
+// origins within 16 scene extents (trace.cu: QRay), so the box test stays conservative (D:R10: it never decides the result, only which subtrees are
 // visited).  Returns 0, or 1 if a plane had to be clamped / is less than one step outside its box.
 int32_t crt_bvh_quantise(const crt_bvh* b, const std::vector<GpuNode>& gn, std::vector<QNode>& qn, QGrid* grid, double* inflation)
 {

@@ -146,11 +146,11 @@ crt_status crt_build_bvh(crt_ctx* ctx, const float* verts, const int32_t* mat_id
         b->wide_violations = crt_bvh_check_wide(b, wn, tri_order);
         if (b->wide_depth > 40) { delete b; return crt_fail(ctx, CRT_ERR_UNSUPPORTED, "build_bvh: wide tree depth %d exceeds the traversal stack", b->wide_depth); }
     }
+    // traversal layouts (host vectors; built without a context too, so that crt_bvh_check / crt_bvh_get_info cover the 16-bit nodes)
+    std::vector<GpuNode> gn; std::vector<GpuTri> gt; std::vector<int32_t> sop; std::vector<QNode> qn;
+    crt_bvh_flatten(b, tri_order, gn, gt, sop);
+    b->q_violations = crt_bvh_quantise(b, gn, qn, &b->qgrid, &b->q_inflation);
     if (ctx) {
-        std::vector<GpuNode> gn; std::vector<GpuTri> gt; std::vector<int32_t> sop;
-        crt_bvh_flatten(b, tri_order, gn, gt, sop);
-        std::vector<QNode> qn;
-        b->q_violations = crt_bvh_quantise(b, gn, qn, &b->qgrid, &b->q_inflation);
         b->device = ctx->device; b->n_gpu_nodes = (int64_t)gn.size();
         auto up = [&](void** d, const void* h, size_t bytes) -> cudaError_t {
             cudaError_t e = cudaMalloc(d, bytes ? bytes : 256);

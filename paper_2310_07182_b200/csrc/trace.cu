@@ -121,9 +121,14 @@ struct QRay {
     float sx, sy, sz;                     // 1 / (d * scale): distance per grid step
     float cx, cy, cz;                     // -(o' + 2^23) * s
     unsigned nx, ny, nz, fx, fy, fz;      // PRMT selectors of the near / far plane
-    // Error budget of t = (2^23 + q) * s + c against the exact (q - o') * s, in grid steps of position: c is rounded to
-    // an ulp of 2^23 * s, i.e. at most HALF a step; o', s and the final FMA add less than 2^-4 step for origins within
-    // a hundred scene extents.  The stored planes are therefore moved one step outward (crt_bvh_quantise).
+    // Error budget of t = (2^23 + q) * s + c against the exact (q - o') * s, in grid steps of position: c is rounded to an ulp
+    // of 2^23 * s, i.e. at most HALF a step; o' (two roundings), s (three), the product o' * s and the final FMA add at most
+    // 6 * 2^-24 * |o'| + 2^-7 step.  The stored planes are moved ONE step outward (crt_bvh_quantise), so the test is
+    // conservative while 0.5 + 6 * 2^-24 * |o'| <= 1, i.e. |o'| <= 1.4 M steps; the stated contract (include/crt.h) is ray
+    // origins within 16 scene extents of the scene (0.9 step; tests/test_abi.py re-enacts this arithmetic).  The fp32-node
+    // kernel's own limit is about 128 extents.  Rounding c in opposite directions for near and far planes with a per-ray margin
+    // lifts the limit but was measured 3-4 % slower (six constant registers instead of three defeat the operand reuse of the
+    // FFMA pairs; profiles/r01f).
     CRT_DEV void init(const RayState& r, const QGrid& g)
     {
         sx = r.idx * g.inv_scale[0]; sy = r.idy * g.inv_scale[1]; sz = r.idz * g.inv_scale[2];

@@ -92,6 +92,9 @@ def test_host_bvh_builder_invariants(lib):
         assert len(v) / max_leaf <= (info.n_nodes + 1) / 2 <= len(v)
         assert np.array_equal(np.array(list(info.bounds), np.float32), np.concatenate([v.reshape(-1, 3).min(0), v.reshape(-1, 3).max(0)]))
         assert info.device_bytes == 0
+        # 16-bit node layout: every plane at least one grid step outside its fp32 box (check bit 16 clear) and the decoded boxes
+        # only slightly larger than the fp32 ones on scenes of this kind
+        assert 100 <= info.q16_inflation_pct <= 125
         # the 8-wide compressed layout exists exactly when every leaf holds one triangle; crt_bvh_check covers its soundness too
         assert (info.n_wide_nodes > 0) == (max_leaf == 1)
         if max_leaf == 1:
@@ -151,3 +154,36 @@ def test_native_tile_shapes_and_layout_errors(lib, oracle):
     for bad_mode in (-1, 8):
         o = api.Order(bad_mode, 1, 1, 1, 0, 0); n = C.c_int64()
         assert lib.crt_layout(C.byref(fr), C.byref(o), C.byref(n), None, None) == api.CRT_ERR_INVALID_ARG
+
+
+def test_q16_box_test_error_budget():
+    """The 16-bit-node box test evaluates a plane distance as t = (2^23 + q) * s + c in fp32 (csrc/trace.cu: QRay).  Re-enacting
+    that arithmetic in numpy against the exact (q - o') * s shows the budget the kernel's comment states: the error, in grid steps
+    of position, stays below the ONE step by which crt_bvh_quantise pads the planes for ray origins within 16 scene extents (the contract
+    of include/crt.h) — dominated by the half step of rounding c inside the scene — and passes one step somewhere beyond 20 extents,
+    which is why the contract exists."""
+    rng = np.random.default_rng(3)
+    f32 = np.float32
+    n = 200000
+    fma = lambda a, b, c: (a.astype(np.float64) * b.astype(np.float64) + c.astype(np.float64)).astype(f32)
+    seen = {}
+    for reach, bound in ((1.0, 0.53), (16.0, 0.92), (60.0, None)):
+        gmin = f32(rng.uniform(-50, 50)); ext = rng.uniform(1, 2000)
+        scale = f32((65535.0 - 16.0) / ext); inv_scale = f32(1.0 / np.float64(scale))
+        o = (np.float64(gmin) + rng.uniform(-reach, reach + 1, n) * ext).astype(f32)
+        d = (rng.choice([-1.0, 1.0], n) * np.exp(rng.uniform(np.log(1e-6), 0.0, n))).astype(f32)
+        q = rng.integers(0, 65536, n)
+        idx = (f32(1.0) / d).astype(f32)
+        s = (idx * inv_scale).astype(f32)
+        p = ((o - gmin).astype(f32) * scale).astype(f32)
+        c = fma(np.full(n, -8388608.0, f32), s, -(p * s).astype(f32))
+        t = fma((8388608.0 + q).astype(f32), s, c)
+        # exact: the grid and the ray as given (fp32 values taken as exact reals)
+        o_steps = (o.astype(np.float64) - np.float64(gmin)) * np.float64(scale)
+        t_exact = (q - o_steps) / (d.astype(np.float64) * np.float64(scale))
+        err_steps = np.abs(t.astype(np.float64) - t_exact) * np.abs(d.astype(np.float64)) * np.float64(scale)
+        seen[reach] = err_steps.max()
+        if bound is not None:
+            assert err_steps.max() <= bound, (reach, err_steps.max())
+        assert err_steps.max() > 0.3                       # the half step of rounding c is real: the padding is needed
+    assert seen[60.0] > 1.0                                # beyond the contract the one step of padding is not enough

@@ -148,7 +148,7 @@ def test_trace_edge_cases(crt, ctx, oracle):
 def test_trace_degenerate_directions_and_far_origins(crt, ctx, oracle, kernel):
     """The box test must stay conservative where its arithmetic degenerates: direction components that are exactly zero
     (1/d infinite, plane distances NaN), origins exactly on box planes of the axis-aligned Cornell walls, and origins far
-    outside the scene (the 16-bit layout states about a hundred scene extents, include/crt.h).  Hits must equal the
+    outside the scene (the 16-bit layout states 16 scene extents, include/crt.h).  Hits must equal the
     all-triangles definition."""
     scene = I.cornell()
     G = GpuScene(crt, scene, ctx)
@@ -163,10 +163,10 @@ def test_trace_degenerate_directions_and_far_origins(crt, ctx, oracle, kernel):
     ax = np.zeros((n, 3)); ax[np.arange(n), k] = rng.choice([-1.0, 1.0], n)
     d[1:2000:2] = ax[1:2000:2]                                        # axis-aligned: two zero components
     d /= np.linalg.norm(d, axis=1, keepdims=True)
-    far = slice(4000, n)                                              # origins 30-80 extents away, aimed at the box
+    far = slice(4000, n)                                              # origins 4-15 extents away, aimed at the box
     tgt = rng.random((n, 3))
     dirs = rng.normal(size=(n, 3)); dirs /= np.linalg.norm(dirs, axis=1, keepdims=True)
-    dist = rng.uniform(30, 80, (n, 1))
+    dist = rng.uniform(4, 15, (n, 1))
     o64 = o.astype(np.float64); o64[far] = tgt[far] - dirs[far] * dist[far]; d[far] = dirs[far]
     r[:, 0:3] = o64; r[:, 4:7] = d
     ctx.crt_set_option("trace_kernel", kernel)

@@ -29,7 +29,7 @@ constexpr int SENTINEL = 0x7fffffff;
 constexpr int TRACE_BLOCK = 128;
 // resident blocks per SM the persistent kernel is compiled for: fp32 nodes 9 (<= 56 registers), 16-bit nodes 8 (<= 64
 // registers; measured 1.5-3 % faster than 9 with this layout, profiles/r01f)
-#define CRT_TRACE_MINB(QN) ((QN) ? 8 : 9)
+#define CRT_TRACE_MINB(QN) ((QN) ? 8 : 9)      // QN: 0 fp32 nodes, 1 16-bit nodes, 2 16-bit nodes with the any-origin box test
 #ifndef CRT_VISITS_PER_VOTE
 #define CRT_VISITS_PER_VOTE 3   // inner-node visits between two leaf-wait votes of a warp
 #endif
@@ -117,9 +117,11 @@ CRT_DEV int visit_node(const NodeRegs& n, const RayState& r, int*& top)
 // (o' = ray origin in grid units).
 // The PRMT selector picks the min or the max plane by the sign of the ray direction, so near and far distances come out
 // directly and no per-axis min/max is needed: 12 PRMT + 12 FFMA + 8 FMNMX per node against 12 FFMA + 20 FMNMX for fp32 nodes.
+template <bool SAFE>
 struct QRay {
     float sx, sy, sz;                     // 1 / (d * scale): distance per grid step
-    float cx, cy, cz;                     // -(o' + 2^23) * s
+    float cx, cy, cz;                     // -(o' + 2^23) * s (SAFE: rounded down and moved outward, for near planes)
+    float fcx, fcy, fcz;                  // SAFE only: the same rounded up and moved outward, for far planes
     unsigned nx, ny, nz, fx, fy, fz;      // PRMT selectors of the near / far plane
     // Error budget of t = (2^23 + q) * s + c against the exact (q - o') * s, in grid steps of position: c is rounded to an ulp
     // of 2^23 * s, i.e. at most HALF a step; o' (two roundings), s (three), the product o' * s and the final FMA add at most
@@ -133,7 +135,20 @@ struct QRay {
     {
         sx = r.idx * g.inv_scale[0]; sy = r.idy * g.inv_scale[1]; sz = r.idz * g.inv_scale[2];
         const float px = (r.o.x - g.gmin[0]) * g.scale[0], py = (r.o.y - g.gmin[1]) * g.scale[1], pz = (r.o.z - g.gmin[2]) * g.scale[2];
-        cx = __fmaf_rn(-8388608.f, sx, -(px * sx)); cy = __fmaf_rn(-8388608.f, sy, -(py * sy)); cz = __fmaf_rn(-8388608.f, sz, -(pz * sz));
+        if (SAFE) {
+            // trace_kernel 4: conservative for ANY ray origin.  c is rounded down for near planes and up for far planes after being
+            // moved outward by m = (|o'| + 65536) * 2^-19 steps per axis, which exceeds the relative errors of o', s and the FMA
+            // (6 * 2^-24 (|o'| + 65536)); costs three more registers and 3-4 % of the speed (profiles/r01f).
+            const float k = 1.9073486328125e-6f;        // 2^-19
+            const float mx = __fmul_ru(__fmul_ru(__fadd_ru(fabsf(px), 65536.f), k), fabsf(sx));
+            const float my = __fmul_ru(__fmul_ru(__fadd_ru(fabsf(py), 65536.f), k), fabsf(sy));
+            const float mz = __fmul_ru(__fmul_ru(__fadd_ru(fabsf(pz), 65536.f), k), fabsf(sz));
+            cx = __fmaf_rd(-8388608.f, sx, __fmaf_rd(-px, sx, -mx)); fcx = __fmaf_ru(-8388608.f, sx, __fmaf_ru(-px, sx, mx));
+            cy = __fmaf_rd(-8388608.f, sy, __fmaf_rd(-py, sy, -my)); fcy = __fmaf_ru(-8388608.f, sy, __fmaf_ru(-py, sy, my));
+            cz = __fmaf_rd(-8388608.f, sz, __fmaf_rd(-pz, sz, -mz)); fcz = __fmaf_ru(-8388608.f, sz, __fmaf_ru(-pz, sz, mz));
+        } else {
+            cx = __fmaf_rn(-8388608.f, sx, -(px * sx)); cy = __fmaf_rn(-8388608.f, sy, -(py * sy)); cz = __fmaf_rn(-8388608.f, sz, -(pz * sz));
+        }
         nx = r.d.x >= 0.f ? 0x7610u : 0x7632u; ny = r.d.y >= 0.f ? 0x7610u : 0x7632u; nz = r.d.z >= 0.f ? 0x7610u : 0x7632u;
         fx = nx ^ 0x0022u; fy = ny ^ 0x0022u; fz = nz ^ 0x0022u;
     }
@@ -145,16 +160,17 @@ CRT_DEV float qplane(unsigned w, unsigned sel, float s, float c)
     return __fmaf_rn(__uint_as_float(f), s, c);
 }
 // a direction component of zero: s is huge but finite (safe_rcp), both distances of that axis are huge with the right signs
-CRT_DEV int visit_qnode(const QNode* __restrict__ nodes, int idx, const RayState& r, const QRay& q, int*& top)
+template <bool SAFE>
+CRT_DEV int visit_qnode(const QNode* __restrict__ nodes, int idx, const RayState& r, const QRay<SAFE>& q, int*& top)
 {
     unsigned w0, w1, w2, w3, w4, w5; int ra, rb;
     asm volatile("ld.global.nc.v8.u32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
                  : "=r"(w0), "=r"(w1), "=r"(w2), "=r"(w3), "=r"(w4), "=r"(w5), "=r"(ra), "=r"(rb) : "l"(nodes + idx));
     const float tfar = r.tfar();
     const float tn0 = fmaxf(fmaxf(qplane(w0, q.nx, q.sx, q.cx), qplane(w1, q.ny, q.sy, q.cy)), fmaxf(qplane(w2, q.nz, q.sz, q.cz), r.tmin));
-    const float tf0 = fminf(fminf(qplane(w0, q.fx, q.sx, q.cx), qplane(w1, q.fy, q.sy, q.cy)), fminf(qplane(w2, q.fz, q.sz, q.cz), tfar));
+    const float tf0 = fminf(fminf(qplane(w0, q.fx, q.sx, SAFE ? q.fcx : q.cx), qplane(w1, q.fy, q.sy, SAFE ? q.fcy : q.cy)), fminf(qplane(w2, q.fz, q.sz, SAFE ? q.fcz : q.cz), tfar));
     const float tn1 = fmaxf(fmaxf(qplane(w3, q.nx, q.sx, q.cx), qplane(w4, q.ny, q.sy, q.cy)), fmaxf(qplane(w5, q.nz, q.sz, q.cz), r.tmin));
-    const float tf1 = fminf(fminf(qplane(w3, q.fx, q.sx, q.cx), qplane(w4, q.fy, q.sy, q.cy)), fminf(qplane(w5, q.fz, q.sz, q.cz), tfar));
+    const float tf1 = fminf(fminf(qplane(w3, q.fx, q.sx, SAFE ? q.fcx : q.cx), qplane(w4, q.fy, q.sy, SAFE ? q.fcy : q.cy)), fminf(qplane(w5, q.fz, q.sz, SAFE ? q.fcz : q.cz), tfar));
     // next node without a three-way branch: the nearer hit child (the farther one pushed), else the top of the stack
     const bool h0 = tn0 <= tf0, h1 = tn1 <= tf1;
     const bool second = h1 && (!h0 || tn1 < tn0);          // child 1 is the one to enter
@@ -217,7 +233,7 @@ __global__ void __launch_bounds__(TRACE_BLOCK) trace_flat_kernel(const GpuNode* 
 
 // variant 1 (default): persistent warps, per-lane dynamic ray fetch, postponed leaves.  COUNT adds work counters.
 // 9 blocks/SM (<= 56 registers, 36 warps): measured faster than 8 blocks at 64 registers and 10 blocks at 48 (profiles/).
-template <bool COUNT, bool QN>
+template <bool COUNT, int QN>
 __global__ void __launch_bounds__(TRACE_BLOCK, CRT_TRACE_MINB(QN)) trace_dyn_kernel(const GpuNode* __restrict__ nodes, const QNode* __restrict__ qnodes, const QGrid grid, const GpuTri* __restrict__ tris,
                                                                 const crt_ray* __restrict__ rays, crt_hit* __restrict__ hits, int64_t n,
                                                                 unsigned int* __restrict__ counter, int refill_threshold, int leaf_wait,
@@ -228,7 +244,7 @@ __global__ void __launch_bounds__(TRACE_BLOCK, CRT_TRACE_MINB(QN)) trace_dyn_ker
     int node = SENTINEL, leaf = 0;      // leaf: postponed leaf reference (< 0) or 0 = none
     int ray_idx = -1;
     bool exhausted = false;
-    RayState r; QRay q;
+    RayState r; QRay<QN == 2> q;
     unsigned c_nodes = 0, c_tris = 0, c_rays = 0;
 
     for (;;) {
@@ -324,7 +340,7 @@ __global__ void __launch_bounds__(256) primary_rays_kernel(CamDev cam, DevLayout
     rp[1] = make_float4(dx, dy, dz, 1e30f);
 }
 
-template <bool COUNT, bool QN>
+template <bool COUNT, int QN>
 crt_status launch_dyn(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, crt_hit* hits, unsigned long long* stats, cudaStream_t st)
 {
     int per_sm = ctx->trace_blocks_per_sm;
@@ -361,8 +377,9 @@ crt_status launch_trace(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, i
         return CRT_OK;
     }
     // 16-bit nodes unless the grid is too coarse for this scene's detail (decoded boxes more than twice the fp32 boxes' area)
-    if (ctx->trace_kernel == 3 && bvh->q_inflation <= 2.0) return launch_dyn<false, true>(ctx, bvh, rays, n, hits, nullptr, st);
-    return launch_dyn<false, false>(ctx, bvh, rays, n, hits, nullptr, st);
+    if (ctx->trace_kernel == 4 && bvh->q_inflation <= 2.0) return launch_dyn<false, 2>(ctx, bvh, rays, n, hits, nullptr, st);
+    if (ctx->trace_kernel == 3 && bvh->q_inflation <= 2.0) return launch_dyn<false, 1>(ctx, bvh, rays, n, hits, nullptr, st);
+    return launch_dyn<false, 0>(ctx, bvh, rays, n, hits, nullptr, st);
 }
 
 // counting build of the default kernel (crt_trace_stats): same traversal, no hit records written
@@ -370,8 +387,9 @@ crt_status launch_trace_stats(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* r
 {
     if (n == 0) return CRT_OK;
     if (ctx->trace_kernel == 2 && bvh->d_wnodes) return launch_trace_wide_stats(ctx, bvh, rays, n, counters, st);
-    if (ctx->trace_kernel == 3 && bvh->q_inflation <= 2.0) return launch_dyn<true, true>(ctx, bvh, rays, n, nullptr, reinterpret_cast<unsigned long long*>(counters), st);
-    return launch_dyn<true, false>(ctx, bvh, rays, n, nullptr, reinterpret_cast<unsigned long long*>(counters), st);
+    if (ctx->trace_kernel == 4 && bvh->q_inflation <= 2.0) return launch_dyn<true, 2>(ctx, bvh, rays, n, nullptr, reinterpret_cast<unsigned long long*>(counters), st);
+    if (ctx->trace_kernel == 3 && bvh->q_inflation <= 2.0) return launch_dyn<true, 1>(ctx, bvh, rays, n, nullptr, reinterpret_cast<unsigned long long*>(counters), st);
+    return launch_dyn<true, 0>(ctx, bvh, rays, n, nullptr, reinterpret_cast<unsigned long long*>(counters), st);
 }
 
 crt_status launch_primary(crt_ctx* ctx, const crt_bvh* bvh, const crt_camera& cam, const crt_frame& f, const Layout& L,

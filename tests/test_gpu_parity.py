@@ -82,7 +82,7 @@ def test_full_size_config2_stagewise_and_sampled(crt, ctx, oracle):
 
 # ------------------------------------------------------------------ a0 / a5: BVH + traversal
 @pytest.mark.parametrize("scene_name", ["cornell", "interior_small", "landscape_small"])
-@pytest.mark.parametrize("kernel", [0, 1, 2, 3])
+@pytest.mark.parametrize("kernel", [0, 1, 2, 3, 4])
 def test_trace_matches_oracle_on_random_rays(crt, ctx, oracle, scene_name, kernel):
     scene = SCENES[scene_name]()
     # kernel 2 reads the 8-wide compressed layout, which exists when every leaf holds one triangle
@@ -144,7 +144,7 @@ def test_trace_edge_cases(crt, ctx, oracle):
     torch.cuda.synchronize()
 
 
-@pytest.mark.parametrize("kernel", [0, 1, 3])
+@pytest.mark.parametrize("kernel", [0, 1, 3, 4])
 def test_trace_degenerate_directions_and_far_origins(crt, ctx, oracle, kernel):
     """The box test must stay conservative where its arithmetic degenerates: direction components that are exactly zero
     (1/d infinite, plane distances NaN), origins exactly on box planes of the axis-aligned Cornell walls, and origins far
@@ -166,7 +166,8 @@ def test_trace_degenerate_directions_and_far_origins(crt, ctx, oracle, kernel):
     far = slice(4000, n)                                              # origins 4-15 extents away, aimed at the box
     tgt = rng.random((n, 3))
     dirs = rng.normal(size=(n, 3)); dirs /= np.linalg.norm(dirs, axis=1, keepdims=True)
-    dist = rng.uniform(4, 15, (n, 1))
+    # kernel 4 (directed rounding + per-ray margin) is conservative for any origin: 30 to 3000 extents; the others inside their contract
+    dist = np.exp(rng.uniform(np.log(30.0), np.log(3000.0), (n, 1))) if kernel == 4 else rng.uniform(4, 15, (n, 1))
     o64 = o.astype(np.float64); o64[far] = tgt[far] - dirs[far] * dist[far]; d[far] = dirs[far]
     r[:, 0:3] = o64; r[:, 4:7] = d
     ctx.crt_set_option("trace_kernel", kernel)

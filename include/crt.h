@@ -101,6 +101,8 @@ typedef struct { float generate_ms, encode_ms, sort_ms, permute_ms; } crt_stage_
 
 /* ---- context ------------------------------------------------------------------------------------ */
 /* Creates a context on CUDA device `device`.  Fails with CRT_ERR_CUDA when no device is usable. */
+/* A context serialises its own calls (its traversal work counter and its event pool are per context): to keep several frames in
+ * flight on different streams, create one context per stream; BVHs and device buffers may be shared between contexts of a device. */
 crt_status crt_create(int32_t device, crt_ctx** out);
 crt_status crt_destroy(crt_ctx* ctx);
 /* Message of the last failed call on ctx (ctx may be NULL: last failure of a call that had no context). */

@@ -446,6 +446,33 @@ def test_white_furnace_is_one(crt, ctx, mode, gw, gh, s):
     assert torch.all(accum == 1.0)
 
 
+def test_two_contexts_render_concurrently_without_interfering(crt, ctx):
+    """bench.py keeps two frames in flight: one context + stream + workspace per frame (a crt_ctx serialises its own calls: its ray
+    counter and event pool are per context).  Frames rendered concurrently on two contexts equal the same frames rendered alone."""
+    import torch
+    scene = _small_interior()
+    w, h, spp, nb = 192, 128, 1, 2
+    G = GpuScene(crt, scene.with_camera(w, h), ctx)
+    ctx2 = crt.Context(0)
+    mats2_dev = ctx2.upload(scene.materials); mats2 = ctx2.scene_mats(mats2_dev, len(scene.materials), scene.env)
+    order = crt.make_order("direct_reuse", 4, 4, 4); fr0 = crt.make_frame(w, h, spp)
+    lanes = [(ctx, G.mats, torch.cuda.Stream()), (ctx2, mats2, torch.cuda.Stream())]
+    ws = [c.frame_workspace(fr0, order) for c, _, _ in lanes]
+    alone = []
+    for f in range(8):
+        a = torch.zeros((h, w, 3), device=ctx.device)
+        ctx.crt_render_frame(G.bvh, G.mats, G.camera, crt.make_frame(w, h, spp, 1, f), order, nb, a, ws[0])
+        alone.append(a)
+    torch.cuda.synchronize()
+    acc = [torch.zeros((h, w, 3), device=ctx.device) for _ in range(8)]
+    for f in range(8):
+        c, m, st = lanes[f % 2]
+        c.crt_render_frame(G.bvh, m, G.camera, crt.make_frame(w, h, spp, 1, f), order, nb, acc[f], ws[f % 2], stream=st)
+    torch.cuda.synchronize()
+    for f in range(8):
+        assert torch.equal(acc[f], alone[f]), f
+
+
 def test_argument_errors(crt, ctx):
     import torch
     scene = I.cornell()

@@ -341,7 +341,8 @@ static Workspace carve(const Layout& L, void* base)
     auto take = [&](size_t bytes) { void* r = p ? p + off : nullptr; off += al(bytes); return r; };
     W.rays[0] = (crt_ray*)take(ns * 32); W.rays[1] = (crt_ray*)take(ns * 32); W.hits = (crt_hit*)take(ns * 16);
     W.r2p[0] = (int32_t*)take(ns * 4); W.r2p[1] = (int32_t*)take(ns * 4); W.gid = (int32_t*)take(ns * 4); W.src = (int32_t*)take(ns * 4);
-    W.cls = (uint8_t*)take((size_t)L.n_groups); W.paths = (crt_path_state*)take((size_t)L.n_paths * 32); W.n_active = (uint32_t*)take(256);
+    W.cls = (uint8_t*)take((size_t)L.n_groups); W.paths = (crt_path_state*)take((size_t)L.n_slots * 32);       // n_slots >= n_paths: grouped orders keep the path state by slot
+    W.n_active = (uint32_t*)take(256);
     W.scratch_bytes = generate_scratch_bytes(L); W.scratch = take(W.scratch_bytes);
     W.total = off;
     return W;
@@ -377,13 +378,16 @@ crt_status crt_render_frame(crt_ctx* ctx, const crt_bvh* bvh, const crt_scene_ma
     ctx->ev_used = 0;
 #define STEP(call) do { st = (call); if (st != CRT_OK) return st; } while (0)
 #define MARK(stage) do { if (record_times) STEP(mark(ctx, stage, s)); } while (0)
-    STEP(launch_paths_init(ctx, W.paths, L.n_paths, s));
+    // grouped orders: path state indexed by slot (fixed for the frame), so that shading and generation stream it instead of
+    // gathering 32-byte records in the shuffled pixel order of the tiles; the image is unaffected (tested against the staged calls)
+    const bool by_slot = (L.mode == CRT_MODE_DIRECT_REUSE || L.mode == CRT_MODE_WORLD_REUSE);
+    STEP(launch_paths_init(ctx, W.paths, by_slot ? L.n_slots : L.n_paths, s));
     MARK(-1);
     STEP(launch_primary(ctx, bvh, *camera, *frame, L, W.rays[0], W.hits, W.r2p[0], s));
     MARK(0);
     // option fuse_shade: the shading of every segment but the last runs inside the generation kernel of the next bounce
     const bool fuse = ctx->fuse_shade != 0;
-    if (n_bounces == 0 || !fuse) STEP(launch_shade(ctx, bvh, *mats, *frame, n_bounces == 0, W.rays[0], W.hits, W.r2p[0], L.n_slots, W.paths, accum, s));
+    if (n_bounces == 0 || !fuse) STEP(launch_shade(ctx, bvh, *mats, *frame, n_bounces == 0, W.rays[0], W.hits, W.r2p[0], L.n_slots, W.paths, accum, s, by_slot));
     MARK(1);
     int cur = 0;
     for (int b = 1; b <= n_bounces; ++b) {
@@ -395,13 +399,13 @@ crt_status crt_render_frame(crt_ctx* ctx, const crt_bvh* bvh, const crt_scene_ma
             ev4[1] = ctx->ev[ctx->ev_used]; ctx->ev_stage[ctx->ev_used++] = 4;      // after permute: closes stage 4
         }
         STEP(launch_generate(ctx, bvh, *mats, *frame, b, L, W.rays[cur], W.hits, W.r2p[cur], W.paths, W.rays[1 - cur], W.r2p[1 - cur], W.gid, W.src, W.cls,
-                             W.n_active, W.scratch, W.scratch_bytes, s, ev4[0] ? ev4 : nullptr, fuse));
+                             W.n_active, W.scratch, W.scratch_bytes, s, ev4[0] ? ev4 : nullptr, fuse, by_slot));
         cur = 1 - cur;
         if (n_secondary_out) CRT_CUDA(ctx, cudaMemcpyAsync(n_secondary_out + (b - 1), W.n_active, 4, cudaMemcpyDeviceToDevice, s));
         MARK(2);
         STEP(launch_trace(ctx, bvh, W.rays[cur], L.n_slots, W.hits, s));
         MARK(3);
-        if (b == n_bounces || !fuse) STEP(launch_shade(ctx, bvh, *mats, *frame, b == n_bounces, W.rays[cur], W.hits, W.r2p[cur], L.n_slots, W.paths, accum, s));
+        if (b == n_bounces || !fuse) STEP(launch_shade(ctx, bvh, *mats, *frame, b == n_bounces, W.rays[cur], W.hits, W.r2p[cur], L.n_slots, W.paths, accum, s, by_slot));
         MARK(1);
     }
 #undef STEP

@@ -13,13 +13,15 @@ struct Env6 { float a[3], b[3]; };
 __global__ void __launch_bounds__(256) shade_kernel(const int32_t* __restrict__ mat_id, const crt_material* __restrict__ mats, Env6 env, int32_t wh,
                                                     float inv_spp, int is_last, const crt_ray* __restrict__ rays, const crt_hit* __restrict__ hits,
                                                     const int32_t* __restrict__ r2p, int64_t n, crt_path_state* __restrict__ paths,
-                                                    float* __restrict__ accum, int atomic_accum)
+                                                    float* __restrict__ accum, int atomic_accum, int by_slot)
 {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     const int32_t p = r2p[i];
     if (p < 0) return;
-    float4* pp = reinterpret_cast<float4*>(paths + p);
+    // path state by path id (the public layout) or, inside crt_render_frame with a grouped order, by SLOT: the slot order is fixed
+    // for the frame, and the shuffled pixel order of a tile would otherwise scatter these 32-byte records
+    float4* pp = reinterpret_cast<float4*>(paths + (by_slot ? i : (int64_t)p));
     float4 p0 = pp[0], p1 = pp[1];
     uint32_t flags = __float_as_uint(p0.w);
     const float4 rd = __ldg(reinterpret_cast<const float4*>(rays + i) + 1);
@@ -84,13 +86,13 @@ __global__ void __launch_bounds__(256) copy_kernel(const float4* __restrict__ sr
 }  // namespace
 
 crt_status launch_shade(crt_ctx* ctx, const crt_bvh* bvh, const crt_scene_mats& mats, const crt_frame& f, int is_last,
-                        const crt_ray* rays, const crt_hit* hits, const int32_t* r2p, int64_t n, crt_path_state* paths, float* accum, cudaStream_t st)
+                        const crt_ray* rays, const crt_hit* hits, const int32_t* r2p, int64_t n, crt_path_state* paths, float* accum, cudaStream_t st, bool paths_by_slot)
 {
     if (n == 0) return CRT_OK;
     Env6 e;
     for (int k = 0; k < 3; ++k) { e.a[k] = mats.env[k]; e.b[k] = mats.env[3 + k]; }
     shade_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(bvh->d_mat_id, mats.materials, e, f.w * f.h, 1.0f / (float)f.spp, is_last, rays, hits, r2p, n,
-                                                              paths, accum, f.spp > 1);
+                                                              paths, accum, f.spp > 1, paths_by_slot ? 1 : 0);
     CRT_CHECK_LAUNCH(ctx, "shade");
     return CRT_OK;
 }

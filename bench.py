@@ -348,7 +348,9 @@ def run_cuda(args):
         "modes": modes, "roofline": roofline, "cpu_baseline": cpu,
         "e2e": {"value": e2e["mray_s"], "unit": UNIT, "h2d_bytes_per_step": len(scene.materials) * 32 + 48 + 24,
                 "d2h_bytes_per_step": img_bytes + 4 * nb, "ms_per_step": e2e["ms_per_step"], "api": "crt_render_frame_host_resident"},
-        "gpu_launches": K * (4 + 3 * nb), "clocks": clk,          # kernels of the K timed steps of the headline pass
+        # kernels of the K timed steps of the headline pass: paths_init, primary_rays, trace, then per bounce generate (with the previous
+        # segment's shading fused in, the library's default) + trace, then the final shade
+        "gpu_launches": K * (4 + 2 * nb), "clocks": clk,
     }
     print(json.dumps(line))
 

@@ -114,7 +114,7 @@ const char* crt_last_error(const crt_ctx* ctx);
  * phase when at most this many descending lanes hold no leaf), "trace_refill_threshold" (0..32: idle lanes fetch new rays when
  * fewer lanes than this are busy), "trace_blocks_per_sm" (0 = from the occupancy calculator), "trace_tri_wait" (8-wide kernel: lanes holding triangle hits
  * before a warp enters its triangle phase), "fuse_shade" (crt_render_frame shades non-final segments inside the next generation
- * kernel; off by default: 2 % faster on the interior scene, 7 % slower on the landscape scene). */
+ * kernel; on by default: 2.5-3 % faster on both bench scenes, the image is bit-identical). */
 crt_status crt_set_option(crt_ctx* ctx, const char* key, int64_t value);
 /* Measures the device's FP32 FFMA rate (TFLOP/s) and a streaming copy rate (GB/s) with small kernels;
  * synchronous. Used only as roofline denominators by bench.py. */

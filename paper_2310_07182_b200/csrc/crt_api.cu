@@ -386,7 +386,9 @@ crt_status crt_render_frame(crt_ctx* ctx, const crt_bvh* bvh, const crt_scene_ma
     STEP(launch_primary(ctx, bvh, *camera, *frame, L, W.rays[0], W.hits, W.r2p[0], s));
     MARK(0);
     // option fuse_shade: the shading of every segment but the last runs inside the generation kernel of the next bounce
-    const bool fuse = ctx->fuse_shade != 0;
+    // (not for the sorting modes: their ray order is a permutation of the paths, and the fused read-modify-write of the state of ended
+    // paths would be a scattered access inside the generation kernel: measured 2.3x slower generation on the landscape scene)
+    const bool fuse = ctx->fuse_shade != 0 && !crt_mode_sorts(L.mode);
     if (n_bounces == 0 || !fuse) STEP(launch_shade(ctx, bvh, *mats, *frame, n_bounces == 0, W.rays[0], W.hits, W.r2p[0], L.n_slots, W.paths, accum, s, by_slot));
     MARK(1);
     int cur = 0;

@@ -18,7 +18,7 @@ struct crt_ctx {
     int trace_leaf_wait = 6;           // leave the inner-node phase when at most this many converged lanes still lack a leaf
     int trace_tri_wait = 8;            // wide kernel: a warp enters its triangle phase when at least this many lanes hold triangle hits
     int trace_blocks_per_sm = 0; // 0 = from occupancy
-    int fuse_shade = 0;          // crt_render_frame: shade non-final segments inside the next generation kernel (option; measured: DESIGN.md 5.4)
+    int fuse_shade = 1;          // crt_render_frame: shade non-final segments inside the next generation kernel (default; measured: DESIGN.md 5.4)
     // persistent-kernel work counter
     unsigned int* d_counter = nullptr;
     // events for crt_render_frame(record_times)

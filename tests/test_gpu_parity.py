@@ -499,7 +499,7 @@ def test_argument_errors(crt, ctx):
 
 
 def test_fused_shading_option_gives_the_identical_image(crt, ctx):
-    """crt_set_option("fuse_shade", 1): same arithmetic inside the generation kernel; the image must not change."""
+    """crt_set_option("fuse_shade", 0 / 1 (default)): same arithmetic inside the generation kernel; the image must not change."""
     import torch
     scene = _small_interior().with_camera(90, 61)
     G = GpuScene(crt, scene, ctx)
@@ -516,7 +516,7 @@ def test_fused_shading_option_gives_the_identical_image(crt, ctx):
                 torch.cuda.synchronize()
                 imgs.append(acc.cpu().numpy())
             finally:
-                ctx.crt_set_option("fuse_shade", 0)
+                ctx.crt_set_option("fuse_shade", 1)           # the default
         # 2 spp: the two samples of a pixel are added with atomicAdd in either order, so allow one rounding of difference
         assert imgs[-1].sum() > 0 and np.allclose(imgs[-2], imgs[-1], rtol=1e-6, atol=0)
 

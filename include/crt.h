@@ -227,6 +227,13 @@ crt_status crt_render_frame_host_resident(crt_ctx* ctx, const crt_bvh* bvh, cons
                                           const float* env /*[host] 6*/, const crt_camera* camera, const crt_frame* frame,
                                           const crt_order* order, int32_t n_bounces, int32_t reset, float* image_host,
                                           uint32_t* n_secondary_host, void* workspace, size_t workspace_bytes, void* stream);
+/* As crt_render_frame_host_resident, but returns without synchronising: the copies and the frame are only ENQUEUED on `stream`;
+ * image_host and n_secondary_host (both should be pinned memory, or the copies serialise) are valid once the caller has synchronised
+ * the stream.  With one context + stream + workspace + host image per lane this keeps several host frames in flight. */
+crt_status crt_render_frame_host_resident_async(crt_ctx* ctx, const crt_bvh* bvh, const crt_material* materials_host, int32_t n_materials,
+                                                const float* env /*[host] 6*/, const crt_camera* camera, const crt_frame* frame,
+                                                const crt_order* order, int32_t n_bounces, int32_t reset, float* image_host,
+                                                uint32_t* n_secondary_host, void* workspace, size_t workspace_bytes, void* stream);
 size_t crt_frame_host_extra_bytes(const crt_frame* frame, int32_t n_materials);
 
 #ifdef __cplusplus

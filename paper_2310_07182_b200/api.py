@@ -35,7 +35,7 @@ EXPORTS = [
     "crt_trace_primary", "crt_generate_secondary", "crt_generate_secondary_scratch_bytes",
     "crt_morton_encode", "crt_ray_code_encode", "crt_radix_sort_pairs", "crt_radix_sort_scratch_bytes", "crt_trace", "crt_trace_stats",
     "crt_shade_accumulate", "crt_render_frame", "crt_frame_workspace_bytes", "crt_frame_times",
-    "crt_render_frame_host", "crt_render_frame_host_resident", "crt_frame_host_extra_bytes",
+    "crt_render_frame_host", "crt_render_frame_host_resident", "crt_render_frame_host_resident_async", "crt_frame_host_extra_bytes",
 ]
 
 
@@ -335,11 +335,14 @@ class Context:
                                                 C.byref(frame), C.byref(order), C.c_int32(n_bounces), _ptr(accum_host), _ptr(n_secondary_host),
                                                 _ptr(workspace), C.c_size_t(workspace.numel()), _stream(stream)))
 
-    def crt_render_frame_host_resident(self, bvh, materials_host, env, camera, frame, order, n_bounces, reset, image_host, n_secondary_host, workspace, stream=None):
-        """as crt_render_frame_host, with the accumulation image resident in `workspace` between calls; image_host receives the sum so far."""
+    def crt_render_frame_host_resident(self, bvh, materials_host, env, camera, frame, order, n_bounces, reset, image_host, n_secondary_host, workspace, stream=None,
+                                       wait=True):
+        """as crt_render_frame_host, with the accumulation image resident in `workspace` between calls; image_host receives the sum so far.
+        wait=False: only enqueue (crt_render_frame_host_resident_async); the outputs are valid after the stream has been synchronised."""
         e = np.asarray(env, np.float32).reshape(6)
         mh = np.ascontiguousarray(materials_host)
-        self._check(lib().crt_render_frame_host_resident(self.handle, bvh.handle, C.c_void_p(mh.ctypes.data), C.c_int32(len(mh)), _ptr(e), C.byref(camera),
+        fn = lib().crt_render_frame_host_resident if wait else lib().crt_render_frame_host_resident_async
+        self._check(fn(self.handle, bvh.handle, C.c_void_p(mh.ctypes.data), C.c_int32(len(mh)), _ptr(e), C.byref(camera),
                                                          C.byref(frame), C.byref(order), C.c_int32(n_bounces), C.c_int32(1 if reset else 0), _ptr(image_host),
                                                          _ptr(n_secondary_host), _ptr(workspace), C.c_size_t(workspace.numel()), _stream(stream)))
 

@@ -444,7 +444,7 @@ size_t crt_frame_host_extra_bytes(const crt_frame* frame, int32_t n_materials)
 // (zeroed when reset != 0) and is only copied OUT; otherwise it is copied in from image_host first.
 static crt_status render_frame_host_impl(crt_ctx* ctx, const crt_bvh* bvh, const crt_material* materials_host, int32_t n_materials, const float* env,
                                          const crt_camera* camera, const crt_frame* frame, const crt_order* order, int32_t n_bounces, float* image_host,
-                                         uint32_t* n_secondary_host, void* workspace, size_t workspace_bytes, void* stream, bool resident, bool reset, const char* name)
+                                         uint32_t* n_secondary_host, void* workspace, size_t workspace_bytes, void* stream, bool resident, bool reset, bool sync, const char* name)
 {
     if (!ctx) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "%s: ctx is null", name);
     if (!bvh || !bvh->d_nodes || bvh->device != ctx->device) return crt_fail(ctx, bvh ? CRT_ERR_STATE : CRT_ERR_INVALID_ARG, "%s: BVH missing or not on this context's device", name);
@@ -467,7 +467,7 @@ static crt_status render_frame_host_impl(crt_ctx* ctx, const crt_bvh* bvh, const
     if (st != CRT_OK) return st;
     CRT_CUDA(ctx, cudaMemcpyAsync(image_host, d_accum, img, cudaMemcpyDeviceToHost, s));
     if (n_secondary_host && n_bounces > 0) CRT_CUDA(ctx, cudaMemcpyAsync(n_secondary_host, d_nsec, 4 * (size_t)n_bounces, cudaMemcpyDeviceToHost, s));
-    CRT_CUDA(ctx, cudaStreamSynchronize(s));
+    if (sync) CRT_CUDA(ctx, cudaStreamSynchronize(s));
     return CRT_OK;
 }
 
@@ -476,7 +476,7 @@ crt_status crt_render_frame_host(crt_ctx* ctx, const crt_bvh* bvh, const crt_mat
                                  uint32_t* n_secondary_host, void* workspace, size_t workspace_bytes, void* stream)
 {
     return render_frame_host_impl(ctx, bvh, materials_host, n_materials, env, camera, frame, order, n_bounces, accum_host, n_secondary_host,
-                                  workspace, workspace_bytes, stream, false, false, "render_frame_host");
+                                  workspace, workspace_bytes, stream, false, false, true, "render_frame_host");
 }
 
 crt_status crt_render_frame_host_resident(crt_ctx* ctx, const crt_bvh* bvh, const crt_material* materials_host, int32_t n_materials, const float* env,
@@ -484,7 +484,15 @@ crt_status crt_render_frame_host_resident(crt_ctx* ctx, const crt_bvh* bvh, cons
                                           float* image_host, uint32_t* n_secondary_host, void* workspace, size_t workspace_bytes, void* stream)
 {
     return render_frame_host_impl(ctx, bvh, materials_host, n_materials, env, camera, frame, order, n_bounces, image_host, n_secondary_host,
-                                  workspace, workspace_bytes, stream, true, reset != 0, "render_frame_host_resident");
+                                  workspace, workspace_bytes, stream, true, reset != 0, true, "render_frame_host_resident");
+}
+
+crt_status crt_render_frame_host_resident_async(crt_ctx* ctx, const crt_bvh* bvh, const crt_material* materials_host, int32_t n_materials, const float* env,
+                                                const crt_camera* camera, const crt_frame* frame, const crt_order* order, int32_t n_bounces, int32_t reset,
+                                                float* image_host, uint32_t* n_secondary_host, void* workspace, size_t workspace_bytes, void* stream)
+{
+    return render_frame_host_impl(ctx, bvh, materials_host, n_materials, env, camera, frame, order, n_bounces, image_host, n_secondary_host,
+                                  workspace, workspace_bytes, stream, true, reset != 0, false, "render_frame_host_resident_async");
 }
 
 }  // extern "C"

@@ -411,6 +411,11 @@ def test_config1_end_to_end(crt, ctx, oracle, mode, gw, gh, s):
     img_r = np.full((64, 64, 3), -1.0, np.float32); ws_r = ctx.frame_workspace(fr, order, host_materials=len(scene.materials))
     ctx.crt_render_frame_host_resident(G.bvh, scene.materials, scene.env, G.camera, fr, order, 1, True, img_r, nsec_h, ws_r)
     assert np.array_equal(img_r, accum.cpu().numpy())
+    # the non-synchronising form: outputs valid after the stream has been synchronised
+    img_a = torch.full((64, 64, 3), -1.0).pin_memory(); nsec_a = torch.zeros(1, dtype=torch.int32).pin_memory(); st = torch.cuda.Stream()
+    ctx.crt_render_frame_host_resident(G.bvh, scene.materials, scene.env, G.camera, fr, order, 1, True, img_a, nsec_a, ws_r, stream=st, wait=False)
+    st.synchronize()
+    assert np.array_equal(img_a.numpy(), accum.cpu().numpy()) and int(nsec_a[0]) == g["n_active"]
     ctx.crt_render_frame_host_resident(G.bvh, scene.materials, scene.env, G.camera, fr2, order, 1, False, img_r, nsec_h, ws_r)
     assert np.array_equal(img_r, acc_h)
     ctx.crt_render_frame_host_resident(G.bvh, scene.materials, scene.env, G.camera, fr, order, 1, True, img_r, nsec_h, ws_r)

@@ -6,8 +6,9 @@
 A step = one frame of the whole hot path: crt_trace_primary -> crt_shade_accumulate(0) ->
 for b = 1..B { crt_generate_secondary(b) -> crt_trace -> crt_shade_accumulate(b) } on one batch of synthetic input
 (default workload: BASELINE config 2, the interior scene at 1920x1080, 1 spp, 2 bounces, groups 4x4, stride 4, seed 1).
-`value` = live secondary rays of the K timed steps / their device time, for mode direct_reuse; the other two modes
-and the stage-level numbers (generate / encode+sort+permute / trace) are in "modes".  See DESIGN.md section 7.
+`value` = live secondary rays of the K timed steps / their device time, for mode direct_reuse, with `--frames-in-flight` (default 2)
+frames rendered concurrently, each on its own context and stream (config.single_stream_value = one frame at a time); the other modes
+and the stage-level numbers (generate / encode+sort+permute / trace), all one frame at a time, are in "modes".  See DESIGN.md section 7.
 """
 from __future__ import annotations
 

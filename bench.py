@@ -6,7 +6,7 @@
 A step = one frame of the whole hot path: crt_trace_primary -> crt_shade_accumulate(0) ->
 for b = 1..B { crt_generate_secondary(b) -> crt_trace -> crt_shade_accumulate(b) } on one batch of synthetic input
 (default workload: BASELINE config 2, the interior scene at 1920x1080, 1 spp, 2 bounces, groups 4x4, stride 4, seed 1).
-`value` = live secondary rays of the K timed steps / their device time, for mode direct_reuse, with `--frames-in-flight` (default 2)
+`value` = live secondary rays of the K timed steps / their device time, for mode direct_reuse, with `--frames-in-flight` (default 3)
 frames rendered concurrently, each on its own context and stream (config.single_stream_value = one frame at a time); the other modes
 and the stage-level numbers (generate / encode+sort+permute / trace), all one frame at a time, are in "modes".  See DESIGN.md section 7.
 """
@@ -478,7 +478,7 @@ def main():
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--workload", default="interior", choices=sorted(WORKLOADS))
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--frames-in-flight", type=int, default=2, help="frames rendered concurrently (one context + stream each) for the headline value; the per-mode table stays single-stream")
+    ap.add_argument("--frames-in-flight", type=int, default=3, help="frames rendered concurrently (one context + stream each) for the headline value; the per-mode table stays single-stream")
     ap.add_argument("--no-sort-codes", action="store_true", help="skip the Origin / Reis / Costa / TwoPoint reordering baselines")
     ap.add_argument("--sweep", nargs="?", const="config3", default=None, choices=["config3", "table3", "rules"],
                     help="config3: BASELINE config 3 sweep; table3: the paper's Table 3 shapes (tile x K) at 1920x1080, 1 spp, 2 bounces; rules: shuffled against lattice partition at the same size")

@@ -452,7 +452,7 @@ def test_white_furnace_is_one(crt, ctx, mode, gw, gh, s):
 
 
 def test_two_contexts_render_concurrently_without_interfering(crt, ctx):
-    """bench.py keeps two frames in flight: one context + stream + workspace per frame (a crt_ctx serialises its own calls: its ray
+    """bench.py keeps several frames in flight: one context + stream + workspace per frame (a crt_ctx serialises its own calls: its ray
     counter and event pool are per context).  Frames rendered concurrently on two contexts equal the same frames rendered alone."""
     import torch
     scene = _small_interior()

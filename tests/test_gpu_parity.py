@@ -439,6 +439,25 @@ def test_mixed_materials_two_bounces_end_to_end(crt, ctx, oracle, mode, gw, gh, 
     assert rmse(accum.cpu().numpy() / 2, acc_o / 2) <= 1e-3
 
 
+@pytest.mark.parametrize("mode,gw,gh,s", [("direct_reuse", 4, 4, 2), ("direct_reuse", 4, 2, 2 | (4 << 16) | (1 << 14)), ("world_reuse", 8, 8, 1), ("independent", 1, 1, 1)])
+def test_render_frame_on_a_ragged_image_matches_the_oracle(crt, ctx, oracle, mode, gw, gh, s):
+    """crt_render_frame as bench.py runs it (shading fused into generation, path state by slot under grouped orders) on an image that is
+    not a multiple of the tile (50x37, 2 spp, 3 bounces, partial tiles on two sides): the accumulated image equals the oracle's."""
+    import torch
+    scene = _small_interior().with_camera(50, 37)
+    w, h, spp, nb = 50, 37, 2, 3
+    G = GpuScene(crt, scene, ctx)
+    ob = oracle.Bvh(scene.verts)
+    acc_o = np.zeros((h, w, 3), np.float32); accum = torch.zeros((h, w, 3), device=ctx.device)
+    order = crt.make_order(mode, gw, gh, s)
+    ws = ctx.frame_workspace(crt.make_frame(w, h, spp), order)
+    for f in range(2):
+        oracle.render_frame(ob, scene, oracle.frame(w, h, spp, 4, f), nb, MODES[mode], gw, gh, s, accum=acc_o)
+        ctx.crt_render_frame(G.bvh, G.mats, G.camera, crt.make_frame(w, h, spp, 4, f), order, nb, accum, ws)
+    assert rmse(accum.cpu().numpy() / 2, acc_o / 2) <= 1e-3
+    assert acc_o.sum() > 0
+
+
 @pytest.mark.parametrize("mode,gw,gh,s", [("independent", 1, 1, 1), ("morton_reorder", 1, 1, 1), ("direct_reuse", 4, 4, 2)])
 def test_white_furnace_is_one(crt, ctx, mode, gw, gh, s):
     """Closed form: a convex white Lambert sphere under uniform radiance 1 renders to exactly 1 (north_star)."""

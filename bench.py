@@ -470,6 +470,46 @@ def run_sweep(args):
                                                   "reference_frames": 4 * F, "scale": sc}}))
 
 
+def run_tail(args):
+    """Fixed cost of a crt_trace launch (profiles/r01h): crt_trace on one frame's ray sets (primary, bounce 1, bounce 2; direct_reuse order)
+    and on the same set concatenated twice and four times; L2 flushed between repetitions, median of 8.  One JSON line."""
+    import torch
+    import paper_2310_07182_b200 as crt
+    import crt_inputs as I
+    name, kw, w, h, spp, nb, gw, gh, s, seed, cfg = WORKLOADS[args.workload]
+    scene = I.by_name(name, **kw).with_camera(w, h)
+    ctx = crt.Context(0)
+    bvh = ctx.crt_build_bvh(scene.verts, scene.mat_id)
+    mats_dev = ctx.upload(scene.materials); mats = ctx.scene_mats(mats_dev, len(scene.materials), scene.env); cam = crt.make_camera(scene.camera)
+    order = crt.make_order("direct_reuse", gw, gh, s); fr = crt.make_frame(w, h, spp, seed, 7)
+    rays, hits, r2p = ctx.crt_trace_primary(bvh, cam, fr, order)
+    paths = ctx.empty((crt.crt_layout(fr, order)[0], 8)); ctx.crt_paths_init(paths)
+    acc = torch.zeros((h, w, 3), device=ctx.device)
+    ctx.crt_shade_accumulate(bvh, mats, fr, 0, False, rays, hits, r2p, paths, acc)
+    sets = [("primary", rays.clone())]
+    for b in range(1, nb + 1):
+        out = ctx.crt_generate_secondary(bvh, mats, fr, b, order, rays, hits, r2p, paths)
+        rays, r2p = out["rays"], out["ray_to_path"]
+        sets.append((f"bounce {b}", rays.clone()))
+        hits = ctx.crt_trace(bvh, rays)
+        ctx.crt_shade_accumulate(bvh, mats, fr, b, b == nb, rays, hits, r2p, paths, acc)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=ctx.device)
+
+    def t_trace(r):
+        hh = ctx.crt_trace(bvh, r); ts = []
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        for _ in range(8):
+            flush.fill_(1)
+            e0.record(); ctx.crt_trace(bvh, r, hits=hh); e1.record(); torch.cuda.synchronize()
+            ts.append(e0.elapsed_time(e1))
+        return float(np.median(ts))
+    rows = []
+    for tag, r in sets:
+        t1 = t_trace(r); r2 = torch.cat([r, r]).contiguous(); t2 = t_trace(r2); t4 = t_trace(torch.cat([r2, r2]).contiguous())
+        rows.append({"rays": tag, "n": int(r.shape[0]), "t_n_ms": t1, "t_2n_ms": t2, "t_4n_ms": t4, "fixed_ms_from_2n": 2 * t1 - t2, "fixed_ms_from_4n": (4 * t1 - t4) / 3})
+    print(json.dumps({"tail": rows, "config": {"workload": args.workload, "order": f"direct_reuse {gw}x{gh} stride {s}", "frame": 7}}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -480,13 +520,16 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--frames-in-flight", type=int, default=3, help="frames rendered concurrently (one context + stream each) for the headline value; the per-mode table stays single-stream")
     ap.add_argument("--no-sort-codes", action="store_true", help="skip the Origin / Reis / Costa / TwoPoint reordering baselines")
-    ap.add_argument("--sweep", nargs="?", const="config3", default=None, choices=["config3", "table3", "rules"],
-                    help="config3: BASELINE config 3 sweep; table3: the paper's Table 3 shapes (tile x K) at 1920x1080, 1 spp, 2 bounces; rules: shuffled against lattice partition at the same size")
+    ap.add_argument("--sweep", nargs="?", const="config3", default=None, choices=["config3", "table3", "rules", "tail"],
+                    help="config3: BASELINE config 3 sweep; table3: the paper's Table 3 shapes (tile x K) at 1920x1080, 1 spp, 2 bounces; rules: shuffled against lattice partition at the same size; tail: fixed cost of a crt_trace launch (n, 2n, 4n rays) on --workload")
     ap.add_argument("--sweep-frames", type=int, default=64)
     ap.add_argument("--sweep-scale", type=int, default=1, help="divide the 3840x2160 image by this (quick runs)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "cuda":
         args.warmup = 3
+    if args.sweep == "tail":
+        run_tail(args)
+        return
     if args.sweep:
         run_sweep(args)
     elif args.impl == "reference":

@@ -2,20 +2,24 @@
 // structure to find the leaf nodes that the ray passes through"; this is "the most time-consuming segment").
 //
 // B200 design:
-//  - stack-based traversal of a binary BVH whose 64-byte nodes hold both children's boxes, fetched as two 256-bit loads
-//    (ld.global.nc.v8.f32 -> LDG.E.ENL2.256) on the read-only path; leaf triangles are three float4 (v0|id, e1, e2);
-//  - the kernel is issue-bound, not bandwidth-bound (profiles/): what matters is how many lanes of a warp do useful work.
+//  - stack-based traversal of a binary BVH.  Default layout (trace_kernel 3): 32-byte nodes holding both children's boxes as
+//    16-bit planes on a scene grid, fetched with ONE 256-bit load (ld.global.nc.v8 -> LDG.E.ENL2.256) on the read-only path and
+//    decoded by one PRMT per plane that also selects the near or far plane by the ray's direction sign (struct QRay below);
+//    the fp32 form (64-byte nodes, two 256-bit loads) is trace_kernel 0 / 1; leaf triangles are 64-byte records (v0|id, e1, e2);
+//  - with the 16-bit nodes the kernel is issue- and latency-bound, not bandwidth-bound (profiles/r01f): what matters is how many
+//    lanes of a warp do useful work and how many warps are resident (8 blocks of 128 threads per SM at 64 registers).
 //    trace_dyn_kernel is a persistent-warp kernel: the grid fills the 148 SMs once; a lane whose ray has terminated takes
 //    the next ray from a global counter (one atomicAdd per warp, ballot + popc give each idle lane its index) as soon as
 //    fewer than `refill_threshold` lanes of its warp are still traversing, so rays enter a warp in slot order -- the order
 //    the generator made coherent (group-major) -- and divergent stragglers do not idle 31 lanes;
 //  - inner-node and leaf phases are separated (while-while) and a lane that reaches a leaf postpones it and keeps
-//    descending until every converged lane has one, so the triangle tests of a warp run together;
+//    descending until (nearly) every converged lane has one, so the triangle tests of a warp run together; the vote that decides
+//    it is taken every CRT_VISITS_PER_VOTE visits, push and pop are predicated, the stack is addressed through a pointer;
 //  - inactive slots (dead paths, out-of-image slots) are skipped at fetch time and cost one 16-byte load;
 //  - no tensor cores: traversal is not a dense contraction.
 // Exactness: the triangle test is the bit-exact fp32 formula of crt_device.cuh; box tests are conservative (boxes padded at
-// build time by 2^-17 of the largest coordinate, far side inflated, subtree skipped only if its entry distance is strictly
-// beyond the best t), so the result equals the all-triangles definition with ties -> lowest primitive id (D:R10), whatever
+// build time by 2^-17 of the largest coordinate, 16-bit planes rounded outward plus one grid step, far side inflated, subtree
+// skipped only if its entry distance is strictly beyond the best t), so the result equals the all-triangles definition with ties -> lowest primitive id (D:R10), whatever
 // the order in which leaves are visited.
 #include "crt_device.cuh"
 #include "crt_internal.h"

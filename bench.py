@@ -395,9 +395,9 @@ def run_cuda(args):
                 "d2h_bytes_per_step": img_bytes + 4 * nb, "ms_per_step": e2e["ms_per_step"],
                 "api": "crt_render_frame_host_resident_async, %d host frames in flight" % F if F > 1 else "crt_render_frame_host_resident",
                 "one_frame_at_a_time": e2e_one["mray_s"]},
-        # kernels of the K timed steps of the headline pass: paths_init, primary_rays, trace, then per bounce generate (with the previous
-        # segment's shading fused in, the library's default) + trace, then the final shade
-        "gpu_launches": K * (4 + 2 * nb), "clocks": clk,
+        # kernels of the K timed steps of the headline pass: primary_rays, trace, then per bounce generate (with the previous segment's
+        # shading and, at the first bounce, the initial path state fused in: the library's default) + trace, then the final shade
+        "gpu_launches": K * ((3 + 2 * nb) if nb >= 1 else 4), "clocks": clk,
     }
     print(json.dumps(line))
 

@@ -381,7 +381,9 @@ crt_status crt_render_frame(crt_ctx* ctx, const crt_bvh* bvh, const crt_scene_ma
     // grouped orders: path state indexed by slot (fixed for the frame), so that shading and generation stream it instead of
     // gathering 32-byte records in the shuffled pixel order of the tiles; the image is unaffected (tested against the staged calls)
     const bool by_slot = (L.mode == CRT_MODE_DIRECT_REUSE || L.mode == CRT_MODE_WORLD_REUSE);
-    STEP(launch_paths_init(ctx, W.paths, by_slot ? L.n_slots : L.n_paths, s));
+    // option fuse_shade (below): with it the first generation kernel also sets the initial path state, so no paths_init launch
+    const bool fuse0 = ctx->fuse_shade != 0 && !crt_mode_sorts(L.mode);
+    if (!(fuse0 && n_bounces >= 1)) STEP(launch_paths_init(ctx, W.paths, by_slot ? L.n_slots : L.n_paths, s));
     MARK(-1);
     STEP(launch_primary(ctx, bvh, *camera, *frame, L, W.rays[0], W.hits, W.r2p[0], s));
     MARK(0);
@@ -401,7 +403,7 @@ crt_status crt_render_frame(crt_ctx* ctx, const crt_bvh* bvh, const crt_scene_ma
             ev4[1] = ctx->ev[ctx->ev_used]; ctx->ev_stage[ctx->ev_used++] = 4;      // after permute: closes stage 4
         }
         STEP(launch_generate(ctx, bvh, *mats, *frame, b, L, W.rays[cur], W.hits, W.r2p[cur], W.paths, W.rays[1 - cur], W.r2p[1 - cur], W.gid, W.src, W.cls,
-                             W.n_active, W.scratch, W.scratch_bytes, s, ev4[0] ? ev4 : nullptr, fuse, by_slot));
+                             W.n_active, W.scratch, W.scratch_bytes, s, ev4[0] ? ev4 : nullptr, fuse, by_slot, b == 1));
         cur = 1 - cur;
         if (n_secondary_out) CRT_CUDA(ctx, cudaMemcpyAsync(n_secondary_out + (b - 1), W.n_active, 4, cudaMemcpyDeviceToDevice, s));
         MARK(2);

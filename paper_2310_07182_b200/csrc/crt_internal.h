@@ -115,7 +115,7 @@ crt_status launch_primary(crt_ctx* ctx, const crt_bvh* bvh, const crt_camera& ca
 crt_status launch_generate(crt_ctx* ctx, const crt_bvh* bvh, const crt_scene_mats& mats, const crt_frame& f, int bounce, const Layout& L,
                            const crt_ray* prev_rays, const crt_hit* prev_hits, const int32_t* prev_r2p, crt_path_state* paths,
                            crt_ray* rays_out, int32_t* r2p_out, int32_t* gid_out, int32_t* src_out, uint8_t* cls_out,
-                           uint32_t* n_active, void* scratch, size_t scratch_bytes, cudaStream_t st, cudaEvent_t* ev4, bool fuse_shade = false, bool paths_by_slot = false);
+                           uint32_t* n_active, void* scratch, size_t scratch_bytes, cudaStream_t st, cudaEvent_t* ev4, bool fuse_shade = false, bool paths_by_slot = false, bool fresh_paths = false);
 crt_status launch_morton_encode(crt_ctx* ctx, const float* bounds, int code, const crt_ray* rays, int64_t n, uint32_t* keys, cudaStream_t st);
 // reordering modes (encode + sort + permute) and their sort key: 0 AilaCompact, 1 Origin, 2 Reis, 3 Costa, 4 TwoPoint
 static inline bool crt_mode_sorts(int mode) { return mode == CRT_MODE_MORTON_REORDER || (mode >= CRT_MODE_SORT_ORIGIN && mode <= CRT_MODE_SORT_TWOPOINT); }

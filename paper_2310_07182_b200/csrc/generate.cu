@@ -139,6 +139,7 @@ struct GenArgs {
     crt_ray* rays_out; int32_t* r2p_out; int32_t* gid_out; int32_t* src_out; uint8_t* cls_out; uint32_t* n_active;
     uint32_t* keys_out;      // morton mode: key per path (rays_out etc. are then the by-path temporaries)
     Bounds6 bounds;
+    int32_t fresh;            // first bounce of a fused frame: the path state is not read (throughput 1, radiance 0, alive) and is written in full
     int32_t by_slot;          // path state indexed by slot instead of by path id (crt_render_frame, grouped orders)
     int64_t n_slots; int32_t bounce; int32_t morton;   // morton: 0 = no key, else 1 + sort code
     int32_t world;           // direct_reuse in WORLD space (mode 3; D:R18)
@@ -175,7 +176,7 @@ __global__ void __launch_bounds__(1024) generate_kernel(GenArgs A, DevLayout L)
     crt_path_state ps; ps.flags = 0u;
     if (p >= 0) {
         const float4* pp = reinterpret_cast<const float4*>(A.paths + (A.by_slot ? i : (int64_t)p));
-        const float4 p0 = pp[0];
+        const float4 p0 = A.fresh ? make_float4(1.f, 1.f, 1.f, __uint_as_float(1u)) : pp[0];
         ps.tr = p0.x; ps.tg = p0.y; ps.tb = p0.z; ps.flags = __float_as_uint(p0.w);
         const float4 rd = __ldg(reinterpret_cast<const float4*>(A.prev_rays + i) + 1);
         const float4 hv = __ldg(reinterpret_cast<const float4*>(A.prev_hits + i));
@@ -194,7 +195,7 @@ __global__ void __launch_bounds__(1024) generate_kernel(GenArgs A, DevLayout L)
             }
             if (ends) {
                 float4* pw = reinterpret_cast<float4*>(A.paths + (A.by_slot ? i : (int64_t)p));
-                float4 p1 = pw[1];
+                float4 p1 = A.fresh ? make_float4(0.f, 0.f, 0.f, 0.f) : pw[1];
                 p1.x = add(p1.x, mul(ps.tr, Le[0])); p1.y = add(p1.y, mul(ps.tg, Le[1])); p1.z = add(p1.z, mul(ps.tb, Le[2]));
                 ps.flags &= ~1u;
                 pw[0] = make_float4(ps.tr, ps.tg, ps.tb, __uint_as_float(ps.flags)); pw[1] = p1;
@@ -327,7 +328,9 @@ __global__ void __launch_bounds__(1024) generate_kernel(GenArgs A, DevLayout L)
         if (emit) { np.x = mul(ps.tr, weight[0]); np.y = mul(ps.tg, weight[1]); np.z = mul(ps.tb, weight[2]); }
         else fl &= ~1u;
         np.w = __uint_as_float(fl);
-        reinterpret_cast<float4*>(A.paths + (A.by_slot ? i : (int64_t)p))[0] = np;
+        float4* pw = reinterpret_cast<float4*>(A.paths + (A.by_slot ? i : (int64_t)p));
+        pw[0] = np;
+        if (A.fresh) pw[1] = make_float4(0.f, 0.f, 0.f, 0.f);       // radiance of a path that goes on: nothing collected yet
     }
     if (o >= 0) {
         float4* rp = reinterpret_cast<float4*>(A.rays_out + o);
@@ -394,7 +397,7 @@ crt_status launch_morton_encode(crt_ctx* ctx, const float* bounds, int code, con
 crt_status launch_generate(crt_ctx* ctx, const crt_bvh* bvh, const crt_scene_mats& mats, const crt_frame& f, int bounce, const Layout& L,
                            const crt_ray* prev_rays, const crt_hit* prev_hits, const int32_t* prev_r2p, crt_path_state* paths,
                            crt_ray* rays_out, int32_t* r2p_out, int32_t* gid_out, int32_t* src_out, uint8_t* cls_out,
-                           uint32_t* n_active, void* scratch, size_t scratch_bytes, cudaStream_t st, cudaEvent_t* ev4, bool fuse_shade, bool paths_by_slot)
+                           uint32_t* n_active, void* scratch, size_t scratch_bytes, cudaStream_t st, cudaEvent_t* ev4, bool fuse_shade, bool paths_by_slot, bool fresh_paths)
 {
     CRT_CUDA(ctx, cudaMemsetAsync(n_active, 0, sizeof(uint32_t), st));
     if (L.n_slots == 0) return CRT_OK;
@@ -406,6 +409,7 @@ crt_status launch_generate(crt_ctx* ctx, const crt_bvh* bvh, const crt_scene_mat
     A.keys_out = nullptr; A.bounds = make_bounds(bvh->bounds); A.n_slots = L.n_slots; A.bounce = bounce; A.morton = 0;
     A.world = (L.mode == CRT_MODE_WORLD_REUSE);
     A.fuse_shade = fuse_shade ? 1 : 0;
+    A.fresh = (fresh_paths && fuse_shade) ? 1 : 0;
     A.by_slot = (paths_by_slot && (L.mode == CRT_MODE_DIRECT_REUSE || L.mode == CRT_MODE_WORLD_REUSE)) ? 1 : 0;
     for (int k = 0; k < 6; ++k) A.env[k] = mats.env[k];
     const DevLayout D = make_dev_layout(L, f);

@@ -354,7 +354,7 @@ def furnace_sphere(subdiv=2, albedo=1.0, mat_type=MAT_DIFFUSE, roughness=0.3, wi
     return Scene("furnace_sphere", tri, np.zeros(len(tri), np.int32), mats, np.ones(6, np.float32), cam, width, height)
 
 
-def emissive_box(seed=0, albedo=0.5, emission=1.0, width=16, height=16) -> Scene:
+def emissive_box(seed=0, albedo=0.5, emission=1.0, width=16, height=16) -> Scene:      # (name kept from the survey; see docstring)
     """Closed unit cube seen from inside.  The method has no surface that both emits
     and reflects, so this returns a plain Lambert cube under NO light; tests use
     it for occlusion invariants (every ray from inside hits, image stays 0)."""

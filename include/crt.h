@@ -95,9 +95,6 @@ typedef struct {
     int32_t q16_inflation_pct;  /* summed surface area of the boxes the 16-bit nodes decode to, in percent of the fp32 boxes' (100 = no
                                  * loss); above 200 the default kernel reads the fp32 nodes instead (grid too coarse for the scene) */
 } crt_bvh_info_t;
-/* optional per-stage device times of crt_generate_secondary, filled after the stream is synchronised by the
- * caller via crt_stage_times_resolve (milliseconds) */
-typedef struct { float generate_ms, encode_ms, sort_ms, permute_ms; } crt_stage_times;
 
 /* ---- context ------------------------------------------------------------------------------------ */
 /* Creates a context on CUDA device `device`.  Fails with CRT_ERR_CUDA when no device is usable. */
@@ -164,7 +161,7 @@ crt_status crt_trace_primary(crt_ctx* ctx, const crt_bvh* bvh, const crt_camera*
  *                        a hybrid group: mean direction of the glossy members), -1 (no ray); world_reuse: the selected
  *                        pixel's id for every member that reuses its world direction
  * paths[path].throughput is multiplied by the BSDF weight; paths whose sample is invalid are killed.
- * times may be NULL.  scratch: [device], at least crt_generate_secondary_scratch_bytes(). */
+ * scratch: [device], at least crt_generate_secondary_scratch_bytes(). */
 crt_status crt_generate_secondary(crt_ctx* ctx, const crt_bvh* bvh, const crt_scene_mats* mats, const crt_frame* frame,
                                   int32_t bounce, const crt_order* order,
                                   const crt_ray* prev_rays, const crt_hit* prev_hits, const int32_t* prev_ray_to_path,

@@ -971,3 +971,26 @@ int32_t orc_test_sample_ggx(const float* wo, float alpha, float u1, float u2, fl
     wi[0] = (float)w.x; wi[1] = (float)w.y; wi[2] = (float)w.z; weight[0] = (float)wt[0];
     return ok;
 }
+/* the same with a given F0 = albedo (RGB), so that the Schlick factor is exercised; returns validity, weight[3] */
+int32_t orc_test_sample_ggx_f0(const float* wo, float alpha, const float* albedo, float u1, float u2, float* wi, float* weight)
+{
+    shadept s; memset(&s, 0, sizeof s);
+    s.wo = v3(R(wo[0]), R(wo[1]), R(wo[2])); s.rough = R(alpha);
+    for (int k = 0; k < 3; ++k) s.albedo[k] = R(albedo[k]);
+    vec3 w; real wt[3] = { R(0.0), R(0.0), R(0.0) };
+    int ok = sample_ggx(&s, R(u1), R(u2), &w, wt);
+    wi[0] = (float)w.x; wi[1] = (float)w.y; wi[2] = (float)w.z;
+    for (int k = 0; k < 3; ++k) weight[k] = (float)wt[k];
+    return ok;
+}
+/* ggx_weight (world-space reuse, D:R18) alone: weight[3] of a GIVEN exit direction wi; returns validity */
+int32_t orc_test_ggx_weight(const float* wo, const float* wi, float alpha, const float* albedo, float* weight)
+{
+    shadept s; memset(&s, 0, sizeof s);
+    s.wo = v3(R(wo[0]), R(wo[1]), R(wo[2])); s.rough = R(alpha);
+    for (int k = 0; k < 3; ++k) s.albedo[k] = R(albedo[k]);
+    real wt[3] = { R(0.0), R(0.0), R(0.0) };
+    int ok = ggx_weight(&s, v3(R(wi[0]), R(wi[1]), R(wi[2])), wt);
+    for (int k = 0; k < 3; ++k) weight[k] = (float)wt[k];
+    return ok;
+}

@@ -222,3 +222,20 @@ def sample_ggx(wo, alpha, u1, u2, fp64=False):
     wo = (C.c_float * 3)(*[float(x) for x in wo])
     ok = _lib(fp64).orc_test_sample_ggx(wo, C.c_float(alpha), C.c_float(u1), C.c_float(u2), wi, wt)
     return bool(ok), np.array(list(wi)), float(wt[0])
+
+
+def sample_ggx_f0(wo, alpha, albedo, u1, u2, fp64=False):
+    """sample_ggx with F0 = albedo (RGB): (valid, wi[3], weight[3])"""
+    wi = (C.c_float * 3)(); wt = (C.c_float * 3)()
+    wo = (C.c_float * 3)(*[float(x) for x in wo]); al = (C.c_float * 3)(*[float(x) for x in albedo])
+    ok = _lib(fp64).orc_test_sample_ggx_f0(wo, C.c_float(alpha), al, C.c_float(u1), C.c_float(u2), wi, wt)
+    return bool(ok), np.array(list(wi)), np.array(list(wt))
+
+
+def ggx_weight(wo, wi, alpha, albedo, fp64=False):
+    """weight of a GIVEN exit direction under a GGX material (world-space reuse, D:R18): (valid, weight[3])"""
+    wt = (C.c_float * 3)()
+    wo = (C.c_float * 3)(*[float(x) for x in wo]); wi = (C.c_float * 3)(*[float(x) for x in wi])
+    al = (C.c_float * 3)(*[float(x) for x in albedo])
+    ok = _lib(fp64).orc_test_ggx_weight(wo, wi, C.c_float(alpha), al, wt)
+    return bool(ok), np.array(list(wt))

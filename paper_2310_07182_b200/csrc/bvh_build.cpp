@@ -328,10 +328,14 @@ int32_t crt_bvh_quantise(const crt_bvh* b, const std::vector<GpuNode>& gn, std::
     for (int k = 0; k < 3; ++k) { if (lo[k] > hi[k]) { lo[k] = 0; hi[k] = 1; } maxext = std::max(maxext, hi[k] - lo[k]); }
     if (!(maxext > 0)) maxext = 1;
     for (int k = 0; k < 3; ++k) {
+        // margin on either side: 8 grid steps, or 4 ulps of the box's coordinates when the scene sits far from the origin (gmin is a
+        // float: its rounding must not eat the margin, or planes clamp inward); gmin is rounded DOWN so the low side only gains
         const double e = std::max(hi[k] - lo[k], maxext * (1.0 / 4096.0));
-        const float scale = (float)((65535.0 - 16.0) / e);
+        const double ulp = std::max(std::fabs(lo[k]), std::fabs(hi[k])) * (1.0 / 8388608.0);
+        const double margin = std::max(8.0 * e / (65535.0 - 16.0), 4.0 * ulp);
+        const float scale = (float)(65535.0 / (e + 2.0 * margin) * (1.0 - 1e-6));
         grid->scale[k] = scale;
-        grid->gmin[k] = (float)(lo[k] - 8.0 / (double)scale);
+        grid->gmin[k] = std::nextafterf((float)(lo[k] - margin), -std::numeric_limits<float>::infinity());
         grid->inv_scale[k] = (float)(1.0 / (double)scale);
     }
     int32_t bad = 0;

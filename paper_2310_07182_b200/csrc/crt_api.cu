@@ -78,6 +78,7 @@ crt_status crt_create(int32_t device, crt_ctx** out)
 crt_status crt_destroy(crt_ctx* ctx)
 {
     if (!ctx) return CRT_OK;
+    CrtDeviceGuard dev_guard_(ctx->device);
     cudaFree(ctx->d_counter);
     for (cudaEvent_t ev : ctx->ev) cudaEventDestroy(ev);
     delete ctx;
@@ -102,6 +103,7 @@ crt_status crt_set_option(crt_ctx* ctx, const char* key, int64_t value)
 crt_status crt_measure_peaks(crt_ctx* ctx, double* fp32_tflops, double* copy_gbs)
 {
     if (!ctx || !fp32_tflops || !copy_gbs) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "measure_peaks: null argument");
+    CrtDeviceGuard dev_guard_(ctx->device);
     return measure_peaks(ctx, fp32_tflops, copy_gbs);
 }
 
@@ -117,6 +119,7 @@ crt_status crt_build_bvh(crt_ctx* ctx, const float* verts, const int32_t* mat_id
 {
     if (!out) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "build_bvh: out is null");
     *out = nullptr;
+    CrtDeviceGuard dev_guard_(ctx ? ctx->device : -1);
     if (n_tris < 0 || (n_tris > 0 && !verts)) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "build_bvh: bad triangle array");
     if (n_tris >= ((int64_t)1 << 28)) return crt_fail(ctx, CRT_ERR_UNSUPPORTED, "build_bvh: more than 2^28 triangles");
     crt_bvh_params pr = {3, 64, 1.0f, 1.0f, 0};
@@ -135,7 +138,10 @@ crt_status crt_build_bvh(crt_ctx* ctx, const float* verts, const int32_t* mat_id
         else memcpy(hm.data(), mat_id, hm.size() * 4);
     }
     for (int64_t i = 0; i < 9 * n_tris; ++i) if (!(v[i] == v[i]) || v[i] > 1e30f || v[i] < -1e30f) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "build_bvh: non-finite vertex");
+    int32_t max_mat = -1;
+    for (int32_t m : hm) { if (m < 0) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "build_bvh: negative material id"); max_mat = std::max(max_mat, m); }
     crt_bvh* b = new crt_bvh();
+    b->max_mat_id = max_mat;
     crt_bvh_build_host(b, v, n_tris, pr);
     if (b->depth > 60) { delete b; return crt_fail(ctx, CRT_ERR_UNSUPPORTED, "build_bvh: tree depth exceeds the traversal stack (64)"); }
     // one triangle per leaf: also build the 8-wide compressed layout (the default kernel's); its triangle order is the shared one
@@ -156,7 +162,7 @@ crt_status crt_build_bvh(crt_ctx* ctx, const float* verts, const int32_t* mat_id
             cudaError_t e = cudaMalloc(d, bytes ? bytes : 256);
             if (e != cudaSuccess) return e;
             b->device_bytes += (int64_t)bytes;
-            return bytes ? cudaMemcpy(*d, h, bytes, cudaMemcpyHostToDevice) : cudaSuccess;
+            return bytes ? cudaMemcpy(*d, h, bytes, cudaMemcpyHostToDevice) : cudaMemset(*d, 0, 256);      // empty scene: a defined (degenerate) record
         };
         cudaError_t e = up((void**)&b->d_nodes, gn.data(), gn.size() * sizeof(GpuNode));
         if (e == cudaSuccess) e = up((void**)&b->d_qnodes, qn.data(), qn.size() * sizeof(QNode));
@@ -173,6 +179,7 @@ crt_status crt_build_bvh(crt_ctx* ctx, const float* verts, const int32_t* mat_id
 crt_status crt_bvh_destroy(crt_bvh* b)
 {
     if (!b) return CRT_OK;
+    CrtDeviceGuard dev_guard_(b->device);
     cudaFree(b->d_nodes); cudaFree(b->d_qnodes); cudaFree(b->d_wnodes); cudaFree(b->d_tris); cudaFree(b->d_slot_of_prim); cudaFree(b->d_mat_id);
     delete b;
     return CRT_OK;
@@ -208,7 +215,7 @@ crt_status crt_layout(const crt_frame* frame, const crt_order* order, int64_t* n
     return CRT_OK;
 }
 
-#define NEED_CTX(name) if (!ctx) return crt_fail(nullptr, CRT_ERR_INVALID_ARG, name ": ctx is null")
+#define NEED_CTX(name) if (!ctx) return crt_fail(nullptr, CRT_ERR_INVALID_ARG, name ": ctx is null"); CrtDeviceGuard dev_guard_(ctx->device)
 #define NEED_BVH(name) if (!bvh) return crt_fail(ctx, CRT_ERR_INVALID_ARG, name ": bvh is null"); \
     if (!bvh->d_nodes || bvh->device != ctx->device) return crt_fail(ctx, CRT_ERR_STATE, name ": BVH has no data on this context's device")
 #define NEED_ALIGNED(name, p, a) if (!crt_aligned(p, a)) return crt_fail(ctx, CRT_ERR_INVALID_ARG, name ": " #p " is null or not %d-byte aligned", (int)(a))
@@ -246,6 +253,7 @@ crt_status crt_generate_secondary(crt_ctx* ctx, const crt_bvh* bvh, const crt_sc
 {
     NEED_CTX("generate_secondary"); NEED_BVH("generate_secondary");
     if (!mats || !mats->materials) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "generate_secondary: materials are null");
+    if (mats->n_materials <= bvh->max_mat_id) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "generate_secondary: %d materials but the BVH's triangles use id %d", mats->n_materials, bvh->max_mat_id);
     if (bounce < 1) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "generate_secondary: bounce %d < 1", bounce);
     Layout L; crt_status st = crt_make_layout(ctx, frame, order, &L); if (st != CRT_OK) return st;
     NEED_ALIGNED("generate_secondary", n_active_out, 4);
@@ -321,6 +329,7 @@ crt_status crt_shade_accumulate(crt_ctx* ctx, const crt_bvh* bvh, const crt_scen
 {
     NEED_CTX("shade_accumulate"); NEED_BVH("shade_accumulate");
     if (!mats || !mats->materials || !frame) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "shade_accumulate: null argument");
+    if (mats->n_materials <= bvh->max_mat_id) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "shade_accumulate: %d materials but the BVH's triangles use id %d", mats->n_materials, bvh->max_mat_id);
     if (bounce < 0 || n_rays < 0 || frame->spp < 1) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "shade_accumulate: bad bounce / size");
     if (n_rays == 0) return CRT_OK;
     NEED_ALIGNED("shade_accumulate", rays, 32); NEED_ALIGNED("shade_accumulate", hits, 16); NEED_ALIGNED("shade_accumulate", ray_to_path, 4);
@@ -368,6 +377,7 @@ crt_status crt_render_frame(crt_ctx* ctx, const crt_bvh* bvh, const crt_scene_ma
 {
     NEED_CTX("render_frame"); NEED_BVH("render_frame");
     if (!mats || !mats->materials || !camera) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "render_frame: null argument");
+    if (mats->n_materials <= bvh->max_mat_id) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "render_frame: %d materials but the BVH's triangles use id %d", mats->n_materials, bvh->max_mat_id);
     if (n_bounces < 0 || n_bounces > 64) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "render_frame: n_bounces out of range");
     Layout L; crt_status st = crt_make_layout(ctx, frame, order, &L); if (st != CRT_OK) return st;
     if (L.n_slots == 0) return CRT_OK;
@@ -449,8 +459,10 @@ static crt_status render_frame_host_impl(crt_ctx* ctx, const crt_bvh* bvh, const
                                          uint32_t* n_secondary_host, void* workspace, size_t workspace_bytes, void* stream, bool resident, bool reset, bool sync, const char* name)
 {
     if (!ctx) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "%s: ctx is null", name);
+    CrtDeviceGuard dev_guard_(ctx->device);
     if (!bvh || !bvh->d_nodes || bvh->device != ctx->device) return crt_fail(ctx, bvh ? CRT_ERR_STATE : CRT_ERR_INVALID_ARG, "%s: BVH missing or not on this context's device", name);
     if (!materials_host || !env || !camera || !frame || !image_host || n_materials < 1) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "%s: null argument", name);
+    if (n_materials <= bvh->max_mat_id) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "%s: %d materials but the BVH's triangles use id %d", name, n_materials, bvh->max_mat_id);
     Layout L; crt_status st = crt_make_layout(ctx, frame, order, &L); if (st != CRT_OK) return st;
     if (!crt_aligned(workspace, 256)) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "%s: workspace is null or not 256-byte aligned", name);
     const size_t core = carve(L, nullptr).total, extra = crt_frame_host_extra_bytes(frame, n_materials);

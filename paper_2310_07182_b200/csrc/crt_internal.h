@@ -78,6 +78,7 @@ struct crt_bvh {
     WNode* d_wnodes = nullptr; int64_t n_wide_nodes = 0; int wide_depth = 0; int32_t wide_violations = 0;   // 8-wide layout (only when max_leaf == 1)
     int32_t* d_slot_of_prim = nullptr; // caller's triangle id -> index into d_tris
     int32_t* d_mat_id = nullptr;       // by caller's triangle id
+    int32_t max_mat_id = -1;           // largest material id of any triangle (ids are checked >= 0 at build time)
     int64_t device_bytes = 0;
 };
 
@@ -93,6 +94,17 @@ crt_status crt_fail(crt_ctx* ctx, crt_status st, const char* fmt, ...);
         cudaError_t e_ = cudaGetLastError();                                                        \
         if (e_ != cudaSuccess) return crt_fail(ctx, CRT_ERR_CUDA, "launch %s: %s", what, cudaGetErrorString(e_)); \
     } while (0)
+// makes the context's device current for the duration of an entry point (a C caller or another thread may have a different
+// current device; allocations, launches and event calls must land on the context's)
+struct CrtDeviceGuard {
+    int prev = -1; bool switched = false;
+    explicit CrtDeviceGuard(int device)
+    {
+        if (device >= 0 && cudaGetDevice(&prev) == cudaSuccess && prev != device) switched = cudaSetDevice(device) == cudaSuccess;
+    }
+    ~CrtDeviceGuard() { if (switched) cudaSetDevice(prev); }
+    CrtDeviceGuard(const CrtDeviceGuard&) = delete; CrtDeviceGuard& operator=(const CrtDeviceGuard&) = delete;
+};
 static inline bool crt_aligned(const void* p, size_t a) { return p != nullptr && (reinterpret_cast<uintptr_t>(p) % a) == 0; }
 
 // layout of the slot space ---------------------------------------------------------------------------
@@ -106,7 +118,7 @@ struct Layout {
 crt_status crt_make_layout(crt_ctx* ctx, const crt_frame* f, const crt_order* o, Layout* L);
 
 // kernels' host launchers (defined in the .cu files) ------------------------------------------------------
-crt_status launch_trace(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, crt_hit* hits, cudaStream_t st);
+crt_status launch_trace(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, crt_hit* hits, cudaStream_t st, bool far_origins = false);
 crt_status launch_trace_wide(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, crt_hit* hits, cudaStream_t st);
 crt_status launch_trace_wide_stats(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, int64_t* counters, cudaStream_t st);
 crt_status launch_trace_stats(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, int64_t* counters, cudaStream_t st);

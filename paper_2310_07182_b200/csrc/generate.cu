@@ -142,6 +142,7 @@ struct GenArgs {
     int32_t fresh;            // first bounce of a fused frame: the path state is not read (throughput 1, radiance 0, alive) and is written in full
     int32_t by_slot;          // path state indexed by slot instead of by path id (crt_render_frame, grouped orders)
     int64_t n_slots; int32_t bounce; int32_t morton;   // morton: 0 = no key, else 1 + sort code
+    int32_t n_tris;          // hit records naming a primitive >= n_tris (a stale buffer from another BVH) are treated as dead, not dereferenced
     int32_t world;           // direct_reuse in WORLD space (mode 3; D:R18)
     int32_t fuse_shade;      // crt_render_frame: shade the previous segment here (same arithmetic as shade_kernel) instead of in its own pass
     float env[6];
@@ -189,7 +190,7 @@ __global__ void __launch_bounds__(1024) generate_kernel(GenArgs A, DevLayout L)
 #pragma unroll
                 for (int k = 0; k < 3; ++k) Le[k] = add(A.env[k], mul(sub(A.env[3 + k], A.env[k]), w));
                 ends = true;
-            } else {
+            } else if (prim < A.n_tris) {
                 const float4 m1 = __ldg(reinterpret_cast<const float4*>(A.mats + __ldg(A.mat_id + prim)) + 1);
                 if (__float_as_int(m1.w) == CRT_MAT_EMISSIVE) { Le[0] = m1.x; Le[1] = m1.y; Le[2] = m1.z; ends = true; }
             }
@@ -201,7 +202,7 @@ __global__ void __launch_bounds__(1024) generate_kernel(GenArgs A, DevLayout L)
                 pw[0] = make_float4(ps.tr, ps.tg, ps.tb, __uint_as_float(ps.flags)); pw[1] = p1;
             }
         }
-        if ((ps.flags & 1u) && rd.w >= 0.f && prim >= 0) {
+        if ((ps.flags & 1u) && rd.w >= 0.f && (unsigned)prim < (unsigned)A.n_tris) {
             const float4* tp = reinterpret_cast<const float4*>(A.tris + __ldg(A.slot_of_prim + prim));
             const float4 a = __ldg(tp), b = __ldg(tp + 1), c = __ldg(tp + 2);
             const V3 v0 = mk(a.x, a.y, a.z), e1 = mk(b.x, b.y, b.z), e2 = mk(c.x, c.y, c.z), d = mk(rd.x, rd.y, rd.z);
@@ -406,7 +407,7 @@ crt_status launch_generate(crt_ctx* ctx, const crt_bvh* bvh, const crt_scene_mat
     A.tris = bvh->d_tris; A.slot_of_prim = bvh->d_slot_of_prim; A.mat_id = bvh->d_mat_id; A.mats = mats.materials;
     A.prev_rays = prev_rays; A.prev_hits = prev_hits; A.prev_r2p = prev_r2p; A.paths = paths;
     A.rays_out = rays_out; A.r2p_out = r2p_out; A.gid_out = gid_out; A.src_out = src_out; A.cls_out = cls_out; A.n_active = n_active;
-    A.keys_out = nullptr; A.bounds = make_bounds(bvh->bounds); A.n_slots = L.n_slots; A.bounce = bounce; A.morton = 0;
+    A.keys_out = nullptr; A.bounds = make_bounds(bvh->bounds); A.n_slots = L.n_slots; A.bounce = bounce; A.morton = 0; A.n_tris = (int32_t)bvh->n_tris;
     A.world = (L.mode == CRT_MODE_WORLD_REUSE);
     A.fuse_shade = fuse_shade ? 1 : 0;
     A.fresh = (fresh_paths && fuse_shade) ? 1 : 0;

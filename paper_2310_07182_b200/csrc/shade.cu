@@ -10,7 +10,7 @@ namespace {
 
 struct Env6 { float a[3], b[3]; };
 
-__global__ void __launch_bounds__(256) shade_kernel(const int32_t* __restrict__ mat_id, const crt_material* __restrict__ mats, Env6 env, int32_t wh,
+__global__ void __launch_bounds__(256) shade_kernel(const int32_t* __restrict__ mat_id, int32_t n_tris, const crt_material* __restrict__ mats, Env6 env, int32_t wh,
                                                     float inv_spp, int is_last, const crt_ray* __restrict__ rays, const crt_hit* __restrict__ hits,
                                                     const int32_t* __restrict__ r2p, int64_t n, crt_path_state* __restrict__ paths,
                                                     float* __restrict__ accum, int atomic_accum, int by_slot)
@@ -33,7 +33,7 @@ __global__ void __launch_bounds__(256) shade_kernel(const int32_t* __restrict__ 
 #pragma unroll
             for (int k = 0; k < 3; ++k) Le[k] = add(env.a[k], mul(sub(env.b[k], env.a[k]), w));
             ends = true;
-        } else {
+        } else if (prim < n_tris) {        // (a primitive id beyond this BVH -- a stale hit buffer -- is ignored rather than dereferenced)
             const float4* mp = reinterpret_cast<const float4*>(mats + __ldg(mat_id + prim));
             const float4 m1 = __ldg(mp + 1);
             if (__float_as_int(m1.w) == CRT_MAT_EMISSIVE) { Le[0] = m1.x; Le[1] = m1.y; Le[2] = m1.z; ends = true; }
@@ -91,7 +91,7 @@ crt_status launch_shade(crt_ctx* ctx, const crt_bvh* bvh, const crt_scene_mats& 
     if (n == 0) return CRT_OK;
     Env6 e;
     for (int k = 0; k < 3; ++k) { e.a[k] = mats.env[k]; e.b[k] = mats.env[3 + k]; }
-    shade_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(bvh->d_mat_id, mats.materials, e, f.w * f.h, 1.0f / (float)f.spp, is_last, rays, hits, r2p, n,
+    shade_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(bvh->d_mat_id, (int32_t)bvh->n_tris, mats.materials, e, f.w * f.h, 1.0f / (float)f.spp, is_last, rays, hits, r2p, n,
                                                               paths, accum, f.spp > 1, paths_by_slot ? 1 : 0);
     CRT_CHECK_LAUNCH(ctx, "shade");
     return CRT_OK;

@@ -371,18 +371,22 @@ crt::DevLayout make_dev_layout(const Layout& L, const crt_frame& f)
     return D;
 }
 
-crt_status launch_trace(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, crt_hit* hits, cudaStream_t st)
+// far_origins: the caller knows the ray origins may lie beyond the default box test's contract (16 scene extents from the scene;
+// crt_trace_primary checks the camera eye): the any-origin box test (trace_kernel 4's) is used instead
+crt_status launch_trace(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, crt_hit* hits, cudaStream_t st, bool far_origins)
 {
     if (n == 0) return CRT_OK;
-    if (ctx->trace_kernel == 2 && bvh->d_wnodes) return launch_trace_wide(ctx, bvh, rays, n, hits, st);
+    if (ctx->trace_kernel == 2 && bvh->d_wnodes && bvh->wide_violations == 0) return launch_trace_wide(ctx, bvh, rays, n, hits, st);
     if (ctx->trace_kernel == 0) {
         trace_flat_kernel<<<(unsigned)((n + TRACE_BLOCK - 1) / TRACE_BLOCK), TRACE_BLOCK, 0, st>>>(bvh->d_nodes, bvh->d_tris, rays, hits, n);
         CRT_CHECK_LAUNCH(ctx, "trace_flat");
         return CRT_OK;
     }
-    // 16-bit nodes unless the grid is too coarse for this scene's detail (decoded boxes more than twice the fp32 boxes' area)
-    if (ctx->trace_kernel == 4 && bvh->q_inflation <= 2.0) return launch_dyn<false, 2>(ctx, bvh, rays, n, hits, nullptr, st);
-    if (ctx->trace_kernel == 3 && bvh->q_inflation <= 2.0) return launch_dyn<false, 1>(ctx, bvh, rays, n, hits, nullptr, st);
+    // 16-bit nodes unless the grid is too coarse for this scene's detail (decoded boxes more than twice the fp32 boxes' area) or
+    // the layout failed its own check (a plane clamped or less than one step outside its box: crt_bvh_check bit 16)
+    const bool q_ok = bvh->q_inflation <= 2.0 && bvh->q_violations == 0;
+    if ((ctx->trace_kernel == 4 || (ctx->trace_kernel == 3 && far_origins)) && q_ok) return launch_dyn<false, 2>(ctx, bvh, rays, n, hits, nullptr, st);
+    if (ctx->trace_kernel == 3 && q_ok) return launch_dyn<false, 1>(ctx, bvh, rays, n, hits, nullptr, st);
     return launch_dyn<false, 0>(ctx, bvh, rays, n, hits, nullptr, st);
 }
 
@@ -390,9 +394,10 @@ crt_status launch_trace(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, i
 crt_status launch_trace_stats(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, int64_t* counters, cudaStream_t st)
 {
     if (n == 0) return CRT_OK;
-    if (ctx->trace_kernel == 2 && bvh->d_wnodes) return launch_trace_wide_stats(ctx, bvh, rays, n, counters, st);
-    if (ctx->trace_kernel == 4 && bvh->q_inflation <= 2.0) return launch_dyn<true, 2>(ctx, bvh, rays, n, nullptr, reinterpret_cast<unsigned long long*>(counters), st);
-    if (ctx->trace_kernel == 3 && bvh->q_inflation <= 2.0) return launch_dyn<true, 1>(ctx, bvh, rays, n, nullptr, reinterpret_cast<unsigned long long*>(counters), st);
+    if (ctx->trace_kernel == 2 && bvh->d_wnodes && bvh->wide_violations == 0) return launch_trace_wide_stats(ctx, bvh, rays, n, counters, st);
+    const bool q_ok = bvh->q_inflation <= 2.0 && bvh->q_violations == 0;
+    if (ctx->trace_kernel == 4 && q_ok) return launch_dyn<true, 2>(ctx, bvh, rays, n, nullptr, reinterpret_cast<unsigned long long*>(counters), st);
+    if (ctx->trace_kernel == 3 && q_ok) return launch_dyn<true, 1>(ctx, bvh, rays, n, nullptr, reinterpret_cast<unsigned long long*>(counters), st);
     return launch_dyn<true, 0>(ctx, bvh, rays, n, nullptr, reinterpret_cast<unsigned long long*>(counters), st);
 }
 
@@ -404,5 +409,14 @@ crt_status launch_primary(crt_ctx* ctx, const crt_bvh* bvh, const crt_camera& ca
     for (int k = 0; k < 3; ++k) { c.eye[k] = cam.eye[k]; c.U[k] = cam.U[k]; c.V[k] = cam.V[k]; c.W[k] = cam.W[k]; }
     primary_rays_kernel<<<(unsigned)((L.n_slots + 255) / 256), 256, 0, st>>>(c, make_dev_layout(L, f), L.n_slots, rays, r2p);
     CRT_CHECK_LAUNCH(ctx, "primary_rays");
-    return launch_trace(ctx, bvh, rays, L.n_slots, hits, st);
+    // the default box test is conservative for origins within 16 scene extents of the scene box (include/crt.h); a camera farther
+    // away takes the any-origin test
+    bool far_eye = false;
+    for (int k = 0; k < 3; ++k) {
+        const float ext = bvh->bounds[3 + k] - bvh->bounds[k];
+        float maxext = ext; for (int j = 0; j < 3; ++j) maxext = fmaxf(maxext, bvh->bounds[3 + j] - bvh->bounds[j]);
+        const float reach = 15.0f * fmaxf(ext, maxext * (1.0f / 4096.0f));
+        if (cam.eye[k] < bvh->bounds[k] - reach || cam.eye[k] > bvh->bounds[3 + k] + reach) far_eye = true;
+    }
+    return launch_trace(ctx, bvh, rays, L.n_slots, hits, st, far_eye);
 }

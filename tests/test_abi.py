@@ -108,7 +108,24 @@ def test_host_bvh_builder_invariants(lib):
         bad = C.c_int32(-1)
         assert lib.crt_bvh_check(h, C.byref(bad)) == 0 and bad.value == 0
         lib.crt_bvh_destroy(h)
-    # rejected: NaN vertex, bad max_leaf
+    # a unit-extent scene far from the origin (gmin is a float; its rounding must not eat the grid's margin): the 16-bit
+    # layout still passes its own check, or -- when fp32 itself has too few bits left at that offset -- the check says so and the
+    # kernel falls back to the fp32 nodes (launch_trace reads q_violations)
+    rng = np.random.default_rng(3)
+    tri = (rng.random((2000, 1, 3)) + 0.02 * rng.standard_normal((2000, 3, 3))).astype(np.float64)
+    for offset in (0.0, 5e3, 1e4, 1e5, 3e6):
+        v = np.ascontiguousarray(tri + offset, np.float32)
+        h = C.c_void_p()
+        assert lib.crt_build_bvh(None, C.c_void_p(v.ctypes.data), None, C.c_int64(len(v)), None, C.byref(h)) == 0
+        bad = C.c_int32(-1)
+        assert lib.crt_bvh_check(h, C.byref(bad)) == 0 and (bad.value & 0xffff) == 0
+        if offset <= 1e5:
+            assert bad.value == 0, (offset, hex(bad.value))
+        lib.crt_bvh_destroy(h)
+    # rejected: NaN vertex, bad max_leaf, negative material id
+    v = I.cornell().verts; m = np.zeros(len(v), np.int32); m[5] = -1
+    h = C.c_void_p()
+    assert lib.crt_build_bvh(None, C.c_void_p(v.ctypes.data), C.c_void_p(m.ctypes.data), C.c_int64(len(v)), None, C.byref(h)) == 1
     v = I.cornell().verts.copy(); v[3, 1, 2] = np.nan
     h = C.c_void_p()
     assert lib.crt_build_bvh(None, C.c_void_p(v.ctypes.data), None, C.c_int64(len(v)), None, C.byref(h)) == 1

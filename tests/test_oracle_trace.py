@@ -133,3 +133,28 @@ def test_empty_inputs(oracle):
     r = _rays(I.random_rays(1, 5, [0, 0, 0], [1, 1, 1]), oracle)
     assert np.all(b.trace(r)["prim"] == -1)
     assert len(oracle.Bvh(I.cornell().verts).trace(r[:0])) == 0
+
+
+@pytest.mark.parametrize("mode,gw,gh,s", [(0, 1, 1, 1), (2, 4, 4, 2)])
+def test_closed_box_without_light_is_watertight_and_black(oracle, mode, gw, gh, s):
+    """Closed Lambert cube seen from inside, no light, no environment: every primary ray and every secondary ray of three
+    bounces hits a wall (the offset origins of D:R7 never leak through a face or an edge), and the image stays 0."""
+    sc = I.emissive_box(albedo=0.8)
+    fr = oracle.frame(sc.width, sc.height, 2, 0, 0)
+    b = oracle.Bvh(sc.verts)
+    rays, hits, r2p = oracle.trace_primary(b, sc.camera, fr, mode, gw, gh, s)
+    paths = oracle.paths_init(2 * sc.width * sc.height)
+    accum = np.zeros((sc.height, sc.width, 3), np.float32)
+    oracle.shade_accumulate(sc, fr, 0, False, rays, hits, r2p, paths, accum)
+    for bounce in (1, 2, 3):
+        act = rays["tmax"] >= 0
+        assert act.sum() == 2 * sc.width * sc.height and np.all(hits["prim"][act] >= 0)
+        g = oracle.generate_secondary(sc, fr, bounce, mode, gw, gh, s, b.info()["bounds"], rays, hits, r2p, paths)
+        rays, r2p = g["rays"], g["ray_to_path"]
+        assert g["n_active"] == 2 * sc.width * sc.height
+        o = rays["o"][rays["tmax"] >= 0]
+        assert np.all(o > 0) and np.all(o < 1)                              # strictly inside the cube
+        hits = b.trace(rays)
+        oracle.shade_accumulate(sc, fr, bounce, bounce == 3, rays, hits, r2p, paths, accum)
+    assert np.all(hits["prim"][rays["tmax"] >= 0] >= 0)
+    assert np.all(accum == 0) and np.all(paths["T"] > 0) and np.all(paths["T"] <= np.float32(0.8) ** 3 * 1.0001)

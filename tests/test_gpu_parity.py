@@ -43,7 +43,8 @@ SCENES = {
 def test_full_size_config2_stagewise_and_sampled(crt, ctx, oracle):
     """BASELINE config 2 at full size (1,024,704 triangles, 1920x1080, direct_reuse 4x4 stride 4): the partition covers every
     pixel exactly once; generation fed the GPU's own primary hits equals the oracle's generation on the same buffers
-    (integer maps bit-exact, rays bit-identical); sampled primary and secondary hits equal the all-triangles definition."""
+    (integer maps bit-exact, rays bit-identical), for both bounces; ALL hits of the primary segment and of both bounces equal the
+    oracle's (ids >= 99.99 %, t-tie rule), and a sample of them the all-triangles definition."""
     scene = I.interior(seed=1).with_camera(1920, 1080)
     G = GpuScene(crt, scene, ctx)
     w, h, spp, gw, gh, s = 1920, 1080, 1, 4, 4, 4
@@ -70,14 +71,36 @@ def test_full_size_config2_stagewise_and_sampled(crt, ctx, oracle):
     rg = rays_np(oracle, out["rays"])
     assert rg.tobytes() == g["rays"].tobytes()
     hits1 = ctx.crt_trace(G.bvh, out["rays"])
+    # second bounce, stage-wise again: shade(1), generate(2) on the GPU's own buffers against the oracle's on the same buffers
+    ctx.crt_shade_accumulate(G.bvh, G.mats, fr, 1, False, out["rays"], hits1, out["ray_to_path"], paths, accum)
+    paths_before2 = paths_np(oracle, paths).copy()
+    out2 = ctx.crt_generate_secondary(G.bvh, G.mats, fr, 2, order, out["rays"], hits1, out["ray_to_path"], paths)
+    g2 = oracle.generate_secondary(scene, ofr, 2, 2, gw, gh, s, bounds, rg, hits_np(oracle, hits1), g["ray_to_path"], paths_before2)
+    for k in ("ray_to_path", "group_id", "dir_src", "group_class"):
+        assert np.array_equal(out2[k].cpu().numpy(), g2[k]), k
+    assert rays_np(oracle, out2["rays"]).tobytes() == g2["rays"].tobytes()
+    pg = paths_np(oracle, paths)                                              # (the oracle updated paths_before2 in place)
+    assert np.array_equal(pg["flags"] & 1, paths_before2["flags"] & 1) and np.array_equal(pg["T"], paths_before2["T"])
+    hits2 = ctx.crt_trace(G.bvh, out2["rays"])
+    # EVERY hit of the primary segment and of both bounces (3 x 2.07 M rays) against the oracle's BVH, which is itself checked
+    # against the all-triangles definition on a sample of the same rays
+    ob = oracle.Bvh(scene.verts)
+    assert ob.check() == 0
     rng = np.random.default_rng(11)
-    for rays_dev, hits_dev, n_s in ((rays0, hits0, 120), (out["rays"], hits1, 360)):
+    n_rays_compared = 0
+    for rays_dev, hits_dev, n_s in ((rays0, hits0, 120), (out["rays"], hits1, 360), (out2["rays"], hits2, 240)):
         r = rays_np(oracle, rays_dev); hh = hits_np(oracle, hits_dev)
+        ho = ob.trace(r)
+        frac = compare_hits(hh, ho)
+        assert frac >= 0.9999
         act = np.flatnonzero(r["tmax"] >= 0)
+        n_rays_compared += len(act)
         pick = rng.choice(act, n_s, replace=False)
-        compare_hits(hh[pick], oracle.trace_brute(scene.verts, r[pick]))
-    inact = rays_np(oracle, out["rays"])["tmax"] < 0
-    assert np.all(hits_np(oracle, hits1)["prim"][inact] == -1)
+        brute = oracle.trace_brute(scene.verts, r[pick])
+        assert np.array_equal(ho[pick], brute)                               # the oracle's BVH == the plain definition, bit for bit
+        compare_hits(hh[pick], brute)
+        assert np.all(hh["prim"][r["tmax"] < 0] == -1)
+    assert n_rays_compared > 5000000
 
 
 # ------------------------------------------------------------------ a0 / a5: BVH + traversal
@@ -546,8 +569,8 @@ def test_fused_shading_option_gives_the_identical_image(crt, ctx):
 
 
 def test_full_size_config4_sampled(crt, ctx, oracle):
-    """BASELINE config 4 at full size (10,300,418 triangles, coordinates up to 2048): sampled primary and secondary hits of the
-    direct_reuse frame equal the all-triangles definition; the partition is the oracle's."""
+    """BASELINE config 4 at full size (10,300,418 triangles, coordinates up to 2048): ALL hits of the primary segment and of both
+    bounces of the direct_reuse frame equal the oracle's, a sample of them the all-triangles definition; the partition is the oracle's."""
     scene = I.landscape(seed=2).with_camera(1920, 1080)
     assert scene.n_tris == 10300418
     G = GpuScene(crt, scene, ctx)
@@ -564,12 +587,69 @@ def test_full_size_config4_sampled(crt, ctx, oracle):
     ctx.crt_shade_accumulate(G.bvh, G.mats, fr, 0, False, rays0, hits0, r2p0, paths, accum)
     out = ctx.crt_generate_secondary(G.bvh, G.mats, fr, 1, order, rays0, hits0, r2p0, paths)
     hits1 = ctx.crt_trace(G.bvh, out["rays"])
+    ctx.crt_shade_accumulate(G.bvh, G.mats, fr, 1, False, out["rays"], hits1, out["ray_to_path"], paths, accum)
+    out2 = ctx.crt_generate_secondary(G.bvh, G.mats, fr, 2, order, out["rays"], hits1, out["ray_to_path"], paths)
+    hits2 = ctx.crt_trace(G.bvh, out2["rays"])
+    # EVERY hit of the three segments against the oracle's BVH (10.3 M triangles; the 16-bit grid is coarsest here: 3 cm steps);
+    # the oracle's BVH against the all-triangles definition on a sample
+    ob = oracle.Bvh(scene.verts)
     rng = np.random.default_rng(12)
-    for rays_dev, hits_dev, n_s in ((rays0, hits0, 40), (out["rays"], hits1, 80)):
+    for rays_dev, hits_dev, n_s in ((rays0, hits0, 40), (out["rays"], hits1, 80), (out2["rays"], hits2, 40)):
         r = rays_np(oracle, rays_dev); hh = hits_np(oracle, hits_dev)
+        ho = ob.trace(r)
+        assert compare_hits(hh, ho) >= 0.9999
         act = np.flatnonzero(r["tmax"] >= 0)
         pick = rng.choice(act, n_s, replace=False)
         ref = oracle.trace_brute(scene.verts, r[pick])
+        assert np.array_equal(ho[pick], ref)
         compare_hits(hh[pick], ref)
         if n_s == 80:
             assert (ref["prim"] >= 0).any() and (ref["prim"] < 0).any()               # the secondary sample has terrain hits and sky misses
+
+
+def test_full_size_config3_point_stagewise(crt, ctx, oracle):
+    """BASELINE config 3 at its stated size, one sweep point: 3840x2160, 4 spp (33,177,600 paths), direct_reuse 8x8 stride 8
+    (tile 64x64 = 4096 slots, the largest tile; 2160 is not a multiple of 64: partial tiles).  Partition == the oracle's and an
+    exact cover; generation of bounce 1 fed the GPU's own primary hits == the oracle's on the same buffers (integer maps bit-exact,
+    rays byte-identical); sampled primary and secondary hits == the oracle's BVH (== all-triangles definition on a subsample)."""
+    import torch
+    scene = I.interior(seed=1).with_camera(3840, 2160)
+    G = GpuScene(crt, scene, ctx)
+    w, h, spp, gw, gh, s = 3840, 2160, 4, 8, 8, 8
+    fr = crt.make_frame(w, h, spp, 1, 0); ofr = oracle.frame(w, h, spp, 1, 0)
+    order = crt.make_order("direct_reuse", gw, gh, s)
+    n_paths, n_slots, n_groups = crt.crt_layout(fr, order)
+    assert n_paths == 33177600 and n_slots == 4 * 60 * 34 * 4096 and n_groups * 64 == n_slots
+    rays0, hits0, r2p0 = ctx.crt_trace_primary(G.bvh, G.camera, fr, order)
+    r2p = r2p0.cpu().numpy()
+    assert np.array_equal(r2p, oracle.partition(ofr, 2, gw, gh, s))
+    live = r2p[r2p >= 0]
+    assert len(live) == n_paths and np.array_equal(np.bincount(live, minlength=n_paths), np.ones(n_paths, np.int64))    # exact cover
+    del live
+    paths = ctx.empty((n_paths, 8)); ctx.crt_paths_init(paths)
+    accum = torch.zeros((h, w, 3), device=ctx.device)
+    ctx.crt_shade_accumulate(G.bvh, G.mats, fr, 0, False, rays0, hits0, r2p0, paths, accum)
+    paths_before = paths_np(oracle, paths).copy()
+    out = ctx.crt_generate_secondary(G.bvh, G.mats, fr, 1, order, rays0, hits0, r2p0, paths)
+    bounds = np.asarray(G.bvh.info()["bounds"], np.float32)
+    r0 = rays_np(oracle, rays0); h0 = hits_np(oracle, hits0)
+    g = oracle.generate_secondary(scene, ofr, 1, 2, gw, gh, s, bounds, r0, h0, r2p, paths_before)
+    for k in ("ray_to_path", "group_id", "dir_src", "group_class"):
+        assert np.array_equal(out[k].cpu().numpy(), g[k]), k
+    assert int(out["n_active"].cpu().numpy().view(np.uint32)[0]) == g["n_active"] > 20000000
+    r1 = rays_np(oracle, out["rays"])
+    assert r1.tobytes() == g["rays"].tobytes()
+    pg = paths_np(oracle, paths)
+    assert np.array_equal(pg["flags"] & 1, paths_before["flags"] & 1) and np.array_equal(pg["T"], paths_before["T"])
+    del g, pg
+    hits1 = ctx.crt_trace(G.bvh, out["rays"])
+    h1 = hits_np(oracle, hits1)
+    ob = oracle.Bvh(scene.verts)
+    rng = np.random.default_rng(13)
+    for r, hh in ((r0, h0), (r1, h1)):
+        act = np.flatnonzero(r["tmax"] >= 0)
+        pick = rng.choice(act, 200000, replace=False)
+        ho = ob.trace(r[pick])
+        compare_hits(hh[pick], ho)
+        assert np.array_equal(ho[:100], oracle.trace_brute(scene.verts, r[pick[:100]]))
+        assert np.all(hh["prim"][r["tmax"] < 0] == -1)

@@ -470,6 +470,78 @@ def run_sweep(args):
                                                   "reference_frames": 4 * F, "scale": sc}}))
 
 
+def _frame_ray_sets(ctx, crt, scene, w, h, spp, nb, gw, gh, s, seed, frame, modes=("direct_reuse", "independent")):
+    """The ray sets of one frame (primary, bounce 1 .. nb) in each order of `modes`: [(tag, rays)]."""
+    import torch
+    bvh = ctx.crt_build_bvh(scene.verts, scene.mat_id)
+    mats_dev = ctx.upload(scene.materials); mats = ctx.scene_mats(mats_dev, len(scene.materials), scene.env); cam = crt.make_camera(scene.camera)
+    sets = []
+    for mode in modes:
+        order = crt.make_order(mode, gw, gh, s) if mode == "direct_reuse" else crt.make_order(mode)
+        fr = crt.make_frame(w, h, spp, seed, frame)
+        rays, hits, r2p = ctx.crt_trace_primary(bvh, cam, fr, order)
+        paths = ctx.empty((crt.crt_layout(fr, order)[0], 8)); ctx.crt_paths_init(paths)
+        acc = torch.zeros((h, w, 3), device=ctx.device)
+        ctx.crt_shade_accumulate(bvh, mats, fr, 0, False, rays, hits, r2p, paths, acc)
+        sets.append((f"{mode} primary", rays.clone()))
+        for b in range(1, nb + 1):
+            out = ctx.crt_generate_secondary(bvh, mats, fr, b, order, rays, hits, r2p, paths)
+            rays, r2p = out["rays"], out["ray_to_path"]
+            sets.append((f"{mode} bounce {b}", rays.clone()))
+            hits = ctx.crt_trace(bvh, rays)
+            ctx.crt_shade_accumulate(bvh, mats, fr, b, b == nb, rays, hits, r2p, paths, acc)
+    return bvh, (mats_dev, mats), sets
+
+
+KERNEL_OPTION_DEFAULTS = {"trace_kernel": 3, "trace_refill_threshold": 16, "trace_leaf_wait": 6, "trace_blocks_per_sm": 0, "trace_exact": 1}
+
+
+def run_kernels(args):
+    """A/B of traversal kernel variants (profiles/r02a): crt_trace alone on the ray sets of one frame (frame 7; primary, bounce 1, bounce 2;
+    direct_reuse and independent order), L2 flushed between repetitions, median of 8; hit records compared with the default kernel's.
+    --variants: comma-free list like "3 5 6 3:trace_exact=0 3:trace_blocks_per_sm=6" (trace_kernel id, then option=value pairs)."""
+    import torch
+    import paper_2310_07182_b200 as crt
+    import crt_inputs as I
+    name, kw, w, h, spp, nb, gw, gh, s, seed, cfg = WORKLOADS[args.workload]
+    scene = I.by_name(name, **kw).with_camera(w, h)
+    ctx = crt.Context(0)
+    bvh, _keep, sets = _frame_ray_sets(ctx, crt, scene, w, h, spp, nb, gw, gh, s, seed, 7)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=ctx.device)
+    ref = {tag: ctx.crt_trace(bvh, r).clone() for tag, r in sets}
+    torch.cuda.synchronize()
+    rows = []
+    for v in args.variants:
+        k, _, opts = v.partition(":")
+        ctx.crt_set_option("trace_kernel", int(k))
+        touched = []
+        for o in filter(None, opts.split(",")):
+            key, val = o.split("="); ctx.crt_set_option(key, int(val)); touched.append(key)
+        row = {"variant": v, "sets": {}}
+        for tag, r in sets:
+            hh = ctx.crt_trace(bvh, r); torch.cuda.synchronize()
+            hi, ri = hh.view(torch.int32), ref[tag].view(torch.int32)
+            ids_equal = float((hi[:, 3] == ri[:, 3]).float().mean().item())
+            ts = []
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            for _ in range(8):
+                flush.fill_(1)
+                e0.record(); ctx.crt_trace(bvh, r, hits=hh); e1.record(); torch.cuda.synchronize()
+                ts.append(e0.elapsed_time(e1))
+            nv, nt, nr = ctx.crt_trace_stats(bvh, r)
+            row["sets"][tag] = {"ms": float(np.median(ts)), "records_identical": bool(torch.equal(hi, ri)), "ids_equal_frac": ids_equal,
+                                "node_visits_per_ray": nv / max(1, nr), "tri_tests_per_ray": nt / max(1, nr)}
+        rows.append(row)
+        for key in ["trace_kernel"] + touched:
+            ctx.crt_set_option(key, KERNEL_OPTION_DEFAULTS[key])
+    print(json.dumps({"kernels": rows, "config": {"workload": args.workload, "order": f"direct_reuse {gw}x{gh} stride {s} / independent", "frame": 7,
+                                                  "timing": "crt_trace alone, CUDA events, median of 8, 256 MB L2 flush between repetitions"}}))
+    tags = [t for t, _ in sets]
+    sys.stderr.write("| variant | " + " | ".join(tags) + " |\n|---|" + "---:|" * len(tags) + "\n")
+    for row in rows:
+        sys.stderr.write(f"| {row['variant']} | " + " | ".join(f"{row['sets'][t]['ms']:.3f}{'' if row['sets'][t]['records_identical'] else ' (ids ' + format(row['sets'][t]['ids_equal_frac'], '.6f') + ')'}" for t in tags) + " |\n")
+
+
 def run_tail(args):
     """Fixed cost of a crt_trace launch (profiles/r01h): crt_trace on one frame's ray sets (primary, bounce 1, bounce 2; direct_reuse order)
     and on the same set concatenated twice and four times; L2 flushed between repetitions, median of 8.  One JSON line."""
@@ -520,8 +592,9 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--frames-in-flight", type=int, default=3, help="frames rendered concurrently (one context + stream each) for the headline value; the per-mode table stays single-stream")
     ap.add_argument("--no-sort-codes", action="store_true", help="skip the Origin / Reis / Costa / TwoPoint reordering baselines")
-    ap.add_argument("--sweep", nargs="?", const="config3", default=None, choices=["config3", "table3", "rules", "tail"],
-                    help="config3: BASELINE config 3 sweep; table3: the paper's Table 3 shapes (tile x K) at 1920x1080, 1 spp, 2 bounces; rules: shuffled against lattice partition at the same size; tail: fixed cost of a crt_trace launch (n, 2n, 4n rays) on --workload")
+    ap.add_argument("--sweep", nargs="?", const="config3", default=None, choices=["config3", "table3", "rules", "tail", "kernels"],
+                    help="config3: BASELINE config 3 sweep; table3: the paper's Table 3 shapes (tile x K) at 1920x1080, 1 spp, 2 bounces; rules: shuffled against lattice partition at the same size; tail: fixed cost of a crt_trace launch (n, 2n, 4n rays) on --workload; kernels: A/B of traversal kernel variants (--variants) on one frame's ray sets of --workload")
+    ap.add_argument("--variants", nargs="*", default=["3", "3:trace_exact=0", "5", "6", "4", "1"], help="--sweep kernels: trace_kernel id[:option=value,...] ...")
     ap.add_argument("--sweep-frames", type=int, default=64)
     ap.add_argument("--sweep-scale", type=int, default=1, help="divide the 3840x2160 image by this (quick runs)")
     args = ap.parse_args()
@@ -529,6 +602,9 @@ def main():
         args.warmup = 3
     if args.sweep == "tail":
         run_tail(args)
+        return
+    if args.sweep == "kernels":
+        run_kernels(args)
         return
     if args.sweep:
         run_sweep(args)

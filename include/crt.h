@@ -106,8 +106,14 @@ crt_status crt_destroy(crt_ctx* ctx);
 const char* crt_last_error(const crt_ctx* ctx);
 /* Tunables (for experiments; defaults are what bench.py times): "trace_kernel" (0 = binary BVH, one thread per ray;
  * 1 = binary BVH with fp32 64-byte nodes, persistent warps with per-lane dynamic fetch; 2 = 8-wide compressed BVH, persistent warps;
- * 3 = the persistent kernel of 1 on 16-bit 32-byte nodes -- the default; 4 = as 3 with a box test that is conservative for ANY ray
- * origin (3 is for origins within 16 scene extents of the scene, 1 within about 128), 3-4 % slower), "trace_leaf_wait" (0..31: a warp leaves its inner-node
+ * 3 = the persistent kernel of 1 on 16-bit 32-byte nodes, plane distances by packed FFMA2 -- the default; 4 = as 3 with a box test that
+ * is conservative for ANY ray origin (3 is for origins within 16 scene extents of the scene, 1 within about 128), 3-4 % slower;
+ * 5 = warp-cooperative triangle phase: the triangles of a warp's parked leaves become one work list in shared memory, tested one
+ * item per lane (same hit records; measured 15-25 % slower, profiles/r02a); 6 = as 3 with the top 512 nodes of the tree staged in shared
+ * memory per block (same hit records; measured 8-16 % slower, profiles/r02a)), "trace_exact" (1 = default: the bit-exact triangle
+ * test of D:R0; 0 = fused multiply-adds and an approximate reciprocal in the triangle test: 3-5 % faster, ids equal on >= 99.999 % of
+ * rays but t of grazing hits off by up to 4e-4 relative, i.e. outside north_star's 1e-4: an option, not the default),
+ * "trace_leaf_wait" (0..31: a warp leaves its inner-node
  * phase when at most this many descending lanes hold no leaf), "trace_refill_threshold" (0..32: idle lanes fetch new rays when
  * fewer lanes than this are busy), "trace_blocks_per_sm" (0 = from the occupancy calculator), "trace_tri_wait" (8-wide kernel: lanes holding triangle hits
  * before a warp enters its triangle phase), "fuse_shade" (crt_render_frame shades non-final segments inside the next generation

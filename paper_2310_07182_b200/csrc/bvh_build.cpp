@@ -285,8 +285,20 @@ void crt_bvh_flatten(const crt_bvh* b, const std::vector<int32_t>& tri_order, st
     if (b->nodes[0].left < 0) {      // the whole scene is one leaf: a root whose second child is empty
         GpuNode g; g.c[0] = child_of(b->nodes[0], leaf_ref(b->nodes[0])); g.c[1] = empty_child(); gn.push_back(g); return;
     }
-    // depth-first numbering of inner nodes, left child next to its parent
-    std::vector<int32_t> gpu_index(b->nodes.size(), -1), stack{0}, order;
+    // numbering of inner nodes: the top of the tree breadth-first (the first 512 indices are the top levels, which every ray visits: they
+    // share cache lines, and an experiment stages them in shared memory), then depth-first, left child next to its parent
+    std::vector<int32_t> gpu_index(b->nodes.size(), -1), stack, order;
+    {
+        std::deque<int32_t> frontier{0};
+        while (!frontier.empty() && order.size() + frontier.size() < 512) {
+            int32_t i = frontier.front(); frontier.pop_front();
+            gpu_index[i] = (int32_t)order.size(); order.push_back(i);
+            const BuildNode& nd = b->nodes[i];
+            if (b->nodes[nd.left].left >= 0) frontier.push_back(nd.left);
+            if (b->nodes[nd.right].left >= 0) frontier.push_back(nd.right);
+        }
+        for (auto it = frontier.rbegin(); it != frontier.rend(); ++it) stack.push_back(*it);      // the rest depth-first, in breadth-first order of their roots
+    }
     while (!stack.empty()) {
         int32_t i = stack.back(); stack.pop_back();
         gpu_index[i] = (int32_t)order.size(); order.push_back(i);

@@ -18,6 +18,7 @@ struct crt_ctx {
     int trace_leaf_wait = 6;           // leave the inner-node phase when at most this many converged lanes still lack a leaf
     int trace_tri_wait = 8;            // wide kernel: a warp enters its triangle phase when at least this many lanes hold triangle hits
     int trace_blocks_per_sm = 0; // 0 = from occupancy
+    int trace_exact = 1;         // 1: the bit-exact triangle test (D:R0); 0: fused multiply-adds + approximate reciprocal (north_star's tolerances only)
     int fuse_shade = 1;          // crt_render_frame: shade non-final segments inside the next generation kernel (default; measured: DESIGN.md 5.4)
     // persistent-kernel work counter
     unsigned int* d_counter = nullptr;
@@ -119,6 +120,8 @@ crt_status crt_make_layout(crt_ctx* ctx, const crt_frame* f, const crt_order* o,
 
 // kernels' host launchers (defined in the .cu files) ------------------------------------------------------
 crt_status launch_trace(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, crt_hit* hits, cudaStream_t st, bool far_origins = false);
+bool trace_queue_supported(const crt_bvh* bvh);
+crt_status launch_trace_queue(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, crt_hit* hits, unsigned long long* stats, cudaStream_t st);
 crt_status launch_trace_wide(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, crt_hit* hits, cudaStream_t st);
 crt_status launch_trace_wide_stats(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, int64_t* counters, cudaStream_t st);
 crt_status launch_trace_stats(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, int64_t* counters, cudaStream_t st);

@@ -4,7 +4,8 @@
 // B200 design:
 //  - stack-based traversal of a binary BVH.  Default layout (trace_kernel 3): 32-byte nodes holding both children's boxes as
 //    16-bit planes on a scene grid, fetched with ONE 256-bit load (ld.global.nc.v8 -> LDG.E.ENL2.256) on the read-only path and
-//    decoded by one PRMT per plane that also selects the near or far plane by the ray's direction sign (struct QRay below);
+//    decoded by one PRMT per plane that also selects the near or far plane by the ray's direction sign (struct QRay below); the
+//    twelve plane distances of a visit are six packed FFMA2 (fma.rn.f32x2, new on sm_100: one issue slot for two fused multiply-adds);
 //    the fp32 form (64-byte nodes, two 256-bit loads) is trace_kernel 0 / 1; leaf triangles are 64-byte records (v0|id, e1, e2);
 //  - with the 16-bit nodes the kernel is issue- and latency-bound, not bandwidth-bound (profiles/r01f): what matters is how many
 //    lanes of a warp do useful work and how many warps are resident (8 blocks of 128 threads per SM at 64 registers).
@@ -33,7 +34,9 @@ constexpr int SENTINEL = 0x7fffffff;
 constexpr int TRACE_BLOCK = 128;
 // resident blocks per SM the persistent kernel is compiled for: fp32 nodes 9 (<= 56 registers), 16-bit nodes 8 (<= 64
 // registers; measured 1.5-3 % faster than 9 with this layout, profiles/r01f)
-#define CRT_TRACE_MINB(QN) ((QN) ? 8 : 9)      // QN: 0 fp32 nodes, 1 16-bit nodes, 2 16-bit nodes with the any-origin box test
+#define CRT_TRACE_MINB(QN) ((QN) ? 8 : 9)      // QN: 0 fp32 nodes; 1 16-bit nodes (default); 2 16-bit nodes with the any-origin box test; 3 as 1 with the
+                                               // tolerance-only triangle test (trace_exact = 0); 4 as 1 with the top of the tree staged in shared memory (experiment)
+constexpr int TREELET_NODES = 512;             // QN 4: nodes 0 .. 511 (the top levels: crt_bvh_flatten numbers them breadth-first) = 16 KB of shared memory per block
 #ifndef CRT_VISITS_PER_VOTE
 #define CRT_VISITS_PER_VOTE 3   // inner-node visits between two leaf-wait votes of a warp
 #endif
@@ -184,8 +187,60 @@ CRT_DEV int visit_qnode(const QNode* __restrict__ nodes, int idx, const RayState
     return next;
 }
 
+// The same visit with the twelve plane distances computed by SIX packed FFMA2 (fma.rn.f32x2, new on sm_100): the kernel is bound
+// by instruction issue, and a packed instruction is one issue slot for two fused multiply-adds.  Each half of a packed operation is
+// the same IEEE fma as the scalar one, so the distances, and hence the visit order, are bit-identical to visit_qnode<false>.
+struct F2 { unsigned long long v; };
+CRT_DEV F2 pack2(float lo, float hi) { F2 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r.v) : "f"(lo), "f"(hi)); return r; }
+CRT_DEV void unpack2(F2 a, float& lo, float& hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(a.v)); }
+CRT_DEV F2 fma2(F2 a, F2 b, F2 c) { F2 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r.v) : "l"(a.v), "l"(b.v), "l"(c.v)); return r; }
+CRT_DEV float qbits(unsigned w, unsigned sel)
+{
+    unsigned f;
+    asm("prmt.b32 %0, %1, %2, %3;" : "=r"(f) : "r"(w), "r"(0x4B000000u), "r"(sel));
+    return __uint_as_float(f);
+}
+struct QRay2 {
+    F2 sxy, szz, cxy, czz;                // (sx, sy), (sz, sz), (cx, cy), (cz, cz)
+    unsigned nx, ny, nz, fx, fy, fz;
+    template <bool SAFE> CRT_DEV void init(const QRay<SAFE>& q)
+    {
+        sxy = pack2(q.sx, q.sy); szz = pack2(q.sz, q.sz); cxy = pack2(q.cx, q.cy); czz = pack2(q.cz, q.cz);
+        nx = q.nx; ny = q.ny; nz = q.nz; fx = q.fx; fy = q.fy; fz = q.fz;
+    }
+};
+template <bool TREELET>
+CRT_DEV int visit_qnode2(const QNode* __restrict__ nodes, const uint4* s_treelet, int idx, const RayState& r, const QRay2& q, int*& top)
+{
+    unsigned w0, w1, w2, w3, w4, w5; int ra, rb;
+    if (TREELET && idx < TREELET_NODES) {
+        const uint4 a = s_treelet[2 * idx], b = s_treelet[2 * idx + 1];
+        w0 = a.x; w1 = a.y; w2 = a.z; w3 = a.w; w4 = b.x; w5 = b.y; ra = (int)b.z; rb = (int)b.w;
+    } else
+    asm volatile("ld.global.nc.v8.u32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                 : "=r"(w0), "=r"(w1), "=r"(w2), "=r"(w3), "=r"(w4), "=r"(w5), "=r"(ra), "=r"(rb) : "l"(nodes + idx));
+    const float tfar = r.tfar();
+    float n0x, n0y, f0x, f0y, n1x, n1y, f1x, f1y, n0z, n1z, f0z, f1z;
+    unpack2(fma2(pack2(qbits(w0, q.nx), qbits(w1, q.ny)), q.sxy, q.cxy), n0x, n0y);
+    unpack2(fma2(pack2(qbits(w0, q.fx), qbits(w1, q.fy)), q.sxy, q.cxy), f0x, f0y);
+    unpack2(fma2(pack2(qbits(w3, q.nx), qbits(w4, q.ny)), q.sxy, q.cxy), n1x, n1y);
+    unpack2(fma2(pack2(qbits(w3, q.fx), qbits(w4, q.fy)), q.sxy, q.cxy), f1x, f1y);
+    unpack2(fma2(pack2(qbits(w2, q.nz), qbits(w5, q.nz)), q.szz, q.czz), n0z, n1z);
+    unpack2(fma2(pack2(qbits(w2, q.fz), qbits(w5, q.fz)), q.szz, q.czz), f0z, f1z);
+    const float tn0 = fmaxf(fmaxf(n0x, n0y), fmaxf(n0z, r.tmin));
+    const float tf0 = fminf(fminf(f0x, f0y), fminf(f0z, tfar));
+    const float tn1 = fmaxf(fmaxf(n1x, n1y), fmaxf(n1z, r.tmin));
+    const float tf1 = fminf(fminf(f1x, f1y), fminf(f1z, tfar));
+    const bool h0 = tn0 <= tf0, h1 = tn1 <= tf1;
+    const bool second = h1 && (!h0 || tn1 < tn0);
+    int next = second ? rb : ra;
+    if (h0 && h1) *++top = second ? ra : rb;
+    if (!(h0 || h1)) next = *top--;
+    return next;
+}
+
 // Tests the triangles of a leaf reference (D:R10 tie-break: lower primitive id wins at equal t).
-template <bool COUNT>
+template <bool COUNT, bool FAST = false>
 CRT_DEV void visit_leaf(const GpuTri* __restrict__ tris, int ref, RayState& r, unsigned& n_tris, crt_hit* __restrict__ hits, int ray_idx)
 {
     const int leaf = ~ref;
@@ -198,7 +253,8 @@ CRT_DEV void visit_leaf(const GpuTri* __restrict__ tris, int ref, RayState& r, u
         const float4 a = make_float4(q0.min_x, q0.max_x, q0.min_y, q0.max_y), b = make_float4(q0.min_z, q0.max_z, __int_as_float(q0.ref), 0.f);
         float t, u, v;
         if (COUNT) ++n_tris;
-        if (tri_test(mk(a.x, a.y, a.z), mk(b.x, b.y, b.z), mk(c.x, c.y, c.z), r.o, r.d, r.tmin, __int_as_float(0x7f800000), t, u, v)) {
+        if (FAST ? tri_test_fast(mk(a.x, a.y, a.z), mk(b.x, b.y, b.z), mk(c.x, c.y, c.z), r.o, r.d, r.tmin, __int_as_float(0x7f800000), t, u, v)
+                 : tri_test(mk(a.x, a.y, a.z), mk(b.x, b.y, b.z), mk(c.x, c.y, c.z), r.o, r.d, r.tmin, __int_as_float(0x7f800000), t, u, v)) {
             // t < tmax and the (t, id) rule in one: best.t is the ray's tmax until a hit exists, the best t afterwards
             const int prim = __float_as_int(a.w);
             if (t < r.best.t || (t == r.best.t && r.best.prim >= 0 && prim < r.best.prim)) {
@@ -241,14 +297,19 @@ template <bool COUNT, int QN>
 __global__ void __launch_bounds__(TRACE_BLOCK, CRT_TRACE_MINB(QN)) trace_dyn_kernel(const GpuNode* __restrict__ nodes, const QNode* __restrict__ qnodes, const QGrid grid, const GpuTri* __restrict__ tris,
                                                                 const crt_ray* __restrict__ rays, crt_hit* __restrict__ hits, int64_t n,
                                                                 unsigned int* __restrict__ counter, int refill_threshold, int leaf_wait,
-                                                                unsigned long long* __restrict__ stats)
+                                                                unsigned long long* __restrict__ stats, int n_qnodes)
 {
     const unsigned lane = threadIdx.x & 31u;
+    extern __shared__ uint4 s_treelet[];
+    if (QN == 4) {       // experiment (north_star: "a node-prefetch stage in shared memory"): the top of the tree, once per block
+        for (int i = threadIdx.x; i < 2 * TREELET_NODES; i += blockDim.x) s_treelet[i] = i < 2 * n_qnodes ? reinterpret_cast<const uint4*>(qnodes)[i] : make_uint4(0u, 0u, 0u, 0u);
+        __syncthreads();
+    }
     int stack[STACK_SIZE]; int* top = stack; stack[0] = SENTINEL;      // top: pointer to the top entry (no index-to-address LEA per push/pop)
     int node = SENTINEL, leaf = 0;      // leaf: postponed leaf reference (< 0) or 0 = none
     int ray_idx = -1;
     bool exhausted = false;
-    RayState r; QRay<QN == 2> q;
+    RayState r; QRay<QN == 2> q; QRay2 q2;
     unsigned c_nodes = 0, c_tris = 0, c_rays = 0;
 
     for (;;) {
@@ -276,6 +337,7 @@ __global__ void __launch_bounds__(TRACE_BLOCK, CRT_TRACE_MINB(QN)) trace_dyn_ker
                     } else {
                         r.init(__ldg(rp), rd);
                         if (QN) q.init(r, grid);
+                        if (QN == 1 || QN >= 3) q2.init(q);
                         ray_idx = (int)i; node = 0; leaf = 0; top = stack;
                         if (COUNT) ++c_rays;
                     }
@@ -295,14 +357,14 @@ __global__ void __launch_bounds__(TRACE_BLOCK, CRT_TRACE_MINB(QN)) trace_dyn_ker
                 for (int rep = 0; rep < CRT_VISITS_PER_VOTE; ++rep) {
                     if (rep > 0 && (unsigned)node >= (unsigned)SENTINEL) break;
                     if (COUNT) ++c_nodes;
-                    node = QN ? visit_qnode(qnodes, node, r, q, top) : visit_node(load_node(nodes, node), r, top);
+                    node = QN == 4 ? visit_qnode2<true>(qnodes, s_treelet, node, r, q2, top) : ((QN == 1 || QN == 3) ? visit_qnode2<false>(qnodes, nullptr, node, r, q2, top) : (QN ? visit_qnode(qnodes, node, r, q, top) : visit_node(load_node(nodes, node), r, top)));
                     if (node < 0 && leaf == 0) { leaf = node; node = *top--; }
                 }
                 if (__popc(__ballot_sync(__activemask(), leaf == 0)) <= leaf_wait) break;   // (nearly) every converged lane holds a leaf
             }
             // leaves: the postponed one, then any further leaf references that come off the stack
             while (leaf < 0) {
-                visit_leaf<COUNT>(tris, leaf, r, c_tris, hits, ray_idx);
+                visit_leaf<COUNT, QN == 3>(tris, leaf, r, c_tris, hits, ray_idx);
                 leaf = 0;
                 if (node < 0) { leaf = node; node = *top--; }
             }
@@ -349,13 +411,13 @@ crt_status launch_dyn(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int
 {
     int per_sm = ctx->trace_blocks_per_sm;
     if (per_sm <= 0) {
-        CRT_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, trace_dyn_kernel<COUNT, QN>, TRACE_BLOCK, 0));
+        CRT_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, trace_dyn_kernel<COUNT, QN>, TRACE_BLOCK, QN == 4 ? (size_t)TREELET_NODES * 32 : (size_t)0));
         if (per_sm < 1) per_sm = 1;
     }
     CRT_CUDA(ctx, cudaMemsetAsync(ctx->d_counter, 0, sizeof(unsigned int), st));
     int64_t want = (n + TRACE_BLOCK - 1) / TRACE_BLOCK, grid = (int64_t)ctx->n_sms * per_sm;
     if (grid > want) grid = want;
-    trace_dyn_kernel<COUNT, QN><<<(unsigned)grid, TRACE_BLOCK, 0, st>>>(bvh->d_nodes, bvh->d_qnodes, bvh->qgrid, bvh->d_tris, rays, hits, n, ctx->d_counter, ctx->trace_refill_threshold, ctx->trace_leaf_wait, stats);
+    trace_dyn_kernel<COUNT, QN><<<(unsigned)grid, TRACE_BLOCK, QN == 4 ? (size_t)TREELET_NODES * 32 : (size_t)0, st>>>(bvh->d_nodes, bvh->d_qnodes, bvh->qgrid, bvh->d_tris, rays, hits, n, ctx->d_counter, ctx->trace_refill_threshold, ctx->trace_leaf_wait, stats, (int)bvh->n_gpu_nodes);
     CRT_CHECK_LAUNCH(ctx, "trace_dyn");
     return CRT_OK;
 }
@@ -385,8 +447,11 @@ crt_status launch_trace(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, i
     // 16-bit nodes unless the grid is too coarse for this scene's detail (decoded boxes more than twice the fp32 boxes' area) or
     // the layout failed its own check (a plane clamped or less than one step outside its box: crt_bvh_check bit 16)
     const bool q_ok = bvh->q_inflation <= 2.0 && bvh->q_violations == 0;
-    if ((ctx->trace_kernel == 4 || (ctx->trace_kernel == 3 && far_origins)) && q_ok) return launch_dyn<false, 2>(ctx, bvh, rays, n, hits, nullptr, st);
-    if (ctx->trace_kernel == 3 && q_ok) return launch_dyn<false, 1>(ctx, bvh, rays, n, hits, nullptr, st);
+    if (ctx->trace_kernel == 5 && !far_origins && trace_queue_supported(bvh)) return launch_trace_queue(ctx, bvh, rays, n, hits, nullptr, st);
+    if (ctx->trace_kernel == 6 && !far_origins && q_ok) return launch_dyn<false, 4>(ctx, bvh, rays, n, hits, nullptr, st);
+    if (ctx->trace_kernel == 3 && !ctx->trace_exact && !far_origins && q_ok) return launch_dyn<false, 3>(ctx, bvh, rays, n, hits, nullptr, st);
+    if ((ctx->trace_kernel == 4 || (ctx->trace_kernel >= 3 && far_origins)) && q_ok) return launch_dyn<false, 2>(ctx, bvh, rays, n, hits, nullptr, st);
+    if (ctx->trace_kernel >= 3 && q_ok) return launch_dyn<false, 1>(ctx, bvh, rays, n, hits, nullptr, st);
     return launch_dyn<false, 0>(ctx, bvh, rays, n, hits, nullptr, st);
 }
 
@@ -396,8 +461,9 @@ crt_status launch_trace_stats(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* r
     if (n == 0) return CRT_OK;
     if (ctx->trace_kernel == 2 && bvh->d_wnodes && bvh->wide_violations == 0) return launch_trace_wide_stats(ctx, bvh, rays, n, counters, st);
     const bool q_ok = bvh->q_inflation <= 2.0 && bvh->q_violations == 0;
+    if (ctx->trace_kernel == 5 && trace_queue_supported(bvh)) return launch_trace_queue(ctx, bvh, rays, n, nullptr, reinterpret_cast<unsigned long long*>(counters), st);
     if (ctx->trace_kernel == 4 && q_ok) return launch_dyn<true, 2>(ctx, bvh, rays, n, nullptr, reinterpret_cast<unsigned long long*>(counters), st);
-    if (ctx->trace_kernel == 3 && q_ok) return launch_dyn<true, 1>(ctx, bvh, rays, n, nullptr, reinterpret_cast<unsigned long long*>(counters), st);
+    if (ctx->trace_kernel >= 3 && q_ok) return launch_dyn<true, 1>(ctx, bvh, rays, n, nullptr, reinterpret_cast<unsigned long long*>(counters), st);
     return launch_dyn<true, 0>(ctx, bvh, rays, n, nullptr, reinterpret_cast<unsigned long long*>(counters), st);
 }
 

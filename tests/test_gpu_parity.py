@@ -105,7 +105,7 @@ def test_full_size_config2_stagewise_and_sampled(crt, ctx, oracle):
 
 # ------------------------------------------------------------------ a0 / a5: BVH + traversal
 @pytest.mark.parametrize("scene_name", ["cornell", "interior_small", "landscape_small"])
-@pytest.mark.parametrize("kernel", [0, 1, 2, 3, 4])
+@pytest.mark.parametrize("kernel", [0, 1, 2, 3, 4, 5, 6])
 def test_trace_matches_oracle_on_random_rays(crt, ctx, oracle, scene_name, kernel):
     scene = SCENES[scene_name]()
     # kernel 2 reads the 8-wide compressed layout, which exists when every leaf holds one triangle
@@ -128,6 +128,27 @@ def test_trace_matches_oracle_on_random_rays(crt, ctx, oracle, scene_name, kerne
     # the triangle test is the same fp32 operation sequence on both sides: where ids agree the record is bit-identical
     same = h["prim"] == ho["prim"]
     assert (h[same].tobytes() == ho[same].tobytes())
+
+
+def test_trace_tolerance_only_triangle_test(crt, ctx, oracle):
+    """Option trace_exact = 0 (fused multiply-adds + approximate reciprocal in the triangle test; measured 3-5 % faster, profiles/r02a):
+    NOT the default, because it only meets part of north_star's bar: ids agree on >= 99.99 % of rays, but t of grazing hits can
+    deviate by a few 1e-4 relative.  Checked here: ids >= 99.99 %, hit/miss decisions equal except at those, t within 1e-3."""
+    scene = _small_interior()
+    G = GpuScene(crt, scene, ctx)
+    info = G.bvh.info()
+    r = I.random_rays(5, 200000 + 13, info["bounds"][:3], info["bounds"][3:], inactive_frac=0.05)
+    ho = hits_np(oracle, ctx.crt_trace(G.bvh, ctx.upload(r)))
+    ctx.crt_set_option("trace_exact", 0)
+    try:
+        h = hits_np(oracle, ctx.crt_trace(G.bvh, ctx.upload(r)))
+    finally:
+        ctx.crt_set_option("trace_exact", 1)
+    same = h["prim"] == ho["prim"]
+    assert same.mean() >= 0.9999
+    m = same & (ho["prim"] >= 0)
+    assert np.all(np.abs(h["t"][m].astype(np.float64) - ho["t"][m]) <= 1e-3 * np.abs(ho["t"][m]))
+    assert np.median(np.abs(h["t"][m].astype(np.float64) - ho["t"][m]) / np.abs(ho["t"][m])) < 1e-6
 
 
 def test_trace_tiny_scene_against_brute_force(crt, ctx, oracle):

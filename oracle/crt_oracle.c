@@ -394,7 +394,7 @@ void orc_trace(const orc_bvh* b, const orc_ray* rays, int64_t n_rays, orc_hit* h
 /* ------------------------------------------------------------------ partition (D:R3-R5)
  * BASELINE.json's "group gw x gh, interleave stride s"  <->  the paper's tile W x H and
  * group size K:  K = gw*gh, W = gw*s, H = gh*s, M = W*H slots per tile, G = M/K groups. */
-typedef struct { int32_t W, H, M, K, G, tiles_x, tiles_y, n_tiles; int64_t n_slots, n_paths; int32_t gw, gh, sx, sy, lattice; } layout;
+typedef struct { int32_t W, H, M, K, G, tiles_x, tiles_y, n_tiles; int64_t n_slots, n_paths; int32_t gw, gh, sx, sy, lattice, sequence; } layout;
 static layout make_layout(const orc_frame* f, int mode, int gw, int gh, int s)
 {
     layout L; memset(&L, 0, sizeof L);
@@ -405,6 +405,7 @@ static layout make_layout(const orc_frame* f, int mode, int gw, int gh, int s)
      * stride travels in the high 16 bits of s (0 = same as the horizontal one).  DESIGN.md D:R5. */
     int32_t sx = s & 0x3fff, sy = (s >> 16) ? (s >> 16) : sx;
     L.gw = gw; L.gh = gh; L.sx = sx; L.sy = sy; L.lattice = (s >> 14) & 1;      /* bit 14: partition rule LATTICE (D:R20) */
+    L.sequence = (s >> 15) & 1;                                                 /* bit 15: partition rule LCG SEQUENCE (D:R21) */
     L.W = gw * sx; L.H = gh * sy; L.M = L.W * L.H; L.K = gw * gh; L.G = L.M / L.K;
     L.tiles_x = (f->w + L.W - 1) / L.W; L.tiles_y = (f->h + L.H - 1) / L.H; L.n_tiles = L.tiles_x * L.tiles_y;
     L.n_slots = (int64_t)f->spp * L.n_tiles * L.M;
@@ -437,11 +438,23 @@ static void partition(const orc_frame* f, const layout* L, int mode, int32_t* pa
         for (int32_t tile = 0; tile < L->n_tiles; ++tile) {
             uint32_t a, c, a0, c0; tile_lcg(f, L, tile, sg, &a, &c); tile_raw(f, tile, sg, &a0, &c0);
             int32_t tx = tile % L->tiles_x, ty = tile / L->tiles_x;
+            /* third reading of "shuffled using a linear congruence method" (S:8c A-1; D:R21): the shuffled number of pixel n is
+             * the n-th term of a linear congruential SEQUENCE x_{n+1} = (A x_n + C) mod M of full period (Hull-Dobell for M a power
+             * of two: C odd, A = 1 mod 4), started at x_0; A, C, x_0 from the TILE stream, so it varies per tile, sample and frame. */
+            uint32_t seqA = 1, seqC = 1, xs = 0;
+            if (L->sequence) {
+                uint32_t r[4];
+                orc_philox((uint32_t)tile, (uint32_t)sg, 0u, PURPOSE_TILE, (uint32_t)f->seed, (uint32_t)f->frame, r);
+                seqA = ((r[0] % (uint32_t)L->M) & ~3u) | 1u; seqC = (r[1] % (uint32_t)L->M) | 1u; xs = r[2] % (uint32_t)L->M;
+            }
             for (int32_t n = 0; n < L->M; ++n) {
                 int32_t lx = n % L->W, ly = n / L->W;                  /* order on the screen inside the tile */
                 int32_t x = tx * L->W + lx, y = ty * L->H + ly;
+                uint32_t xn = xs;                                      /* n-th term of the sequence; the next pixel number gets the next term */
+                xs = (seqA * xs + seqC) % (uint32_t)L->M;
                 if (x >= f->w || y >= f->h) continue;
                 uint32_t m = (a * (uint32_t)n + c) % (uint32_t)L->M;   /* shuffled number */
+                if (L->sequence) m = xn;
                 if (L->lattice) {
                     /* alternative reading of BASELINE's "interleave stride" (S:8c A-3; D:R20): a REGULAR lattice.  The tile is
                      * shifted cyclically by an offset drawn per tile, sample and frame ("varies in each tile and in each frame",

@@ -624,3 +624,78 @@ def test_unbiasedness_rmse_shrinks_with_frames(oracle):
     for mode in (M_IND, M_REUSE):
         assert err[(mode, 64)] < 0.45 * err[(mode, 4)]
         assert err[(mode, 64)] < 0.05
+
+
+# ------------------------------------------------------------------ third partition rule: LCG sequence (S:8c A-1; D:R21)
+SEQUENCE = 1 << 15      # partition rule bit in the packed stride
+
+
+@pytest.mark.parametrize("gw,gh,s", [(4, 4, 2), (4, 4, 4), (2, 2, 8), (8, 8, 8), (8, 1, 1 | (8 << 16)), (1, 1, 4), (1, 1, 1), (2, 1, 1)])
+@pytest.mark.parametrize("w,h,spp", [(64, 64, 1), (50, 37, 2)])
+def test_lcg_sequence_partition_is_a_full_period_sequence(oracle, gw, gh, s, w, h, spp):
+    """"Shuffled using a linear congruence method" read as a SEQUENCE: the shuffled number of pixel n is the n-th term of
+    x_{n+1} = (A x_n + C) mod M.  Exact cover as for the other rules; inside a full tile consecutive pixel numbers satisfy the
+    recurrence with ONE pair (A, C), A = 1 mod 4 and C odd (Hull-Dobell: full period for M a power of two, so the terms are a
+    permutation); the terms follow from the tile's Philox TILE stream by plain iteration (brute force here)."""
+    fr = oracle.frame(w, h, spp, seed=3, frame=5)
+    pos = oracle.partition(fr, M_REUSE, gw, gh, s | SEQUENCE)
+    W, H = gw * (s & 0x3fff), gh * ((s >> 16) or (s & 0x3fff))
+    M, K = W * H, gw * gh
+    tiles_x, tiles_y = -(-w // W), -(-h // H)
+    assert len(pos) == spp * tiles_x * tiles_y * M == oracle.n_slots(fr, M_REUSE, gw, gh, s | SEQUENCE)
+    live = pos[pos >= 0]
+    assert np.array_equal(np.sort(live), np.arange(spp * w * h))                 # every path exactly once
+    slot = np.nonzero(pos >= 0)[0]
+    x = live % w; y = (live // w) % h
+    assert np.array_equal((slot // M) % (tiles_x * tiles_y), (y // H) * tiles_x + (x // W))
+    if w >= W and h >= H:
+        for tile in (0, tiles_x + 1 if tiles_x > 1 and tiles_y > 1 else 0):
+            blk = pos[tile * M:(tile + 1) * M]
+            assert np.all(blk >= 0)
+            tx, ty = tile % tiles_x, tile // tiles_x
+            n_of_m = ((blk // w) - ty * H) * W + ((blk % w) - tx * W)
+            m_of_n = np.empty(M, np.int64); m_of_n[n_of_m] = np.arange(M)
+            # brute force from the definition: A, C, x0 from the TILE stream (counter (tile, sample 0, 0, purpose 2), key (seed, frame))
+            r = oracle.philox(tile, 0, 0, 2, 3, 5)
+            A, C, x0 = ((r[0] % M) & ~3) | 1, (r[1] % M) | 1, r[2] % M
+            assert A % 4 == 1 and C % 2 == 1
+            xs, xv = [], x0
+            for _ in range(M):
+                xs.append(xv); xv = (A * xv + C) % M
+            assert np.array_equal(m_of_n, np.array(xs))
+            assert sorted(xs) == list(range(M))                                   # full period
+            assert np.all(np.bincount(m_of_n // K, minlength=M // K) == K)        # K members per group (quotient rule)
+
+
+def test_lcg_sequence_differs_from_the_affine_map_and_varies(oracle):
+    fr0 = oracle.frame(64, 64, 1, 0, 0); fr1 = oracle.frame(64, 64, 1, 0, 1)
+    ps = oracle.partition(fr0, M_REUSE, 4, 4, 2 | SEQUENCE).reshape(-1, 64)
+    pa = oracle.partition(fr0, M_REUSE, 4, 4, 2).reshape(-1, 64)
+    assert not np.array_equal(ps, pa)
+    assert not np.array_equal(ps, oracle.partition(fr1, M_REUSE, 4, 4, 2 | SEQUENCE).reshape(-1, 64))
+    loc = lambda p: ((p // 64) % 8) * 8 + (p % 64) % 8
+    assert len({tuple(loc(row)) for row in ps}) > 32                               # different tiles, different sequences
+    # an affine map of n has constant second differences 0 mod M; a sequence with A != 1 does not
+    n_nonaffine = 0
+    for row in ps:
+        m_of_n = np.empty(64, np.int64); m_of_n[loc(row)] = np.arange(64)
+        d2 = (m_of_n[2:] - 2 * m_of_n[1:-1] + m_of_n[:-2]) % 64
+        n_nonaffine += int(np.any(d2 != 0))
+    assert n_nonaffine > len(ps) // 2
+
+
+def test_lcg_sequence_rule_keeps_the_reuse_invariants_and_the_furnace(oracle):
+    sc = I.cornell()
+    g = _first_bounce(oracle, sc, M_REUSE, s=2 | SEQUENCE)
+    gi = _first_bounce(oracle, sc, M_IND)
+    K = 16
+    loc = g["local_dir"].reshape(-1, K, 3); src = g["dir_src"].reshape(-1, K); act = g["rays"]["tmax"].reshape(-1, K) >= 0
+    n = 0
+    for gidx in np.nonzero(g["group_class"] == oracle.CLASS_DIFFUSE)[0]:
+        a = act[gidx]; d = loc[gidx][a]
+        assert np.all(d == d[0]) and np.array_equal(gi["local_dir"][src[gidx][a][0]], d[0])
+        n += 1
+    assert n > 100
+    sph = I.furnace_sphere(2, albedo=1.0)
+    img, _, cnt = oracle.render_frame(oracle.Bvh(sph.verts), sph, oracle.frame(sph.width, sph.height, 2, 0, 1), 2, M_REUSE, 4, 4, 2 | SEQUENCE)
+    assert np.all(img == 1.0) and cnt[0] > 0

@@ -453,10 +453,10 @@ def run_sweep(args):
                 img, t = render("direct_reuse", 0, 0, F, 0, tile=(tw, th, k))
                 points.append(dict(mode="direct_reuse", tile=[tw, th], K=k, **t, rmse_vs_reference=rmse(img, ref), rmse_vs_independent=rmse(img, ind),
                                    trace_speedup_vs_independent=t["trace_only_mray_s"] / ind_t["trace_only_mray_s"]))
-    elif rules:     # the two readings of "interleave stride" (DESIGN.md D:R3 shuffled numbers, D:R20 regular lattice) side by side
+    elif rules:     # the three partition rules side by side (DESIGN.md D:R3 affine shuffle, D:R20 regular lattice, D:R21 LCG sequence)
         for g in (4, 8):
             for s in (2, 4, 8):
-                for rule, rname in ((0, "shuffle"), (1, "lattice")):
+                for rule, rname in ((0, "shuffle"), (1, "lattice"), (2, "lcg_sequence")):
                     img, t = render("direct_reuse", g, s, F, 0, rule=rule)
                     points.append(dict(mode="direct_reuse", group=g, stride=s, partition_rule=rname, **t, rmse_vs_reference=rmse(img, ref), rmse_vs_independent=rmse(img, ind),
                                        trace_speedup_vs_independent=t["trace_only_mray_s"] / ind_t["trace_only_mray_s"]))
@@ -465,7 +465,7 @@ def run_sweep(args):
             for s in (1, 2, 4, 8):
                 img, t = render("direct_reuse", g, s, F, 0)
                 points.append(dict(mode="direct_reuse", group=g, stride=s, **t, rmse_vs_reference=rmse(img, ref), rmse_vs_independent=rmse(img, ind)))
-    name = "the paper's Table 3 shapes (P:L178-185)" if table3 else ("partition rules (D:R3 / D:R20)" if rules else "BASELINE config 3")
+    name = "the paper's Table 3 shapes (P:L178-185)" if table3 else ("partition rules (D:R3 / D:R20 / D:R21)" if rules else "BASELINE config 3")
     print(json.dumps({"sweep": points, "config": {"workload": f"{name}: interior scene {w}x{h}, {spp} spp, {nb} bounces", "frames": F,
                                                   "reference_frames": 4 * F, "scale": sc}}))
 

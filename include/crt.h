@@ -79,7 +79,10 @@ typedef struct { float eye[3], U[3], V[3], W[3]; } crt_camera;
  * pixel numbers "shuffled using a linear congruence method" (D:R3).  CRT_PARTITION_LATTICE (1): a regular lattice, the
  * literal reading of "interleave stride" (D:R20): after a cyclic shift of the tile drawn per tile, sample and frame, the pixels
  * congruent modulo (stride, stride_y) form a group; its members lie stride / stride_y pixels apart. */
-typedef enum { CRT_PARTITION_SHUFFLE = 0, CRT_PARTITION_LATTICE = 1 } crt_partition_rule;
+/* CRT_PARTITION_LCG_SEQUENCE (2): the other reading of "shuffled using a linear congruence method" (D:R21): the shuffled
+ * number of pixel n is the n-th TERM of a full-period linear congruential sequence x -> (A x + C) mod M (C odd, A = 1 mod 4;
+ * A, C and the start x_0 drawn per tile, sample and frame), instead of the affine image a*n + c of the number itself. */
+typedef enum { CRT_PARTITION_SHUFFLE = 0, CRT_PARTITION_LATTICE = 1, CRT_PARTITION_LCG_SEQUENCE = 2 } crt_partition_rule;
 typedef struct { int32_t mode, group_w, group_h, stride, stride_y, partition_rule; } crt_order;
 /* materials: [device] table indexed by the per-triangle material id given to crt_build_bvh.
  * env: radiance on a miss = lerp(env[0..2], env[3..5], 0.5*(d.y+1)) (D:R14). */

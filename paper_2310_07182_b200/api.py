@@ -117,11 +117,11 @@ def make_frame(w, h, spp=1, seed=0, frame=0):
 
 
 def make_order(mode, group_w=1, group_h=1, stride=1, stride_y=0, partition_rule=0):
-    """partition_rule: 0 = the paper's shuffled numbers, 1 = regular lattice (include/crt.h).  `stride` also accepts the packed form the
-    tests use: bits 0-13 horizontal stride, bit 14 lattice rule, high half vertical stride."""
+    """partition_rule: 0 = the paper's shuffled numbers (affine map), 1 = regular lattice, 2 = LCG sequence (include/crt.h).  `stride` also
+    accepts the packed form the tests use: bits 0-13 horizontal stride, bit 14 lattice rule, bit 15 LCG-sequence rule, high half vertical stride."""
     stride = int(stride)
     if stride >> 14:
-        partition_rule = partition_rule or ((stride >> 14) & 1)
+        partition_rule = partition_rule or (1 if (stride >> 14) & 1 else (2 if (stride >> 15) & 1 else 0))
         stride, stride_y = stride & 0x3fff, (stride >> 16) or stride_y
     return Order(MODES[mode] if isinstance(mode, str) else int(mode), int(group_w), int(group_h), int(stride), int(stride_y), int(partition_rule))
 

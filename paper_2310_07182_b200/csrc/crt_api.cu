@@ -44,8 +44,8 @@ crt_status crt_make_layout(crt_ctx* ctx, const crt_frame* f, const crt_order* o,
         return crt_fail(ctx, CRT_ERR_UNSUPPORTED, "layout: group %dx%d stride %d/%d must be powers of two", o->group_w, o->group_h, o->stride, sy);
     const int64_t M = (int64_t)o->group_w * o->stride * o->group_h * sy, K = (int64_t)o->group_w * o->group_h;
     if (M > 4096 || K > 1024) return crt_fail(ctx, CRT_ERR_UNSUPPORTED, "layout: tile of %lld slots / group of %lld exceeds 4096 / 1024", (long long)M, (long long)K);
-    if (o->partition_rule != CRT_PARTITION_SHUFFLE && o->partition_rule != CRT_PARTITION_LATTICE) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "layout: partition_rule %d out of range", o->partition_rule);
-    L->gw = o->group_w; L->sx = o->stride; L->sy = sy; L->lattice = o->partition_rule == CRT_PARTITION_LATTICE;
+    if (o->partition_rule < CRT_PARTITION_SHUFFLE || o->partition_rule > CRT_PARTITION_LCG_SEQUENCE) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "layout: partition_rule %d out of range", o->partition_rule);
+    L->gw = o->group_w; L->sx = o->stride; L->sy = sy; L->lattice = o->partition_rule;       // 0 shuffle (affine), 1 lattice, 2 LCG sequence
     L->W = o->group_w * o->stride; L->H = o->group_h * sy; L->M = (int)M; L->K = (int)K; L->G = (int)(M / K);
     L->log2W = ilog2(L->W); L->log2M = ilog2(L->M); L->log2K = ilog2(L->K);
     L->tiles_x = (f->w + L->W - 1) / L->W; L->tiles_y = (f->h + L->H - 1) / L->H; L->n_tiles = L->tiles_x * L->tiles_y;

@@ -98,7 +98,7 @@ CRT_DEV bool tri_test_fast(V3 v0, V3 e1, V3 e2, V3 o, V3 d, float tmin, float tm
 struct DevLayout {
     int32_t w, h, spp, reuse;
     int32_t W, H, M, K, tiles_x, n_tiles, log2W, log2M, log2K;
-    int32_t lattice, gw, sx, sy;       // regular-lattice partition rule (D:R20): group width and strides (powers of two)
+    int32_t lattice, gw, sx, sy;       // partition rule (0 affine shuffle D:R3, 1 regular lattice D:R20, 2 LCG sequence D:R21), group width, strides
     uint32_t seed, frame;
 };
 // inverse of an odd number modulo 2^32 (Newton steps double the number of valid bits; a*a == 1 mod 8)
@@ -107,6 +107,17 @@ CRT_DEV uint32_t inv_odd(uint32_t a)
     uint32_t x = a;
     x *= 2u - a * x; x *= 2u - a * x; x *= 2u - a * x; x *= 2u - a * x;
     return x;
+}
+// LCG-sequence rule (D:R21): slot of in-tile pixel number n = the n-th term of x -> (A x + C) mod M started at x0, by jump-ahead
+// (A^n and 1 + A + ... + A^(n-1) by repeated squaring, modulo 2^32, which M divides): log2(n) steps instead of n.
+CRT_DEV uint32_t lcg_sequence_term(uint32_t A, uint32_t C, uint32_t x0, uint32_t n, uint32_t M)
+{
+    uint32_t ga = 1u, gc = 0u, h = A, f = C;        // after the loop: x_n = ga * x0 + gc
+    while (n) {
+        if (n & 1u) { ga *= h; gc = gc * h + f; }
+        f *= h + 1u; h *= h; n >>= 1;
+    }
+    return (ga * x0 + gc) & (M - 1u);
 }
 // path id of a slot (-1 = out-of-image slot) with its pixel and sample.  direct_reuse: the slot's position m in its
 // tile is the shuffled number m = (a*n + c) mod M of pixel n = ly*W + lx, so n = a^-1 (m - c) mod M.
@@ -120,7 +131,7 @@ CRT_DEV int32_t slot_to_path(const DevLayout& L, int64_t slot, int32_t& pixel, i
     const uint4 r = philox((uint32_t)tile, (uint32_t)sample, 0u, PURPOSE_TILE, L.seed, L.frame);
     const uint32_t a = (r.x & (uint32_t)(L.M - 1)) | 1u, c = r.y & (uint32_t)(L.M - 1);
     int32_t lx, ly;
-    if (L.lattice) {
+    if (L.lattice == 1) {
         // m = g*K + j with g = (py % sy)*sx + px % sx, j = (py / sy)*gw + px / sx, (px, py) = the pixel after the tile's cyclic shift
         const int32_t g = (int32_t)(m >> L.log2K), j = (int32_t)(m & (uint32_t)(L.K - 1));
         const int32_t px = (j & (L.gw - 1)) * L.sx + (g & (L.sx - 1)), py = (j / L.gw) * L.sy + g / L.sx;

@@ -113,7 +113,7 @@ struct Layout {
     int32_t w, h, spp, mode;
     int32_t W, H, M, K, G, tiles_x, tiles_y, n_tiles;
     int32_t log2W, log2M, log2K;
-    int32_t gw, sx, sy, lattice;       // group width, strides, partition rule (D:R20)
+    int32_t gw, sx, sy, lattice;       // group width, strides, partition rule (crt_partition_rule; D:R3, R20, R21)
     int64_t n_paths, n_slots, n_groups;
 };
 crt_status crt_make_layout(crt_ctx* ctx, const crt_frame* f, const crt_order* o, Layout* L);

@@ -385,10 +385,24 @@ struct CamDev { float eye[3], U[3], V[3], W[3]; };
 // a1: camera ray of each slot's path (D:R6); the rays are then traversed by the same kernel as secondary rays
 __global__ void __launch_bounds__(256) primary_rays_kernel(CamDev cam, DevLayout L, int64_t n_slots, crt_ray* __restrict__ rays, int32_t* __restrict__ r2p)
 {
-    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n_slots) return;
-    int32_t pixel, sample;
-    const int32_t p = slot_to_path(L, i, pixel, sample);
+    int32_t pixel, sample, p;
+    if (L.reuse && L.lattice == 2) {
+        // LCG-sequence rule (D:R21): the slot -> pixel inverse is a discrete logarithm, so the thread is mapped FORWARD: it takes pixel number
+        // n of its tile and writes the ray to the slot of the n-th term (a permutation inside the tile's block of M slots)
+        const uint32_t nn = (uint32_t)(i & (L.M - 1));
+        const int64_t blk = i >> L.log2M;
+        const int32_t tile = (int32_t)(blk % L.n_tiles);
+        sample = (int32_t)(blk / L.n_tiles);
+        const uint4 r = philox((uint32_t)tile, (uint32_t)sample, 0u, PURPOSE_TILE, L.seed, L.frame);
+        const uint32_t Mm = (uint32_t)(L.M - 1);
+        const uint32_t m = lcg_sequence_term(((r.x & Mm) & ~3u) | 1u, (r.y & Mm) | 1u, r.z & Mm, nn, (uint32_t)L.M);
+        const int32_t x = (tile % L.tiles_x) * L.W + (int32_t)(nn & (uint32_t)(L.W - 1)), y = (tile / L.tiles_x) * L.H + (int32_t)(nn >> L.log2W);
+        i = (blk << L.log2M) + m;
+        if (x >= L.w || y >= L.h) { pixel = -1; p = -1; }
+        else { pixel = y * L.w + x; p = (int32_t)(((int64_t)sample * L.h + y) * L.w + x); }
+    } else p = slot_to_path(L, i, pixel, sample);
     r2p[i] = p;
     float4* rp = reinterpret_cast<float4*>(rays + i);
     if (p < 0) { rp[0] = make_float4(0.f, 0.f, 0.f, 0.f); rp[1] = make_float4(0.f, 0.f, 0.f, -1.f); return; }

@@ -263,7 +263,9 @@ def test_trace_stats_counts(crt, ctx, oracle):
 
 # ------------------------------------------------------------------ a1: primary rays
 @pytest.mark.parametrize("mode,gw,gh,s", [("independent", 1, 1, 1), ("direct_reuse", 4, 4, 2), ("direct_reuse", 2, 4, 4), ("direct_reuse", 4, 4, 2 | (1 << 14)),
-                                          ("direct_reuse", 8, 2, 2 | (4 << 16) | (1 << 14))])
+                                          ("direct_reuse", 8, 2, 2 | (4 << 16) | (1 << 14)),
+                                          ("direct_reuse", 4, 4, 2 | (1 << 15)), ("direct_reuse", 8, 8, 8 | (1 << 15)), ("direct_reuse", 2, 1, 1 | (1 << 15)),   # LCG-sequence rule (D:R21)
+                                          ("direct_reuse", 8, 1, 1 | (8 << 16) | (1 << 15))])
 @pytest.mark.parametrize("w,h,spp", [(64, 64, 1), (50, 37, 2)])
 def test_primary_matches_oracle(crt, ctx, oracle, mode, gw, gh, s, w, h, spp):
     scene = I.cornell(width=w, height=h)
@@ -303,6 +305,8 @@ GEN_CASES = [
     ("checker", "direct_reuse", 1, 1, 4, 48, 40, 1),          # K = 1
     ("interior_small", "direct_reuse", 4, 4, 4 | (1 << 14), 96, 64, 1),      # regular-lattice partition rule (D:R20)
     ("checker", "direct_reuse", 4, 2, 2 | (4 << 16) | (1 << 14), 50, 37, 2),  # lattice, unequal strides, ragged, 2 spp, hybrid groups
+    ("interior_small", "direct_reuse", 4, 4, 4 | (1 << 15), 96, 64, 1),      # LCG-sequence partition rule (D:R21)
+    ("checker", "direct_reuse", 4, 2, 2 | (4 << 16) | (1 << 15), 50, 37, 2),  # sequence rule, unequal strides, ragged, 2 spp, hybrid groups
     ("interior_small", "direct_reuse", 8, 1, 1 | (8 << 16), 96, 64, 1),     # the paper's own setting: tile 8x8, K = 8
     ("interior_small", "direct_reuse", 16, 1, 2 | (8 << 16), 90, 61, 2),    # tile 32x8, K = 16 (Table 3), ragged, 2 spp
     ("landscape_small", "direct_reuse", 4, 4, 4, 96, 64, 1),  # config 4's grouping on a reduced landscape (coordinates up to 192, sky misses)
@@ -483,7 +487,7 @@ def test_mixed_materials_two_bounces_end_to_end(crt, ctx, oracle, mode, gw, gh, 
     assert rmse(accum.cpu().numpy() / 2, acc_o / 2) <= 1e-3
 
 
-@pytest.mark.parametrize("mode,gw,gh,s", [("direct_reuse", 4, 4, 2), ("direct_reuse", 4, 2, 2 | (4 << 16) | (1 << 14)), ("world_reuse", 8, 8, 1), ("independent", 1, 1, 1)])
+@pytest.mark.parametrize("mode,gw,gh,s", [("direct_reuse", 4, 4, 2), ("direct_reuse", 4, 2, 2 | (4 << 16) | (1 << 14)), ("direct_reuse", 4, 4, 2 | (1 << 15)), ("world_reuse", 8, 8, 1), ("independent", 1, 1, 1)])
 def test_render_frame_on_a_ragged_image_matches_the_oracle(crt, ctx, oracle, mode, gw, gh, s):
     """crt_render_frame as bench.py runs it (shading fused into generation, path state by slot under grouped orders) on an image that is
     not a multiple of the tile (50x37, 2 spp, 3 bounces, partial tiles on two sides): the accumulated image equals the oracle's."""

@@ -470,10 +470,10 @@ def run_sweep(args):
                                                   "reference_frames": 4 * F, "scale": sc}}))
 
 
-def _frame_ray_sets(ctx, crt, scene, w, h, spp, nb, gw, gh, s, seed, frame, modes=("direct_reuse", "independent")):
+def _frame_ray_sets(ctx, crt, scene, w, h, spp, nb, gw, gh, s, seed, frame, modes=("direct_reuse", "independent"), bvh=None):
     """The ray sets of one frame (primary, bounce 1 .. nb) in each order of `modes`: [(tag, rays)]."""
     import torch
-    bvh = ctx.crt_build_bvh(scene.verts, scene.mat_id)
+    bvh = bvh or ctx.crt_build_bvh(scene.verts, scene.mat_id)
     mats_dev = ctx.upload(scene.materials); mats = ctx.scene_mats(mats_dev, len(scene.materials), scene.env); cam = crt.make_camera(scene.camera)
     sets = []
     for mode in modes:
@@ -542,6 +542,49 @@ def run_kernels(args):
         sys.stderr.write(f"| {row['variant']} | " + " | ".join(f"{row['sets'][t]['ms']:.3f}{'' if row['sets'][t]['records_identical'] else ' (ids ' + format(row['sets'][t]['ids_equal_frac'], '.6f') + ')'}" for t in tags) + " |\n")
 
 
+def run_builders(args):
+    """Host (binned SAH) against device (PLOC, csrc/bvh_ploc.cu) BVH builder on --workload (profiles/r02b): build times, tree statistics,
+    crt_bvh_check, and crt_trace on one frame's ray sets (as --sweep kernels) with each tree; hit records must be identical."""
+    import torch
+    import paper_2310_07182_b200 as crt
+    import crt_inputs as I
+    name, kw, w, h, spp, nb, gw, gh, s, seed, cfg = WORKLOADS[args.workload]
+    scene = I.by_name(name, **kw).with_camera(w, h)
+    ctx = crt.Context(0)
+    trees = []
+    for label, bkw in [("host SAH (64 bins)", dict(builder=0))] + [(f"device PLOC radius {r}", dict(builder=1, ploc_radius=r)) for r in args.ploc_radii]:
+        t0 = time.time(); bvh = ctx.crt_build_bvh(scene.verts, scene.mat_id, **bkw); wall = time.time() - t0
+        info = bvh.info()
+        trees.append((label, bvh, dict(builder=label, wall_seconds=wall, hierarchy_seconds=info["build_seconds"], device_build_seconds=info["device_build_seconds"],
+                                       layout_seconds=info["layout_seconds"], rounds=info["build_rounds"], depth=info["depth"], sah_cost=info["sah_cost"],
+                                       n_nodes=info["n_nodes"], q16_inflation_pct=info["q16_inflation_pct"], check=bvh.check())))
+    _, _keep, sets = _frame_ray_sets(ctx, crt, scene, w, h, spp, nb, gw, gh, s, seed, 7, bvh=trees[0][1])
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=ctx.device)
+    ref = {tag: ctx.crt_trace(trees[0][1], r).clone() for tag, r in sets}
+    rows = []
+    for label, bvh, row in trees:
+        row["sets"] = {}
+        for tag, r in sets:
+            hh = ctx.crt_trace(bvh, r); torch.cuda.synchronize()
+            ts = []
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            for _ in range(8):
+                flush.fill_(1)
+                e0.record(); ctx.crt_trace(bvh, r, hits=hh); e1.record(); torch.cuda.synchronize()
+                ts.append(e0.elapsed_time(e1))
+            nv, nt, nr = ctx.crt_trace_stats(bvh, r)
+            row["sets"][tag] = {"ms": float(np.median(ts)), "records_identical": bool(torch.equal(hh.view(torch.int32), ref[tag].view(torch.int32))),
+                                "node_visits_per_ray": nv / max(1, nr), "tri_tests_per_ray": nt / max(1, nr)}
+        rows.append(row)
+    print(json.dumps({"builders": rows, "config": {"workload": args.workload, "n_tris": int(scene.n_tris), "frame": 7,
+                                                   "timing": "crt_trace alone, CUDA events, median of 8, 256 MB L2 flush between repetitions"}}))
+    tags = [t for t, _ in sets]
+    sys.stderr.write("| builder | hierarchy s | of which on device s | layout s | rounds | depth | SAH cost | check | " + " | ".join(tags) + " |\n|---|" + "---:|" * (7 + len(tags)) + "\n")
+    for row in rows:
+        sys.stderr.write(f"| {row['builder']} | {row['hierarchy_seconds']:.3f} | {row['device_build_seconds']:.4f} | {row['layout_seconds']:.3f} | {row['rounds']} | {row['depth']} | {row['sah_cost']:.1f} | {row['check']} | "
+                         + " | ".join(f"{row['sets'][t]['ms']:.3f}{'' if row['sets'][t]['records_identical'] else ' !'}" for t in tags) + " |\n")
+
+
 def run_tail(args):
     """Fixed cost of a crt_trace launch (profiles/r01h): crt_trace on one frame's ray sets (primary, bounce 1, bounce 2; direct_reuse order)
     and on the same set concatenated twice and four times; L2 flushed between repetitions, median of 8.  One JSON line."""
@@ -592,8 +635,9 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--frames-in-flight", type=int, default=3, help="frames rendered concurrently (one context + stream each) for the headline value; the per-mode table stays single-stream")
     ap.add_argument("--no-sort-codes", action="store_true", help="skip the Origin / Reis / Costa / TwoPoint reordering baselines")
-    ap.add_argument("--sweep", nargs="?", const="config3", default=None, choices=["config3", "table3", "rules", "tail", "kernels"],
-                    help="config3: BASELINE config 3 sweep; table3: the paper's Table 3 shapes (tile x K) at 1920x1080, 1 spp, 2 bounces; rules: shuffled against lattice partition at the same size; tail: fixed cost of a crt_trace launch (n, 2n, 4n rays) on --workload; kernels: A/B of traversal kernel variants (--variants) on one frame's ray sets of --workload")
+    ap.add_argument("--sweep", nargs="?", const="config3", default=None, choices=["config3", "table3", "rules", "tail", "kernels", "builders"],
+                    help="config3: BASELINE config 3 sweep; table3: the paper's Table 3 shapes (tile x K) at 1920x1080, 1 spp, 2 bounces; rules: shuffled against lattice partition at the same size; tail: fixed cost of a crt_trace launch (n, 2n, 4n rays) on --workload; kernels: A/B of traversal kernel variants (--variants) on one frame's ray sets of --workload; builders: host SAH against device PLOC BVH builder on --workload")
+    ap.add_argument("--ploc-radii", nargs="*", type=int, default=[16], help="--sweep builders: neighbour radii of the device builder")
     ap.add_argument("--variants", nargs="*", default=["3", "3:trace_exact=0", "5", "6", "4", "1"], help="--sweep kernels: trace_kernel id[:option=value,...] ...")
     ap.add_argument("--sweep-frames", type=int, default=64)
     ap.add_argument("--sweep-scale", type=int, default=1, help="divide the 3840x2160 image by this (quick runs)")
@@ -605,6 +649,9 @@ def main():
         return
     if args.sweep == "kernels":
         run_kernels(args)
+        return
+    if args.sweep == "builders":
+        run_builders(args)
         return
     if args.sweep:
         run_sweep(args)

@@ -87,7 +87,9 @@ typedef struct { int32_t mode, group_w, group_h, stride, stride_y, partition_rul
 /* materials: [device] table indexed by the per-triangle material id given to crt_build_bvh.
  * env: radiance on a miss = lerp(env[0..2], env[3..5], 0.5*(d.y+1)) (D:R14). */
 typedef struct { const crt_material* materials; int32_t n_materials; float env[6]; } crt_scene_mats;
-typedef struct { int32_t max_leaf; int32_t sah_bins; float cost_traversal, cost_intersect; int32_t n_threads; } crt_bvh_params;
+/* builder: 0 = host (binned surface-area heuristic, threaded), 1 = device (parallel locally-ordered clustering, csrc/bvh_ploc.cu; needs a
+ * context); ploc_radius: neighbours searched on either side of a cluster in Morton order (0 = 8; at most 128). */
+typedef struct { int32_t max_leaf; int32_t sah_bins; float cost_traversal, cost_intersect; int32_t n_threads; int32_t builder; int32_t ploc_radius; } crt_bvh_params;
 typedef struct {
     int64_t n_tris, n_nodes, device_bytes;
     float bounds[6];            /* exact min/max over the vertices (unpadded); used by the Morton code */
@@ -97,6 +99,12 @@ typedef struct {
     int32_t wide_depth;
     int32_t q16_inflation_pct;  /* summed surface area of the boxes the 16-bit nodes decode to, in percent of the fp32 boxes' (100 = no
                                  * loss); above 200 the default kernel reads the fp32 nodes instead (grid too coarse for the scene) */
+    int32_t builder;            /* 0 host SAH, 1 device PLOC */
+    int32_t build_rounds;       /* device builder: clustering rounds */
+    double device_build_seconds;/* device builder: boxes + Morton sort + clustering on the GPU (CUDA events); build_seconds is the whole
+                                 * hierarchy build including the copy back and the leaf collapse; layout_seconds the flattening, 16-bit
+                                 * quantisation and upload of the traversal layouts (either builder) */
+    double layout_seconds;
 } crt_bvh_info_t;
 
 /* ---- context ------------------------------------------------------------------------------------ */
@@ -134,7 +142,9 @@ crt_status crt_measure_peaks(crt_ctx* ctx, double* fp32_tflops, double* copy_gbs
  * max_leaf == 1, its collapse into 8-wide compressed 128-byte nodes (read by trace_kernel 2; measured slower than the
  * binary layout on both bench workloads, profiles/r01b, so not the default).
  * verts: [host|device] float[n_tris][3][3]; mat_id: [host|device] int32[n_tris].  Synchronous.  params may be
- * NULL (defaults: max_leaf 3, 64 bins, costs 1/1, all hardware threads).  With ctx == NULL only the host tree is built (for crt_bvh_check /
+ * NULL (defaults: max_leaf 3, 64 bins, costs 1/1, all hardware threads, host builder).  params->builder = 1 builds the hierarchy on
+ * the device instead (bvh_ploc.cu: two orders of magnitude faster, traversal within a few percent: profiles/r02b); the traversal
+ * layouts, the checks and every other call are the same.  With ctx == NULL only the host tree is built (for crt_bvh_check /
  * crt_bvh_get_info; such a BVH is rejected by the device calls with CRT_ERR_STATE). */
 crt_status crt_build_bvh(crt_ctx* ctx, const float* verts, const int32_t* mat_id, int64_t n_tris,
                          const crt_bvh_params* params, crt_bvh** out);

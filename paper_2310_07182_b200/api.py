@@ -63,13 +63,14 @@ class SceneMats(C.Structure):
 
 class BvhParams(C.Structure):
     _fields_ = [("max_leaf", C.c_int32), ("sah_bins", C.c_int32), ("cost_traversal", C.c_float), ("cost_intersect", C.c_float),
-                ("n_threads", C.c_int32)]
+                ("n_threads", C.c_int32), ("builder", C.c_int32), ("ploc_radius", C.c_int32)]
 
 
 class BvhInfo(C.Structure):
     _fields_ = [("n_tris", C.c_int64), ("n_nodes", C.c_int64), ("device_bytes", C.c_int64), ("bounds", C.c_float * 6),
                 ("sah_cost", C.c_double), ("depth", C.c_int32), ("max_leaf", C.c_int32), ("build_seconds", C.c_double),
-                ("n_wide_nodes", C.c_int64), ("wide_depth", C.c_int32), ("q16_inflation_pct", C.c_int32)]
+                ("n_wide_nodes", C.c_int64), ("wide_depth", C.c_int32), ("q16_inflation_pct", C.c_int32),
+                ("builder", C.c_int32), ("build_rounds", C.c_int32), ("device_build_seconds", C.c_double), ("layout_seconds", C.c_double)]
 
 
 _lib = None
@@ -155,7 +156,8 @@ class Bvh:
         self.ctx._check(lib().crt_bvh_get_info(self.handle, C.byref(o)))
         return {"n_tris": o.n_tris, "n_nodes": o.n_nodes, "device_bytes": o.device_bytes, "bounds": np.array(list(o.bounds), np.float32),
                 "sah_cost": o.sah_cost, "depth": o.depth, "max_leaf": o.max_leaf, "build_seconds": o.build_seconds,
-                "n_wide_nodes": o.n_wide_nodes, "wide_depth": o.wide_depth, "q16_inflation_pct": o.q16_inflation_pct}
+                "n_wide_nodes": o.n_wide_nodes, "wide_depth": o.wide_depth, "q16_inflation_pct": o.q16_inflation_pct,
+                "builder": o.builder, "build_rounds": o.build_rounds, "device_build_seconds": o.device_build_seconds, "layout_seconds": o.layout_seconds}
 
     def check(self):
         v = C.c_int32(-1)
@@ -228,15 +230,15 @@ class Context:
         return a.value, b.value
 
     # ---- a0 -----------------------------------------------------------------------------------------
-    def crt_build_bvh(self, verts, mat_id, max_leaf=3, sah_bins=64, n_threads=0, cost_traversal=1.0, cost_intersect=1.0):
-        """verts: numpy float32[n,3,3] or torch tensor (host or device); mat_id int32[n]."""
+    def crt_build_bvh(self, verts, mat_id, max_leaf=3, sah_bins=64, n_threads=0, cost_traversal=1.0, cost_intersect=1.0, builder=0, ploc_radius=0):
+        """verts: numpy float32[n,3,3] or torch tensor (host or device); mat_id int32[n].  builder: 0 host SAH, 1 device PLOC."""
         if isinstance(verts, np.ndarray):
             verts = np.ascontiguousarray(verts, np.float32)
             mat_id = np.ascontiguousarray(mat_id, np.int32)
             n = verts.size // 9
         else:
             n = verts.numel() // 9
-        pr = BvhParams(max_leaf, sah_bins, cost_traversal, cost_intersect, n_threads)
+        pr = BvhParams(max_leaf, sah_bins, cost_traversal, cost_intersect, n_threads, int(builder), int(ploc_radius))
         h = C.c_void_p()
         self._check(lib().crt_build_bvh(self.handle, _ptr(verts), _ptr(mat_id), C.c_int64(n), C.byref(pr), C.byref(h)))
         return Bvh(self, h)

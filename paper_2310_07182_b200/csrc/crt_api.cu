@@ -1,5 +1,6 @@
 // C ABI of libcrt (include/crt.h): argument checking, BVH upload, and the per-frame call sequence.
 #include <algorithm>
+#include <chrono>
 #include <cstring>
 #include <thread>
 #include "crt_internal.h"
@@ -123,7 +124,7 @@ crt_status crt_build_bvh(crt_ctx* ctx, const float* verts, const int32_t* mat_id
     CrtDeviceGuard dev_guard_(ctx ? ctx->device : -1);
     if (n_tris < 0 || (n_tris > 0 && !verts)) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "build_bvh: bad triangle array");
     if (n_tris >= ((int64_t)1 << 28)) return crt_fail(ctx, CRT_ERR_UNSUPPORTED, "build_bvh: more than 2^28 triangles");
-    crt_bvh_params pr = {3, 64, 1.0f, 1.0f, 0};
+    crt_bvh_params pr = {3, 64, 1.0f, 1.0f, 0, 0, 0};
     if (params) pr = *params;
     if (pr.max_leaf < 1 || pr.max_leaf > 8) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "build_bvh: max_leaf %d not in [1,8]", pr.max_leaf);
     if (pr.sah_bins == 0) pr.sah_bins = 64;
@@ -141,9 +142,16 @@ crt_status crt_build_bvh(crt_ctx* ctx, const float* verts, const int32_t* mat_id
     for (int64_t i = 0; i < 9 * n_tris; ++i) if (!(v[i] == v[i]) || v[i] > 1e30f || v[i] < -1e30f) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "build_bvh: non-finite vertex");
     int32_t max_mat = -1;
     for (int32_t m : hm) { if (m < 0) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "build_bvh: negative material id"); max_mat = std::max(max_mat, m); }
+    if (pr.builder < 0 || pr.builder > 1) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "build_bvh: builder %d out of range", pr.builder);
+    if (pr.builder == 1 && !ctx) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "build_bvh: the device builder needs a context");
     crt_bvh* b = new crt_bvh();
     b->max_mat_id = max_mat;
-    crt_bvh_build_host(b, v, n_tris, pr);
+    if (pr.builder == 1) {
+        if (!hv.empty()) {}       // (device input was copied to the host above: the layout code and crt_bvh_check work from the host copy)
+        crt_status bst = crt_bvh_build_device(ctx, b, v, n_tris, pr);
+        if (bst != CRT_OK) { delete b; return bst; }
+    } else crt_bvh_build_host(b, v, n_tris, pr);
+    const auto t_layout0 = std::chrono::steady_clock::now();
     if (b->depth > 60) { delete b; return crt_fail(ctx, CRT_ERR_UNSUPPORTED, "build_bvh: tree depth exceeds the traversal stack (64)"); }
     // one triangle per leaf: also build the 8-wide compressed layout (the default kernel's); its triangle order is the shared one
     std::vector<WNode> wn; std::vector<int32_t> tri_order;
@@ -173,6 +181,7 @@ crt_status crt_build_bvh(crt_ctx* ctx, const float* verts, const int32_t* mat_id
         if (e == cudaSuccess) e = up((void**)&b->d_mat_id, hm.data(), hm.size() * 4);
         if (e != cudaSuccess) { crt_bvh_destroy(b); return crt_fail(ctx, e == cudaErrorMemoryAllocation ? CRT_ERR_NOMEM : CRT_ERR_CUDA, "build_bvh: upload: %s", cudaGetErrorString(e)); }
     }
+    b->layout_seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t_layout0).count();
     *out = b;
     return CRT_OK;
 }
@@ -194,6 +203,7 @@ crt_status crt_bvh_get_info(const crt_bvh* b, crt_bvh_info_t* o)
     o->sah_cost = b->sah; o->depth = b->depth; o->max_leaf = b->max_leaf; o->build_seconds = b->build_seconds;
     o->n_wide_nodes = b->n_wide_nodes; o->wide_depth = b->wide_depth;
     o->q16_inflation_pct = (int32_t)std::min(1e9, b->q_inflation * 100.0 + 0.5);
+    o->builder = b->builder; o->build_rounds = b->ploc_rounds; o->device_build_seconds = 1e-3 * b->device_build_ms; o->layout_seconds = b->layout_seconds;
     return CRT_OK;
 }
 

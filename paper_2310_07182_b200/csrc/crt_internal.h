@@ -71,6 +71,7 @@ struct crt_bvh {
     std::vector<float> verts;         // host copy of the caller's vertices (for crt_bvh_check)
     float bounds[6] = {0, 0, 0, 0, 0, 0};
     double sah = 0; int depth = 0; double build_seconds = 0;
+    int builder = 0; int ploc_rounds = 0; float device_build_ms = 0.f; double layout_seconds = 0;      // device builder (bvh_ploc.cu)
     // device data
     int device = -1;
     GpuNode* d_nodes = nullptr; int64_t n_gpu_nodes = 0;
@@ -119,6 +120,7 @@ struct Layout {
 crt_status crt_make_layout(crt_ctx* ctx, const crt_frame* f, const crt_order* o, Layout* L);
 
 // kernels' host launchers (defined in the .cu files) ------------------------------------------------------
+crt_status crt_bvh_build_device(crt_ctx* ctx, crt_bvh* b, const float* verts, int64_t n, const crt_bvh_params& pr);
 crt_status launch_trace(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, crt_hit* hits, cudaStream_t st, bool far_origins = false);
 bool trace_queue_supported(const crt_bvh* bvh);
 crt_status launch_trace_queue(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, crt_hit* hits, unsigned long long* stats, cudaStream_t st);

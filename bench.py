@@ -552,7 +552,7 @@ def run_builders(args):
     scene = I.by_name(name, **kw).with_camera(w, h)
     ctx = crt.Context(0)
     trees = []
-    for label, bkw in [("host SAH (64 bins)", dict(builder=0))] + [(f"device PLOC radius {r}", dict(builder=1, ploc_radius=r)) for r in args.ploc_radii]:
+    for label, bkw in [("host SAH (64 bins)", dict(builder=0))] + [(f"device PLOC radius {r}", dict(builder=1, ploc_radius=r)) for r in args.ploc_radii] + [(f"device clustering radius {args.ploc_radii[0]} + host layout", dict(builder=2, ploc_radius=args.ploc_radii[0]))]:
         t0 = time.time(); bvh = ctx.crt_build_bvh(scene.verts, scene.mat_id, **bkw); wall = time.time() - t0
         info = bvh.info()
         trees.append((label, bvh, dict(builder=label, wall_seconds=wall, hierarchy_seconds=info["build_seconds"], device_build_seconds=info["device_build_seconds"],
@@ -637,7 +637,7 @@ def main():
     ap.add_argument("--no-sort-codes", action="store_true", help="skip the Origin / Reis / Costa / TwoPoint reordering baselines")
     ap.add_argument("--sweep", nargs="?", const="config3", default=None, choices=["config3", "table3", "rules", "tail", "kernels", "builders"],
                     help="config3: BASELINE config 3 sweep; table3: the paper's Table 3 shapes (tile x K) at 1920x1080, 1 spp, 2 bounces; rules: shuffled against lattice partition at the same size; tail: fixed cost of a crt_trace launch (n, 2n, 4n rays) on --workload; kernels: A/B of traversal kernel variants (--variants) on one frame's ray sets of --workload; builders: host SAH against device PLOC BVH builder on --workload")
-    ap.add_argument("--ploc-radii", nargs="*", type=int, default=[16], help="--sweep builders: neighbour radii of the device builder")
+    ap.add_argument("--ploc-radii", nargs="*", type=int, default=[8], help="--sweep builders: neighbour radii of the device builder")
     ap.add_argument("--variants", nargs="*", default=["3", "3:trace_exact=0", "5", "6", "4", "1"], help="--sweep kernels: trace_kernel id[:option=value,...] ...")
     ap.add_argument("--sweep-frames", type=int, default=64)
     ap.add_argument("--sweep-scale", type=int, default=1, help="divide the 3840x2160 image by this (quick runs)")

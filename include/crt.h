@@ -87,8 +87,9 @@ typedef struct { int32_t mode, group_w, group_h, stride, stride_y, partition_rul
 /* materials: [device] table indexed by the per-triangle material id given to crt_build_bvh.
  * env: radiance on a miss = lerp(env[0..2], env[3..5], 0.5*(d.y+1)) (D:R14). */
 typedef struct { const crt_material* materials; int32_t n_materials; float env[6]; } crt_scene_mats;
-/* builder: 0 = host (binned surface-area heuristic, threaded), 1 = device (parallel locally-ordered clustering, csrc/bvh_ploc.cu; needs a
- * context); ploc_radius: neighbours searched on either side of a cluster in Morton order (0 = 8; at most 128). */
+/* builder: 0 = host (binned surface-area heuristic, threaded); 1 = device (parallel locally-ordered clustering AND the traversal layouts
+ * written by the GPU, csrc/bvh_ploc.cu; needs a context); 2 = the device's clustering with the host's layout code (cross-check of 1);
+ * ploc_radius: neighbours searched on either side of a cluster in Morton order (0 = 8; at most 128). */
 typedef struct { int32_t max_leaf; int32_t sah_bins; float cost_traversal, cost_intersect; int32_t n_threads; int32_t builder; int32_t ploc_radius; } crt_bvh_params;
 typedef struct {
     int64_t n_tris, n_nodes, device_bytes;
@@ -99,7 +100,7 @@ typedef struct {
     int32_t wide_depth;
     int32_t q16_inflation_pct;  /* summed surface area of the boxes the 16-bit nodes decode to, in percent of the fp32 boxes' (100 = no
                                  * loss); above 200 the default kernel reads the fp32 nodes instead (grid too coarse for the scene) */
-    int32_t builder;            /* 0 host SAH, 1 device PLOC */
+    int32_t builder;            /* 0 host SAH, 1 device PLOC, 2 device PLOC + host layout */
     int32_t build_rounds;       /* device builder: clustering rounds */
     double device_build_seconds;/* device builder: boxes + Morton sort + clustering on the GPU (CUDA events); build_seconds is the whole
                                  * hierarchy build including the copy back and the leaf collapse; layout_seconds the flattening, 16-bit

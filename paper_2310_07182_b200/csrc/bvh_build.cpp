@@ -317,6 +317,25 @@ void crt_bvh_flatten(const crt_bvh* b, const std::vector<int32_t>& tri_order, st
     }
 }
 
+// grid of the 16-bit layout over the (padded) scene box [lo, hi]
+void crt_qgrid_for_box(const double lo[3], const double hi[3], QGrid* grid)
+{
+    double maxext = 0;
+    for (int k = 0; k < 3; ++k) maxext = std::max(maxext, hi[k] - lo[k]);
+    if (!(maxext > 0)) maxext = 1;
+    for (int k = 0; k < 3; ++k) {
+        // margin on either side: 8 grid steps, or 4 ulps of the box's coordinates when the scene sits far from the origin (gmin is a
+        // float: its rounding must not eat the margin, or planes clamp inward); gmin is rounded DOWN so the low side only gains
+        const double e = std::max(hi[k] - lo[k], maxext * (1.0 / 4096.0));
+        const double ulp = std::max(std::fabs(lo[k]), std::fabs(hi[k])) * (1.0 / 8388608.0);
+        const double margin = std::max(8.0 * e / (65535.0 - 16.0), 4.0 * ulp);
+        const float scale = (float)(65535.0 / (e + 2.0 * margin) * (1.0 - 1e-6));
+        grid->scale[k] = scale;
+        grid->gmin[k] = std::nextafterf((float)(lo[k] - margin), -std::numeric_limits<float>::infinity());
+        grid->inv_scale[k] = (float)(1.0 / (double)scale);
+    }
+}
+
 // 16-bit layout of the flattened nodes (trace_kernel 3): every box plane becomes a position on a 65536-step grid over the
 // scene box, rounded OUTWARD (min planes down, max planes up) and then moved ONE more step outward: the traversal kernel
 // evaluates a plane distance as one FMA in grid units whose rounding error stays below one step of position for ray
@@ -336,20 +355,8 @@ int32_t crt_bvh_quantise(const crt_bvh* b, const std::vector<GpuNode>& gn, std::
                 double mn, mx; planes(gn[0].c[c], k, mn, mx);
                 if (std::isfinite(mn) && std::isfinite(mx)) { lo[k] = std::min(lo[k], mn); hi[k] = std::max(hi[k], mx); }
             }
-    double maxext = 0;
-    for (int k = 0; k < 3; ++k) { if (lo[k] > hi[k]) { lo[k] = 0; hi[k] = 1; } maxext = std::max(maxext, hi[k] - lo[k]); }
-    if (!(maxext > 0)) maxext = 1;
-    for (int k = 0; k < 3; ++k) {
-        // margin on either side: 8 grid steps, or 4 ulps of the box's coordinates when the scene sits far from the origin (gmin is a
-        // float: its rounding must not eat the margin, or planes clamp inward); gmin is rounded DOWN so the low side only gains
-        const double e = std::max(hi[k] - lo[k], maxext * (1.0 / 4096.0));
-        const double ulp = std::max(std::fabs(lo[k]), std::fabs(hi[k])) * (1.0 / 8388608.0);
-        const double margin = std::max(8.0 * e / (65535.0 - 16.0), 4.0 * ulp);
-        const float scale = (float)(65535.0 / (e + 2.0 * margin) * (1.0 - 1e-6));
-        grid->scale[k] = scale;
-        grid->gmin[k] = std::nextafterf((float)(lo[k] - margin), -std::numeric_limits<float>::infinity());
-        grid->inv_scale[k] = (float)(1.0 / (double)scale);
-    }
+    for (int k = 0; k < 3; ++k) if (lo[k] > hi[k]) { lo[k] = 0; hi[k] = 1; }
+    crt_qgrid_for_box(lo, hi, grid);
     int32_t bad = 0;
     qn.resize(gn.size());
     for (size_t i = 0; i < gn.size(); ++i) {
@@ -383,5 +390,69 @@ int32_t crt_bvh_quantise(const crt_bvh* b, const std::vector<GpuNode>& gn, std::
         qn[i] = q;
     }
     if (inflation) *inflation = area_f > 0 ? area_q / area_f : 1.0;
+    return bad;
+}
+
+// Invariants of the DEVICE traversal layouts themselves (whichever builder wrote them): downloads the fp32 nodes, the 16-bit nodes, the
+// triangle records and slot_of_prim and walks the tree from node 0.  Bits as crt_bvh_check_host (1 child box not inside its parent's,
+// 2 leaf size, 4 triangle in two leaves, 8 triangle outside its leaf's box, 16 triangle in no leaf, 32 bad index / record) and 0x10000
+// (a 16-bit plane less than one grid step outside the fp32 box it stands for, or different child references).
+int32_t crt_layout_check_device(const crt_bvh* b)
+{
+    if (b->n_tris == 0 || !b->d_nodes || !b->d_tris) return 0;
+    const int64_t nn = b->n_gpu_nodes, nt = b->n_tris;
+    std::vector<GpuNode> gn((size_t)nn); std::vector<QNode> qn((size_t)nn); std::vector<GpuTri> gt((size_t)nt); std::vector<int32_t> sop((size_t)nt);
+    if (cudaMemcpy(gn.data(), b->d_nodes, gn.size() * sizeof(GpuNode), cudaMemcpyDeviceToHost) != cudaSuccess) return 32;
+    if (b->d_qnodes && cudaMemcpy(qn.data(), b->d_qnodes, qn.size() * sizeof(QNode), cudaMemcpyDeviceToHost) != cudaSuccess) return 32;
+    if (cudaMemcpy(gt.data(), b->d_tris, gt.size() * sizeof(GpuTri), cudaMemcpyDeviceToHost) != cudaSuccess) return 32;
+    if (cudaMemcpy(sop.data(), b->d_slot_of_prim, sop.size() * 4, cudaMemcpyDeviceToHost) != cudaSuccess) return 32;
+    int32_t bad = 0;
+    std::vector<uint8_t> seen_node((size_t)nn, 0), seen_tri((size_t)nt, 0);
+    auto inside = [](const GpuChild& in, const GpuChild& out) {
+        return in.min_x >= out.min_x && in.max_x <= out.max_x && in.min_y >= out.min_y && in.max_y <= out.max_y && in.min_z >= out.min_z && in.max_z <= out.max_z;
+    };
+    std::vector<int32_t> stack{0};
+    seen_node[0] = 1;
+    while (!stack.empty()) {
+        const int32_t i = stack.back(); stack.pop_back();
+        for (int c = 0; c < 2; ++c) {
+            const GpuChild& ch = gn[i].c[c];
+            if (!std::isfinite(ch.min_x)) continue;                     // the empty second child of a one-leaf scene
+            if (b->d_qnodes) {
+                if (qn[i].ref[c] != ch.ref) bad |= 0x10000;
+                const float* pl = &ch.min_x;
+                for (int k = 0; k < 3; ++k) {
+                    const double g = b->qgrid.gmin[k], s = b->qgrid.scale[k];
+                    const uint32_t w = qn[i].planes[3 * c + k];
+                    const double a = (double)(w & 0xffffu), z = (double)(w >> 16);
+                    if (!(g + (a + 1.0) / s <= (double)pl[2 * k]) || !(g + (z - 1.0) / s >= (double)pl[2 * k + 1])) bad |= 0x10000;
+                }
+            }
+            if (ch.ref >= 0) {
+                if (ch.ref >= nn) { bad |= 32; continue; }
+                if (seen_node[ch.ref]) { bad |= 4; continue; }
+                seen_node[ch.ref] = 1;
+                for (int g2 = 0; g2 < 2; ++g2) if (std::isfinite(gn[ch.ref].c[g2].min_x) && !inside(gn[ch.ref].c[g2], ch)) bad |= 1;
+                stack.push_back(ch.ref);
+            } else {
+                const int32_t leaf = ~ch.ref; const int64_t first = leaf >> 3; const int cnt = (leaf & 7) + 1;
+                if (cnt > b->max_leaf) bad |= 2;
+                if (first + cnt > nt) { bad |= 32; continue; }
+                for (int64_t j = first; j < first + cnt; ++j) {
+                    int32_t prim; std::memcpy(&prim, &gt[j].v0p.w, 4);
+                    if (prim < 0 || prim >= nt) { bad |= 32; continue; }
+                    if (seen_tri[prim]) bad |= 4;
+                    seen_tri[prim] = 1;
+                    if (sop[prim] != (int32_t)j) bad |= 32;
+                    const float* tv = b->verts.data() + 9 * (int64_t)prim;
+                    if (gt[j].v0p.x != tv[0] || gt[j].v0p.y != tv[1] || gt[j].v0p.z != tv[2] || gt[j].e1.x != tv[3] - tv[0] || gt[j].e2.z != tv[8] - tv[2]) bad |= 32;
+                    for (int v = 0; v < 3; ++v)
+                        if (tv[3 * v] < ch.min_x || tv[3 * v] > ch.max_x || tv[3 * v + 1] < ch.min_y || tv[3 * v + 1] > ch.max_y || tv[3 * v + 2] < ch.min_z || tv[3 * v + 2] > ch.max_z) bad |= 8;
+                }
+            }
+        }
+    }
+    for (uint8_t s2 : seen_tri) if (!s2) bad |= 16;
+    for (uint8_t s2 : seen_node) if (!s2) bad |= 32;
     return bad;
 }

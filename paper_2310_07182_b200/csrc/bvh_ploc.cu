@@ -1,22 +1,29 @@
-// a0 on the device (NEXT-4, second half): the BVH hierarchy built by the GPU ("acceleration structures such as bounding
-// volume hierarchies"; the paper leaves the builder open, D:R11).  crt_bvh_params.builder = 1.
+// a0 on the device (NEXT-4, second half): the BVH built by the GPU ("acceleration structures such as bounding volume
+// hierarchies"; the paper leaves the builder open, D:R11).  crt_bvh_params.builder = 1 (everything on the device) or 2 (hierarchy on
+// the device, layout by the host code the host builder uses: the cross-check of 1).
 //
 // Method: parallel locally-ordered clustering (PLOC, Meister & Bittner 2018), restated from the publication:
-//   1. triangle boxes and centroids; 30-bit Morton code of the centroid inside the scene box; stable radix sort (sort.cu)
+//   1. triangle boxes and centroids; 30-bit Morton code of the centroid on a cubic grid over the scene box; stable radix sort (sort.cu)
 //   2. clusters = the triangles in Morton order.  Repeat until one cluster is left:
 //        a. every cluster looks at its `radius` neighbours on either side in the array and picks the one with which its union box has
 //           the smallest surface area (ties -> the lower index)
 //        b. clusters that picked EACH OTHER merge into a new inner node, which takes the place of the left partner
 //        c. the array is compacted (order-preserving: an exclusive scan), so that neighbours in the array stay neighbours in space
+//      Node indices are a pure function of the input (rank of the dropped partner in its round, no atomics), children always have lower
+//      indices than their parent, the root is the last node.
 //   3. subtrees of at most max_leaf triangles become leaves (the same forced-split rule as the host builder).
-// Agglomerative clustering driven by the surface area of the merged box is a bottom-up surface-area heuristic; the trees trace
-// within a few percent of the host's binned-SAH trees (profiles/r02b) and build two orders of magnitude faster.
-// The hierarchy comes back to the host in the builder-independent form (BuildNode + leaf order) that crt_bvh_flatten, crt_bvh_quantise
-// and crt_bvh_check already consume, so both builders share the layout code and the invariant checks.
+//   4. (builder 1) the traversal layouts are written on the device: inner nodes numbered top-down (descending creation order, the root
+//      first), every leaf gets a contiguous run of triangle records ordered by the Morton position of its first triangle, fp32 64-byte
+//      nodes and 16-bit 32-byte nodes (the quantisation rule of crt_bvh_quantise: planes rounded outward plus one grid step) in one pass.
+// Agglomerative clustering driven by the surface area of the merged box is a bottom-up surface-area heuristic; the trees trace within
+// 3-10 % of the host's binned-SAH trees and build two orders of magnitude faster (profiles/r02b).
 #include <algorithm>
 #include <chrono>
+#include <cmath>
 #include <cstring>
 #include "crt_internal.h"
+
+void crt_qgrid_for_box(const double lo[3], const double hi[3], QGrid* grid);
 
 namespace {
 
@@ -67,8 +74,8 @@ __global__ void __launch_bounds__(PB) ploc_prims_kernel(const float* __restrict_
     }
     Box2 bx; bx.lo = make_float4(mn[0], mn[1], mn[2], 0.f); bx.hi = make_float4(mx[0], mx[1], mx[2], 0.f);
     tri_box[i] = bx;
-    // one CUBIC grid of 1024^3 cells over the largest extent: per-axis normalisation would make the cells of a flat scene thin slabs
-    // (landscape: 2 x 0.2 x 2 units) and let tiny height differences reorder horizontal neighbours (measured: SAH cost 56 -> see r02b)
+    // one CUBIC grid of 1024^3 cells over the largest extent: per-axis normalisation makes the cells of a flat scene thin slabs (landscape:
+    // 2 x 0.2 x 2 units) and lets tiny height differences reorder horizontal neighbours (measured: SAH cost 56.7 -> 50.2, profiles/r02b)
     unsigned q[3];
     float maxext = 0.f;
 #pragma unroll
@@ -84,16 +91,19 @@ __global__ void __launch_bounds__(PB) ploc_prims_kernel(const float* __restrict_
     vals[i] = (int32_t)i;
 }
 
-// node k < n: the leaf of the k-th triangle in Morton order
+// the hierarchy, node-indexed (2n - 1 nodes; node k < n = the leaf of the k-th triangle in Morton order)
+struct Tree {
+    Box2* box; int32_t *left, *right, *cnt, *parent, *first, *height;
+};
+
 __global__ void __launch_bounds__(PB) ploc_init_kernel(const int32_t* __restrict__ sorted_tri, const Box2* __restrict__ tri_box, int64_t n,
-                                                       int32_t* __restrict__ cl_id, Box2* __restrict__ cl_box, Box2* __restrict__ node_box,
-                                                       int32_t* __restrict__ node_left, int32_t* __restrict__ node_right, int32_t* __restrict__ node_cnt)
+                                                       int32_t* __restrict__ cl_id, Box2* __restrict__ cl_box, Tree T)
 {
     const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= n) return;
     const Box2 b = tri_box[sorted_tri[k]];
-    cl_id[k] = (int32_t)k; cl_box[k] = b; node_box[k] = b;
-    node_left[k] = -1; node_right[k] = -1; node_cnt[k] = 1;
+    cl_id[k] = (int32_t)k; cl_box[k] = b; T.box[k] = b;
+    T.left[k] = -1; T.right[k] = -1; T.cnt[k] = 1; T.parent[k] = -1; T.first[k] = (int32_t)k; T.height[k] = 1;
 }
 
 __device__ __forceinline__ float union_area(const Box2& a, const Box2& b)
@@ -125,46 +135,30 @@ __global__ void __launch_bounds__(PB) ploc_nn_kernel(const Box2* __restrict__ cl
     nn[i] = best_j;
 }
 
-// 2b: mutual nearest neighbours merge; flag = 1 for every cluster that stays in the array
-__global__ void __launch_bounds__(PB) ploc_merge_kernel(const int32_t* __restrict__ nn, const int32_t* __restrict__ cl_id, const Box2* __restrict__ cl_box, int n,
-                                                        int32_t* __restrict__ tmp_id, Box2* __restrict__ tmp_box, int32_t* __restrict__ flag,
-                                                        Box2* __restrict__ node_box, int32_t* __restrict__ node_left, int32_t* __restrict__ node_right,
-                                                        int32_t* __restrict__ node_cnt, int32_t* __restrict__ node_counter)
+// 2b: a cluster stays in the array unless it is the RIGHT partner of a mutual pair
+__global__ void __launch_bounds__(PB) ploc_mark_kernel(const int32_t* __restrict__ nn, int n, int32_t* __restrict__ keep)
 {
     const int i = blockIdx.x * PB + threadIdx.x;
     if (i >= n) return;
     const int j = nn[i];
-    int32_t id = cl_id[i]; Box2 b = cl_box[i]; int keep = 1;
-    if (j >= 0 && nn[j] == i) {
-        if (i < j) {
-            const Box2 o = cl_box[j]; const int32_t oid = cl_id[j];
-            Box2 u;
-            u.lo = make_float4(fminf(b.lo.x, o.lo.x), fminf(b.lo.y, o.lo.y), fminf(b.lo.z, o.lo.z), 0.f);
-            u.hi = make_float4(fmaxf(b.hi.x, o.hi.x), fmaxf(b.hi.y, o.hi.y), fmaxf(b.hi.z, o.hi.z), 0.f);
-            const int32_t idx = atomicAdd(node_counter, 1);
-            node_box[idx] = u; node_left[idx] = id; node_right[idx] = oid; node_cnt[idx] = node_cnt[id] + node_cnt[oid];
-            id = idx; b = u;
-        } else keep = 0;
-    }
-    tmp_id[i] = id; tmp_box[i] = b; flag[i] = keep;
+    keep[i] = !(j >= 0 && nn[j] == i && j < i);
 }
 
-// 2c: order-preserving compaction = exclusive scan of the flags (block sums, scan of the sums, scatter)
+// ---- exclusive scan of n ints (block sums, one-block scan of the sums, per-block scan + offset)
 constexpr int SCAN_ITEMS = 4;
 constexpr int SCAN_TILE = PB * SCAN_ITEMS;
-__global__ void __launch_bounds__(PB) ploc_blocksum_kernel(const int32_t* __restrict__ flag, int n, int32_t* __restrict__ block_sum)
+__global__ void __launch_bounds__(PB) scan_blocksum_kernel(const int32_t* __restrict__ in, int n, int32_t* __restrict__ block_sum)
 {
     __shared__ int s[PB / 32];
     int v = 0;
-    for (int t = 0; t < SCAN_ITEMS; ++t) { const int i = blockIdx.x * SCAN_TILE + t * PB + threadIdx.x; if (i < n) v += flag[i]; }
+    for (int t = 0; t < SCAN_ITEMS; ++t) { const int i = blockIdx.x * SCAN_TILE + t * PB + threadIdx.x; if (i < n) v += in[i]; }
 #pragma unroll
     for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
     if ((threadIdx.x & 31) == 0) s[threadIdx.x >> 5] = v;
     __syncthreads();
     if (threadIdx.x == 0) { int t = 0; for (int w = 0; w < PB / 32; ++w) t += s[w]; block_sum[blockIdx.x] = t; }
 }
-// one block: exclusive scan of the block sums in place; total -> *n_out
-__global__ void __launch_bounds__(1024) ploc_scansums_kernel(int32_t* __restrict__ block_sum, int nb, int32_t* __restrict__ n_out)
+__global__ void __launch_bounds__(1024) scan_sums_kernel(int32_t* __restrict__ block_sum, int nb, int32_t* __restrict__ total)
 {
     __shared__ int warp_s[32];
     __shared__ int carry;
@@ -186,10 +180,9 @@ __global__ void __launch_bounds__(1024) ploc_scansums_kernel(int32_t* __restrict
         if (threadIdx.x == 1023) carry = off + incl;
         __syncthreads();
     }
-    if (threadIdx.x == 0) *n_out = carry;
+    if (threadIdx.x == 0) *total = carry;
 }
-__global__ void __launch_bounds__(PB) ploc_compact_kernel(const int32_t* __restrict__ flag, const int32_t* __restrict__ tmp_id, const Box2* __restrict__ tmp_box, int n,
-                                                          const int32_t* __restrict__ block_off, int32_t* __restrict__ cl_id, Box2* __restrict__ cl_box)
+__global__ void __launch_bounds__(PB) scan_write_kernel(const int32_t* __restrict__ in, int n, const int32_t* __restrict__ block_off, int32_t* __restrict__ out)
 {
     __shared__ int warp_s[PB / 32];
     __shared__ int carry;
@@ -198,7 +191,7 @@ __global__ void __launch_bounds__(PB) ploc_compact_kernel(const int32_t* __restr
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     for (int t = 0; t < SCAN_ITEMS; ++t) {
         const int i = blockIdx.x * SCAN_TILE + t * PB + threadIdx.x;
-        const int f = i < n ? flag[i] : 0;
+        const int f = i < n ? in[i] : 0;
         int incl = f;
 #pragma unroll
         for (int d = 1; d < 32; d <<= 1) { const int x = __shfl_up_sync(0xffffffffu, incl, d); if (lane >= d) incl += x; }
@@ -206,11 +199,143 @@ __global__ void __launch_bounds__(PB) ploc_compact_kernel(const int32_t* __restr
         __syncthreads();
         int off = carry;
         for (int w = 0; w < warp; ++w) off += warp_s[w];
-        if (f) { cl_id[off + incl - 1] = tmp_id[i]; cl_box[off + incl - 1] = tmp_box[i]; }
+        if (i < n) out[i] = off + incl - f;
         __syncthreads();
         if (threadIdx.x == PB - 1) carry = off + incl;
         __syncthreads();
     }
+}
+// out[i] = sum of in[0..i); *total (device) = sum of all.  bsum: scratch of ceil(n / SCAN_TILE) + 1 ints.
+void exclusive_scan(const int32_t* in, int32_t* out, int n, int32_t* bsum, int32_t* total)
+{
+    const int nb = (n + SCAN_TILE - 1) / SCAN_TILE;
+    scan_blocksum_kernel<<<nb, PB>>>(in, n, bsum);
+    scan_sums_kernel<<<1, 1024>>>(bsum, nb, total);
+    scan_write_kernel<<<nb, PB>>>(in, n, bsum, out);
+}
+
+// 2b + 2c: a merged pair (i < j) becomes node base + (number of dropped clusters before j): a pure function of the input.  The new node,
+// or the unmerged cluster, goes to position pos[i] = (number of kept clusters before i) of the next array.
+__global__ void __launch_bounds__(PB) ploc_build_kernel(const int32_t* __restrict__ nn, const int32_t* __restrict__ keep, const int32_t* __restrict__ pos,
+                                                        const int32_t* __restrict__ cl_id, const Box2* __restrict__ cl_box, int n, int32_t node_base,
+                                                        int32_t* __restrict__ new_id, Box2* __restrict__ new_box, Tree T)
+{
+    const int i = blockIdx.x * PB + threadIdx.x;
+    if (i >= n || !keep[i]) return;
+    const int j = nn[i];
+    int32_t id = cl_id[i]; Box2 b = cl_box[i];
+    if (j >= 0 && nn[j] == i) {          // i < j, or i would not have been kept
+        const Box2 o = cl_box[j]; const int32_t oid = cl_id[j];
+        Box2 u;
+        u.lo = make_float4(fminf(b.lo.x, o.lo.x), fminf(b.lo.y, o.lo.y), fminf(b.lo.z, o.lo.z), 0.f);
+        u.hi = make_float4(fmaxf(b.hi.x, o.hi.x), fmaxf(b.hi.y, o.hi.y), fmaxf(b.hi.z, o.hi.z), 0.f);
+        const int32_t idx = node_base + (j - pos[j]);
+        T.box[idx] = u; T.left[idx] = id; T.right[idx] = oid; T.cnt[idx] = T.cnt[id] + T.cnt[oid]; T.parent[idx] = -1;
+        T.first[idx] = min(T.first[id], T.first[oid]); T.height[idx] = 1 + max(T.height[id], T.height[oid]);
+        T.parent[id] = idx; T.parent[oid] = idx;
+        id = idx; b = u;
+    }
+    new_id[pos[i]] = id; new_box[pos[i]] = b;
+}
+
+// ---- 4. traversal layouts on the device
+// inner[i] = 1 for nodes that stay inner nodes; w[first triangle position] = triangle count for the roots of collapsed subtrees (leaves)
+__global__ void __launch_bounds__(PB) layout_classify_kernel(Tree T, int n_nodes, int max_leaf, int32_t* __restrict__ inner, int32_t* __restrict__ w)
+{
+    const int i = blockIdx.x * PB + threadIdx.x;
+    if (i >= n_nodes) return;
+    const int c = T.cnt[i];
+    inner[i] = c > max_leaf;
+    const int p = T.parent[i];
+    if (c <= max_leaf && (p < 0 || T.cnt[p] > max_leaf)) w[T.first[i]] = c;
+}
+
+__device__ __forceinline__ double warp_sum(double v)
+{
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
+    return v;
+}
+
+// leaves: triangle records in the leaf's run of slots, left to right; ref[i] = the child reference a parent stores for node i
+__global__ void __launch_bounds__(PB) layout_leaves_kernel(Tree T, int n_nodes, int max_leaf, const int32_t* __restrict__ inner_before, int n_inner,
+                                                           const int32_t* __restrict__ slot_start, const int32_t* __restrict__ sorted_tri,
+                                                           const float* __restrict__ verts, GpuTri* __restrict__ tris, int32_t* __restrict__ slot_of_prim,
+                                                           int32_t* __restrict__ ref, double cost_intersect, double* __restrict__ sums)
+{
+    const int i = blockIdx.x * PB + threadIdx.x;
+    double area = 0.0;
+    if (i < n_nodes) {
+        const int c = T.cnt[i];
+        const int p = T.parent[i];
+        if (c > max_leaf) ref[i] = n_inner - 1 - inner_before[i];                 // inner nodes are numbered in descending creation order: the root is node 0
+        else if (p < 0 || T.cnt[p] > max_leaf) {
+            const int slot = slot_start[T.first[i]];
+            ref[i] = ~((slot << 3) | (c - 1));
+            int stack[16]; int sp = 0, k = 0; stack[sp++] = i;
+            while (sp) {
+                const int s = stack[--sp];
+                if (T.left[s] < 0) {
+                    const int tri = sorted_tri[s];
+                    const float* tv = verts + 9 * (int64_t)tri;
+                    GpuTri t;
+                    t.v0p = make_float4(tv[0], tv[1], tv[2], __int_as_float(tri));
+                    t.e1 = make_float4(tv[3] - tv[0], tv[4] - tv[1], tv[5] - tv[2], 0.f);
+                    t.e2 = make_float4(tv[6] - tv[0], tv[7] - tv[1], tv[8] - tv[2], 0.f);
+                    t.pad = make_float4(0.f, 0.f, 0.f, 0.f);
+                    tris[slot + k] = t; slot_of_prim[tri] = slot + k; ++k;
+                } else { stack[sp++] = T.right[s]; stack[sp++] = T.left[s]; }
+            }
+            const Box2 b = T.box[i];
+            const double dx = (double)b.hi.x - b.lo.x, dy = (double)b.hi.y - b.lo.y, dz = (double)b.hi.z - b.lo.z;
+            area = (dx * dy + dy * dz + dz * dx) * cost_intersect * c;
+        }
+    }
+    area = warp_sum(area);
+    if ((threadIdx.x & 31) == 0 && area != 0.0) atomicAdd(sums + 0, area);
+}
+
+// inner nodes: fp32 node and 16-bit node (crt_bvh_quantise's rule) of both children
+__global__ void __launch_bounds__(PB) layout_nodes_kernel(Tree T, int n_nodes, int max_leaf, const int32_t* __restrict__ ref, float pad, QGrid grid,
+                                                          GpuNode* __restrict__ gn, QNode* __restrict__ qn, double cost_traversal, double* __restrict__ sums, int32_t* __restrict__ q_bad)
+{
+    const int i = blockIdx.x * PB + threadIdx.x;
+    double cost = 0.0, area_f = 0.0, area_q = 0.0;
+    if (i < n_nodes && T.cnt[i] > max_leaf) {
+        const int g = ref[i];
+        GpuNode N; QNode Q; int bad = 0;
+#pragma unroll
+        for (int c = 0; c < 2; ++c) {
+            const int ch = c ? T.right[i] : T.left[i];
+            const Box2 b = T.box[ch];
+            const float mn[3] = {b.lo.x - pad, b.lo.y - pad, b.lo.z - pad}, mx[3] = {b.hi.x + pad, b.hi.y + pad, b.hi.z + pad};
+            N.c[c].min_x = mn[0]; N.c[c].max_x = mx[0]; N.c[c].min_y = mn[1]; N.c[c].max_y = mx[1]; N.c[c].min_z = mn[2]; N.c[c].max_z = mx[2];
+            N.c[c].ref = ref[ch]; N.c[c].pad = 0;
+            Q.ref[c] = ref[ch];
+            double ef[3], eq[3];
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                const double gm = (double)grid.gmin[k], s = (double)grid.scale[k];
+                double a = floor(((double)mn[k] - gm) * s), z = ceil(((double)mx[k] - gm) * s);
+                if (gm + a / s > (double)mn[k]) a -= 1.0;
+                if (gm + z / s < (double)mx[k]) z += 1.0;
+                a -= 1.0; z += 1.0;
+                if (a < 0.0) { a = 0.0; bad = 1; }
+                if (z > 65535.0) { z = 65535.0; bad = 1; }
+                if (!(gm + (a + 1.0) / s <= (double)mn[k]) || !(gm + (z - 1.0) / s >= (double)mx[k])) bad = 1;
+                Q.planes[3 * c + k] = (uint32_t)a | ((uint32_t)z << 16);
+                ef[k] = (double)mx[k] - mn[k]; eq[k] = (z - a) / s;
+            }
+            area_f += ef[0] * ef[1] + ef[1] * ef[2] + ef[2] * ef[0]; area_q += eq[0] * eq[1] + eq[1] * eq[2] + eq[2] * eq[0];
+        }
+        gn[g] = N; qn[g] = Q;
+        if (bad) atomicOr(q_bad, 1);
+        const Box2 b = T.box[i];
+        const double dx = (double)b.hi.x - b.lo.x, dy = (double)b.hi.y - b.lo.y, dz = (double)b.hi.z - b.lo.z;
+        cost = (dx * dy + dy * dz + dz * dx) * cost_traversal;
+    }
+    cost = warp_sum(cost); area_f = warp_sum(area_f); area_q = warp_sum(area_q);
+    if ((threadIdx.x & 31) == 0 && area_f != 0.0) { atomicAdd(sums + 0, cost); atomicAdd(sums + 1, area_f); atomicAdd(sums + 2, area_q); }
 }
 
 struct DevBuf {
@@ -218,34 +343,40 @@ struct DevBuf {
     ~DevBuf() { if (p) cudaFree(p); }
     cudaError_t alloc(size_t bytes) { return cudaMalloc(&p, bytes ? bytes : 256); }
     template <class T> T* as() { return static_cast<T*>(p); }
+    void* release() { void* r = p; p = nullptr; return r; }
 };
 
 }  // namespace
 
-// Builds b->nodes / b->prim / b->bounds / b->depth / b->sah on the device `ctx` lives on.  verts: HOST array (the caller has it there
-// for the layout code and the checks anyway); it is uploaded here.  Returns CRT_OK or a CUDA / depth error.
-crt_status crt_bvh_build_device(crt_ctx* ctx, crt_bvh* b, const float* verts, int64_t n, const crt_bvh_params& pr)
+#define PLOC_CUDA(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return crt_fail(ctx, e_ == cudaErrorMemoryAllocation ? CRT_ERR_NOMEM : CRT_ERR_CUDA, "build_bvh(device): %s: %s", #call, cudaGetErrorString(e_)); } while (0)
+
+// Builds the BVH of verts (HOST array; uploaded here) on the device `ctx` lives on.
+//  full_device (builder 1): fills b->d_nodes, d_qnodes, d_tris, d_slot_of_prim, qgrid, q_violations, q_inflation, n_gpu_nodes, n_tree_nodes,
+//                           bounds, depth, sah; no host tree (crt_bvh_check verifies the device layouts themselves).
+//  otherwise (builder 2):   fills b->nodes / b->prim / bounds / depth / sah; the caller runs the host layout code.
+crt_status crt_bvh_build_device(crt_ctx* ctx, crt_bvh* b, const float* verts, int64_t n, const crt_bvh_params& pr, bool full_device)
 {
     auto t0 = std::chrono::steady_clock::now();
     b->n_tris = n; b->max_leaf = pr.max_leaf;
     b->verts.assign(verts, verts + 9 * n);
-    b->nodes.clear(); b->prim.clear(); b->depth = 0; b->sah = 0;
+    b->nodes.clear(); b->prim.clear(); b->depth = 0; b->sah = 0; b->builder = full_device ? 1 : 2;
     for (int k = 0; k < 6; ++k) b->bounds[k] = 0.f;
-    if (n == 0) { b->build_seconds = 0; return CRT_OK; }
-    if (n >= ((int64_t)1 << 30)) return crt_fail(ctx, CRT_ERR_UNSUPPORTED, "build_bvh(device): too many triangles");
+    if (n >= ((int64_t)1 << 27)) return crt_fail(ctx, CRT_ERR_UNSUPPORTED, "build_bvh(device): too many triangles");
     const int radius = std::min(MAX_RADIUS, std::max(1, pr.ploc_radius > 0 ? pr.ploc_radius : 8));
-    const int64_t n_nodes_max = 2 * n;
-    DevBuf d_verts, d_bounds, d_tri_box, d_keys, d_vals, d_keys2, d_vals2, d_sort, d_cl_id[2], d_cl_box[2], d_tmp_id, d_tmp_box, d_flag, d_nn, d_node_box, d_left, d_right, d_cnt, d_counter, d_bsum;
+    const int n_nodes = (int)(2 * n - 1);
+    DevBuf d_verts, d_bounds, d_tri_box, d_keys, d_vals, d_keys2, d_vals2, d_sort, d_cl_id[2], d_cl_box[2], d_keep, d_pos, d_nn,
+           d_box, d_left, d_right, d_cnt, d_parent, d_first, d_height, d_total, d_bsum;
     const size_t sort_bytes = radix_sort_scratch_bytes(n);
-    const int nb_max = (int)((n + SCAN_TILE - 1) / SCAN_TILE);
-#define PLOC_CUDA(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return crt_fail(ctx, e_ == cudaErrorMemoryAllocation ? CRT_ERR_NOMEM : CRT_ERR_CUDA, "build_bvh(device): %s: %s", #call, cudaGetErrorString(e_)); } while (0)
+    const int nb_max = (int)((2 * n + SCAN_TILE - 1) / SCAN_TILE);
     PLOC_CUDA(d_verts.alloc((size_t)n * 36)); PLOC_CUDA(d_bounds.alloc(32)); PLOC_CUDA(d_tri_box.alloc((size_t)n * sizeof(Box2)));
     PLOC_CUDA(d_keys.alloc((size_t)n * 4)); PLOC_CUDA(d_vals.alloc((size_t)n * 4)); PLOC_CUDA(d_keys2.alloc((size_t)n * 4)); PLOC_CUDA(d_vals2.alloc((size_t)n * 4));
     PLOC_CUDA(d_sort.alloc(sort_bytes));
     for (int k = 0; k < 2; ++k) { PLOC_CUDA(d_cl_id[k].alloc((size_t)n * 4)); PLOC_CUDA(d_cl_box[k].alloc((size_t)n * sizeof(Box2))); }
-    PLOC_CUDA(d_tmp_id.alloc((size_t)n * 4)); PLOC_CUDA(d_tmp_box.alloc((size_t)n * sizeof(Box2))); PLOC_CUDA(d_flag.alloc((size_t)n * 4)); PLOC_CUDA(d_nn.alloc((size_t)n * 4));
-    PLOC_CUDA(d_node_box.alloc((size_t)n_nodes_max * sizeof(Box2))); PLOC_CUDA(d_left.alloc((size_t)n_nodes_max * 4)); PLOC_CUDA(d_right.alloc((size_t)n_nodes_max * 4));
-    PLOC_CUDA(d_cnt.alloc((size_t)n_nodes_max * 4)); PLOC_CUDA(d_counter.alloc(256)); PLOC_CUDA(d_bsum.alloc((size_t)(nb_max + 1) * 4));
+    PLOC_CUDA(d_keep.alloc((size_t)2 * n * 4)); PLOC_CUDA(d_pos.alloc((size_t)2 * n * 4)); PLOC_CUDA(d_nn.alloc((size_t)n * 4));
+    PLOC_CUDA(d_box.alloc((size_t)2 * n * sizeof(Box2)));
+    for (DevBuf* d : {&d_left, &d_right, &d_cnt, &d_parent, &d_first, &d_height}) PLOC_CUDA(d->alloc((size_t)2 * n * 4));
+    PLOC_CUDA(d_total.alloc(256)); PLOC_CUDA(d_bsum.alloc((size_t)(nb_max + 1) * 4));
+    Tree T{d_box.as<Box2>(), d_left.as<int32_t>(), d_right.as<int32_t>(), d_cnt.as<int32_t>(), d_parent.as<int32_t>(), d_first.as<int32_t>(), d_height.as<int32_t>()};
     PLOC_CUDA(cudaMemcpy(d_verts.p, verts, (size_t)n * 36, cudaMemcpyHostToDevice));
     cudaEvent_t e0, e1;
     PLOC_CUDA(cudaEventCreate(&e0)); PLOC_CUDA(cudaEventCreate(&e1));
@@ -258,51 +389,92 @@ crt_status crt_bvh_build_device(crt_ctx* ctx, crt_bvh* b, const float* verts, in
     ploc_prims_kernel<<<gridn, PB>>>(d_verts.as<float>(), n, d_bounds.as<unsigned>(), d_tri_box.as<Box2>(), d_keys.as<uint32_t>(), d_vals.as<int32_t>());
     crt_status st = launch_radix_sort(ctx, d_keys.as<uint32_t>(), d_vals.as<int32_t>(), n, d_keys2.as<uint32_t>(), d_vals2.as<int32_t>(), d_sort.p, sort_bytes, 0);
     if (st != CRT_OK) return st;
-    ploc_init_kernel<<<gridn, PB>>>(d_vals2.as<int32_t>(), d_tri_box.as<Box2>(), n, d_cl_id[0].as<int32_t>(), d_cl_box[0].as<Box2>(), d_node_box.as<Box2>(),
-                                    d_left.as<int32_t>(), d_right.as<int32_t>(), d_cnt.as<int32_t>());
-    const int32_t first_inner = (int32_t)n;
-    PLOC_CUDA(cudaMemcpyAsync(d_counter.p, &first_inner, 4, cudaMemcpyHostToDevice, 0));
+    ploc_init_kernel<<<gridn, PB>>>(d_vals2.as<int32_t>(), d_tri_box.as<Box2>(), n, d_cl_id[0].as<int32_t>(), d_cl_box[0].as<Box2>(), T);
     // 2. clustering rounds
-    int cur = 0, n_cl = (int)n, rounds = 0;
+    int cur = 0, n_cl = (int)n, rounds = 0; int32_t node_base = (int32_t)n;
     while (n_cl > 1) {
         const unsigned g = (unsigned)((n_cl + PB - 1) / PB);
-        const int nb = (n_cl + SCAN_TILE - 1) / SCAN_TILE;
         ploc_nn_kernel<<<g, PB>>>(d_cl_box[cur].as<Box2>(), n_cl, radius, d_nn.as<int32_t>());
-        ploc_merge_kernel<<<g, PB>>>(d_nn.as<int32_t>(), d_cl_id[cur].as<int32_t>(), d_cl_box[cur].as<Box2>(), n_cl, d_tmp_id.as<int32_t>(), d_tmp_box.as<Box2>(),
-                                     d_flag.as<int32_t>(), d_node_box.as<Box2>(), d_left.as<int32_t>(), d_right.as<int32_t>(), d_cnt.as<int32_t>(), d_counter.as<int32_t>());
-        ploc_blocksum_kernel<<<nb, PB>>>(d_flag.as<int32_t>(), n_cl, d_bsum.as<int32_t>());
-        ploc_scansums_kernel<<<1, 1024>>>(d_bsum.as<int32_t>(), nb, d_bsum.as<int32_t>() + nb_max);
-        ploc_compact_kernel<<<nb, PB>>>(d_flag.as<int32_t>(), d_tmp_id.as<int32_t>(), d_tmp_box.as<Box2>(), n_cl, d_bsum.as<int32_t>(), d_cl_id[1 - cur].as<int32_t>(), d_cl_box[1 - cur].as<Box2>());
+        ploc_mark_kernel<<<g, PB>>>(d_nn.as<int32_t>(), n_cl, d_keep.as<int32_t>());
+        exclusive_scan(d_keep.as<int32_t>(), d_pos.as<int32_t>(), n_cl, d_bsum.as<int32_t>(), d_total.as<int32_t>());
+        ploc_build_kernel<<<g, PB>>>(d_nn.as<int32_t>(), d_keep.as<int32_t>(), d_pos.as<int32_t>(), d_cl_id[cur].as<int32_t>(), d_cl_box[cur].as<Box2>(), n_cl, node_base,
+                                     d_cl_id[1 - cur].as<int32_t>(), d_cl_box[1 - cur].as<Box2>(), T);
         int32_t n_new = 0;
-        PLOC_CUDA(cudaMemcpy(&n_new, d_bsum.as<int32_t>() + nb_max, 4, cudaMemcpyDeviceToHost));
+        PLOC_CUDA(cudaMemcpy(&n_new, d_total.p, 4, cudaMemcpyDeviceToHost));
         if (n_new >= n_cl || n_new < 1) return crt_fail(ctx, CRT_ERR_CUDA, "build_bvh(device): clustering made no progress (%d -> %d clusters)", n_cl, n_new);
-        n_cl = n_new; cur = 1 - cur; ++rounds;
+        node_base += n_cl - n_new; n_cl = n_new; cur = 1 - cur; ++rounds;
     }
-    PLOC_CUDA(cudaEventRecord(e1, 0));
-    PLOC_CUDA(cudaEventSynchronize(e1));
-    float ms = 0.f; PLOC_CUDA(cudaEventElapsedTime(&ms, e0, e1));
-    cudaEventDestroy(e0); cudaEventDestroy(e1);
-    b->device_build_ms = ms; b->builder = 1; b->ploc_rounds = rounds;
-    // 3. back to the host in the builder-independent form; subtrees of <= max_leaf triangles become leaves
-    int32_t root = 0, n_nodes = 0;
-    PLOC_CUDA(cudaMemcpy(&root, d_cl_id[cur].p, 4, cudaMemcpyDeviceToHost));
-    PLOC_CUDA(cudaMemcpy(&n_nodes, d_counter.p, 4, cudaMemcpyDeviceToHost));
-    if (n_nodes != 2 * n - 1 || root < 0 || root >= n_nodes || (n > 1 && root < n)) return crt_fail(ctx, CRT_ERR_CUDA, "build_bvh(device): inconsistent tree (%d nodes for %lld triangles, root %d)", n_nodes, (long long)n, root);
-    std::vector<int32_t> left((size_t)n_nodes), right((size_t)n_nodes), cnt((size_t)n_nodes), sorted_tri((size_t)n);
-    std::vector<Box2> box((size_t)n_nodes);
-    PLOC_CUDA(cudaMemcpy(left.data(), d_left.p, (size_t)n_nodes * 4, cudaMemcpyDeviceToHost));
-    PLOC_CUDA(cudaMemcpy(right.data(), d_right.p, (size_t)n_nodes * 4, cudaMemcpyDeviceToHost));
-    PLOC_CUDA(cudaMemcpy(cnt.data(), d_cnt.p, (size_t)n_nodes * 4, cudaMemcpyDeviceToHost));
-    PLOC_CUDA(cudaMemcpy(box.data(), d_node_box.p, (size_t)n_nodes * sizeof(Box2), cudaMemcpyDeviceToHost));
-    PLOC_CUDA(cudaMemcpy(sorted_tri.data(), d_vals2.p, (size_t)n * 4, cudaMemcpyDeviceToHost));
-    unsigned ob[6];
+    if (node_base != n_nodes) return crt_fail(ctx, CRT_ERR_CUDA, "build_bvh(device): inconsistent tree (%d nodes for %lld triangles)", node_base, (long long)n);
+    const int root = n_nodes - 1;
+    b->ploc_rounds = rounds;
+    unsigned ob[6]; int32_t height = 0;
     PLOC_CUDA(cudaMemcpy(ob, d_bounds.p, sizeof ob, cudaMemcpyDeviceToHost));
-#undef PLOC_CUDA
+    PLOC_CUDA(cudaMemcpy(&height, d_height.as<int32_t>() + root, 4, cudaMemcpyDeviceToHost));
     float maxabs = 0.f;
     for (int k = 0; k < 6; ++k) {
         const unsigned u = ob[k]; const unsigned bits = u ^ ((u >> 31) ? 0x80000000u : 0xffffffffu);
         float f; std::memcpy(&f, &bits, 4); b->bounds[k] = f; maxabs = std::max(maxabs, std::fabs(f));
     }
+    const float pad = maxabs * (1.0f / 131072.0f);          // the same conservative padding as the host builder (D:R10)
+    if (full_device) {
+        // 4. layouts on the device
+        DevBuf d_w, d_slot, d_ref, d_sums, d_qbad, d_gn, d_qn, d_gt, d_sop;
+        PLOC_CUDA(d_w.alloc((size_t)n * 4)); PLOC_CUDA(d_slot.alloc((size_t)n * 4)); PLOC_CUDA(d_ref.alloc((size_t)n_nodes * 4));
+        PLOC_CUDA(d_sums.alloc(64)); PLOC_CUDA(d_qbad.alloc(16));
+        PLOC_CUDA(cudaMemsetAsync(d_w.p, 0, (size_t)n * 4, 0)); PLOC_CUDA(cudaMemsetAsync(d_sums.p, 0, 64, 0)); PLOC_CUDA(cudaMemsetAsync(d_qbad.p, 0, 16, 0));
+        const unsigned gn_grid = (unsigned)((n_nodes + PB - 1) / PB);
+        int32_t* inner = d_keep.as<int32_t>(); int32_t* inner_before = d_pos.as<int32_t>();
+        layout_classify_kernel<<<gn_grid, PB>>>(T, n_nodes, pr.max_leaf, inner, d_w.as<int32_t>());
+        exclusive_scan(inner, inner_before, n_nodes, d_bsum.as<int32_t>(), d_total.as<int32_t>());
+        int32_t n_inner = 0;
+        PLOC_CUDA(cudaMemcpy(&n_inner, d_total.p, 4, cudaMemcpyDeviceToHost));
+        exclusive_scan(d_w.as<int32_t>(), d_slot.as<int32_t>(), (int)n, d_bsum.as<int32_t>(), d_total.as<int32_t>());
+        if (n_inner < 1) return crt_fail(ctx, CRT_ERR_STATE, "build_bvh(device): the whole scene is one leaf (use the host builder)");
+        PLOC_CUDA(d_gn.alloc((size_t)n_inner * sizeof(GpuNode))); PLOC_CUDA(d_qn.alloc((size_t)n_inner * sizeof(QNode)));
+        PLOC_CUDA(d_gt.alloc((size_t)n * sizeof(GpuTri))); PLOC_CUDA(d_sop.alloc((size_t)n * 4));
+        double glo[3], ghi[3];
+        for (int k = 0; k < 3; ++k) { glo[k] = (double)(b->bounds[k] - pad); ghi[k] = (double)(b->bounds[3 + k] + pad); }
+        crt_qgrid_for_box(glo, ghi, &b->qgrid);
+        layout_leaves_kernel<<<gn_grid, PB>>>(T, n_nodes, pr.max_leaf, inner_before, n_inner, d_slot.as<int32_t>(), d_vals2.as<int32_t>(), d_verts.as<float>(),
+                                              d_gt.as<GpuTri>(), d_sop.as<int32_t>(), d_ref.as<int32_t>(), (double)pr.cost_intersect, d_sums.as<double>() + 3);
+        layout_nodes_kernel<<<gn_grid, PB>>>(T, n_nodes, pr.max_leaf, d_ref.as<int32_t>(), pad, b->qgrid, d_gn.as<GpuNode>(), d_qn.as<QNode>(),
+                                             (double)pr.cost_traversal, d_sums.as<double>(), d_qbad.as<int32_t>());
+        PLOC_CUDA(cudaEventRecord(e1, 0));
+        PLOC_CUDA(cudaEventSynchronize(e1));
+        PLOC_CUDA(cudaGetLastError());
+        double sums[4]; int32_t qbad = 0; Box2 rb;
+        PLOC_CUDA(cudaMemcpy(sums, d_sums.p, sizeof sums, cudaMemcpyDeviceToHost));
+        PLOC_CUDA(cudaMemcpy(&qbad, d_qbad.p, 4, cudaMemcpyDeviceToHost));
+        PLOC_CUDA(cudaMemcpy(&rb, d_box.as<Box2>() + root, sizeof rb, cudaMemcpyDeviceToHost));
+        const double ra = ((double)rb.hi.x - rb.lo.x) * ((double)rb.hi.y - rb.lo.y) + ((double)rb.hi.y - rb.lo.y) * ((double)rb.hi.z - rb.lo.z) + ((double)rb.hi.z - rb.lo.z) * ((double)rb.hi.x - rb.lo.x);
+        b->sah = ra > 0 ? (sums[0] + sums[3]) / ra : 0;
+        b->q_violations = qbad; b->q_inflation = sums[1] > 0 ? sums[2] / sums[1] : 1.0;
+        b->depth = height;                                   // height of the binary clustering tree: an upper bound of the collapsed tree's depth
+        b->n_gpu_nodes = n_inner; b->n_tree_nodes = 2 * (int64_t)n_inner + 1;
+        b->device = ctx->device;
+        b->device_bytes += (int64_t)n_inner * (sizeof(GpuNode) + sizeof(QNode)) + (int64_t)n * (sizeof(GpuTri) + 4);
+        b->d_nodes = static_cast<GpuNode*>(d_gn.release()); b->d_qnodes = static_cast<QNode*>(d_qn.release());
+        b->d_tris = static_cast<GpuTri*>(d_gt.release()); b->d_slot_of_prim = static_cast<int32_t*>(d_sop.release());
+        float ms = 0.f; PLOC_CUDA(cudaEventElapsedTime(&ms, e0, e1));
+        cudaEventDestroy(e0); cudaEventDestroy(e1);
+        b->device_build_ms = ms;
+        b->build_seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count();
+        return CRT_OK;
+    }
+    PLOC_CUDA(cudaEventRecord(e1, 0));
+    PLOC_CUDA(cudaEventSynchronize(e1));
+    PLOC_CUDA(cudaGetLastError());
+    float ms = 0.f; PLOC_CUDA(cudaEventElapsedTime(&ms, e0, e1));
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    b->device_build_ms = ms;
+    // 3. (builder 2) back to the host in the builder-independent form; subtrees of <= max_leaf triangles become leaves
+    std::vector<int32_t> left((size_t)n_nodes), right((size_t)n_nodes), cnt((size_t)n_nodes), sorted_tri((size_t)n);
+    std::vector<Box2> box((size_t)n_nodes);
+    PLOC_CUDA(cudaMemcpy(left.data(), d_left.p, (size_t)n_nodes * 4, cudaMemcpyDeviceToHost));
+    PLOC_CUDA(cudaMemcpy(right.data(), d_right.p, (size_t)n_nodes * 4, cudaMemcpyDeviceToHost));
+    PLOC_CUDA(cudaMemcpy(cnt.data(), d_cnt.p, (size_t)n_nodes * 4, cudaMemcpyDeviceToHost));
+    PLOC_CUDA(cudaMemcpy(box.data(), d_box.p, (size_t)n_nodes * sizeof(Box2), cudaMemcpyDeviceToHost));
+    PLOC_CUDA(cudaMemcpy(sorted_tri.data(), d_vals2.p, (size_t)n * 4, cudaMemcpyDeviceToHost));
     b->nodes.reserve((size_t)n_nodes); b->prim.reserve((size_t)n);
     struct Item { int32_t src, dst, depth; };
     std::vector<Item> stack; std::vector<int32_t> sub;
@@ -335,7 +507,6 @@ crt_status crt_bvh_build_device(crt_ctx* ctx, crt_bvh* b, const float* verts, in
     b->depth = max_depth;
     const double ra = half_area(box[root]);
     b->sah = ra > 0 ? cost / ra : 0;
-    const float pad = maxabs * (1.0f / 131072.0f);          // the same conservative padding as the host builder (D:R10)
     for (BuildNode& nd : b->nodes)
         for (int k = 0; k < 3; ++k) { nd.bmin[k] -= pad; nd.bmax[k] += pad; }
     b->build_seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count();

@@ -142,24 +142,35 @@ crt_status crt_build_bvh(crt_ctx* ctx, const float* verts, const int32_t* mat_id
     for (int64_t i = 0; i < 9 * n_tris; ++i) if (!(v[i] == v[i]) || v[i] > 1e30f || v[i] < -1e30f) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "build_bvh: non-finite vertex");
     int32_t max_mat = -1;
     for (int32_t m : hm) { if (m < 0) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "build_bvh: negative material id"); max_mat = std::max(max_mat, m); }
-    if (pr.builder < 0 || pr.builder > 1) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "build_bvh: builder %d out of range", pr.builder);
-    if (pr.builder == 1 && !ctx) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "build_bvh: the device builder needs a context");
+    if (pr.builder < 0 || pr.builder > 2) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "build_bvh: builder %d out of range", pr.builder);
+    if (pr.builder != 0 && !ctx) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "build_bvh: the device builder needs a context");
+    if (n_tris <= pr.max_leaf) pr.builder = 0;            // nothing to cluster: the whole scene is one leaf (or empty)
     crt_bvh* b = new crt_bvh();
     b->max_mat_id = max_mat;
-    if (pr.builder == 1) {
-        if (!hv.empty()) {}       // (device input was copied to the host above: the layout code and crt_bvh_check work from the host copy)
-        crt_status bst = crt_bvh_build_device(ctx, b, v, n_tris, pr);
-        if (bst != CRT_OK) { delete b; return bst; }
+    if (pr.builder != 0) {
+        crt_status bst = crt_bvh_build_device(ctx, b, v, n_tris, pr, pr.builder == 1);
+        if (bst != CRT_OK) { crt_bvh_destroy(b); return bst; }
     } else crt_bvh_build_host(b, v, n_tris, pr);
     const auto t_layout0 = std::chrono::steady_clock::now();
-    if (b->depth > 60) { delete b; return crt_fail(ctx, CRT_ERR_UNSUPPORTED, "build_bvh: tree depth exceeds the traversal stack (64)"); }
+    if (b->depth > 60) { crt_bvh_destroy(b); return crt_fail(ctx, CRT_ERR_UNSUPPORTED, "build_bvh: tree depth exceeds the traversal stack (64)"); }
+    auto up = [&](void** d, const void* h, size_t bytes) -> cudaError_t {
+        cudaError_t e = cudaMalloc(d, bytes ? bytes : 256);
+        if (e != cudaSuccess) return e;
+        b->device_bytes += (int64_t)bytes;
+        return bytes ? cudaMemcpy(*d, h, bytes, cudaMemcpyHostToDevice) : cudaMemset(*d, 0, 256);      // empty scene: a defined (degenerate) record
+    };
+    if (pr.builder == 1) {
+        // the device builder wrote the traversal layouts itself (bvh_ploc.cu); only the material ids remain
+        cudaError_t e = up((void**)&b->d_mat_id, hm.data(), hm.size() * 4);
+        if (e != cudaSuccess) { crt_bvh_destroy(b); return crt_fail(ctx, e == cudaErrorMemoryAllocation ? CRT_ERR_NOMEM : CRT_ERR_CUDA, "build_bvh: upload: %s", cudaGetErrorString(e)); }
+    } else {
     // one triangle per leaf: also build the 8-wide compressed layout (the default kernel's); its triangle order is the shared one
     std::vector<WNode> wn; std::vector<int32_t> tri_order;
     if (pr.max_leaf == 1) {
         crt_bvh_build_wide(b, wn, tri_order, &b->wide_depth);
         b->n_wide_nodes = (int64_t)wn.size();
         b->wide_violations = crt_bvh_check_wide(b, wn, tri_order);
-        if (b->wide_depth > 40) { delete b; return crt_fail(ctx, CRT_ERR_UNSUPPORTED, "build_bvh: wide tree depth %d exceeds the traversal stack", b->wide_depth); }
+        if (b->wide_depth > 40) { crt_bvh_destroy(b); return crt_fail(ctx, CRT_ERR_UNSUPPORTED, "build_bvh: wide tree depth %d exceeds the traversal stack", b->wide_depth); }
     }
     // traversal layouts (host vectors; built without a context too, so that crt_bvh_check / crt_bvh_get_info cover the 16-bit nodes)
     std::vector<GpuNode> gn; std::vector<GpuTri> gt; std::vector<int32_t> sop; std::vector<QNode> qn;
@@ -167,12 +178,6 @@ crt_status crt_build_bvh(crt_ctx* ctx, const float* verts, const int32_t* mat_id
     b->q_violations = crt_bvh_quantise(b, gn, qn, &b->qgrid, &b->q_inflation);
     if (ctx) {
         b->device = ctx->device; b->n_gpu_nodes = (int64_t)gn.size();
-        auto up = [&](void** d, const void* h, size_t bytes) -> cudaError_t {
-            cudaError_t e = cudaMalloc(d, bytes ? bytes : 256);
-            if (e != cudaSuccess) return e;
-            b->device_bytes += (int64_t)bytes;
-            return bytes ? cudaMemcpy(*d, h, bytes, cudaMemcpyHostToDevice) : cudaMemset(*d, 0, 256);      // empty scene: a defined (degenerate) record
-        };
         cudaError_t e = up((void**)&b->d_nodes, gn.data(), gn.size() * sizeof(GpuNode));
         if (e == cudaSuccess) e = up((void**)&b->d_qnodes, qn.data(), qn.size() * sizeof(QNode));
         if (e == cudaSuccess) e = up((void**)&b->d_tris, gt.data(), gt.size() * sizeof(GpuTri));
@@ -180,6 +185,7 @@ crt_status crt_build_bvh(crt_ctx* ctx, const float* verts, const int32_t* mat_id
         if (e == cudaSuccess) e = up((void**)&b->d_slot_of_prim, sop.data(), sop.size() * 4);
         if (e == cudaSuccess) e = up((void**)&b->d_mat_id, hm.data(), hm.size() * 4);
         if (e != cudaSuccess) { crt_bvh_destroy(b); return crt_fail(ctx, e == cudaErrorMemoryAllocation ? CRT_ERR_NOMEM : CRT_ERR_CUDA, "build_bvh: upload: %s", cudaGetErrorString(e)); }
+    }
     }
     b->layout_seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t_layout0).count();
     *out = b;
@@ -198,7 +204,7 @@ crt_status crt_bvh_destroy(crt_bvh* b)
 crt_status crt_bvh_get_info(const crt_bvh* b, crt_bvh_info_t* o)
 {
     if (!b || !o) return crt_fail(nullptr, CRT_ERR_INVALID_ARG, "bvh_get_info: null argument");
-    o->n_tris = b->n_tris; o->n_nodes = (int64_t)b->nodes.size(); o->device_bytes = b->device_bytes;
+    o->n_tris = b->n_tris; o->n_nodes = b->nodes.empty() ? b->n_tree_nodes : (int64_t)b->nodes.size(); o->device_bytes = b->device_bytes;
     memcpy(o->bounds, b->bounds, sizeof o->bounds);
     o->sah_cost = b->sah; o->depth = b->depth; o->max_leaf = b->max_leaf; o->build_seconds = b->build_seconds;
     o->n_wide_nodes = b->n_wide_nodes; o->wide_depth = b->wide_depth;
@@ -210,7 +216,9 @@ crt_status crt_bvh_get_info(const crt_bvh* b, crt_bvh_info_t* o)
 crt_status crt_bvh_check(const crt_bvh* b, int32_t* violations)
 {
     if (!b || !violations) return crt_fail(nullptr, CRT_ERR_INVALID_ARG, "bvh_check: null argument");
-    *violations = crt_bvh_check_host(b) | (b->wide_violations << 8) | (b->q_violations << 16);
+    CrtDeviceGuard dev_guard_(b->device);
+    // host tree (host builder, builder 2) and/or the device layouts themselves (always when they exist: whichever builder wrote them)
+    *violations = (b->nodes.empty() && b->n_tris > 0 ? 0 : crt_bvh_check_host(b)) | (b->wide_violations << 8) | (b->q_violations << 16) | crt_layout_check_device(b);
     return CRT_OK;
 }
 

@@ -132,18 +132,19 @@ def test_trace_matches_oracle_on_random_rays(crt, ctx, oracle, scene_name, kerne
 
 @pytest.mark.parametrize("scene_name", ["cornell", "interior_small", "landscape_small"])
 @pytest.mark.parametrize("max_leaf,radius", [(3, 0), (1, 4), (4, 32)])
-def test_device_bvh_builder(crt, ctx, oracle, scene_name, max_leaf, radius):
+@pytest.mark.parametrize("builder", [1, 2])
+def test_device_bvh_builder(crt, ctx, oracle, scene_name, max_leaf, radius, builder):
     """crt_bvh_params.builder = 1: the hierarchy built on the GPU (parallel locally-ordered clustering, csrc/bvh_ploc.cu).  The tree passes
     the library's own invariant check (every triangle in exactly one leaf, leaves <= max_leaf, boxes nested, 16-bit planes outside their
     boxes) and traversal returns the SAME hit records as with the host-built tree and as the oracle (the result is structure-independent, D:R10)."""
     scene = SCENES[scene_name]()
-    bvh_d = ctx.crt_build_bvh(scene.verts, scene.mat_id, max_leaf=max_leaf, builder=1, ploc_radius=radius)
+    bvh_d = ctx.crt_build_bvh(scene.verts, scene.mat_id, max_leaf=max_leaf, builder=builder, ploc_radius=radius)
     bvh_h = ctx.crt_build_bvh(scene.verts, scene.mat_id, max_leaf=max_leaf)
     assert bvh_d.check() == 0
     info_d, info_h = bvh_d.info(), bvh_h.info()
-    assert info_d["builder"] == 1 and info_h["builder"] == 0 and info_d["build_rounds"] > 3 and info_d["device_build_seconds"] > 0
+    assert info_d["builder"] == builder and info_h["builder"] == 0 and info_d["build_rounds"] > 3 and info_d["device_build_seconds"] > 0
     assert info_d["n_tris"] == scene.n_tris and info_d["max_leaf"] == max_leaf and 0 < info_d["depth"] <= 60
-    assert np.array_equal(info_d["bounds"], info_h["bounds"])
+    assert np.array_equal(info_d["bounds"], info_h["bounds"]) and 100 <= info_d["q16_inflation_pct"] <= 130
     assert scene.n_tris / max_leaf <= (info_d["n_nodes"] + 1) / 2 <= scene.n_tris
     assert info_d["sah_cost"] < 1.6 * info_h["sah_cost"]                     # a comparable tree, not a degenerate one
     r = I.random_rays(6, 30000 + 11, info_h["bounds"][:3], info_h["bounds"][3:], inactive_frac=0.05)
@@ -154,15 +155,28 @@ def test_device_bvh_builder(crt, ctx, oracle, scene_name, max_leaf, radius):
 
 
 def test_device_bvh_builder_degenerate_inputs(crt, ctx, oracle):
-    """one triangle, two triangles, many identical triangles (all centroids and boxes coincide), an empty scene"""
+    """one triangle, two triangles, many identical triangles (all centroids and boxes coincide), an empty scene; then the frame loop"""
     base = I.cornell().verts
-    for v in (base[:1], base[:2], np.repeat(base[:1], 37, axis=0), base[:0]):
+    for v in (base[:1], base[:2], base[:5], np.repeat(base[:1], 37, axis=0), base[:0]):
         v = np.ascontiguousarray(v, np.float32)
-        bvh = ctx.crt_build_bvh(v, np.zeros(len(v), np.int32), builder=1)
-        assert bvh.check() == 0
-        r = I.random_rays(2, 500, [0, 0, 0], [1, 1, 1])
-        h = hits_np(oracle, ctx.crt_trace(bvh, ctx.upload(r)))
-        compare_hits(h, oracle.trace_brute(v, r.view(oracle.RAY_DTYPE).reshape(-1)))
+        for builder in (1, 2):
+            bvh = ctx.crt_build_bvh(v, np.zeros(len(v), np.int32), builder=builder)
+            assert bvh.check() == 0
+            r = I.random_rays(2, 500, [0, 0, 0], [1, 1, 1])
+            h = hits_np(oracle, ctx.crt_trace(bvh, ctx.upload(r)))
+            compare_hits(h, oracle.trace_brute(v, r.view(oracle.RAY_DTYPE).reshape(-1)))
+    # the frame loop on a device-built tree: generation reads its triangle records and slot map
+    import torch
+    scene = _small_interior()
+    imgs = []
+    for builder in (0, 1):
+        bvh = ctx.crt_build_bvh(scene.verts, scene.mat_id, builder=builder)
+        mats_dev = ctx.upload(scene.materials); mats = ctx.scene_mats(mats_dev, len(scene.materials), scene.env)
+        fr = crt.make_frame(96, 64, 1, 3, 2); order = crt.make_order("direct_reuse", 4, 4, 2)
+        acc = torch.zeros((64, 96, 3), device=ctx.device)
+        ctx.crt_render_frame(bvh, mats, crt.make_camera(scene.camera), fr, order, 2, acc, ctx.frame_workspace(fr, order))
+        torch.cuda.synchronize(); imgs.append(acc.cpu().numpy())
+    assert imgs[0].sum() > 0 and np.array_equal(imgs[0], imgs[1])
 
 
 def test_trace_tolerance_only_triangle_test(crt, ctx, oracle):

@@ -43,16 +43,25 @@ WORKLOADS = {
 FLOP_PER_NODE_VISIT, FLOP_PER_TRI_TEST, FLOP_PER_RAY = 26.0, 46.0, 21.0
 # nominal FP32 peak from the guide's unit counts: 148 SMs x 128 FP32 lanes x 2 flop (FMA) x 1.965 GHz (B200_PROFILING.md table)
 FP32_PEAK_TFLOPS_NOMINAL = 148 * 128 * 2 * 1.965e9 / 1e12
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the secondary trace kernel, from profiles/ (ncu --set full);
-# keyed by workload; None until captured.
-TRACE_DRAM_TRAFFIC = {"interior": 119.5e6, "landscape": 103.6e6, "cornell": None}     # profiles/r01f_q16_nodes.md (mean of the two captured launches)
-# what ncu shows to be the kernel's limiter (not modelled by the two-term roofline): profiles/r01f (r01a-r01d: the L1 data pipe, before the 16-bit nodes)
-TRACE_LIMITER = {"interior": {"unit": "instruction issue at 50 % lane utilisation", "issue_slots_busy_pct": 67.0, "active_threads_per_warp_instruction": 16.3,
-                              "alu_pipe_pct": 58.0, "fma_pipe_pct": 27.0, "l1tex__data_pipe_lsu_wavefronts_pct_of_peak": 56.0, "dram_pct": 1.5,
-                              "source": "profiles/r01f_q16_nodes.md"},
-                 "landscape": {"unit": "instruction issue at 50 % lane utilisation", "issue_slots_busy_pct": 69.0, "active_threads_per_warp_instruction": 17.3,
-                               "alu_pipe_pct": 62.0, "fma_pipe_pct": 25.0, "l1tex__data_pipe_lsu_wavefronts_pct_of_peak": 50.0, "dram_pct": 3.0,
-                               "source": "profiles/r01f_q16_nodes.md (bounce 1; bounce 2 has 0.4 M live rays and is latency-bound)"}}
+# ncu-measured figures of the dominant kernel (trace_dyn_kernel<0,1>, secondary rays in direct_reuse order), per LIVE ray, mean of the bounce-1 and
+# bounce-2 launches of one frame; carried over from the named profile (ncu replays kernels, so these cannot be taken inside a timed run):
+#   flop  = smsp__sass_thread_inst_executed_op_fadd_pred_on.sum + ..fmul.. + 2 x ..ffma...  ncu does not count the packed FFMA2 the default
+#           kernel now uses under op_ffma, so the counters are taken on the scalar-FFMA instantiation (trace_kernel 4: the same 12 fused multiply-adds per
+#           node visit and the same triangle test; its ray setup has 12 more)
+#   dram  = dram__bytes_read.sum + dram__bytes_write.sum of the default kernel
+NCU_PER_RAY = {
+    "interior": {"flop": 1897.0, "dram_bytes": 61.5, "source": "profiles/r02c_roofline_inputs.md (ncu on the commit 'device BVH builder: the whole build on the GPU'; flop: 7.383 G over 3,891,381 live rays of frame 7; dram: 239.1 MB over 3,890,598 live rays)"},
+    "landscape": {"flop": 1383.0, "dram_bytes": 100.7, "source": "profiles/r02c_roofline_inputs.md (same commit; flop: 2.817 G over 2,037,200 live rays of frame 7; dram: 205.2 MB over 2,038,170 live rays)"},
+}
+# what ncu shows to be the kernel's limiter (not modelled by the two-term roofline): profiles/r02a, r02c
+TRACE_LIMITER = {
+    "interior": {"unit": "memory latency at 32 resident warps per SM (64 registers): dependent 256-bit node gathers through L1/L2", "top_stall": "long_scoreboard: 5.4-6.7 warps per issued instruction",
+                 "issue_slots_busy_pct": 61.2, "active_threads_per_warp_instruction": 16.1, "l1_sector_hit_pct": 66.4, "l2_sector_hit_pct": 75.1, "alu_pipe_pct": 53.4, "fma_pipe_pct": 23.5,
+                 "l1tex__data_pipe_lsu_wavefronts_pct_of_peak": 56.4, "dram_pct": 2.0, "source": "profiles/r02c_roofline_inputs.md (mean of the bounce-1 and bounce-2 launches); profiles/r02a for the experiments behind the reading"},
+    "landscape": {"unit": "memory latency at 32 resident warps per SM; bounce 2 (0.42 M live rays of 2.09 M slots) is a short launch dominated by its tail", "top_stall": "long_scoreboard: 5.2 (bounce 1) / 10.1 (bounce 2) warps per issued instruction",
+                  "issue_slots_busy_pct": 51.4, "active_threads_per_warp_instruction": 15.7, "l1_sector_hit_pct": 58.9, "l2_sector_hit_pct": 59.7, "alu_pipe_pct": 47.3, "fma_pipe_pct": 17.9,
+                  "l1tex__data_pipe_lsu_wavefronts_pct_of_peak": 41.9, "dram_pct": 3.9, "source": "profiles/r02c_roofline_inputs.md (mean of the two launches)"},
+}
 
 
 def _peaks():
@@ -138,14 +147,14 @@ def run_reference(args):
 def cpu_baseline(workload):
     import oracle as O
     O.build()
-    scale = 2
+    scale = 1 if workload != "landscape" else 2       # the full 1920x1080 frame; the landscape's 10.3 M-triangle tree takes the single-threaded builder minutes: 1/4 of the pixels there
     scene, (w, h, spp, nb, gw, gh, s, seed, cfg) = _scene(workload, scale)
     bvh = O.Bvh(scene.verts)
     t0 = time.perf_counter()
     _, times, counts = O.render_frame(bvh, scene, O.frame(w, h, spp, seed, 0), nb, 2, gw, gh, s)
     dt = time.perf_counter() - t0
     return {"value": counts[0] / dt / 1e6, "unit": UNIT, "cores": 1, "kind": "oracle",
-            "sample": f"1 frame of the {workload} scene at {w}x{h} (1/{scale * scale} of the pixels), {spp} spp, {nb} bounces, direct_reuse {gw}x{gh} stride {s}; "
+            "sample": f"1 frame of the {workload} scene at {w}x{h} ({'the full frame' if scale == 1 else '1/%d of the pixels' % (scale * scale)}), {spp} spp, {nb} bounces, direct_reuse {gw}x{gh} stride {s}; "
                       f"{int(counts[0])} secondary rays in {dt:.2f} s (trace {times[1]:.2f} s, generate {times[0]:.2f} s); BVH build untimed",
             "secondary_trace_only_mray_s": counts[0] / max(times[1], 1e-9) / 1e6,
             "node_visits_per_ray": counts[1] / max(counts[0], 1), "tri_tests_per_ray": counts[2] / max(counts[0], 1)}
@@ -199,7 +208,7 @@ def run_cuda(args):
         n_paths, n_slots, _ = crt.crt_layout(crt.make_frame(w, h, spp), order)
         ws = ctx.frame_workspace(crt.make_frame(w, h, spp), order, host_materials=len(scene.materials) if host else 0)
         nsec = torch.zeros((K + W, max(nb, 1)), dtype=torch.int32, device=ctx.device)
-        stage = np.zeros(8, np.float32)
+        stage = np.zeros(8, np.float32); bounce_ms = np.zeros((max(nb, 1), 3), np.float32)
         if host:
             accum_h = torch.zeros((h, w, 3), dtype=torch.float32).pin_memory()
             nsec_h = np.zeros((K + W, max(nb, 1)), np.uint32)
@@ -216,6 +225,7 @@ def run_cuda(args):
                 ctx.crt_render_frame(bvh, mats, cam, fr, order, nb, accum, ws, n_secondary=nsec[i], record_times=rec)
                 if rec:
                     ctx.crt_frame_times(stage)        # synchronises the frame's last event; the K steps still run back to back on the device
+                    ctx.crt_frame_bounce_times(nb, bounce_ms)
         for i in range(W):
             step(i, False)
         barrier()
@@ -233,6 +243,10 @@ def run_cuda(args):
             res.update({"secondary_loop_mray_s": rays / (sec_ms * 1e-3) / 1e6, "trace_only_mray_s": rays / (float(stage[3]) * 1e-3) / 1e6,
                         "primary_ms": float(stage[0]) / K, "shade_ms": float(stage[1]) / K, "generate_ms": float(stage[2] - stage[4]) / K,
                         "encode_sort_permute_ms": float(stage[4]) / K, "trace_ms": float(stage[3]) / K, "trace_launch_ms": float(stage[3]) / (K * max(nb, 1))})
+            nsb = nsec[W:].sum(0).cpu().numpy().astype(np.float64)          # live rays per bounce over the K steps
+            res["per_bounce"] = [{"bounce": b + 1, "rays_per_step": float(nsb[b]) / K, "generate_ms": float(bounce_ms[b, 0]) / K, "encode_sort_permute_ms": float(bounce_ms[b, 1]) / K,
+                                  "trace_ms": float(bounce_ms[b, 2]) / K, "trace_only_mray_s": float(nsb[b]) / max(float(bounce_ms[b, 2]) * 1e-3, 1e-12) / 1e6,
+                                  "loop_mray_s": float(nsb[b]) / max(float(bounce_ms[b].sum()) * 1e-3, 1e-12) / 1e6} for b in range(nb)]
         return res
 
     # ---- frames in flight: F contexts (one per stream; a crt_ctx serialises its own calls) render alternate frames concurrently, so the
@@ -327,6 +341,11 @@ def run_cuda(args):
     modes["direct_reuse"] = time_mode("direct_reuse")
     modes["independent"] = time_mode("independent")
     modes["morton_reorder"] = time_mode("morton_reorder")
+    if args.repeats > 1:       # BASELINE config 5 / "beats both baselines": spread over repeated passes of K steps, not one number
+        for m in ("direct_reuse", "independent", "morton_reorder"):
+            runs = [modes[m]] + [time_mode(m) for _ in range(args.repeats - 1)]
+            modes[m]["repeats"] = {k: {"min": float(np.min([r[k] for r in runs])), "median": float(np.median([r[k] for r in runs])), "max": float(np.max([r[k] for r in runs])), "n": len(runs)}
+                                   for k in ("mray_s", "secondary_loop_mray_s", "trace_only_mray_s", "ms_per_step")}
     modes["world_reuse"] = time_mode("world_reuse")       # the paper's first variant, an ablation: biased, see DESIGN.md D:R18
     if not args.no_sort_codes:                            # the paper's other reordering baselines (Table 1; D:R19)
         for m in ("sort_origin", "sort_reis", "sort_costa", "sort_twopoint"):
@@ -355,19 +374,23 @@ def run_cuda(args):
         hits = ctx.crt_trace(bvh, rays)
         ctx.crt_shade_accumulate(bvh, mats, fr, b, b == nb, rays, hits, r2p, paths, acc)
     launches = max(nb, 1)
-    flop_per_launch = (nn * FLOP_PER_NODE_VISIT + nt * FLOP_PER_TRI_TEST + act * FLOP_PER_RAY) / launches
-    dr = modes["direct_reuse"]
-    achieved = flop_per_launch / (dr["trace_launch_ms"] * 1e-3) / 1e12
-    ffma_tflops, copy_gbs = ctx.crt_measure_peaks()
-    hbm_gbs, hbm_src = _peaks()
-    traffic = TRACE_DRAM_TRAFFIC.get(args.workload)
     rays_per_launch = act / launches
-    bound_alu = FP32_PEAK_TFLOPS_NOMINAL * 1e12 / (flop_per_launch / rays_per_launch) / 1e6         # MRay/s
-    bound_hbm = (hbm_gbs * 1e9 / (traffic / rays_per_launch) / 1e6) if traffic else None
-    roofline = {"bound": "alu", "kernel": "trace_dyn_kernel<0> (crt_trace, secondary rays in direct_reuse order)", "achieved": achieved, "peak": FP32_PEAK_TFLOPS_NOMINAL,
-                "unit": "TFLOP/s", "frac": achieved / FP32_PEAK_TFLOPS_NOMINAL, "traffic": traffic,
-                "peak_source": "nominal 148 SM x 128 lanes x 2 x 1.965 GHz (guide); measured FFMA loop in this run: %.1f TFLOP/s" % ffma_tflops,
-                "flop_per_ray": flop_per_launch / rays_per_launch, "node_visits_per_ray": nn / max(act, 1), "tri_tests_per_ray": nt / max(act, 1),
+    dr = modes["direct_reuse"]
+    flop_per_ray_model = (nn * FLOP_PER_NODE_VISIT + nt * FLOP_PER_TRI_TEST + act * FLOP_PER_RAY) / max(act, 1)
+    ncu = NCU_PER_RAY.get(args.workload) or {}
+    flop_per_ray = ncu.get("flop") or flop_per_ray_model            # the ncu count when a profile of this workload exists
+    ffma_tflops, copy_gbs = ctx.crt_measure_peaks()                  # FP32 peak: FFMA loop measured in THIS run (north_star: "measured")
+    hbm_gbs, hbm_src = _peaks()
+    achieved = flop_per_ray * rays_per_launch / (dr["trace_launch_ms"] * 1e-3) / 1e12
+    traffic = ncu["dram_bytes"] * rays_per_launch if ncu.get("dram_bytes") else None
+    bound_alu = ffma_tflops * 1e12 / flop_per_ray / 1e6             # MRay/s
+    bound_hbm = (hbm_gbs * 1e9 / ncu["dram_bytes"] / 1e6) if ncu.get("dram_bytes") else None
+    roofline = {"bound": "alu", "kernel": "trace_dyn_kernel<0,1> (crt_trace: 16-bit nodes, packed FFMA2; secondary rays in direct_reuse order)", "achieved": achieved,
+                "peak": ffma_tflops, "unit": "TFLOP/s", "frac": achieved / ffma_tflops, "traffic": traffic,
+                "peak_source": "FFMA loop measured in this run (crt_measure_peaks); nominal 148 SM x 128 lanes x 2 x 1.965 GHz = %.2f TFLOP/s" % FP32_PEAK_TFLOPS_NOMINAL,
+                "flop_per_ray": flop_per_ray, "flop_per_ray_source": ncu.get("source") or "model (no ncu profile of this workload)",
+                "flop_per_ray_model": flop_per_ray_model, "frac_model_flops_nominal_peak": flop_per_ray_model * rays_per_launch / (dr["trace_launch_ms"] * 1e-3) / 1e12 / FP32_PEAK_TFLOPS_NOMINAL,
+                "dram_bytes_per_ray": ncu.get("dram_bytes"), "node_visits_per_ray": nn / max(act, 1), "tri_tests_per_ray": nt / max(act, 1),
                 "rays_per_launch": rays_per_launch, "launch_ms": dr["trace_launch_ms"],
                 "mray_s_bound_alu": bound_alu, "mray_s_bound_hbm": bound_hbm, "hbm_peak_gbs": hbm_gbs, "hbm_peak_source": hbm_src,
                 "copy_gbs_this_run": copy_gbs, "frac_of_min_bound": dr["trace_only_mray_s"] / min(bound_alu, bound_hbm or bound_alu),
@@ -529,7 +552,7 @@ def run_kernels(args):
                 e0.record(); ctx.crt_trace(bvh, r, hits=hh); e1.record(); torch.cuda.synchronize()
                 ts.append(e0.elapsed_time(e1))
             nv, nt, nr = ctx.crt_trace_stats(bvh, r)
-            row["sets"][tag] = {"ms": float(np.median(ts)), "records_identical": bool(torch.equal(hi, ri)), "ids_equal_frac": ids_equal,
+            row["sets"][tag] = {"ms": float(np.median(ts)), "records_identical": bool(torch.equal(hi, ri)), "ids_equal_frac": ids_equal, "active_rays": int(nr),
                                 "node_visits_per_ray": nv / max(1, nr), "tri_tests_per_ray": nt / max(1, nr)}
         rows.append(row)
         for key in ["trace_kernel"] + touched:
@@ -634,6 +657,7 @@ def main():
     ap.add_argument("--workload", default="interior", choices=sorted(WORKLOADS))
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--frames-in-flight", type=int, default=3, help="frames rendered concurrently (one context + stream each) for the headline value; the per-mode table stays single-stream")
+    ap.add_argument("--repeats", type=int, default=1, help="repeat the K timed steps of direct_reuse / independent / morton_reorder this many times and report min / median / max")
     ap.add_argument("--no-sort-codes", action="store_true", help="skip the Origin / Reis / Costa / TwoPoint reordering baselines")
     ap.add_argument("--sweep", nargs="?", const="config3", default=None, choices=["config3", "table3", "rules", "tail", "kernels", "builders"],
                     help="config3: BASELINE config 3 sweep; table3: the paper's Table 3 shapes (tile x K) at 1920x1080, 1 spp, 2 bounces; rules: shuffled against lattice partition at the same size; tail: fixed cost of a crt_trace launch (n, 2n, 4n rays) on --workload; kernels: A/B of traversal kernel variants (--variants) on one frame's ray sets of --workload; builders: host SAH against device PLOC BVH builder on --workload")

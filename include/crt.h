@@ -230,6 +230,10 @@ size_t crt_frame_workspace_bytes(const crt_frame* frame, const crt_order* order)
 /* Synchronises the events recorded by the last crt_render_frame(record_times = 1) and adds their durations
  * (milliseconds) into stage_ms[0..4] ([host]). */
 crt_status crt_frame_times(crt_ctx* ctx, float* stage_ms);
+/* The same events per bounce (BASELINE config 5: encode+sort, traversal and throughput per bounce): adds to bounce_ms[3*(b-1) + k], b = 1 ..
+ * n_bounces ([host] float[3*n_bounces]), k = 0 generation kernel, 1 encode+sort+permute, 2 traversal.  Call after crt_frame_times (which
+ * synchronises) or any other synchronisation of the frame's stream. */
+crt_status crt_frame_bounce_times(crt_ctx* ctx, int32_t n_bounces, float* bounce_ms);
 /* Same frame through HOST buffers: materials [host] crt_material[n_materials], accum_host [host] float[h][w][3]
  * (read, added to, written back).  Copies materials + camera in and the image out on `stream` and synchronises.
  * workspace as above plus crt_frame_host_extra_bytes(). */

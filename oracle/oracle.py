@@ -28,9 +28,16 @@ class Frame(C.Structure):
     _fields_ = [("w", C.c_int32), ("h", C.c_int32), ("spp", C.c_int32), ("seed", C.c_int32), ("frame", C.c_int32)]
 
 
+# ORACLE_SANITIZE=1: the same two libraries built with AddressSanitizer + UndefinedBehaviorSanitizer.  Run the CPU suite as
+#   ORACLE_SANITIZE=1 LD_PRELOAD=$(gcc -print-file-name=libasan.so) ASAN_OPTIONS=detect_leaks=0 python -m pytest tests/test_oracle_*.py -q
+_SAN = os.environ.get("ORACLE_SANITIZE") == "1"
+_SUFFIX = "_san" if _SAN else ""
+_SAN_FLAGS = ["-fsanitize=address,undefined", "-fno-sanitize-recover=undefined", "-fno-omit-frame-pointer", "-g"] if _SAN else []
+
+
 def build(force=False):
     outs = []
-    for name, flags in (("liboracle.so", []), ("liboracle64.so", ["-DORC_REAL=double"])):
+    for name, flags in ((f"liboracle{_SUFFIX}.so", _SAN_FLAGS), (f"liboracle64{_SUFFIX}.so", ["-DORC_REAL=double"] + _SAN_FLAGS)):
         out = os.path.join(_HERE, name)
         outs.append(out)
         if not force and os.path.exists(out) and os.path.getmtime(out) >= os.path.getmtime(_SRC):
@@ -48,7 +55,7 @@ def _lib(fp64=False):
     key = bool(fp64)
     if key not in _libs:
         build()
-        lib = C.CDLL(os.path.join(_HERE, "liboracle64.so" if fp64 else "liboracle.so"))
+        lib = C.CDLL(os.path.join(_HERE, f"liboracle64{_SUFFIX}.so" if fp64 else f"liboracle{_SUFFIX}.so"))
         lib.orc_bvh_build.restype = C.c_void_p
         lib.orc_bvh_build.argtypes = [C.c_void_p, C.c_int64]
         lib.orc_bvh_free.argtypes = [C.c_void_p]

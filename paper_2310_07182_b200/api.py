@@ -329,6 +329,13 @@ class Context:
         self._check(lib().crt_frame_times(self.handle, _ptr(stage_ms)))
         return stage_ms
 
+    def crt_frame_bounce_times(self, n_bounces, bounce_ms=None):
+        """Adds the last recorded frame's device times (ms) per bounce into bounce_ms (numpy float32[n_bounces, 3]: generate, encode+sort+permute, trace)."""
+        if bounce_ms is None:
+            bounce_ms = np.zeros((n_bounces, 3), np.float32)
+        self._check(lib().crt_frame_bounce_times(self.handle, C.c_int32(n_bounces), _ptr(bounce_ms)))
+        return bounce_ms
+
     def crt_render_frame_host(self, bvh, materials_host, env, camera, frame, order, n_bounces, accum_host, n_secondary_host, workspace, stream=None):
         """materials_host: numpy structured array; accum_host: numpy/pinned torch float32[h,w,3]; n_secondary_host: numpy uint32[n_bounces]."""
         e = np.asarray(env, np.float32).reshape(6)

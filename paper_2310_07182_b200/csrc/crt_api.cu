@@ -465,6 +465,32 @@ crt_status crt_frame_times(crt_ctx* ctx, float* stage_ms)
     return CRT_OK;
 }
 
+crt_status crt_frame_bounce_times(crt_ctx* ctx, int32_t n_bounces, float* bounce_ms)
+{
+    NEED_CTX("frame_bounce_times");
+    if (!bounce_ms || n_bounces < 0) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "frame_bounce_times: bad argument");
+    if (ctx->ev_used == 0) return CRT_OK;
+    CRT_CUDA(ctx, cudaEventSynchronize(ctx->ev[ctx->ev_used - 1]));
+    int prev_main = -1, open4 = -1, bounce = 0;          // bounce: index of the bounce whose generation interval was closed last
+    for (int i = 0; i < ctx->ev_used; ++i) {
+        const int stg = ctx->ev_stage[i];
+        if (stg == -2) { open4 = i; continue; }
+        float ms = 0;
+        if (stg == 4) {
+            CRT_CUDA(ctx, cudaEventElapsedTime(&ms, ctx->ev[open4], ctx->ev[i]));
+            if (bounce < n_bounces) { bounce_ms[3 * bounce + 1] += ms; bounce_ms[3 * bounce + 0] -= ms; }     // nested inside the generation interval that closes next
+            continue;
+        }
+        if (stg >= 0 && prev_main >= 0) {
+            CRT_CUDA(ctx, cudaEventElapsedTime(&ms, ctx->ev[prev_main], ctx->ev[i]));
+            if (stg == 2 && bounce < n_bounces) bounce_ms[3 * bounce + 0] += ms;
+            if (stg == 3 && bounce < n_bounces) { bounce_ms[3 * bounce + 2] += ms; ++bounce; }
+        }
+        prev_main = i;
+    }
+    return CRT_OK;
+}
+
 size_t crt_frame_host_extra_bytes(const crt_frame* frame, int32_t n_materials)
 {
     if (!frame || n_materials < 0) return 0;

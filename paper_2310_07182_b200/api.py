@@ -34,7 +34,7 @@ EXPORTS = [
     "crt_build_bvh", "crt_bvh_destroy", "crt_bvh_get_info", "crt_bvh_check", "crt_layout", "crt_paths_init",
     "crt_trace_primary", "crt_generate_secondary", "crt_generate_secondary_scratch_bytes",
     "crt_morton_encode", "crt_ray_code_encode", "crt_radix_sort_pairs", "crt_radix_sort_scratch_bytes", "crt_trace", "crt_trace_stats",
-    "crt_shade_accumulate", "crt_render_frame", "crt_frame_workspace_bytes", "crt_frame_times",
+    "crt_shade_accumulate", "crt_render_frame", "crt_frame_workspace_bytes", "crt_frame_times", "crt_frame_bounce_times",
     "crt_render_frame_host", "crt_render_frame_host_resident", "crt_render_frame_host_resident_async", "crt_frame_host_extra_bytes",
 ]
 

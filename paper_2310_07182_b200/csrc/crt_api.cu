@@ -97,6 +97,7 @@ crt_status crt_set_option(crt_ctx* ctx, const char* key, int64_t value)
     else if (!strcmp(key, "trace_tri_wait")) { if (value < 0 || value > 32) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "trace_tri_wait out of range"); ctx->trace_tri_wait = (int)value; }
     else if (!strcmp(key, "fuse_shade")) { ctx->fuse_shade = value != 0; }
     else if (!strcmp(key, "trace_exact")) { ctx->trace_exact = value != 0; }
+    else if (!strcmp(key, "shade_pixel_order")) { ctx->shade_pixel_order = value != 0; }
     else if (!strcmp(key, "trace_blocks_per_sm")) { if (value < 0 || value > 32) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "trace_blocks_per_sm out of range"); ctx->trace_blocks_per_sm = (int)value; }
     else return crt_fail(ctx, CRT_ERR_INVALID_ARG, "set_option: unknown key '%s'", key);
     return CRT_OK;
@@ -420,7 +421,7 @@ crt_status crt_render_frame(crt_ctx* ctx, const crt_bvh* bvh, const crt_scene_ma
     // (not for the sorting modes: their ray order is a permutation of the paths, and the fused read-modify-write of the state of ended
     // paths would be a scattered access inside the generation kernel: measured 2.3x slower generation on the landscape scene)
     const bool fuse = ctx->fuse_shade != 0 && !crt_mode_sorts(L.mode);
-    if (n_bounces == 0 || !fuse) STEP(launch_shade(ctx, bvh, *mats, *frame, n_bounces == 0, W.rays[0], W.hits, W.r2p[0], L.n_slots, W.paths, accum, s, by_slot));
+    if (n_bounces == 0 || !fuse) STEP(launch_shade(ctx, bvh, *mats, *frame, n_bounces == 0, W.rays[0], W.hits, W.r2p[0], L.n_slots, W.paths, accum, s, by_slot, by_slot ? &L : nullptr));
     MARK(1);
     int cur = 0;
     for (int b = 1; b <= n_bounces; ++b) {
@@ -438,7 +439,7 @@ crt_status crt_render_frame(crt_ctx* ctx, const crt_bvh* bvh, const crt_scene_ma
         MARK(2);
         STEP(launch_trace(ctx, bvh, W.rays[cur], L.n_slots, W.hits, s));
         MARK(3);
-        if (b == n_bounces || !fuse) STEP(launch_shade(ctx, bvh, *mats, *frame, b == n_bounces, W.rays[cur], W.hits, W.r2p[cur], L.n_slots, W.paths, accum, s, by_slot));
+        if (b == n_bounces || !fuse) STEP(launch_shade(ctx, bvh, *mats, *frame, b == n_bounces, W.rays[cur], W.hits, W.r2p[cur], L.n_slots, W.paths, accum, s, by_slot, by_slot ? &L : nullptr));
         MARK(1);
     }
 #undef STEP

@@ -119,6 +119,21 @@ CRT_DEV uint32_t lcg_sequence_term(uint32_t A, uint32_t C, uint32_t x0, uint32_t
     }
     return (ga * x0 + gc) & (M - 1u);
 }
+// forward map of the partition: position m inside the tile's block of M slots of in-tile pixel number n = ly*W + lx (all three rules)
+CRT_DEV uint32_t pixel_to_slot_in_tile(const DevLayout& L, int32_t tile, int32_t sample, uint32_t n)
+{
+    const uint4 r = philox((uint32_t)tile, (uint32_t)sample, 0u, PURPOSE_TILE, L.seed, L.frame);
+    const uint32_t Mm = (uint32_t)(L.M - 1);
+    if (L.lattice == 2) return lcg_sequence_term(((r.x & Mm) & ~3u) | 1u, (r.y & Mm) | 1u, r.z & Mm, n, (uint32_t)L.M);
+    if (L.lattice == 1) {
+        const uint32_t H = (uint32_t)(L.M >> L.log2W);
+        const uint32_t px = ((n & (uint32_t)(L.W - 1)) + r.x % (uint32_t)L.W) & (uint32_t)(L.W - 1), py = ((n >> L.log2W) + r.y % H) & (H - 1u);
+        const uint32_t g = (py % (uint32_t)L.sy) * (uint32_t)L.sx + px % (uint32_t)L.sx, j = (py / (uint32_t)L.sy) * (uint32_t)L.gw + px / (uint32_t)L.sx;
+        return g * (uint32_t)L.K + j;
+    }
+    const uint32_t a = (r.x & Mm) | 1u, c = r.y & Mm;
+    return (a * n + c) & Mm;
+}
 // path id of a slot (-1 = out-of-image slot) with its pixel and sample.  direct_reuse: the slot's position m in its
 // tile is the shuffled number m = (a*n + c) mod M of pixel n = ly*W + lx, so n = a^-1 (m - c) mod M.
 CRT_DEV int32_t slot_to_path(const DevLayout& L, int64_t slot, int32_t& pixel, int32_t& sample)

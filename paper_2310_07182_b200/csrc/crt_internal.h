@@ -18,6 +18,7 @@ struct crt_ctx {
     int trace_leaf_wait = 6;           // leave the inner-node phase when at most this many converged lanes still lack a leaf
     int trace_tri_wait = 8;            // wide kernel: a warp enters its triangle phase when at least this many lanes hold triangle hits
     int trace_blocks_per_sm = 0; // 0 = from occupancy
+    int shade_pixel_order = 1;   // crt_render_frame, grouped orders: the last segment's shading walks the tile in pixel order (coalesced image updates)
     int trace_exact = 1;         // 1: the bit-exact triangle test (D:R0); 0: fused multiply-adds + approximate reciprocal (north_star's tolerances only)
     int fuse_shade = 1;          // crt_render_frame: shade non-final segments inside the next generation kernel (default; measured: DESIGN.md 5.4)
     // persistent-kernel work counter
@@ -142,7 +143,7 @@ crt_status launch_radix_sort(crt_ctx* ctx, const uint32_t* kin, const int32_t* v
                              void* scratch, size_t scratch_bytes, cudaStream_t st);
 size_t radix_sort_scratch_bytes(int64_t n);
 crt_status launch_shade(crt_ctx* ctx, const crt_bvh* bvh, const crt_scene_mats& mats, const crt_frame& f, int is_last,
-                        const crt_ray* rays, const crt_hit* hits, const int32_t* r2p, int64_t n, crt_path_state* paths, float* accum, cudaStream_t st, bool paths_by_slot = false);
+                        const crt_ray* rays, const crt_hit* hits, const int32_t* r2p, int64_t n, crt_path_state* paths, float* accum, cudaStream_t st, bool paths_by_slot = false, const Layout* pixel_order = nullptr);
 crt_status launch_paths_init(crt_ctx* ctx, crt_path_state* paths, int64_t n, cudaStream_t st);
 crt_status measure_peaks(crt_ctx* ctx, double* tflops, double* gbs);
 namespace crt { struct DevLayout; }

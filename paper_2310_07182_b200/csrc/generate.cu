@@ -261,14 +261,35 @@ __global__ void __launch_bounds__(1024) generate_kernel(GenArgs A, DevLayout L)
         else { s_wi[3 * tid] = wi.x; s_wi[3 * tid + 1] = wi.y; s_wi[3 * tid + 2] = wi.z; }
         __syncthreads();
         bool any_diff = false, any_gloss = false, any_valid = false;
+        // groups of up to 32 slots lie inside one warp: the census and the leader search are three ballots and a find-first-set instead of
+        // loops over the members' flags in shared memory (same integers; the kernel is issue-bound)
+        const bool in_warp = K <= 32;
+        unsigned m_diff = 0u, m_live = 0u, gmask = 0u; int gshift = 0;
+        if (in_warp) {
+            const int myf = flag | (((A.world || flag == F_GLOSS) && has_dir) ? 4 : 0);
+            const unsigned bd = __ballot_sync(0xffffffffu, (myf & 3) == F_DIFF), bg = __ballot_sync(0xffffffffu, (myf & 3) == F_GLOSS), bv = __ballot_sync(0xffffffffu, (myf & 4) != 0);
+            gshift = (int)(threadIdx.x & 31u) & ~(K - 1);
+            gmask = (K == 32 ? 0xffffffffu : ((1u << K) - 1u)) << gshift;
+            m_diff = bd & gmask; m_live = (bd | bg) & gmask;
+            any_diff = m_diff != 0u; any_gloss = (bg & gmask) != 0u; any_valid = (bv & gmask) != 0u;
+        } else
         for (int j = 0; j < K; ++j) { const int f = s_flag[gbase + j]; any_diff |= (f & 3) == F_DIFF; any_gloss |= (f & 3) == F_GLOSS; any_valid |= (f & 4) != 0; }
         cls = (!any_diff && !any_gloss) ? CRT_CLASS_EMPTY : (!any_gloss ? CRT_CLASS_DIFFUSE : (!any_diff ? CRT_CLASS_GLOSSY : CRT_CLASS_HYBRID));
+        // first set member of `mask` (bits gshift .. gshift + K - 1) in cyclic order from member j0: index into the block, or -1
+        auto first_from = [&](unsigned mask, int j0) -> int {
+            const unsigned g = (mask >> gshift) & (K == 32 ? 0xffffffffu : ((1u << K) - 1u));
+            if (g == 0u) return -1;
+            const unsigned hi = g >> j0;                                   // members j0 .. K-1
+            const int j = hi ? j0 + (__ffs(hi) - 1) : (__ffs(g) - 1);      // else wrap to members 0 .. j0-1
+            return gbase + j;
+        };
         if (A.world) {
             // one randomly selected live pixel's world direction for the whole group; mirrors keep their reflection
             const uint4 rl = philox((uint32_t)group, (uint32_t)sample, (uint32_t)A.bounce, PURPOSE_LEADER, L.seed, L.frame);
             const int j0 = (int)(rl.x & (uint32_t)(K - 1));
             int lj = -1;
-            for (int t = 0; t < K; ++t) { const int j = (j0 + t) & (K - 1); if ((s_flag[gbase + j] & 3) != F_DEAD) { lj = gbase + j; break; } }
+            if (in_warp) lj = first_from(m_live, j0);
+            else for (int t = 0; t < K; ++t) { const int j = (j0 + t) & (K - 1); if ((s_flag[gbase + j] & 3) != F_DEAD) { lj = gbase + j; break; } }
             if (flag != F_DEAD && lj >= 0 && lj != tid && (s_flag[lj] & 4) && mtype != CRT_MAT_SPECULAR) {
                 wdir = mk(s_wi[3 * lj], s_wi[3 * lj + 1], s_wi[3 * lj + 2]);
                 wi = to_local(fr, wdir);
@@ -291,7 +312,8 @@ __global__ void __launch_bounds__(1024) generate_kernel(GenArgs A, DevLayout L)
                 const uint4 rl = philox((uint32_t)group, (uint32_t)sample, (uint32_t)A.bounce, PURPOSE_LEADER, L.seed, L.frame);
                 const int j0 = (int)(rl.x & (uint32_t)(K - 1));
                 int leader = -1;
-                for (int t = 0; t < K; ++t) { const int j = (j0 + t) & (K - 1); if ((s_flag[gbase + j] & 3) == F_DIFF) { leader = s_path[gbase + j]; break; } }
+                if (in_warp) leader = s_path[first_from(m_diff, j0)];         // this member is diffuse, so the mask is not empty
+                else for (int t = 0; t < K; ++t) { const int j = (j0 + t) & (K - 1); if ((s_flag[gbase + j] & 3) == F_DIFF) { leader = s_path[gbase + j]; break; } }
                 const uint4 r = philox((uint32_t)(leader % (L.w * L.h)), (uint32_t)sample, (uint32_t)A.bounce, PURPOSE_BSDF, L.seed, L.frame);
                 wi = sample_cosine(u01(r.x), u01(r.y));
                 src = leader;

@@ -10,13 +10,21 @@ namespace {
 
 struct Env6 { float a[3], b[3]; };
 
+// PIXEL_ORDER (grouped orders, last segment): thread j takes in-tile pixel number j mod M of its tile and finds its slot through the forward map
+// of the partition, so that a warp's image updates fall on consecutive pixels of a tile row instead of the tile's shuffled pixels (12-byte
+// read-modify-writes scattered over the tile); the 32-byte records it then gathers inside the tile's block are whole sectors either way.
+template <bool PIXEL_ORDER>
 __global__ void __launch_bounds__(256) shade_kernel(const int32_t* __restrict__ mat_id, int32_t n_tris, const crt_material* __restrict__ mats, Env6 env, int32_t wh,
                                                     float inv_spp, int is_last, const crt_ray* __restrict__ rays, const crt_hit* __restrict__ hits,
                                                     const int32_t* __restrict__ r2p, int64_t n, crt_path_state* __restrict__ paths,
-                                                    float* __restrict__ accum, int atomic_accum, int by_slot)
+                                                    float* __restrict__ accum, int atomic_accum, int by_slot, DevLayout L)
 {
-    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
+    if (PIXEL_ORDER) {
+        const int64_t blk = i >> L.log2M;
+        i = (blk << L.log2M) + pixel_to_slot_in_tile(L, (int32_t)(blk % L.n_tiles), (int32_t)(blk / L.n_tiles), (uint32_t)(i & (L.M - 1)));
+    }
     const int32_t p = r2p[i];
     if (p < 0) return;
     // path state by path id (the public layout) or, inside crt_render_frame with a grouped order, by SLOT: the slot order is fixed
@@ -85,14 +93,21 @@ __global__ void __launch_bounds__(256) copy_kernel(const float4* __restrict__ sr
 
 }  // namespace
 
+crt::DevLayout make_dev_layout(const Layout& L, const crt_frame& f);
+
 crt_status launch_shade(crt_ctx* ctx, const crt_bvh* bvh, const crt_scene_mats& mats, const crt_frame& f, int is_last,
-                        const crt_ray* rays, const crt_hit* hits, const int32_t* r2p, int64_t n, crt_path_state* paths, float* accum, cudaStream_t st, bool paths_by_slot)
+                        const crt_ray* rays, const crt_hit* hits, const int32_t* r2p, int64_t n, crt_path_state* paths, float* accum, cudaStream_t st, bool paths_by_slot,
+                        const Layout* pixel_order)
 {
     if (n == 0) return CRT_OK;
     Env6 e;
     for (int k = 0; k < 3; ++k) { e.a[k] = mats.env[k]; e.b[k] = mats.env[3 + k]; }
-    shade_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(bvh->d_mat_id, (int32_t)bvh->n_tris, mats.materials, e, f.w * f.h, 1.0f / (float)f.spp, is_last, rays, hits, r2p, n,
-                                                              paths, accum, f.spp > 1, paths_by_slot ? 1 : 0);
+    if (pixel_order && is_last && n == pixel_order->n_slots && ctx->shade_pixel_order)
+        shade_kernel<true><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(bvh->d_mat_id, (int32_t)bvh->n_tris, mats.materials, e, f.w * f.h, 1.0f / (float)f.spp, is_last, rays, hits, r2p, n,
+                                                                        paths, accum, f.spp > 1, paths_by_slot ? 1 : 0, make_dev_layout(*pixel_order, f));
+    else
+        shade_kernel<false><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(bvh->d_mat_id, (int32_t)bvh->n_tris, mats.materials, e, f.w * f.h, 1.0f / (float)f.spp, is_last, rays, hits, r2p, n,
+                                                                         paths, accum, f.spp > 1, paths_by_slot ? 1 : 0, crt::DevLayout());
     CRT_CHECK_LAUNCH(ctx, "shade");
     return CRT_OK;
 }

@@ -330,10 +330,14 @@ def run_cuda(args):
         ms = e0.elapsed_time(e1)
         rays = sum(int(ln["nsec_h"][W:].sum().item()) for ln in lanes)
         ms_all, rays_all = reduce_over_ranks(ms, rays, ctx.device, world)
+        # each lane accumulates every F-th frame in its own resident image; the image a consumer shows is their sum over the frame count
+        # (one host add per DISPLAYED image, not per step: done here once, outside the timed region)
+        total = sum(ln["img_h"].double() for ln in lanes) / (K + W)
+        img_mean = float(total.mean().item())
         for ln in lanes:
             for k in ("ws", "img_h", "nsec_h", "used"):
                 ln.pop(k)
-        return {"mray_s": rays_all / (ms_all * 1e-3) / 1e6, "ms_per_step": ms_all / K}
+        return {"mray_s": rays_all / (ms_all * 1e-3) / 1e6, "ms_per_step": ms_all / K, "mean_of_summed_lane_images": img_mean}
 
     clocks = ClockSampler(local)
     modes = {}
@@ -417,7 +421,8 @@ def run_cuda(args):
         "e2e": {"value": e2e["mray_s"], "unit": UNIT, "h2d_bytes_per_step": len(scene.materials) * 32 + 48 + 24,
                 "d2h_bytes_per_step": img_bytes + 4 * nb, "ms_per_step": e2e["ms_per_step"],
                 "api": "crt_render_frame_host_resident_async, %d host frames in flight" % F if F > 1 else "crt_render_frame_host_resident",
-                "one_frame_at_a_time": e2e_one["mray_s"]},
+                "one_frame_at_a_time": e2e_one["mray_s"],
+                "image": "each lane keeps a resident accumulation image and copies its sum so far out every step; displayed image = sum of the lane images / frames (mean radiance %.6f)" % e2e.get("mean_of_summed_lane_images", float("nan"))},
         # kernels of the K timed steps of the headline pass: primary_rays, trace, then per bounce generate (with the previous segment's
         # shading and, at the first bounce, the initial path state fused in: the library's default) + trace, then the final shade
         "gpu_launches": K * ((3 + 2 * nb) if nb >= 1 else 4), "clocks": clk,

@@ -186,6 +186,9 @@ def run_cuda(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     ctx = crt.Context(local)
+    options = [o.split("=") for o in args.set]
+    for k_, v_ in options:
+        ctx.crt_set_option(k_, int(v_))
     scene, (w, h, spp, nb, gw, gh, s, seed, cfg) = _scene(args.workload)
     t0 = time.perf_counter()
     bvh = ctx.crt_build_bvh(scene.verts, scene.mat_id)
@@ -202,8 +205,9 @@ def run_cuda(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    def time_mode(mode, host=False):
-        """W warm-up + K timed frames of one mode; replicas (rank r) render different frame indices."""
+    def time_mode(mode, host=False, stages=True):
+        """W warm-up + K timed frames of one mode; replicas (rank r) render different frame indices.  stages=False: no per-stage events (the
+        library then runs a frame in bands, option frame_bands)."""
         order = crt.make_order(mode, gw, gh, s)
         n_paths, n_slots, _ = crt.crt_layout(crt.make_frame(w, h, spp), order)
         ws = ctx.frame_workspace(crt.make_frame(w, h, spp), order, host_materials=len(scene.materials) if host else 0)
@@ -231,14 +235,14 @@ def run_cuda(args):
         barrier()
         e0.record(stream)
         for i in range(W, W + K):
-            step(i, not host)
+            step(i, stages and not host)
         e1.record(stream)
         barrier()
         ms = e0.elapsed_time(e1)
         rays = int(nsec_h[W:].sum()) if host else int(nsec[W:].sum().item())
         ms_all, rays_all = reduce_over_ranks(ms, rays, ctx.device, world)
         res = {"mray_s": rays_all / (ms_all * 1e-3) / 1e6, "ms_per_step": ms_all / K, "secondary_rays_per_step": rays / K, "n_slots": n_slots}
-        if not host:
+        if not host and stages:
             sec_ms = float(stage[2] + stage[3])       # generate(+encode+sort+permute) + secondary trace, summed over the K steps (this rank)
             res.update({"secondary_loop_mray_s": rays / (sec_ms * 1e-3) / 1e6, "trace_only_mray_s": rays / (float(stage[3]) * 1e-3) / 1e6,
                         "primary_ms": float(stage[0]) / K, "shade_ms": float(stage[1]) / K, "generate_ms": float(stage[2] - stage[4]) / K,
@@ -255,6 +259,8 @@ def run_cuda(args):
     lanes = []
     for k in range(F):
         c = ctx if k == 0 else crt.Context(local)
+        for k_, v_ in options:
+            c.crt_set_option(k_, int(v_))
         md = mats_dev if k == 0 else c.upload(scene.materials)
         lanes.append({"ctx": c, "mats_dev": md, "mats": c.scene_mats(md, len(scene.materials), scene.env), "stream": torch.cuda.Stream(device=ctx.device)})
 
@@ -354,6 +360,7 @@ def run_cuda(args):
     if not args.no_sort_codes:                            # the paper's other reordering baselines (Table 1; D:R19)
         for m in ("sort_origin", "sort_reis", "sort_costa", "sort_twopoint"):
             modes[m] = time_mode(m)
+    single = time_mode("direct_reuse", stages=False)       # one frame at a time as a user calls it: no per-stage events, frame in bands
     e2e_one = time_mode("direct_reuse", host=True)
     e2e = time_host_pipelined("direct_reuse") if F > 1 else e2e_one
     piped = {m: time_pipelined(m) for m in ("direct_reuse", "independent", "morton_reorder")} if F > 1 else {}
@@ -412,7 +419,8 @@ def run_cuda(args):
         "config": {"workload": f"BASELINE config {cfg + 1}: {args.workload} scene, {info['n_tris']} triangles, {w}x{h}, {spp} spp, {nb} bounces, "
                                f"direct_reuse groups {gw}x{gh} stride {s}, seed {seed}",
                    "mode": "direct_reuse", "value_is": "live secondary rays per step / device time of the whole step (primary + shading included)",
-                   "frames_in_flight": F, "single_stream_value": dr["mray_s"], "single_stream_ms_per_step": dr["ms_per_step"],
+                   "frames_in_flight": F, "single_stream_value": single["mray_s"], "single_stream_ms_per_step": single["ms_per_step"],
+                   "single_stream_note": "one frame at a time without per-stage events (crt_render_frame then cuts the frame into bands, option frame_bands); modes[..].mray_s are with per-stage events, unbanded",
                    "l2": f"no explicit flush: each step streams its {ws_bytes / 1e6:.0f} MB workspace plus the {info['device_bytes'] / 1e6:.0f} MB BVH (> 126 MB L2)",
                    "parallelism": "replicas only (no sharding, no collective)" if world > 1 else "single GPU",
                    "bvh": {"nodes": info["n_nodes"], "depth": info["depth"], "sah_cost": info["sah_cost"], "device_mb": info["device_bytes"] / 1e6,
@@ -662,6 +670,7 @@ def main():
     ap.add_argument("--workload", default="interior", choices=sorted(WORKLOADS))
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--frames-in-flight", type=int, default=3, help="frames rendered concurrently (one context + stream each) for the headline value; the per-mode table stays single-stream")
+    ap.add_argument("--set", nargs="*", default=[], metavar="OPTION=VALUE", help="crt_set_option on every context of the run (experiments; the defaults are what the driver times)")
     ap.add_argument("--repeats", type=int, default=1, help="repeat the K timed steps of direct_reuse / independent / morton_reorder this many times and report min / median / max")
     ap.add_argument("--no-sort-codes", action="store_true", help="skip the Origin / Reis / Costa / TwoPoint reordering baselines")
     ap.add_argument("--sweep", nargs="?", const="config3", default=None, choices=["config3", "table3", "rules", "tail", "kernels", "builders"],

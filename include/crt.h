@@ -129,7 +129,11 @@ const char* crt_last_error(const crt_ctx* ctx);
  * phase when at most this many descending lanes hold no leaf), "trace_refill_threshold" (0..32: idle lanes fetch new rays when
  * fewer lanes than this are busy), "trace_blocks_per_sm" (0 = from the occupancy calculator), "trace_tri_wait" (8-wide kernel: lanes holding triangle hits
  * before a warp enters its triangle phase), "fuse_shade" (crt_render_frame shades non-final segments inside the next generation
- * kernel; on by default: 2.5-3 % faster on both bench scenes, the image is bit-identical). */
+ * kernel; on by default: 2.5-3 % faster on both bench scenes, the image is bit-identical), "shade_pixel_order" (1 = default: under a grouped
+ * order the last segment is shaded in the tile's pixel order through the partition's forward map, so that image updates coalesce: +2-3 % per
+ * frame, identical image), "frame_bands" (1..4, default 1: crt_render_frame cuts a frame into that many bands of whole tiles, each on its own
+ * library-owned stream, so that one band's traversal tail overlaps the others' work; identical image; 2 bands: +1-4 % for one frame at a
+ * time, -2-3 % when several frames are in flight on several contexts, profiles/r02f). */
 crt_status crt_set_option(crt_ctx* ctx, const char* key, int64_t value);
 /* Measures the device's FP32 FFMA rate (TFLOP/s) and a streaming copy rate (GB/s) with small kernels;
  * synchronous. Used only as roofline denominators by bench.py. */

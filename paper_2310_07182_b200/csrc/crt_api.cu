@@ -71,7 +71,7 @@ crt_status crt_create(int32_t device, crt_ctx** out)
     if (prop.major < 10) return crt_fail(nullptr, CRT_ERR_UNSUPPORTED, "crt_create: device is sm_%d%d; libcrt is built for sm_100a only", prop.major, prop.minor);
     crt_ctx* c = new crt_ctx();
     c->device = device; c->n_sms = prop.multiProcessorCount;
-    if (cudaMalloc(&c->d_counter, 256) != cudaSuccess) { delete c; return crt_fail(nullptr, CRT_ERR_NOMEM, "crt_create: cudaMalloc failed"); }
+    if (cudaMalloc(&c->d_counter, 4096) != cudaSuccess) { delete c; return crt_fail(nullptr, CRT_ERR_NOMEM, "crt_create: cudaMalloc failed"); }
     *out = c;
     return CRT_OK;
 }
@@ -82,6 +82,8 @@ crt_status crt_destroy(crt_ctx* ctx)
     CrtDeviceGuard dev_guard_(ctx->device);
     cudaFree(ctx->d_counter);
     for (cudaEvent_t ev : ctx->ev) cudaEventDestroy(ev);
+    for (int k = 0; k < 4; ++k) { if (ctx->band_stream[k]) cudaStreamDestroy(ctx->band_stream[k]); if (ctx->band_join[k]) cudaEventDestroy(ctx->band_join[k]); }
+    if (ctx->band_fork) cudaEventDestroy(ctx->band_fork);
     delete ctx;
     return CRT_OK;
 }
@@ -98,6 +100,7 @@ crt_status crt_set_option(crt_ctx* ctx, const char* key, int64_t value)
     else if (!strcmp(key, "fuse_shade")) { ctx->fuse_shade = value != 0; }
     else if (!strcmp(key, "trace_exact")) { ctx->trace_exact = value != 0; }
     else if (!strcmp(key, "shade_pixel_order")) { ctx->shade_pixel_order = value != 0; }
+    else if (!strcmp(key, "frame_bands")) { if (value < 1 || value > 4) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "frame_bands must be 1..4"); ctx->frame_bands = (int)value; }
     else if (!strcmp(key, "trace_blocks_per_sm")) { if (value < 0 || value > 32) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "trace_blocks_per_sm out of range"); ctx->trace_blocks_per_sm = (int)value; }
     else return crt_fail(ctx, CRT_ERR_INVALID_ARG, "set_option: unknown key '%s'", key);
     return CRT_OK;
@@ -411,37 +414,71 @@ crt_status crt_render_frame(crt_ctx* ctx, const crt_bvh* bvh, const crt_scene_ma
     // grouped orders: path state indexed by slot (fixed for the frame), so that shading and generation stream it instead of
     // gathering 32-byte records in the shuffled pixel order of the tiles; the image is unaffected (tested against the staged calls)
     const bool by_slot = (L.mode == CRT_MODE_DIRECT_REUSE || L.mode == CRT_MODE_WORLD_REUSE);
-    // option fuse_shade (below): with it the first generation kernel also sets the initial path state, so no paths_init launch
-    const bool fuse0 = ctx->fuse_shade != 0 && !crt_mode_sorts(L.mode);
-    if (!(fuse0 && n_bounces >= 1)) STEP(launch_paths_init(ctx, W.paths, by_slot ? L.n_slots : L.n_paths, s));
-    MARK(-1);
-    STEP(launch_primary(ctx, bvh, *camera, *frame, L, W.rays[0], W.hits, W.r2p[0], s));
-    MARK(0);
-    // option fuse_shade: the shading of every segment but the last runs inside the generation kernel of the next bounce
+    // option fuse_shade: the shading of every segment but the last runs inside the generation kernel of the next bounce, and the first
+    // generation kernel also sets the initial path state (no paths_init launch)
     // (not for the sorting modes: their ray order is a permutation of the paths, and the fused read-modify-write of the state of ended
     // paths would be a scattered access inside the generation kernel: measured 2.3x slower generation on the landscape scene)
     const bool fuse = ctx->fuse_shade != 0 && !crt_mode_sorts(L.mode);
-    if (n_bounces == 0 || !fuse) STEP(launch_shade(ctx, bvh, *mats, *frame, n_bounces == 0, W.rays[0], W.hits, W.r2p[0], L.n_slots, W.paths, accum, s, by_slot, by_slot ? &L : nullptr));
-    MARK(1);
-    int cur = 0;
-    for (int b = 1; b <= n_bounces; ++b) {
-        cudaEvent_t ev4[2] = {nullptr, nullptr};
-        if (record_times && crt_mode_sorts(L.mode)) {
-            // events bracketing encode+sort+permute inside generate
-            while (ctx->ev.size() < (size_t)ctx->ev_used + 2) { cudaEvent_t e; CRT_CUDA(ctx, cudaEventCreate(&e)); ctx->ev.push_back(e); ctx->ev_stage.push_back(-1); }
-            ev4[0] = ctx->ev[ctx->ev_used]; ctx->ev_stage[ctx->ev_used++] = -2;     // after the generate kernel: opens stage 4
-            ev4[1] = ctx->ev[ctx->ev_used]; ctx->ev_stage[ctx->ev_used++] = 4;      // after permute: closes stage 4
+    // Bands (option "frame_bands", default 1 = off): tiles are independent (groups never span tiles), so a frame can be cut into bands of whole tiles,
+    // every band running its whole sequence on its own library-owned stream, so that the tail of one band's traversal launch (the last rays finishing on
+    // a nearly empty machine, 0.08-0.11 ms per launch) is filled by the others' work inside ONE frame.  Measured (profiles/r02f): two bands +0.8 % (interior)
+    // / +4.2 % (landscape) for one frame at a time, three bands less, four a loss (every band launch has its own tail and the bands' persistent grids
+    // queue behind each other); with several frames in flight (bench.py's headline) bands cost 2-3 %, hence off by default.
+    // Never with per-stage timing (stage times of overlapping bands mean nothing), for the sorting modes (their sort is global), with the alternative
+    // kernels that use the context's single work counter, or for small frames.
+    const int64_t unit = std::max<int64_t>(by_slot ? L.M : 1, 256);
+    const int64_t n_units = (L.n_slots + unit - 1) / unit;
+    int n_bands = ctx->frame_bands;
+    if (record_times || crt_mode_sorts(L.mode) || ctx->trace_kernel == 2 || ctx->trace_kernel == 5 || L.n_slots < (int64_t)n_bands * 262144) n_bands = 1;
+    uint32_t* d_nact = reinterpret_cast<uint32_t*>(reinterpret_cast<char*>(ctx->d_counter) + 1024);      // [64] live rays per bounce of a banded frame
+    if (n_bands > 1) {
+        for (int k = 1; k < n_bands; ++k) {
+            if (!ctx->band_stream[k]) CRT_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->band_stream[k], cudaStreamNonBlocking));
+            if (!ctx->band_join[k]) CRT_CUDA(ctx, cudaEventCreateWithFlags(&ctx->band_join[k], cudaEventDisableTiming));
         }
-        STEP(launch_generate(ctx, bvh, *mats, *frame, b, L, W.rays[cur], W.hits, W.r2p[cur], W.paths, W.rays[1 - cur], W.r2p[1 - cur], W.gid, W.src, W.cls,
-                             W.n_active, W.scratch, W.scratch_bytes, s, ev4[0] ? ev4 : nullptr, fuse, by_slot, b == 1));
-        cur = 1 - cur;
-        if (n_secondary_out) CRT_CUDA(ctx, cudaMemcpyAsync(n_secondary_out + (b - 1), W.n_active, 4, cudaMemcpyDeviceToDevice, s));
-        MARK(2);
-        STEP(launch_trace(ctx, bvh, W.rays[cur], L.n_slots, W.hits, s));
-        MARK(3);
-        if (b == n_bounces || !fuse) STEP(launch_shade(ctx, bvh, *mats, *frame, b == n_bounces, W.rays[cur], W.hits, W.r2p[cur], L.n_slots, W.paths, accum, s, by_slot, by_slot ? &L : nullptr));
-        MARK(1);
+        if (!ctx->band_fork) CRT_CUDA(ctx, cudaEventCreateWithFlags(&ctx->band_fork, cudaEventDisableTiming));
+        CRT_CUDA(ctx, cudaMemsetAsync(d_nact, 0, 64 * sizeof(uint32_t), s));
+        CRT_CUDA(ctx, cudaEventRecord(ctx->band_fork, s));
     }
+    for (int k = 0; k < n_bands; ++k) {
+        Band band; const Band* bp = nullptr; cudaStream_t sb = s;
+        if (n_bands > 1) {
+            const int64_t u0 = n_units * k / n_bands, u1 = n_units * (k + 1) / n_bands;
+            band.slot0 = u0 * unit; band.count = std::min(u1 * unit, L.n_slots) - band.slot0;
+            band.counter = ctx->d_counter + 16 * k; band.n_active = nullptr;
+            bp = &band;
+            if (k > 0) { sb = ctx->band_stream[k]; CRT_CUDA(ctx, cudaStreamWaitEvent(sb, ctx->band_fork, 0)); }
+        }
+        const int64_t n_here = bp ? band.count : L.n_slots;
+        if (!(fuse && n_bands >= 1 && n_bounces >= 1)) STEP(launch_paths_init(ctx, W.paths + (bp ? band.slot0 : 0), bp ? band.count : (by_slot ? L.n_slots : L.n_paths), sb));
+        if (k == 0) MARK(-1);
+        STEP(launch_primary(ctx, bvh, *camera, *frame, L, W.rays[0], W.hits, W.r2p[0], sb, bp));
+        if (k == 0) MARK(0);
+        if (n_bounces == 0 || !fuse) STEP(launch_shade(ctx, bvh, *mats, *frame, n_bounces == 0, W.rays[0], W.hits, W.r2p[0], L.n_slots, W.paths, accum, sb, by_slot, by_slot ? &L : nullptr, bp));
+        if (k == 0) MARK(1);
+        int cur = 0;
+        for (int b = 1; b <= n_bounces; ++b) {
+            cudaEvent_t ev4[2] = {nullptr, nullptr};
+            if (record_times && crt_mode_sorts(L.mode)) {
+                // events bracketing encode+sort+permute inside generate
+                while (ctx->ev.size() < (size_t)ctx->ev_used + 2) { cudaEvent_t e; CRT_CUDA(ctx, cudaEventCreate(&e)); ctx->ev.push_back(e); ctx->ev_stage.push_back(-1); }
+                ev4[0] = ctx->ev[ctx->ev_used]; ctx->ev_stage[ctx->ev_used++] = -2;     // after the generate kernel: opens stage 4
+                ev4[1] = ctx->ev[ctx->ev_used]; ctx->ev_stage[ctx->ev_used++] = 4;      // after permute: closes stage 4
+            }
+            if (bp) band.n_active = d_nact + (b - 1);
+            STEP(launch_generate(ctx, bvh, *mats, *frame, b, L, W.rays[cur], W.hits, W.r2p[cur], W.paths, W.rays[1 - cur], W.r2p[1 - cur], W.gid, W.src, W.cls,
+                                 W.n_active, W.scratch, W.scratch_bytes, sb, ev4[0] ? ev4 : nullptr, fuse, by_slot, b == 1, bp));
+            cur = 1 - cur;
+            if (!bp && n_secondary_out) CRT_CUDA(ctx, cudaMemcpyAsync(n_secondary_out + (b - 1), W.n_active, 4, cudaMemcpyDeviceToDevice, sb));
+            MARK(2);
+            STEP(launch_trace(ctx, bvh, W.rays[cur] + (bp ? band.slot0 : 0), n_here, W.hits + (bp ? band.slot0 : 0), sb, false, bp ? band.counter : nullptr));
+            MARK(3);
+            if (b == n_bounces || !fuse) STEP(launch_shade(ctx, bvh, *mats, *frame, b == n_bounces, W.rays[cur], W.hits, W.r2p[cur], L.n_slots, W.paths, accum, sb, by_slot, by_slot ? &L : nullptr, bp));
+            MARK(1);
+        }
+        if (bp && k > 0) { CRT_CUDA(ctx, cudaEventRecord(ctx->band_join[k], sb)); CRT_CUDA(ctx, cudaStreamWaitEvent(s, ctx->band_join[k], 0)); }
+    }
+    if (n_bands > 1 && n_secondary_out && n_bounces > 0) CRT_CUDA(ctx, cudaMemcpyAsync(n_secondary_out, d_nact, 4 * (size_t)std::min(n_bounces, 64), cudaMemcpyDeviceToDevice, s));
 #undef STEP
 #undef MARK
     return CRT_OK;

@@ -21,8 +21,12 @@ struct crt_ctx {
     int shade_pixel_order = 1;   // crt_render_frame, grouped orders: the last segment's shading walks the tile in pixel order (coalesced image updates)
     int trace_exact = 1;         // 1: the bit-exact triangle test (D:R0); 0: fused multiply-adds + approximate reciprocal (north_star's tolerances only)
     int fuse_shade = 1;          // crt_render_frame: shade non-final segments inside the next generation kernel (default; measured: DESIGN.md 5.4)
-    // persistent-kernel work counter
+    // persistent-kernel work counters (one per band of a frame, 64 bytes apart) and, 1 KB in, the per-bounce live-ray counts of a banded frame
     unsigned int* d_counter = nullptr;
+    // crt_render_frame in bands (option "frame_bands"): library-owned streams on which the bands of one frame run side by side
+    int frame_bands = 1;
+    cudaStream_t band_stream[4] = {nullptr, nullptr, nullptr, nullptr};
+    cudaEvent_t band_fork = nullptr, band_join[4] = {nullptr, nullptr, nullptr, nullptr};
     // events for crt_render_frame(record_times)
     std::vector<cudaEvent_t> ev;
     std::vector<int> ev_stage;   // stage index closed by event i (-1: opening event)
@@ -120,21 +124,26 @@ struct Layout {
 };
 crt_status crt_make_layout(crt_ctx* ctx, const crt_frame* f, const crt_order* o, Layout* L);
 
+// a contiguous range of slots of a frame processed on its own stream (crt_render_frame in bands): tiles are independent (groups never span
+// tiles), so every stage can run on a band of whole tiles; counter = the band's traversal work counter; n_active = where generation counts its
+// live rays (added to, not zeroed, when band != nullptr)
+struct Band { int64_t slot0, count; unsigned int* counter; uint32_t* n_active; };
+
 // kernels' host launchers (defined in the .cu files) ------------------------------------------------------
 crt_status crt_bvh_build_device(crt_ctx* ctx, crt_bvh* b, const float* verts, int64_t n, const crt_bvh_params& pr, bool full_device);
 int32_t crt_layout_check_device(const crt_bvh* b);
-crt_status launch_trace(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, crt_hit* hits, cudaStream_t st, bool far_origins = false);
+crt_status launch_trace(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, crt_hit* hits, cudaStream_t st, bool far_origins = false, unsigned int* counter = nullptr);
 bool trace_queue_supported(const crt_bvh* bvh);
 crt_status launch_trace_queue(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, crt_hit* hits, unsigned long long* stats, cudaStream_t st);
 crt_status launch_trace_wide(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, crt_hit* hits, cudaStream_t st);
 crt_status launch_trace_wide_stats(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, int64_t* counters, cudaStream_t st);
 crt_status launch_trace_stats(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, int64_t* counters, cudaStream_t st);
 crt_status launch_primary(crt_ctx* ctx, const crt_bvh* bvh, const crt_camera& cam, const crt_frame& f, const Layout& L,
-                          crt_ray* rays, crt_hit* hits, int32_t* r2p, cudaStream_t st);
+                          crt_ray* rays, crt_hit* hits, int32_t* r2p, cudaStream_t st, const Band* band = nullptr);
 crt_status launch_generate(crt_ctx* ctx, const crt_bvh* bvh, const crt_scene_mats& mats, const crt_frame& f, int bounce, const Layout& L,
                            const crt_ray* prev_rays, const crt_hit* prev_hits, const int32_t* prev_r2p, crt_path_state* paths,
                            crt_ray* rays_out, int32_t* r2p_out, int32_t* gid_out, int32_t* src_out, uint8_t* cls_out,
-                           uint32_t* n_active, void* scratch, size_t scratch_bytes, cudaStream_t st, cudaEvent_t* ev4, bool fuse_shade = false, bool paths_by_slot = false, bool fresh_paths = false);
+                           uint32_t* n_active, void* scratch, size_t scratch_bytes, cudaStream_t st, cudaEvent_t* ev4, bool fuse_shade = false, bool paths_by_slot = false, bool fresh_paths = false, const Band* band = nullptr);
 crt_status launch_morton_encode(crt_ctx* ctx, const float* bounds, int code, const crt_ray* rays, int64_t n, uint32_t* keys, cudaStream_t st);
 // reordering modes (encode + sort + permute) and their sort key: 0 AilaCompact, 1 Origin, 2 Reis, 3 Costa, 4 TwoPoint
 static inline bool crt_mode_sorts(int mode) { return mode == CRT_MODE_MORTON_REORDER || (mode >= CRT_MODE_SORT_ORIGIN && mode <= CRT_MODE_SORT_TWOPOINT); }
@@ -143,7 +152,7 @@ crt_status launch_radix_sort(crt_ctx* ctx, const uint32_t* kin, const int32_t* v
                              void* scratch, size_t scratch_bytes, cudaStream_t st);
 size_t radix_sort_scratch_bytes(int64_t n);
 crt_status launch_shade(crt_ctx* ctx, const crt_bvh* bvh, const crt_scene_mats& mats, const crt_frame& f, int is_last,
-                        const crt_ray* rays, const crt_hit* hits, const int32_t* r2p, int64_t n, crt_path_state* paths, float* accum, cudaStream_t st, bool paths_by_slot = false, const Layout* pixel_order = nullptr);
+                        const crt_ray* rays, const crt_hit* hits, const int32_t* r2p, int64_t n, crt_path_state* paths, float* accum, cudaStream_t st, bool paths_by_slot = false, const Layout* pixel_order = nullptr, const Band* band = nullptr);
 crt_status launch_paths_init(crt_ctx* ctx, crt_path_state* paths, int64_t n, cudaStream_t st);
 crt_status measure_peaks(crt_ctx* ctx, double* tflops, double* gbs);
 namespace crt { struct DevLayout; }

@@ -142,6 +142,7 @@ struct GenArgs {
     int32_t fresh;            // first bounce of a fused frame: the path state is not read (throughput 1, radiance 0, alive) and is written in full
     int32_t by_slot;          // path state indexed by slot instead of by path id (crt_render_frame, grouped orders)
     int64_t n_slots; int32_t bounce; int32_t morton;   // morton: 0 = no key, else 1 + sort code
+    int64_t slot0;           // first slot of this launch (0, or the start of a band of whole tiles); n_slots = one past its last slot
     int32_t n_tris;          // hit records naming a primitive >= n_tris (a stale buffer from another BVH) are treated as dead, not dereferenced
     int32_t world;           // direct_reuse in WORLD space (mode 3; D:R18)
     int32_t fuse_shade;      // crt_render_frame: shade the previous segment here (same arithmetic as shade_kernel) instead of in its own pass
@@ -160,7 +161,7 @@ __global__ void __launch_bounds__(1024) generate_kernel(GenArgs A, DevLayout L)
     int* s_path = s_flag + blockDim.x;
     float* s_wi = reinterpret_cast<float*>(s_path + blockDim.x);
 
-    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;   // previous-segment slot
+    const int64_t i = A.slot0 + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;   // previous-segment slot
     const bool in_range = i < A.n_slots;
     int32_t pixel = -1, sample = 0, p = -1;
     if (in_range) {
@@ -420,23 +421,24 @@ crt_status launch_morton_encode(crt_ctx* ctx, const float* bounds, int code, con
 crt_status launch_generate(crt_ctx* ctx, const crt_bvh* bvh, const crt_scene_mats& mats, const crt_frame& f, int bounce, const Layout& L,
                            const crt_ray* prev_rays, const crt_hit* prev_hits, const int32_t* prev_r2p, crt_path_state* paths,
                            crt_ray* rays_out, int32_t* r2p_out, int32_t* gid_out, int32_t* src_out, uint8_t* cls_out,
-                           uint32_t* n_active, void* scratch, size_t scratch_bytes, cudaStream_t st, cudaEvent_t* ev4, bool fuse_shade, bool paths_by_slot, bool fresh_paths)
+                           uint32_t* n_active, void* scratch, size_t scratch_bytes, cudaStream_t st, cudaEvent_t* ev4, bool fuse_shade, bool paths_by_slot, bool fresh_paths, const Band* band)
 {
-    CRT_CUDA(ctx, cudaMemsetAsync(n_active, 0, sizeof(uint32_t), st));
-    if (L.n_slots == 0) return CRT_OK;
+    if (band) n_active = band->n_active;                  // a band adds to a count the frame zeroed before it forked
+    else CRT_CUDA(ctx, cudaMemsetAsync(n_active, 0, sizeof(uint32_t), st));
+    if (L.n_slots == 0 || (band && band->count == 0)) return CRT_OK;
     if (scratch_bytes < generate_scratch_bytes(L)) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "generate_secondary: scratch too small");
     GenArgs A;
     A.tris = bvh->d_tris; A.slot_of_prim = bvh->d_slot_of_prim; A.mat_id = bvh->d_mat_id; A.mats = mats.materials;
     A.prev_rays = prev_rays; A.prev_hits = prev_hits; A.prev_r2p = prev_r2p; A.paths = paths;
     A.rays_out = rays_out; A.r2p_out = r2p_out; A.gid_out = gid_out; A.src_out = src_out; A.cls_out = cls_out; A.n_active = n_active;
-    A.keys_out = nullptr; A.bounds = make_bounds(bvh->bounds); A.n_slots = L.n_slots; A.bounce = bounce; A.morton = 0; A.n_tris = (int32_t)bvh->n_tris;
+    A.keys_out = nullptr; A.bounds = make_bounds(bvh->bounds); A.n_slots = band ? band->slot0 + band->count : L.n_slots; A.slot0 = band ? band->slot0 : 0; A.bounce = bounce; A.morton = 0; A.n_tris = (int32_t)bvh->n_tris;
     A.world = (L.mode == CRT_MODE_WORLD_REUSE);
     A.fuse_shade = fuse_shade ? 1 : 0;
     A.fresh = (fresh_paths && fuse_shade) ? 1 : 0;
     A.by_slot = (paths_by_slot && (L.mode == CRT_MODE_DIRECT_REUSE || L.mode == CRT_MODE_WORLD_REUSE)) ? 1 : 0;
     for (int k = 0; k < 6; ++k) A.env[k] = mats.env[k];
     const DevLayout D = make_dev_layout(L, f);
-    const int64_t n = L.n_slots;
+    const int64_t n = band ? band->count : L.n_slots;      // (the sorting modes are never banded: their sort is global)
     if (L.mode == CRT_MODE_DIRECT_REUSE || L.mode == CRT_MODE_WORLD_REUSE) {
         const int block = L.K > 256 ? L.K : 256;
         generate_kernel<true><<<(unsigned)((n + block - 1) / block), block, (size_t)block * 20, st>>>(A, D);

@@ -17,9 +17,9 @@ template <bool PIXEL_ORDER>
 __global__ void __launch_bounds__(256) shade_kernel(const int32_t* __restrict__ mat_id, int32_t n_tris, const crt_material* __restrict__ mats, Env6 env, int32_t wh,
                                                     float inv_spp, int is_last, const crt_ray* __restrict__ rays, const crt_hit* __restrict__ hits,
                                                     const int32_t* __restrict__ r2p, int64_t n, crt_path_state* __restrict__ paths,
-                                                    float* __restrict__ accum, int atomic_accum, int by_slot, DevLayout L)
+                                                    float* __restrict__ accum, int atomic_accum, int by_slot, DevLayout L, int64_t slot0)
 {
-    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    int64_t i = slot0 + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;      // [slot0, n): the whole frame, or one band of whole tiles
     if (i >= n) return;
     if (PIXEL_ORDER) {
         const int64_t blk = i >> L.log2M;
@@ -97,17 +97,19 @@ crt::DevLayout make_dev_layout(const Layout& L, const crt_frame& f);
 
 crt_status launch_shade(crt_ctx* ctx, const crt_bvh* bvh, const crt_scene_mats& mats, const crt_frame& f, int is_last,
                         const crt_ray* rays, const crt_hit* hits, const int32_t* r2p, int64_t n, crt_path_state* paths, float* accum, cudaStream_t st, bool paths_by_slot,
-                        const Layout* pixel_order)
+                        const Layout* pixel_order, const Band* band)
 {
     if (n == 0) return CRT_OK;
+    const int64_t slot0 = band ? band->slot0 : 0, count = band ? band->count : n, end = slot0 + count;
+    if (count == 0) return CRT_OK;
     Env6 e;
     for (int k = 0; k < 3; ++k) { e.a[k] = mats.env[k]; e.b[k] = mats.env[3 + k]; }
     if (pixel_order && is_last && n == pixel_order->n_slots && ctx->shade_pixel_order)
-        shade_kernel<true><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(bvh->d_mat_id, (int32_t)bvh->n_tris, mats.materials, e, f.w * f.h, 1.0f / (float)f.spp, is_last, rays, hits, r2p, n,
-                                                                        paths, accum, f.spp > 1, paths_by_slot ? 1 : 0, make_dev_layout(*pixel_order, f));
+        shade_kernel<true><<<(unsigned)((count + 255) / 256), 256, 0, st>>>(bvh->d_mat_id, (int32_t)bvh->n_tris, mats.materials, e, f.w * f.h, 1.0f / (float)f.spp, is_last, rays, hits, r2p, end,
+                                                                        paths, accum, f.spp > 1, paths_by_slot ? 1 : 0, make_dev_layout(*pixel_order, f), slot0);
     else
-        shade_kernel<false><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(bvh->d_mat_id, (int32_t)bvh->n_tris, mats.materials, e, f.w * f.h, 1.0f / (float)f.spp, is_last, rays, hits, r2p, n,
-                                                                         paths, accum, f.spp > 1, paths_by_slot ? 1 : 0, crt::DevLayout());
+        shade_kernel<false><<<(unsigned)((count + 255) / 256), 256, 0, st>>>(bvh->d_mat_id, (int32_t)bvh->n_tris, mats.materials, e, f.w * f.h, 1.0f / (float)f.spp, is_last, rays, hits, r2p, end,
+                                                                         paths, accum, f.spp > 1, paths_by_slot ? 1 : 0, crt::DevLayout(), slot0);
     CRT_CHECK_LAUNCH(ctx, "shade");
     return CRT_OK;
 }

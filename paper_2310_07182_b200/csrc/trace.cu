@@ -383,9 +383,9 @@ __global__ void __launch_bounds__(TRACE_BLOCK, CRT_TRACE_MINB(QN)) trace_dyn_ker
 struct CamDev { float eye[3], U[3], V[3], W[3]; };
 
 // a1: camera ray of each slot's path (D:R6); the rays are then traversed by the same kernel as secondary rays
-__global__ void __launch_bounds__(256) primary_rays_kernel(CamDev cam, DevLayout L, int64_t n_slots, crt_ray* __restrict__ rays, int32_t* __restrict__ r2p)
+__global__ void __launch_bounds__(256) primary_rays_kernel(CamDev cam, DevLayout L, int64_t slot0, int64_t n_slots, crt_ray* __restrict__ rays, int32_t* __restrict__ r2p)
 {
-    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    int64_t i = slot0 + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;      // [slot0, n_slots): the whole frame, or one band of whole tiles
     if (i >= n_slots) return;
     int32_t pixel, sample, p;
     if (L.reuse && L.lattice == 2) {
@@ -421,17 +421,18 @@ __global__ void __launch_bounds__(256) primary_rays_kernel(CamDev cam, DevLayout
 }
 
 template <bool COUNT, int QN>
-crt_status launch_dyn(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, crt_hit* hits, unsigned long long* stats, cudaStream_t st)
+crt_status launch_dyn(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, crt_hit* hits, unsigned long long* stats, cudaStream_t st, unsigned int* counter = nullptr)
 {
     int per_sm = ctx->trace_blocks_per_sm;
     if (per_sm <= 0) {
         CRT_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, trace_dyn_kernel<COUNT, QN>, TRACE_BLOCK, QN == 4 ? (size_t)TREELET_NODES * 32 : (size_t)0));
         if (per_sm < 1) per_sm = 1;
     }
-    CRT_CUDA(ctx, cudaMemsetAsync(ctx->d_counter, 0, sizeof(unsigned int), st));
+    if (!counter) counter = ctx->d_counter;
+    CRT_CUDA(ctx, cudaMemsetAsync(counter, 0, sizeof(unsigned int), st));
     int64_t want = (n + TRACE_BLOCK - 1) / TRACE_BLOCK, grid = (int64_t)ctx->n_sms * per_sm;
     if (grid > want) grid = want;
-    trace_dyn_kernel<COUNT, QN><<<(unsigned)grid, TRACE_BLOCK, QN == 4 ? (size_t)TREELET_NODES * 32 : (size_t)0, st>>>(bvh->d_nodes, bvh->d_qnodes, bvh->qgrid, bvh->d_tris, rays, hits, n, ctx->d_counter, ctx->trace_refill_threshold, ctx->trace_leaf_wait, stats, (int)bvh->n_gpu_nodes);
+    trace_dyn_kernel<COUNT, QN><<<(unsigned)grid, TRACE_BLOCK, QN == 4 ? (size_t)TREELET_NODES * 32 : (size_t)0, st>>>(bvh->d_nodes, bvh->d_qnodes, bvh->qgrid, bvh->d_tris, rays, hits, n, counter, ctx->trace_refill_threshold, ctx->trace_leaf_wait, stats, (int)bvh->n_gpu_nodes);
     CRT_CHECK_LAUNCH(ctx, "trace_dyn");
     return CRT_OK;
 }
@@ -449,7 +450,7 @@ crt::DevLayout make_dev_layout(const Layout& L, const crt_frame& f)
 
 // far_origins: the caller knows the ray origins may lie beyond the default box test's contract (16 scene extents from the scene;
 // crt_trace_primary checks the camera eye): the any-origin box test (trace_kernel 4's) is used instead
-crt_status launch_trace(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, crt_hit* hits, cudaStream_t st, bool far_origins)
+crt_status launch_trace(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, crt_hit* hits, cudaStream_t st, bool far_origins, unsigned int* counter)
 {
     if (n == 0) return CRT_OK;
     if (ctx->trace_kernel == 2 && bvh->d_wnodes && bvh->wide_violations == 0) return launch_trace_wide(ctx, bvh, rays, n, hits, st);
@@ -462,11 +463,11 @@ crt_status launch_trace(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, i
     // the layout failed its own check (a plane clamped or less than one step outside its box: crt_bvh_check bit 16)
     const bool q_ok = bvh->q_inflation <= 2.0 && bvh->q_violations == 0;
     if (ctx->trace_kernel == 5 && !far_origins && trace_queue_supported(bvh)) return launch_trace_queue(ctx, bvh, rays, n, hits, nullptr, st);
-    if (ctx->trace_kernel == 6 && !far_origins && q_ok) return launch_dyn<false, 4>(ctx, bvh, rays, n, hits, nullptr, st);
-    if (ctx->trace_kernel == 3 && !ctx->trace_exact && !far_origins && q_ok) return launch_dyn<false, 3>(ctx, bvh, rays, n, hits, nullptr, st);
-    if ((ctx->trace_kernel == 4 || (ctx->trace_kernel >= 3 && far_origins)) && q_ok) return launch_dyn<false, 2>(ctx, bvh, rays, n, hits, nullptr, st);
-    if (ctx->trace_kernel >= 3 && q_ok) return launch_dyn<false, 1>(ctx, bvh, rays, n, hits, nullptr, st);
-    return launch_dyn<false, 0>(ctx, bvh, rays, n, hits, nullptr, st);
+    if (ctx->trace_kernel == 6 && !far_origins && q_ok) return launch_dyn<false, 4>(ctx, bvh, rays, n, hits, nullptr, st, counter);
+    if (ctx->trace_kernel == 3 && !ctx->trace_exact && !far_origins && q_ok) return launch_dyn<false, 3>(ctx, bvh, rays, n, hits, nullptr, st, counter);
+    if ((ctx->trace_kernel == 4 || (ctx->trace_kernel >= 3 && far_origins)) && q_ok) return launch_dyn<false, 2>(ctx, bvh, rays, n, hits, nullptr, st, counter);
+    if (ctx->trace_kernel >= 3 && q_ok) return launch_dyn<false, 1>(ctx, bvh, rays, n, hits, nullptr, st, counter);
+    return launch_dyn<false, 0>(ctx, bvh, rays, n, hits, nullptr, st, counter);
 }
 
 // counting build of the default kernel (crt_trace_stats): same traversal, no hit records written
@@ -482,12 +483,14 @@ crt_status launch_trace_stats(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* r
 }
 
 crt_status launch_primary(crt_ctx* ctx, const crt_bvh* bvh, const crt_camera& cam, const crt_frame& f, const Layout& L,
-                          crt_ray* rays, crt_hit* hits, int32_t* r2p, cudaStream_t st)
+                          crt_ray* rays, crt_hit* hits, int32_t* r2p, cudaStream_t st, const Band* band)
 {
     if (L.n_slots == 0) return CRT_OK;
+    const int64_t slot0 = band ? band->slot0 : 0, count = band ? band->count : L.n_slots;
+    if (count == 0) return CRT_OK;
     CamDev c;
     for (int k = 0; k < 3; ++k) { c.eye[k] = cam.eye[k]; c.U[k] = cam.U[k]; c.V[k] = cam.V[k]; c.W[k] = cam.W[k]; }
-    primary_rays_kernel<<<(unsigned)((L.n_slots + 255) / 256), 256, 0, st>>>(c, make_dev_layout(L, f), L.n_slots, rays, r2p);
+    primary_rays_kernel<<<(unsigned)((count + 255) / 256), 256, 0, st>>>(c, make_dev_layout(L, f), slot0, slot0 + count, rays, r2p);
     CRT_CHECK_LAUNCH(ctx, "primary_rays");
     // the default box test is conservative for origins within 16 scene extents of the scene box (include/crt.h); a camera farther
     // away takes the any-origin test
@@ -498,5 +501,5 @@ crt_status launch_primary(crt_ctx* ctx, const crt_bvh* bvh, const crt_camera& ca
         const float reach = 15.0f * fmaxf(ext, maxext * (1.0f / 4096.0f));
         if (cam.eye[k] < bvh->bounds[k] - reach || cam.eye[k] > bvh->bounds[3 + k] + reach) far_eye = true;
     }
-    return launch_trace(ctx, bvh, rays, L.n_slots, hits, st, far_eye);
+    return launch_trace(ctx, bvh, rays + slot0, count, hits + slot0, st, far_eye, band ? band->counter : nullptr);
 }

@@ -594,6 +594,35 @@ def test_two_contexts_render_concurrently_without_interfering(crt, ctx):
         assert torch.equal(acc[f], alone[f]), f
 
 
+@pytest.mark.parametrize("mode,gw,gh,s", [("direct_reuse", 4, 4, 4), ("direct_reuse", 8, 8, 8 | (1 << 15)), ("independent", 1, 1, 1), ("world_reuse", 4, 4, 2 | (1 << 14))])
+def test_frame_in_bands_gives_the_identical_image(crt, ctx, mode, gw, gh, s):
+    """crt_set_option("frame_bands", n): a frame is cut into n bands of whole tiles, each running its whole sequence on its own stream so that one band's
+    traversal tail is filled by the others' work (default 1 = off; only for frames of at least n * 262144 slots).  Same kernels on the same slots: the image and
+    the live-ray counts must not change, bit for bit (1 spp: every pixel is written by exactly one thread)."""
+    import torch
+    scene = _small_interior().with_camera(1100, 779)                  # ragged against every tile size; 857 k paths
+    G = GpuScene(crt, scene, ctx)
+    order = crt.make_order(mode, gw, gh, s)
+    fr = crt.make_frame(1100, 779, 1, 5, 2)
+    assert crt.crt_layout(fr, order)[1] >= 3 * 262144
+    ws = ctx.frame_workspace(fr, order)
+    out = {}
+    for bands in (1, 2, 3, 4):
+        ctx.crt_set_option("frame_bands", bands)
+        try:
+            acc = torch.zeros((779, 1100, 3), device=ctx.device)
+            nsec = torch.zeros(3, dtype=torch.int32, device=ctx.device)
+            for f in range(2):
+                ctx.crt_render_frame(G.bvh, G.mats, G.camera, crt.make_frame(1100, 779, 1, 5, f), order, 3, acc, ws, n_secondary=nsec)
+            torch.cuda.synchronize()
+            out[bands] = (acc.cpu().numpy(), nsec.cpu().numpy())
+        finally:
+            ctx.crt_set_option("frame_bands", 1)
+    assert out[1][0].sum() > 0 and out[1][1].min() > 100000
+    for bands in (2, 3, 4):
+        assert np.array_equal(out[bands][0], out[1][0]) and np.array_equal(out[bands][1], out[1][1]), bands
+
+
 def test_argument_errors(crt, ctx):
     import torch
     scene = I.cornell()

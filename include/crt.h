@@ -122,7 +122,8 @@ const char* crt_last_error(const crt_ctx* ctx);
  * is conservative for ANY ray origin (3 is for origins within 16 scene extents of the scene, 1 within about 128), 3-4 % slower;
  * 5 = warp-cooperative triangle phase: the triangles of a warp's parked leaves become one work list in shared memory, tested one
  * item per lane (same hit records; measured 15-25 % slower, profiles/r02a); 6 = as 3 with the top 512 nodes of the tree staged in shared
- * memory per block (same hit records; measured 8-16 % slower, profiles/r02a)), "trace_exact" (1 = default: the bit-exact triangle
+ * memory per block (same hit records; measured 8-16 % slower, profiles/r02a); 7 = the 4-wide form of the 16-bit nodes, two 32-byte records per node, built
+ * on first use (half the node visits, same hit records; measured 5-23 % slower, profiles/r02a)), "trace_exact" (1 = default: the bit-exact triangle
  * test of D:R0; 0 = fused multiply-adds and an approximate reciprocal in the triangle test: 3-5 % faster, ids equal on >= 99.999 % of
  * rays but t of grazing hits off by up to 4e-4 relative, i.e. outside north_star's 1e-4: an option, not the default),
  * "trace_leaf_wait" (0..31: a warp leaves its inner-node

@@ -393,6 +393,49 @@ int32_t crt_bvh_quantise(const crt_bvh* b, const std::vector<GpuNode>& gn, std::
     return bad;
 }
 
+// 4-wide form of the 16-bit layout (trace_kernel 7): node j = TWO consecutive 32-byte records, 2j holding the boxes and references of the children of
+// binary node i's first child, 2j + 1 those of its second child, i.e. the four GRANDCHILDREN of i; a child of i that is a leaf stands for itself
+// (its own planes, second slot empty: planes inverted, never hit).  The planes are copied from the binary 16-bit nodes, so the layout inherits their
+// outward rounding; inner references are renumbered to 4-wide nodes (breadth-first from the root).  One visit = two independent 256-bit loads and four
+// box tests: the same bytes and about 17 % fewer box tests per ray than two binary levels, and half as many DEPENDENT fetches (the kernel is bound by
+// their latency, profiles/r02a).
+void crt_bvh_collapse4(const std::vector<GpuNode>& gn, const std::vector<QNode>& qn, std::vector<QNode>& q4)
+{
+    q4.clear();
+    if (gn.empty()) return;
+    const uint32_t EMPTY_PLANES = 65535u;            // lo = 65535, hi = 0
+    std::vector<int32_t> map4(gn.size(), -1), order;
+    map4[0] = 0; order.push_back(0);
+    for (size_t h = 0; h < order.size(); ++h) {       // breadth-first over the binary nodes that head a 4-wide node
+        const int32_t i = order[h];
+        for (int c = 0; c < 2; ++c) {
+            const int32_t cr = gn[i].c[c].ref;
+            if (cr < 0 || !std::isfinite(gn[i].c[c].min_x)) continue;          // leaf or empty child: stands for itself
+            for (int g = 0; g < 2; ++g) {
+                const int32_t gr = gn[cr].c[g].ref;
+                if (gr >= 0 && std::isfinite(gn[cr].c[g].min_x) && map4[gr] < 0) { map4[gr] = (int32_t)order.size(); order.push_back(gr); }
+            }
+        }
+    }
+    q4.resize(2 * order.size());
+    for (size_t h = 0; h < order.size(); ++h) {
+        const int32_t i = order[h];
+        for (int c = 0; c < 2; ++c) {
+            QNode rec;
+            const int32_t cr = gn[i].c[c].ref;
+            const bool empty = !std::isfinite(gn[i].c[c].min_x);
+            if (!empty && cr >= 0) {
+                rec = qn[cr];
+                for (int g = 0; g < 2; ++g) if (rec.ref[g] >= 0 && std::isfinite(gn[cr].c[g].min_x)) rec.ref[g] = map4[rec.ref[g]];
+            } else {
+                for (int k = 0; k < 3; ++k) { rec.planes[k] = empty ? EMPTY_PLANES : qn[i].planes[3 * c + k]; rec.planes[3 + k] = EMPTY_PLANES; }
+                rec.ref[0] = empty ? ~0 : cr; rec.ref[1] = ~0;
+            }
+            q4[2 * h + c] = rec;
+        }
+    }
+}
+
 // Invariants of the DEVICE traversal layouts themselves (whichever builder wrote them): downloads the fp32 nodes, the 16-bit nodes, the
 // triangle records and slot_of_prim and walks the tree from node 0.  Bits as crt_bvh_check_host (1 child box not inside its parent's,
 // 2 leaf size, 4 triangle in two leaves, 8 triangle outside its leaf's box, 16 triangle in no leaf, 32 bad index / record) and 0x10000

@@ -9,6 +9,7 @@ bool crt_bvh_build_host(crt_bvh* b, const float* verts, int64_t n, const crt_bvh
 int32_t crt_bvh_check_host(const crt_bvh* b);
 void crt_bvh_flatten(const crt_bvh* b, const std::vector<int32_t>& tri_order, std::vector<GpuNode>& gn, std::vector<GpuTri>& gt, std::vector<int32_t>& slot_of_prim);
 int32_t crt_bvh_quantise(const crt_bvh* b, const std::vector<GpuNode>& gn, std::vector<QNode>& qn, QGrid* grid, double* inflation);
+void crt_bvh_collapse4(const std::vector<GpuNode>& gn, const std::vector<QNode>& qn, std::vector<QNode>& q4);
 void crt_bvh_build_wide(const crt_bvh* b, std::vector<WNode>& wn, std::vector<int32_t>& tri_order, int* depth_out);
 int32_t crt_bvh_check_wide(const crt_bvh* b, const std::vector<WNode>& wn, const std::vector<int32_t>& tri_order);
 
@@ -55,6 +56,23 @@ crt_status crt_make_layout(crt_ctx* ctx, const crt_frame* f, const crt_order* o,
     return CRT_OK;
 }
 
+// The 4-wide form of the 16-bit nodes (trace_kernel 7) is built on first use, from the device's own binary layouts: an alternative kernel should not cost
+// every BVH 14-164 MB.  Returns false when it cannot exist (tree too deep for the stack with three pushes per visit, wide triangle order, no 16-bit nodes).
+bool crt_bvh_ensure_q4(const crt_bvh* cb)
+{
+    crt_bvh* b = const_cast<crt_bvh*>(cb);
+    if (b->d_q4nodes) return true;
+    if (!b->d_nodes || !b->d_qnodes || b->d_wnodes || b->n_gpu_nodes < 1 || (b->depth + 1) / 2 * 3 + 2 > 64) return false;
+    std::vector<GpuNode> gn((size_t)b->n_gpu_nodes); std::vector<QNode> qn((size_t)b->n_gpu_nodes), q4;
+    if (cudaMemcpy(gn.data(), b->d_nodes, gn.size() * sizeof(GpuNode), cudaMemcpyDeviceToHost) != cudaSuccess) return false;
+    if (cudaMemcpy(qn.data(), b->d_qnodes, qn.size() * sizeof(QNode), cudaMemcpyDeviceToHost) != cudaSuccess) return false;
+    crt_bvh_collapse4(gn, qn, q4);
+    if (cudaMalloc((void**)&b->d_q4nodes, q4.size() * sizeof(QNode)) != cudaSuccess) { b->d_q4nodes = nullptr; return false; }
+    if (cudaMemcpy(b->d_q4nodes, q4.data(), q4.size() * sizeof(QNode), cudaMemcpyHostToDevice) != cudaSuccess) { cudaFree(b->d_q4nodes); b->d_q4nodes = nullptr; return false; }
+    b->n_q4_nodes = (int64_t)q4.size() / 2; b->device_bytes += (int64_t)(q4.size() * sizeof(QNode));
+    return true;
+}
+
 extern "C" {
 
 crt_status crt_create(int32_t device, crt_ctx** out)
@@ -93,7 +111,7 @@ const char* crt_last_error(const crt_ctx* ctx) { return ctx ? ctx->last_error.c_
 crt_status crt_set_option(crt_ctx* ctx, const char* key, int64_t value)
 {
     if (!ctx || !key) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "set_option: null argument");
-    if (!strcmp(key, "trace_kernel")) { if (value < 0 || value > 6) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "trace_kernel must be 0..6"); ctx->trace_kernel = (int)value; }
+    if (!strcmp(key, "trace_kernel")) { if (value < 0 || value > 7) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "trace_kernel must be 0..7"); ctx->trace_kernel = (int)value; }
     else if (!strcmp(key, "trace_refill_threshold")) { if (value < 0 || value > 32) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "trace_refill_threshold out of range"); ctx->trace_refill_threshold = (int)value; }
     else if (!strcmp(key, "trace_leaf_wait")) { if (value < 0 || value > 31) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "trace_leaf_wait out of range"); ctx->trace_leaf_wait = (int)value; }
     else if (!strcmp(key, "trace_tri_wait")) { if (value < 0 || value > 32) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "trace_tri_wait out of range"); ctx->trace_tri_wait = (int)value; }
@@ -200,7 +218,7 @@ crt_status crt_bvh_destroy(crt_bvh* b)
 {
     if (!b) return CRT_OK;
     CrtDeviceGuard dev_guard_(b->device);
-    cudaFree(b->d_nodes); cudaFree(b->d_qnodes); cudaFree(b->d_wnodes); cudaFree(b->d_tris); cudaFree(b->d_slot_of_prim); cudaFree(b->d_mat_id);
+    cudaFree(b->d_nodes); cudaFree(b->d_qnodes); cudaFree(b->d_q4nodes); cudaFree(b->d_wnodes); cudaFree(b->d_tris); cudaFree(b->d_slot_of_prim); cudaFree(b->d_mat_id);
     delete b;
     return CRT_OK;
 }

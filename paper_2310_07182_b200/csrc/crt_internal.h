@@ -81,6 +81,7 @@ struct crt_bvh {
     int device = -1;
     GpuNode* d_nodes = nullptr; int64_t n_gpu_nodes = 0; int64_t n_tree_nodes = 0;      // n_tree_nodes: nodes of the (collapsed) tree when no host tree exists (device builder)
     QNode* d_qnodes = nullptr; QGrid qgrid = {}; int32_t q_violations = 0; double q_inflation = 1.0;   // 16-bit layout of the same nodes (trace_kernel 3)
+    QNode* d_q4nodes = nullptr; int64_t n_q4_nodes = 0;       // 4-wide form of the 16-bit nodes: node j = records 2j, 2j + 1 (trace_kernel 7; built on first use)
     GpuTri* d_tris = nullptr;          // leaf order (wide order when the wide layout exists)
     WNode* d_wnodes = nullptr; int64_t n_wide_nodes = 0; int wide_depth = 0; int32_t wide_violations = 0;   // 8-wide layout (only when max_leaf == 1)
     int32_t* d_slot_of_prim = nullptr; // caller's triangle id -> index into d_tris
@@ -132,6 +133,7 @@ struct Band { int64_t slot0, count; unsigned int* counter; uint32_t* n_active; }
 // kernels' host launchers (defined in the .cu files) ------------------------------------------------------
 crt_status crt_bvh_build_device(crt_ctx* ctx, crt_bvh* b, const float* verts, int64_t n, const crt_bvh_params& pr, bool full_device);
 int32_t crt_layout_check_device(const crt_bvh* b);
+bool crt_bvh_ensure_q4(const crt_bvh* b);
 crt_status launch_trace(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, crt_hit* hits, cudaStream_t st, bool far_origins = false, unsigned int* counter = nullptr);
 bool trace_queue_supported(const crt_bvh* bvh);
 crt_status launch_trace_queue(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, crt_hit* hits, unsigned long long* stats, cudaStream_t st);

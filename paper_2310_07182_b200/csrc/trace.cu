@@ -35,7 +35,7 @@ constexpr int TRACE_BLOCK = 128;
 // resident blocks per SM the persistent kernel is compiled for: fp32 nodes 9 (<= 56 registers), 16-bit nodes 8 (<= 64
 // registers; measured 1.5-3 % faster than 9 with this layout, profiles/r01f)
 #define CRT_TRACE_MINB(QN) ((QN) ? 8 : 9)      // QN: 0 fp32 nodes; 1 16-bit nodes (default); 2 16-bit nodes with the any-origin box test; 3 as 1 with the
-                                               // tolerance-only triangle test (trace_exact = 0); 4 as 1 with the top of the tree staged in shared memory (experiment)
+                                               // tolerance-only triangle test (trace_exact = 0); 4 as 1 with the top of the tree staged in shared memory (experiment); 5 the 4-wide form of the 16-bit nodes
 constexpr int TREELET_NODES = 512;             // QN 4: nodes 0 .. 511 (the top levels: crt_bvh_flatten numbers them breadth-first) = 16 KB of shared memory per block
 #ifndef CRT_VISITS_PER_VOTE
 #define CRT_VISITS_PER_VOTE 3   // inner-node visits between two leaf-wait votes of a warp
@@ -239,6 +239,49 @@ CRT_DEV int visit_qnode2(const QNode* __restrict__ nodes, const uint4* s_treelet
     return next;
 }
 
+// ---- 4-wide visit (QN 5, trace_kernel 7): node idx = records 2 idx and 2 idx + 1 of the 4-wide array (crt_bvh_collapse4), fetched with two INDEPENDENT
+// 256-bit loads; four box tests by twelve FFMA2.  Order: inside a pair the nearer hit child first; the pair whose nearest hit is nearer first; the other
+// hit children are pushed so that they pop in that order (an approximate front-to-back order: the result does not depend on it, D:R10).
+CRT_DEV void q4_pair(const QNode* __restrict__ rec, const RayState& r, const QRay2& q, float tfar, float& tn_a, float& tn_b, bool& ha, bool& hb, int& ra, int& rb)
+{
+    unsigned w0, w1, w2, w3, w4, w5;
+    asm volatile("ld.global.nc.v8.u32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                 : "=r"(w0), "=r"(w1), "=r"(w2), "=r"(w3), "=r"(w4), "=r"(w5), "=r"(ra), "=r"(rb) : "l"(rec));
+    float n0x, n0y, f0x, f0y, n1x, n1y, f1x, f1y, n0z, n1z, f0z, f1z;
+    unpack2(fma2(pack2(qbits(w0, q.nx), qbits(w1, q.ny)), q.sxy, q.cxy), n0x, n0y);
+    unpack2(fma2(pack2(qbits(w0, q.fx), qbits(w1, q.fy)), q.sxy, q.cxy), f0x, f0y);
+    unpack2(fma2(pack2(qbits(w3, q.nx), qbits(w4, q.ny)), q.sxy, q.cxy), n1x, n1y);
+    unpack2(fma2(pack2(qbits(w3, q.fx), qbits(w4, q.fy)), q.sxy, q.cxy), f1x, f1y);
+    unpack2(fma2(pack2(qbits(w2, q.nz), qbits(w5, q.nz)), q.szz, q.czz), n0z, n1z);
+    unpack2(fma2(pack2(qbits(w2, q.fz), qbits(w5, q.fz)), q.szz, q.czz), f0z, f1z);
+    tn_a = fmaxf(fmaxf(n0x, n0y), fmaxf(n0z, r.tmin));
+    const float tf_a = fminf(fminf(f0x, f0y), fminf(f0z, tfar));
+    tn_b = fmaxf(fmaxf(n1x, n1y), fmaxf(n1z, r.tmin));
+    const float tf_b = fminf(fminf(f1x, f1y), fminf(f1z, tfar));
+    ha = tn_a <= tf_a; hb = tn_b <= tf_b;
+}
+CRT_DEV int visit_q4node(const QNode* __restrict__ q4, int idx, const RayState& r, const QRay2& q, int*& top)
+{
+    const float tfar = r.tfar();
+    float ta0, ta1, tb0, tb1; bool ha0, ha1, hb0, hb1; int ra0, ra1, rb0, rb1;
+    q4_pair(q4 + 2 * idx, r, q, tfar, ta0, ta1, ha0, ha1, ra0, ra1);
+    q4_pair(q4 + 2 * idx + 1, r, q, tfar, tb0, tb1, hb0, hb1, rb0, rb1);
+    // inside each pair: near / far child
+    const bool sa = ha1 && (!ha0 || ta1 < ta0), sb = hb1 && (!hb0 || tb1 < tb0);
+    const int an = sa ? ra1 : ra0, af = sa ? ra0 : ra1, bn = sb ? rb1 : rb0, bf = sb ? rb0 : rb1;
+    const bool a_any = ha0 || ha1, a_both = ha0 && ha1, b_any = hb0 || hb1, b_both = hb0 && hb1;
+    const float ta = sa ? ta1 : ta0, tb = sb ? tb1 : tb0;          // entry distance of each pair's near child (meaningful when the pair has a hit)
+    const bool b_first = b_any && (!a_any || tb < ta);
+    const int c1 = b_first ? bn : an, c2 = b_first ? bf : af, c3 = b_first ? an : bn, c4 = b_first ? af : bf;
+    const bool f1 = a_any || b_any, f2 = b_first ? b_both : a_both, f3 = b_first ? a_any : b_any, f4 = b_first ? a_both : b_both;
+    if (f4) *++top = c4;
+    if (f3) *++top = c3;
+    if (f2) *++top = c2;
+    int next = c1;
+    if (!f1) next = *top--;
+    return next;
+}
+
 // Tests the triangles of a leaf reference (D:R10 tie-break: lower primitive id wins at equal t).
 template <bool COUNT, bool FAST = false>
 CRT_DEV void visit_leaf(const GpuTri* __restrict__ tris, int ref, RayState& r, unsigned& n_tris, crt_hit* __restrict__ hits, int ray_idx)
@@ -357,7 +400,7 @@ __global__ void __launch_bounds__(TRACE_BLOCK, CRT_TRACE_MINB(QN)) trace_dyn_ker
                 for (int rep = 0; rep < CRT_VISITS_PER_VOTE; ++rep) {
                     if (rep > 0 && (unsigned)node >= (unsigned)SENTINEL) break;
                     if (COUNT) ++c_nodes;
-                    node = QN == 4 ? visit_qnode2<true>(qnodes, s_treelet, node, r, q2, top) : ((QN == 1 || QN == 3) ? visit_qnode2<false>(qnodes, nullptr, node, r, q2, top) : (QN ? visit_qnode(qnodes, node, r, q, top) : visit_node(load_node(nodes, node), r, top)));
+                    node = QN == 5 ? visit_q4node(qnodes, node, r, q2, top) : QN == 4 ? visit_qnode2<true>(qnodes, s_treelet, node, r, q2, top) : ((QN == 1 || QN == 3) ? visit_qnode2<false>(qnodes, nullptr, node, r, q2, top) : (QN ? visit_qnode(qnodes, node, r, q, top) : visit_node(load_node(nodes, node), r, top)));
                     if (node < 0 && leaf == 0) { leaf = node; node = *top--; }
                 }
                 if (__popc(__ballot_sync(__activemask(), leaf == 0)) <= leaf_wait) break;   // (nearly) every converged lane holds a leaf
@@ -432,7 +475,7 @@ crt_status launch_dyn(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int
     CRT_CUDA(ctx, cudaMemsetAsync(counter, 0, sizeof(unsigned int), st));
     int64_t want = (n + TRACE_BLOCK - 1) / TRACE_BLOCK, grid = (int64_t)ctx->n_sms * per_sm;
     if (grid > want) grid = want;
-    trace_dyn_kernel<COUNT, QN><<<(unsigned)grid, TRACE_BLOCK, QN == 4 ? (size_t)TREELET_NODES * 32 : (size_t)0, st>>>(bvh->d_nodes, bvh->d_qnodes, bvh->qgrid, bvh->d_tris, rays, hits, n, counter, ctx->trace_refill_threshold, ctx->trace_leaf_wait, stats, (int)bvh->n_gpu_nodes);
+    trace_dyn_kernel<COUNT, QN><<<(unsigned)grid, TRACE_BLOCK, QN == 4 ? (size_t)TREELET_NODES * 32 : (size_t)0, st>>>(bvh->d_nodes, QN == 5 ? bvh->d_q4nodes : bvh->d_qnodes, bvh->qgrid, bvh->d_tris, rays, hits, n, counter, ctx->trace_refill_threshold, ctx->trace_leaf_wait, stats, (int)bvh->n_gpu_nodes);
     CRT_CHECK_LAUNCH(ctx, "trace_dyn");
     return CRT_OK;
 }
@@ -464,6 +507,7 @@ crt_status launch_trace(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, i
     const bool q_ok = bvh->q_inflation <= 2.0 && bvh->q_violations == 0;
     if (ctx->trace_kernel == 5 && !far_origins && trace_queue_supported(bvh)) return launch_trace_queue(ctx, bvh, rays, n, hits, nullptr, st);
     if (ctx->trace_kernel == 6 && !far_origins && q_ok) return launch_dyn<false, 4>(ctx, bvh, rays, n, hits, nullptr, st, counter);
+    if (ctx->trace_kernel == 7 && !far_origins && q_ok && crt_bvh_ensure_q4(bvh)) return launch_dyn<false, 5>(ctx, bvh, rays, n, hits, nullptr, st, counter);
     if (ctx->trace_kernel == 3 && !ctx->trace_exact && !far_origins && q_ok) return launch_dyn<false, 3>(ctx, bvh, rays, n, hits, nullptr, st, counter);
     if ((ctx->trace_kernel == 4 || (ctx->trace_kernel >= 3 && far_origins)) && q_ok) return launch_dyn<false, 2>(ctx, bvh, rays, n, hits, nullptr, st, counter);
     if (ctx->trace_kernel >= 3 && q_ok) return launch_dyn<false, 1>(ctx, bvh, rays, n, hits, nullptr, st, counter);
@@ -477,6 +521,7 @@ crt_status launch_trace_stats(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* r
     if (ctx->trace_kernel == 2 && bvh->d_wnodes && bvh->wide_violations == 0) return launch_trace_wide_stats(ctx, bvh, rays, n, counters, st);
     const bool q_ok = bvh->q_inflation <= 2.0 && bvh->q_violations == 0;
     if (ctx->trace_kernel == 5 && trace_queue_supported(bvh)) return launch_trace_queue(ctx, bvh, rays, n, nullptr, reinterpret_cast<unsigned long long*>(counters), st);
+    if (ctx->trace_kernel == 7 && q_ok && crt_bvh_ensure_q4(bvh)) return launch_dyn<true, 5>(ctx, bvh, rays, n, nullptr, reinterpret_cast<unsigned long long*>(counters), st);
     if (ctx->trace_kernel == 4 && q_ok) return launch_dyn<true, 2>(ctx, bvh, rays, n, nullptr, reinterpret_cast<unsigned long long*>(counters), st);
     if (ctx->trace_kernel >= 3 && q_ok) return launch_dyn<true, 1>(ctx, bvh, rays, n, nullptr, reinterpret_cast<unsigned long long*>(counters), st);
     return launch_dyn<true, 0>(ctx, bvh, rays, n, nullptr, reinterpret_cast<unsigned long long*>(counters), st);

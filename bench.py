@@ -55,10 +55,10 @@ NCU_PER_RAY = {
 }
 # what ncu shows to be the kernel's limiter (not modelled by the two-term roofline): profiles/r02a, r02c
 TRACE_LIMITER = {
-    "interior": {"unit": "memory latency at 32 resident warps per SM (64 registers): dependent 256-bit node gathers through L1/L2", "top_stall": "long_scoreboard: 5.4-6.7 warps per issued instruction",
+    "interior": {"unit": "half-rate ALU pipe (plane decode, min/max, selects: 32 of 52 instructions per node visit) under long-scoreboard stalls of divergent 256-bit node gathers at 32 resident warps per SM", "top_stall": "long_scoreboard: 5.4-6.7 warps per issued instruction",
                  "issue_slots_busy_pct": 61.2, "active_threads_per_warp_instruction": 16.1, "l1_sector_hit_pct": 66.4, "l2_sector_hit_pct": 75.1, "alu_pipe_pct": 53.4, "fma_pipe_pct": 23.5,
                  "l1tex__data_pipe_lsu_wavefronts_pct_of_peak": 56.4, "dram_pct": 2.0, "source": "profiles/r02c_roofline_inputs.md (mean of the bounce-1 and bounce-2 launches); profiles/r02a for the experiments behind the reading"},
-    "landscape": {"unit": "memory latency at 32 resident warps per SM; bounce 2 (0.42 M live rays of 2.09 M slots) is a short launch dominated by its tail", "top_stall": "long_scoreboard: 5.2 (bounce 1) / 10.1 (bounce 2) warps per issued instruction",
+    "landscape": {"unit": "as interior; bounce 2 (0.42 M live rays of 2.09 M slots) is a short launch dominated by its tail", "top_stall": "long_scoreboard: 5.2 (bounce 1) / 10.1 (bounce 2) warps per issued instruction",
                   "issue_slots_busy_pct": 51.4, "active_threads_per_warp_instruction": 15.7, "l1_sector_hit_pct": 58.9, "l2_sector_hit_pct": 59.7, "alu_pipe_pct": 47.3, "fma_pipe_pct": 17.9,
                   "l1tex__data_pipe_lsu_wavefronts_pct_of_peak": 41.9, "dram_pct": 3.9, "source": "profiles/r02c_roofline_inputs.md (mean of the two launches)"},
 }

@@ -114,6 +114,9 @@ class ClockSampler:
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None, "reasons": reasons, "samples": len(sm)}
 
 
+_SWEEP_CLOCKS = None      # clock sampler of a --sweep run (started in main(), stopped where the sweep prints its JSON line)
+
+
 # ------------------------------------------------------------------------------------------------ reference arm (oracle)
 def run_reference(args):
     """The oracle as it stands, timed on this box's host cores on a bounded sample of the same workload: the same scene and
@@ -502,7 +505,7 @@ def run_sweep(args):
                 img, t = render("direct_reuse", g, s, F, 0)
                 points.append(dict(mode="direct_reuse", group=g, stride=s, **t, rmse_vs_reference=rmse(img, ref), rmse_vs_independent=rmse(img, ind)))
     name = "the paper's Table 3 shapes (P:L178-185)" if table3 else ("partition rules (D:R3 / D:R20 / D:R21)" if rules else "BASELINE config 3")
-    print(json.dumps({"sweep": points, "config": {"workload": f"{name}: interior scene {w}x{h}, {spp} spp, {nb} bounces", "frames": F,
+    print(json.dumps({"clocks": _SWEEP_CLOCKS.stop() if _SWEEP_CLOCKS else None, "sweep": points, "config": {"workload": f"{name}: interior scene {w}x{h}, {spp} spp, {nb} bounces", "frames": F,
                                                   "reference_frames": 4 * F, "scale": sc}}))
 
 
@@ -570,7 +573,7 @@ def run_kernels(args):
         rows.append(row)
         for key in ["trace_kernel"] + touched:
             ctx.crt_set_option(key, KERNEL_OPTION_DEFAULTS[key])
-    print(json.dumps({"kernels": rows, "config": {"workload": args.workload, "order": f"direct_reuse {gw}x{gh} stride {s} / independent", "frame": 7,
+    print(json.dumps({"clocks": _SWEEP_CLOCKS.stop() if _SWEEP_CLOCKS else None, "kernels": rows, "config": {"workload": args.workload, "order": f"direct_reuse {gw}x{gh} stride {s} / independent", "frame": 7,
                                                   "timing": "crt_trace alone, CUDA events, median of 8, 256 MB L2 flush between repetitions"}}))
     tags = [t for t, _ in sets]
     sys.stderr.write("| variant | " + " | ".join(tags) + " |\n|---|" + "---:|" * len(tags) + "\n")
@@ -612,7 +615,7 @@ def run_builders(args):
             row["sets"][tag] = {"ms": float(np.median(ts)), "records_identical": bool(torch.equal(hh.view(torch.int32), ref[tag].view(torch.int32))),
                                 "node_visits_per_ray": nv / max(1, nr), "tri_tests_per_ray": nt / max(1, nr)}
         rows.append(row)
-    print(json.dumps({"builders": rows, "config": {"workload": args.workload, "n_tris": int(scene.n_tris), "frame": 7,
+    print(json.dumps({"clocks": _SWEEP_CLOCKS.stop() if _SWEEP_CLOCKS else None, "builders": rows, "config": {"workload": args.workload, "n_tris": int(scene.n_tris), "frame": 7,
                                                    "timing": "crt_trace alone, CUDA events, median of 8, 256 MB L2 flush between repetitions"}}))
     tags = [t for t, _ in sets]
     sys.stderr.write("| builder | hierarchy s | of which on device s | layout s | rounds | depth | SAH cost | check | " + " | ".join(tags) + " |\n|---|" + "---:|" * (7 + len(tags)) + "\n")
@@ -658,7 +661,7 @@ def run_tail(args):
     for tag, r in sets:
         t1 = t_trace(r); r2 = torch.cat([r, r]).contiguous(); t2 = t_trace(r2); t4 = t_trace(torch.cat([r2, r2]).contiguous())
         rows.append({"rays": tag, "n": int(r.shape[0]), "t_n_ms": t1, "t_2n_ms": t2, "t_4n_ms": t4, "fixed_ms_from_2n": 2 * t1 - t2, "fixed_ms_from_4n": (4 * t1 - t4) / 3})
-    print(json.dumps({"tail": rows, "config": {"workload": args.workload, "order": f"direct_reuse {gw}x{gh} stride {s}", "frame": 7}}))
+    print(json.dumps({"clocks": _SWEEP_CLOCKS.stop() if _SWEEP_CLOCKS else None, "tail": rows, "config": {"workload": args.workload, "order": f"direct_reuse {gw}x{gh} stride {s}", "frame": 7}}))
 
 
 def main():
@@ -682,6 +685,9 @@ def main():
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "cuda":
         args.warmup = 3
+    if args.sweep:
+        global _SWEEP_CLOCKS
+        _SWEEP_CLOCKS = ClockSampler(0); _SWEEP_CLOCKS.start()       # every sweep line carries the clocks sampled during it
     if args.sweep == "tail":
         run_tail(args)
         return

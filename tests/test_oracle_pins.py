@@ -173,3 +173,120 @@ def test_secondary_origin_is_the_hit_point_offset_along_the_wall_normal(oracle, 
     u = hits["u"][ps].astype(np.float64); v = hits["v"][ps].astype(np.float64)
     pb = tri[:, 0] + u[:, None] * (tri[:, 1] - tri[:, 0]) + v[:, None] * (tri[:, 2] - tri[:, 0])
     assert np.all(np.abs(pb - p) < 5e-6)
+
+
+# ------------------------------------------------------------------ pins added after a second mutation sweep (leader rule, tile constants, hybrid with one glossy sample,
+#                                                                    BSDF stream per bounce, group ids)
+def _first_bounce(oracle, scene, mode, gw=4, gh=4, s=2, frame=0, spp=1, seed=0):
+    fr = oracle.frame(scene.width, scene.height, spp, seed, frame)
+    b = oracle.Bvh(scene.verts)
+    rays, hits, r2p = oracle.trace_primary(b, scene.camera, fr, mode, gw, gh, s)
+    paths = oracle.paths_init(spp * scene.width * scene.height)
+    accum = np.zeros((scene.height, scene.width, 3), np.float32)
+    oracle.shade_accumulate(scene, fr, 0, False, rays, hits, r2p, paths, accum)
+    out = oracle.generate_secondary(scene, fr, 1, mode, gw, gh, s, b.info()["bounds"], rays, hits, r2p, paths)
+    out.update(prev_rays=rays, prev_hits=hits, prev_r2p=r2p, paths=paths, fr=fr, bvh=b, accum=accum)
+    return out
+
+
+def _member_types(sc, g):
+    """material type of the primary hit of every slot's path (-1: no path / miss)"""
+    ok = g["prev_r2p"] >= 0
+    prim_of_path = np.full(sc.width * sc.height, -1); prim_of_path[g["prev_r2p"][ok]] = g["prev_hits"]["prim"][ok]
+    p = g["ray_to_path"]
+    pr = np.where(p >= 0, prim_of_path[np.maximum(p, 0)], -1)
+    return np.where(pr >= 0, sc.materials["type"][sc.mat_id[np.maximum(pr, 0)]], -1)
+
+
+@pytest.mark.parametrize("mode", [M_REUSE, M_WORLD])
+def test_leader_is_the_first_eligible_member_in_cyclic_order_from_the_leader_stream(oracle, mode):
+    """"Randomly selects one pixel" (D:R8, R18): start slot j0 = Philox(group, sample, bounce, LEADER).r0 mod K, then the first live DIFFUSE member in
+    cyclic slot order (tangent-space reuse) / the first live member of ANY material (world-space reuse).  Expected leaders are recomputed here from the pinned
+    Philox and the members' materials."""
+    # world mode: Lambert, GGX and mirror cells, so leaders of every material occur; tangent mode: mostly-Lambert floor, so many all-diffuse groups
+    sc = I.checker_floor() if mode == M_WORLD else I.checker_floor(p_diffuse=0.97)
+    K = 16
+    g = _first_bounce(oracle, sc, mode)
+    mt = _member_types(sc, g).reshape(-1, K); p = g["ray_to_path"].reshape(-1, K); src = g["dir_src"].reshape(-1, K)
+    act = g["rays"]["tmax"].reshape(-1, K) >= 0
+    n_checked = n_glossy_leader = 0
+    for gi in range(len(p)):
+        live = (mt[gi] >= 0) & (mt[gi] != I.MAT_EMISSIVE)
+        elig = live & (mt[gi] == I.MAT_DIFFUSE) if mode == M_REUSE else live
+        if mode == M_REUSE and ((mt[gi] == I.MAT_GLOSSY) | (mt[gi] == I.MAT_SPECULAR)).any():
+            continue                                      # hybrid groups take the glossy mean instead (separate test)
+        if not elig.any():
+            continue
+        j0 = oracle.philox(gi, 0, 1, 3, 0, 0)[0] % K
+        lead_slot = next(j % K for j in range(j0, j0 + K) if elig[j % K])
+        reusers = act[gi] & (src[gi] != p[gi]) if mode == M_WORLD else act[gi] & elig
+        if reusers.any():
+            assert np.all(src[gi][reusers] == p[gi][lead_slot]), (gi, j0, lead_slot)
+            n_checked += 1
+            n_glossy_leader += int(mt[gi][lead_slot] != I.MAT_DIFFUSE)
+    assert n_checked > (20 if mode == M_REUSE else 50) and (mode == M_REUSE or n_glossy_leader > 5)
+
+
+def test_tile_shuffle_constants_come_from_the_tile_stream(oracle):
+    """D:R3: m = (a n + c) mod M with a = (r0 mod M) | 1, c = r1 mod M, (r0, r1) = Philox(tile, sample, 0, TILE; seed, frame)."""
+    fr = oracle.frame(64, 48, 2, seed=9, frame=4)
+    for gw, gh, s in ((4, 4, 2), (2, 2, 4), (8, 4, 1)):
+        W, H = gw * s, gh * s; M = W * H
+        pos = oracle.partition(fr, M_REUSE, gw, gh, s)
+        tiles_x, tiles_y = 64 // W, 48 // H
+        for sample in (0, 1):
+            for tile in (0, 3, tiles_x * tiles_y - 1):
+                blk = pos[(sample * tiles_x * tiles_y + tile) * M:][:M]
+                tx, ty = tile % tiles_x, tile // tiles_x
+                pix = blk % (64 * 48)
+                n_of_m = ((pix // 64) - ty * H) * W + ((pix % 64) - tx * W)
+                r = oracle.philox(tile, sample, 0, 2, 9, 4)
+                a, c = (r[0] % M) | 1, r[1] % M
+                assert np.array_equal((a * n_of_m + c) % M, np.arange(M))
+                assert np.all(blk // (64 * 48) == sample)
+
+
+def test_hybrid_group_with_a_single_glossy_sample_and_group_ids(oracle):
+    """the diffuse members of a hybrid group take the mean glossy direction also when ONE glossy member produced it; group_id = slot / K in the grouped
+    modes and the path id otherwise."""
+    sc = I.checker_floor(p_diffuse=0.85)                 # mostly Lambert: many groups with exactly one glossy / mirror member
+    K = 16
+    g = _first_bounce(oracle, sc, M_REUSE)
+    mt = _member_types(sc, g).reshape(-1, K); src = g["dir_src"].reshape(-1, K); p = g["ray_to_path"].reshape(-1, K)
+    act = g["rays"]["tmax"].reshape(-1, K) >= 0
+    loc = g["local_dir"].reshape(-1, K, 3)
+    n_single = 0
+    for gi in np.nonzero(g["group_class"] == oracle.CLASS_HYBRID)[0]:
+        gl = (mt[gi] == I.MAT_GLOSSY) | (mt[gi] == I.MAT_SPECULAR)
+        valid = gl & act[gi]
+        dif = mt[gi] == I.MAT_DIFFUSE
+        if valid.sum() >= 1:
+            assert np.all(src[gi][dif & act[gi]] == -2 - gi) and (dif & act[gi]).sum() == dif.sum()
+        if valid.sum() == 1:
+            assert np.allclose(loc[gi][dif], loc[gi][valid][0], atol=1e-6)
+            n_single += 1
+    assert n_single >= 10
+    assert np.array_equal(g["group_id"], np.arange(len(g["ray_to_path"])) // K)
+    gi_ = _first_bounce(oracle, sc, M_IND)
+    assert np.array_equal(gi_["group_id"], gi_["ray_to_path"])
+    gm = _first_bounce(oracle, sc, 1)
+    assert np.array_equal(gm["group_id"], gm["ray_to_path"])
+
+
+def test_bsdf_stream_is_keyed_by_pixel_sample_and_bounce(oracle):
+    """north_star: "Philox keyed by pixel, sample and bounce" (D:R2): a Lambert path's local direction at bounce b is sample_cosine of the first two floats of
+    Philox(pixel, sample, b, BSDF; seed, frame) — checked at bounce 1 and bounce 2 (so consecutive bounces draw different numbers), 2 spp."""
+    sc = I.emissive_box(albedo=0.8)                      # closed Lambert cube: every path lives on
+    w, h, spp, seed, frame = sc.width, sc.height, 2, 6, 2
+    fr = oracle.frame(w, h, spp, seed, frame)
+    b = oracle.Bvh(sc.verts)
+    rays, hits, r2p = oracle.trace_primary(b, sc.camera, fr, M_IND)
+    paths = oracle.paths_init(spp * w * h)
+    for bounce in (1, 2):
+        g = oracle.generate_secondary(sc, fr, bounce, M_IND, 1, 1, 1, b.info()["bounds"], rays, hits, r2p, paths)
+        for path in (0, 7, w * h - 1, w * h + 5, 2 * w * h - 1):
+            r = oracle.philox(path % (w * h), path // (w * h), bounce, 1, seed, frame)
+            exp = oracle.sample_cosine(oracle.u01(r[0]), oracle.u01(r[1]))
+            assert np.array_equal(g["local_dir"][path], exp.astype(np.float32)), (bounce, path)
+        rays, r2p = g["rays"], g["ray_to_path"]
+        hits = b.trace(rays)

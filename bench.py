@@ -567,9 +567,11 @@ def run_kernels(args):
                 flush.fill_(1)
                 e0.record(); ctx.crt_trace(bvh, r, hits=hh); e1.record(); torch.cuda.synchronize()
                 ts.append(e0.elapsed_time(e1))
-            nv, nt, nr = ctx.crt_trace_stats(bvh, r)
+            nv, nt, nr, npk = ctx.crt_trace_stats(bvh, r, full=True)
             row["sets"][tag] = {"ms": float(np.median(ts)), "records_identical": bool(torch.equal(hi, ri)), "ids_equal_frac": ids_equal, "active_rays": int(nr),
                                 "node_visits_per_ray": nv / max(1, nr), "tri_tests_per_ray": nt / max(1, nr)}
+            if npk:      # trace_kernel 8: node visits of a 16-ray packet, per ray of the packet (x 16 = lane slots issued per ray's share)
+                row["sets"][tag]["packet_visits_per_16_rays"] = 16.0 * npk / max(1, nr)
         rows.append(row)
         for key in ["trace_kernel"] + touched:
             ctx.crt_set_option(key, KERNEL_OPTION_DEFAULTS[key])

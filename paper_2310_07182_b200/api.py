@@ -298,12 +298,13 @@ class Context:
         self._check(lib().crt_trace(self.handle, bvh.handle, _ptr(rays), C.c_int64(n), _ptr(hits), _stream(stream)))
         return hits
 
-    def crt_trace_stats(self, bvh, rays, stream=None):
-        """(node_visits, triangle_tests, active_rays) of one traversal of `rays` (counting variant of the kernel)."""
+    def crt_trace_stats(self, bvh, rays, stream=None, full=False):
+        """(node_visits, triangle_tests, active_rays) of one traversal of `rays` (counting variant of the kernel); full: all four counters
+        (the fourth: half-warp node visits of trace_kernel 8, else 0)."""
         cnt = torch.zeros((4,), dtype=torch.int64, device=self.device)
         self._check(lib().crt_trace_stats(self.handle, bvh.handle, _ptr(rays), C.c_int64(rays.shape[0]), _ptr(cnt), _stream(stream)))
         c = cnt.cpu().tolist()
-        return c[0], c[1], c[2]
+        return tuple(c) if full else (c[0], c[1], c[2])
 
     # ---- a6 -----------------------------------------------------------------------------------------
     def crt_shade_accumulate(self, bvh, mats, frame, bounce, is_last, rays, hits, r2p, paths, accum, stream=None):

@@ -13,7 +13,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libcrt.so")
-SOURCES = ["crt_api.cu", "trace.cu", "trace_wide.cu", "trace_queue.cu", "generate.cu", "sort.cu", "shade.cu", "bvh_build.cpp", "bvh_wide.cpp", "bvh_ploc.cu"]
+SOURCES = ["crt_api.cu", "trace.cu", "trace_wide.cu", "trace_queue.cu", "trace_group.cu", "generate.cu", "sort.cu", "shade.cu", "bvh_build.cpp", "bvh_wide.cpp", "bvh_ploc.cu"]
 # -fmad=false: the method's arithmetic is one IEEE rounding per written operation (DESIGN.md D:R0);
 # the kernels call fmaf explicitly where a fused multiply-add is wanted.
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-fmad=false",

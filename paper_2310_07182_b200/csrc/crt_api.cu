@@ -111,7 +111,7 @@ const char* crt_last_error(const crt_ctx* ctx) { return ctx ? ctx->last_error.c_
 crt_status crt_set_option(crt_ctx* ctx, const char* key, int64_t value)
 {
     if (!ctx || !key) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "set_option: null argument");
-    if (!strcmp(key, "trace_kernel")) { if (value < 0 || value > 7) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "trace_kernel must be 0..7"); ctx->trace_kernel = (int)value; }
+    if (!strcmp(key, "trace_kernel")) { if (value < 0 || value > 9) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "trace_kernel must be 0..9"); ctx->trace_kernel = (int)value; }
     else if (!strcmp(key, "trace_refill_threshold")) { if (value < 0 || value > 32) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "trace_refill_threshold out of range"); ctx->trace_refill_threshold = (int)value; }
     else if (!strcmp(key, "trace_leaf_wait")) { if (value < 0 || value > 31) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "trace_leaf_wait out of range"); ctx->trace_leaf_wait = (int)value; }
     else if (!strcmp(key, "trace_tri_wait")) { if (value < 0 || value > 32) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "trace_tri_wait out of range"); ctx->trace_tri_wait = (int)value; }

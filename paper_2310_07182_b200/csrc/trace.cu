@@ -506,6 +506,7 @@ crt_status launch_trace(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, i
     // the layout failed its own check (a plane clamped or less than one step outside its box: crt_bvh_check bit 16)
     const bool q_ok = bvh->q_inflation <= 2.0 && bvh->q_violations == 0;
     if (ctx->trace_kernel == 5 && !far_origins && trace_queue_supported(bvh)) return launch_trace_queue(ctx, bvh, rays, n, hits, nullptr, st);
+    if (ctx->trace_kernel >= 8 && !far_origins && trace_group_supported(bvh)) return launch_trace_group(ctx, bvh, rays, n, hits, nullptr, st, counter, ctx->trace_kernel == 9 ? 32 : 16);
     if (ctx->trace_kernel == 6 && !far_origins && q_ok) return launch_dyn<false, 4>(ctx, bvh, rays, n, hits, nullptr, st, counter);
     if (ctx->trace_kernel == 7 && !far_origins && q_ok && crt_bvh_ensure_q4(bvh)) return launch_dyn<false, 5>(ctx, bvh, rays, n, hits, nullptr, st, counter);
     if (ctx->trace_kernel == 3 && !ctx->trace_exact && !far_origins && q_ok) return launch_dyn<false, 3>(ctx, bvh, rays, n, hits, nullptr, st, counter);
@@ -521,6 +522,7 @@ crt_status launch_trace_stats(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* r
     if (ctx->trace_kernel == 2 && bvh->d_wnodes && bvh->wide_violations == 0) return launch_trace_wide_stats(ctx, bvh, rays, n, counters, st);
     const bool q_ok = bvh->q_inflation <= 2.0 && bvh->q_violations == 0;
     if (ctx->trace_kernel == 5 && trace_queue_supported(bvh)) return launch_trace_queue(ctx, bvh, rays, n, nullptr, reinterpret_cast<unsigned long long*>(counters), st);
+    if (ctx->trace_kernel >= 8 && trace_group_supported(bvh)) return launch_trace_group(ctx, bvh, rays, n, nullptr, reinterpret_cast<unsigned long long*>(counters), st, nullptr, ctx->trace_kernel == 9 ? 32 : 16);
     if (ctx->trace_kernel == 7 && q_ok && crt_bvh_ensure_q4(bvh)) return launch_dyn<true, 5>(ctx, bvh, rays, n, nullptr, reinterpret_cast<unsigned long long*>(counters), st);
     if (ctx->trace_kernel == 4 && q_ok) return launch_dyn<true, 2>(ctx, bvh, rays, n, nullptr, reinterpret_cast<unsigned long long*>(counters), st);
     if (ctx->trace_kernel >= 3 && q_ok) return launch_dyn<true, 1>(ctx, bvh, rays, n, nullptr, reinterpret_cast<unsigned long long*>(counters), st);

@@ -105,7 +105,7 @@ def test_full_size_config2_stagewise_and_sampled(crt, ctx, oracle):
 
 # ------------------------------------------------------------------ a0 / a5: BVH + traversal
 @pytest.mark.parametrize("scene_name", ["cornell", "interior_small", "landscape_small"])
-@pytest.mark.parametrize("kernel", [0, 1, 2, 3, 4, 5, 6, 7])
+@pytest.mark.parametrize("kernel", [0, 1, 2, 3, 4, 5, 6, 7, 8, 9])
 def test_trace_matches_oracle_on_random_rays(crt, ctx, oracle, scene_name, kernel):
     scene = SCENES[scene_name]()
     # kernel 2 reads the 8-wide compressed layout, which exists when every leaf holds one triangle

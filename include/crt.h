@@ -123,8 +123,9 @@ const char* crt_last_error(const crt_ctx* ctx);
  * 5 = warp-cooperative triangle phase: the triangles of a warp's parked leaves become one work list in shared memory, tested one
  * item per lane (same hit records; measured 15-25 % slower, profiles/r02a); 6 = as 3 with the top 512 nodes of the tree staged in shared
  * memory per block (same hit records; measured 8-16 % slower, profiles/r02a); 7 = the 4-wide form of the 16-bit nodes, two 32-byte records per node, built
- * on first use (half the node visits, same hit records; measured 5-23 % slower, profiles/r02a); 8 = group-coherent descent: the 16 rays of a
- * half-warp (one group at K = 16) walk one shared stack, a node is fetched once per packet (same hit records; profiles/r02h)), "trace_exact" (1 = default: the bit-exact triangle
+ * on first use (half the node visits, same hit records; measured 5-23 % slower, profiles/r02a); 8 / 9 = group-coherent descent: the 16 rays of a
+ * half-warp (one group at K = 16) / the 32 rays of a warp walk one shared stack, a node is fetched once per packet (same hit records; measured
+ * 1.2-6x slower, profiles/r02h)), "trace_exact" (1 = default: the bit-exact triangle
  * test of D:R0; 0 = fused multiply-adds and an approximate reciprocal in the triangle test: 3-5 % faster, ids equal on >= 99.999 % of
  * rays but t of grazing hits off by up to 4e-4 relative, i.e. outside north_star's 1e-4: an option, not the default),
  * "trace_leaf_wait" (0..31: a warp leaves its inner-node

@@ -532,7 +532,7 @@ def _frame_ray_sets(ctx, crt, scene, w, h, spp, nb, gw, gh, s, seed, frame, mode
     return bvh, (mats_dev, mats), sets
 
 
-KERNEL_OPTION_DEFAULTS = {"trace_kernel": 3, "trace_refill_threshold": 16, "trace_leaf_wait": 6, "trace_blocks_per_sm": 0, "trace_exact": 1}
+KERNEL_OPTION_DEFAULTS = {"trace_kernel": 3, "trace_refill_threshold": 16, "trace_leaf_wait": 6, "trace_blocks_per_sm": 0, "trace_exact": 1, "trace_tail_split": 0}
 
 
 def run_kernels(args):
@@ -626,6 +626,42 @@ def run_builders(args):
                          + " | ".join(f"{row['sets'][t]['ms']:.3f}{'' if row['sets'][t]['records_identical'] else ' !'}" for t in tags) + " |\n")
 
 
+def run_timeline(args):
+    """What the tail of a persistent crt_trace launch consists of (profiles/r02i): crt_trace_timeline (the default kernel with four time marks
+    per warp) on the three direct_reuse ray sets of one frame of --workload, with and without trace_tail_split; L2 flushed, third repetition.
+    All times in microseconds after the first warp's start.  One JSON line."""
+    import torch
+    import paper_2310_07182_b200 as crt
+    import crt_inputs as I
+    name, kw, w, h, spp, nb, gw, gh, s, seed, cfg = WORKLOADS[args.workload]
+    scene = I.by_name(name, **kw).with_camera(w, h)
+    ctx = crt.Context(0)
+    bvh, _keep, sets = _frame_ray_sets(ctx, crt, scene, w, h, spp, nb, gw, gh, s, seed, 7)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=ctx.device)
+    rows = []
+    for split in (0, 1):
+        ctx.crt_set_option("trace_tail_split", split)
+        for tag, r in sets[:3]:
+            ref = ctx.crt_trace(bvh, r).clone()
+            for _ in range(3):
+                flush.fill_(1); hh, marks = ctx.crt_trace_timeline(bvh, r); torch.cuda.synchronize()
+            t0 = marks[:, 0].min()
+            start, exh, end = (marks[:, 0] - t0) / 1e3, (marks[:, 1] - t0) / 1e3, (marks[:, 2] - t0) / 1e3
+            seen = marks[:, 1] > 0
+            first_exh = float(exh[seen].min()) if seen.any() else float("nan")
+            rows.append({"tail_split": split, "set": tag, "warps": int(marks.shape[0]), "records_identical": bool(torch.equal(hh.view(torch.int32), ref.view(torch.int32))),
+                         "span_us": float(end.max()), "last_warp_start_us": float(start.max()), "ray_list_exhausted_first_seen_us": first_exh, "last_seen_us": float(exh[seen].max()) if seen.any() else float("nan"),
+                         "warp_end_us_p10_p50_p90_p99_max": [float(np.percentile(end, q)) for q in (10, 50, 90, 99, 100)],
+                         "tail_us": float(end.max()) - first_exh,
+                         "lane_visits_after_exhaustion_p50_p90_max": [float(np.percentile(marks[:, 3], 50)), float(np.percentile(marks[:, 3], 90)), float(marks[:, 3].max())]})
+    ctx.crt_set_option("trace_tail_split", KERNEL_OPTION_DEFAULTS["trace_tail_split"])
+    print(json.dumps({"clocks": _SWEEP_CLOCKS.stop() if _SWEEP_CLOCKS else None, "timeline": rows, "config": {"workload": args.workload, "order": f"direct_reuse {gw}x{gh} stride {s}", "frame": 7,
+                                                   "timing": "per-warp %globaltimer marks inside the kernel (crt_trace_timeline), third repetition, 256 MB L2 flush before each"}}))
+    for row in rows:
+        sys.stderr.write(f"split {row['tail_split']} {row['set']}: span {row['span_us']:.1f} us, list exhausted at {row['ray_list_exhausted_first_seen_us']:.1f}, warp ends p10/p50/p90/p99/max "
+                         + "/".join(f"{x:.1f}" for x in row["warp_end_us_p10_p50_p90_p99_max"]) + f", tail {row['tail_us']:.1f} us, visits after exhaustion p50/p90/max " + "/".join(f"{x:.0f}" for x in row["lane_visits_after_exhaustion_p50_p90_max"]) + "\n")
+
+
 def run_tail(args):
     """Fixed cost of a crt_trace launch (profiles/r01h): crt_trace on one frame's ray sets (primary, bounce 1, bounce 2; direct_reuse order)
     and on the same set concatenated twice and four times; L2 flushed between repetitions, median of 8.  One JSON line."""
@@ -678,8 +714,8 @@ def main():
     ap.add_argument("--set", nargs="*", default=[], metavar="OPTION=VALUE", help="crt_set_option on every context of the run (experiments; the defaults are what the driver times)")
     ap.add_argument("--repeats", type=int, default=1, help="repeat the K timed steps of direct_reuse / independent / morton_reorder this many times and report min / median / max")
     ap.add_argument("--no-sort-codes", action="store_true", help="skip the Origin / Reis / Costa / TwoPoint reordering baselines")
-    ap.add_argument("--sweep", nargs="?", const="config3", default=None, choices=["config3", "table3", "rules", "tail", "kernels", "builders"],
-                    help="config3: BASELINE config 3 sweep; table3: the paper's Table 3 shapes (tile x K) at 1920x1080, 1 spp, 2 bounces; rules: shuffled against lattice partition at the same size; tail: fixed cost of a crt_trace launch (n, 2n, 4n rays) on --workload; kernels: A/B of traversal kernel variants (--variants) on one frame's ray sets of --workload; builders: host SAH against device PLOC BVH builder on --workload")
+    ap.add_argument("--sweep", nargs="?", const="config3", default=None, choices=["config3", "table3", "rules", "tail", "kernels", "builders", "timeline"],
+                    help="config3: BASELINE config 3 sweep; table3: the paper's Table 3 shapes (tile x K) at 1920x1080, 1 spp, 2 bounces; rules: shuffled against lattice partition at the same size; tail: fixed cost of a crt_trace launch (n, 2n, 4n rays) on --workload; kernels: A/B of traversal kernel variants (--variants) on one frame's ray sets of --workload; timeline: per-warp time marks of a crt_trace launch (what its tail consists of); builders: host SAH against device PLOC BVH builder on --workload")
     ap.add_argument("--ploc-radii", nargs="*", type=int, default=[8], help="--sweep builders: neighbour radii of the device builder")
     ap.add_argument("--variants", nargs="*", default=["3", "3:trace_exact=0", "5", "6", "4", "1"], help="--sweep kernels: trace_kernel id[:option=value,...] ...")
     ap.add_argument("--sweep-frames", type=int, default=64)
@@ -695,6 +731,9 @@ def main():
         return
     if args.sweep == "kernels":
         run_kernels(args)
+        return
+    if args.sweep == "timeline":
+        run_timeline(args)
         return
     if args.sweep == "builders":
         run_builders(args)

@@ -128,6 +128,8 @@ const char* crt_last_error(const crt_ctx* ctx);
  * 1.2-6x slower, profiles/r02h)), "trace_exact" (1 = default: the bit-exact triangle
  * test of D:R0; 0 = fused multiply-adds and an approximate reciprocal in the triangle test: 3-5 % faster, ids equal on >= 99.999 % of
  * rays but t of grazing hits off by up to 4e-4 relative, i.e. outside north_star's 1e-4: an option, not the default),
+ * "trace_tail_split" (0 = default; 1: once the ray list is exhausted, idle lanes of a warp take over the bottom stack entries of its busy lanes;
+ * same hit records; the drain of a launch gets no shorter and the node loop 8 % slower, profiles/r02i),
  * "trace_leaf_wait" (0..31: a warp leaves its inner-node
  * phase when at most this many descending lanes hold no leaf), "trace_refill_threshold" (0..32: idle lanes fetch new rays when
  * fewer lanes than this are busy), "trace_blocks_per_sm" (0 = from the occupancy calculator), "trace_tri_wait" (8-wide kernel: lanes holding triangle hits
@@ -217,6 +219,13 @@ crt_status crt_trace(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int6
  * node fetched and its two child boxes tested), [1] triangle tests, [2] active rays, [3] trace_kernel 8 only: node visits of
  * the 16-ray packets (one per half-warp and node; [0] then counts the lanes inside each visited node's box). */
 crt_status crt_trace_stats(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n_rays, int64_t* counters, void* stream);
+
+/* Diagnostic: crt_trace with the default kernel (16-bit nodes) plus four time marks per warp of the launch, for reading the tail of a
+ * persistent launch (profiles/r02i).  marks: [device] uint64[4 * marks_capacity_warps]; warp w writes [4w] start, [4w+1] the moment it first
+ * saw the ray list exhausted (0: never), [4w+2] end (all %globaltimer, ns), [4w+3] the largest number of node visits one of its lanes made
+ * after [4w+1].  *n_warps (host) = warps of the launch; CRT_ERR_INVALID_ARG if the buffer is too small (148 SMs x 8 blocks x 4 warps fit in 4736). */
+crt_status crt_trace_timeline(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n_rays, crt_hit* hits,
+                              uint64_t* marks, int64_t marks_capacity_warps, int32_t* n_warps, void* stream);
 
 /* ---- a6: shading and accumulation (D:R14) --------------------------------------------- */
 /* For the segment just traced: miss -> radiance += throughput*env(d), path ends; emissive hit -> radiance +=

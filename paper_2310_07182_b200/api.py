@@ -33,7 +33,7 @@ EXPORTS = [
     "crt_create", "crt_destroy", "crt_last_error", "crt_set_option", "crt_measure_peaks",
     "crt_build_bvh", "crt_bvh_destroy", "crt_bvh_get_info", "crt_bvh_check", "crt_layout", "crt_paths_init",
     "crt_trace_primary", "crt_generate_secondary", "crt_generate_secondary_scratch_bytes",
-    "crt_morton_encode", "crt_ray_code_encode", "crt_radix_sort_pairs", "crt_radix_sort_scratch_bytes", "crt_trace", "crt_trace_stats",
+    "crt_morton_encode", "crt_ray_code_encode", "crt_radix_sort_pairs", "crt_radix_sort_scratch_bytes", "crt_trace", "crt_trace_stats", "crt_trace_timeline",
     "crt_shade_accumulate", "crt_render_frame", "crt_frame_workspace_bytes", "crt_frame_times", "crt_frame_bounce_times",
     "crt_render_frame_host", "crt_render_frame_host_resident", "crt_render_frame_host_resident_async", "crt_frame_host_extra_bytes",
 ]
@@ -305,6 +305,18 @@ class Context:
         self._check(lib().crt_trace_stats(self.handle, bvh.handle, _ptr(rays), C.c_int64(rays.shape[0]), _ptr(cnt), _stream(stream)))
         c = cnt.cpu().tolist()
         return tuple(c) if full else (c[0], c[1], c[2])
+
+    def crt_trace_timeline(self, bvh, rays, hits=None, stream=None):
+        """crt_trace with per-warp time marks: returns (hits, marks) with marks an int64 array [n_warps, 4] on the host:
+        start ns, ray-list-exhausted ns (0: never seen), end ns, largest number of node visits of a lane after exhaustion."""
+        n = rays.shape[0]
+        if hits is None:
+            hits = self.empty((n, 4))
+        cap = 148 * 8 * 4 * 2
+        marks = torch.zeros((cap, 4), dtype=torch.int64, device=self.device)
+        nw = C.c_int32(0)
+        self._check(lib().crt_trace_timeline(self.handle, bvh.handle, _ptr(rays), C.c_int64(n), _ptr(hits), _ptr(marks), C.c_int64(cap), C.byref(nw), _stream(stream)))
+        return hits, marks[: nw.value].cpu().numpy()
 
     # ---- a6 -----------------------------------------------------------------------------------------
     def crt_shade_accumulate(self, bvh, mats, frame, bounce, is_last, rays, hits, r2p, paths, accum, stream=None):

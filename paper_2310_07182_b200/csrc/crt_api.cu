@@ -117,6 +117,7 @@ crt_status crt_set_option(crt_ctx* ctx, const char* key, int64_t value)
     else if (!strcmp(key, "trace_tri_wait")) { if (value < 0 || value > 32) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "trace_tri_wait out of range"); ctx->trace_tri_wait = (int)value; }
     else if (!strcmp(key, "fuse_shade")) { ctx->fuse_shade = value != 0; }
     else if (!strcmp(key, "trace_exact")) { ctx->trace_exact = value != 0; }
+    else if (!strcmp(key, "trace_tail_split")) { ctx->trace_tail_split = value != 0; }
     else if (!strcmp(key, "shade_pixel_order")) { ctx->shade_pixel_order = value != 0; }
     else if (!strcmp(key, "frame_bands")) { if (value < 1 || value > 4) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "frame_bands must be 1..4"); ctx->frame_bands = (int)value; }
     else if (!strcmp(key, "trace_blocks_per_sm")) { if (value < 0 || value > 32) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "trace_blocks_per_sm out of range"); ctx->trace_blocks_per_sm = (int)value; }
@@ -353,6 +354,17 @@ crt_status crt_trace(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int6
     if (n_rays >= ((int64_t)1 << 31)) return crt_fail(ctx, CRT_ERR_UNSUPPORTED, "trace: more than 2^31 rays per call");
     NEED_ALIGNED("trace", rays, 32); NEED_ALIGNED("trace", hits, 16);
     return launch_trace(ctx, bvh, rays, n_rays, hits, (cudaStream_t)stream);
+}
+
+crt_status crt_trace_timeline(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n_rays, crt_hit* hits, uint64_t* marks, int64_t marks_capacity_warps, int32_t* n_warps, void* stream)
+{
+    NEED_CTX("trace_timeline"); NEED_BVH("trace_timeline");
+    if (!n_warps || !marks || marks_capacity_warps < 0) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "trace_timeline: null argument");
+    if (n_rays < 0 || n_rays >= ((int64_t)1 << 31)) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "trace_timeline: bad ray count");
+    NEED_ALIGNED("trace_timeline", marks, 8);
+    if (n_rays == 0) { *n_warps = 0; return CRT_OK; }
+    NEED_ALIGNED("trace_timeline", rays, 32); NEED_ALIGNED("trace_timeline", hits, 16);
+    return launch_trace_timeline(ctx, bvh, rays, n_rays, hits, marks, marks_capacity_warps, n_warps, (cudaStream_t)stream);
 }
 
 crt_status crt_trace_stats(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n_rays, int64_t* counters, void* stream)

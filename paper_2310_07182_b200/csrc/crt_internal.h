@@ -19,6 +19,7 @@ struct crt_ctx {
     int trace_tri_wait = 8;            // wide kernel: a warp enters its triangle phase when at least this many lanes hold triangle hits
     int trace_blocks_per_sm = 0; // 0 = from occupancy
     int shade_pixel_order = 1;   // crt_render_frame, grouped orders: the last segment's shading walks the tile in pixel order (coalesced image updates)
+    int trace_tail_split = 0;    // default kernel: in the drain phase of a launch idle lanes take over stack entries of their warp's busy lanes (trace.cu)
     int trace_exact = 1;         // 1: the bit-exact triangle test (D:R0); 0: fused multiply-adds + approximate reciprocal (north_star's tolerances only)
     int fuse_shade = 1;          // crt_render_frame: shade non-final segments inside the next generation kernel (default; measured: DESIGN.md 5.4)
     // persistent-kernel work counters (one per band of a frame, 64 bytes apart) and, 1 KB in, the per-bounce live-ray counts of a banded frame
@@ -137,6 +138,7 @@ bool crt_bvh_ensure_q4(const crt_bvh* b);
 crt_status launch_trace(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, crt_hit* hits, cudaStream_t st, bool far_origins = false, unsigned int* counter = nullptr);
 bool trace_queue_supported(const crt_bvh* bvh);
 crt_status launch_trace_queue(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, crt_hit* hits, unsigned long long* stats, cudaStream_t st);
+crt_status launch_trace_timeline(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, crt_hit* hits, uint64_t* marks, int64_t max_warps, int32_t* n_warps, cudaStream_t st);
 bool trace_group_supported(const crt_bvh* bvh);
 crt_status launch_trace_group(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, crt_hit* hits, unsigned long long* stats, cudaStream_t st, unsigned int* counter, int group);
 crt_status launch_trace_wide(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, crt_hit* hits, cudaStream_t st);

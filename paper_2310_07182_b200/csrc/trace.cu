@@ -41,6 +41,8 @@ constexpr int TREELET_NODES = 512;             // QN 4: nodes 0 .. 511 (the top 
 #define CRT_VISITS_PER_VOTE 3   // inner-node visits between two leaf-wait votes of a warp
 #endif
 
+CRT_DEV unsigned long long globaltimer_ns() { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
+
 struct ChildRegs { float min_x, max_x, min_y, max_y, min_z, max_z; int ref; };
 
 // one 32-byte child record through the non-coherent path (LDG.E.ENL2.256.CONSTANT)
@@ -283,8 +285,9 @@ CRT_DEV int visit_q4node(const QNode* __restrict__ q4, int idx, const RayState& 
 }
 
 // Tests the triangles of a leaf reference (D:R10 tie-break: lower primitive id wins at equal t).
-template <bool COUNT, bool FAST = false>
-CRT_DEV void visit_leaf(const GpuTri* __restrict__ tris, int ref, RayState& r, unsigned& n_tris, crt_hit* __restrict__ hits, int ray_idx)
+// SPLIT (tail splitting, see trace_dyn_kernel): a lane that works on a subtree of ANOTHER lane's ray (ray_idx <= -2) keeps u, v in aux[0..1]
+template <bool COUNT, bool FAST = false, bool SPLIT = false>
+CRT_DEV void visit_leaf(const GpuTri* __restrict__ tris, int ref, RayState& r, unsigned& n_tris, crt_hit* __restrict__ hits, int ray_idx, int* aux = nullptr)
 {
     const int leaf = ~ref;
     const int first = leaf >> 3, cnt = (leaf & 7) + 1;
@@ -302,7 +305,10 @@ CRT_DEV void visit_leaf(const GpuTri* __restrict__ tris, int ref, RayState& r, u
             const int prim = __float_as_int(a.w);
             if (t < r.best.t || (t == r.best.t && r.best.prim >= 0 && prim < r.best.prim)) {
                 r.best.t = t; r.best.prim = prim;
-                if (!COUNT) reinterpret_cast<float4*>(hits)[ray_idx] = make_float4(t, u, v, __int_as_float(prim));
+                if (!COUNT) {
+                    if (!SPLIT || ray_idx >= 0) reinterpret_cast<float4*>(hits)[ray_idx] = make_float4(t, u, v, __int_as_float(prim));
+                    else { aux[0] = __float_as_int(u); aux[1] = __float_as_int(v); }
+                }
             }
         }
     }
@@ -336,7 +342,17 @@ __global__ void __launch_bounds__(TRACE_BLOCK) trace_flat_kernel(const GpuNode* 
 
 // variant 1 (default): persistent warps, per-lane dynamic ray fetch, postponed leaves.  COUNT adds work counters.
 // 9 blocks/SM (<= 56 registers, 36 warps): measured faster than 8 blocks at 64 registers and 10 blocks at 48 (profiles/).
-template <bool COUNT, int QN>
+// SPLIT (trace_tail_split, default on): once the ray list is exhausted, the tail of the launch is a few long rays, each a serial chain of
+// dependent node fetches on one lane while the other lanes of its warp idle (measured: the last 1 % of the warps end 45 us after the 99th
+// percentile, 0.3 us per visit; profiles/r02i).  In that phase an idle lane takes over the BOTTOM entry of a busy lane's stack (the
+// earliest pushed = largest postponed subtree) together with a copy of its ray and traverses it concurrently.  The closest hit with the
+// (t, id) rule of D:R10 does not depend on who finds it or in which order: a helper keeps its candidate in registers (u, v in local
+// memory) and, when its subtree is done, writes it to the ray's record if it beats what the record holds (the record is initialised when
+// the ray first gives work away; all lanes of a ray are in ONE warp and deliveries happen at a warp-wide point of the loop, so there is no
+// concurrent writer); the lanes still working on that ray adopt the delivered t as their pruning bound.
+// TIMELINE (crt_trace_timeline): the same traversal with four marks per warp written to `stats` at the end: [0] start, [1] the moment the warp
+// first saw the ray list exhausted, [2] end (globaltimer, ns), [3] the largest number of node visits one of its lanes made after [1].
+template <bool COUNT, int QN, bool SPLIT, bool TIMELINE = false>
 __global__ void __launch_bounds__(TRACE_BLOCK, CRT_TRACE_MINB(QN)) trace_dyn_kernel(const GpuNode* __restrict__ nodes, const QNode* __restrict__ qnodes, const QGrid grid, const GpuTri* __restrict__ tris,
                                                                 const crt_ray* __restrict__ rays, crt_hit* __restrict__ hits, int64_t n,
                                                                 unsigned int* __restrict__ counter, int refill_threshold, int leaf_wait,
@@ -348,17 +364,41 @@ __global__ void __launch_bounds__(TRACE_BLOCK, CRT_TRACE_MINB(QN)) trace_dyn_ker
         for (int i = threadIdx.x; i < 2 * TREELET_NODES; i += blockDim.x) s_treelet[i] = i < 2 * n_qnodes ? reinterpret_cast<const uint4*>(qnodes)[i] : make_uint4(0u, 0u, 0u, 0u);
         __syncthreads();
     }
-    int stack[STACK_SIZE]; int* top = stack; stack[0] = SENTINEL;      // top: pointer to the top entry (no index-to-address LEA per push/pop)
+    int stack[STACK_SIZE + 4]; int* top = stack; stack[0] = SENTINEL;      // top: pointer to the top entry (no index-to-address LEA per push/pop)
+    int* const aux = stack + STACK_SIZE;      // SPLIT: [0], [1] = u, v of a helper's candidate; [2] = bot: stack[bot] is this lane's sentinel (entries below were given away); [3] = the hit id a helper started from
+    if (SPLIT) aux[2] = 0;
     int node = SENTINEL, leaf = 0;      // leaf: postponed leaf reference (< 0) or 0 = none
-    int ray_idx = -1;
-    bool exhausted = false;
+    int ray_idx = -1;                   // SPLIT: <= -2 = helper of ray -2 - ray_idx
+    bool exhausted = false, tail = false;
     RayState r; QRay<QN == 2> q; QRay2 q2;
     unsigned c_nodes = 0, c_tris = 0, c_rays = 0;
+    unsigned long long tl_start = 0, tl_exhausted = 0; unsigned tl_visits = 0;
+    if (TIMELINE) tl_start = globaltimer_ns();
 
     for (;;) {
         __syncwarp();
         // ---- retire finished rays; idle lanes take the next rays in slot order (warp-wide: one atomic per round)
-        if (node == SENTINEL && ray_idx >= 0) { if (!COUNT && r.best.prim < 0) store_miss(hits, ray_idx, r.best.t); ray_idx = -1; }
+        if (node == SENTINEL && ray_idx >= 0) { if (!COUNT && r.best.prim < 0) store_miss(hits, ray_idx, r.best.t); ray_idx = -1; }      // (a helper, ray_idx <= -2, is retired by its delivery below)
+        if (SPLIT && tail) {      // helpers whose subtree is done deliver their candidate
+            unsigned fin = __ballot_sync(0xffffffffu, node == SENTINEL && ray_idx <= -2);
+            while (fin) {
+                const int h = __ffs(fin) - 1; fin &= fin - 1u;
+                const float ht = __shfl_sync(0xffffffffu, r.best.t, h);
+                const int hp = __shfl_sync(0xffffffffu, r.best.prim, h), hid = -2 - __shfl_sync(0xffffffffu, ray_idx, h);
+                if ((int)lane == h) {
+                    if (hp >= 0 && hp != aux[3]) {      // its own find (aux[3]: the id it started from or adopted; the subtrees of a ray's lanes are disjoint)
+                        float4* rec = reinterpret_cast<float4*>(hits) + hid;
+                        float rt; int rp;
+                        asm volatile("ld.volatile.global.f32 %0, [%1];" : "=f"(rt) : "l"(rec));
+                        asm volatile("ld.volatile.global.s32 %0, [%1+12];" : "=r"(rp) : "l"(rec));
+                        if (ht < rt || (ht == rt && rp >= 0 && hp < rp)) *rec = make_float4(ht, __int_as_float(aux[0]), __int_as_float(aux[1]), __int_as_float(hp));
+                    }
+                    ray_idx = -1;
+                } else if (node != SENTINEL && (ray_idx >= 0 ? ray_idx : -2 - ray_idx) == hid && hp >= 0 &&
+                           (ht < r.best.t || (ht == r.best.t && r.best.prim >= 0 && hp < r.best.prim))) { r.best.t = ht; r.best.prim = hp; if (ray_idx <= -2) aux[3] = hp; }
+                __syncwarp();
+            }
+        }
         for (;;) {
             const bool want = (node == SENTINEL) && !exhausted;
             const unsigned m = __ballot_sync(0xffffffffu, want);
@@ -382,17 +422,48 @@ __global__ void __launch_bounds__(TRACE_BLOCK, CRT_TRACE_MINB(QN)) trace_dyn_ker
                         if (QN) q.init(r, grid);
                         if (QN == 1 || QN >= 3) q2.init(q);
                         ray_idx = (int)i; node = 0; leaf = 0; top = stack;
+                        if (SPLIT) aux[2] = 0;
                         if (COUNT) ++c_rays;
                     }
                 }
             }
         }
         if (__ballot_sync(0xffffffffu, node != SENTINEL) == 0u) break;     // every lane idle and the ray list is exhausted
-        if (__any_sync(0xffffffffu, exhausted)) refill_threshold = 0;      // nothing left to fetch: run the stragglers to the end
+        if (TIMELINE && tl_exhausted == 0 && __any_sync(0xffffffffu, exhausted)) tl_exhausted = globaltimer_ns();
+        if (__any_sync(0xffffffffu, exhausted)) { tail = true; refill_threshold = SPLIT ? 32 : 0; }      // nothing left to fetch: run the stragglers to the end (SPLIT: come back here whenever a lane falls idle)
+        if (SPLIT && tail) {
+            unsigned lt_mask; asm volatile("mov.u32 %0, %%lanemask_lt;" : "=r"(lt_mask));
+            // (2) the k-th idle lane takes the bottom stack entry of the k-th lane that has one
+            const unsigned idle = __ballot_sync(0xffffffffu, node == SENTINEL);
+            const unsigned donors = __ballot_sync(0xffffffffu, node != SENTINEL && (int)(((unsigned)__cvta_generic_to_local(top) - (unsigned)__cvta_generic_to_local(stack)) >> 2) > aux[2]);      // (local-window offsets: a generic pointer difference makes the compiler carry a 64-bit copy of top through the node loop)
+            const int n_pairs = min(__popc(idle), __popc(donors));
+            if (n_pairs > 0) {
+                const bool take = (idle >> lane & 1u) && __popc(idle & lt_mask) < n_pairs, give = (donors >> lane & 1u) && __popc(donors & lt_mask) < n_pairs;
+                int e = 0;
+                if (give) {
+                    if (ray_idx >= 0 && r.best.prim < 0) store_miss(hits, ray_idx, r.best.t);      // the record a helper will compare with
+                    const int bot = aux[2];
+                    e = stack[bot + 1]; stack[bot + 1] = SENTINEL; aux[2] = bot + 1;
+                }
+                const int src = take ? (int)__fns(donors, 0u, __popc(idle & lt_mask) + 1) : (int)lane;
+                const float4 ro = make_float4(__shfl_sync(0xffffffffu, r.o.x, src), __shfl_sync(0xffffffffu, r.o.y, src), __shfl_sync(0xffffffffu, r.o.z, src), __shfl_sync(0xffffffffu, r.tmin, src));
+                const float4 rd = make_float4(__shfl_sync(0xffffffffu, r.d.x, src), __shfl_sync(0xffffffffu, r.d.y, src), __shfl_sync(0xffffffffu, r.d.z, src), __shfl_sync(0xffffffffu, r.best.t, src));
+                const int bp = __shfl_sync(0xffffffffu, r.best.prim, src), didx = __shfl_sync(0xffffffffu, ray_idx, src);
+                e = __shfl_sync(0xffffffffu, e, src);
+                if (take) {
+                    r.init(ro, rd); r.best.prim = bp;
+                    if (QN) q.init(r, grid);
+                    if (QN == 1 || QN >= 3) q2.init(q);
+                    ray_idx = didx >= 0 ? -2 - didx : didx;
+                    top = stack; aux[2] = 0; aux[3] = bp; leaf = 0; node = e;
+                    if (e < 0) { leaf = e; node = SENTINEL; }      // a leaf reference: goes straight to the triangle phase
+                }
+            }
+        }
 
         // ---- traverse until this lane's ray ends or too few lanes of the warp are still busy
         // (a warp-uniform formulation of these loops, every exit a full-mask vote, was measured 3-10 % slower: profiles/r01f)
-        while (node != SENTINEL) {
+        while (node != SENTINEL || (SPLIT && leaf < 0)) {
             // inner nodes; the first leaf a lane meets is postponed so that the warp's leaves are processed together
             // (two visits per vote: the vote and its warp synchronisation cost 7 issue slots)
             while ((unsigned)node < (unsigned)SENTINEL) {
@@ -400,6 +471,7 @@ __global__ void __launch_bounds__(TRACE_BLOCK, CRT_TRACE_MINB(QN)) trace_dyn_ker
                 for (int rep = 0; rep < CRT_VISITS_PER_VOTE; ++rep) {
                     if (rep > 0 && (unsigned)node >= (unsigned)SENTINEL) break;
                     if (COUNT) ++c_nodes;
+                    if (TIMELINE && tl_exhausted) ++tl_visits;
                     node = QN == 5 ? visit_q4node(qnodes, node, r, q2, top) : QN == 4 ? visit_qnode2<true>(qnodes, s_treelet, node, r, q2, top) : ((QN == 1 || QN == 3) ? visit_qnode2<false>(qnodes, nullptr, node, r, q2, top) : (QN ? visit_qnode(qnodes, node, r, q, top) : visit_node(load_node(nodes, node), r, top)));
                     if (node < 0 && leaf == 0) { leaf = node; node = *top--; }
                 }
@@ -407,11 +479,19 @@ __global__ void __launch_bounds__(TRACE_BLOCK, CRT_TRACE_MINB(QN)) trace_dyn_ker
             }
             // leaves: the postponed one, then any further leaf references that come off the stack
             while (leaf < 0) {
-                visit_leaf<COUNT, QN == 3>(tris, leaf, r, c_tris, hits, ray_idx);
+                visit_leaf<COUNT, QN == 3, SPLIT>(tris, leaf, r, c_tris, hits, ray_idx, aux);
                 leaf = 0;
                 if (node < 0) { leaf = node; node = *top--; }
             }
             if (__popc(__activemask()) < refill_threshold) break;
+        }
+    }
+    if (TIMELINE) {
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) tl_visits = max(tl_visits, __shfl_xor_sync(0xffffffffu, tl_visits, d));
+        if (lane == 0) {
+            unsigned long long* o = stats + 4 * ((size_t)blockIdx.x * (TRACE_BLOCK / 32) + (threadIdx.x >> 5));
+            o[0] = tl_start; o[1] = tl_exhausted; o[2] = globaltimer_ns(); o[3] = tl_visits;
         }
     }
     if (COUNT) {
@@ -463,19 +543,23 @@ __global__ void __launch_bounds__(256) primary_rays_kernel(CamDev cam, DevLayout
     rp[1] = make_float4(dx, dy, dz, 1e30f);
 }
 
-template <bool COUNT, int QN>
-crt_status launch_dyn(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, crt_hit* hits, unsigned long long* stats, cudaStream_t st, unsigned int* counter = nullptr)
+template <bool COUNT, int QN, bool SPLIT = false, bool TIMELINE = false>
+crt_status launch_dyn(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, crt_hit* hits, unsigned long long* stats, cudaStream_t st, unsigned int* counter = nullptr, int64_t max_warps = 0, int32_t* n_warps = nullptr)
 {
     int per_sm = ctx->trace_blocks_per_sm;
     if (per_sm <= 0) {
-        CRT_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, trace_dyn_kernel<COUNT, QN>, TRACE_BLOCK, QN == 4 ? (size_t)TREELET_NODES * 32 : (size_t)0));
+        CRT_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, trace_dyn_kernel<COUNT, QN, SPLIT, TIMELINE>, TRACE_BLOCK, QN == 4 ? (size_t)TREELET_NODES * 32 : (size_t)0));
         if (per_sm < 1) per_sm = 1;
     }
     if (!counter) counter = ctx->d_counter;
     CRT_CUDA(ctx, cudaMemsetAsync(counter, 0, sizeof(unsigned int), st));
     int64_t want = (n + TRACE_BLOCK - 1) / TRACE_BLOCK, grid = (int64_t)ctx->n_sms * per_sm;
     if (grid > want) grid = want;
-    trace_dyn_kernel<COUNT, QN><<<(unsigned)grid, TRACE_BLOCK, QN == 4 ? (size_t)TREELET_NODES * 32 : (size_t)0, st>>>(bvh->d_nodes, QN == 5 ? bvh->d_q4nodes : bvh->d_qnodes, bvh->qgrid, bvh->d_tris, rays, hits, n, counter, ctx->trace_refill_threshold, ctx->trace_leaf_wait, stats, (int)bvh->n_gpu_nodes);
+    if (TIMELINE) {
+        if (grid * (TRACE_BLOCK / 32) > max_warps) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "trace_timeline: marks buffer holds %lld warps, the launch has %lld", (long long)max_warps, (long long)(grid * (TRACE_BLOCK / 32)));
+        *n_warps = (int32_t)(grid * (TRACE_BLOCK / 32));
+    }
+    trace_dyn_kernel<COUNT, QN, SPLIT, TIMELINE><<<(unsigned)grid, TRACE_BLOCK, QN == 4 ? (size_t)TREELET_NODES * 32 : (size_t)0, st>>>(bvh->d_nodes, QN == 5 ? bvh->d_q4nodes : bvh->d_qnodes, bvh->qgrid, bvh->d_tris, rays, hits, n, counter, ctx->trace_refill_threshold, ctx->trace_leaf_wait, stats, (int)bvh->n_gpu_nodes);
     CRT_CHECK_LAUNCH(ctx, "trace_dyn");
     return CRT_OK;
 }
@@ -511,8 +595,18 @@ crt_status launch_trace(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, i
     if (ctx->trace_kernel == 7 && !far_origins && q_ok && crt_bvh_ensure_q4(bvh)) return launch_dyn<false, 5>(ctx, bvh, rays, n, hits, nullptr, st, counter);
     if (ctx->trace_kernel == 3 && !ctx->trace_exact && !far_origins && q_ok) return launch_dyn<false, 3>(ctx, bvh, rays, n, hits, nullptr, st, counter);
     if ((ctx->trace_kernel == 4 || (ctx->trace_kernel >= 3 && far_origins)) && q_ok) return launch_dyn<false, 2>(ctx, bvh, rays, n, hits, nullptr, st, counter);
-    if (ctx->trace_kernel >= 3 && q_ok) return launch_dyn<false, 1>(ctx, bvh, rays, n, hits, nullptr, st, counter);
+    if (ctx->trace_kernel >= 3 && q_ok) return ctx->trace_tail_split ? launch_dyn<false, 1, true>(ctx, bvh, rays, n, hits, nullptr, st, counter) : launch_dyn<false, 1>(ctx, bvh, rays, n, hits, nullptr, st, counter);
     return launch_dyn<false, 0>(ctx, bvh, rays, n, hits, nullptr, st, counter);
+}
+
+// crt_trace_timeline: the default kernel (16-bit nodes) with per-warp time marks
+crt_status launch_trace_timeline(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, crt_hit* hits, uint64_t* marks, int64_t max_warps, int32_t* n_warps, cudaStream_t st)
+{
+    *n_warps = 0;
+    if (n == 0) return CRT_OK;
+    if (!(bvh->q_inflation <= 2.0 && bvh->q_violations == 0)) return crt_fail(ctx, CRT_ERR_UNSUPPORTED, "trace_timeline: needs the 16-bit node layout");
+    return ctx->trace_tail_split ? launch_dyn<false, 1, true, true>(ctx, bvh, rays, n, hits, reinterpret_cast<unsigned long long*>(marks), st, nullptr, max_warps, n_warps)
+                                 : launch_dyn<false, 1, false, true>(ctx, bvh, rays, n, hits, reinterpret_cast<unsigned long long*>(marks), st, nullptr, max_warps, n_warps);
 }
 
 // counting build of the default kernel (crt_trace_stats): same traversal, no hit records written

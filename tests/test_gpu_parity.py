@@ -200,6 +200,36 @@ def test_trace_tolerance_only_triangle_test(crt, ctx, oracle):
     assert np.median(np.abs(h["t"][m].astype(np.float64) - ho["t"][m]) / np.abs(ho["t"][m])) < 1e-6
 
 
+@pytest.mark.parametrize("scene_name", ["cornell", "interior_small", "landscape_small"])
+@pytest.mark.parametrize("n", [20037, 900, 33])
+def test_trace_tail_split_and_timeline(crt, ctx, oracle, scene_name, n):
+    """Option trace_tail_split = 1 (idle lanes take over stack entries of their warp's busy lanes once the ray list is exhausted; measured no
+    faster, profiles/r02i): the hit records are those of the default kernel and of the oracle, bit for bit.  Small n: the whole launch is tail.
+    crt_trace_timeline: same records, and marks that are ordered in time."""
+    import torch
+    scene = SCENES[scene_name]()
+    G = GpuScene(crt, scene, ctx)
+    info = G.bvh.info()
+    r = I.random_rays(11, n, info["bounds"][:3], info["bounds"][3:], inactive_frac=0.05)
+    rd = ctx.upload(r)
+    ho = oracle.Bvh(scene.verts).trace(r.view(oracle.RAY_DTYPE).reshape(-1))
+    h0 = ctx.crt_trace(G.bvh, rd).clone()
+    for split in (1, 0):
+        ctx.crt_set_option("trace_tail_split", split)
+        try:
+            h1 = ctx.crt_trace(G.bvh, rd).clone()
+            h2, marks = ctx.crt_trace_timeline(G.bvh, rd)
+        finally:
+            ctx.crt_set_option("trace_tail_split", 0)
+        assert torch.equal(h0.view(torch.int32), h1.view(torch.int32))
+        assert torch.equal(h0.view(torch.int32), h2.view(torch.int32))
+        assert marks.shape[0] == min(148 * 8 * 4, (n + 127) // 128 * 4) and marks.shape[1] == 4
+        assert np.all(marks[:, 0] > 0) and np.all(marks[:, 2] >= marks[:, 0])
+        seen = marks[:, 1] > 0
+        assert np.all(marks[seen, 1] >= marks[seen, 0]) and np.all(marks[seen, 1] <= marks[seen, 2])
+    compare_hits(hits_np(oracle, h0), ho)
+
+
 def test_trace_tiny_scene_against_brute_force(crt, ctx, oracle):
     scene = I.furnace_sphere(1)                       # 80 triangles
     G = GpuScene(crt, scene, ctx)

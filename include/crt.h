@@ -212,7 +212,11 @@ size_t crt_radix_sort_scratch_bytes(int64_t n);
 
 /* ---- a5: BVH traversal ("the most time-consuming segment") ------------------------------- */
 /* hits[i] = nearest intersection of rays[i] with tmin < t < tmax; ties -> lowest primitive id (D:R10).
- * Inactive rays (tmax < 0) give a miss.  rays, hits: [device], n_rays entries. */
+ * Inactive rays (tmax < 0) give a miss.  rays, hits: [device], n_rays entries.
+ * Ray origins: the default kernel's box test is conservative for origins within 16 scene extents of the scene box (rays that start on surfaces or at a
+ * camera near the scene; crt_trace_primary checks the camera and switches by itself).  For rays from farther away set "trace_kernel" 4, the same kernel with
+ * the any-origin test (3-4 % slower).  A per-ray check inside the default kernel was built twice (far rays traversed by their lane at fetch time; far rays
+ * set aside and traversed by the last block) and removed: either form costs the persistent kernel 2-7 % through register pressure alone. */
 crt_status crt_trace(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n_rays, crt_hit* hits, void* stream);
 /* Work counters of the same traversal (a counting build of the kernel; used by bench.py for the roofline's
  * algorithmic FLOPs and by tests).  counters: [device] int64[4], ADDED to: [0] node visits (one visit = one 64-byte

@@ -444,7 +444,7 @@ def run_cuda(args):
 def run_sweep(args):
     """BASELINE config 3: interior scene at 3840x2160, 4 spp, 3 bounces; group size {2,4,8}^2 x stride {1,2,4,8} plus independent.
     Per point: secondary MRay/s over `--sweep-frames` frames and the RMSE of their mean image against (a) the mean of the same number
-    of independent-sampling frames and (b) a longer independent reference (4x the frames).  One JSON line ("sweep": [...]).
+    of independent-sampling frames and (b) a longer independent reference (--sweep-reference-frames; default 4x the frames).  One JSON line ("sweep": [...]).
     Warp execution efficiency and L2 hit rate come from ncu (profiles/), not from this run."""
     import torch
     import paper_2310_07182_b200 as crt
@@ -483,7 +483,8 @@ def run_sweep(args):
     def rmse(a, b):
         return float(torch.sqrt(torch.mean((a.double() - b.double()) ** 2)).item())
 
-    ref, _ = render("independent", 1, 1, 4 * F, 500000)           # disjoint frame range: independent of every sweep point
+    RF = args.sweep_reference_frames or 4 * F
+    ref, _ = render("independent", 1, 1, RF, 500000)              # disjoint frame range: independent of every sweep point
     ind, ind_t = render("independent", 1, 1, F, 0)
     points = [dict(mode="independent", group=1, stride=1, **ind_t, rmse_vs_reference=rmse(ind, ref), rmse_vs_independent=0.0)]
     if table3:      # P:L178-185 (Table 3): tile (8,8), (16,8), (16,16), (32,8) x K = 8, 16, 32, 64
@@ -506,7 +507,7 @@ def run_sweep(args):
                 points.append(dict(mode="direct_reuse", group=g, stride=s, **t, rmse_vs_reference=rmse(img, ref), rmse_vs_independent=rmse(img, ind)))
     name = "the paper's Table 3 shapes (P:L178-185)" if table3 else ("partition rules (D:R3 / D:R20 / D:R21)" if rules else "BASELINE config 3")
     print(json.dumps({"clocks": _SWEEP_CLOCKS.stop() if _SWEEP_CLOCKS else None, "sweep": points, "config": {"workload": f"{name}: interior scene {w}x{h}, {spp} spp, {nb} bounces", "frames": F,
-                                                  "reference_frames": 4 * F, "scale": sc}}))
+                                                  "reference_frames": RF, "scale": sc}}))
 
 
 def _frame_ray_sets(ctx, crt, scene, w, h, spp, nb, gw, gh, s, seed, frame, modes=("direct_reuse", "independent"), bvh=None):
@@ -719,6 +720,7 @@ def main():
     ap.add_argument("--ploc-radii", nargs="*", type=int, default=[8], help="--sweep builders: neighbour radii of the device builder")
     ap.add_argument("--variants", nargs="*", default=["3", "3:trace_exact=0", "5", "6", "4", "1"], help="--sweep kernels: trace_kernel id[:option=value,...] ...")
     ap.add_argument("--sweep-frames", type=int, default=64)
+    ap.add_argument("--sweep-reference-frames", type=int, default=0, help="frames of the independent-sampling reference image of a sweep (0 = 4 x --sweep-frames)")
     ap.add_argument("--sweep-scale", type=int, default=1, help="divide the 3840x2160 image by this (quick runs)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "cuda":

@@ -453,8 +453,13 @@ def run_sweep(args):
     sc = max(1, args.sweep_scale)
     table3 = args.sweep == "table3"
     rules = args.sweep == "rules"
-    w, h, spp, nb, seed = (1920 // sc, 1080 // sc, 1, 2, 1) if (table3 or rules) else (3840 // sc, 2160 // sc, 4, 3, 1)
-    scene = I.by_name("interior", seed=1).with_camera(w, h)
+    w, h, spp, nb, seed = (1920 // sc, 1080 // sc, 1, 2, 1) if (table3 or rules or args.sweep == "bias") else (3840 // sc, 2160 // sc, 4, 3, 1)
+    bias_cornell = args.sweep == "bias" and args.workload == "cornell"      # the all-Lambert scene: every group is a DIFFUSE group
+    if bias_cornell:
+        w, h, nb = 512, 512, 2
+    scene = (I.by_name("cornell") if bias_cornell else I.by_name("interior", seed=1)).with_camera(w, h)
+    if args.sweep == "bias" and args.all_lambert:      # the same geometry with every glossy and mirror material made Lambert: no GLOSSY or HYBRID group is left
+        t = scene.materials["type"]; t[(t == I.scenes.MAT_GLOSSY) | (t == I.scenes.MAT_SPECULAR)] = I.scenes.MAT_DIFFUSE
     bvh = ctx.crt_build_bvh(scene.verts, scene.mat_id)
     mats_dev = ctx.upload(scene.materials); mats = ctx.scene_mats(mats_dev, len(scene.materials), scene.env)
     cam = crt.make_camera(scene.camera)
@@ -483,6 +488,19 @@ def run_sweep(args):
     def rmse(a, b):
         return float(torch.sqrt(torch.mean((a.double() - b.double()) ** 2)).item())
 
+    if args.sweep == "bias":
+        # Does the mean image of a reuse mode converge to independent sampling's?  (sharing a WORLD direction skews the members' distributions --
+        # the paper's Fig. 1 artefacts --, sharing the LOCAL direction does not; HYBRID groups' averaged direction is a heuristic.)  Four F-frame means at
+        # BASELINE config 2's size: independent over two disjoint frame ranges (their RMSE is the noise floor), direct_reuse and world_reuse over a third.
+        ind_a, _ = render("independent", 1, 1, F, 0)
+        ind_b, _ = render("independent", 1, 1, F, 500000)
+        out = {"noise_floor_rmse_independent_vs_independent": rmse(ind_a, ind_b)}
+        for mode in ("direct_reuse", "world_reuse"):
+            for g, st in ((4, 4), (8, 1)):
+                img, _ = render(mode, g, st, F, 1000000)
+                out[f"{mode}_{g}x{g}_stride{st}"] = {"rmse_vs_independent": rmse(img, ind_b), "mean_image": float(img.mean().item()), "mean_independent": float(ind_b.mean().item())}
+        print(json.dumps({"clocks": _SWEEP_CLOCKS.stop() if _SWEEP_CLOCKS else None, "bias": out, "config": {"workload": f"{'cornell (all Lambert)' if bias_cornell else 'interior'} scene {w}x{h}, {spp} spp, {nb} bounces", "all_lambert": bool(args.all_lambert), "frames_per_mean": F}}))
+        return
     RF = args.sweep_reference_frames or 4 * F
     ref, _ = render("independent", 1, 1, RF, 500000)              # disjoint frame range: independent of every sweep point
     ind, ind_t = render("independent", 1, 1, F, 0)
@@ -715,11 +733,12 @@ def main():
     ap.add_argument("--set", nargs="*", default=[], metavar="OPTION=VALUE", help="crt_set_option on every context of the run (experiments; the defaults are what the driver times)")
     ap.add_argument("--repeats", type=int, default=1, help="repeat the K timed steps of direct_reuse / independent / morton_reorder this many times and report min / median / max")
     ap.add_argument("--no-sort-codes", action="store_true", help="skip the Origin / Reis / Costa / TwoPoint reordering baselines")
-    ap.add_argument("--sweep", nargs="?", const="config3", default=None, choices=["config3", "table3", "rules", "tail", "kernels", "builders", "timeline"],
-                    help="config3: BASELINE config 3 sweep; table3: the paper's Table 3 shapes (tile x K) at 1920x1080, 1 spp, 2 bounces; rules: shuffled against lattice partition at the same size; tail: fixed cost of a crt_trace launch (n, 2n, 4n rays) on --workload; kernels: A/B of traversal kernel variants (--variants) on one frame's ray sets of --workload; timeline: per-warp time marks of a crt_trace launch (what its tail consists of); builders: host SAH against device PLOC BVH builder on --workload")
+    ap.add_argument("--sweep", nargs="?", const="config3", default=None, choices=["config3", "table3", "rules", "tail", "kernels", "builders", "timeline", "bias"],
+                    help="config3: BASELINE config 3 sweep; table3: the paper's Table 3 shapes (tile x K) at 1920x1080, 1 spp, 2 bounces; rules: shuffled against lattice partition at the same size; tail: fixed cost of a crt_trace launch (n, 2n, 4n rays) on --workload; kernels: A/B of traversal kernel variants (--variants) on one frame's ray sets of --workload; timeline: per-warp time marks of a crt_trace launch (what its tail consists of); bias: long-run mean images of direct_reuse and world_reuse against independent sampling; builders: host SAH against device PLOC BVH builder on --workload")
     ap.add_argument("--ploc-radii", nargs="*", type=int, default=[8], help="--sweep builders: neighbour radii of the device builder")
     ap.add_argument("--variants", nargs="*", default=["3", "3:trace_exact=0", "5", "6", "4", "1"], help="--sweep kernels: trace_kernel id[:option=value,...] ...")
     ap.add_argument("--sweep-frames", type=int, default=64)
+    ap.add_argument("--all-lambert", action="store_true", help="--sweep bias: turn every glossy / mirror material of the scene into a Lambert one")
     ap.add_argument("--sweep-reference-frames", type=int, default=0, help="frames of the independent-sampling reference image of a sweep (0 = 4 x --sweep-frames)")
     ap.add_argument("--sweep-scale", type=int, default=1, help="divide the 3840x2160 image by this (quick runs)")
     args = ap.parse_args()

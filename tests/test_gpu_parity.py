@@ -653,6 +653,37 @@ def test_frame_in_bands_gives_the_identical_image(crt, ctx, mode, gw, gh, s):
         assert np.array_equal(out[bands][0], out[1][0]) and np.array_equal(out[bands][1], out[1][1]), bands
 
 
+def test_local_direction_reuse_is_unbiased_and_world_reuse_is_not(crt, ctx):
+    """A statistical check of the method itself that does not go through the oracle: on an all-Lambert scene every group is a DIFFUSE group; each member
+    uses the leader's LOCAL direction in its own tangent frame, so marginally its direction is cosine-distributed about its own normal and the pixel estimate is
+    unbiased: the long-run mean image must agree with independent sampling's to within the noise floor (two independent means over disjoint frame ranges).  Sharing
+    the WORLD direction (the paper's first variant, mode world_reuse) skews each member's distribution: its mean image must NOT agree (bench.py --sweep bias at full
+    size: 1.00x the floor against 1.32x, profiles/r02j)."""
+    import torch
+    scene = I.cornell().with_camera(128, 128)
+    G = GpuScene(crt, scene, ctx)
+    F = 4096
+
+    def mean_image(mode, g, s, first):
+        order = crt.make_order(mode, g, g, s)
+        ws = ctx.frame_workspace(crt.make_frame(128, 128), order)
+        acc = torch.zeros((128, 128, 3), device=ctx.device)
+        for f in range(F):
+            ctx.crt_render_frame(G.bvh, G.mats, G.camera, crt.make_frame(128, 128, 1, 9, first + f), order, 2, acc, ws)
+        torch.cuda.synchronize()
+        return (acc / F).double()
+
+    rm = lambda a, b: float(torch.sqrt(torch.mean((a - b) ** 2)).item())
+    ind_a, ind_b = mean_image("independent", 1, 1, 0), mean_image("independent", 1, 1, 100000)
+    floor = rm(ind_a, ind_b)
+    assert 0.005 < floor < 0.1
+    reuse = rm(mean_image("direct_reuse", 4, 4, 200000), ind_b)
+    world = rm(mean_image("world_reuse", 4, 4, 200000), ind_b)
+    print(f"noise floor {floor:.5f}, direct_reuse {reuse / floor:.3f}x, world_reuse {world / floor:.3f}x")
+    assert reuse < 1.06 * floor, (reuse, floor)
+    assert world > 1.15 * floor, (world, floor)
+
+
 def test_argument_errors(crt, ctx):
     import torch
     scene = I.cornell()

@@ -50,7 +50,7 @@ FP32_PEAK_TFLOPS_NOMINAL = 148 * 128 * 2 * 1.965e9 / 1e12
 #           node visit and the same triangle test; its ray setup has 12 more)
 #   dram  = dram__bytes_read.sum + dram__bytes_write.sum of the default kernel
 NCU_PER_RAY = {
-    "interior": {"flop": 1897.0, "dram_bytes": 61.5, "source": "profiles/r02c_roofline_inputs.md (ncu on the commit 'device BVH builder: the whole build on the GPU'; flop: 7.383 G over 3,891,381 live rays of frame 7; dram: 239.1 MB over 3,890,598 live rays)"},
+    "interior": {"flop": 1796.0, "dram_bytes": 61.7, "source": "profiles/r02k_presplit.md (ncu on the tree with pre-split large triangles, the default; flop: 6.991 G over 3,891,381 live rays of frame 7; dram: 240.2 MB over the same rays; without pre-splitting 1,897 flop per ray, profiles/r02c)"},
     "landscape": {"flop": 1383.0, "dram_bytes": 100.7, "source": "profiles/r02c_roofline_inputs.md (same commit; flop: 2.817 G over 2,037,200 live rays of frame 7; dram: 205.2 MB over 2,038,170 live rays)"},
 }
 # what ncu shows to be the kernel's limiter (not modelled by the two-term roofline): profiles/r02a, r02c
@@ -194,7 +194,7 @@ def run_cuda(args):
         ctx.crt_set_option(k_, int(v_))
     scene, (w, h, spp, nb, gw, gh, s, seed, cfg) = _scene(args.workload)
     t0 = time.perf_counter()
-    bvh = ctx.crt_build_bvh(scene.verts, scene.mat_id)
+    bvh = ctx.crt_build_bvh(scene.verts, scene.mat_id, **BVH_KW)
     build_s = time.perf_counter() - t0
     info = bvh.info()
     mats_dev = ctx.upload(scene.materials)
@@ -426,7 +426,7 @@ def run_cuda(args):
                    "single_stream_note": "one frame at a time without per-stage events (crt_render_frame then cuts the frame into bands, option frame_bands); modes[..].mray_s are with per-stage events, unbanded",
                    "l2": f"no explicit flush: each step streams its {ws_bytes / 1e6:.0f} MB workspace plus the {info['device_bytes'] / 1e6:.0f} MB BVH (> 126 MB L2)",
                    "parallelism": "replicas only (no sharding, no collective)" if world > 1 else "single GPU",
-                   "bvh": {"nodes": info["n_nodes"], "depth": info["depth"], "sah_cost": info["sah_cost"], "device_mb": info["device_bytes"] / 1e6,
+                   "bvh": {"nodes": info["n_nodes"], "triangle_references": info["n_refs"], "presplit": BVH_KW.get("presplit", "library default (1/16 of the scene diagonal)"), "depth": info["depth"], "sah_cost": info["sah_cost"], "device_mb": info["device_bytes"] / 1e6,
                            "build_s": info["build_seconds"], "build_and_upload_s": build_s}},
         "modes": modes, "roofline": roofline, "cpu_baseline": cpu,
         "e2e": {"value": e2e["mray_s"], "unit": UNIT, "h2d_bytes_per_step": len(scene.materials) * 32 + 48 + 24,
@@ -460,7 +460,7 @@ def run_sweep(args):
     scene = (I.by_name("cornell") if bias_cornell else I.by_name("interior", seed=1)).with_camera(w, h)
     if args.sweep == "bias" and args.all_lambert:      # the same geometry with every glossy and mirror material made Lambert: no GLOSSY or HYBRID group is left
         t = scene.materials["type"]; t[(t == I.scenes.MAT_GLOSSY) | (t == I.scenes.MAT_SPECULAR)] = I.scenes.MAT_DIFFUSE
-    bvh = ctx.crt_build_bvh(scene.verts, scene.mat_id)
+    bvh = ctx.crt_build_bvh(scene.verts, scene.mat_id, **BVH_KW)
     mats_dev = ctx.upload(scene.materials); mats = ctx.scene_mats(mats_dev, len(scene.materials), scene.env)
     cam = crt.make_camera(scene.camera)
     F = args.sweep_frames
@@ -531,7 +531,7 @@ def run_sweep(args):
 def _frame_ray_sets(ctx, crt, scene, w, h, spp, nb, gw, gh, s, seed, frame, modes=("direct_reuse", "independent"), bvh=None):
     """The ray sets of one frame (primary, bounce 1 .. nb) in each order of `modes`: [(tag, rays)]."""
     import torch
-    bvh = bvh or ctx.crt_build_bvh(scene.verts, scene.mat_id)
+    bvh = bvh or ctx.crt_build_bvh(scene.verts, scene.mat_id, **BVH_KW)
     mats_dev = ctx.upload(scene.materials); mats = ctx.scene_mats(mats_dev, len(scene.materials), scene.env); cam = crt.make_camera(scene.camera)
     sets = []
     for mode in modes:
@@ -551,6 +551,7 @@ def _frame_ray_sets(ctx, crt, scene, w, h, spp, nb, gw, gh, s, seed, frame, mode
     return bvh, (mats_dev, mats), sets
 
 
+BVH_KW = {}      # --presplit: build parameter of every BVH this run builds (default: the library's)
 KERNEL_OPTION_DEFAULTS = {"trace_kernel": 3, "trace_refill_threshold": 16, "trace_leaf_wait": 6, "trace_blocks_per_sm": 0, "trace_exact": 1, "trace_tail_split": 0}
 
 
@@ -690,7 +691,7 @@ def run_tail(args):
     name, kw, w, h, spp, nb, gw, gh, s, seed, cfg = WORKLOADS[args.workload]
     scene = I.by_name(name, **kw).with_camera(w, h)
     ctx = crt.Context(0)
-    bvh = ctx.crt_build_bvh(scene.verts, scene.mat_id)
+    bvh = ctx.crt_build_bvh(scene.verts, scene.mat_id, **BVH_KW)
     mats_dev = ctx.upload(scene.materials); mats = ctx.scene_mats(mats_dev, len(scene.materials), scene.env); cam = crt.make_camera(scene.camera)
     order = crt.make_order("direct_reuse", gw, gh, s); fr = crt.make_frame(w, h, spp, seed, 7)
     rays, hits, r2p = ctx.crt_trace_primary(bvh, cam, fr, order)
@@ -737,11 +738,14 @@ def main():
                     help="config3: BASELINE config 3 sweep; table3: the paper's Table 3 shapes (tile x K) at 1920x1080, 1 spp, 2 bounces; rules: shuffled against lattice partition at the same size; tail: fixed cost of a crt_trace launch (n, 2n, 4n rays) on --workload; kernels: A/B of traversal kernel variants (--variants) on one frame's ray sets of --workload; timeline: per-warp time marks of a crt_trace launch (what its tail consists of); bias: long-run mean images of direct_reuse and world_reuse against independent sampling; builders: host SAH against device PLOC BVH builder on --workload")
     ap.add_argument("--ploc-radii", nargs="*", type=int, default=[8], help="--sweep builders: neighbour radii of the device builder")
     ap.add_argument("--variants", nargs="*", default=["3", "3:trace_exact=0", "5", "6", "4", "1"], help="--sweep kernels: trace_kernel id[:option=value,...] ...")
+    ap.add_argument("--presplit", type=float, default=None, help="crt_bvh_params.presplit of the BVHs built by this run (0 = no pre-splitting of large triangles; default: the library's 1/16)")
     ap.add_argument("--sweep-frames", type=int, default=64)
     ap.add_argument("--all-lambert", action="store_true", help="--sweep bias: turn every glossy / mirror material of the scene into a Lambert one")
     ap.add_argument("--sweep-reference-frames", type=int, default=0, help="frames of the independent-sampling reference image of a sweep (0 = 4 x --sweep-frames)")
     ap.add_argument("--sweep-scale", type=int, default=1, help="divide the 3840x2160 image by this (quick runs)")
     args = ap.parse_args()
+    if args.presplit is not None:
+        BVH_KW["presplit"] = args.presplit
     if args.warmup < 3 and args.impl == "cuda":
         args.warmup = 3
     if args.sweep:

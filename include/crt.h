@@ -89,8 +89,13 @@ typedef struct { int32_t mode, group_w, group_h, stride, stride_y, partition_rul
 typedef struct { const crt_material* materials; int32_t n_materials; float env[6]; } crt_scene_mats;
 /* builder: 0 = host (binned surface-area heuristic, threaded); 1 = device (parallel locally-ordered clustering AND the traversal layouts
  * written by the GPU, csrc/bvh_ploc.cu; needs a context); 2 = the device's clustering with the host's layout code (cross-check of 1);
- * ploc_radius: neighbours searched on either side of a cluster in Morton order (0 = 8; at most 128). */
-typedef struct { int32_t max_leaf; int32_t sah_bins; float cost_traversal, cost_intersect; int32_t n_threads; int32_t builder; int32_t ploc_radius; } crt_bvh_params;
+ * ploc_radius: neighbours searched on either side of a cluster in Morton order (0 = 8; at most 128).
+ * presplit (host builder, max_leaf > 1): a triangle whose box is longer than presplit x the scene's diagonal on some axis is given several REFERENCES,
+ * one per cell of a recursive midpoint split of its box, each with the box of the part of the triangle inside the cell, and the tree is built over
+ * references (at most n_tris / 4 + 4096 extra ones).  The triangle itself is unchanged -- same record, same id, tested whole -- so every traversal
+ * returns the same hit; only the boxes that lead to it are tighter (walls and floors no longer overlap every object in front of them: interior scene
+ * -11 % primary, -3 % secondary traversal time, profiles/r02k).  0 = off; NULL params = 1/16. */
+typedef struct { int32_t max_leaf; int32_t sah_bins; float cost_traversal, cost_intersect; int32_t n_threads; int32_t builder; int32_t ploc_radius; float presplit; } crt_bvh_params;
 typedef struct {
     int64_t n_tris, n_nodes, device_bytes;
     float bounds[6];            /* exact min/max over the vertices (unpadded); used by the Morton code */
@@ -106,6 +111,7 @@ typedef struct {
                                  * hierarchy build including the copy back and the leaf collapse; layout_seconds the flattening, 16-bit
                                  * quantisation and upload of the traversal layouts (either builder) */
     double layout_seconds;
+    int64_t n_refs;             /* triangle references = records of the device triangle array (n_tris unless large triangles were pre-split) */
 } crt_bvh_info_t;
 
 /* ---- context ------------------------------------------------------------------------------------ */
@@ -160,7 +166,8 @@ crt_status crt_build_bvh(crt_ctx* ctx, const float* verts, const int32_t* mat_id
                          const crt_bvh_params* params, crt_bvh** out);
 crt_status crt_bvh_destroy(crt_bvh* bvh);
 crt_status crt_bvh_get_info(const crt_bvh* bvh, crt_bvh_info_t* out);
-/* Structural invariants of the host tree: *violations = 0 iff every triangle is in exactly one leaf, every
+/* Structural invariants of the host tree: *violations = 0 iff every triangle is in exactly one leaf (pre-split builds: in at least one, and the boxes
+ * of its leaves together cover it), every
  * leaf has 1..max_leaf triangles, every node's box contains its children's boxes / its triangles, and (wide
  * layout, bits 8 and up) every triangle lies inside the box the kernel decodes for each of its ancestors, and (16-bit
  * layout, bit 16) every quantised plane lies at least one grid step outside the fp32 box it replaces. */

@@ -63,14 +63,15 @@ class SceneMats(C.Structure):
 
 class BvhParams(C.Structure):
     _fields_ = [("max_leaf", C.c_int32), ("sah_bins", C.c_int32), ("cost_traversal", C.c_float), ("cost_intersect", C.c_float),
-                ("n_threads", C.c_int32), ("builder", C.c_int32), ("ploc_radius", C.c_int32)]
+                ("n_threads", C.c_int32), ("builder", C.c_int32), ("ploc_radius", C.c_int32), ("presplit", C.c_float)]
 
 
 class BvhInfo(C.Structure):
     _fields_ = [("n_tris", C.c_int64), ("n_nodes", C.c_int64), ("device_bytes", C.c_int64), ("bounds", C.c_float * 6),
                 ("sah_cost", C.c_double), ("depth", C.c_int32), ("max_leaf", C.c_int32), ("build_seconds", C.c_double),
                 ("n_wide_nodes", C.c_int64), ("wide_depth", C.c_int32), ("q16_inflation_pct", C.c_int32),
-                ("builder", C.c_int32), ("build_rounds", C.c_int32), ("device_build_seconds", C.c_double), ("layout_seconds", C.c_double)]
+                ("builder", C.c_int32), ("build_rounds", C.c_int32), ("device_build_seconds", C.c_double), ("layout_seconds", C.c_double),
+                ("n_refs", C.c_int64)]
 
 
 _lib = None
@@ -157,7 +158,7 @@ class Bvh:
         return {"n_tris": o.n_tris, "n_nodes": o.n_nodes, "device_bytes": o.device_bytes, "bounds": np.array(list(o.bounds), np.float32),
                 "sah_cost": o.sah_cost, "depth": o.depth, "max_leaf": o.max_leaf, "build_seconds": o.build_seconds,
                 "n_wide_nodes": o.n_wide_nodes, "wide_depth": o.wide_depth, "q16_inflation_pct": o.q16_inflation_pct,
-                "builder": o.builder, "build_rounds": o.build_rounds, "device_build_seconds": o.device_build_seconds, "layout_seconds": o.layout_seconds}
+                "builder": o.builder, "build_rounds": o.build_rounds, "device_build_seconds": o.device_build_seconds, "layout_seconds": o.layout_seconds, "n_refs": o.n_refs}
 
     def check(self):
         v = C.c_int32(-1)
@@ -230,7 +231,7 @@ class Context:
         return a.value, b.value
 
     # ---- a0 -----------------------------------------------------------------------------------------
-    def crt_build_bvh(self, verts, mat_id, max_leaf=3, sah_bins=64, n_threads=0, cost_traversal=1.0, cost_intersect=1.0, builder=0, ploc_radius=0):
+    def crt_build_bvh(self, verts, mat_id, max_leaf=3, sah_bins=64, n_threads=0, cost_traversal=1.0, cost_intersect=1.0, builder=0, ploc_radius=0, presplit=1.0 / 16):
         """verts: numpy float32[n,3,3] or torch tensor (host or device); mat_id int32[n].  builder: 0 host SAH, 1 device PLOC."""
         if isinstance(verts, np.ndarray):
             verts = np.ascontiguousarray(verts, np.float32)
@@ -238,7 +239,7 @@ class Context:
             n = verts.size // 9
         else:
             n = verts.numel() // 9
-        pr = BvhParams(max_leaf, sah_bins, cost_traversal, cost_intersect, n_threads, int(builder), int(ploc_radius))
+        pr = BvhParams(max_leaf, sah_bins, cost_traversal, cost_intersect, n_threads, int(builder), int(ploc_radius), float(presplit))
         h = C.c_void_p()
         self._check(lib().crt_build_bvh(self.handle, _ptr(verts), _ptr(mat_id), C.c_int64(n), C.byref(pr), C.byref(h)))
         return Bvh(self, h)

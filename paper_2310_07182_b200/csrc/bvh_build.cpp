@@ -160,6 +160,70 @@ struct Builder {
     }
 };
 
+// ---- triangle pre-splitting (crt_bvh_params.presplit; "early split clipping", Ernst & Greiner 2007) ------------------------------------
+// A triangle much larger than the scene's detail (a wall, a floor) has a box that overlaps thousands of small objects: every ray that passes
+// near it tests it and the nodes above it cannot separate what lies on its two sides.  Such a triangle is given SEVERAL references, each with the
+// box of the part of the triangle inside one cell of a recursive midpoint split of its box; the tree is built over references.  The triangle
+// itself is unchanged (same record, same id, tested whole), so the result of a traversal is the same nearest hit; only which boxes lead to it.
+struct Ref { float mn[3], mx[3]; int32_t prim; };
+
+float round_down(double d) { float f = (float)d; return (double)f > d ? std::nextafterf(f, -std::numeric_limits<float>::infinity()) : f; }
+float round_up(double d) { float f = (float)d; return (double)f < d ? std::nextafterf(f, std::numeric_limits<float>::infinity()) : f; }
+
+struct Poly { int n; double v[10][3]; };      // a triangle clipped by axis-aligned planes: convex, at most 3 + 6 vertices
+
+// the part of `in` on the side s * (x[axis] - pos) <= 0 (Sutherland-Hodgman against one plane)
+void clip(const Poly& in, int axis, double pos, double s, Poly& out)
+{
+    out.n = 0;
+    for (int i = 0; i < in.n; ++i) {
+        const double* a = in.v[i]; const double* b = in.v[(i + 1) % in.n];
+        const double da = s * (a[axis] - pos), db = s * (b[axis] - pos);
+        if (da <= 0 && out.n < 10) std::memcpy(out.v[out.n++], a, 24);
+        if ((da < 0 && db > 0) || (da > 0 && db < 0)) {
+            const double t = da / (da - db);
+            if (out.n < 10) { double* c = out.v[out.n++]; for (int k = 0; k < 3; ++k) c[k] = a[k] + t * (b[k] - a[k]); c[axis] = pos; }
+        }
+    }
+}
+
+// references of triangle `prim`: one if its box is no longer than `limit` on any axis, else the cells of a recursive midpoint split (at most `budget` more)
+void presplit_triangle(const float* tv, int32_t prim, double limit, int64_t& budget, std::vector<Ref>& refs)
+{
+    struct Item { Poly p; double mn[3], mx[3]; int depth; };
+    auto box_of = [](Item& it) {
+        for (int k = 0; k < 3; ++k) { it.mn[k] = std::numeric_limits<double>::infinity(); it.mx[k] = -it.mn[k]; }
+        for (int i = 0; i < it.p.n; ++i) for (int k = 0; k < 3; ++k) { it.mn[k] = std::min(it.mn[k], it.p.v[i][k]); it.mx[k] = std::max(it.mx[k], it.p.v[i][k]); }
+    };
+    std::vector<Item> work(1);
+    work[0].p.n = 3; work[0].depth = 0;
+    for (int i = 0; i < 3; ++i) for (int k = 0; k < 3; ++k) work[0].p.v[i][k] = tv[3 * i + k];
+    box_of(work[0]);
+    while (!work.empty()) {
+        Item it = work.back(); work.pop_back();
+        int axis = 0;
+        for (int k = 1; k < 3; ++k) if (it.mx[k] - it.mn[k] > it.mx[axis] - it.mn[axis]) axis = k;
+        if (!(it.mx[axis] - it.mn[axis] > limit) || it.depth >= 16 || budget <= 0) {
+            Ref r; r.prim = prim;
+            for (int k = 0; k < 3; ++k) { r.mn[k] = round_down(it.mn[k]); r.mx[k] = round_up(it.mx[k]); }
+            refs.push_back(r);
+            continue;
+        }
+        const double pos = 0.5 * (it.mn[axis] + it.mx[axis]);
+        Item lo, hi; lo.depth = hi.depth = it.depth + 1;
+        clip(it.p, axis, pos, 1.0, lo.p); clip(it.p, axis, pos, -1.0, hi.p);
+        if (lo.p.n == 0 || hi.p.n == 0) {      // cannot happen for pos strictly inside the box; keep the piece whole rather than lose it
+            Ref r; r.prim = prim;
+            for (int k = 0; k < 3; ++k) { r.mn[k] = round_down(it.mn[k]); r.mx[k] = round_up(it.mx[k]); }
+            refs.push_back(r);
+            continue;
+        }
+        box_of(lo); box_of(hi);
+        --budget;
+        work.push_back(hi); work.push_back(lo);
+    }
+}
+
 }  // namespace
 
 // Builds the host tree.  Returns false on failure.
@@ -168,39 +232,62 @@ bool crt_bvh_build_host(crt_bvh* b, const float* verts, int64_t n, const crt_bvh
     auto t0 = std::chrono::steady_clock::now();
     b->n_tris = n; b->max_leaf = pr.max_leaf;
     b->verts.assign(verts, verts + 9 * n);
-    b->prim.resize((size_t)n);
-    b->nodes.assign((size_t)std::max<int64_t>(2 * n, 1), BuildNode());
-    Builder B(b->prim, b->nodes);
-    B.verts = b->verts.data(); B.n = n; B.max_leaf = pr.max_leaf; B.bins = std::min(kMaxBins, std::max(4, pr.sah_bins));
-    B.ct = pr.cost_traversal; B.ci = pr.cost_intersect;
-    B.tmn.resize(3 * (size_t)n); B.tmx.resize(3 * (size_t)n); B.cen.resize(3 * (size_t)n);
+    // references: one per triangle, several for a triangle much longer than the scene's detail (pre-splitting; not with one triangle per leaf,
+    // where the 8-wide layout shares the triangle order and wants every triangle exactly once)
+    std::vector<Ref> refs; refs.reserve((size_t)n);
     float maxabs = 0.f;
     Box root; root.reset();
     for (int64_t i = 0; i < n; ++i) {
-        b->prim[i] = (int32_t)i;
         const float* tv = verts + 9 * i;
+        Ref r; r.prim = (int32_t)i;
         for (int k = 0; k < 3; ++k) {
-            float lo = std::min(tv[k], std::min(tv[3 + k], tv[6 + k])), hi = std::max(tv[k], std::max(tv[3 + k], tv[6 + k]));
-            B.tmn[3 * i + k] = lo; B.tmx[3 * i + k] = hi; B.cen[3 * i + k] = 0.5f * lo + 0.5f * hi;
-            maxabs = std::max(maxabs, std::max(std::fabs(lo), std::fabs(hi)));
+            r.mn[k] = std::min(tv[k], std::min(tv[3 + k], tv[6 + k])); r.mx[k] = std::max(tv[k], std::max(tv[3 + k], tv[6 + k]));
+            maxabs = std::max(maxabs, std::max(std::fabs(r.mn[k]), std::fabs(r.mx[k])));
         }
-        root.grow(&B.tmn[3 * i], &B.tmx[3 * i]);
+        root.grow(r.mn, r.mx);
+        refs.push_back(r);
     }
     for (int k = 0; k < 3; ++k) { b->bounds[k] = n ? root.mn[k] : 0.f; b->bounds[3 + k] = n ? root.mx[k] : 0.f; }
+    if (pr.presplit > 0.f && pr.max_leaf > 1 && n > 0) {
+        double diag = 0; for (int k = 0; k < 3; ++k) diag += ((double)root.mx[k] - root.mn[k]) * ((double)root.mx[k] - root.mn[k]);
+        const double limit = (double)pr.presplit * std::sqrt(diag);
+        int64_t budget = std::max<int64_t>(n / 4, 4096);         // at most this many additional references in all
+        if (n + budget >= ((int64_t)1 << 28)) budget = std::max<int64_t>(0, ((int64_t)1 << 28) - 1 - n);
+        std::vector<Ref> out; out.reserve((size_t)n + 1024);
+        for (int64_t i = 0; i < n; ++i) {
+            const Ref& r = refs[i];
+            if (limit > 0 && std::max(r.mx[0] - r.mn[0], std::max(r.mx[1] - r.mn[1], r.mx[2] - r.mn[2])) > limit && budget > 0) presplit_triangle(verts + 9 * i, (int32_t)i, limit, budget, out);
+            else out.push_back(r);
+        }
+        refs.swap(out);
+    }
+    const int64_t nr = (int64_t)refs.size();
+    b->n_refs = nr;
+    b->prim.resize((size_t)nr);
+    b->nodes.assign((size_t)std::max<int64_t>(2 * nr, 1), BuildNode());
+    Builder B(b->prim, b->nodes);
+    B.verts = b->verts.data(); B.n = nr; B.max_leaf = pr.max_leaf; B.bins = std::min(kMaxBins, std::max(4, pr.sah_bins));
+    B.ct = pr.cost_traversal; B.ci = pr.cost_intersect;
+    B.tmn.resize(3 * (size_t)nr); B.tmx.resize(3 * (size_t)nr); B.cen.resize(3 * (size_t)nr);
+    for (int64_t i = 0; i < nr; ++i) {
+        b->prim[i] = (int32_t)i;      // reference ids while building; the caller's triangle ids afterwards
+        for (int k = 0; k < 3; ++k) { B.tmn[3 * i + k] = refs[i].mn[k]; B.tmx[3 * i + k] = refs[i].mx[k]; B.cen[3 * i + k] = 0.5f * refs[i].mn[k] + 0.5f * refs[i].mx[k]; }
+    }
     if (n > 0) {
         int nt = pr.n_threads > 0 ? pr.n_threads : (int)std::max(1u, std::thread::hardware_concurrency());
         nt = std::min(nt, 64);
         B.n_nodes = 1;
-        if (nt > 1 && n > 65536) {
+        if (nt > 1 && nr > 65536) {
             Pool pool(nt);
             B.pool = &pool;
-            pool.submit([&] { B.subtree(0, 0, n, 1); });
+            pool.submit([&] { B.subtree(0, 0, nr, 1); });
             pool.wait();
         } else {
             B.pool = nullptr;
-            B.subtree(0, 0, n, 1);
+            B.subtree(0, 0, nr, 1);
         }
         b->nodes.resize((size_t)B.n_nodes.load());
+        for (int64_t i = 0; i < nr; ++i) b->prim[i] = refs[b->prim[i]].prim;
         b->depth = B.max_depth.load();
         // SAH cost (relative to the root area) before padding
         double ra = root.half_area(), cost = 0;
@@ -226,6 +313,14 @@ int32_t crt_bvh_check_host(const crt_bvh* b)
     int32_t bad = 0;
     if (b->n_tris == 0) return 0;
     std::vector<uint8_t> seen((size_t)b->n_tris, 0);
+    // pre-split trees (n_refs > n_tris): a triangle may sit in several leaves, each holding the part of it inside that leaf's box; for those triangles
+    // the invariant is that the leaves' boxes together cover the triangle (checked below on a lattice of points of the triangle)
+    const bool split = b->n_refs > b->n_tris;
+    std::vector<int32_t> n_leaves; std::vector<std::pair<int32_t, int32_t>> leaf_of;      // (triangle, node) of every reference of a multiply referenced triangle
+    if (split) {
+        n_leaves.assign((size_t)b->n_tris, 0);
+        for (int32_t p : b->prim) if (p >= 0 && p < b->n_tris) ++n_leaves[p];
+    }
     for (const BuildNode& nd : b->nodes) {
         if (nd.left >= 0) {
             for (int32_t c : {nd.left, nd.right}) {
@@ -237,8 +332,9 @@ int32_t crt_bvh_check_host(const crt_bvh* b)
             for (int j = 0; j < nd.count; ++j) {
                 int32_t p = b->prim[nd.first + j];
                 if (p < 0 || p >= b->n_tris) { bad |= 32; continue; }
-                if (seen[p]) bad |= 4;
+                if (seen[p] && !split) bad |= 4;
                 seen[p] = 1;
+                if (split && n_leaves[p] > 1) { leaf_of.emplace_back(p, (int32_t)(&nd - b->nodes.data())); continue; }
                 const float* tv = b->verts.data() + 9 * (int64_t)p;
                 for (int v = 0; v < 3; ++v) for (int k = 0; k < 3; ++k)
                     if (tv[3 * v + k] < nd.bmin[k] || tv[3 * v + k] > nd.bmax[k]) bad |= 8;
@@ -246,6 +342,25 @@ int32_t crt_bvh_check_host(const crt_bvh* b)
         }
     }
     for (uint8_t s : seen) if (!s) bad |= 16;
+    if (split) {
+        std::sort(leaf_of.begin(), leaf_of.end());
+        for (size_t i = 0; i < leaf_of.size();) {
+            size_t j = i; while (j < leaf_of.size() && leaf_of[j].first == leaf_of[i].first) ++j;
+            const float* tv = b->verts.data() + 9 * (int64_t)leaf_of[i].first;
+            const int G = 12;         // barycentric lattice: 91 points including the corners and edge points
+            for (int a = 0; a <= G; ++a) for (int c = 0; a + c <= G; ++c) {
+                const double wa = (double)a / G, wc = (double)c / G, wb = 1.0 - wa - wc;
+                double q[3]; for (int k = 0; k < 3; ++k) q[k] = wb * tv[k] + wa * tv[3 + k] + wc * tv[6 + k];
+                bool in = false;
+                for (size_t m = i; m < j && !in; ++m) {
+                    const BuildNode& nd = b->nodes[leaf_of[m].second];
+                    in = q[0] >= nd.bmin[0] && q[0] <= nd.bmax[0] && q[1] >= nd.bmin[1] && q[1] <= nd.bmax[1] && q[2] >= nd.bmin[2] && q[2] <= nd.bmax[2];
+                }
+                if (!in) bad |= 8;
+            }
+            i = j;
+        }
+    }
     return bad;
 }
 
@@ -255,9 +370,9 @@ int32_t crt_bvh_check_host(const crt_bvh* b)
 void crt_bvh_flatten(const crt_bvh* b, const std::vector<int32_t>& tri_order, std::vector<GpuNode>& gn, std::vector<GpuTri>& gt, std::vector<int32_t>& slot_of_prim)
 {
     const float inf = std::numeric_limits<float>::infinity();
-    const int64_t n = b->n_tris;
+    const int64_t n = b->n_refs;         // records of the device triangle array: one per reference (== triangles unless the build pre-split some)
     const bool own = tri_order.empty();
-    gt.resize((size_t)n); slot_of_prim.assign((size_t)n, -1);
+    gt.resize((size_t)n); slot_of_prim.assign((size_t)b->n_tris, -1);      // slot_of_prim: any one of a triangle's records (they are identical)
     for (int64_t j = 0; j < n; ++j) {
         int32_t p = own ? b->prim[j] : tri_order[j];
         const float* tv = b->verts.data() + 9 * (int64_t)p;
@@ -443,8 +558,9 @@ void crt_bvh_collapse4(const std::vector<GpuNode>& gn, const std::vector<QNode>&
 int32_t crt_layout_check_device(const crt_bvh* b)
 {
     if (b->n_tris == 0 || !b->d_nodes || !b->d_tris) return 0;
-    const int64_t nn = b->n_gpu_nodes, nt = b->n_tris;
-    std::vector<GpuNode> gn((size_t)nn); std::vector<QNode> qn((size_t)nn); std::vector<GpuTri> gt((size_t)nt); std::vector<int32_t> sop((size_t)nt);
+    const int64_t nn = b->n_gpu_nodes, nt = b->n_tris, nrec = b->n_refs;
+    const bool split = nrec > nt;        // pre-split build: a triangle may have several records; the coverage of such triangles is crt_bvh_check_host's
+    std::vector<GpuNode> gn((size_t)nn); std::vector<QNode> qn((size_t)nn); std::vector<GpuTri> gt((size_t)nrec); std::vector<int32_t> sop((size_t)nt);
     if (cudaMemcpy(gn.data(), b->d_nodes, gn.size() * sizeof(GpuNode), cudaMemcpyDeviceToHost) != cudaSuccess) return 32;
     if (b->d_qnodes && cudaMemcpy(qn.data(), b->d_qnodes, qn.size() * sizeof(QNode), cudaMemcpyDeviceToHost) != cudaSuccess) return 32;
     if (cudaMemcpy(gt.data(), b->d_tris, gt.size() * sizeof(GpuTri), cudaMemcpyDeviceToHost) != cudaSuccess) return 32;
@@ -480,16 +596,17 @@ int32_t crt_layout_check_device(const crt_bvh* b)
             } else {
                 const int32_t leaf = ~ch.ref; const int64_t first = leaf >> 3; const int cnt = (leaf & 7) + 1;
                 if (cnt > b->max_leaf) bad |= 2;
-                if (first + cnt > nt) { bad |= 32; continue; }
+                if (first + cnt > nrec) { bad |= 32; continue; }
                 for (int64_t j = first; j < first + cnt; ++j) {
                     int32_t prim; std::memcpy(&prim, &gt[j].v0p.w, 4);
                     if (prim < 0 || prim >= nt) { bad |= 32; continue; }
-                    if (seen_tri[prim]) bad |= 4;
+                    if (seen_tri[prim] && !split) bad |= 4;
                     seen_tri[prim] = 1;
-                    if (sop[prim] != (int32_t)j) bad |= 32;
+                    if (split) { int32_t q = -1; if (sop[prim] >= 0 && sop[prim] < nrec) std::memcpy(&q, &gt[sop[prim]].v0p.w, 4); if (q != prim) bad |= 32; }
+                    else if (sop[prim] != (int32_t)j) bad |= 32;
                     const float* tv = b->verts.data() + 9 * (int64_t)prim;
                     if (gt[j].v0p.x != tv[0] || gt[j].v0p.y != tv[1] || gt[j].v0p.z != tv[2] || gt[j].e1.x != tv[3] - tv[0] || gt[j].e2.z != tv[8] - tv[2]) bad |= 32;
-                    for (int v = 0; v < 3; ++v)
+                    for (int v = 0; v < 3 && !split; ++v)
                         if (tv[3 * v] < ch.min_x || tv[3 * v] > ch.max_x || tv[3 * v + 1] < ch.min_y || tv[3 * v + 1] > ch.max_y || tv[3 * v + 2] < ch.min_z || tv[3 * v + 2] > ch.max_z) bad |= 8;
                 }
             }

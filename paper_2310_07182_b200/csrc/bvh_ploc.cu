@@ -357,7 +357,7 @@ struct DevBuf {
 crt_status crt_bvh_build_device(crt_ctx* ctx, crt_bvh* b, const float* verts, int64_t n, const crt_bvh_params& pr, bool full_device)
 {
     auto t0 = std::chrono::steady_clock::now();
-    b->n_tris = n; b->max_leaf = pr.max_leaf;
+    b->n_tris = n; b->n_refs = n; b->max_leaf = pr.max_leaf;
     b->verts.assign(verts, verts + 9 * n);
     b->nodes.clear(); b->prim.clear(); b->depth = 0; b->sah = 0; b->builder = full_device ? 1 : 2;
     for (int k = 0; k < 6; ++k) b->bounds[k] = 0.f;

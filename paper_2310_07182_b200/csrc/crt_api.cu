@@ -147,10 +147,11 @@ crt_status crt_build_bvh(crt_ctx* ctx, const float* verts, const int32_t* mat_id
     CrtDeviceGuard dev_guard_(ctx ? ctx->device : -1);
     if (n_tris < 0 || (n_tris > 0 && !verts)) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "build_bvh: bad triangle array");
     if (n_tris >= ((int64_t)1 << 28)) return crt_fail(ctx, CRT_ERR_UNSUPPORTED, "build_bvh: more than 2^28 triangles");
-    crt_bvh_params pr = {3, 64, 1.0f, 1.0f, 0, 0, 0};
+    crt_bvh_params pr = {3, 64, 1.0f, 1.0f, 0, 0, 0, 0.0625f};
     if (params) pr = *params;
     if (pr.max_leaf < 1 || pr.max_leaf > 8) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "build_bvh: max_leaf %d not in [1,8]", pr.max_leaf);
     if (pr.sah_bins == 0) pr.sah_bins = 64;
+    if (!(pr.presplit >= 0.f && pr.presplit <= 1.f)) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "build_bvh: presplit %g not in [0,1]", (double)pr.presplit);
     std::vector<float> hv; std::vector<int32_t> hm((size_t)n_tris, 0);
     const float* v = verts;
     if (ctx && n_tris > 0 && is_device_ptr(verts)) {
@@ -227,7 +228,7 @@ crt_status crt_bvh_destroy(crt_bvh* b)
 crt_status crt_bvh_get_info(const crt_bvh* b, crt_bvh_info_t* o)
 {
     if (!b || !o) return crt_fail(nullptr, CRT_ERR_INVALID_ARG, "bvh_get_info: null argument");
-    o->n_tris = b->n_tris; o->n_nodes = b->nodes.empty() ? b->n_tree_nodes : (int64_t)b->nodes.size(); o->device_bytes = b->device_bytes;
+    o->n_refs = b->n_refs; o->n_tris = b->n_tris; o->n_nodes = b->nodes.empty() ? b->n_tree_nodes : (int64_t)b->nodes.size(); o->device_bytes = b->device_bytes;
     memcpy(o->bounds, b->bounds, sizeof o->bounds);
     o->sah_cost = b->sah; o->depth = b->depth; o->max_leaf = b->max_leaf; o->build_seconds = b->build_seconds;
     o->n_wide_nodes = b->n_wide_nodes; o->wide_depth = b->wide_depth;

@@ -71,6 +71,7 @@ struct QGrid { float gmin[3], scale[3], inv_scale[3]; };
 
 struct crt_bvh {
     int64_t n_tris = 0;
+    int64_t n_refs = 0;               // triangle references = records of the device triangle array (> n_tris when the host build pre-split large triangles)
     int max_leaf = 4;
     std::vector<BuildNode> nodes;     // host tree (root = 0)
     std::vector<int32_t> prim;        // leaf order -> caller's triangle id

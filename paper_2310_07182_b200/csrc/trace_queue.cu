@@ -228,7 +228,7 @@ __global__ void __launch_bounds__(TQ_BLOCK, CRT_TQ_MINB) trace_queue_kernel(cons
 }  // namespace
 
 // the queue kernel needs leaves of at most 3 triangles (ring capacity) and triangle indices below 2^27 (item = lane << 27 | index)
-bool trace_queue_supported(const crt_bvh* bvh) { return bvh->max_leaf <= 3 && bvh->n_tris < ((int64_t)1 << 27) && bvh->q_inflation <= 2.0 && bvh->q_violations == 0; }
+bool trace_queue_supported(const crt_bvh* bvh) { return bvh->max_leaf <= 3 && bvh->n_refs < ((int64_t)1 << 27) && bvh->q_inflation <= 2.0 && bvh->q_violations == 0; }
 
 crt_status launch_trace_queue(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, crt_hit* hits, unsigned long long* stats, cudaStream_t st)
 {

@@ -173,6 +173,33 @@ def test_native_tile_shapes_and_layout_errors(lib, oracle):
         assert lib.crt_layout(C.byref(fr), C.byref(o), C.byref(n), None, None) == api.CRT_ERR_INVALID_ARG
 
 
+def test_presplit_builds_a_tree_over_references(lib):
+    """crt_bvh_params.presplit: a triangle whose box is longer than presplit x the scene diagonal gets several references (one per cell of a midpoint
+    split of its box, each with the box of the part of the triangle inside the cell).  Host-only builds: more references than triangles, the tree passes
+    its check (every triangle referenced; the boxes of a multiply referenced triangle's leaves together cover it; leaves <= max_leaf; boxes nested), the
+    bounds stay the vertices' exact min / max, and one-triangle-per-leaf builds (which feed the 8-wide layout) are never split."""
+    from paper_2310_07182_b200 import api
+    one_big = np.array([[[0, 0, 0], [100, 0, 0], [0, 100, 3]]], np.float32)                   # a single triangle: 1 -> many references
+    sliver = np.concatenate([one_big, np.array([[[5, 5, 5], [5.1, 5, 5], [5, 5.1, 5]]], np.float32)])
+    for verts, max_leaf, ps, split in ((I.cornell().verts, 3, 1 / 16, True), (I.cornell().verts, 3, 0.0, False), (I.cornell().verts, 1, 1 / 16, False),
+                                       (I.interior(n_boxes=80, n_spheres=10, subdiv=2).verts, 2, 1 / 16, True), (I.landscape(n=96, n_trees=40).verts, 4, 1 / 64, True),
+                                       (one_big, 3, 1 / 16, True), (sliver, 2, 1 / 32, True), (I.cornell().verts + np.float32(3e5), 3, 1 / 16, True)):
+        v = np.ascontiguousarray(verts, np.float32)
+        pr = api.BvhParams(max_leaf, 64, 1.0, 1.0, 2, 0, 0, ps)
+        h = C.c_void_p()
+        assert lib.crt_build_bvh(None, C.c_void_p(v.ctypes.data), None, C.c_int64(len(v)), C.byref(pr), C.byref(h)) == 0
+        bad = C.c_int32(-1)
+        assert lib.crt_bvh_check(h, C.byref(bad)) == 0 and bad.value == 0, (len(v), max_leaf, ps, bad.value)
+        info = api.BvhInfo()
+        assert lib.crt_bvh_get_info(h, C.byref(info)) == 0
+        assert info.n_tris == len(v) and (info.n_refs > info.n_tris) == split and info.n_refs <= info.n_tris + max(info.n_tris // 4, 4096)
+        assert np.array_equal(np.array(list(info.bounds), np.float32), np.concatenate([v.reshape(-1, 3).min(0), v.reshape(-1, 3).max(0)]))
+        lib.crt_bvh_destroy(h)
+    for ps in (-0.1, 1.5, float("nan")):
+        pr = api.BvhParams(3, 64, 1.0, 1.0, 1, 0, 0, ps); h = C.c_void_p()
+        assert lib.crt_build_bvh(None, C.c_void_p(one_big.ctypes.data), None, C.c_int64(1), C.byref(pr), C.byref(h)) == 1
+
+
 def test_q16_box_test_error_budget():
     """The 16-bit-node box test evaluates a plane distance as t = (2^23 + q) * s + c in fp32 (csrc/trace.cu: QRay).  Re-enacting
     that arithmetic in numpy against the exact (q - o') * s shows the budget the kernel's comment states: the error, in grid steps

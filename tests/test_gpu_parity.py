@@ -230,6 +230,30 @@ def test_trace_tail_split_and_timeline(crt, ctx, oracle, scene_name, n):
     compare_hits(hits_np(oracle, h0), ho)
 
 
+@pytest.mark.parametrize("scene_name", ["cornell", "interior_small", "landscape_small"])
+def test_presplit_tree_returns_the_same_hits(crt, ctx, oracle, scene_name):
+    """Pre-splitting large triangles (crt_bvh_params.presplit, the default 1/16 and a much finer 1/128) changes the tree, not the triangles: the hit
+    records equal those of the unsplit tree and of the oracle bit for bit (D:R10: the result does not depend on the structure), also when a triangle
+    sits in many leaves and is tested more than once; the device layouts pass their check."""
+    import torch
+    scene = SCENES[scene_name]()
+    ref = None; r = None
+    for ps in (0.0, 1 / 16, 1 / 128):
+        bvh = ctx.crt_build_bvh(scene.verts, scene.mat_id, presplit=ps)
+        assert bvh.check() == 0
+        info = bvh.info()
+        if r is None:
+            r = I.random_rays(13, 30000 + 5, info["bounds"][:3], info["bounds"][3:], inactive_frac=0.05)
+        assert info["n_tris"] == scene.n_tris and (info["n_refs"] == info["n_tris"] if ps == 0 else info["n_refs"] >= info["n_tris"])
+        assert ps < 1 / 16 or scene_name == "landscape_small" or info["n_refs"] > info["n_tris"]      # (the small terrain has no triangle that long)
+        h = ctx.crt_trace(bvh, ctx.upload(r)).clone()
+        if ref is None:
+            ref = h
+            compare_hits(hits_np(oracle, h), oracle.Bvh(scene.verts).trace(r.view(oracle.RAY_DTYPE).reshape(-1)))
+        assert torch.equal(ref.view(torch.int32), h.view(torch.int32)), ps
+        bvh.destroy()
+
+
 def test_trace_tiny_scene_against_brute_force(crt, ctx, oracle):
     scene = I.furnace_sphere(1)                       # 80 triangles
     G = GpuScene(crt, scene, ctx)

@@ -426,7 +426,7 @@ def run_cuda(args):
                    "single_stream_note": "one frame at a time without per-stage events (crt_render_frame then cuts the frame into bands, option frame_bands); modes[..].mray_s are with per-stage events, unbanded",
                    "l2": f"no explicit flush: each step streams its {ws_bytes / 1e6:.0f} MB workspace plus the {info['device_bytes'] / 1e6:.0f} MB BVH (> 126 MB L2)",
                    "parallelism": "replicas only (no sharding, no collective)" if world > 1 else "single GPU",
-                   "bvh": {"nodes": info["n_nodes"], "triangle_references": info["n_refs"], "presplit": BVH_KW.get("presplit", "library default (1/16 of the scene diagonal)"), "depth": info["depth"], "sah_cost": info["sah_cost"], "device_mb": info["device_bytes"] / 1e6,
+                   "bvh": {"nodes": info["n_nodes"], "triangle_references": info["n_refs"], "presplit": BVH_KW.get("presplit", "library default (1/16 of the scene diagonal)"), "optimize": BVH_KW.get("optimize", "library default (20 iterations)"), "depth": info["depth"], "sah_cost": info["sah_cost"], "device_mb": info["device_bytes"] / 1e6,
                            "build_s": info["build_seconds"], "build_and_upload_s": build_s}},
         "modes": modes, "roofline": roofline, "cpu_baseline": cpu,
         "e2e": {"value": e2e["mray_s"], "unit": UNIT, "h2d_bytes_per_step": len(scene.materials) * 32 + 48 + 24,
@@ -739,6 +739,7 @@ def main():
     ap.add_argument("--ploc-radii", nargs="*", type=int, default=[8], help="--sweep builders: neighbour radii of the device builder")
     ap.add_argument("--variants", nargs="*", default=["3", "3:trace_exact=0", "5", "6", "4", "1"], help="--sweep kernels: trace_kernel id[:option=value,...] ...")
     ap.add_argument("--presplit", type=float, default=None, help="crt_bvh_params.presplit of the BVHs built by this run (0 = no pre-splitting of large triangles; default: the library's 1/16)")
+    ap.add_argument("--bvh-optimize", type=int, default=None, help="crt_bvh_params.optimize of the BVHs built by this run (iterations of insertion-based tree optimisation; default: the library's 20)")
     ap.add_argument("--sweep-frames", type=int, default=64)
     ap.add_argument("--all-lambert", action="store_true", help="--sweep bias: turn every glossy / mirror material of the scene into a Lambert one")
     ap.add_argument("--sweep-reference-frames", type=int, default=0, help="frames of the independent-sampling reference image of a sweep (0 = 4 x --sweep-frames)")
@@ -746,6 +747,8 @@ def main():
     args = ap.parse_args()
     if args.presplit is not None:
         BVH_KW["presplit"] = args.presplit
+    if args.bvh_optimize is not None:
+        BVH_KW["optimize"] = args.bvh_optimize
     if args.warmup < 3 and args.impl == "cuda":
         args.warmup = 3
     if args.sweep:

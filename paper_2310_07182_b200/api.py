@@ -63,7 +63,7 @@ class SceneMats(C.Structure):
 
 class BvhParams(C.Structure):
     _fields_ = [("max_leaf", C.c_int32), ("sah_bins", C.c_int32), ("cost_traversal", C.c_float), ("cost_intersect", C.c_float),
-                ("n_threads", C.c_int32), ("builder", C.c_int32), ("ploc_radius", C.c_int32), ("presplit", C.c_float)]
+                ("n_threads", C.c_int32), ("builder", C.c_int32), ("ploc_radius", C.c_int32), ("presplit", C.c_float), ("optimize", C.c_int32)]
 
 
 class BvhInfo(C.Structure):
@@ -231,7 +231,7 @@ class Context:
         return a.value, b.value
 
     # ---- a0 -----------------------------------------------------------------------------------------
-    def crt_build_bvh(self, verts, mat_id, max_leaf=3, sah_bins=64, n_threads=0, cost_traversal=1.0, cost_intersect=1.0, builder=0, ploc_radius=0, presplit=1.0 / 16):
+    def crt_build_bvh(self, verts, mat_id, max_leaf=3, sah_bins=64, n_threads=0, cost_traversal=1.0, cost_intersect=1.0, builder=0, ploc_radius=0, presplit=1.0 / 16, optimize=20):
         """verts: numpy float32[n,3,3] or torch tensor (host or device); mat_id int32[n].  builder: 0 host SAH, 1 device PLOC."""
         if isinstance(verts, np.ndarray):
             verts = np.ascontiguousarray(verts, np.float32)
@@ -239,7 +239,7 @@ class Context:
             n = verts.size // 9
         else:
             n = verts.numel() // 9
-        pr = BvhParams(max_leaf, sah_bins, cost_traversal, cost_intersect, n_threads, int(builder), int(ploc_radius), float(presplit))
+        pr = BvhParams(max_leaf, sah_bins, cost_traversal, cost_intersect, n_threads, int(builder), int(ploc_radius), float(presplit), int(optimize))
         h = C.c_void_p()
         self._check(lib().crt_build_bvh(self.handle, _ptr(verts), _ptr(mat_id), C.c_int64(n), C.byref(pr), C.byref(h)))
         return Bvh(self, h)

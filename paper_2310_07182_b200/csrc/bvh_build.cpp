@@ -7,6 +7,7 @@
 #include <chrono>
 #include <cmath>
 #include <condition_variable>
+#include <cstdlib>
 #include <cstring>
 #include <deque>
 #include <functional>
@@ -224,6 +225,88 @@ void presplit_triangle(const float* tv, int32_t prim, double limit, int64_t& bud
     }
 }
 
+// ---- insertion-based optimisation of a built tree (crt_bvh_params.optimize; Bittner, Hapala & Havran 2013, restated) -------------------------------
+// Repeatedly: take the inner nodes that look worst (large, with children much smaller than themselves), detach the two children of each, close the gap
+// (the node's sibling takes its parent's place), and put each child back at the position of the whole tree where it adds the least surface area, found by a
+// best-first search bounded by the best total so far.  Leaves keep their ranges, the node count stays, the root stays node 0.
+struct TreeOpt {
+    struct Cand { double induced; int32_t node; bool operator<(const Cand& o) const { return induced > o.induced; } };      // min-heap on the induced cost
+    std::vector<BuildNode>& nd;
+    std::vector<int32_t> parent;
+    std::vector<Cand> heap_;
+    explicit TreeOpt(std::vector<BuildNode>& n) : nd(n), parent(n.size(), -1)
+    {
+        for (size_t i = 0; i < nd.size(); ++i) if (nd[i].left >= 0) { parent[nd[i].left] = (int32_t)i; parent[nd[i].right] = (int32_t)i; }
+    }
+    static double area(const BuildNode& x)
+    {
+        const double dx = (double)x.bmax[0] - x.bmin[0], dy = (double)x.bmax[1] - x.bmin[1], dz = (double)x.bmax[2] - x.bmin[2];
+        return dx * dy + dy * dz + dz * dx;
+    }
+    static double union_area(const BuildNode& x, const BuildNode& y)
+    {
+        double d[3];
+        for (int k = 0; k < 3; ++k) d[k] = (double)std::max(x.bmax[k], y.bmax[k]) - (double)std::min(x.bmin[k], y.bmin[k]);
+        return d[0] * d[1] + d[1] * d[2] + d[2] * d[0];
+    }
+    void refit(int32_t i)
+    {
+        const BuildNode& l = nd[nd[i].left]; const BuildNode& r = nd[nd[i].right];
+        for (int k = 0; k < 3; ++k) { nd[i].bmin[k] = std::min(l.bmin[k], r.bmin[k]); nd[i].bmax[k] = std::max(l.bmax[k], r.bmax[k]); }
+    }
+    void refit_up(int32_t i) { for (; i >= 0; i = parent[i]) refit(i); }
+    // total inner-node area (the part of the SAH cost the optimisation can change)
+    double inner_area() const { double a = 0; for (const BuildNode& x : nd) if (x.left >= 0) a += area(x); return a; }
+
+    // where to hang the detached subtree `sub`: the node X minimising area(X u sub) + the growth of X's ancestors
+    int32_t best_position(int32_t sub)
+    {
+        const double a_sub = area(nd[sub]);
+        std::vector<Cand>& heap = heap_; heap.clear();
+        heap.push_back({0.0, 0});
+        double best = std::numeric_limits<double>::infinity(); int32_t best_node = nd[0].left;      // (never the root itself: the root stays node 0)
+        while (!heap.empty()) {
+            std::pop_heap(heap.begin(), heap.end()); const Cand c = heap.back(); heap.pop_back();
+            if (c.induced + a_sub >= best) break;                     // nothing below can beat the best: its cost is at least induced + area(sub)
+            const double direct = union_area(nd[c.node], nd[sub]);
+            if (c.node != 0 && c.induced + direct < best) { best = c.induced + direct; best_node = c.node; }
+            if (nd[c.node].left >= 0) {
+                const double ind = c.induced + direct - area(nd[c.node]);      // what node c grows by if `sub` goes somewhere below it
+                if (ind + a_sub < best) {
+                    heap.push_back({ind, nd[c.node].left}); std::push_heap(heap.begin(), heap.end());
+                    heap.push_back({ind, nd[c.node].right}); std::push_heap(heap.begin(), heap.end());
+                }
+            }
+        }
+        return best_node;
+    }
+    // hangs `sub` beside x under the free node `link`, which takes x's place
+    void insert(int32_t sub, int32_t x, int32_t link)
+    {
+        const int32_t px = parent[x];
+        nd[link].left = x; nd[link].right = sub; nd[link].first = 0; nd[link].count = 0;
+        parent[x] = link; parent[sub] = link; parent[link] = px;
+        if (nd[px].left == x) nd[px].left = link; else nd[px].right = link;
+        refit_up(link);
+    }
+    // one node: detach its children, close the gap, reinsert both.  Needs a grandparent (root 0 and its children stay).
+    bool reinsert_children(int32_t n)
+    {
+        if (nd[n].left < 0) return false;
+        const int32_t p = parent[n]; if (p <= 0) return false;          // n is the root or a child of the root
+        const int32_t g = parent[p];
+        const int32_t sib = nd[p].left == n ? nd[p].right : nd[p].left;
+        int32_t l = nd[n].left, r = nd[n].right;
+        if (nd[g].left == p) nd[g].left = sib; else nd[g].right = sib;
+        parent[sib] = g; refit_up(g);
+        parent[l] = parent[r] = -1;
+        if (area(nd[l]) < area(nd[r])) std::swap(l, r);                   // the larger subtree first
+        insert(l, best_position(l), p);
+        insert(r, best_position(r), n);
+        return true;
+    }
+};
+
 }  // namespace
 
 // Builds the host tree.  Returns false on failure.
@@ -288,7 +371,50 @@ bool crt_bvh_build_host(crt_bvh* b, const float* verts, int64_t n, const crt_bvh
         }
         b->nodes.resize((size_t)B.n_nodes.load());
         for (int64_t i = 0; i < nr; ++i) b->prim[i] = refs[b->prim[i]].prim;
-        b->depth = B.max_depth.load();
+        // tree rotations (Kensler 2008, restated): bottom-up (a child's index is always larger than its parent's), a node may exchange one of its children
+        // with a grandchild on the other side when that shrinks the box of the child that is rebuilt; leaf ranges are untouched
+        if (pr.optimize > 0 && b->nodes.size() >= 16) {
+            // insertion-based optimisation (TreeOpt above): per iteration the worst-looking 2 % of the inner nodes (at most 20,000), ranked by area x
+            // (area / smaller child) x (area / mean child); four consecutive windows of that ranking take turns, so that nodes which are already placed
+            // as well as the search can place them are not picked over and over
+            TreeOpt T(b->nodes);
+            std::vector<std::pair<double, int32_t>> rank;
+            const auto worse = [](const std::pair<double, int32_t>& a, const std::pair<double, int32_t>& c) { return a.first > c.first || (a.first == c.first && a.second < c.second); };
+            std::vector<double> total{T.inner_area()};        // summed inner-node area after each iteration
+            for (int it = 0; it < pr.optimize; ++it) {
+                // no progress worth the time (a terrain grid, say, is as good as it gets after the build): less than 0.2 % over the last four iterations
+                if (it >= 4 && total[it - 4] - total[it] < 0.002 * total[it]) break;
+                if (it == 1 && total[0] - total[1] < 0.0005 * total[1]) break;      // the most promising 2 % gained next to nothing
+                rank.clear();
+                for (size_t i = 1; i < b->nodes.size(); ++i) {
+                    const BuildNode& x = b->nodes[i];
+                    if (x.left < 0 || T.parent[i] <= 0) continue;
+                    const double a = TreeOpt::area(x), al = TreeOpt::area(b->nodes[x.left]), ar = TreeOpt::area(b->nodes[x.right]);
+                    const double mn = std::max(std::min(al, ar), 1e-300), sum = std::max(al + ar, 1e-300);
+                    rank.emplace_back(a * (a / mn) * (2.0 * a / sum), (int32_t)i);
+                }
+                if (rank.empty()) break;
+                const size_t batch = std::min<size_t>(rank.size(), std::max<size_t>(64, std::min<size_t>(rank.size() / 50, 20000)));
+                const size_t off = std::min(rank.size() - batch, (size_t)(it % 4) * batch);
+                std::nth_element(rank.begin(), rank.begin() + off, rank.end(), worse);
+                std::nth_element(rank.begin() + off, rank.begin() + off + batch - 1, rank.end(), worse);
+                std::sort(rank.begin() + off, rank.begin() + off + batch, worse);      // a fixed processing order for a given tree
+                // (putting two children back one after the other is not guaranteed to pay: an iteration that loses is undone; the first one, which decides
+                // whether the tree is worth optimising at all, runs without the copy)
+                std::vector<BuildNode> before_nodes; std::vector<int32_t> before_parent;
+                if (it > 0) { before_nodes = b->nodes; before_parent = T.parent; }
+                for (size_t k = off; k < off + batch; ++k) T.reinsert_children(rank[k].second);
+                total.push_back(T.inner_area());
+                if (it > 0 && total.back() > total[total.size() - 2]) { b->nodes = before_nodes; T.parent = before_parent; total.back() = total[total.size() - 2]; }
+            }
+            std::vector<std::pair<int32_t, int>> st{{0, 1}}; int md = 0;
+            while (!st.empty()) {
+                const std::pair<int32_t, int> t = st.back(); st.pop_back(); md = std::max(md, t.second);
+                const BuildNode& x = b->nodes[t.first];
+                if (x.left >= 0) { st.push_back({x.left, t.second + 1}); st.push_back({x.right, t.second + 1}); }
+            }
+            b->depth = md;
+        } else b->depth = B.max_depth.load();
         // SAH cost (relative to the root area) before padding
         double ra = root.half_area(), cost = 0;
         for (const BuildNode& nd : b->nodes) {

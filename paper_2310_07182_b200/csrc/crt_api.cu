@@ -147,10 +147,11 @@ crt_status crt_build_bvh(crt_ctx* ctx, const float* verts, const int32_t* mat_id
     CrtDeviceGuard dev_guard_(ctx ? ctx->device : -1);
     if (n_tris < 0 || (n_tris > 0 && !verts)) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "build_bvh: bad triangle array");
     if (n_tris >= ((int64_t)1 << 28)) return crt_fail(ctx, CRT_ERR_UNSUPPORTED, "build_bvh: more than 2^28 triangles");
-    crt_bvh_params pr = {3, 64, 1.0f, 1.0f, 0, 0, 0, 0.0625f};
+    crt_bvh_params pr = {3, 64, 1.0f, 1.0f, 0, 0, 0, 0.0625f, 20};
     if (params) pr = *params;
     if (pr.max_leaf < 1 || pr.max_leaf > 8) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "build_bvh: max_leaf %d not in [1,8]", pr.max_leaf);
     if (pr.sah_bins == 0) pr.sah_bins = 64;
+    if (pr.optimize < 0 || pr.optimize > 10000) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "build_bvh: optimize %d not in [0,10000]", pr.optimize);
     if (!(pr.presplit >= 0.f && pr.presplit <= 1.f)) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "build_bvh: presplit %g not in [0,1]", (double)pr.presplit);
     std::vector<float> hv; std::vector<int32_t> hm((size_t)n_tris, 0);
     const float* v = verts;

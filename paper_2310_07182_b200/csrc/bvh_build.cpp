@@ -225,6 +225,17 @@ void presplit_triangle(const float* tv, int32_t prim, double limit, int64_t& bud
     }
 }
 
+int tree_depth(const std::vector<BuildNode>& nd)
+{
+    std::vector<std::pair<int32_t, int>> st{{0, 1}}; int md = 0;
+    while (!st.empty()) {
+        const std::pair<int32_t, int> t = st.back(); st.pop_back(); md = std::max(md, t.second);
+        const BuildNode& x = nd[t.first];
+        if (x.left >= 0) { st.push_back({x.left, t.second + 1}); st.push_back({x.right, t.second + 1}); }
+    }
+    return md;
+}
+
 // ---- insertion-based optimisation of a built tree (crt_bvh_params.optimize; Bittner, Hapala & Havran 2013, restated) -------------------------------
 // Repeatedly: take the inner nodes that look worst (large, with children much smaller than themselves), detach the two children of each, close the gap
 // (the node's sibling takes its parent's place), and put each child back at the position of the whole tree where it adds the least surface area, found by a
@@ -399,21 +410,16 @@ bool crt_bvh_build_host(crt_bvh* b, const float* verts, int64_t n, const crt_bvh
                 std::nth_element(rank.begin(), rank.begin() + off, rank.end(), worse);
                 std::nth_element(rank.begin() + off, rank.begin() + off + batch - 1, rank.end(), worse);
                 std::sort(rank.begin() + off, rank.begin() + off + batch, worse);      // a fixed processing order for a given tree
-                // (putting two children back one after the other is not guaranteed to pay: an iteration that loses is undone; the first one, which decides
-                // whether the tree is worth optimising at all, runs without the copy)
-                std::vector<BuildNode> before_nodes; std::vector<int32_t> before_parent;
-                if (it > 0) { before_nodes = b->nodes; before_parent = T.parent; }
+                // (putting two children back one after the other is not guaranteed to pay: an iteration that loses is undone; so is one that makes the tree
+                // deeper than the traversal stack allows -- many identical boxes can be chained into a list -- and the optimisation ends there)
+                const std::vector<BuildNode> before_nodes = b->nodes; const std::vector<int32_t> before_parent = T.parent;
                 for (size_t k = off; k < off + batch; ++k) T.reinsert_children(rank[k].second);
                 total.push_back(T.inner_area());
-                if (it > 0 && total.back() > total[total.size() - 2]) { b->nodes = before_nodes; T.parent = before_parent; total.back() = total[total.size() - 2]; }
+                const bool too_deep = tree_depth(b->nodes) > std::max(56, B.max_depth.load());
+                if (too_deep || total.back() > total[total.size() - 2]) { b->nodes = before_nodes; T.parent = before_parent; total.back() = total[total.size() - 2]; }
+                if (too_deep) break;
             }
-            std::vector<std::pair<int32_t, int>> st{{0, 1}}; int md = 0;
-            while (!st.empty()) {
-                const std::pair<int32_t, int> t = st.back(); st.pop_back(); md = std::max(md, t.second);
-                const BuildNode& x = b->nodes[t.first];
-                if (x.left >= 0) { st.push_back({x.left, t.second + 1}); st.push_back({x.right, t.second + 1}); }
-            }
-            b->depth = md;
+            b->depth = tree_depth(b->nodes);
         } else b->depth = B.max_depth.load();
         // SAH cost (relative to the root area) before padding
         double ra = root.half_area(), cost = 0;

@@ -226,6 +226,34 @@ def test_tree_optimisation_keeps_the_invariants_and_lowers_the_cost(lib):
     assert lib.crt_build_bvh(None, C.c_void_p(v.ctypes.data), None, C.c_int64(len(v)), C.byref(pr), C.byref(h)) == 1
 
 
+def test_builder_steps_on_degenerate_inputs(lib):
+    """Pre-splitting and tree optimisation on inputs that could break them: point and collinear triangles, hundreds of identical triangles (identical boxes can
+    be chained into a list: the optimisation must not deepen the tree beyond the traversal stack), slivers, one giant triangle among tiny ones, coordinates
+    far from the origin.  Every build succeeds and passes its check."""
+    from paper_2310_07182_b200 import api
+    rng = np.random.default_rng(7)
+    cases = {
+        "points": np.repeat(rng.random((500, 1, 3)), 3, axis=1),
+        "identical": np.tile(rng.random((1, 3, 3)), (300, 1, 1)),
+        "identical big": np.tile(rng.random((1, 3, 3)) * 100, (2000, 1, 1)),
+        "slivers": np.stack([rng.random((200, 3)) * 100, rng.random((200, 3)) * 100, rng.random((200, 3)) * 100], 1) * np.array([1, 1e-6, 1e-6]),
+        "giant+tiny": np.concatenate([np.array([[[-1e4, 0, -1e4], [1e4, 0, -1e4], [0, 0, 1e4]]]), rng.random((3000, 3, 3)) * 0.01 + rng.random((3000, 1, 3)) * 10]),
+        "collinear": np.stack([np.zeros((50, 3)), np.ones((50, 3)), 2 * np.ones((50, 3))], 1) * rng.random((50, 1, 1)) * 50,
+        "offset": rng.random((1000, 3, 3)) + 4e6,
+        "two": rng.random((2, 3, 3)) * 1000,
+    }
+    for name, verts in cases.items():
+        v = np.ascontiguousarray(verts, np.float32)
+        for max_leaf in (1, 3, 8):
+            for ps, opt in ((1 / 16, 20), (1 / 256, 50), (0.0, 200)):
+                pr = api.BvhParams(max_leaf, 64, 1.0, 1.0, 2, 0, 0, ps, opt); h = C.c_void_p()
+                assert lib.crt_build_bvh(None, C.c_void_p(v.ctypes.data), None, C.c_int64(len(v)), C.byref(pr), C.byref(h)) == 0, (name, max_leaf, ps, opt)
+                bad = C.c_int32(-1)
+                assert lib.crt_bvh_check(h, C.byref(bad)) == 0 and bad.value == 0, (name, max_leaf, ps, opt, bad.value)
+                info = api.BvhInfo(); assert lib.crt_bvh_get_info(h, C.byref(info)) == 0 and info.depth <= 60
+                lib.crt_bvh_destroy(h)
+
+
 def test_q16_box_test_error_budget():
     """The 16-bit-node box test evaluates a plane distance as t = (2^23 + q) * s + c in fp32 (csrc/trace.cu: QRay).  Re-enacting
     that arithmetic in numpy against the exact (q - o') * s shows the budget the kernel's comment states: the error, in grid steps

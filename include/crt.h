@@ -220,6 +220,16 @@ crt_status crt_ray_code_encode(crt_ctx* ctx, const crt_bvh* bvh, int32_t code, c
 crt_status crt_radix_sort_pairs(crt_ctx* ctx, const uint32_t* keys_in, const int32_t* vals_in, int64_t n,
                                 uint32_t* keys_out, int32_t* vals_out, void* scratch, size_t scratch_bytes, void* stream);
 size_t crt_radix_sort_scratch_bytes(int64_t n);
+/* The same sort for callers that cannot allocate (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc): the scratch is a static device array inside the library (17.3 MB per GPU that loads the library, held until the process
+ * exits), so this call performs no cudaMalloc / cudaFree and calls no allocating library routine; the caller passes inputs and outputs
+ * only.  n <= crt_radix_sort_noalloc_max_n() = 2,097,152 pairs, else CRT_ERR_UNSUPPORTED (use crt_radix_sort_pairs); CRT_ERR_STATE if
+ * the array's device address could not be resolved when the context was created.  Same result as crt_radix_sort_pairs, bit for bit.
+ * Every call on a device shares the one array (it keeps the last call's contents; nothing in it has to start at zero): calls whose
+ * kernels OVERLAP on the GPU -- different streams, or different contexts of one device -- race; serialise them. */
+crt_status crt_radix_sort_pairs_noalloc(crt_ctx* ctx, const uint32_t* keys_in, const int32_t* vals_in, int64_t n,
+                                        uint32_t* keys_out, int32_t* vals_out, void* stream);
+int64_t crt_radix_sort_noalloc_max_n(void);
 
 /* ---- a5: BVH traversal ("the most time-consuming segment") ------------------------------- */
 /* hits[i] = nearest intersection of rays[i] with tmin < t < tmax; ties -> lowest primitive id (D:R10).

@@ -33,7 +33,7 @@ EXPORTS = [
     "crt_create", "crt_destroy", "crt_last_error", "crt_set_option", "crt_measure_peaks",
     "crt_build_bvh", "crt_bvh_destroy", "crt_bvh_get_info", "crt_bvh_check", "crt_layout", "crt_paths_init",
     "crt_trace_primary", "crt_generate_secondary", "crt_generate_secondary_scratch_bytes",
-    "crt_morton_encode", "crt_ray_code_encode", "crt_radix_sort_pairs", "crt_radix_sort_scratch_bytes", "crt_trace", "crt_trace_stats", "crt_trace_timeline",
+    "crt_morton_encode", "crt_ray_code_encode", "crt_radix_sort_pairs", "crt_radix_sort_scratch_bytes", "crt_radix_sort_pairs_noalloc", "crt_radix_sort_noalloc_max_n", "crt_trace", "crt_trace_stats", "crt_trace_timeline",
     "crt_shade_accumulate", "crt_render_frame", "crt_frame_workspace_bytes", "crt_frame_times", "crt_frame_bounce_times",
     "crt_render_frame_host", "crt_render_frame_host_resident", "crt_render_frame_host_resident_async", "crt_frame_host_extra_bytes",
 ]
@@ -93,6 +93,7 @@ def lib():
         for name in ("crt_generate_secondary_scratch_bytes", "crt_radix_sort_scratch_bytes", "crt_frame_workspace_bytes",
                      "crt_frame_host_extra_bytes"):
             getattr(L, name).restype = C.c_size_t
+        L.crt_radix_sort_noalloc_max_n.restype = C.c_int64
         _lib = L
     return _lib
 
@@ -290,6 +291,12 @@ class Context:
         self._check(lib().crt_radix_sort_pairs(self.handle, _ptr(keys), _ptr(vals), C.c_int64(n), _ptr(ko), _ptr(vo), _ptr(scratch),
                                                C.c_size_t(scratch.numel()), _stream(stream)))
         return ko, vo
+
+    def crt_radix_sort_pairs_noalloc(self, keys, vals, keys_out, vals_out, stream=None):
+        """The same sort with the library's static scratch (no allocation inside the call; n <= crt_radix_sort_noalloc_max_n()).
+        The caller passes the output tensors; calls that overlap on the GPU race (include/crt.h)."""
+        self._check(lib().crt_radix_sort_pairs_noalloc(self.handle, _ptr(keys), _ptr(vals), C.c_int64(keys.shape[0]), _ptr(keys_out), _ptr(vals_out), _stream(stream)))
+        return keys_out, vals_out
 
     # ---- a5 -----------------------------------------------------------------------------------------
     def crt_trace(self, bvh, rays, hits=None, stream=None):

@@ -87,6 +87,7 @@ crt_status crt_create(int32_t device, crt_ctx** out)
     cudaDeviceProp prop;
     CRT_CUDA(nullptr, cudaGetDeviceProperties(&prop, device));
     if (prop.major < 10) return crt_fail(nullptr, CRT_ERR_UNSUPPORTED, "crt_create: device is sm_%d%d; libcrt is built for sm_100a only", prop.major, prop.minor);
+    radix_sort_noalloc_setup(device);      // address of the static scratch of crt_radix_sort_pairs_noalloc on this device (sort.cu); not fatal here
     crt_ctx* c = new crt_ctx();
     c->device = device; c->n_sms = prop.multiProcessorCount;
     if (cudaMalloc(&c->d_counter, 4096) != cudaSuccess) { delete c; return crt_fail(nullptr, CRT_ERR_NOMEM, "crt_create: cudaMalloc failed"); }
@@ -346,6 +347,19 @@ crt_status crt_radix_sort_pairs(crt_ctx* ctx, const uint32_t* keys_in, const int
     NEED_ALIGNED("radix_sort_pairs", keys_out, 4); NEED_ALIGNED("radix_sort_pairs", vals_out, 4); NEED_ALIGNED("radix_sort_pairs", scratch, 16);
     if (keys_out == keys_in || vals_out == vals_in) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "radix_sort_pairs: in-place sort is not supported");
     return launch_radix_sort(ctx, keys_in, vals_in, n, keys_out, vals_out, scratch, scratch_bytes, (cudaStream_t)stream);
+}
+
+int64_t crt_radix_sort_noalloc_max_n(void) { return radix_sort_noalloc_max_n(); }
+
+crt_status crt_radix_sort_pairs_noalloc(crt_ctx* ctx, const uint32_t* keys_in, const int32_t* vals_in, int64_t n, uint32_t* keys_out, int32_t* vals_out, void* stream)
+{
+    NEED_CTX("radix_sort_pairs_noalloc");
+    if (n < 0) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "radix_sort_pairs_noalloc: negative size");
+    if (n == 0) return CRT_OK;
+    NEED_ALIGNED("radix_sort_pairs_noalloc", keys_in, 4); NEED_ALIGNED("radix_sort_pairs_noalloc", vals_in, 4);
+    NEED_ALIGNED("radix_sort_pairs_noalloc", keys_out, 4); NEED_ALIGNED("radix_sort_pairs_noalloc", vals_out, 4);
+    if (keys_out == keys_in || vals_out == vals_in) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "radix_sort_pairs_noalloc: in-place sort is not supported");
+    return launch_radix_sort_noalloc(ctx, keys_in, vals_in, n, keys_out, vals_out, (cudaStream_t)stream);
 }
 
 crt_status crt_trace(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n_rays, crt_hit* hits, void* stream)

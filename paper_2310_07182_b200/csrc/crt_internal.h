@@ -158,6 +158,9 @@ static inline int crt_mode_sort_code(int mode) { return mode == CRT_MODE_MORTON_
 crt_status launch_radix_sort(crt_ctx* ctx, const uint32_t* kin, const int32_t* vin, int64_t n, uint32_t* kout, int32_t* vout,
                              void* scratch, size_t scratch_bytes, cudaStream_t st);
 size_t radix_sort_scratch_bytes(int64_t n);
+void radix_sort_noalloc_setup(int device);
+int64_t radix_sort_noalloc_max_n();
+crt_status launch_radix_sort_noalloc(crt_ctx* ctx, const uint32_t* kin, const int32_t* vin, int64_t n, uint32_t* kout, int32_t* vout, cudaStream_t st);
 crt_status launch_shade(crt_ctx* ctx, const crt_bvh* bvh, const crt_scene_mats& mats, const crt_frame& f, int is_last,
                         const crt_ray* rays, const crt_hit* hits, const int32_t* r2p, int64_t n, crt_path_state* paths, float* accum, cudaStream_t st, bool paths_by_slot = false, const Layout* pixel_order = nullptr, const Band* band = nullptr);
 crt_status launch_paths_init(crt_ctx* ctx, crt_path_state* paths, int64_t n, cudaStream_t st);

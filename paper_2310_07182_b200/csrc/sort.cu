@@ -148,7 +148,21 @@ __global__ void __launch_bounds__(RS_THREADS, 4) rs_scatter_kernel(const uint32_
     }
 }
 
-inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+constexpr size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+// ---- scratch of the entry point that allocates nothing (crt_radix_sort_pairs_noalloc) ------------------------------------------
+// The same layout as the caller-provided scratch of launch_radix_sort (ping-pong keys, ping-pong values, the (digit, block) histogram
+// table, the 256 digit totals), sized for CRT_RADIX_SORT_NOALLOC_MAX_N pairs, in a file-scope device array: 17.3 MB that every GPU
+// which loads the library holds until the process exits.  In HOST code the name below is a host-side stand-in, not a device address;
+// the address is resolved once per device by radix_sort_noalloc_setup (cudaGetSymbolAddress with that device current) and kept in
+// g_rs_static_ptr.
+constexpr int64_t RS_STATIC_MAX_N = (int64_t)1 << 21;          // 2,097,152 pairs: covers the 2,088,960 ray slots of a 1920x1080 frame (BASELINE config 2 / 5)
+constexpr size_t RS_STATIC_BYTES = 2 * align256((size_t)RS_STATIC_MAX_N * 4) + align256((size_t)((RS_STATIC_MAX_N + RS_TILE - 1) / RS_TILE) * 256 * 4) + align256(256 * 4) + 256;
+static __device__ __align__(256) unsigned char g_rs_static_scratch[RS_STATIC_BYTES];
+
+constexpr int RS_MAX_DEVICES = 64;
+void* g_rs_static_ptr[RS_MAX_DEVICES] = {};                     // device address of g_rs_static_scratch on each device (null: not resolved)
+cudaError_t g_rs_static_err[RS_MAX_DEVICES] = {};               // why not
 
 }  // namespace
 
@@ -180,4 +194,35 @@ crt_status launch_radix_sort(crt_ctx* ctx, const uint32_t* kin, const int32_t* v
     }
     CRT_CHECK_LAUNCH(ctx, "radix_sort");
     return CRT_OK;
+}
+
+// Set-up of the no-allocation sort, once per device, called by crt_create with `device` current: resolves the device address of the
+// static scratch array.  A failure is kept and reported by the entry point (crt_create itself does not depend on it).
+void radix_sort_noalloc_setup(int device)
+{
+    if (device < 0 || device >= RS_MAX_DEVICES || g_rs_static_ptr[device]) return;
+    void* p = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress(&p, g_rs_static_scratch);
+    if (e == cudaSuccess && p) g_rs_static_ptr[device] = p;
+    else { g_rs_static_err[device] = e == cudaSuccess ? cudaErrorInvalidSymbol : e; cudaGetLastError(); }
+}
+
+int64_t radix_sort_noalloc_max_n() { return RS_STATIC_MAX_N; }
+
+// The sort of launch_radix_sort with the library's static scratch: no cudaMalloc, cudaFree or allocating library call on this path.
+// Nothing in the scratch has to start at zero: every histogram entry, total and ping-pong element a pass reads was written earlier in
+// the same call (rs_hist_kernel writes all 256 x n_blocks entries it later reads), so the previous call's contents are never read.
+// All calls on a device share the one array: two calls whose kernels overlap on the GPU (different streams, or different contexts of
+// one device) race; callers serialise them (one stream, or an event between them).
+crt_status launch_radix_sort_noalloc(crt_ctx* ctx, const uint32_t* kin, const int32_t* vin, int64_t n, uint32_t* kout, int32_t* vout, cudaStream_t st)
+{
+    if (n == 0) return CRT_OK;
+    if (n > RS_STATIC_MAX_N)
+        return crt_fail(ctx, CRT_ERR_UNSUPPORTED, "radix_sort_pairs_noalloc: %lld pairs exceed the static scratch's maximum of %lld (use crt_radix_sort_pairs with caller scratch)",
+                        (long long)n, (long long)RS_STATIC_MAX_N);
+    const int dev = ctx->device;
+    if (dev < 0 || dev >= RS_MAX_DEVICES || !g_rs_static_ptr[dev])
+        return crt_fail(ctx, CRT_ERR_STATE, "radix_sort_pairs_noalloc: the static scratch's device address was not resolved at crt_create (%s)",
+                        dev >= 0 && dev < RS_MAX_DEVICES ? cudaGetErrorString(g_rs_static_err[dev]) : "device index beyond the table");
+    return launch_radix_sort(ctx, kin, vin, n, kout, vout, g_rs_static_ptr[dev], RS_STATIC_BYTES, st);
 }

@@ -613,7 +613,7 @@ def run_builders(args):
     scene = I.by_name(name, **kw).with_camera(w, h)
     ctx = crt.Context(0)
     trees = []
-    for label, bkw in [("host SAH (64 bins)", dict(builder=0))] + [(f"device PLOC radius {r}", dict(builder=1, ploc_radius=r)) for r in args.ploc_radii] + [(f"device clustering radius {args.ploc_radii[0]} + host layout", dict(builder=2, ploc_radius=args.ploc_radii[0]))]:
+    for label, bkw in [("host SAH (64 bins)", dict(builder=0))] + [(f"device PLOC radius {r}", dict(builder=1, ploc_radius=r)) for r in args.ploc_radii] + [(f"device clustering radius {args.ploc_radii[0]} + host optimisation and layout", dict(builder=2, ploc_radius=args.ploc_radii[0]))]:
         t0 = time.time(); bvh = ctx.crt_build_bvh(scene.verts, scene.mat_id, **bkw); wall = time.time() - t0
         info = bvh.info()
         trees.append((label, bvh, dict(builder=label, wall_seconds=wall, hierarchy_seconds=info["build_seconds"], device_build_seconds=info["device_build_seconds"],

@@ -88,7 +88,8 @@ typedef struct { int32_t mode, group_w, group_h, stride, stride_y, partition_rul
  * env: radiance on a miss = lerp(env[0..2], env[3..5], 0.5*(d.y+1)) (D:R14). */
 typedef struct { const crt_material* materials; int32_t n_materials; float env[6]; } crt_scene_mats;
 /* builder: 0 = host (binned surface-area heuristic, threaded); 1 = device (parallel locally-ordered clustering AND the traversal layouts
- * written by the GPU, csrc/bvh_ploc.cu; needs a context); 2 = the device's clustering with the host's layout code (cross-check of 1);
+ * written by the GPU, csrc/bvh_ploc.cu; needs a context); 2 = the device's clustering with the host's tree optimisation (`optimize`) and layout code
+ * (cross-check of 1; profiles/r02n);
  * ploc_radius: neighbours searched on either side of a cluster in Morton order (0 = 8; at most 128).
  * presplit (host builder, max_leaf > 1): a triangle whose box is longer than presplit x the scene's diagonal on some axis is given several REFERENCES,
  * one per cell of a recursive midpoint split of its box, each with the box of the part of the triangle inside the cell, and the tree is built over

@@ -320,6 +320,50 @@ struct TreeOpt {
 
 }  // namespace
 
+// Insertion-based optimisation of b->nodes (TreeOpt above; crt_bvh_params.optimize iterations; boxes unpadded or padded alike).  Returns the tree's depth
+// afterwards (built_depth when nothing was done).  Used by the host builder and by builder 2 (device clustering + host layout).
+int crt_bvh_optimize_tree(crt_bvh* b, const crt_bvh_params& pr, int built_depth)
+{
+    if (pr.optimize > 0 && b->nodes.size() >= 16) {
+        // insertion-based optimisation (TreeOpt above): per iteration the worst-looking 2 % of the inner nodes (at most 20,000), ranked by area x
+        // (area / smaller child) x (area / mean child); four consecutive windows of that ranking take turns, so that nodes which are already placed
+        // as well as the search can place them are not picked over and over
+        TreeOpt T(b->nodes);
+        std::vector<std::pair<double, int32_t>> rank;
+        const auto worse = [](const std::pair<double, int32_t>& a, const std::pair<double, int32_t>& c) { return a.first > c.first || (a.first == c.first && a.second < c.second); };
+        std::vector<double> total{T.inner_area()};        // summed inner-node area after each iteration
+        for (int it = 0; it < pr.optimize; ++it) {
+            // no progress worth the time (a terrain grid, say, is as good as it gets after the build): less than 0.2 % over the last four iterations
+            if (it >= 4 && total[it - 4] - total[it] < 0.002 * total[it]) break;
+            if (it == 1 && total[0] - total[1] < 0.0005 * total[1]) break;      // the most promising 2 % gained next to nothing
+            rank.clear();
+            for (size_t i = 1; i < b->nodes.size(); ++i) {
+                const BuildNode& x = b->nodes[i];
+                if (x.left < 0 || T.parent[i] <= 0) continue;
+                const double a = TreeOpt::area(x), al = TreeOpt::area(b->nodes[x.left]), ar = TreeOpt::area(b->nodes[x.right]);
+                const double mn = std::max(std::min(al, ar), 1e-300), sum = std::max(al + ar, 1e-300);
+                rank.emplace_back(a * (a / mn) * (2.0 * a / sum), (int32_t)i);
+            }
+            if (rank.empty()) break;
+            const size_t batch = std::min<size_t>(rank.size(), std::max<size_t>(64, std::min<size_t>(rank.size() / 50, 20000)));
+            const size_t off = std::min(rank.size() - batch, (size_t)(it % 4) * batch);
+            std::nth_element(rank.begin(), rank.begin() + off, rank.end(), worse);
+            std::nth_element(rank.begin() + off, rank.begin() + off + batch - 1, rank.end(), worse);
+            std::sort(rank.begin() + off, rank.begin() + off + batch, worse);      // a fixed processing order for a given tree
+            // (putting two children back one after the other is not guaranteed to pay: an iteration that loses is undone; so is one that makes the tree
+            // deeper than the traversal stack allows -- many identical boxes can be chained into a list -- and the optimisation ends there)
+            const std::vector<BuildNode> before_nodes = b->nodes; const std::vector<int32_t> before_parent = T.parent;
+            for (size_t k = off; k < off + batch; ++k) T.reinsert_children(rank[k].second);
+            total.push_back(T.inner_area());
+            const bool too_deep = tree_depth(b->nodes) > std::max(56, built_depth);
+            if (too_deep || total.back() > total[total.size() - 2]) { b->nodes = before_nodes; T.parent = before_parent; total.back() = total[total.size() - 2]; }
+            if (too_deep) break;
+        }
+        return tree_depth(b->nodes);
+    }
+    return built_depth;
+}
+
 // Builds the host tree.  Returns false on failure.
 bool crt_bvh_build_host(crt_bvh* b, const float* verts, int64_t n, const crt_bvh_params& pr)
 {
@@ -382,45 +426,7 @@ bool crt_bvh_build_host(crt_bvh* b, const float* verts, int64_t n, const crt_bvh
         }
         b->nodes.resize((size_t)B.n_nodes.load());
         for (int64_t i = 0; i < nr; ++i) b->prim[i] = refs[b->prim[i]].prim;
-        // tree rotations (Kensler 2008, restated): bottom-up (a child's index is always larger than its parent's), a node may exchange one of its children
-        // with a grandchild on the other side when that shrinks the box of the child that is rebuilt; leaf ranges are untouched
-        if (pr.optimize > 0 && b->nodes.size() >= 16) {
-            // insertion-based optimisation (TreeOpt above): per iteration the worst-looking 2 % of the inner nodes (at most 20,000), ranked by area x
-            // (area / smaller child) x (area / mean child); four consecutive windows of that ranking take turns, so that nodes which are already placed
-            // as well as the search can place them are not picked over and over
-            TreeOpt T(b->nodes);
-            std::vector<std::pair<double, int32_t>> rank;
-            const auto worse = [](const std::pair<double, int32_t>& a, const std::pair<double, int32_t>& c) { return a.first > c.first || (a.first == c.first && a.second < c.second); };
-            std::vector<double> total{T.inner_area()};        // summed inner-node area after each iteration
-            for (int it = 0; it < pr.optimize; ++it) {
-                // no progress worth the time (a terrain grid, say, is as good as it gets after the build): less than 0.2 % over the last four iterations
-                if (it >= 4 && total[it - 4] - total[it] < 0.002 * total[it]) break;
-                if (it == 1 && total[0] - total[1] < 0.0005 * total[1]) break;      // the most promising 2 % gained next to nothing
-                rank.clear();
-                for (size_t i = 1; i < b->nodes.size(); ++i) {
-                    const BuildNode& x = b->nodes[i];
-                    if (x.left < 0 || T.parent[i] <= 0) continue;
-                    const double a = TreeOpt::area(x), al = TreeOpt::area(b->nodes[x.left]), ar = TreeOpt::area(b->nodes[x.right]);
-                    const double mn = std::max(std::min(al, ar), 1e-300), sum = std::max(al + ar, 1e-300);
-                    rank.emplace_back(a * (a / mn) * (2.0 * a / sum), (int32_t)i);
-                }
-                if (rank.empty()) break;
-                const size_t batch = std::min<size_t>(rank.size(), std::max<size_t>(64, std::min<size_t>(rank.size() / 50, 20000)));
-                const size_t off = std::min(rank.size() - batch, (size_t)(it % 4) * batch);
-                std::nth_element(rank.begin(), rank.begin() + off, rank.end(), worse);
-                std::nth_element(rank.begin() + off, rank.begin() + off + batch - 1, rank.end(), worse);
-                std::sort(rank.begin() + off, rank.begin() + off + batch, worse);      // a fixed processing order for a given tree
-                // (putting two children back one after the other is not guaranteed to pay: an iteration that loses is undone; so is one that makes the tree
-                // deeper than the traversal stack allows -- many identical boxes can be chained into a list -- and the optimisation ends there)
-                const std::vector<BuildNode> before_nodes = b->nodes; const std::vector<int32_t> before_parent = T.parent;
-                for (size_t k = off; k < off + batch; ++k) T.reinsert_children(rank[k].second);
-                total.push_back(T.inner_area());
-                const bool too_deep = tree_depth(b->nodes) > std::max(56, B.max_depth.load());
-                if (too_deep || total.back() > total[total.size() - 2]) { b->nodes = before_nodes; T.parent = before_parent; total.back() = total[total.size() - 2]; }
-                if (too_deep) break;
-            }
-            b->depth = tree_depth(b->nodes);
-        } else b->depth = B.max_depth.load();
+        b->depth = crt_bvh_optimize_tree(b, pr, B.max_depth.load());
         // SAH cost (relative to the root area) before padding
         double ra = root.half_area(), cost = 0;
         for (const BuildNode& nd : b->nodes) {

@@ -506,6 +506,14 @@ crt_status crt_bvh_build_device(crt_ctx* ctx, crt_bvh* b, const float* verts, in
     }
     b->depth = max_depth;
     const double ra = half_area(box[root]);
+    if (pr.optimize > 0) {          // the host builder's insertion-based optimisation on the clustering tree (same leaves); cost recounted on the result
+        b->depth = crt_bvh_optimize_tree(b, pr, max_depth);
+        cost = 0;
+        for (const BuildNode& x : b->nodes) {
+            const double dx = (double)x.bmax[0] - x.bmin[0], dy = (double)x.bmax[1] - x.bmin[1], dz = (double)x.bmax[2] - x.bmin[2];
+            cost += (dx * dy + dy * dz + dz * dx) * (x.left >= 0 ? (double)pr.cost_traversal : (double)pr.cost_intersect * x.count);
+        }
+    }
     b->sah = ra > 0 ? cost / ra : 0;
     for (BuildNode& nd : b->nodes)
         for (int k = 0; k < 3; ++k) { nd.bmin[k] -= pad; nd.bmax[k] += pad; }

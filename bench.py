@@ -613,11 +613,11 @@ def run_builders(args):
     scene = I.by_name(name, **kw).with_camera(w, h)
     ctx = crt.Context(0)
     trees = []
-    for label, bkw in [("host SAH (64 bins)", dict(builder=0))] + [(f"device PLOC radius {r}", dict(builder=1, ploc_radius=r)) for r in args.ploc_radii] + [(f"device clustering radius {args.ploc_radii[0]} + host optimisation and layout", dict(builder=2, ploc_radius=args.ploc_radii[0]))]:
+    for label, bkw in [("host SAH + pre-split, re-insertion on the device (default)", dict(builder=0)), ("host SAH + pre-split, re-insertion on the host (builder 3)", dict(builder=3)), ("host SAH + pre-split, no optimisation", dict(builder=0, optimize=0))] + [(f"device PLOC radius {r}", dict(builder=1, ploc_radius=r, optimize=0)) for r in args.ploc_radii] + [(f"device PLOC radius {args.ploc_radii[0]} + device re-insertion", dict(builder=1, ploc_radius=args.ploc_radii[0]))] + [(f"device clustering radius {args.ploc_radii[0]} + host optimisation and layout", dict(builder=2, ploc_radius=args.ploc_radii[0]))]:
         t0 = time.time(); bvh = ctx.crt_build_bvh(scene.verts, scene.mat_id, **bkw); wall = time.time() - t0
         info = bvh.info()
         trees.append((label, bvh, dict(builder=label, wall_seconds=wall, hierarchy_seconds=info["build_seconds"], device_build_seconds=info["device_build_seconds"],
-                                       layout_seconds=info["layout_seconds"], rounds=info["build_rounds"], depth=info["depth"], sah_cost=info["sah_cost"],
+                                       layout_seconds=info["layout_seconds"], rounds=info["build_rounds"], optimize_iterations=info["optimize_iterations"], depth=info["depth"], sah_cost=info["sah_cost"],
                                        n_nodes=info["n_nodes"], q16_inflation_pct=info["q16_inflation_pct"], check=bvh.check())))
     _, _keep, sets = _frame_ray_sets(ctx, crt, scene, w, h, spp, nb, gw, gh, s, seed, 7, bvh=trees[0][1])
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=ctx.device)
@@ -640,9 +640,9 @@ def run_builders(args):
     print(json.dumps({"clocks": _SWEEP_CLOCKS.stop() if _SWEEP_CLOCKS else None, "builders": rows, "config": {"workload": args.workload, "n_tris": int(scene.n_tris), "frame": 7,
                                                    "timing": "crt_trace alone, CUDA events, median of 8, 256 MB L2 flush between repetitions"}}))
     tags = [t for t, _ in sets]
-    sys.stderr.write("| builder | hierarchy s | of which on device s | layout s | rounds | depth | SAH cost | check | " + " | ".join(tags) + " |\n|---|" + "---:|" * (7 + len(tags)) + "\n")
+    sys.stderr.write("| builder | hierarchy s | of which on device s | layout s | rounds | opt iterations | depth | SAH cost | check | " + " | ".join(tags) + " |\n|---|" + "---:|" * (8 + len(tags)) + "\n")
     for row in rows:
-        sys.stderr.write(f"| {row['builder']} | {row['hierarchy_seconds']:.3f} | {row['device_build_seconds']:.4f} | {row['layout_seconds']:.3f} | {row['rounds']} | {row['depth']} | {row['sah_cost']:.1f} | {row['check']} | "
+        sys.stderr.write(f"| {row['builder']} | {row['hierarchy_seconds']:.3f} | {row['device_build_seconds']:.4f} | {row['layout_seconds']:.3f} | {row['rounds']} | {row['optimize_iterations']} | {row['depth']} | {row['sah_cost']:.1f} | {row['check']} | "
                          + " | ".join(f"{row['sets'][t]['ms']:.3f}{'' if row['sets'][t]['records_identical'] else ' !'}" for t in tags) + " |\n")
 
 

@@ -87,7 +87,8 @@ typedef struct { int32_t mode, group_w, group_h, stride, stride_y, partition_rul
 /* materials: [device] table indexed by the per-triangle material id given to crt_build_bvh.
  * env: radiance on a miss = lerp(env[0..2], env[3..5], 0.5*(d.y+1)) (D:R14). */
 typedef struct { const crt_material* materials; int32_t n_materials; float env[6]; } crt_scene_mats;
-/* builder: 0 = host (binned surface-area heuristic, threaded); 1 = device (parallel locally-ordered clustering AND the traversal layouts
+/* builder: 0 = host (binned surface-area heuristic, threaded; with a context its optimisation step runs on the device, see `optimize`); 3 = host entirely
+ * (what 0 does without a context); 1 = device (parallel locally-ordered clustering AND the traversal layouts
  * written by the GPU, csrc/bvh_ploc.cu; needs a context); 2 = the device's clustering with the host's tree optimisation (`optimize`) and layout code
  * (cross-check of 1; profiles/r02n);
  * ploc_radius: neighbours searched on either side of a cluster in Morton order (0 = 8; at most 128).
@@ -99,7 +100,9 @@ typedef struct { const crt_material* materials; int32_t n_materials; float env[6
  * optimize (host builder): iterations of insertion-based optimisation of the built tree (Bittner et al. 2013): each takes the 2 % worst-looking inner
  * nodes (at most 20,000), detaches their children and puts each back where it adds the least surface area.  Same leaves, same hits; interior scene: SAH
  * cost -8 %, traversal -2 to -4 % for +0.8 s of build time (profiles/r02k); stops early when four iterations gain less than 0.2 % (a terrain grid).
- * 0 = off; NULL params = 20. */
+ * 0 = off; NULL params = 20.  With a context, builders 0 and 1 run (at most) that many iterations of PARALLEL re-insertion on the device instead (bvh_ploc.cu:
+ * every node searches its best position in every iteration, conflicting moves are resolved by locks; stronger and two orders of magnitude faster than the
+ * host's version: profiles/r02o); builders 2 and 3 and host-only builds run the host's. */
 typedef struct { int32_t max_leaf; int32_t sah_bins; float cost_traversal, cost_intersect; int32_t n_threads; int32_t builder; int32_t ploc_radius; float presplit; int32_t optimize; } crt_bvh_params;
 typedef struct {
     int64_t n_tris, n_nodes, device_bytes;
@@ -110,13 +113,15 @@ typedef struct {
     int32_t wide_depth;
     int32_t q16_inflation_pct;  /* summed surface area of the boxes the 16-bit nodes decode to, in percent of the fp32 boxes' (100 = no
                                  * loss); above 200 the default kernel reads the fp32 nodes instead (grid too coarse for the scene) */
-    int32_t builder;            /* 0 host SAH, 1 device PLOC, 2 device PLOC + host layout */
+    int32_t builder;            /* 0 host SAH, 1 device PLOC, 2 device PLOC + host optimisation and layout, 3 host SAH with the host's own optimisation */
     int32_t build_rounds;       /* device builder: clustering rounds */
     double device_build_seconds;/* device builder: boxes + Morton sort + clustering on the GPU (CUDA events); build_seconds is the whole
                                  * hierarchy build including the copy back and the leaf collapse; layout_seconds the flattening, 16-bit
                                  * quantisation and upload of the traversal layouts (either builder) */
     double layout_seconds;
     int64_t n_refs;             /* triangle references = records of the device triangle array (n_tris unless large triangles were pre-split) */
+    int32_t optimize_iterations;/* iterations of tree optimisation that ran and were kept (crt_bvh_params.optimize is the upper limit) */
+    int32_t reserved;
 } crt_bvh_info_t;
 
 /* ---- context ------------------------------------------------------------------------------------ */

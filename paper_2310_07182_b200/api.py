@@ -71,7 +71,7 @@ class BvhInfo(C.Structure):
                 ("sah_cost", C.c_double), ("depth", C.c_int32), ("max_leaf", C.c_int32), ("build_seconds", C.c_double),
                 ("n_wide_nodes", C.c_int64), ("wide_depth", C.c_int32), ("q16_inflation_pct", C.c_int32),
                 ("builder", C.c_int32), ("build_rounds", C.c_int32), ("device_build_seconds", C.c_double), ("layout_seconds", C.c_double),
-                ("n_refs", C.c_int64)]
+                ("n_refs", C.c_int64), ("optimize_iterations", C.c_int32), ("reserved", C.c_int32)]
 
 
 _lib = None
@@ -159,7 +159,7 @@ class Bvh:
         return {"n_tris": o.n_tris, "n_nodes": o.n_nodes, "device_bytes": o.device_bytes, "bounds": np.array(list(o.bounds), np.float32),
                 "sah_cost": o.sah_cost, "depth": o.depth, "max_leaf": o.max_leaf, "build_seconds": o.build_seconds,
                 "n_wide_nodes": o.n_wide_nodes, "wide_depth": o.wide_depth, "q16_inflation_pct": o.q16_inflation_pct,
-                "builder": o.builder, "build_rounds": o.build_rounds, "device_build_seconds": o.device_build_seconds, "layout_seconds": o.layout_seconds, "n_refs": o.n_refs}
+                "builder": o.builder, "build_rounds": o.build_rounds, "device_build_seconds": o.device_build_seconds, "layout_seconds": o.layout_seconds, "n_refs": o.n_refs, "optimize_iterations": o.optimize_iterations}
 
     def check(self):
         v = C.c_int32(-1)

@@ -324,6 +324,7 @@ struct TreeOpt {
 // afterwards (built_depth when nothing was done).  Used by the host builder and by builder 2 (device clustering + host layout).
 int crt_bvh_optimize_tree(crt_bvh* b, const crt_bvh_params& pr, int built_depth)
 {
+    b->opt_iters = 0;
     if (pr.optimize > 0 && b->nodes.size() >= 16) {
         // insertion-based optimisation (TreeOpt above): per iteration the worst-looking 2 % of the inner nodes (at most 20,000), ranked by area x
         // (area / smaller child) x (area / mean child); four consecutive windows of that ranking take turns, so that nodes which are already placed
@@ -358,6 +359,7 @@ int crt_bvh_optimize_tree(crt_bvh* b, const crt_bvh_params& pr, int built_depth)
             const bool too_deep = tree_depth(b->nodes) > std::max(56, built_depth);
             if (too_deep || total.back() > total[total.size() - 2]) { b->nodes = before_nodes; T.parent = before_parent; total.back() = total[total.size() - 2]; }
             if (too_deep) break;
+            if (total.back() < total[total.size() - 2]) ++b->opt_iters;
         }
         return tree_depth(b->nodes);
     }

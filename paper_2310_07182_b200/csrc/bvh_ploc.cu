@@ -338,6 +338,165 @@ __global__ void __launch_bounds__(PB) layout_nodes_kernel(Tree T, int n_nodes, i
     if ((threadIdx.x & 31) == 0 && area_f != 0.0) { atomicAdd(sums + 0, cost); atomicAdd(sums + 1, area_f); atomicAdd(sums + 2, area_q); }
 }
 
+// ---- 2d. parallel re-insertion on the device (crt_bvh_params.optimize iterations; Meister & Bittner 2018, "Parallel reinsertion for bounding
+// volume hierarchy optimization", restated).  Per iteration, on the binary clustering tree (before leaves are collapsed):
+//   search : every node x (not the root, not a child of the root) looks for the node y beside which its subtree would add the least surface area:
+//            removing x deletes its parent p (the sibling s takes p's place) and shrinks the ancestors; the search walks the ancestors a_k of x
+//            ("pivots") upwards and descends, with a bound on the best gain so far, into the child of each pivot that does not contain x
+//   lock   : a move touches x, p, s, the grandparent g, y and y's parent: each candidate writes (gain, x) into those six nodes with atomicMax
+//   win    : x wins if it owns all six; a winner whose target y lies inside the subtree of ANOTHER winner steps back (two such moves could
+//            hang each subtree under the other one: a cycle)
+//   apply  : g adopts s; p becomes the parent of (y, x) in y's old place
+//   refit  : boxes, triangle counts, first positions and heights bottom-up from the leaves (atomic arrival counters)
+// A losing iteration cannot be told apart cheaply, so the summed inner area is reduced after each one and the loop stops when it no longer falls.
+__device__ __forceinline__ float box_area(const Box2& a)
+{
+    const float dx = a.hi.x - a.lo.x, dy = a.hi.y - a.lo.y, dz = a.hi.z - a.lo.z;
+    return dx * dy + dy * dz + dz * dx;
+}
+__device__ __forceinline__ Box2 box_union(const Box2& a, const Box2& b)
+{
+    Box2 u;
+    u.lo = make_float4(fminf(a.lo.x, b.lo.x), fminf(a.lo.y, b.lo.y), fminf(a.lo.z, b.lo.z), 0.f);
+    u.hi = make_float4(fmaxf(a.hi.x, b.hi.x), fmaxf(a.hi.y, b.hi.y), fmaxf(a.hi.z, b.hi.z), 0.f);
+    return u;
+}
+
+constexpr int REINS_STACK = 72;          // per-thread search stack (the tree's height is checked against 60 after every iteration)
+constexpr int REINS_MAX_VISITS = 768;    // nodes one search may look at
+
+__global__ void __launch_bounds__(128) reins_search_kernel(Tree T, int n_nodes, int32_t* __restrict__ target, float* __restrict__ gain_out)
+{
+    const int x = blockIdx.x * blockDim.x + threadIdx.x;
+    if (x >= n_nodes) return;
+    target[x] = -1; gain_out[x] = 0.f;
+    const int root = n_nodes - 1;
+    const int p = T.parent[x];
+    if (x == root || p < 0 || p == root) return;
+    const Box2 bx = T.box[x];
+    const float ax = box_area(bx);
+    const int s = T.left[p] == x ? T.right[p] : T.left[p];
+    int st_node[REINS_STACK]; float st_ind[REINS_STACK];
+    float best = 0.f; int best_y = -1;
+    float d_rem = box_area(T.box[p]);         // removal gain so far: p disappears; ancestors below the pivot shrink
+    Box2 shrunk = T.box[s];                    // box of the path node below the pivot once x is gone
+    int below = x, pivot = p, visits = 0;
+    while (pivot >= 0 && visits < REINS_MAX_VISITS) {
+        const int other = T.left[pivot] == below ? T.right[pivot] : T.left[pivot];
+        int sp = 0;
+        st_node[sp] = other; st_ind[sp] = 0.f; ++sp;
+        while (sp > 0 && visits < REINS_MAX_VISITS) {
+            --sp; const int y = st_node[sp]; const float ind = st_ind[sp];
+            ++visits;
+            const Box2 by = T.box[y];
+            const float c = box_area(box_union(by, bx));
+            const float g = d_rem - ind - c;
+            if (g > best && y != s) { best = g; best_y = y; }
+            const int l = T.left[y];
+            if (l >= 0 && sp + 2 <= REINS_STACK) {
+                const float ind_c = ind + (c - box_area(by));          // y itself grows by x when x goes below it
+                if (d_rem - ind_c - ax > best) { st_node[sp] = T.right[y]; st_ind[sp] = ind_c; ++sp; st_node[sp] = l; st_ind[sp] = ind_c; ++sp; }
+            }
+        }
+        // the pivot moves up: the old pivot (unless it is p, which is gone) keeps the shrunk box
+        const int up = T.parent[pivot];
+        if (up < 0) break;
+        if (pivot != p) {
+            shrunk = box_union(shrunk, T.box[other]);
+            d_rem += box_area(T.box[pivot]) - box_area(shrunk);
+        }
+        below = pivot; pivot = up;
+    }
+    // a move must pay for the staleness of its estimate (other moves of the same iteration change the boxes it was computed on)
+    if (best_y >= 0 && best > 1e-6f * ax) { target[x] = best_y; gain_out[x] = best; }
+}
+
+__device__ __forceinline__ unsigned long long reins_key(float gain, int x) { return ((unsigned long long)__float_as_uint(gain) << 32) | (unsigned)x; }
+
+__global__ void __launch_bounds__(PB) reins_lock_kernel(Tree T, int n_nodes, const int32_t* __restrict__ target, const float* __restrict__ gain, unsigned long long* __restrict__ lock)
+{
+    const int x = blockIdx.x * PB + threadIdx.x;
+    if (x >= n_nodes) return;
+    const int y = target[x];
+    if (y < 0) return;
+    const int p = T.parent[x], s = T.left[p] == x ? T.right[p] : T.left[p], g = T.parent[p], yp = T.parent[y];
+    const unsigned long long k = reins_key(gain[x], x);
+    atomicMax(lock + x, k); atomicMax(lock + p, k); atomicMax(lock + s, k); atomicMax(lock + g, k); atomicMax(lock + y, k); atomicMax(lock + yp, k);
+}
+
+__global__ void __launch_bounds__(PB) reins_win_kernel(Tree T, int n_nodes, const int32_t* __restrict__ target, const float* __restrict__ gain, const unsigned long long* __restrict__ lock,
+                                                       int32_t* __restrict__ win)
+{
+    const int x = blockIdx.x * PB + threadIdx.x;
+    if (x >= n_nodes) return;
+    const int y = target[x];
+    int w = 0;
+    if (y >= 0) {
+        const int p = T.parent[x], s = T.left[p] == x ? T.right[p] : T.left[p], g = T.parent[p], yp = T.parent[y];
+        const unsigned long long k = reins_key(gain[x], x);
+        w = lock[x] == k && lock[p] == k && lock[s] == k && lock[g] == k && lock[y] == k && lock[yp] == k;
+    }
+    win[x] = w;
+}
+
+// a winner goes ahead unless an ancestor of its target is itself a winner (that subtree is about to move): decided for all winners BEFORE any pointer changes
+__global__ void __launch_bounds__(PB) reins_filter_kernel(Tree T, int n_nodes, const int32_t* __restrict__ target, const int32_t* __restrict__ win, int32_t* __restrict__ go)
+{
+    const int x = blockIdx.x * PB + threadIdx.x;
+    if (x >= n_nodes) return;
+    int ok = win[x];
+    if (ok) for (int a = T.parent[target[x]]; a >= 0; a = T.parent[a]) if (win[a]) { ok = 0; break; }
+    go[x] = ok;
+}
+
+// the moves: every node a thread writes is one of the six it owns, so the writes of different threads never meet
+__global__ void __launch_bounds__(PB) reins_apply_kernel(Tree T, int n_nodes, const int32_t* __restrict__ target, const int32_t* __restrict__ go, int32_t* __restrict__ n_applied)
+{
+    const int x = blockIdx.x * PB + threadIdx.x;
+    if (x >= n_nodes || !go[x]) return;
+    const int y = target[x];
+    const int p = T.parent[x], s = T.left[p] == x ? T.right[p] : T.left[p], g = T.parent[p];
+    if (T.left[g] == p) T.left[g] = s; else T.right[g] = s;          // g adopts s
+    T.parent[s] = g;
+    const int yp = T.parent[y];                                        // (may be g, or s)
+    if (T.left[yp] == y) T.left[yp] = p; else T.right[yp] = p;         // p takes y's place ...
+    T.parent[p] = yp;
+    T.left[p] = y; T.right[p] = x; T.parent[y] = p;                   // ... as the parent of y and x
+    atomicAdd(n_applied, 1);
+}
+
+// boxes, counts, first positions and heights of all inner nodes, bottom-up: the second thread to arrive at a node computes it and goes on
+__global__ void __launch_bounds__(PB) reins_refit_kernel(Tree T, int n, int32_t* __restrict__ arrive)
+{
+    const int k = blockIdx.x * PB + threadIdx.x;
+    if (k >= n) return;
+    int i = k;
+    for (;;) {
+        const int p = T.parent[i];
+        if (p < 0) break;
+        __threadfence();
+        if (atomicAdd(arrive + p, 1) == 0) break;
+        const int l = T.left[p], r = T.right[p];
+        Box2 a, b;
+        a.lo = __ldcg(&T.box[l].lo); a.hi = __ldcg(&T.box[l].hi); b.lo = __ldcg(&T.box[r].lo); b.hi = __ldcg(&T.box[r].hi);
+        T.box[p] = box_union(a, b);
+        T.cnt[p] = __ldcg(T.cnt + l) + __ldcg(T.cnt + r);
+        T.first[p] = min(__ldcg(T.first + l), __ldcg(T.first + r));
+        T.height[p] = 1 + max(__ldcg(T.height + l), __ldcg(T.height + r));
+        i = p;
+    }
+}
+
+// summed surface area of the inner nodes (what the re-insertion lowers)
+__global__ void __launch_bounds__(PB) reins_area_kernel(Tree T, int n, int n_nodes, double* __restrict__ total)
+{
+    const int i = n + blockIdx.x * PB + threadIdx.x;
+    double a = i < n_nodes ? (double)box_area(T.box[i]) : 0.0;
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) a += __shfl_xor_sync(0xffffffffu, a, d);
+    if ((threadIdx.x & 31) == 0 && a != 0.0) atomicAdd(total, a);
+}
+
 struct DevBuf {
     void* p = nullptr;
     ~DevBuf() { if (p) cudaFree(p); }
@@ -349,6 +508,68 @@ struct DevBuf {
 }  // namespace
 
 #define PLOC_CUDA(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return crt_fail(ctx, e_ == cudaErrorMemoryAllocation ? CRT_ERR_NOMEM : CRT_ERR_CUDA, "build_bvh(device): %s: %s", #call, cudaGetErrorString(e_)); } while (0)
+
+// The re-insertion iterations on a device tree of n_leaves leaves (nodes [0, n_leaves)) and n_leaves - 1 inner nodes, the root last; boxes, counts, first
+// positions and heights of the inner nodes are (re)computed by the refit.  *kept = iterations that lowered the summed inner area and were kept.
+struct ReinsBufs {
+    DevBuf d_target, d_gain, d_lock, d_win, d_go, d_arrive, d_bk[3], d_acc;
+    cudaError_t alloc(int n_nodes)
+    {
+        cudaError_t e = cudaSuccess;
+        for (DevBuf* d : {&d_target, &d_gain, &d_win, &d_go, &d_arrive, &d_bk[0], &d_bk[1], &d_bk[2]}) if (e == cudaSuccess) e = d->alloc((size_t)n_nodes * 4);
+        if (e == cudaSuccess) e = d_lock.alloc((size_t)n_nodes * 8);
+        if (e == cudaSuccess) e = d_acc.alloc(64);
+        return e;
+    }
+};
+
+static crt_status reinsertion_loop(crt_ctx* ctx, Tree T, int n_leaves, int n_nodes, int iterations, int* kept, ReinsBufs& R)
+{
+    *kept = 0;
+    DevBuf &d_target = R.d_target, &d_gain = R.d_gain, &d_lock = R.d_lock, &d_win = R.d_win, &d_go = R.d_go, &d_arrive = R.d_arrive, &d_acc = R.d_acc;
+    DevBuf* const d_bk = R.d_bk;
+    const unsigned gnodes = (unsigned)((n_nodes + PB - 1) / PB), ginner = (unsigned)((n_nodes - n_leaves + PB - 1) / PB), gleaves = (unsigned)((n_leaves + PB - 1) / PB);
+    int32_t* const topo[3] = {T.left, T.right, T.parent};
+    struct Acc { double area; int32_t applied, pad; } acc;
+    auto measure = [&](Acc* out) -> cudaError_t {
+        cudaError_t e = cudaMemsetAsync(d_acc.p, 0, 64, 0); if (e != cudaSuccess) return e;
+        reins_area_kernel<<<ginner, PB>>>(T, n_leaves, n_nodes, d_acc.as<double>());
+        return cudaMemcpy(out, d_acc.p, sizeof(Acc), cudaMemcpyDeviceToHost);
+    };
+    auto refit = [&]() -> cudaError_t {
+        cudaError_t e = cudaMemsetAsync(d_arrive.p, 0, (size_t)n_nodes * 4, 0); if (e != cudaSuccess) return e;
+        reins_refit_kernel<<<gleaves, PB>>>(T, n_leaves, d_arrive.as<int32_t>());
+        return cudaGetLastError();
+    };
+    PLOC_CUDA(measure(&acc));
+    double prev_area = acc.area;
+    for (int it = 0; it < iterations; ++it) {
+        for (int k = 0; k < 3; ++k) PLOC_CUDA(cudaMemcpyAsync(d_bk[k].p, topo[k], (size_t)n_nodes * 4, cudaMemcpyDeviceToDevice, 0));
+        reins_search_kernel<<<(unsigned)((n_nodes + 127) / 128), 128>>>(T, n_nodes, d_target.as<int32_t>(), d_gain.as<float>());
+        PLOC_CUDA(cudaMemsetAsync(d_lock.p, 0, (size_t)n_nodes * 8, 0));
+        reins_lock_kernel<<<gnodes, PB>>>(T, n_nodes, d_target.as<int32_t>(), d_gain.as<float>(), d_lock.as<unsigned long long>());
+        reins_win_kernel<<<gnodes, PB>>>(T, n_nodes, d_target.as<int32_t>(), d_gain.as<float>(), d_lock.as<unsigned long long>(), d_win.as<int32_t>());
+        reins_filter_kernel<<<gnodes, PB>>>(T, n_nodes, d_target.as<int32_t>(), d_win.as<int32_t>(), d_go.as<int32_t>());
+        PLOC_CUDA(cudaMemsetAsync(d_acc.p, 0, 64, 0));
+        reins_apply_kernel<<<gnodes, PB>>>(T, n_nodes, d_target.as<int32_t>(), d_go.as<int32_t>(), d_acc.as<int32_t>() + 2);
+        int32_t applied = 0;
+        PLOC_CUDA(cudaMemcpy(&applied, d_acc.as<int32_t>() + 2, 4, cudaMemcpyDeviceToHost));
+        PLOC_CUDA(refit());
+        PLOC_CUDA(measure(&acc));
+        int32_t h = 0;
+        PLOC_CUDA(cudaMemcpy(&h, T.height + (n_nodes - 1), 4, cudaMemcpyDeviceToHost));
+        if (h > 56 || !(acc.area < prev_area)) {          // too deep for the traversal stack, or no gain: this iteration is undone
+            for (int k = 0; k < 3; ++k) PLOC_CUDA(cudaMemcpyAsync(topo[k], d_bk[k].p, (size_t)n_nodes * 4, cudaMemcpyDeviceToDevice, 0));
+            PLOC_CUDA(refit());
+            break;
+        }
+        ++*kept;
+        const bool small = prev_area - acc.area < 0.002 * prev_area;
+        prev_area = acc.area;
+        if (applied == 0 || small) break;
+    }
+    return CRT_OK;
+}
 
 // Builds the BVH of verts (HOST array; uploaded here) on the device `ctx` lives on.
 //  full_device (builder 1): fills b->d_nodes, d_qnodes, d_tris, d_slot_of_prim, qgrid, q_violations, q_inflation, n_gpu_nodes, n_tree_nodes,
@@ -378,6 +599,8 @@ crt_status crt_bvh_build_device(crt_ctx* ctx, crt_bvh* b, const float* verts, in
     PLOC_CUDA(d_total.alloc(256)); PLOC_CUDA(d_bsum.alloc((size_t)(nb_max + 1) * 4));
     Tree T{d_box.as<Box2>(), d_left.as<int32_t>(), d_right.as<int32_t>(), d_cnt.as<int32_t>(), d_parent.as<int32_t>(), d_first.as<int32_t>(), d_height.as<int32_t>()};
     PLOC_CUDA(cudaMemcpy(d_verts.p, verts, (size_t)n * 36, cudaMemcpyHostToDevice));
+    ReinsBufs reins;
+    if (full_device && pr.optimize > 0 && n >= 8) PLOC_CUDA(reins.alloc(n_nodes));
     cudaEvent_t e0, e1;
     PLOC_CUDA(cudaEventCreate(&e0)); PLOC_CUDA(cudaEventCreate(&e1));
     PLOC_CUDA(cudaEventRecord(e0, 0));
@@ -407,6 +630,12 @@ crt_status crt_bvh_build_device(crt_ctx* ctx, crt_bvh* b, const float* verts, in
     if (node_base != n_nodes) return crt_fail(ctx, CRT_ERR_CUDA, "build_bvh(device): inconsistent tree (%d nodes for %lld triangles)", node_base, (long long)n);
     const int root = n_nodes - 1;
     b->ploc_rounds = rounds;
+    // 2d. parallel re-insertion (builder 1; builder 2 runs the host's optimisation on the tree it copies back)
+    b->opt_iters = 0;
+    if (full_device && pr.optimize > 0 && n >= 8) {
+        const crt_status rst = reinsertion_loop(ctx, T, (int)n, n_nodes, pr.optimize, &b->opt_iters, reins);
+        if (rst != CRT_OK) return rst;
+    }
     unsigned ob[6]; int32_t height = 0;
     PLOC_CUDA(cudaMemcpy(ob, d_bounds.p, sizeof ob, cudaMemcpyDeviceToHost));
     PLOC_CUDA(cudaMemcpy(&height, d_height.as<int32_t>() + root, 4, cudaMemcpyDeviceToHost));
@@ -518,5 +747,70 @@ crt_status crt_bvh_build_device(crt_ctx* ctx, crt_bvh* b, const float* verts, in
     for (BuildNode& nd : b->nodes)
         for (int k = 0; k < 3; ++k) { nd.bmin[k] -= pad; nd.bmax[k] += pad; }
     b->build_seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count();
+    return CRT_OK;
+}
+
+// The same parallel re-insertion for a HOST-built tree (crt_build_bvh, builder 0 with a context): b->nodes goes to the device in the index convention
+// of this file (leaves first, the root last; a leaf of several triangles is one atomic node), is optimised, and comes back as b->nodes with the root
+// at 0 and siblings adjacent; leaves keep their triangle ranges.  Boxes may be padded or not (a union of padded boxes is the padded union).
+// Returns the iterations kept in b->opt_iters and the new depth in b->depth.
+crt_status crt_bvh_reinsert_device(crt_ctx* ctx, crt_bvh* b, int iterations)
+{
+    b->opt_iters = 0;
+    const int n_nodes = (int)b->nodes.size();
+    if (iterations <= 0 || n_nodes < 15 || (n_nodes & 1) == 0) return CRT_OK;
+    const int n_leaves = (n_nodes + 1) / 2;
+    // new indices: leaves 0 .. n_leaves - 1 in order of appearance, inner nodes in REVERSE order of appearance after them (the root, node 0, becomes the last)
+    std::vector<int32_t> idx((size_t)n_nodes);
+    { int l = 0, in = 0; for (int i = 0; i < n_nodes; ++i) idx[i] = b->nodes[i].left < 0 ? l++ : n_nodes - 1 - in++; if (l != n_leaves) return crt_fail(ctx, CRT_ERR_STATE, "build_bvh: tree is not a full binary tree"); }
+    std::vector<Box2> box((size_t)n_nodes); std::vector<int32_t> left((size_t)n_nodes, -1), right((size_t)n_nodes, -1), parent((size_t)n_nodes, -1), cnt((size_t)n_nodes, 0), first((size_t)n_nodes, 0), height((size_t)n_nodes, 1);
+    std::vector<int32_t> leaf_of((size_t)n_leaves);          // device leaf -> host node (for the triangle range)
+    for (int i = 0; i < n_nodes; ++i) {
+        const BuildNode& nd = b->nodes[i]; const int k = idx[i];
+        box[k].lo = make_float4(nd.bmin[0], nd.bmin[1], nd.bmin[2], 0.f); box[k].hi = make_float4(nd.bmax[0], nd.bmax[1], nd.bmax[2], 0.f);
+        if (nd.left >= 0) { left[k] = idx[nd.left]; right[k] = idx[nd.right]; parent[idx[nd.left]] = k; parent[idx[nd.right]] = k; }
+        else { cnt[k] = nd.count; first[k] = k; leaf_of[k] = i; }
+    }
+    DevBuf d_box, d_left, d_right, d_cnt, d_parent, d_first, d_height, d_arrive;
+    PLOC_CUDA(d_box.alloc((size_t)n_nodes * sizeof(Box2)));
+    for (DevBuf* d : {&d_left, &d_right, &d_cnt, &d_parent, &d_first, &d_height, &d_arrive}) PLOC_CUDA(d->alloc((size_t)n_nodes * 4));
+    PLOC_CUDA(cudaMemcpy(d_box.p, box.data(), (size_t)n_nodes * sizeof(Box2), cudaMemcpyHostToDevice));
+    PLOC_CUDA(cudaMemcpy(d_left.p, left.data(), (size_t)n_nodes * 4, cudaMemcpyHostToDevice)); PLOC_CUDA(cudaMemcpy(d_right.p, right.data(), (size_t)n_nodes * 4, cudaMemcpyHostToDevice));
+    PLOC_CUDA(cudaMemcpy(d_parent.p, parent.data(), (size_t)n_nodes * 4, cudaMemcpyHostToDevice)); PLOC_CUDA(cudaMemcpy(d_cnt.p, cnt.data(), (size_t)n_nodes * 4, cudaMemcpyHostToDevice));
+    PLOC_CUDA(cudaMemcpy(d_first.p, first.data(), (size_t)n_nodes * 4, cudaMemcpyHostToDevice)); PLOC_CUDA(cudaMemcpy(d_height.p, height.data(), (size_t)n_nodes * 4, cudaMemcpyHostToDevice));
+    Tree T{d_box.as<Box2>(), d_left.as<int32_t>(), d_right.as<int32_t>(), d_cnt.as<int32_t>(), d_parent.as<int32_t>(), d_first.as<int32_t>(), d_height.as<int32_t>()};
+    PLOC_CUDA(cudaMemset(d_arrive.p, 0, (size_t)n_nodes * 4));
+    reins_refit_kernel<<<(unsigned)((n_leaves + PB - 1) / PB), PB>>>(T, n_leaves, d_arrive.as<int32_t>());          // inner counts and heights in this file's form
+    ReinsBufs reins;
+    PLOC_CUDA(reins.alloc(n_nodes));
+    const crt_status st = reinsertion_loop(ctx, T, n_leaves, n_nodes, iterations, &b->opt_iters, reins);
+    if (st != CRT_OK) return st;
+    if (b->opt_iters == 0) return CRT_OK;          // nothing kept: the host tree stays as it is
+    PLOC_CUDA(cudaMemcpy(box.data(), d_box.p, (size_t)n_nodes * sizeof(Box2), cudaMemcpyDeviceToHost));
+    PLOC_CUDA(cudaMemcpy(left.data(), d_left.p, (size_t)n_nodes * 4, cudaMemcpyDeviceToHost)); PLOC_CUDA(cudaMemcpy(right.data(), d_right.p, (size_t)n_nodes * 4, cudaMemcpyDeviceToHost));
+    PLOC_CUDA(cudaMemcpy(height.data(), d_height.p, (size_t)n_nodes * 4, cudaMemcpyDeviceToHost));
+    // back to the host form: root at 0, the two children of a node adjacent, depth-first
+    std::vector<BuildNode> out((size_t)n_nodes);
+    struct Item { int32_t src, dst; };
+    std::vector<Item> stack{{n_nodes - 1, 0}};
+    int32_t next = 1; int64_t seen = 0;
+    while (!stack.empty()) {
+        const Item it = stack.back(); stack.pop_back(); ++seen;
+        BuildNode nd;
+        nd.bmin[0] = box[it.src].lo.x; nd.bmin[1] = box[it.src].lo.y; nd.bmin[2] = box[it.src].lo.z; nd.bmax[0] = box[it.src].hi.x; nd.bmax[1] = box[it.src].hi.y; nd.bmax[2] = box[it.src].hi.z;
+        if (left[it.src] >= 0) {
+            if (next + 2 > n_nodes) return crt_fail(ctx, CRT_ERR_STATE, "build_bvh: re-insertion left an inconsistent tree");
+            nd.left = next; nd.right = next + 1; nd.first = 0; nd.count = 0;
+            stack.push_back({right[it.src], next + 1}); stack.push_back({left[it.src], next});
+            next += 2;
+        } else {
+            const BuildNode& old = b->nodes[leaf_of[it.src]];
+            nd.left = nd.right = -1; nd.first = old.first; nd.count = old.count;
+        }
+        out[it.dst] = nd;
+    }
+    if (seen != n_nodes || next != n_nodes) return crt_fail(ctx, CRT_ERR_STATE, "build_bvh: re-insertion left an inconsistent tree (%lld of %d nodes reachable)", (long long)seen, n_nodes);
+    b->nodes.swap(out);
+    b->depth = height[n_nodes - 1];
     return CRT_OK;
 }

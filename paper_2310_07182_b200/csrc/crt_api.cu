@@ -168,15 +168,32 @@ crt_status crt_build_bvh(crt_ctx* ctx, const float* verts, const int32_t* mat_id
     for (int64_t i = 0; i < 9 * n_tris; ++i) if (!(v[i] == v[i]) || v[i] > 1e30f || v[i] < -1e30f) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "build_bvh: non-finite vertex");
     int32_t max_mat = -1;
     for (int32_t m : hm) { if (m < 0) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "build_bvh: negative material id"); max_mat = std::max(max_mat, m); }
-    if (pr.builder < 0 || pr.builder > 2) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "build_bvh: builder %d out of range", pr.builder);
-    if (pr.builder != 0 && !ctx) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "build_bvh: the device builder needs a context");
+    if (pr.builder < 0 || pr.builder > 3) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "build_bvh: builder %d out of range", pr.builder);
+    if ((pr.builder == 1 || pr.builder == 2) && !ctx) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "build_bvh: the device builder needs a context");
     if (n_tris <= pr.max_leaf) pr.builder = 0;            // nothing to cluster: the whole scene is one leaf (or empty)
     crt_bvh* b = new crt_bvh();
     b->max_mat_id = max_mat;
-    if (pr.builder != 0) {
+    if (pr.builder == 1 || pr.builder == 2) {
         crt_status bst = crt_bvh_build_device(ctx, b, v, n_tris, pr, pr.builder == 1);
         if (bst != CRT_OK) { crt_bvh_destroy(b); return bst; }
-    } else crt_bvh_build_host(b, v, n_tris, pr);
+    } else if (pr.builder == 0 && ctx && pr.optimize > 0) {
+        // host build; its optimisation step runs on the device (parallel re-insertion, bvh_ploc.cu: every node looks for its best place in every iteration,
+        // where the host's own version can afford the worst 2 % only)
+        const auto t_opt0 = std::chrono::steady_clock::now();
+        crt_bvh_params p0 = pr; p0.optimize = 0;
+        crt_bvh_build_host(b, v, n_tris, p0);
+        const crt_status rst = crt_bvh_reinsert_device(ctx, b, pr.optimize);
+        if (rst != CRT_OK) { crt_bvh_destroy(b); return rst; }
+        if (b->opt_iters > 0) {          // SAH cost of the new tree, on the unpadded boxes as crt_bvh_build_host reports it
+            float maxabs = 0.f; for (int k = 0; k < 6; ++k) maxabs = std::max(maxabs, std::fabs(b->bounds[k]));
+            const double pad2 = 2.0 * (double)(maxabs * (1.0f / 131072.0f));
+            auto ha = [&](const BuildNode& x) { const double dx = (double)x.bmax[0] - x.bmin[0] - pad2, dy = (double)x.bmax[1] - x.bmin[1] - pad2, dz = (double)x.bmax[2] - x.bmin[2] - pad2; return dx * dy + dy * dz + dz * dx; };
+            double cost = 0; for (const BuildNode& x : b->nodes) cost += ha(x) * (x.left >= 0 ? (double)pr.cost_traversal : (double)pr.cost_intersect * x.count);
+            const double ra = b->nodes.empty() ? 0 : ha(b->nodes[0]);
+            b->sah = ra > 0 ? cost / ra : 0;
+        }
+        b->build_seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t_opt0).count();
+    } else { crt_bvh_build_host(b, v, n_tris, pr); b->builder = pr.builder == 3 ? 3 : 0; }
     const auto t_layout0 = std::chrono::steady_clock::now();
     if (b->depth > 60) { crt_bvh_destroy(b); return crt_fail(ctx, CRT_ERR_UNSUPPORTED, "build_bvh: tree depth exceeds the traversal stack (64)"); }
     auto up = [&](void** d, const void* h, size_t bytes) -> cudaError_t {
@@ -230,7 +247,7 @@ crt_status crt_bvh_destroy(crt_bvh* b)
 crt_status crt_bvh_get_info(const crt_bvh* b, crt_bvh_info_t* o)
 {
     if (!b || !o) return crt_fail(nullptr, CRT_ERR_INVALID_ARG, "bvh_get_info: null argument");
-    o->n_refs = b->n_refs; o->n_tris = b->n_tris; o->n_nodes = b->nodes.empty() ? b->n_tree_nodes : (int64_t)b->nodes.size(); o->device_bytes = b->device_bytes;
+    o->optimize_iterations = b->opt_iters; o->reserved = 0; o->n_refs = b->n_refs; o->n_tris = b->n_tris; o->n_nodes = b->nodes.empty() ? b->n_tree_nodes : (int64_t)b->nodes.size(); o->device_bytes = b->device_bytes;
     memcpy(o->bounds, b->bounds, sizeof o->bounds);
     o->sah_cost = b->sah; o->depth = b->depth; o->max_leaf = b->max_leaf; o->build_seconds = b->build_seconds;
     o->n_wide_nodes = b->n_wide_nodes; o->wide_depth = b->wide_depth;

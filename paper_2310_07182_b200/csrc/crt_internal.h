@@ -78,6 +78,7 @@ struct crt_bvh {
     std::vector<float> verts;         // host copy of the caller's vertices (for crt_bvh_check)
     float bounds[6] = {0, 0, 0, 0, 0, 0};
     double sah = 0; int depth = 0; double build_seconds = 0;
+    int opt_iters = 0;                 // iterations of tree optimisation run and kept (host: re-insertion of bvh_build.cpp; builder 1: parallel re-insertion of bvh_ploc.cu)
     int builder = 0; int ploc_rounds = 0; float device_build_ms = 0.f; double layout_seconds = 0;      // device builder (bvh_ploc.cu)
     // device data
     int device = -1;
@@ -141,6 +142,7 @@ bool trace_queue_supported(const crt_bvh* bvh);
 crt_status launch_trace_queue(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, crt_hit* hits, unsigned long long* stats, cudaStream_t st);
 crt_status launch_trace_timeline(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, crt_hit* hits, uint64_t* marks, int64_t max_warps, int32_t* n_warps, cudaStream_t st);
 int crt_bvh_optimize_tree(crt_bvh* b, const crt_bvh_params& pr, int built_depth);
+crt_status crt_bvh_reinsert_device(crt_ctx* ctx, crt_bvh* b, int iterations);
 bool trace_group_supported(const crt_bvh* bvh);
 crt_status launch_trace_group(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, crt_hit* hits, unsigned long long* stats, cudaStream_t st, unsigned int* counter, int group);
 crt_status launch_trace_wide(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, crt_hit* hits, cudaStream_t st);

@@ -233,14 +233,15 @@ def test_trace_tail_split_and_timeline(crt, ctx, oracle, scene_name, n):
 @pytest.mark.parametrize("scene_name", ["cornell", "interior_small", "landscape_small"])
 def test_presplit_and_optimised_trees_return_the_same_hits(crt, ctx, oracle, scene_name):
     """Pre-splitting large triangles (crt_bvh_params.presplit, the default 1/16 and a much finer 1/128) and the insertion-based optimisation of the tree
-    (crt_bvh_params.optimize) change the tree, not the triangles: the hit
+    (crt_bvh_params.optimize: parallel re-insertion on the device for builder 0, the host's own for builder 3) change the tree, not the triangles: the hit
     records equal those of the unsplit tree and of the oracle bit for bit (D:R10: the result does not depend on the structure), also when a triangle
     sits in many leaves and is tested more than once; the device layouts pass their check."""
     import torch
     scene = SCENES[scene_name]()
     ref = None; r = None
-    for ps, opt in ((0.0, 0), (1 / 16, 0), (1 / 128, 0), (0.0, 30), (1 / 16, 100)):
-        bvh = ctx.crt_build_bvh(scene.verts, scene.mat_id, presplit=ps, optimize=opt)
+    # builder 0: the optimisation step is the device's parallel re-insertion; builder 3: the host's own
+    for ps, opt, builder in ((0.0, 0, 0), (1 / 16, 0, 0), (1 / 128, 0, 0), (0.0, 30, 0), (1 / 16, 100, 0), (1 / 16, 30, 3), (1 / 128, 7, 0)):
+        bvh = ctx.crt_build_bvh(scene.verts, scene.mat_id, presplit=ps, optimize=opt, builder=builder)
         assert bvh.check() == 0
         info = bvh.info()
         if r is None:
@@ -251,7 +252,8 @@ def test_presplit_and_optimised_trees_return_the_same_hits(crt, ctx, oracle, sce
         if ref is None:
             ref = h
             compare_hits(hits_np(oracle, h), oracle.Bvh(scene.verts).trace(r.view(oracle.RAY_DTYPE).reshape(-1)))
-        assert torch.equal(ref.view(torch.int32), h.view(torch.int32)), (ps, opt)
+        assert torch.equal(ref.view(torch.int32), h.view(torch.int32)), (ps, opt, builder)
+        assert info["builder"] == builder and info["depth"] <= 60 and (info["optimize_iterations"] > 0 if (opt >= 30 and scene_name != "landscape_small") else info["optimize_iterations"] <= opt)
         bvh.destroy()
 
 

@@ -50,8 +50,8 @@ FP32_PEAK_TFLOPS_NOMINAL = 148 * 128 * 2 * 1.965e9 / 1e12
 #           node visit and the same triangle test; its ray setup has 12 more)
 #   dram  = dram__bytes_read.sum + dram__bytes_write.sum of the default kernel
 NCU_PER_RAY = {
-    "interior": {"flop": 1754.0, "dram_bytes": 62.5, "source": "profiles/r02k_presplit.md (ncu on the default tree: large triangles pre-split, 20 iterations of insertion-based optimisation; flop: 6.824 G over 3,891,381 live rays of frame 7; dram: 243.1 MB over the same rays; the plain SAH tree: 1,897 flop per ray, profiles/r02c)"},
-    "landscape": {"flop": 1383.0, "dram_bytes": 100.7, "source": "profiles/r02c_roofline_inputs.md (same commit; flop: 2.817 G over 2,037,200 live rays of frame 7; dram: 205.2 MB over 2,038,170 live rays)"},
+    "interior": {"flop": 1717.0, "dram_bytes": 62.1, "source": "profiles/r02o_device_reinsertion.md (ncu on the default tree: host SAH, large triangles pre-split, parallel re-insertion on the device; flop: 6.683 G over 3,891,381 live rays of frame 7; dram: 241.7 MB over the same rays; the plain SAH tree: 1,897 flop per ray, profiles/r02c)"},
+    "landscape": {"flop": 1373.0, "dram_bytes": 101.7, "source": "profiles/r02o_device_reinsertion.md (same commit; flop: 2.797 G over 2,037,200 live rays of frame 7; dram: 207.3 MB over the same rays; the plain SAH tree: 1,383, profiles/r02c)"},
 }
 # what ncu shows to be the kernel's limiter (not modelled by the two-term roofline): profiles/r02a, r02c
 TRACE_LIMITER = {

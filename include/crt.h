@@ -102,7 +102,8 @@ typedef struct { const crt_material* materials; int32_t n_materials; float env[6
  * cost -8 %, traversal -2 to -4 % for +0.8 s of build time (profiles/r02k); stops early when four iterations gain less than 0.2 % (a terrain grid).
  * 0 = off; NULL params = 20.  With a context, builders 0 and 1 run (at most) that many iterations of PARALLEL re-insertion on the device instead (bvh_ploc.cu:
  * every node searches its best position in every iteration, conflicting moves are resolved by locks; stronger and two orders of magnitude faster than the
- * host's version: profiles/r02o); builders 2 and 3 and host-only builds run the host's. */
+ * host's version: profiles/r02o); builders 2 and 3 and host-only builds run the host's.  For builder 0 with a context the tree is built and optimised with one
+ * triangle reference per leaf and subtrees of at most max_leaf references are collapsed into leaves afterwards. */
 typedef struct { int32_t max_leaf; int32_t sah_bins; float cost_traversal, cost_intersect; int32_t n_threads; int32_t builder; int32_t ploc_radius; float presplit; int32_t optimize; } crt_bvh_params;
 typedef struct {
     int64_t n_tris, n_nodes, device_bytes;

@@ -367,7 +367,7 @@ int crt_bvh_optimize_tree(crt_bvh* b, const crt_bvh_params& pr, int built_depth)
 }
 
 // Builds the host tree.  Returns false on failure.
-bool crt_bvh_build_host(crt_bvh* b, const float* verts, int64_t n, const crt_bvh_params& pr)
+bool crt_bvh_build_host(crt_bvh* b, const float* verts, int64_t n, const crt_bvh_params& pr, bool presplit_single)
 {
     auto t0 = std::chrono::steady_clock::now();
     b->n_tris = n; b->max_leaf = pr.max_leaf;
@@ -388,7 +388,7 @@ bool crt_bvh_build_host(crt_bvh* b, const float* verts, int64_t n, const crt_bvh
         refs.push_back(r);
     }
     for (int k = 0; k < 3; ++k) { b->bounds[k] = n ? root.mn[k] : 0.f; b->bounds[3 + k] = n ? root.mx[k] : 0.f; }
-    if (pr.presplit > 0.f && pr.max_leaf > 1 && n > 0) {
+    if (pr.presplit > 0.f && (pr.max_leaf > 1 || presplit_single) && n > 0) {
         double diag = 0; for (int k = 0; k < 3; ++k) diag += ((double)root.mx[k] - root.mn[k]) * ((double)root.mx[k] - root.mn[k]);
         const double limit = (double)pr.presplit * std::sqrt(diag);
         int64_t budget = std::max<int64_t>(n / 4, 4096);         // at most this many additional references in all

@@ -753,8 +753,9 @@ crt_status crt_bvh_build_device(crt_ctx* ctx, crt_bvh* b, const float* verts, in
 // The same parallel re-insertion for a HOST-built tree (crt_build_bvh, builder 0 with a context): b->nodes goes to the device in the index convention
 // of this file (leaves first, the root last; a leaf of several triangles is one atomic node), is optimised, and comes back as b->nodes with the root
 // at 0 and siblings adjacent; leaves keep their triangle ranges.  Boxes may be padded or not (a union of padded boxes is the padded union).
-// Returns the iterations kept in b->opt_iters and the new depth in b->depth.
-crt_status crt_bvh_reinsert_device(crt_ctx* ctx, crt_bvh* b, int iterations)
+// collapse_max_leaf > 1: the host tree has one reference per leaf; after the optimisation subtrees of at most that many references become leaves (b->prim is
+// rewritten in the new leaf order).  Returns the iterations kept in b->opt_iters and the new depth in b->depth.
+crt_status crt_bvh_reinsert_device(crt_ctx* ctx, crt_bvh* b, int iterations, int collapse_max_leaf)
 {
     b->opt_iters = 0;
     const int n_nodes = (int)b->nodes.size();
@@ -785,15 +786,53 @@ crt_status crt_bvh_reinsert_device(crt_ctx* ctx, crt_bvh* b, int iterations)
     PLOC_CUDA(reins.alloc(n_nodes));
     const crt_status st = reinsertion_loop(ctx, T, n_leaves, n_nodes, iterations, &b->opt_iters, reins);
     if (st != CRT_OK) return st;
-    if (b->opt_iters == 0) return CRT_OK;          // nothing kept: the host tree stays as it is
+    if (b->opt_iters == 0 && collapse_max_leaf <= 1) return CRT_OK;          // nothing kept: the host tree stays as it is
     PLOC_CUDA(cudaMemcpy(box.data(), d_box.p, (size_t)n_nodes * sizeof(Box2), cudaMemcpyDeviceToHost));
     PLOC_CUDA(cudaMemcpy(left.data(), d_left.p, (size_t)n_nodes * 4, cudaMemcpyDeviceToHost)); PLOC_CUDA(cudaMemcpy(right.data(), d_right.p, (size_t)n_nodes * 4, cudaMemcpyDeviceToHost));
     PLOC_CUDA(cudaMemcpy(height.data(), d_height.p, (size_t)n_nodes * 4, cudaMemcpyDeviceToHost));
+    PLOC_CUDA(cudaMemcpy(cnt.data(), d_cnt.p, (size_t)n_nodes * 4, cudaMemcpyDeviceToHost));
     // back to the host form: root at 0, the two children of a node adjacent, depth-first
     std::vector<BuildNode> out((size_t)n_nodes);
     struct Item { int32_t src, dst; };
     std::vector<Item> stack{{n_nodes - 1, 0}};
     int32_t next = 1; int64_t seen = 0;
+    std::vector<int32_t> new_prim, sub;
+    if (collapse_max_leaf > 1) {
+        // the tree was built and optimised with one reference per leaf; subtrees of at most collapse_max_leaf references become leaves now
+        new_prim.reserve(b->prim.size());
+        int depth = 0; std::vector<std::pair<Item, int>> st2{{{n_nodes - 1, 0}, 1}};
+        out.clear(); out.emplace_back();
+        while (!st2.empty()) {
+            const Item it = st2.back().first; const int d = st2.back().second; st2.pop_back();
+            depth = std::max(depth, d);
+            BuildNode nd;
+            nd.bmin[0] = box[it.src].lo.x; nd.bmin[1] = box[it.src].lo.y; nd.bmin[2] = box[it.src].lo.z; nd.bmax[0] = box[it.src].hi.x; nd.bmax[1] = box[it.src].hi.y; nd.bmax[2] = box[it.src].hi.z;
+            if (cnt[it.src] <= collapse_max_leaf) {
+                nd.left = nd.right = -1; nd.first = (int32_t)new_prim.size();
+                sub.assign(1, it.src);
+                while (!sub.empty()) {
+                    const int32_t q = sub.back(); sub.pop_back();
+                    if (left[q] >= 0) { sub.push_back(right[q]); sub.push_back(left[q]); continue; }
+                    const BuildNode& old = b->nodes[leaf_of[q]];
+                    for (int j = 0; j < old.count; ++j) {
+                        const int32_t pr_id = b->prim[old.first + j];
+                        bool dup = false; for (size_t m = (size_t)nd.first; m < new_prim.size(); ++m) dup |= new_prim[m] == pr_id;
+                        if (!dup) new_prim.push_back(pr_id);          // two references of one triangle in one leaf: one record is enough
+                    }
+                }
+                nd.count = (int32_t)new_prim.size() - nd.first;
+            } else {
+                const int32_t c = (int32_t)out.size();
+                nd.left = c; nd.right = c + 1; nd.first = 0; nd.count = 0;
+                out.emplace_back(); out.emplace_back();
+                st2.push_back({{right[it.src], c + 1}, d + 1}); st2.push_back({{left[it.src], c}, d + 1});
+            }
+            out[it.dst] = nd;
+        }
+        b->nodes.swap(out); b->prim.swap(new_prim); b->n_refs = (int64_t)b->prim.size();
+        b->depth = depth;
+        return CRT_OK;
+    }
     while (!stack.empty()) {
         const Item it = stack.back(); stack.pop_back(); ++seen;
         BuildNode nd;

@@ -5,7 +5,7 @@
 #include <thread>
 #include "crt_internal.h"
 
-bool crt_bvh_build_host(crt_bvh* b, const float* verts, int64_t n, const crt_bvh_params& pr);
+bool crt_bvh_build_host(crt_bvh* b, const float* verts, int64_t n, const crt_bvh_params& pr, bool presplit_single = false);
 int32_t crt_bvh_check_host(const crt_bvh* b);
 void crt_bvh_flatten(const crt_bvh* b, const std::vector<int32_t>& tri_order, std::vector<GpuNode>& gn, std::vector<GpuTri>& gt, std::vector<int32_t>& slot_of_prim);
 int32_t crt_bvh_quantise(const crt_bvh* b, const std::vector<GpuNode>& gn, std::vector<QNode>& qn, QGrid* grid, double* inflation);
@@ -181,10 +181,15 @@ crt_status crt_build_bvh(crt_ctx* ctx, const float* verts, const int32_t* mat_id
         // where the host's own version can afford the worst 2 % only)
         const auto t_opt0 = std::chrono::steady_clock::now();
         crt_bvh_params p0 = pr; p0.optimize = 0;
-        crt_bvh_build_host(b, v, n_tris, p0);
-        const crt_status rst = crt_bvh_reinsert_device(ctx, b, pr.optimize);
+        // the tree is built and optimised with ONE reference per leaf, so that the re-insertion can move single triangles; subtrees of at most max_leaf
+        // references are collapsed into leaves afterwards (interior scene: 8 % fewer triangle tests per ray, secondary traversal -2 %; profiles/r02o)
+        const bool fine = pr.max_leaf > 1;
+        if (fine) p0.max_leaf = 1;
+        crt_bvh_build_host(b, v, n_tris, p0, fine);
+        const crt_status rst = crt_bvh_reinsert_device(ctx, b, pr.optimize, fine ? pr.max_leaf : 0);
         if (rst != CRT_OK) { crt_bvh_destroy(b); return rst; }
-        if (b->opt_iters > 0) {          // SAH cost of the new tree, on the unpadded boxes as crt_bvh_build_host reports it
+        if (fine) b->max_leaf = pr.max_leaf;
+        if (b->opt_iters > 0 || fine) {          // SAH cost of the new tree, on the unpadded boxes as crt_bvh_build_host reports it
             float maxabs = 0.f; for (int k = 0; k < 6; ++k) maxabs = std::max(maxabs, std::fabs(b->bounds[k]));
             const double pad2 = 2.0 * (double)(maxabs * (1.0f / 131072.0f));
             auto ha = [&](const BuildNode& x) { const double dx = (double)x.bmax[0] - x.bmin[0] - pad2, dy = (double)x.bmax[1] - x.bmin[1] - pad2, dz = (double)x.bmax[2] - x.bmin[2] - pad2; return dx * dy + dy * dz + dz * dx; };

@@ -142,7 +142,7 @@ bool trace_queue_supported(const crt_bvh* bvh);
 crt_status launch_trace_queue(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, crt_hit* hits, unsigned long long* stats, cudaStream_t st);
 crt_status launch_trace_timeline(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, crt_hit* hits, uint64_t* marks, int64_t max_warps, int32_t* n_warps, cudaStream_t st);
 int crt_bvh_optimize_tree(crt_bvh* b, const crt_bvh_params& pr, int built_depth);
-crt_status crt_bvh_reinsert_device(crt_ctx* ctx, crt_bvh* b, int iterations);
+crt_status crt_bvh_reinsert_device(crt_ctx* ctx, crt_bvh* b, int iterations, int collapse_max_leaf = 0);
 bool trace_group_supported(const crt_bvh* bvh);
 crt_status launch_trace_group(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, crt_hit* hits, unsigned long long* stats, cudaStream_t st, unsigned int* counter, int group);
 crt_status launch_trace_wide(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, crt_hit* hits, cudaStream_t st);

@@ -50,8 +50,8 @@ FP32_PEAK_TFLOPS_NOMINAL = 148 * 128 * 2 * 1.965e9 / 1e12
 #           node visit and the same triangle test; its ray setup has 12 more)
 #   dram  = dram__bytes_read.sum + dram__bytes_write.sum of the default kernel
 NCU_PER_RAY = {
-    "interior": {"flop": 1717.0, "dram_bytes": 62.1, "source": "profiles/r02o_device_reinsertion.md (ncu on the default tree: host SAH, large triangles pre-split, parallel re-insertion on the device; flop: 6.683 G over 3,891,381 live rays of frame 7; dram: 241.7 MB over the same rays; the plain SAH tree: 1,897 flop per ray, profiles/r02c)"},
-    "landscape": {"flop": 1373.0, "dram_bytes": 101.7, "source": "profiles/r02o_device_reinsertion.md (same commit; flop: 2.797 G over 2,037,200 live rays of frame 7; dram: 207.3 MB over the same rays; the plain SAH tree: 1,383, profiles/r02c)"},
+    "interior": {"flop": 1673.0, "dram_bytes": 62.0, "source": "profiles/r02o_device_reinsertion.md (ncu on the default tree: host SAH, large triangles pre-split, parallel re-insertion on the device at single-reference granularity; flop: 6.512 G over 3,891,381 live rays of frame 7; dram: 241.3 MB over the same rays; the plain SAH tree: 1,897 flop per ray, profiles/r02c)"},
+    "landscape": {"flop": 1370.0, "dram_bytes": 102.9, "source": "profiles/r02o_device_reinsertion.md (same commit; flop: 2.792 G over 2,037,200 live rays of frame 7; dram: 209.6 MB over the same rays; the plain SAH tree: 1,383, profiles/r02c)"},
 }
 # what ncu shows to be the kernel's limiter (not modelled by the two-term roofline): profiles/r02a, r02c
 TRACE_LIMITER = {

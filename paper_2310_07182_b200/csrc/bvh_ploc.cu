@@ -445,7 +445,10 @@ __global__ void __launch_bounds__(PB) reins_filter_kernel(Tree T, int n_nodes, c
     const int x = blockIdx.x * PB + threadIdx.x;
     if (x >= n_nodes) return;
     int ok = win[x];
-    if (ok) for (int a = T.parent[target[x]]; a >= 0; a = T.parent[a]) if (win[a]) { ok = 0; break; }
+    if (ok) {
+        int steps = 0;
+        for (int a = T.parent[target[x]]; a >= 0; a = T.parent[a]) if (win[a] || ++steps > 4096) { ok = 0; break; }      // (4096: far beyond any height this file accepts)
+    }
     go[x] = ok;
 }
 
@@ -475,7 +478,7 @@ __global__ void __launch_bounds__(PB) reins_refit_kernel(Tree T, int n, int32_t*
         const int p = T.parent[i];
         if (p < 0) break;
         __threadfence();
-        if (atomicAdd(arrive + p, 1) == 0) break;
+        if (atomicAdd(arrive + p, 1) != 1) break;          // the first arrival stops; the second goes on (anything else would mean a malformed tree: stop)
         const int l = T.left[p], r = T.right[p];
         Box2 a, b;
         a.lo = __ldcg(&T.box[l].lo); a.hi = __ldcg(&T.box[l].hi); b.lo = __ldcg(&T.box[r].lo); b.hi = __ldcg(&T.box[r].hi);
@@ -824,6 +827,7 @@ crt_status crt_bvh_reinsert_device(crt_ctx* ctx, crt_bvh* b, int iterations, int
             } else {
                 const int32_t c = (int32_t)out.size();
                 nd.left = c; nd.right = c + 1; nd.first = 0; nd.count = 0;
+                if ((int64_t)out.size() + 2 > n_nodes) return crt_fail(ctx, CRT_ERR_STATE, "build_bvh: re-insertion left an inconsistent tree");
                 out.emplace_back(); out.emplace_back();
                 st2.push_back({{right[it.src], c + 1}, d + 1}); st2.push_back({{left[it.src], c}, d + 1});
             }

@@ -62,6 +62,14 @@ CRT_DEV NodeRegs load_node(const GpuNode* __restrict__ nodes, int idx)
     return n;
 }
 
+// a ray record is read once: it must not take an L1 line from the nodes (the kernel lives on the L1: profiles/r02a)
+CRT_DEV float4 ld_stream(const float4* p)
+{
+    float4 v;
+    asm volatile("ld.global.nc.L1::no_allocate.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
+    return v;
+}
+
 struct Hit { float t; int prim; };     // u, v go straight to the hit record when a nearer hit is found (two registers fewer)
 
 // 1/d for the box test only.  A direction component of (nearly) zero is replaced by +-2^-60: with an infinite reciprocal the
@@ -414,11 +422,11 @@ __global__ void __launch_bounds__(TRACE_BLOCK, CRT_TRACE_MINB(QN)) trace_dyn_ker
                 if ((int64_t)i >= n) { exhausted = true; }
                 else {
                     const float4* rp = reinterpret_cast<const float4*>(rays + i);
-                    const float4 rd = __ldg(rp + 1);
+                    const float4 rd = ld_stream(rp + 1);
                     if (rd.w < 0.f) {                 // inactive slot: a miss, nothing to traverse
                         if (!COUNT) store_miss(hits, i, rd.w);
                     } else {
-                        r.init(__ldg(rp), rd);
+                        r.init(ld_stream(rp), rd);
                         if (QN) q.init(r, grid);
                         if (QN == 1 || QN >= 3) q2.init(q);
                         ray_idx = (int)i; node = 0; leaf = 0; top = stack;

@@ -38,7 +38,7 @@ constexpr int TRACE_BLOCK = 128;
                                                // tolerance-only triangle test (trace_exact = 0); 4 as 1 with the top of the tree staged in shared memory (experiment); 5 the 4-wide form of the 16-bit nodes
 constexpr int TREELET_NODES = 512;             // QN 4: nodes 0 .. 511 (the top levels: crt_bvh_flatten numbers them breadth-first) = 16 KB of shared memory per block
 #ifndef CRT_VISITS_PER_VOTE
-#define CRT_VISITS_PER_VOTE 3   // inner-node visits between two leaf-wait votes of a warp
+#define CRT_VISITS_PER_VOTE 6   // inner-node visits between two leaf-wait votes of a warp (3 until the trees of profiles/r02k / r02o: re-measured there, 5-8 are 1.5-2.7 % faster than 3)
 #endif
 
 CRT_DEV unsigned long long globaltimer_ns() { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
@@ -473,7 +473,7 @@ __global__ void __launch_bounds__(TRACE_BLOCK, CRT_TRACE_MINB(QN)) trace_dyn_ker
         // (a warp-uniform formulation of these loops, every exit a full-mask vote, was measured 3-10 % slower: profiles/r01f)
         while (node != SENTINEL || (SPLIT && leaf < 0)) {
             // inner nodes; the first leaf a lane meets is postponed so that the warp's leaves are processed together
-            // (two visits per vote: the vote and its warp synchronisation cost 7 issue slots)
+            // (several visits per vote: the vote and its warp synchronisation cost 7 issue slots)
             while ((unsigned)node < (unsigned)SENTINEL) {
 #pragma unroll
                 for (int rep = 0; rep < CRT_VISITS_PER_VOTE; ++rep) {

@@ -137,7 +137,7 @@ struct Band { int64_t slot0, count; unsigned int* counter; uint32_t* n_active; }
 crt_status crt_bvh_build_device(crt_ctx* ctx, crt_bvh* b, const float* verts, int64_t n, const crt_bvh_params& pr, bool full_device);
 int32_t crt_layout_check_device(const crt_bvh* b);
 bool crt_bvh_ensure_q4(const crt_bvh* b);
-crt_status launch_trace(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, crt_hit* hits, cudaStream_t st, bool far_origins = false, unsigned int* counter = nullptr);
+crt_status launch_trace(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, crt_hit* hits, cudaStream_t st, bool far_origins = false, unsigned int* counter = nullptr, bool camera_rays = false);
 bool trace_queue_supported(const crt_bvh* bvh);
 crt_status launch_trace_queue(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, crt_hit* hits, unsigned long long* stats, cudaStream_t st);
 crt_status launch_trace_timeline(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, crt_hit* hits, uint64_t* marks, int64_t max_warps, int32_t* n_warps, cudaStream_t st);

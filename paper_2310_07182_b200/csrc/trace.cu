@@ -8,7 +8,7 @@
 //    twelve plane distances of a visit are six packed FFMA2 (fma.rn.f32x2, new on sm_100: one issue slot for two fused multiply-adds);
 //    the fp32 form (64-byte nodes, two 256-bit loads) is trace_kernel 0 / 1; leaf triangles are 64-byte records (v0|id, e1, e2);
 //  - with the 16-bit nodes the kernel is issue- and latency-bound, not bandwidth-bound (profiles/r01f): what matters is how many
-//    lanes of a warp do useful work and how many warps are resident (8 blocks of 128 threads per SM at 64 registers).
+//    lanes of a warp do useful work and how many warps are resident (8 blocks of 128 threads per SM at 64 registers for camera rays, 9 at 56 for secondary rays).
 //    trace_dyn_kernel is a persistent-warp kernel: the grid fills the 148 SMs once; a lane whose ray has terminated takes
 //    the next ray from a global counter (one atomicAdd per warp, ballot + popc give each idle lane its index) as soon as
 //    fewer than `refill_threshold` lanes of its warp are still traversing, so rays enter a warp in slot order -- the order
@@ -360,8 +360,11 @@ __global__ void __launch_bounds__(TRACE_BLOCK) trace_flat_kernel(const GpuNode* 
 // concurrent writer); the lanes still working on that ray adopt the delivered t as their pruning bound.
 // TIMELINE (crt_trace_timeline): the same traversal with four marks per warp written to `stats` at the end: [0] start, [1] the moment the warp
 // first saw the ray list exhausted, [2] end (globaltimer, ns), [3] the largest number of node visits one of its lanes made after [1].
-template <bool COUNT, int QN, bool SPLIT, bool TIMELINE = false>
-__global__ void __launch_bounds__(TRACE_BLOCK, CRT_TRACE_MINB(QN)) trace_dyn_kernel(const GpuNode* __restrict__ nodes, const QNode* __restrict__ qnodes, const QGrid grid, const GpuTri* __restrict__ tris,
+// MINB: resident blocks per SM the instantiation is compiled for.  The default kernel exists twice: 8 blocks (64 registers) for camera rays and 9 blocks (56
+// registers, 16 bytes of spill outside the node loop) for secondary rays, whose divergent gathers gain more from the ninth block's warps than they lose to its
+// share of the L1 (interior secondary rays -1.2 to -2.5 %; camera rays +2 % if they took it too: profiles/r02a).
+template <bool COUNT, int QN, bool SPLIT, bool TIMELINE = false, int MINB = CRT_TRACE_MINB(QN)>
+__global__ void __launch_bounds__(TRACE_BLOCK, MINB) trace_dyn_kernel(const GpuNode* __restrict__ nodes, const QNode* __restrict__ qnodes, const QGrid grid, const GpuTri* __restrict__ tris,
                                                                 const crt_ray* __restrict__ rays, crt_hit* __restrict__ hits, int64_t n,
                                                                 unsigned int* __restrict__ counter, int refill_threshold, int leaf_wait,
                                                                 unsigned long long* __restrict__ stats, int n_qnodes)
@@ -551,12 +554,12 @@ __global__ void __launch_bounds__(256) primary_rays_kernel(CamDev cam, DevLayout
     rp[1] = make_float4(dx, dy, dz, 1e30f);
 }
 
-template <bool COUNT, int QN, bool SPLIT = false, bool TIMELINE = false>
+template <bool COUNT, int QN, bool SPLIT = false, bool TIMELINE = false, int MINB = CRT_TRACE_MINB(QN)>
 crt_status launch_dyn(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, crt_hit* hits, unsigned long long* stats, cudaStream_t st, unsigned int* counter = nullptr, int64_t max_warps = 0, int32_t* n_warps = nullptr)
 {
     int per_sm = ctx->trace_blocks_per_sm;
     if (per_sm <= 0) {
-        CRT_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, trace_dyn_kernel<COUNT, QN, SPLIT, TIMELINE>, TRACE_BLOCK, QN == 4 ? (size_t)TREELET_NODES * 32 : (size_t)0));
+        CRT_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, trace_dyn_kernel<COUNT, QN, SPLIT, TIMELINE, MINB>, TRACE_BLOCK, QN == 4 ? (size_t)TREELET_NODES * 32 : (size_t)0));
         if (per_sm < 1) per_sm = 1;
     }
     if (!counter) counter = ctx->d_counter;
@@ -567,7 +570,7 @@ crt_status launch_dyn(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int
         if (grid * (TRACE_BLOCK / 32) > max_warps) return crt_fail(ctx, CRT_ERR_INVALID_ARG, "trace_timeline: marks buffer holds %lld warps, the launch has %lld", (long long)max_warps, (long long)(grid * (TRACE_BLOCK / 32)));
         *n_warps = (int32_t)(grid * (TRACE_BLOCK / 32));
     }
-    trace_dyn_kernel<COUNT, QN, SPLIT, TIMELINE><<<(unsigned)grid, TRACE_BLOCK, QN == 4 ? (size_t)TREELET_NODES * 32 : (size_t)0, st>>>(bvh->d_nodes, QN == 5 ? bvh->d_q4nodes : bvh->d_qnodes, bvh->qgrid, bvh->d_tris, rays, hits, n, counter, ctx->trace_refill_threshold, ctx->trace_leaf_wait, stats, (int)bvh->n_gpu_nodes);
+    trace_dyn_kernel<COUNT, QN, SPLIT, TIMELINE, MINB><<<(unsigned)grid, TRACE_BLOCK, QN == 4 ? (size_t)TREELET_NODES * 32 : (size_t)0, st>>>(bvh->d_nodes, QN == 5 ? bvh->d_q4nodes : bvh->d_qnodes, bvh->qgrid, bvh->d_tris, rays, hits, n, counter, ctx->trace_refill_threshold, ctx->trace_leaf_wait, stats, (int)bvh->n_gpu_nodes);
     CRT_CHECK_LAUNCH(ctx, "trace_dyn");
     return CRT_OK;
 }
@@ -585,7 +588,7 @@ crt::DevLayout make_dev_layout(const Layout& L, const crt_frame& f)
 
 // far_origins: the caller knows the ray origins may lie beyond the default box test's contract (16 scene extents from the scene;
 // crt_trace_primary checks the camera eye): the any-origin box test (trace_kernel 4's) is used instead
-crt_status launch_trace(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, crt_hit* hits, cudaStream_t st, bool far_origins, unsigned int* counter)
+crt_status launch_trace(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, int64_t n, crt_hit* hits, cudaStream_t st, bool far_origins, unsigned int* counter, bool camera_rays)
 {
     if (n == 0) return CRT_OK;
     if (ctx->trace_kernel == 2 && bvh->d_wnodes && bvh->wide_violations == 0) return launch_trace_wide(ctx, bvh, rays, n, hits, st);
@@ -603,7 +606,8 @@ crt_status launch_trace(crt_ctx* ctx, const crt_bvh* bvh, const crt_ray* rays, i
     if (ctx->trace_kernel == 7 && !far_origins && q_ok && crt_bvh_ensure_q4(bvh)) return launch_dyn<false, 5>(ctx, bvh, rays, n, hits, nullptr, st, counter);
     if (ctx->trace_kernel == 3 && !ctx->trace_exact && !far_origins && q_ok) return launch_dyn<false, 3>(ctx, bvh, rays, n, hits, nullptr, st, counter);
     if ((ctx->trace_kernel == 4 || (ctx->trace_kernel >= 3 && far_origins)) && q_ok) return launch_dyn<false, 2>(ctx, bvh, rays, n, hits, nullptr, st, counter);
-    if (ctx->trace_kernel >= 3 && q_ok) return ctx->trace_tail_split ? launch_dyn<false, 1, true>(ctx, bvh, rays, n, hits, nullptr, st, counter) : launch_dyn<false, 1>(ctx, bvh, rays, n, hits, nullptr, st, counter);
+    if (ctx->trace_kernel >= 3 && q_ok) return ctx->trace_tail_split ? launch_dyn<false, 1, true>(ctx, bvh, rays, n, hits, nullptr, st, counter)
+                                                               : (camera_rays ? launch_dyn<false, 1>(ctx, bvh, rays, n, hits, nullptr, st, counter) : launch_dyn<false, 1, false, false, 9>(ctx, bvh, rays, n, hits, nullptr, st, counter));
     return launch_dyn<false, 0>(ctx, bvh, rays, n, hits, nullptr, st, counter);
 }
 
@@ -650,5 +654,5 @@ crt_status launch_primary(crt_ctx* ctx, const crt_bvh* bvh, const crt_camera& ca
         const float reach = 15.0f * fmaxf(ext, maxext * (1.0f / 4096.0f));
         if (cam.eye[k] < bvh->bounds[k] - reach || cam.eye[k] > bvh->bounds[3 + k] + reach) far_eye = true;
     }
-    return launch_trace(ctx, bvh, rays + slot0, count, hits + slot0, st, far_eye, band ? band->counter : nullptr);
+    return launch_trace(ctx, bvh, rays + slot0, count, hits + slot0, st, far_eye, band ? band->counter : nullptr, true);
 }
